@@ -13,6 +13,7 @@ from .gen import (  # noqa: F401
     make_workload,
     protocol_workload,
     audit_distribution,
+    AUDIT_KINDS,
     token_ids,
     tokens_for_samples,
     describe,
