@@ -1,0 +1,190 @@
+/*
+ * odb.h -- C ABI of the B200-native ODB hot path: group -> align -> collate.
+ *
+ * What it computes (paper: "Online Dynamic Batching", /root/reference/PAPER.md, cited P:<line>):
+ *   for R data-parallel ranks (virtual ranks: independent segments on ONE GPU), given the realized
+ *   post-tokenization sample lengths and the ragged token buffers,
+ *     1. per rank, sort the buffered window by length and form variable-size token-budget groups
+ *        (section 2.2, Eq. 1; worked example App. D);
+ *     2. align the per-rank group counts to the common target T_grp with the Max-Based
+ *        Bidirectional Group Alignment protocol (section 2.3; Eq. 3; Alg. 1):
+ *        split upward, overflow + recirculation downward, IDLE slots for finished ranks,
+ *        join (default, Thm 1) or non-join termination with sample-quota closure (Thm 2);
+ *     3. collate every aligned group into padded tensors input_ids / attention_mask /
+ *        position_ids / labels (collate_fn P:28; pad to the group max P:416-420) and count the
+ *        valid tokens per group for token-level loss scaling (Eq. 2).
+ *   All work is integer / index work; results are bit-exact and run-to-run deterministic.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  The caller owns every
+ *     buffer it passes; the library never frees or reallocates them.  The library owns only the
+ *     scratch inside odb_ctx.
+ *   - `stream` is a cudaStream_t passed as void* (0 = the legacy default stream).  Kernel launches
+ *     are asynchronous on it; the calls documented as "synchronises" wait for that stream.
+ *   - Samples are laid out rank-major: rank r owns samples h_rank_ptr[r] .. h_rank_ptr[r+1]-1 in
+ *     sampler order; a "local id" is the index inside the rank.
+ *   - d_sample_ptr[g] .. d_sample_ptr[g+1] are the token offsets of global sample g in d_tokens and
+ *     must equal the prefix sum of d_lengths.  d_tokens must be 16-byte aligned.
+ *   - Masked spans (labels -> ignore_index) are CSR per sample: spans d_span_ptr[g] .. d_span_ptr[g+1]-1,
+ *     half-open [lo,hi) token positions, sorted and disjoint.
+ *   - Every call returns an ODB_* status (0 = OK).  No exceptions, no abort, nothing printed.
+ *   - There is no CPU fallback: without a CUDA device odb_create returns ODB_ERR_CUDA.
+ *
+ * Output layout
+ *   Slot index s = r * n_steps + k (rank-major; step k of rank r).  Every rank holds exactly
+ *   n_steps slots; an IDLE slot has count 0 and width 0 (reading U14).  Slot s is a dense
+ *   row-major [grp_count[s] x grp_width[s]] block, right-padded, placed at element offset
+ *   grp_offset[s] (a multiple of 16) in each of the four arenas; the <= 15 gap elements between
+ *   blocks are never written.  Rows are the group's samples ascending by (length, local id).
+ */
+#ifndef ODB_H_
+#define ODB_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct odb_ctx odb_ctx;
+
+enum {
+    ODB_OK = 0,
+    ODB_ERR_INVALID_ARG = 1,
+    ODB_ERR_BAD_LENGTH = 2, /* some length < 1 */
+    ODB_ERR_CAPACITY = 3,   /* an output arena or table is too small; nothing is written past capacity */
+    ODB_ERR_CUDA = 4,       /* a CUDA call failed (odb_last_cuda_error gives the code) */
+    ODB_ERR_STATE = 5       /* call order violated */
+};
+enum {
+    ODB_RULE_THRESHOLD = 0, /* paper section 2.2: threshold carry-over greedy (default) */
+    ODB_RULE_MAXFIT_ASC = 1 /* App. I: longest ascending run with count*max_len <= budget */
+};
+enum {
+    ODB_STOP_ALL_FINISHED = 0, /* join: every rank drained (Thm 1) */
+    ODB_STOP_LOGICAL = 1,      /* non-join: some rank advertised "finished" */
+    ODB_STOP_QUOTA = 2         /* non-join: cumulative emitted samples reached sample_quota (Thm 2) */
+};
+
+typedef struct {
+    int32_t n_ranks;        /* R = W >= 1 */
+    int32_t rule;           /* ODB_RULE_* */
+    int32_t join_mode;      /* 1 = join (default), 0 = non-join */
+    int32_t buffer_size;    /* per-round window per rank (the paper's grouping buffer); 0 = all */
+    int32_t slot_capacity;  /* C_r, output slots per round (Eq. 3); 0 = unlimited */
+    int32_t pad_id;         /* input_ids pad value */
+    int32_t ignore_index;   /* label of pad / masked positions (-100) */
+    int32_t shift_labels;   /* 1: labels[t] = token t+1 (default); 0: labels[t] = token t */
+    int64_t budget;         /* L_max, 1 .. 2^31-1 */
+    int64_t sample_quota;   /* non-join only; <= 0 = no quota */
+    int64_t emitted_so_far; /* non-join only; S_emit carried in from earlier logical iterations */
+} odb_params;
+
+typedef struct { /* host-side; filled by odb_plan_query / odb_run */
+    int32_t n_rounds;    /* protocol rounds including the terminal check */
+    int32_t n_steps;     /* slots per rank = sum over rounds of T_grp */
+    int32_t stop_reason; /* ODB_STOP_* */
+    int32_t reserved;
+    int64_t n_slots;         /* R * n_steps */
+    int64_t total_elems;     /* elements per output arena (sum of round_up(count*width, 16)) */
+    int64_t samples_emitted; /* S_emit of this call */
+    int64_t samples_left;    /* un-emitted samples (non-join) */
+    int64_t real_tokens;     /* sum of lengths of emitted samples */
+    int64_t padded_elems;    /* sum of count*width */
+} odb_plan_info;
+
+typedef struct { /* device outputs, caller-allocated; any table pointer may be NULL (not wanted) */
+    int32_t *d_input_ids;
+    int32_t *d_labels;
+    int32_t *d_position_ids;
+    uint8_t *d_attention_mask;
+    int64_t arena_capacity; /* elements available in each of the four arenas */
+    /* per-slot tables, n_slots entries each (d_grp_sample_ptr: n_slots+1) */
+    int32_t *d_grp_count;
+    int32_t *d_grp_width;
+    int32_t *d_grp_round;
+    int32_t *d_grp_valid_tokens; /* #{labels != ignore_index} in the slot (Eq. 2's t_{r,k}) */
+    int32_t *d_grp_real_tokens;  /* sum of the slot's sample lengths */
+    int64_t *d_grp_offset;
+    int64_t *d_grp_sample_ptr;
+    int64_t slot_capacity_alloc; /* slots available in the per-slot tables */
+    int32_t *d_grp_sample_ids;   /* local sample ids, row order, samples_emitted entries */
+    int64_t ids_capacity;
+    /* per-step tables, n_steps entries */
+    int32_t *d_step_samples;      /* e_k = sum over ranks of count */
+    int64_t *d_step_valid_tokens; /* T_tok,k = sum over ranks of valid tokens (Eq. 2) */
+    int64_t step_capacity_alloc;
+    /* un-emitted local ids per rank, ascending (non-join): d_left_ptr R+1, d_left_ids samples_left */
+    int64_t *d_left_ptr;
+    int32_t *d_left_ids;
+    int64_t left_capacity;
+} odb_outputs;
+
+/* Create a context on CUDA device `device` for at most max_samples_total samples over all ranks.
+ * Validates params (ODB_ERR_INVALID_ARG).  Allocates scratch (~70 bytes per sample). */
+int odb_create(const odb_params *params, int device, int64_t max_samples_total, odb_ctx **out);
+int odb_destroy(odb_ctx *ctx);
+/* Forget all rounds and start over with the same params; keeps scratch. */
+int odb_reset(odb_ctx *ctx);
+
+/* One protocol round, first half (section 2.2): fill each rank's window (recirculated leftovers +
+ * the next un-fetched samples, up to buffer_size), sort it by (length, id), compute the greedy
+ * successor of every start position and extract the candidate groups and G_r.  Lengths only; no
+ * token is touched.  The first call after create/reset fixes d_lengths / h_rank_ptr (R+1 entries,
+ * h_rank_ptr[R] <= max_samples_total) for the following rounds.  Asynchronous. */
+int odb_form_groups(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, void *stream);
+
+/* Second half (section 2.3, Alg. 1): T_grp by an on-device reduction over the R ranks, split /
+ * overflow, IDLE slots, step totals, the non-join quota cut, leftovers.  Asynchronous. */
+int odb_align(odb_ctx *ctx, void *stream);
+
+/* Synchronises.  *h_done != 0 when the protocol has terminated (no further round may be formed);
+ * *h_T = T_grp of the round just aligned (0 if the round was the terminal check).  Must be called
+ * after every odb_align.  Returns ODB_ERR_BAD_LENGTH if some length < 1. */
+int odb_round_status(odb_ctx *ctx, int32_t *h_done, int32_t *h_T);
+
+/* Synchronises.  Builds the rank-major slot tables and block offsets; fills *h_out so the caller
+ * can size the output arenas.  Only after termination (ODB_ERR_STATE otherwise). */
+int odb_plan_query(odb_ctx *ctx, odb_plan_info *h_out);
+
+/* Collate every emitted slot (C.4 in DESIGN.md) and fill the tables of `out`.  Requires
+ * odb_plan_query.  ODB_ERR_CAPACITY if an arena or table is too small.  Asynchronous. */
+int odb_collate(odb_ctx *ctx, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
+                const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *out, void *stream);
+
+/* Everything: reset, the round loop until termination, plan query, one collate over all emitted
+ * steps.  Synchronises once per round (a few bytes of status) and once for the plan sizes; returns
+ * with the collate kernels enqueued on `stream`.  On ODB_ERR_CAPACITY *h_out is still filled. */
+int odb_run(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
+            const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
+            const int32_t *d_span_hi, const odb_outputs *out, odb_plan_info *h_out, void *stream);
+
+/* End-to-end variant with HOST buffers (pinned memory recommended): copies lengths, sample_ptr,
+ * spans and tokens host->device, runs the whole path, copies the four arenas and every non-NULL
+ * table of `h_out_bufs` (same struct, HOST pointers) back, rank by rank so that copies overlap the
+ * collate kernel.  Synchronises before returning.  n_spans = h_span_ptr[N]. */
+int odb_run_host(odb_ctx *ctx, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
+                 const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
+                 const int32_t *h_span_hi, const odb_outputs *h_out_bufs, odb_plan_info *h_out, void *stream);
+
+/* Device times of the last odb_run / odb_collate on this context, in milliseconds, measured with
+ * CUDA events on the launching stream: ms[0] = planning (all rounds, plan query, row descriptors and
+ * the tile table), ms[1] = the collate kernel alone, ms[2] = what follows it (step totals, table
+ * copies).  Synchronises.  Enabled by odb_set_timing(ctx, 1); off by default. */
+int odb_set_timing(odb_ctx *ctx, int enable);
+int odb_get_timing(odb_ctx *ctx, float *ms3);
+/* Number of kernels this context has launched since odb_create (diagnostics / bench accounting). */
+int64_t odb_kernel_launches(const odb_ctx *ctx);
+
+/* Diagnostics: copy an internal device table to the host (synchronises).  `what`: 0 = G_r (int32[R])
+ * of the last round, 1 = S_r (int32[R]), 2 = sorted keys of the last round ((len<<32)|id, uint64[N],
+ * rank regions at h_rank_ptr), 3 = candidate start flags (uint8[N]).  Returns bytes copied or < 0. */
+int64_t odb_debug_read(odb_ctx *ctx, int what, void *h_dst, int64_t max_bytes);
+
+int odb_last_cuda_error(const odb_ctx *ctx);
+const char *odb_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ODB_H_ */

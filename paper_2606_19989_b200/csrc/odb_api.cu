@@ -1,0 +1,700 @@
+// C ABI of libodb (include/odb.h): argument checks, the host-side round loop / state machine,
+// scratch management.  Every step of the path runs in the kernels of odb_plan.cu / odb_collate.cu;
+// there is no CPU fallback.
+#include <algorithm>
+#include <cstddef>
+#include <cstring>
+#include <new>
+
+#include "odb_internal.cuh"
+
+using namespace odb;
+
+#define CU(c, expr)                                 \
+    do {                                            \
+        cudaError_t e__ = (expr);                   \
+        if (e__ != cudaSuccess) {                   \
+            (c)->last_cuda_error = (int)e__;        \
+            (void)cudaGetLastError();               \
+            return ODB_ERR_CUDA;                    \
+        }                                           \
+    } while (0)
+
+template <class T>
+static cudaError_t dev_alloc(T **p, size_t n) {
+    return cudaMalloc((void **)p, std::max<size_t>(n, 1) * sizeof(T));
+}
+
+// grow a step-major staging table, preserving `used` entries and zero-filling the rest
+template <class T>
+static cudaError_t grow_preserve(DevBuf<T> &b, size_t want, size_t used, cudaStream_t st) {
+    if (want <= b.cap) return cudaSuccess;
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return e;
+    T *np = nullptr;
+    e = cudaMalloc((void **)&np, want * sizeof(T));
+    if (e != cudaSuccess) return e;
+    e = cudaMemset(np, 0, want * sizeof(T));
+    if (e != cudaSuccess) return e;
+    if (b.p && used) {
+        e = cudaMemcpy(np, b.p, used * sizeof(T), cudaMemcpyDeviceToDevice);
+        if (e != cudaSuccess) return e;
+    }
+    if (b.p) cudaFree(b.p);
+    b.p = np;
+    b.cap = want;
+    return cudaSuccess;
+}
+
+template <class T>
+static cudaError_t copy_tab(T *dst, const T *src, size_t n, cudaStream_t st) {
+    if (!dst || n == 0) return cudaSuccess;
+    return cudaMemcpyAsync(dst, src, n * sizeof(T), cudaMemcpyDeviceToDevice, st);
+}
+
+static void free_all(odb_ctx *c) {
+    cudaFree(c->d_rank_ptr);
+    cudaFree(c->keyA);
+    cudaFree(c->keyB);
+    cudaFree(c->ovf);
+    cudaFree(c->jA);
+    cudaFree(c->jB);
+    cudaFree(c->mark);
+    cudaFree(c->flag);
+    cudaFree(c->posflag);
+    cudaFree(c->emitted);
+    cudaFree(c->gpos);
+    cudaFree(c->agpos);
+    cudaFree(c->agcnt);
+    cudaFree(c->agoff);
+    cudaFree(c->left_ids);
+    cudaFree(c->emit_ids);
+    cudaFree(c->n_left);
+    cudaFree(c->fetch_pos);
+    cudaFree(c->emit_cur);
+    cudaFree(c->G);
+    cudaFree(c->S);
+    cudaFree(c->d_rec);
+    cudaFree(c->d_tot);
+    if (c->h_rec) cudaFreeHost(c->h_rec);
+    if (c->h_tot) cudaFreeHost(c->h_tot);
+    c->st_count.release();
+    c->st_width.release();
+    c->st_idoff.release();
+    c->st_round.release();
+    c->step_samples.release();
+    c->grp_count.release();
+    c->grp_width.release();
+    c->grp_round.release();
+    c->grp_valid.release();
+    c->grp_real.release();
+    c->grp_idoff.release();
+    c->grp_offset.release();
+    c->grp_sample_ptr.release();
+    c->grp_sample_ids.release();
+    c->left_out.release();
+    c->left_ptr.release();
+    c->step_valid.release();
+    c->rows.release();
+    c->row_sp.release();
+    c->tile_slot.release();
+    c->hs_lengths.release();
+    c->hs_tokens.release();
+    c->hs_span_lo.release();
+    c->hs_span_hi.release();
+    c->hs_ids.release();
+    c->hs_labels.release();
+    c->hs_pos.release();
+    c->hs_sample_ptr.release();
+    c->hs_span_ptr.release();
+    c->hs_mask.release();
+    for (int i = 0; i < 4; ++i)
+        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    if (c->ev_status) cudaEventDestroy(c->ev_status);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->copy_ev) cudaEventDestroy(c->copy_ev);
+}
+
+extern "C" {
+
+const char *odb_status_string(int status) {
+    switch (status) {
+    case ODB_OK: return "ok";
+    case ODB_ERR_INVALID_ARG: return "invalid argument";
+    case ODB_ERR_BAD_LENGTH: return "bad length (some sample length < 1)";
+    case ODB_ERR_CAPACITY: return "output capacity too small";
+    case ODB_ERR_CUDA: return "CUDA error";
+    case ODB_ERR_STATE: return "call order violated";
+    default: return "unknown status";
+    }
+}
+
+int odb_last_cuda_error(const odb_ctx *ctx) { return ctx ? ctx->last_cuda_error : 0; }
+int64_t odb_kernel_launches(const odb_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_ctx **out) {
+    if (!p || !out) return ODB_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (p->n_ranks < 1 || p->n_ranks > 65535 || p->budget < 1 || p->budget > 0x7fffffffll ||
+        (p->rule != ODB_RULE_THRESHOLD && p->rule != ODB_RULE_MAXFIT_ASC) || p->buffer_size < 0 || p->slot_capacity < 0 ||
+        max_samples_total < 0 || max_samples_total > 0x7fffff00ll || (p->join_mode != 0 && p->join_mode != 1) ||
+        (p->shift_labels != 0 && p->shift_labels != 1))
+        return ODB_ERR_INVALID_ARG;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) {
+        (void)cudaGetLastError();
+        return ODB_ERR_CUDA;  // no CPU fallback
+    }
+    odb_ctx *c = new (std::nothrow) odb_ctx();
+    if (!c) return ODB_ERR_CUDA;
+    c->prm = *p;
+    c->device = device;
+    c->n_max = max_samples_total;
+    memset(&c->info, 0, sizeof(c->info));
+    cudaError_t e = cudaSetDevice(device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e == cudaSuccess) c->sm_count = prop.multiProcessorCount;
+    const size_t N = (size_t)max_samples_total, R = (size_t)p->n_ranks;
+    if (e == cudaSuccess) e = dev_alloc(&c->d_rank_ptr, R + 1);
+    if (e == cudaSuccess) e = dev_alloc(&c->keyA, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->keyB, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->ovf, 2 * N + 2);
+    if (e == cudaSuccess) e = dev_alloc(&c->jA, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->jB, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->mark, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->flag, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->posflag, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->emitted, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->gpos, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->agpos, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->agcnt, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->agoff, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->left_ids, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->emit_ids, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->n_left, R);
+    if (e == cudaSuccess) e = dev_alloc(&c->fetch_pos, R);
+    if (e == cudaSuccess) e = dev_alloc(&c->emit_cur, R);
+    if (e == cudaSuccess) e = dev_alloc(&c->G, R);
+    if (e == cudaSuccess) e = dev_alloc(&c->S, R);
+    if (e == cudaSuccess) e = dev_alloc(&c->d_rec, 1);
+    if (e == cudaSuccess) e = dev_alloc(&c->d_tot, 1);
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_rec, sizeof(RoundRec));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_tot, sizeof(PlanTotals));
+    for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_status, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        free_all(c);
+        delete c;
+        return ODB_ERR_CUDA;
+    }
+    *out = c;
+    return ODB_OK;
+}
+
+int odb_destroy(odb_ctx *c) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    free_all(c);
+    delete c;
+    return ODB_OK;
+}
+
+int odb_reset(odb_ctx *c) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    c->state = 0;
+    c->round = 0;
+    c->n_rounds = 0;
+    c->n_steps = 0;
+    c->samples_emitted = 0;
+    c->n_finished = 0;
+    c->last_T = 0;
+    c->stop_reason = 0;
+    c->info_valid = false;
+    c->d_lengths = nullptr;
+    c->ev_valid = false;
+    return ODB_OK;
+}
+
+int odb_set_timing(odb_ctx *c, int enable) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    c->timing = enable ? 1 : 0;
+    c->ev_valid = false;
+    return ODB_OK;
+}
+
+int odb_get_timing(odb_ctx *c, float *ms3) {
+    if (!c || !ms3) return ODB_ERR_INVALID_ARG;
+    if (!c->timing || !c->ev_valid) return ODB_ERR_STATE;
+    CU(c, cudaEventSynchronize(c->ev[3]));
+    float plan = 0.f, col = 0.f, all = 0.f;
+    CU(c, cudaEventElapsedTime(&plan, c->ev[0], c->ev[1]));
+    CU(c, cudaEventElapsedTime(&col, c->ev[1], c->ev[2]));
+    CU(c, cudaEventElapsedTime(&all, c->ev[2], c->ev[3]));
+    ms3[0] = plan;
+    ms3[1] = col;
+    ms3[2] = all;
+    return ODB_OK;
+}
+
+// first round after create / reset: bind inputs, clear the per-run device state
+static int begin_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, cudaStream_t st) {
+    const int R = c->prm.n_ranks;
+    if (!h_rank_ptr) return ODB_ERR_INVALID_ARG;
+    if (h_rank_ptr[0] != 0) return ODB_ERR_INVALID_ARG;
+    int64_t max_nr = 0;
+    for (int r = 0; r < R; ++r) {
+        int64_t n = h_rank_ptr[r + 1] - h_rank_ptr[r];
+        if (n < 0) return ODB_ERR_INVALID_ARG;
+        max_nr = std::max(max_nr, n);
+    }
+    if (h_rank_ptr[R] > c->n_max) return ODB_ERR_INVALID_ARG;
+    if (h_rank_ptr[R] > 0 && !d_lengths) return ODB_ERR_INVALID_ARG;
+    c->h_rank_ptr.assign(h_rank_ptr, h_rank_ptr + R + 1);
+    c->n_total = h_rank_ptr[R];
+    c->max_nr = (int32_t)max_nr;
+    c->d_lengths = d_lengths;
+    CU(c, cudaSetDevice(c->device));
+    CU(c, cudaMemcpyAsync(c->d_rank_ptr, c->h_rank_ptr.data(), (R + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    CU(c, cudaMemsetAsync(c->n_left, 0, R * sizeof(int32_t), st));
+    CU(c, cudaMemsetAsync(c->fetch_pos, 0, R * sizeof(int32_t), st));
+    CU(c, cudaMemsetAsync(c->emit_cur, 0, R * sizeof(int32_t), st));
+    CU(c, cudaMemsetAsync(c->G, 0, R * sizeof(int32_t), st));
+    CU(c, cudaMemsetAsync(c->S, 0, R * sizeof(int32_t), st));
+    CU(c, cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st));
+    if (c->n_total > 0) CU(c, cudaMemsetAsync(c->emitted, 0, (size_t)c->n_total, st));
+    if (c->step_samples.p) CU(c, cudaMemsetAsync(c->step_samples.p, 0, c->step_samples.cap * sizeof(int32_t), st));
+    CU(c, launch_validate_lengths(c, st));
+    c->n_finished = 0;
+    for (int r = 0; r < R; ++r)
+        if (h_rank_ptr[r + 1] == h_rank_ptr[r]) c->n_finished++;
+    return ODB_OK;
+}
+
+// termination predicates, evaluated on the status shared by all ranks (Thm 3 proof P:341)
+static bool check_terminated(odb_ctx *c) {
+    const int R = c->prm.n_ranks;
+    if (c->prm.join_mode && c->n_finished == R) {
+        c->stop_reason = ODB_STOP_ALL_FINISHED;
+        return true;
+    }
+    if (!c->prm.join_mode && c->n_finished > 0) {
+        c->stop_reason = ODB_STOP_LOGICAL;
+        return true;
+    }
+    return false;
+}
+
+int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, void *stream) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_stream = st;
+    if (c->state == 0) {
+        int rc = begin_run(c, d_lengths, h_rank_ptr, st);
+        if (rc != ODB_OK) return rc;
+    } else if (c->state != 3) {
+        return ODB_ERR_STATE;
+    }
+    CU(c, cudaSetDevice(c->device));
+    if (check_terminated(c)) {
+        // the terminal check round: nothing to form; odb_align / odb_round_status report done
+        c->state = 1;
+        c->last_T = 0;
+        return ODB_OK;
+    }
+    const int R = c->prm.n_ranks;
+    // make room for this round's steps: T <= the largest window, and <= slot_capacity
+    int64_t bound = c->max_nr;
+    if (c->prm.buffer_size > 0) bound = std::min<int64_t>(bound, c->prm.buffer_size);
+    if (c->prm.slot_capacity > 0) bound = std::min<int64_t>(bound, c->prm.slot_capacity);
+    bound = std::max<int64_t>(bound, 1);
+    const int64_t need = (int64_t)c->n_steps + bound;
+    if (need > c->step_cap) {
+        const int64_t want = need + need / 2 + 64;
+        const size_t used = (size_t)c->n_steps * R;
+        CU(c, grow_preserve(c->st_count, (size_t)want * R, used, st));
+        CU(c, grow_preserve(c->st_width, (size_t)want * R, used, st));
+        CU(c, grow_preserve(c->st_idoff, (size_t)want * R, used, st));
+        CU(c, grow_preserve(c->st_round, (size_t)want * R, used, st));
+        CU(c, grow_preserve(c->step_samples, (size_t)want, (size_t)c->n_steps, st));
+        c->step_cap = want;
+    }
+    CU(c, cudaMemsetAsync(&c->d_rec->n_finished, 0, sizeof(int32_t), st));
+    CU(c, launch_round_form(c, st));
+    c->state = 1;
+    c->last_T = -1;
+    return ODB_OK;
+}
+
+int odb_align(odb_ctx *c, void *stream) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (c->state != 1) return ODB_ERR_STATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(c, cudaSetDevice(c->device));
+    if (c->last_T == 0) {  // terminal check round
+        c->state = 2;
+        return ODB_OK;
+    }
+    CU(c, launch_round_align(c, st));
+    CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, st));
+    CU(c, cudaEventRecord(c->ev_status, st));
+    c->state = 2;
+    return ODB_OK;
+}
+
+int odb_round_status(odb_ctx *c, int32_t *h_done, int32_t *h_T) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (c->state != 2) return ODB_ERR_STATE;
+    if (c->last_T == 0) {  // the terminal check round
+        if (c->round == 0 && c->n_total > 0) {  // no emitting round ran: still report bad lengths
+            CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, c->last_stream));
+            CU(c, cudaStreamSynchronize(c->last_stream));
+            if (c->h_rec->bad_length) {
+                c->state = 0;
+                return ODB_ERR_BAD_LENGTH;
+            }
+        }
+        c->n_rounds = c->round + 1;
+        c->state = 4;
+        if (h_done) *h_done = 1;
+        if (h_T) *h_T = 0;
+        return ODB_OK;
+    }
+    CU(c, cudaEventSynchronize(c->ev_status));
+    const RoundRec rec = *c->h_rec;
+    if (rec.bad_length) {
+        c->state = 0;
+        return ODB_ERR_BAD_LENGTH;
+    }
+    c->last_T = rec.T;
+    c->n_steps += rec.T_emit;
+    c->samples_emitted += rec.emitted_round;
+    c->n_finished = rec.n_finished;
+    c->round += 1;
+    if (h_T) *h_T = rec.T;
+    if (rec.quota_hit) {
+        c->stop_reason = ODB_STOP_QUOTA;
+        c->n_rounds = c->round;
+        c->state = 4;
+        if (h_done) *h_done = 1;
+        return ODB_OK;
+    }
+    c->state = 3;
+    if (h_done) *h_done = 0;
+    return ODB_OK;
+}
+
+int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
+    if (!c || !h_out) return ODB_ERR_INVALID_ARG;
+    if (c->state == 5 && c->info_valid) {
+        *h_out = c->info;
+        return ODB_OK;
+    }
+    if (c->state != 4) return ODB_ERR_STATE;
+    CU(c, cudaSetDevice(c->device));
+    cudaStream_t st = c->last_stream;  // the stream of the last odb_form_groups / odb_align
+    const int R = c->prm.n_ranks;
+    const size_t n_slots = (size_t)R * (size_t)c->n_steps;
+    CU(c, c->grp_count.ensure(n_slots + 1));
+    CU(c, c->grp_width.ensure(n_slots + 1));
+    CU(c, c->grp_round.ensure(n_slots + 1));
+    CU(c, c->grp_valid.ensure(n_slots + 1));
+    CU(c, c->grp_real.ensure(n_slots + 1));
+    CU(c, c->grp_idoff.ensure(n_slots + 1));
+    CU(c, c->grp_offset.ensure(n_slots + 1));
+    CU(c, c->grp_sample_ptr.ensure(n_slots + 1));
+    CU(c, c->grp_sample_ids.ensure((size_t)c->n_total + 1));
+    CU(c, c->left_out.ensure((size_t)c->n_total + 1));
+    CU(c, c->left_ptr.ensure((size_t)R + 1));
+    CU(c, c->step_valid.ensure((size_t)c->n_steps + 1));
+    CU(c, launch_finalize(c, st));
+    CU(c, cudaMemcpyAsync(c->h_tot, c->d_tot, sizeof(PlanTotals), cudaMemcpyDeviceToHost, st));
+    CU(c, cudaStreamSynchronize(st));
+    odb_plan_info &I = c->info;
+    I.n_rounds = c->n_rounds;
+    I.n_steps = c->n_steps;
+    I.stop_reason = c->stop_reason;
+    I.reserved = 0;
+    I.n_slots = (int64_t)n_slots;
+    I.total_elems = c->h_tot->total_elems;
+    I.samples_emitted = c->h_tot->samples_emitted;
+    I.samples_left = c->h_tot->samples_left;
+    I.real_tokens = (int64_t)c->h_tot->real_tokens;
+    I.padded_elems = c->h_tot->padded_elems;
+    c->info_valid = true;
+    c->state = 5;
+    *h_out = I;
+    return ODB_OK;
+}
+
+static int check_capacity(const odb_ctx *c, const odb_outputs *o) {
+    const odb_plan_info &I = c->info;
+    if (I.total_elems > 0) {
+        if (!o->d_input_ids || !o->d_labels || !o->d_position_ids || !o->d_attention_mask) return ODB_ERR_INVALID_ARG;
+        if (o->arena_capacity < I.total_elems) return ODB_ERR_CAPACITY;
+    }
+    const bool any_slot_tab = o->d_grp_count || o->d_grp_width || o->d_grp_round || o->d_grp_valid_tokens ||
+                              o->d_grp_real_tokens || o->d_grp_offset || o->d_grp_sample_ptr;
+    if (any_slot_tab && o->slot_capacity_alloc < I.n_slots) return ODB_ERR_CAPACITY;
+    if (o->d_grp_sample_ids && o->ids_capacity < I.samples_emitted) return ODB_ERR_CAPACITY;
+    if ((o->d_step_samples || o->d_step_valid_tokens) && o->step_capacity_alloc < I.n_steps) return ODB_ERR_CAPACITY;
+    if (o->d_left_ids && o->left_capacity < I.samples_left) return ODB_ERR_CAPACITY;
+    return ODB_OK;
+}
+
+// collate slots of ranks [r_lo, r_hi) (rank-major slots are contiguous in the arenas)
+static int collate_ranks(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_span_lo, const int32_t *d_span_hi,
+                         const odb_outputs *o, int r_lo, int r_hi, const std::vector<int64_t> &h_rank_off,
+                         cudaStream_t st) {
+    CollateArgs A;
+    A.tokens = d_tokens;
+    A.rows = c->rows.p;
+    A.row_sp = c->row_sp.p;
+    A.span_lo = d_span_lo;
+    A.span_hi = d_span_hi;
+    A.grp_offset = c->grp_offset.p;
+    A.grp_sample_ptr = c->grp_sample_ptr.p;
+    A.grp_count = c->grp_count.p;
+    A.grp_width = c->grp_width.p;
+    A.tile_slot = c->tile_slot.p;
+    A.ids = o->d_input_ids;
+    A.labels = o->d_labels;
+    A.pos = o->d_position_ids;
+    A.mask = o->d_attention_mask;
+    A.grp_valid = c->grp_valid.p;
+    A.total_elems = h_rank_off[r_hi];
+    // tiles are arena-aligned; a rank boundary inside a tile is handled by processing the boundary
+    // tile in the launch that owns its first element (offsets are multiples of 16, tiles of 4096)
+    A.tile_lo = (h_rank_off[r_lo] + kColTile - 1) / kColTile;
+    if (r_lo == 0) A.tile_lo = 0;
+    A.tile_hi = (h_rank_off[r_hi] + kColTile - 1) / kColTile;
+    A.pad_id = c->prm.pad_id;
+    A.ignore_index = c->prm.ignore_index;
+    A.shift_labels = c->prm.shift_labels;
+    CU(c, launch_collate(c, A, st));
+    return ODB_OK;
+}
+
+static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
+                        const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *o, cudaStream_t st) {
+    const odb_plan_info &I = c->info;
+    const int R = c->prm.n_ranks;
+    const size_t n_slots = (size_t)I.n_slots;
+    if (I.samples_emitted > 0 && (!d_tokens || !d_sample_ptr)) return ODB_ERR_INVALID_ARG;
+    if (((uintptr_t)d_tokens & 15u) != 0) return ODB_ERR_INVALID_ARG;
+    if (((uintptr_t)o->d_input_ids & 15u) || ((uintptr_t)o->d_labels & 15u) || ((uintptr_t)o->d_position_ids & 15u) ||
+        ((uintptr_t)o->d_attention_mask & 15u))
+        return ODB_ERR_INVALID_ARG;
+    const int64_t n_tiles = (I.total_elems + kColTile - 1) / kColTile;
+    CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
+    CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
+    CU(c, c->tile_slot.ensure((size_t)n_tiles + 1));
+    CU(c, launch_row_desc(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st));
+    CU(c, launch_tile_slots(c, n_tiles, st));
+    if (n_slots) CU(c, cudaMemsetAsync(c->grp_valid.p, 0, n_slots * sizeof(int32_t), st));
+    // ev[1]..ev[2] brackets the collate kernel alone; the pre/post work is ev[0]..ev[1] / ev[2]..ev[3]
+    if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
+    std::vector<int64_t> rank_off(2);
+    rank_off[0] = 0;
+    rank_off[1] = I.total_elems;
+    {
+        // whole arena in one launch: pretend one "rank" spanning everything
+        int rc = collate_ranks(c, d_tokens, d_span_lo, d_span_hi, o, 0, 1, rank_off, st);
+        if (rc != ODB_OK) return rc;
+    }
+    if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
+    CU(c, launch_step_valid(c, c->step_valid.p, st));
+    // tables
+    CU(c, copy_tab(o->d_grp_count, c->grp_count.p, n_slots, st));
+    CU(c, copy_tab(o->d_grp_width, c->grp_width.p, n_slots, st));
+    CU(c, copy_tab(o->d_grp_round, c->grp_round.p, n_slots, st));
+    CU(c, copy_tab(o->d_grp_valid_tokens, c->grp_valid.p, n_slots, st));
+    CU(c, copy_tab(o->d_grp_real_tokens, c->grp_real.p, n_slots, st));
+    CU(c, copy_tab(o->d_grp_offset, c->grp_offset.p, n_slots, st));
+    CU(c, copy_tab(o->d_grp_sample_ptr, c->grp_sample_ptr.p, n_slots + 1, st));
+    CU(c, copy_tab(o->d_grp_sample_ids, c->grp_sample_ids.p, (size_t)I.samples_emitted, st));
+    CU(c, copy_tab(o->d_step_samples, c->step_samples.p, (size_t)I.n_steps, st));
+    CU(c, copy_tab(o->d_step_valid_tokens, c->step_valid.p, (size_t)I.n_steps, st));
+    CU(c, copy_tab(o->d_left_ptr, c->left_ptr.p, (size_t)R + 1, st));
+    CU(c, copy_tab(o->d_left_ids, c->left_out.p, (size_t)I.samples_left, st));
+    if (c->timing) {
+        CU(c, cudaEventRecord(c->ev[3], st));
+        c->ev_valid = true;
+    }
+    return ODB_OK;
+}
+
+int odb_collate(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
+                const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *o, void *stream) {
+    if (!c || !o) return ODB_ERR_INVALID_ARG;
+    if (c->state != 5) return ODB_ERR_STATE;
+    CU(c, cudaSetDevice(c->device));
+    int rc = check_capacity(c, o);
+    if (rc != ODB_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (c->timing) CU(c, cudaEventRecord(c->ev[0], st));
+    return collate_impl(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
+}
+
+static int run_rounds(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out,
+                      cudaStream_t st) {
+    odb_reset(c);
+    if (c->timing) CU(c, cudaEventRecord(c->ev[0], st));
+    int32_t done = 0, T = 0;
+    while (!done) {
+        int rc = odb_form_groups(c, d_lengths, h_rank_ptr, st);
+        if (rc != ODB_OK) return rc;
+        rc = odb_align(c, st);
+        if (rc != ODB_OK) return rc;
+        rc = odb_round_status(c, &done, &T);
+        if (rc != ODB_OK) return rc;
+    }
+    return odb_plan_query(c, h_out);
+}
+
+int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
+            const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo, const int32_t *d_span_hi,
+            const odb_outputs *o, odb_plan_info *h_out, void *stream) {
+    if (!c || !o || !h_out) return ODB_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = run_rounds(c, d_lengths, h_rank_ptr, h_out, st);
+    if (rc != ODB_OK) return rc;
+    rc = check_capacity(c, o);
+    if (rc != ODB_OK) return rc;
+    c->ev_valid = c->timing != 0;  // ev[0] was recorded by run_rounds
+    rc = collate_impl(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
+    return rc;
+}
+
+int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
+                 const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
+                 const int32_t *h_span_hi, const odb_outputs *ho, odb_plan_info *h_out, void *stream) {
+    if (!c || !ho || !h_out || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(c, cudaSetDevice(c->device));
+    const int R = c->prm.n_ranks;
+    const int64_t N = h_rank_ptr[R];
+    if (N < 0 || N > c->n_max) return ODB_ERR_INVALID_ARG;
+    if (N > 0 && (!h_lengths || !h_sample_ptr || !h_tokens)) return ODB_ERR_INVALID_ARG;
+    const int64_t n_tok = N > 0 ? h_sample_ptr[N] : 0;
+    const int64_t n_span = (h_span_ptr && N > 0) ? h_span_ptr[N] : 0;
+    // inputs host -> device (lengths first: planning needs nothing else)
+    CU(c, c->hs_lengths.ensure((size_t)N + 1));
+    CU(c, c->hs_sample_ptr.ensure((size_t)N + 1));
+    CU(c, c->hs_span_ptr.ensure((size_t)N + 1));
+    CU(c, c->hs_span_lo.ensure((size_t)n_span + 1));
+    CU(c, c->hs_span_hi.ensure((size_t)n_span + 1));
+    CU(c, c->hs_tokens.ensure((size_t)n_tok + 4));
+    if (!c->copy_stream) {
+        CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        CU(c, cudaEventCreateWithFlags(&c->copy_ev, cudaEventDisableTiming));
+    }
+    if (N > 0) CU(c, cudaMemcpyAsync(c->hs_lengths.p, h_lengths, (size_t)N * 4, cudaMemcpyHostToDevice, st));
+    // tokens and the CSR arrays go on the copy stream, overlapping the planning kernels
+    CU(c, cudaEventRecord(c->copy_ev, st));
+    CU(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev, 0));
+    if (N > 0) {
+        CU(c, cudaMemcpyAsync(c->hs_sample_ptr.p, h_sample_ptr, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, c->copy_stream));
+        if (h_span_ptr) {
+            CU(c, cudaMemcpyAsync(c->hs_span_ptr.p, h_span_ptr, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, c->copy_stream));
+            if (n_span) {
+                CU(c, cudaMemcpyAsync(c->hs_span_lo.p, h_span_lo, (size_t)n_span * 4, cudaMemcpyHostToDevice, c->copy_stream));
+                CU(c, cudaMemcpyAsync(c->hs_span_hi.p, h_span_hi, (size_t)n_span * 4, cudaMemcpyHostToDevice, c->copy_stream));
+            }
+        }
+        if (n_tok) CU(c, cudaMemcpyAsync(c->hs_tokens.p, h_tokens, (size_t)n_tok * 4, cudaMemcpyHostToDevice, c->copy_stream));
+    }
+    CU(c, cudaEventRecord(c->copy_ev, c->copy_stream));
+    int rc = run_rounds(c, c->hs_lengths.p, h_rank_ptr, h_out, st);
+    if (rc != ODB_OK) {
+        cudaStreamSynchronize(c->copy_stream);
+        return rc;
+    }
+    const odb_plan_info I = *h_out;
+    // host capacities
+    rc = ODB_OK;
+    {
+        odb_outputs chk = *ho;
+        const odb_plan_info &J = I;
+        if (J.total_elems > 0 && (!chk.d_input_ids || !chk.d_labels || !chk.d_position_ids || !chk.d_attention_mask))
+            rc = ODB_ERR_INVALID_ARG;
+        else if (J.total_elems > chk.arena_capacity)
+            rc = ODB_ERR_CAPACITY;
+        const bool any_slot_tab = chk.d_grp_count || chk.d_grp_width || chk.d_grp_round || chk.d_grp_valid_tokens ||
+                                  chk.d_grp_real_tokens || chk.d_grp_offset || chk.d_grp_sample_ptr;
+        if (rc == ODB_OK && any_slot_tab && chk.slot_capacity_alloc < J.n_slots) rc = ODB_ERR_CAPACITY;
+        if (rc == ODB_OK && chk.d_grp_sample_ids && chk.ids_capacity < J.samples_emitted) rc = ODB_ERR_CAPACITY;
+        if (rc == ODB_OK && (chk.d_step_samples || chk.d_step_valid_tokens) && chk.step_capacity_alloc < J.n_steps)
+            rc = ODB_ERR_CAPACITY;
+        if (rc == ODB_OK && chk.d_left_ids && chk.left_capacity < J.samples_left) rc = ODB_ERR_CAPACITY;
+    }
+    if (rc != ODB_OK) {
+        cudaStreamSynchronize(c->copy_stream);
+        return rc;
+    }
+    const size_t E = (size_t)I.total_elems;
+    CU(c, c->hs_ids.ensure(E + 16));
+    CU(c, c->hs_labels.ensure(E + 16));
+    CU(c, c->hs_pos.ensure(E + 16));
+    CU(c, c->hs_mask.ensure(E + 16));
+    odb_outputs dev;
+    memset(&dev, 0, sizeof(dev));
+    dev.d_input_ids = c->hs_ids.p;
+    dev.d_labels = c->hs_labels.p;
+    dev.d_position_ids = c->hs_pos.p;
+    dev.d_attention_mask = c->hs_mask.p;
+    dev.arena_capacity = (int64_t)E;
+    CU(c, cudaStreamWaitEvent(st, c->copy_ev, 0));  // tokens have landed
+    c->ev_valid = c->timing != 0;
+    rc = collate_impl(c, c->hs_tokens.p, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p,
+                      c->hs_span_hi.p, &dev, st);
+    if (rc != ODB_OK) return rc;
+    // results device -> host
+    const size_t n_slots = (size_t)I.n_slots;
+    auto d2h = [&](void *dst, const void *src, size_t bytes) -> cudaError_t {
+        if (!dst || bytes == 0) return cudaSuccess;
+        return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
+    };
+    CU(c, d2h(ho->d_input_ids, c->hs_ids.p, E * 4));
+    CU(c, d2h(ho->d_labels, c->hs_labels.p, E * 4));
+    CU(c, d2h(ho->d_position_ids, c->hs_pos.p, E * 4));
+    CU(c, d2h(ho->d_attention_mask, c->hs_mask.p, E));
+    CU(c, d2h(ho->d_grp_count, c->grp_count.p, n_slots * 4));
+    CU(c, d2h(ho->d_grp_width, c->grp_width.p, n_slots * 4));
+    CU(c, d2h(ho->d_grp_round, c->grp_round.p, n_slots * 4));
+    CU(c, d2h(ho->d_grp_valid_tokens, c->grp_valid.p, n_slots * 4));
+    CU(c, d2h(ho->d_grp_real_tokens, c->grp_real.p, n_slots * 4));
+    CU(c, d2h(ho->d_grp_offset, c->grp_offset.p, n_slots * 8));
+    CU(c, d2h(ho->d_grp_sample_ptr, c->grp_sample_ptr.p, (n_slots + 1) * 8));
+    CU(c, d2h(ho->d_grp_sample_ids, c->grp_sample_ids.p, (size_t)I.samples_emitted * 4));
+    CU(c, d2h(ho->d_step_samples, c->step_samples.p, (size_t)I.n_steps * 4));
+    CU(c, d2h(ho->d_step_valid_tokens, c->step_valid.p, (size_t)I.n_steps * 8));
+    CU(c, d2h(ho->d_left_ptr, c->left_ptr.p, (size_t)(R + 1) * 8));
+    CU(c, d2h(ho->d_left_ids, c->left_out.p, (size_t)I.samples_left * 4));
+    CU(c, cudaStreamSynchronize(st));
+    return ODB_OK;
+}
+
+int64_t odb_debug_read(odb_ctx *c, int what, void *h_dst, int64_t max_bytes) {
+    if (!c || !h_dst) return -1;
+    const void *src = nullptr;
+    int64_t bytes = 0;
+    const int R = c->prm.n_ranks;
+    switch (what) {
+    case 0: src = c->G; bytes = (int64_t)R * 4; break;
+    case 1: src = c->S; bytes = (int64_t)R * 4; break;
+    case 2: src = c->sorted; bytes = c->n_total * 8; break;
+    case 3: src = c->flag; bytes = c->n_total; break;
+    default: return -1;
+    }
+    if (!src) return -1;
+    bytes = std::min(bytes, max_bytes);
+    if (cudaSetDevice(c->device) != cudaSuccess) return -1;
+    if (cudaDeviceSynchronize() != cudaSuccess) return -1;
+    if (bytes > 0 && cudaMemcpy(h_dst, src, (size_t)bytes, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+    return bytes;
+}
+
+}  // extern "C"

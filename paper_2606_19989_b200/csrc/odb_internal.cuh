@@ -1,0 +1,192 @@
+// Internal declarations shared by the translation units of libodb (CUDA path only).
+// Nothing here is used by, or shared with, the CPU oracle under oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "odb.h"
+
+#define ODB_FULL_MASK 0xffffffffu
+
+namespace odb {
+
+// ---------------------------------------------------------------------------------------------
+// compile-time configuration
+// ---------------------------------------------------------------------------------------------
+constexpr int kSortChunk = 4096;    // keys sorted in shared memory by one CTA (A1)
+constexpr int kSortThreads = 512;
+constexpr int kMergeThreads = 256;
+constexpr int kRankThreads = 1024;  // one CTA per rank for A2..A8
+constexpr int kColThreads = 256;    // collate CTA (A10)
+constexpr int kColTile = 4096;      // padded elements per collate tile (multiple of 8 warps * 128)
+
+// Per-round status record: written by the round's kernels, copied to pinned host memory (A7).
+struct RoundRec {
+    int32_t T;           // Eq. 3 target of the round
+    int32_t T_emit;      // steps actually emitted (== T unless the quota cut fired)
+    int32_t quota_hit;   // 1 if the non-join sample quota was reached in this round
+    int32_t n_finished;  // ranks that will be "finished" (status -1) at the start of the next round
+    int32_t bad_length;  // some length < 1 was seen
+    int32_t pad_;
+    int64_t emitted_round;  // samples emitted in this round over all ranks
+};
+
+// Totals produced by the finalize kernels.
+struct PlanTotals {
+    int64_t total_elems;
+    int64_t samples_emitted;
+    int64_t padded_elems;
+    unsigned long long real_tokens;
+    int64_t samples_left;
+};
+
+// One emitted row (sample) as the collate kernel wants it: 32 bytes, two 16-byte loads.
+struct __align__(16) RowDesc {
+    int64_t tok;    // offset of the sample's first token in d_tokens
+    int32_t len;    // realized length
+    int32_t nspan;  // number of masked spans; the first two are inlined below
+    int32_t lo0, hi0, lo1, hi1;
+};
+
+struct CollateArgs {
+    const int32_t *tokens;
+    const RowDesc *rows;
+    const int64_t *row_sp;  // first span index of each row (only read when nspan > 2)
+    const int32_t *span_lo;
+    const int32_t *span_hi;
+    const int64_t *grp_offset;      // n_slots + 1
+    const int64_t *grp_sample_ptr;  // n_slots + 1
+    const int32_t *grp_count;
+    const int32_t *grp_width;
+    const int32_t *tile_slot;  // first slot overlapping each tile
+    int32_t *ids;
+    int32_t *labels;
+    int32_t *pos;
+    uint8_t *mask;
+    int32_t *grp_valid;
+    int64_t total_elems;
+    int64_t tile_lo, tile_hi;  // tiles [tile_lo, tile_hi) are processed by this launch
+    int32_t pad_id, ignore_index, shift_labels;
+};
+
+// growable device buffer (cudaMalloc on growth only)
+template <class T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t n, bool zero = false, cudaStream_t st = 0) {
+        if (n <= cap) return cudaSuccess;
+        if (p) {
+            cudaError_t e = cudaFree(p);
+            p = nullptr;
+            cap = 0;
+            if (e != cudaSuccess) return e;
+        }
+        size_t want = n + n / 4 + 16;
+        cudaError_t e = cudaMalloc((void **)&p, want * sizeof(T));
+        if (e != cudaSuccess) {
+            p = nullptr;
+            return e;
+        }
+        cap = want;
+        if (zero) return cudaMemsetAsync(p, 0, want * sizeof(T), st);
+        return cudaSuccess;
+    }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+};
+
+}  // namespace odb
+
+// The context.  Host-side state machine + device scratch.
+struct odb_ctx {
+    odb_params prm;
+    int device = 0;
+    int64_t n_max = 0;  // max_samples_total
+    int sm_count = 148;
+    int last_cuda_error = 0;
+    int64_t launches = 0;
+    int timing = 0;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+    cudaEvent_t ev_status = nullptr;
+    cudaStream_t last_stream = nullptr;
+
+    // inputs fixed by the first odb_form_groups after create / reset
+    const int32_t *d_lengths = nullptr;
+    std::vector<int64_t> h_rank_ptr;
+    int64_t n_total = 0;
+    int32_t max_nr = 0;
+
+    // state machine: 0 = fresh, 1 = groups formed, 2 = aligned (status pending), 3 = status read,
+    // 4 = terminated, 5 = plan queried
+    int state = 0;
+    int32_t round = 0;     // rounds fully processed (emitting rounds)
+    int32_t n_rounds = 0;  // including the terminal check once terminated
+    int32_t n_steps = 0;
+    int64_t samples_emitted = 0;
+    int32_t n_finished = 0;
+    int32_t last_T = 0;
+    int stop_reason = 0;
+    odb_plan_info info;
+    bool info_valid = false;
+
+    // device scratch sized by n_max (+ R)
+    int64_t *d_rank_ptr = nullptr;      // R+1
+    uint64_t *keyA = nullptr, *keyB = nullptr;  // n_max
+    uint64_t *sorted = nullptr;         // = keyA or keyB after the merge passes
+    uint64_t *ovf = nullptr;            // 2*n_max + 2 (overflow sort keys)
+    int32_t *jA = nullptr, *jB = nullptr;  // n_max + R
+    uint8_t *mark = nullptr;            // n_max + R
+    uint8_t *flag = nullptr;            // n_max
+    uint8_t *posflag = nullptr;         // n_max
+    uint8_t *emitted = nullptr;         // n_max
+    int32_t *gpos = nullptr;            // n_max + R
+    int32_t *agpos = nullptr, *agcnt = nullptr, *agoff = nullptr;  // n_max + R
+    int32_t *left_ids = nullptr, *emit_ids = nullptr;              // n_max
+    int32_t *n_left = nullptr, *fetch_pos = nullptr, *emit_cur = nullptr, *G = nullptr, *S = nullptr;  // R
+    odb::RoundRec *d_rec = nullptr;
+    odb::RoundRec *h_rec = nullptr;  // pinned
+    odb::PlanTotals *d_tot = nullptr;
+    odb::PlanTotals *h_tot = nullptr;  // pinned
+
+    // step-major staging tables [step * R + r], growable
+    odb::DevBuf<int32_t> st_count, st_width, st_idoff, st_round, step_samples;
+    int64_t step_cap = 0;
+
+    // rank-major plan tables built by odb_plan_query
+    odb::DevBuf<int32_t> grp_count, grp_width, grp_round, grp_valid, grp_real, grp_idoff;
+    odb::DevBuf<int64_t> grp_offset, grp_sample_ptr;
+    odb::DevBuf<int32_t> grp_sample_ids, left_out;
+    odb::DevBuf<int64_t> left_ptr, step_valid;
+    odb::DevBuf<odb::RowDesc> rows;
+    odb::DevBuf<int64_t> row_sp;
+    odb::DevBuf<int32_t> tile_slot;
+
+    // device staging for odb_run_host
+    odb::DevBuf<int32_t> hs_lengths, hs_tokens, hs_span_lo, hs_span_hi, hs_ids, hs_labels, hs_pos;
+    odb::DevBuf<int64_t> hs_sample_ptr, hs_span_ptr;
+    odb::DevBuf<uint8_t> hs_mask;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t copy_ev = nullptr;
+};
+
+namespace odb {
+// ---- launchers implemented in odb_plan.cu ----------------------------------------------------
+cudaError_t launch_validate_lengths(odb_ctx *c, cudaStream_t st);
+cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st);   // A0..A3
+cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commit
+cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st);     // A9 + tables + leftovers
+// ---- launchers implemented in odb_collate.cu -------------------------------------------------
+cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
+                            const int32_t *d_span_lo, const int32_t *d_span_hi, cudaStream_t st);
+cudaError_t launch_tile_slots(odb_ctx *c, int64_t n_tiles, cudaStream_t st);
+cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st);
+cudaError_t launch_step_valid(odb_ctx *c, int64_t *d_step_valid, cudaStream_t st);
+}  // namespace odb
