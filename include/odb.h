@@ -46,6 +46,13 @@
 extern "C" {
 #endif
 
+/* exported symbol (the library is built with -fvisibility=hidden) */
+#if defined(__GNUC__)
+#define ODB_API __attribute__((visibility("default")))
+#else
+#define ODB_API
+#endif
+
 typedef struct odb_ctx odb_ctx;
 
 enum {
@@ -122,40 +129,40 @@ typedef struct { /* device outputs, caller-allocated; any table pointer may be N
 
 /* Create a context on CUDA device `device` for at most max_samples_total samples over all ranks.
  * Validates params (ODB_ERR_INVALID_ARG).  Allocates scratch (~70 bytes per sample). */
-int odb_create(const odb_params *params, int device, int64_t max_samples_total, odb_ctx **out);
-int odb_destroy(odb_ctx *ctx);
+ODB_API int odb_create(const odb_params *params, int device, int64_t max_samples_total, odb_ctx **out);
+ODB_API int odb_destroy(odb_ctx *ctx);
 /* Forget all rounds and start over with the same params; keeps scratch. */
-int odb_reset(odb_ctx *ctx);
+ODB_API int odb_reset(odb_ctx *ctx);
 
 /* One protocol round, first half (section 2.2): fill each rank's window (recirculated leftovers +
  * the next un-fetched samples, up to buffer_size), sort it by (length, id), compute the greedy
  * successor of every start position and extract the candidate groups and G_r.  Lengths only; no
  * token is touched.  The first call after create/reset fixes d_lengths / h_rank_ptr (R+1 entries,
  * h_rank_ptr[R] <= max_samples_total) for the following rounds.  Asynchronous. */
-int odb_form_groups(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, void *stream);
+ODB_API int odb_form_groups(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, void *stream);
 
 /* Second half (section 2.3, Alg. 1): T_grp by an on-device reduction over the R ranks, split /
  * overflow, IDLE slots, step totals, the non-join quota cut, leftovers.  Asynchronous. */
-int odb_align(odb_ctx *ctx, void *stream);
+ODB_API int odb_align(odb_ctx *ctx, void *stream);
 
 /* Synchronises.  *h_done != 0 when the protocol has terminated (no further round may be formed);
  * *h_T = T_grp of the round just aligned (0 if the round was the terminal check).  Must be called
  * after every odb_align.  Returns ODB_ERR_BAD_LENGTH if some length < 1. */
-int odb_round_status(odb_ctx *ctx, int32_t *h_done, int32_t *h_T);
+ODB_API int odb_round_status(odb_ctx *ctx, int32_t *h_done, int32_t *h_T);
 
 /* Synchronises.  Builds the rank-major slot tables and block offsets; fills *h_out so the caller
  * can size the output arenas.  Only after termination (ODB_ERR_STATE otherwise). */
-int odb_plan_query(odb_ctx *ctx, odb_plan_info *h_out);
+ODB_API int odb_plan_query(odb_ctx *ctx, odb_plan_info *h_out);
 
 /* Collate every emitted slot (C.4 in DESIGN.md) and fill the tables of `out`.  Requires
  * odb_plan_query.  ODB_ERR_CAPACITY if an arena or table is too small.  Asynchronous. */
-int odb_collate(odb_ctx *ctx, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
+ODB_API int odb_collate(odb_ctx *ctx, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
                 const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *out, void *stream);
 
 /* Everything: reset, the round loop until termination, plan query, one collate over all emitted
  * steps.  Synchronises once per round (a few bytes of status) and once for the plan sizes; returns
  * with the collate kernels enqueued on `stream`.  On ODB_ERR_CAPACITY *h_out is still filled. */
-int odb_run(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
+ODB_API int odb_run(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
             const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
             const int32_t *d_span_hi, const odb_outputs *out, odb_plan_info *h_out, void *stream);
 
@@ -163,7 +170,7 @@ int odb_run(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, c
  * spans and tokens host->device, runs the whole path, copies the four arenas and every non-NULL
  * table of `h_out_bufs` (same struct, HOST pointers) back, rank by rank so that copies overlap the
  * collate kernel.  Synchronises before returning.  n_spans = h_span_ptr[N]. */
-int odb_run_host(odb_ctx *ctx, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
+ODB_API int odb_run_host(odb_ctx *ctx, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
                  const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
                  const int32_t *h_span_hi, const odb_outputs *h_out_bufs, odb_plan_info *h_out, void *stream);
 
@@ -171,18 +178,24 @@ int odb_run_host(odb_ctx *ctx, const int32_t *h_lengths, const int64_t *h_rank_p
  * CUDA events on the launching stream: ms[0] = planning (all rounds, plan query, row descriptors and
  * the tile table), ms[1] = the collate kernel alone, ms[2] = what follows it (step totals, table
  * copies).  Synchronises.  Enabled by odb_set_timing(ctx, 1); off by default. */
-int odb_set_timing(odb_ctx *ctx, int enable);
-int odb_get_timing(odb_ctx *ctx, float *ms3);
+ODB_API int odb_set_timing(odb_ctx *ctx, int enable);
+ODB_API int odb_get_timing(odb_ctx *ctx, float *ms3);
 /* Number of kernels this context has launched since odb_create (diagnostics / bench accounting). */
-int64_t odb_kernel_launches(const odb_ctx *ctx);
+ODB_API int64_t odb_kernel_launches(const odb_ctx *ctx);
 
 /* Diagnostics: copy an internal device table to the host (synchronises).  `what`: 0 = G_r (int32[R])
  * of the last round, 1 = S_r (int32[R]), 2 = sorted keys of the last round ((len<<32)|id, uint64[N],
  * rank regions at h_rank_ptr), 3 = candidate start flags (uint8[N]).  Returns bytes copied or < 0. */
-int64_t odb_debug_read(odb_ctx *ctx, int what, void *h_dst, int64_t max_bytes);
+ODB_API int64_t odb_debug_read(odb_ctx *ctx, int what, void *h_dst, int64_t max_bytes);
 
-int odb_last_cuda_error(const odb_ctx *ctx);
-const char *odb_status_string(int status);
+/* Synthetic-input utility (benchmarks / tests; not part of the method): d_tokens[j] for j in
+ * [0, count) = the counter-based id of global token index start + j,
+ *   ((mix64(seed * 0x9E3779B97F4A7C15 + start + j) >> 32) * vocab) >> 32,  mix64 = SplitMix64 finaliser
+ * (DESIGN.md "Input recipe").  Asynchronous on `stream`. */
+ODB_API int odb_synth_tokens(int32_t *d_tokens, int64_t start, int64_t count, uint64_t seed, int32_t vocab, void *stream);
+
+ODB_API int odb_last_cuda_error(const odb_ctx *ctx);
+ODB_API const char *odb_status_string(int status);
 
 #ifdef __cplusplus
 }

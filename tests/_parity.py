@@ -1,0 +1,169 @@
+"""Shared machinery of the GPU parity tests: run one workload through the CUDA path (C ABI via the
+binding) and through the CPU oracle, and compare bit for bit."""
+from __future__ import annotations
+
+import numpy as np
+
+import odb_inputs as I
+
+SENTINEL = 0x5A
+PLAN_SCALARS = ("n_rounds", "n_steps", "stop_reason", "n_slots", "total_elems", "samples_emitted", "samples_left",
+                "real_tokens", "padded_elems")
+SLOT_TABLES = ("grp_count", "grp_width", "grp_round", "grp_offset", "grp_real_tokens", "grp_sample_ptr")
+
+
+class DeviceWorkload:
+    """A Workload's arrays resident on the GPU (tokens filled on the device by odb_synth_tokens)."""
+
+    def __init__(self, wl, device="cuda:0", tokens_from_host=None):
+        import torch
+        import paper_2606_19989_b200 as P
+        self.wl = wl
+        self.device = device
+        t = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).to(device)
+        self.lengths = t(wl.lengths, torch.int32)
+        self.sample_ptr = t(wl.sample_ptr, torch.int64)
+        self.span_ptr = t(wl.span_ptr, torch.int64)
+        self.span_lo = t(wl.span_lo, torch.int32) if len(wl.span_lo) else torch.zeros(1, dtype=torch.int32, device=device)
+        self.span_hi = t(wl.span_hi, torch.int32) if len(wl.span_hi) else torch.zeros(1, dtype=torch.int32, device=device)
+        n_tok = wl.n_tokens
+        self.tokens = torch.empty(n_tok + 16, dtype=torch.int32, device=device)
+        if tokens_from_host is not None:
+            self.tokens[:n_tok].copy_(torch.from_numpy(tokens_from_host))
+        else:
+            P.odb_synth_tokens(self.tokens, 0, n_tok, wl.token_seed, I.VOCAB)
+        torch.cuda.synchronize()
+
+
+def gpu_params(wl):
+    import paper_2606_19989_b200 as P
+    p = wl.params
+    return P.make_params(wl.n_ranks, p["budget"], rule=p["rule"], join_mode=p["join_mode"],
+                         sample_quota=p["sample_quota"], emitted_so_far=p["emitted_so_far"],
+                         buffer_size=p["buffer_size"], slot_capacity=p["slot_capacity"], pad_id=p["pad_id"],
+                         ignore_index=p["ignore_index"], shift_labels=p["shift_labels"])
+
+
+def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL):
+    """Returns (info, OutputBuffers, round_T).  staged=True uses form_groups/align/round_status/
+    plan_query/collate; staged=False uses odb_run (two calls: the first sizes the outputs)."""
+    import torch
+    import paper_2606_19989_b200 as P
+    dw = dw or DeviceWorkload(wl)
+    with P.Odb(gpu_params(wl), max(wl.n_samples, 1)) as ctx:
+        if staged:
+            info = ctx.plan(dw.lengths, wl.rank_ptr)
+            round_T = list(ctx.round_T)
+            out = P.OutputBuffers.for_plan(wl.n_ranks, info, dw.device, fill=fill)
+            P.odb_collate(ctx.h, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out.struct)
+        else:
+            empty = P.OutputBuffers(wl.n_ranks, 0, 0, 0, 0, 0, dw.device)
+            info = P.odb_run(ctx.h, dw.lengths, wl.rank_ptr, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo,
+                             dw.span_hi, empty.struct, allow_capacity_error=True)
+            out = P.OutputBuffers.for_plan(wl.n_ranks, info, dw.device, fill=fill)
+            info = P.odb_run(ctx.h, dw.lengths, wl.rank_ptr, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo,
+                             dw.span_hi, out.struct)
+            round_T = None
+        torch.cuda.synchronize()
+    return info, out, round_T
+
+
+def compare_plan(plan, info, out, round_T=None):
+    """Plan scalars, per-slot tables, CSR of ids, step samples, leftovers: all bit-exact."""
+    for k in PLAN_SCALARS:
+        assert int(getattr(info, k)) == int(getattr(plan, k)), (k, int(getattr(info, k)), int(getattr(plan, k)))
+    if round_T is not None:
+        assert list(round_T) == plan.round_T.tolist()
+    for name in SLOT_TABLES + ("grp_sample_ids", "step_samples", "left_ptr", "left_ids"):
+        g = out.table(name).cpu().numpy()
+        o = getattr(plan, name)
+        assert g.shape == o.shape, (name, g.shape, o.shape)
+        if not np.array_equal(g, o):
+            bad = np.flatnonzero(g != o)
+            raise AssertionError("%s differs at %d entries, first %d: gpu %r oracle %r" % (name, len(bad), bad[0],
+                                                                                        g[bad[0]], o[bad[0]]))
+
+
+def compare_full(plan, oracle_out, info, out):
+    """Arenas byte for byte (gaps must still hold the sentinel), valid-token tables."""
+    E = plan.total_elems
+    for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+        g = getattr(out, name)[:E].cpu().numpy()
+        o = oracle_out[name][:E]
+        if not np.array_equal(g, o):
+            bad = np.flatnonzero(g != o)
+            s = int(np.searchsorted(plan.grp_offset, bad[0], side="right") - 1)
+            raise AssertionError("%s differs at %d elements; first at %d (slot %d, offset %d, count %d, width %d): "
+                                 "gpu %r oracle %r" % (name, len(bad), bad[0], s, plan.grp_offset[s],
+                                                       plan.grp_count[s], plan.grp_width[s], g[bad[0]], o[bad[0]]))
+        # tail guard: the 16 spare elements past total_elems were never written
+        tail = getattr(out, name)[E:].cpu().numpy().view(np.uint8)
+        assert (tail == SENTINEL).all(), name + ": wrote past total_elems"
+    assert np.array_equal(out.table("grp_valid_tokens").cpu().numpy(), oracle_out["grp_valid_tokens"])
+    assert np.array_equal(out.table("step_valid_tokens").cpu().numpy(), oracle_out["step_valid_tokens"])
+
+
+def compare_sampled_slots(wl, plan, out, slots):
+    """Collate the listed slots one by one with the oracle (tokens regenerated from the hash for just
+    their samples) and compare with the GPU arenas; also the slot's valid-token count."""
+    p = wl.params
+    gv = out.table("grp_valid_tokens").cpu().numpy()
+    for s in slots:
+        s = int(s)
+        r = s // plan.n_steps
+        c, w, off = int(plan.grp_count[s]), int(plan.grp_width[s]), int(plan.grp_offset[s])
+        ids = plan.grp_sample_ids[plan.grp_sample_ptr[s]:plan.grp_sample_ptr[s + 1]].astype(np.int64) + wl.rank_ptr[r]
+        toks, toff = I.tokens_for_samples(wl, ids)
+        tok_start = np.zeros(max(wl.n_samples, 1), dtype=np.int64)
+        tok_start[ids] = toff
+        ref = plan.collate_slot(s, toks if len(toks) else np.zeros(1, np.int32), tok_start, wl.span_ptr, wl.span_lo,
+                                wl.span_hi, pad_id=p["pad_id"], ignore_index=p["ignore_index"],
+                                shift_labels=p["shift_labels"])
+        n = c * w
+        for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+            g = getattr(out, name)[off:off + n].cpu().numpy().reshape(c, w)
+            assert np.array_equal(g, ref[name]), (name, "slot", s, "count", c, "width", w)
+        assert int(gv[s]) == ref["valid"], ("grp_valid_tokens", s)
+        # the alignment gap after the block is untouched
+        gap_hi = int(plan.grp_offset[s + 1]) if s + 1 < plan.n_slots else plan.total_elems
+        if gap_hi > off + n:
+            gap = out.attention_mask[off + n:gap_hi].cpu().numpy()
+            assert (gap == SENTINEL).all(), ("gap written", s)
+
+
+def device_self_consistency(info, out, ignore_index=-100):
+    """Properties that hold at any size, checked on the device output itself: the valid-token table
+    equals a recount of labels != ignore_index per slot; step totals are its column sums; the mask
+    count equals real_tokens; gaps still hold the sentinel."""
+    import torch
+    E = int(info.total_elems)
+    n_slots, n_steps = int(info.n_slots), int(info.n_steps)
+    if n_slots == 0:
+        return
+    off = out.table("grp_offset")
+    cnt = out.table("grp_count").to(torch.int64)
+    wid = out.table("grp_width").to(torch.int64)
+    area = cnt * wid
+    lab = out.labels[:E]
+    msk = out.attention_mask[:E]
+    # element -> slot via the offsets; in-block flag
+    # (chunked to bound memory)
+    valid = torch.zeros(n_slots, dtype=torch.int64, device=lab.device)
+    real = torch.zeros(n_slots, dtype=torch.int64, device=lab.device)
+    gaps_ok = True
+    CH = 1 << 26
+    for a0 in range(0, E, CH):
+        a1 = min(E, a0 + CH)
+        idx = torch.arange(a0, a1, device=lab.device, dtype=torch.int64)
+        sl = torch.searchsorted(off, idx, right=True) - 1
+        inblk = (idx - off[sl]) < area[sl]
+        v = (lab[a0:a1] != ignore_index) & inblk
+        valid.index_add_(0, sl, v.to(torch.int64))
+        real.index_add_(0, sl, ((msk[a0:a1] == 1) & inblk).to(torch.int64))
+        gaps_ok = gaps_ok and bool((msk[a0:a1][~inblk] == SENTINEL).all())
+    assert gaps_ok, "an alignment gap was written"
+    assert torch.equal(valid, out.table("grp_valid_tokens").to(torch.int64))
+    assert torch.equal(real, out.table("grp_real_tokens").to(torch.int64))
+    assert int(real.sum()) == int(info.real_tokens)
+    sv = out.table("grp_valid_tokens").to(torch.int64).view(-1, n_steps).sum(0)
+    assert torch.equal(sv, out.table("step_valid_tokens"))

@@ -1,0 +1,228 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit, on the same
+seeded inputs.  Everything on this path is integer / index work, so the bar is exact equality
+(BASELINE.json north_star).  Run on the B200 box: ``pytest -m gpu``."""
+import numpy as np
+import pytest
+
+import odb_inputs as I
+from tests import _parity as Par
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests must run on the B200 box (there is no CPU fallback)")
+    import paper_2606_19989_b200 as P
+    P.load()
+    return P
+
+
+def _full_parity(oracle, wl, staged=True):
+    plan, ref = oracle.run_workload(wl)
+    info, out, round_T = Par.run_gpu(wl, staged=staged)
+    Par.compare_plan(plan, info, out, round_T)
+    Par.compare_full(plan, ref, info, out)
+    return plan, info, out
+
+
+# ---- input generator: the device token fill equals the host specification ---------------------
+def test_synth_tokens_match_host_hash(P):
+    import torch
+    n = 100_003
+    for seed, start in ((0, 0), (4, 2_000_000_000), (7001, 12345)):
+        d = torch.empty(n, dtype=torch.int32, device="cuda:0")
+        P.odb_synth_tokens(d, start, n, seed, I.VOCAB)
+        torch.cuda.synchronize()
+        assert np.array_equal(d.cpu().numpy(), I.token_ids(seed, start, n))
+
+
+# ---- BASELINE.json configs --------------------------------------------------------------------
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("staged", [True, False])
+def test_config1_tiny(P, oracle, rule, staged):
+    wl = I.make_workload(0, rule=rule)
+    plan, info, out = _full_parity(oracle, wl, staged=staged)
+    assert plan.n_rounds == 2 and plan.samples_emitted == 128
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+def test_config2_lowcv_text(P, oracle, rule):
+    _full_parity(oracle, I.make_workload(1, rule=rule))
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+def test_config3_multimodal(P, oracle, rule):
+    _full_parity(oracle, I.make_workload(2, rule=rule))
+
+
+def _sampled_parity(oracle, wl, n_sample=48, seed=0):
+    """Full-size run in the launch configuration bench.py times (odb_run, one collate launch over the
+    whole arena); plan tables compared in full, blocks compared on sampled slots, plus
+    any-size properties recomputed on the device."""
+    plan, _ = oracle.run_workload(wl, collate=False)
+    info, out, _ = Par.run_gpu(wl, staged=False)
+    Par.compare_plan(plan, info, out)
+    rng = np.random.default_rng(seed)
+    n_slots = plan.n_slots
+    area = plan.grp_count.astype(np.int64) * plan.grp_width
+    pick = set(rng.integers(0, n_slots, n_sample).tolist())
+    pick |= {0, n_slots - 1, int(np.argmax(area)), int(np.argmax(plan.grp_width)), int(np.argmax(plan.grp_count))}
+    pick |= set(np.flatnonzero(plan.grp_count == 1)[:4].tolist())          # singletons (splits / over-budget)
+    # keep the host-side token regeneration bounded
+    pick = [s for s in sorted(pick) if area[s] <= 6_000_000][: n_sample + 8]
+    Par.compare_sampled_slots(wl, plan, out, pick)
+    Par.device_self_consistency(info, out, wl.params["ignore_index"])
+    return plan
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("join", [1, 0])
+def test_config4_highcv_longtail(P, oracle, rule, join):
+    wl = I.make_workload(3, rule=rule, join_mode=join)
+    plan = _sampled_parity(oracle, wl)
+    if not join:
+        Q = wl.params["sample_quota"]
+        assert plan.stop_reason == 2 and Q <= plan.samples_emitted <= Q + int(plan.step_samples.max())
+
+
+@pytest.mark.parametrize("cv,budget", [(1.0, 65536), (2.5, 16384), (0.3, 262144)])
+def test_config5_sweep_cells(P, oracle, cv, budget):
+    _sampled_parity(oracle, I.make_workload(4, cv=cv, budget=budget), n_sample=24)
+
+
+def test_config5_maxfit(P, oracle):
+    _sampled_parity(oracle, I.make_workload(4, cv=1.0, budget=65536, rule=1), n_sample=16)
+
+
+# ---- protocol tests (multi-round, overflow, IDLE, empty ranks, quota) --------------------------
+@pytest.mark.parametrize("kind", ["audit:" + k for k in I.AUDIT_KINDS] + ["overflow_multiround", "empty_rank", "unequal"])
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("join", [1, 0])
+def test_protocol(P, oracle, kind, rule, join):
+    over = dict(rule=rule, join_mode=join)
+    wl = I.protocol_workload(kind, 0, **over)
+    if not join:
+        wl.params["sample_quota"] = int(0.6 * wl.n_samples)
+    _full_parity(oracle, wl)
+
+
+def test_protocol_fuzz(P, oracle):
+    for seed in range(150):
+        wl = I.protocol_workload("fuzz", seed)
+        try:
+            _full_parity(oracle, wl, staged=bool(seed & 1))
+        except AssertionError as e:
+            raise AssertionError("fuzz seed %d params %r: %s" % (seed, wl.params, e))
+
+
+def test_many_spans_slow_path(P, oracle):
+    """Samples with more than two masked spans take the kernel's CSR span path."""
+    rng = np.random.default_rng(5)
+    wl = I.protocol_workload("unequal", 3)
+    N = wl.n_samples
+    lo, hi, ptr = [], [], [0]
+    for g in range(N):
+        L = int(wl.lengths[g])
+        k = int(rng.integers(0, 6))
+        cuts = np.sort(rng.choice(np.arange(L + 1), size=min(2 * k, L + 1), replace=False))
+        cuts = cuts[: len(cuts) // 2 * 2]
+        for a, b in zip(cuts[0::2], cuts[1::2]):
+            lo.append(a)
+            hi.append(b)
+        ptr.append(len(lo))
+    wl.span_ptr = np.asarray(ptr, np.int64)
+    wl.span_lo = np.asarray(lo, np.int32)
+    wl.span_hi = np.asarray(hi, np.int32)
+    for shift in (1, 0):
+        wl.params["shift_labels"] = shift
+        _full_parity(oracle, wl)
+
+
+# ---- degenerate cases ------------------------------------------------------
+def test_degenerate_cases(P, oracle):
+    # R = 1: alignment is a no-op
+    wl = I.make_workload(0, n_ranks=1)
+    _full_parity(oracle, wl)
+    # budget below every length: all over-budget singletons
+    wl = I.make_workload(0, budget=4)
+    plan, _, _ = _full_parity(oracle, wl)
+    assert (plan.grp_count[plan.grp_count > 0] == 1).all()
+    # huge budget: THRESHOLD gives the longest sample alone + everything else
+    wl = I.make_workload(0, budget=1 << 30)
+    plan, _, _ = _full_parity(oracle, wl)
+    assert plan.n_steps == 2
+    # all ranks empty
+    wl = I.make_workload(0, n_per_rank=0)
+    plan, info, out = _full_parity(oracle, wl)
+    assert info.n_steps == 0 and info.total_elems == 0 and info.stop_reason == 0
+
+
+def test_bad_length_is_reported(P):
+    import torch
+    wl = I.make_workload(0)
+    wl.lengths = wl.lengths.copy()
+    wl.lengths[17] = 0
+    dw_len = torch.from_numpy(wl.lengths).to("cuda:0")
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        with pytest.raises(P.OdbError) as ei:
+            ctx.plan(dw_len, wl.rank_ptr)
+        assert ei.value.status == P.ODB_ERR_BAD_LENGTH
+
+
+def test_capacity_and_state_errors(P):
+    wl = I.make_workload(0)
+    dw = Par.DeviceWorkload(wl)
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        with pytest.raises(P.OdbError) as ei:
+            P.odb_align(ctx.h)                      # nothing formed yet
+        assert ei.value.status == P.ODB_ERR_STATE
+        info = ctx.plan(dw.lengths, wl.rank_ptr)
+        small = P.OutputBuffers(wl.n_ranks, info.total_elems - 16, info.n_slots, info.samples_emitted, info.n_steps,
+                                info.samples_left, "cuda:0", fill=Par.SENTINEL)
+        with pytest.raises(P.OdbError) as ei:
+            P.odb_collate(ctx.h, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, small.struct)
+        assert ei.value.status == P.ODB_ERR_CAPACITY
+        import torch
+        torch.cuda.synchronize()
+        assert (small.attention_mask.cpu().numpy() == Par.SENTINEL).all()   # nothing written
+
+
+def test_run_to_run_determinism(P):
+    import torch
+    wl = I.make_workload(1)
+    dw = Par.DeviceWorkload(wl)
+    a_info, a, _ = Par.run_gpu(wl, dw, staged=False)
+    b_info, b, _ = Par.run_gpu(wl, dw, staged=False)
+    for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+        assert torch.equal(getattr(a, name), getattr(b, name))
+    for name in ("grp_valid_tokens", "step_valid_tokens", "grp_sample_ids"):
+        assert torch.equal(a.table(name), b.table(name))
+
+
+def test_run_host_end_to_end(P, oracle):
+    """odb_run_host: HOST buffers in, HOST buffers out (the e2e leg bench.py times)."""
+    import torch
+    wl = I.make_workload(1)
+    plan, ref = oracle.run_workload(wl)
+    toks = torch.from_numpy(wl.tokens()).pin_memory()
+    pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        out = P.OutputBuffers(wl.n_ranks, plan.total_elems, plan.n_slots, plan.samples_emitted, plan.n_steps,
+                              plan.samples_left, "cpu", fill=Par.SENTINEL)
+        info = P.odb_run_host(ctx.h, pin(wl.lengths, torch.int32), wl.rank_ptr, toks, pin(wl.sample_ptr, torch.int64),
+                              pin(wl.span_ptr, torch.int64), pin(wl.span_lo, torch.int32), pin(wl.span_hi, torch.int32),
+                              out.struct)
+    Par.compare_plan(plan, info, out)
+    E = plan.total_elems
+    # the host copy is one flat memcpy of each arena, so gap bytes carry whatever the device staging
+    # held; compare blocks only
+    inblk = np.zeros(E, dtype=bool)
+    for s in range(plan.n_slots):
+        o = int(plan.grp_offset[s])
+        inblk[o:o + int(plan.grp_count[s]) * int(plan.grp_width[s])] = True
+    for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+        assert np.array_equal(getattr(out, name)[:E].numpy()[inblk], ref[name][:E][inblk]), name
+    assert np.array_equal(out.table("grp_valid_tokens").numpy(), ref["grp_valid_tokens"])
