@@ -1,0 +1,467 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the ODB hot path (group -> align -> collate) on B200.
+
+One "step" = one pass of the whole hot path (window fill, segmented
+sort, greedy successor, list ranking, cross-rank reduction, split/overflow, step totals, offsets,
+collation with valid-token counts) through ``odb_run`` over one batch of synthetic input that is
+already resident in HBM.  Default workload = BASELINE.json configs[4] (the throughput sweep, the
+largest config, on which north_star states its target), cell CV=1.0 / budget=65536, paper rule
+(THRESHOLD), join mode.  ``--sweep`` adds the nine (CV, budget) cells; ``--config k`` picks another
+BASELINE.json config.
+
+Prints ONE JSON line (rank 0).  Extra objects: ``roofline`` (collate kernel, CUDA events on the
+launching stream inside the timed region), ``e2e`` (odb_run_host with pinned HOST buffers, copies
+inside the timed region), ``cpu_baseline`` (the oracle, as it stands, on a bounded sample on the
+box's host cores), ``clocks`` (nvidia-smi sampled during the timed region).
+
+``--impl reference`` times the CPU oracle instead (rank 0 only), per the tier contract.
+Multi-GPU: the path does not shard across GPUs (north_star: virtual ranks on ONE GPU, no inter-GPU
+collectives) -> "replicas only": N independent replicas, max-over-ranks time, value = N x units / t.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import odb_inputs as I  # noqa: E402
+
+METRIC = "samples/s grouped+aligned+collated (with tokens/s and achieved HBM GB/s vs peak)"
+UNIT = "samples/s"
+RULE_NAMES = {0: "threshold", 1: "maxfit_asc"}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (0-based)")
+    ap.add_argument("--cv", type=float, default=1.0)
+    ap.add_argument("--budget", type=int, default=None)
+    ap.add_argument("--rule", type=int, default=0)
+    ap.add_argument("--join", type=int, default=1)
+    ap.add_argument("--sweep", action="store_true", help="also time the nine config-5 cells (extra key 'sweep')")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sample-ranks", type=int, default=16)
+    ap.add_argument("--ref-sample-ranks", type=int, default=2)
+    return ap.parse_args()
+
+
+def workload_name(args, wl):
+    b = wl.params["budget"]
+    if args.config == 4:
+        return ("configs[4] throughput sweep cell: %d virtual ranks x %d samples, lognormal(mean 2048, CV %g), budget %d"
+                % (wl.n_ranks, wl.n_samples // max(wl.n_ranks, 1), args.cv, b))
+    return "configs[%d] %s: %d virtual ranks, %d samples, budget %d" % (args.config, wl.name, wl.n_ranks,
+                                                                         wl.n_samples, b)
+
+
+def make_wl(args, **over):
+    kw = dict(rule=args.rule, join_mode=args.join, budget=args.budget)
+    if args.config == 4:
+        kw["cv"] = args.cv
+    kw.update(over)
+    return I.make_workload(args.config, **kw)
+
+
+def algorithmic_bytes(real_tokens, padded_elems):
+    """4 B read per real token + 13 B written per padded element (3 x int32 + uint8)."""
+    return 4 * int(real_tokens) + 13 * int(padded_elems)
+
+
+# --------------------------------------------------------------------------------------------
+# clocks sampling (B200_PROFILING.md "clocks DURING the timed region")
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+        time.sleep(0.25)
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+                pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs: torch copy, read+write bytes)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def ncu_traffic(workload_key):
+    """dram bytes per collate launch from the committed ncu --set full summary (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", "collate_traffic.txt")
+    try:
+        with open(p) as f:
+            for line in f:
+                if line.startswith("#") or ":" not in line:
+                    continue
+                k, v = line.split(":", 1)
+                if k.strip() == workload_key:
+                    return float(v.split()[0])
+    except OSError:
+        pass
+    return None
+
+
+# --------------------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline and --impl reference).  The only place bench.py touches oracle/.
+# --------------------------------------------------------------------------------------------
+def oracle_time_once(wl, tokens):
+    """One pass of the oracle (plan + collation of every slot) over `wl`; returns seconds."""
+    from oracle import odb_oracle as O
+    p = wl.params
+    t0 = time.perf_counter()
+    plan = O.OraclePlan(wl.lengths, wl.rank_ptr, **p)
+    plan.collate_all(tokens, wl.sample_ptr[:-1], wl.span_ptr, wl.span_lo, wl.span_hi, pad_id=p["pad_id"],
+                     ignore_index=p["ignore_index"], shift_labels=p["shift_labels"])
+    dt = time.perf_counter() - t0
+    return dt, plan
+
+
+def cpu_baseline(args, n_ranks_sample):
+    from oracle import odb_oracle as O
+    O.build()
+    full = I.bj_config(args.config)
+    R = min(n_ranks_sample, full["R"])
+    wl = make_wl(args, n_ranks=R)
+    tokens = wl.tokens()          # host-side hash, untimed (token generation is excluded on both sides)
+    dt, plan = oracle_time_once(wl, tokens)
+    return {"value": plan.samples_emitted / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "%d of %d virtual ranks of the same recipe (%d samples, %d real tokens), one pass, %.2f s; "
+                      "single thread of %d host cores" % (R, full["R"], plan.samples_emitted, plan.real_tokens, dt,
+                                                          os.cpu_count() or 0),
+            "tokens_per_s": plan.real_tokens / dt, "seconds": dt}, wl
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import odb_oracle as O
+    O.build()
+    full = I.bj_config(args.config)
+    R = min(args.ref_sample_ranks, full["R"])
+    wl = make_wl(args, n_ranks=R)
+    tokens = wl.tokens()
+    for _ in range(args.warmup):
+        oracle_time_once(wl, tokens)
+    tot, plan = 0.0, None
+    for _ in range(args.steps):
+        dt, plan = oracle_time_once(wl, tokens)
+        tot += dt
+    ms = 1e3 * tot / max(args.steps, 1)
+    val = plan.samples_emitted / (ms / 1e3)
+    sample = "each step = %d of %d virtual ranks of the same recipe (%d samples, %d real tokens)" % (
+        R, full["R"], plan.samples_emitted, plan.real_tokens)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": workload_name(args, make_wl_desc(args)), "rule": RULE_NAMES[args.rule],
+                       "join_mode": args.join, "sample": sample},
+            "tokens_per_s": plan.real_tokens / (ms / 1e3),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+class _Desc:
+    pass
+
+
+def make_wl_desc(args):
+    """Cheap stand-in with the full config's shape for workload_name (no arrays drawn)."""
+    c = I.bj_config(args.config)
+    d = _Desc()
+    d.n_ranks, d.n_samples, d.name = c["R"], c["R"] * c["n"], c["name"]
+    d.params = {"budget": args.budget if args.budget is not None else c["budget"]}
+    return d
+
+
+# --------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------
+class DeviceInputs:
+    def __init__(self, wl, device, P):
+        import torch
+        t = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).to(device)
+        self.lengths = t(wl.lengths, torch.int32)
+        self.sample_ptr = t(wl.sample_ptr, torch.int64)
+        self.span_ptr = t(wl.span_ptr, torch.int64)
+        z = torch.zeros(1, dtype=torch.int32, device=device)
+        self.span_lo = t(wl.span_lo, torch.int32) if len(wl.span_lo) else z
+        self.span_hi = t(wl.span_hi, torch.int32) if len(wl.span_hi) else z
+        self.tokens = torch.empty(wl.n_tokens + 16, dtype=torch.int32, device=device)
+        P.odb_synth_tokens(self.tokens, 0, wl.n_tokens, wl.token_seed, I.VOCAB)
+        torch.cuda.synchronize()
+
+
+def gpu_params(P, wl):
+    p = wl.params
+    return P.make_params(wl.n_ranks, p["budget"], rule=p["rule"], join_mode=p["join_mode"],
+                         sample_quota=p["sample_quota"], emitted_so_far=p["emitted_so_far"],
+                         buffer_size=p["buffer_size"], slot_capacity=p["slot_capacity"], pad_id=p["pad_id"],
+                         ignore_index=p["ignore_index"], shift_labels=p["shift_labels"])
+
+
+def time_device(P, ctx, wl, din, out, steps, warmup, barrier):
+    """W warm-up + K timed odb_run passes; CUDA events on the launching (current) stream.
+    Returns (ms_per_step, collate_ms_avg, plan_ms_avg, post_ms_avg, launches_per_step, info)."""
+    import torch
+
+    def one():
+        return P.odb_run(ctx.h, din.lengths, wl.rank_ptr, din.tokens, din.sample_ptr, din.span_ptr, din.span_lo,
+                         din.span_hi, out.struct)
+
+    info = None
+    for _ in range(warmup):
+        info = one()
+    torch.cuda.synchronize()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = P.odb_kernel_launches(ctx.h)
+    stage = np.zeros(3)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(steps):
+        info = one()
+        stage += np.asarray(P.odb_get_timing(ctx.h))     # waits for this step's last event (no extra work)
+    ev1.record()
+    torch.cuda.synchronize()
+    barrier()
+    ms = ev0.elapsed_time(ev1) / max(steps, 1)
+    launches = (P.odb_kernel_launches(ctx.h) - l0) / max(steps, 1)
+    stage /= max(steps, 1)
+    return ms, float(stage[1]), float(stage[0]), float(stage[2]), launches, info
+
+
+def time_e2e(P, ctx, wl, din, info, steps, device):
+    """odb_run_host: pinned HOST inputs -> device -> whole path -> pinned HOST outputs, all inside the
+    timed region (wall clock around the synchronous C call, which ends with a stream synchronize)."""
+    import torch
+    pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
+    h_len = pin(wl.lengths, torch.int32)
+    h_sp = pin(wl.sample_ptr, torch.int64)
+    h_spp = pin(wl.span_ptr, torch.int64)
+    h_lo = pin(wl.span_lo if len(wl.span_lo) else np.zeros(1, np.int32), torch.int32)
+    h_hi = pin(wl.span_hi if len(wl.span_hi) else np.zeros(1, np.int32), torch.int32)
+    h_tok = torch.empty(wl.n_tokens + 16, dtype=torch.int32, pin_memory=True)
+    h_tok.copy_(din.tokens)                      # same ids as the device buffer (untimed set-up)
+    hout = P.OutputBuffers.for_plan(wl.n_ranks, info, "cpu")
+    torch.cuda.synchronize()
+
+    def one():
+        return P.odb_run_host(ctx.h, h_len, wl.rank_ptr, h_tok, h_sp, h_spp, h_lo, h_hi, hout.struct)
+
+    one()                                        # warm-up: sizes the library's device staging
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one()
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    h2d = (h_len.numel() * 4 + h_sp.numel() * 8 + h_spp.numel() * 8 + len(wl.span_lo) * 8 + wl.n_tokens * 4)
+    E = int(info.total_elems)
+    d2h = 13 * E + int(info.n_slots) * (5 * 4 + 8) + (int(info.n_slots) + 1) * 8 + int(info.samples_emitted) * 4 \
+        + int(info.n_steps) * 12 + (wl.n_ranks + 1) * 8 + int(info.samples_left) * 4
+    return dt, int(h2d), int(d2h)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device. The product path has no CPU fallback.")
+    import paper_2606_19989_b200 as P
+    P.load()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    wl = make_wl(args)
+    din = DeviceInputs(wl, device, P)
+    desc = I.describe(wl)
+    result = {}
+    with P.Odb(gpu_params(P, wl), max(wl.n_samples, 1), device=local) as ctx:
+        P.odb_set_timing(ctx.h, True)
+        info = ctx.plan(din.lengths, wl.rank_ptr)
+        out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+        ms, col_ms, plan_ms, post_ms, launches, info = time_device(P, ctx, wl, din, out, args.steps, args.warmup, barrier)
+        clocks = sampler.stop() if rank == 0 else None
+        ms = max_over_ranks(ms)
+        col_ms_max = max_over_ranks(col_ms)
+        n_samples, n_tok = int(info.samples_emitted), int(info.real_tokens)
+        abytes = algorithmic_bytes(info.real_tokens, info.padded_elems)
+        peak, peak_src = measured_peak()
+        achieved = abytes / (col_ms_max * 1e-3) / 1e9
+        wkey = "config%d_cv%g_L%d_rule%d" % (args.config, args.cv, wl.params["budget"], args.rule)
+        result = {
+            "metric": METRIC, "value": world * n_samples / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": workload_name(args, wl), "rule": RULE_NAMES[args.rule], "join_mode": args.join,
+                       "samples": n_samples, "real_tokens": n_tok, "padded_elems": int(info.padded_elems),
+                       "pad_frac": 1.0 - n_tok / max(int(info.padded_elems), 1), "n_steps": int(info.n_steps),
+                       "n_slots": int(info.n_slots), "n_rounds": int(info.n_rounds),
+                       "length_mean": desc["mean"], "length_cv": desc["cv"], "length_max": desc["max"],
+                       "parallelism": "replicas only (virtual ranks live on one GPU; no inter-GPU collective)",
+                       "l2": "no flush: every step reads %.1f GB of tokens and writes %.1f GB of outputs, both far "
+                             "larger than the 126 MB L2" % (4 * n_tok / 1e9, 13 * int(info.padded_elems) / 1e9)},
+            "tokens_per_s": world * n_tok / (ms * 1e-3),
+            "hbm_gbs_whole_step": abytes / (ms * 1e-3) / 1e9,
+            "stage_ms": {"planning": plan_ms, "collate_kernel": col_ms, "post": post_ms},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": ncu_traffic(wkey), "kernel": "k_collate", "algorithmic_bytes": abytes,
+                         "kernel_ms": col_ms_max, "peak_source": peak_src,
+                         "frac_of_nominal_8180": achieved / 8180.0},
+            "gpu_launches": int(round(launches * args.steps)),
+            "clocks": clocks,
+        }
+        if args.sweep and args.config == 4 and world == 1:
+            result["sweep"] = run_sweep(P, args, device, peak)
+        # ---- e2e through the C ABI with HOST buffers (odb_run_host) -------------------------
+        if not args.no_e2e:
+            need = 4 * wl.n_tokens + 13 * int(info.total_elems)
+            try:
+                import psutil
+                avail = psutil.virtual_memory().available
+            except Exception:
+                avail = 0
+            if avail and need * 1.3 * world > avail:
+                result["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                                 "note": "host RAM too small to pin %d bytes per rank" % need}
+            else:
+                del out
+                torch.cuda.empty_cache()
+                barrier()
+                dt, h2d, d2h = time_e2e(P, ctx, wl, din, info, args.e2e_steps, device)
+                dt = max_over_ranks(dt)
+                result["e2e"] = {"value": world * n_samples / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                                 "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": args.e2e_steps,
+                                 "tokens_per_s": world * n_tok / dt, "pcie_gbs": (h2d + d2h) / dt / 1e9,
+                                 "api": "odb_run_host (pinned host buffers in and out)"}
+    del din
+    torch.cuda.empty_cache()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cb, _ = cpu_baseline(args, args.cpu_sample_ranks)
+        result["cpu_baseline"] = cb
+    elif rank == 0:
+        result["cpu_baseline"] = None
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(result), flush=True)
+
+
+def run_sweep(P, args, device, peak):
+    """The nine (CV, budget) cells of configs[4], both rules: samples/s, tokens/s, collate GB/s."""
+    import torch
+    rows = []
+    for cv, L in I.config5_cells():
+        for rule in (0, 1):
+            wl = I.make_workload(4, cv=cv, budget=L, rule=rule)
+            din = DeviceInputs(wl, device, P)
+            with P.Odb(gpu_params(P, wl), wl.n_samples, device=int(device.split(":")[1])) as ctx:
+                P.odb_set_timing(ctx.h, True)
+                info = ctx.plan(din.lengths, wl.rank_ptr)
+                out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
+                ms, col_ms, plan_ms, post_ms, _, info = time_device(P, ctx, wl, din, out, 5, 3, lambda: None)
+                ab = algorithmic_bytes(info.real_tokens, info.padded_elems)
+                rows.append({"cv": cv, "budget": L, "rule": RULE_NAMES[rule], "ms_per_step": ms,
+                             "samples_per_s": int(info.samples_emitted) / (ms * 1e-3),
+                             "tokens_per_s": int(info.real_tokens) / (ms * 1e-3), "collate_ms": col_ms,
+                             "planning_ms": plan_ms, "collate_gbs": ab / (col_ms * 1e-3) / 1e9,
+                             "frac": ab / (col_ms * 1e-3) / 1e9 / peak, "n_steps": int(info.n_steps),
+                             "pad_frac": 1.0 - int(info.real_tokens) / max(int(info.padded_elems), 1)})
+                del out
+            del din
+            torch.cuda.empty_cache()
+    return rows
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
