@@ -97,7 +97,7 @@ static void free_all(odb_ctx *c) {
     c->step_valid.release();
     c->rows.release();
     c->row_sp.release();
-    c->tile_slot.release();
+    c->chunks.release();
     c->hs_lengths.release();
     c->hs_tokens.release();
     c->hs_span_lo.release();
@@ -458,7 +458,7 @@ static int collate_ranks(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_s
     A.grp_sample_ptr = c->grp_sample_ptr.p;
     A.grp_count = c->grp_count.p;
     A.grp_width = c->grp_width.p;
-    A.tile_slot = c->tile_slot.p;
+    A.chunks = c->chunks.p;
     A.ids = o->d_input_ids;
     A.labels = o->d_labels;
     A.pos = o->d_position_ids;
@@ -487,12 +487,12 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
     if (((uintptr_t)o->d_input_ids & 15u) || ((uintptr_t)o->d_labels & 15u) || ((uintptr_t)o->d_position_ids & 15u) ||
         ((uintptr_t)o->d_attention_mask & 15u))
         return ODB_ERR_INVALID_ARG;
-    const int64_t n_tiles = (I.total_elems + kColTile - 1) / kColTile;
     CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
     CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
-    CU(c, c->tile_slot.ensure((size_t)n_tiles + 1));
+    const int64_t n_chunks = (I.total_elems + kColChunk - 1) / kColChunk;
+    CU(c, c->chunks.ensure((size_t)n_chunks + 1));
     CU(c, launch_row_desc(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st));
-    CU(c, launch_tile_slots(c, n_tiles, st));
+    CU(c, launch_chunk_table(c, n_chunks, st));
     if (n_slots) CU(c, cudaMemsetAsync(c->grp_valid.p, 0, n_slots * sizeof(int32_t), st));
     // ev[1]..ev[2] brackets the collate kernel alone; the pre/post work is ev[0]..ev[1] / ev[2]..ev[3]
     if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));

@@ -50,21 +50,64 @@ __global__ void k_row_desc(int R, int n_steps, const int64_t *__restrict__ rank_
     }
 }
 
-// tile t (elements [t*kColTile, (t+1)*kColTile) of the arenas) -> the slot that contains its first
-// element.  One thread per slot fills the tiles that start inside the slot's [offset, next offset).
-__global__ void k_tile_slots(int64_t n_slots, const int64_t *__restrict__ grp_offset, int32_t *__restrict__ tile_slot) {
-    for (int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; s < n_slots; s += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t lo = grp_offset[s], hi = grp_offset[s + 1];
-        for (int64_t t = (lo + kColTile - 1) / kColTile; t * kColTile < hi; ++t) tile_slot[t] = (int32_t)s;
+// Chunk table: chunk c = arena elements [512 c, 512 c + 512).  One thread per chunk finds the slot
+// that holds the chunk's first element (binary search in grp_offset; among equal offsets -- IDLE
+// slots have no elements -- the last one) and stores everything the collate kernel needs to start
+// on the chunk with ONE 32-byte load: the slot's geometry and (row, column) of the first element.
+__global__ void k_chunk_table(int64_t n_chunks, int64_t n_slots, const int64_t *__restrict__ grp_offset,
+                              const int32_t *__restrict__ grp_count, const int32_t *__restrict__ grp_width,
+                              const int64_t *__restrict__ grp_sample_ptr, ChunkRec *__restrict__ chunks) {
+    for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < n_chunks; c += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t a0 = c * kColChunk;
+        int64_t lo = 0, hi = n_slots;  // last s in [0, n_slots) with grp_offset[s] <= a0
+        while (hi - lo > 1) {
+            const int64_t m = (lo + hi) >> 1;
+            if (__ldg(grp_offset + m) <= a0) lo = m;
+            else hi = m;
+        }
+        const int64_t s = lo;
+        ChunkRec r;
+        r.off_s = grp_offset[s];
+        r.slot = (int32_t)s;
+        r.W = (uint32_t)grp_width[s];
+        r.area = (uint32_t)grp_count[s] * r.W;
+        r.sp_s = (uint32_t)grp_sample_ptr[s];
+        const uint64_t e0 = (uint64_t)(a0 - r.off_s);
+        if (r.W > 0 && e0 < r.area) {
+            r.b0 = (uint32_t)(e0 / r.W);
+            r.t0 = (uint32_t)(e0 - (uint64_t)r.b0 * r.W);
+        } else {
+            r.b0 = 0;
+            r.t0 = 0;
+        }
+        chunks[c] = r;
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// collate, version 1: direct global loads, 16-byte streaming stores.
-// A warp covers 128 consecutive arena elements per iteration (lane = 4 elements = one int4 store
-// per int32 arena and one 4-byte store of the uint8 mask); a CTA's 8 warps cover 1024 consecutive
-// elements; a tile is 4 such iterations.  Block offsets are multiples of 16, so a lane's vector never
-// straddles two slots.  Persistent CTAs stride over the tiles.
+// collate
+//
+// The four arenas are treated as flat arrays.  A tile is kColTile = 4096 consecutive arena elements;
+// each of a CTA's 8 warps owns a CHUNK of 512 consecutive elements.  Block offsets are multiples of
+// 16, so 4-element vectors (one int4 per int32 arena) and 16-element groups (one int4 of the uint8
+// mask) never straddle two slots.
+//
+//   interior chunk (all 512 elements inside one slot's [count x width] block; > 95 % of the chunks
+//   of the BASELINE.json configs): lane l owns the vectors k*32 + l, k = 0..3, so every store
+//   instruction of the warp writes 512 contiguous bytes.  Tokens are fetched with 16-byte ALIGNED
+//   loads: a row's tokens start at an arbitrary 4-byte offset, so the lane loads the aligned vector
+//   that holds its first token and takes the following vector from its right-hand neighbour by
+//   shuffle (or loads it when the neighbour is in another row); the 5 tokens t..t+4 it needs (4
+//   ids + the shifted label of the last) are selected by the skew.  Real / masked / valid flags are
+//   4-bit sets built with range arithmetic, not per-element compares.  The mask bytes are transposed
+//   through 512 B of shared memory per warp so that each lane stores ONE int4 covering 16 elements.
+//   Vectors that cross a row end (one per row) are handled by the warp together, one element per
+//   lane, while the aligned loads are in flight.
+//
+//   boundary chunk (slot change, alignment gap, block end, end of arena): the per-vector generic
+//   path (scalar loads, 4-byte mask stores).
+//
+// A11: valid-token counts are integer sums: warp reduce, one atomicAdd per chunk and slot.
 // ---------------------------------------------------------------------------------------------
 struct RowRegs {
     int64_t tok;
@@ -85,15 +128,27 @@ __device__ __forceinline__ RowRegs load_row(const RowDesc *__restrict__ rows, in
     return r;
 }
 
-__device__ __forceinline__ bool masked_at(const RowRegs &r, int c, const CollateArgs &A, int64_t q) {
-    if (r.nspan <= 2) return (c >= r.lo0 && c < r.hi0) || (c >= r.lo1 && c < r.hi1);
-    const int64_t sp = A.row_sp[q];
-    for (int j = 0; j < r.nspan; ++j)
-        if (c >= A.span_lo[sp + j] && c < A.span_hi[sp + j]) return true;
-    return false;
+__device__ __forceinline__ int clamp04(int v) { return min(max(v, 0), 4); }
+
+// bits j in [0, 4) with lo <= c0 + j < hi
+__device__ __forceinline__ uint32_t range_bits(int lo, int hi, int c0) {
+    const uint32_t below_hi = (1u << clamp04(hi - c0)) - 1u;
+    const uint32_t below_lo = (1u << clamp04(lo - c0)) - 1u;
+    return below_hi & ~below_lo;
 }
 
-// one output element (row r, column c); used by the slow path
+// bits j in [0, 4) whose position c0 + j lies in a masked span of the row
+__device__ __forceinline__ uint32_t masked_bits(const RowRegs &r, int c0, const CollateArgs &A, int64_t q) {
+    uint32_t m = range_bits(r.lo0, r.hi0, c0) | range_bits(r.lo1, r.hi1, c0);
+    if (r.nspan > 2) {  // rare: walk the CSR
+        const int64_t sp = A.row_sp[q];
+        for (int j = 2; j < r.nspan; ++j) m |= range_bits(A.span_lo[sp + j], A.span_hi[sp + j], c0);
+    }
+    return m;
+}
+
+// one output element (row r, column c)
+template <bool SHIFT>
 __device__ __forceinline__ void one_element(const CollateArgs &A, const RowRegs &r, int64_t q, int c, int32_t &id,
                                             int32_t &lab, int32_t &pos, uint32_t &m) {
     const int32_t *tp = A.tokens + r.tok;
@@ -101,114 +156,249 @@ __device__ __forceinline__ void one_element(const CollateArgs &A, const RowRegs 
     id = real ? __ldg(tp + c) : A.pad_id;
     pos = real ? c : 0;
     m = real ? 1u : 0u;
-    if (A.shift_labels) {
-        const bool ok = (c + 1 < r.len) && !masked_at(r, c + 1, A, q);
+    if (SHIFT) {
+        const bool ok = (c + 1 < r.len) && !(masked_bits(r, c + 1, A, q) & 1u);
         lab = ok ? __ldg(tp + c + 1) : A.ignore_index;
     } else {
-        const bool ok = real && !masked_at(r, c, A, q);
+        const bool ok = real && !(masked_bits(r, c, A, q) & 1u);
         lab = ok ? id : A.ignore_index;
     }
 }
 
-__global__ void __launch_bounds__(kColThreads, 4) k_collate_v1(const CollateArgs A) {
+// 4 consecutive elements starting at block element e, which may cross row ends (and, when
+// `area` < e + 4, the end of the block): element by element.  Returns the mask bytes; counts valid
+// labels into acc.  Boundary chunks only.
+template <bool SHIFT>
+__device__ __forceinline__ uint32_t straddle_vector(const CollateArgs &A, int64_t a, uint32_t e, uint32_t W, uint32_t area,
+                                                    int64_t sp_s, int &acc) {
+    uint32_t mw = 0;
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        const uint32_t ee = e + j;
+        if (ee >= area) break;
+        const uint32_t bb = ee / W;
+        const int c = (int)(ee - bb * W);
+        const int64_t q = sp_s + bb;
+        const RowRegs r = load_row(A.rows, q);
+        int32_t id, lb, ps;
+        uint32_t m;
+        one_element<SHIFT>(A, r, q, c, id, lb, ps, m);
+        A.ids[a + j] = id;
+        A.labels[a + j] = lb;
+        A.pos[a + j] = ps;
+        mw |= m << (8 * j);
+        acc += (lb != A.ignore_index) ? 1 : 0;
+    }
+    return mw;
+}
+
+// A vector inside one row: ids / labels / position ids / mask word from the 5 tokens
+// x[0..4] = tokens t .. t+4 of the row (anything beyond the sample).
+template <bool SHIFT>
+__device__ __forceinline__ void emit_vector(const CollateArgs &A, const RowRegs &r, int64_t q, int t, const int32_t (&x)[5],
+                                            int64_t a, uint32_t &mword, int &acc) {
+    const int nreal = clamp04(r.len - t);  // elements t .. t+3 that are real tokens
+    uint32_t ok;                            // elements whose label carries a loss term
+    if (SHIFT) ok = ((1u << clamp04(r.len - 1 - t)) - 1u) & ~masked_bits(r, t + 1, A, q);
+    else ok = ((1u << nreal) - 1u) & ~masked_bits(r, t, A, q);
+    acc += __popc(ok);
+    const int4 oid = make_int4(nreal > 0 ? x[0] : A.pad_id, nreal > 1 ? x[1] : A.pad_id, nreal > 2 ? x[2] : A.pad_id,
+                               nreal > 3 ? x[3] : A.pad_id);
+    const int4 opos = make_int4(nreal > 0 ? t : 0, nreal > 1 ? t + 1 : 0, nreal > 2 ? t + 2 : 0, nreal > 3 ? t + 3 : 0);
+    const int4 olab = make_int4((ok & 1u) ? x[SHIFT ? 1 : 0] : A.ignore_index, (ok & 2u) ? x[SHIFT ? 2 : 1] : A.ignore_index,
+                                (ok & 4u) ? x[SHIFT ? 3 : 2] : A.ignore_index, (ok & 8u) ? x[SHIFT ? 4 : 3] : A.ignore_index);
+    __stcs(reinterpret_cast<int4 *>(A.ids + a), oid);
+    __stcs(reinterpret_cast<int4 *>(A.labels + a), olab);
+    __stcs(reinterpret_cast<int4 *>(A.pos + a), opos);
+    mword = (((1u << nreal) - 1u) * 0x00204081u) & 0x01010101u;  // bit j -> byte j
+}
+
+template <bool SHIFT>
+__global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A) {
+    __shared__ __align__(16) uint32_t s_mask[kColThreads / 32][128];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     constexpr int kWarps = kColThreads / 32;
-    constexpr int kIters = kColTile / (kWarps * 128);
+    static_assert(kColChunk == 512 && kColTile == kWarps * kColChunk, "a chunk is 4 vectors per lane");
+    uint32_t *sm = s_mask[warp];
+    const int4 *tok4 = reinterpret_cast<const int4 *>(A.tokens);
     for (int64_t tile = A.tile_lo + blockIdx.x; tile < A.tile_hi; tile += gridDim.x) {
-        int64_t s = A.tile_slot[tile];
-        int64_t off_s = A.grp_offset[s], off_n = A.grp_offset[s + 1];
-        int64_t s_loaded = -1;
-        uint32_t W = 0, area = 0;
-        int64_t sp_s = 0;
+        const int64_t chunk = tile * kWarps + warp;
+        const int64_t a0 = chunk * kColChunk;
+        if (a0 >= A.total_elems) continue;
+        const int4 *cp = reinterpret_cast<const int4 *>(A.chunks + chunk);
+        const int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
+        int64_t off_s = (int64_t)(((uint64_t)(uint32_t)c0.y << 32) | (uint32_t)c0.x);
+        int64_t s = c0.z;
+        uint32_t W = (uint32_t)c0.w, area = (uint32_t)c1.x;
+        int64_t sp_s = (int64_t)(uint32_t)c1.y;
+        const int64_t e0 = a0 - off_s;
         int acc = 0;
-        int64_t acc_slot = -1;
-#pragma unroll 1
-        for (int it = 0; it < kIters; ++it) {
-            const int64_t a = tile * kColTile + (int64_t)(it * kWarps + warp) * 128 + lane * 4;
-            if (a >= A.total_elems) break;
-            while (a >= off_n) {
-                ++s;
-                off_s = off_n;
-                off_n = A.grp_offset[s + 1];
-            }
-            if (s != s_loaded) {
-                W = (uint32_t)A.grp_width[s];
-                area = (uint32_t)A.grp_count[s] * W;
-                sp_s = A.grp_sample_ptr[s];
-                s_loaded = s;
-            }
-            const uint32_t e = (uint32_t)(a - off_s);
-            if (e >= area) continue;  // alignment gap: never written
-            if (s != acc_slot) {
-                if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
-                acc = 0;
-                acc_slot = s;
-            }
-            const uint32_t b = e / W;
-            const uint32_t t = e - b * W;
-            if (t + 4 <= W) {
-                // fast path: the vector lies inside one row (and therefore inside the block)
-                const int64_t q = sp_s + b;
-                const RowRegs r = load_row(A.rows, q);
-                const int32_t *tp = A.tokens + r.tok + t;
-                const int nreal = max(0, min(5, r.len - (int)t));  // tokens t .. t+4 that exist
-                int32_t v[5];
+        if (e0 + kColChunk <= (int64_t)area) {
+            // ---------------- interior chunk ----------------
+            const uint32_t b0 = (uint32_t)c1.z, t0 = (uint32_t)c1.w;
+            const bool wide = W >= (uint32_t)kColChunk;            // then t0 + x < 2 W: quotient 0 or 1
+            const uint32_t M = (W >= 2u && !wide) ? 0xFFFFFFFFu / W + 1u : 0u;  // ceil(2^32 / W); exact for n < 1024
+            uint32_t q[4];
+            int t[4];
+            bool fast[4];
 #pragma unroll
-                for (int j = 0; j < 5; ++j) v[j] = (j < nreal) ? __ldg(tp + j) : A.pad_id;
-                int4 oid, olab, opos;
-                uint32_t om = 0;
-                int32_t lab[4];
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t n = t0 + (uint32_t)(k * 32 + lane) * 4u;  // column if the row never ended
+                const uint32_t d = wide ? (n >= W ? 1u : 0u) : (W >= 2u ? __umulhi(n, M) : n);
+                t[k] = (int)(n - d * W);
+                q[k] = (uint32_t)sp_s + b0 + d;  // samples_emitted < 2^31
+                fast[k] = (uint32_t)t[k] + 4u <= W;
+            }
+            RowRegs r[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int c = (int)t + j;
-                    const bool real = c < r.len;
-                    if (real) om |= 1u << (8 * j);
-                    if (A.shift_labels) {
-                        const bool ok = (c + 1 < r.len) && !masked_at(r, c + 1, A, q);
-                        lab[j] = ok ? v[j + 1] : A.ignore_index;
-                    } else {
-                        const bool ok = real && !masked_at(r, c, A, q);
-                        lab[j] = ok ? v[j] : A.ignore_index;
+            for (int k = 0; k < 4; ++k) r[k] = load_row(A.rows, (int64_t)q[k]);
+            int4 v0[4];
+            bool ld[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                ld[k] = fast[k] && t[k] < r[k].len;
+                v0[k] = ld[k] ? __ldg(tok4 + ((r[k].tok + t[k]) >> 2)) : make_int4(0, 0, 0, 0);
+            }
+            uint32_t mword[4];
+            // vectors that cross a row end (one per row of the block: rare, but a dependent chain of
+            // row-descriptor and token loads): the warp handles them together, one element per lane,
+            // while the aligned loads above are in flight
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                mword[k] = 0;
+                uint32_t sb = __ballot_sync(ODB_FULL_MASK, !fast[k]);
+                while (sb) {  // warp-uniform; up to 8 straddling vectors per pass, 4 lanes each
+                    uint32_t rest = sb;
+                    int src = -1;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int l = rest ? __ffs(rest) - 1 : -1;
+                        if (l >= 0) rest &= rest - 1;
+                        if ((lane >> 2) == j) src = l;
                     }
-                    acc += (lab[j] != A.ignore_index) ? 1 : 0;
-                }
-                oid = make_int4(v[0], v[1], v[2], v[3]);  // v[j] is pad_id beyond the sample
-                opos = make_int4((int)t < r.len ? (int)t : 0, (int)t + 1 < r.len ? (int)t + 1 : 0,
-                                 (int)t + 2 < r.len ? (int)t + 2 : 0, (int)t + 3 < r.len ? (int)t + 3 : 0);
-                olab = make_int4(lab[0], lab[1], lab[2], lab[3]);
-                __stcs(reinterpret_cast<int4 *>(A.ids + a), oid);
-                __stcs(reinterpret_cast<int4 *>(A.labels + a), olab);
-                __stcs(reinterpret_cast<int4 *>(A.pos + a), opos);
-                __stcs(reinterpret_cast<unsigned int *>(A.mask + a), om);
-            } else {
-                // slow path: the vector crosses a row end and / or the end of the block
-#pragma unroll 1
-                for (int j = 0; j < 4; ++j) {
-                    const uint32_t ee = e + j;
-                    if (ee >= area) break;
-                    const uint32_t bb = ee / W;
-                    const int c = (int)(ee - bb * W);
-                    const int64_t q = sp_s + bb;
-                    const RowRegs r = load_row(A.rows, q);
-                    int32_t id, lb, ps;
-                    uint32_t m;
-                    one_element(A, r, q, c, id, lb, ps, m);
-                    A.ids[a + j] = id;
-                    A.labels[a + j] = lb;
-                    A.pos[a + j] = ps;
-                    A.mask[a + j] = (uint8_t)m;
-                    acc += (lb != A.ignore_index) ? 1 : 0;
+                    uint32_t m = 0;
+                    if (src >= 0) {
+                        const int j = lane & 3;
+                        const uint32_t ee = (uint32_t)e0 + (uint32_t)(k * 32 + src) * 4u + (uint32_t)j;
+                        const uint32_t bb = ee / W;
+                        const int c = (int)(ee - bb * W);
+                        const int64_t qq = sp_s + bb;
+                        const RowRegs rr = load_row(A.rows, qq);
+                        int32_t id, lb, ps;
+                        one_element<SHIFT>(A, rr, qq, c, id, lb, ps, m);
+                        const int64_t aa = a0 + (int64_t)(k * 32 + src) * 4 + j;
+                        A.ids[aa] = id;
+                        A.labels[aa] = lb;
+                        A.pos[aa] = ps;
+                        acc += (lb != A.ignore_index) ? 1 : 0;
+                        m <<= 8 * j;
+                    }
+                    // combine the 4 mask bytes of each quad and hand the word to the owning lane
+                    m |= __shfl_xor_sync(ODB_FULL_MASK, m, 1);
+                    m |= __shfl_xor_sync(ODB_FULL_MASK, m, 2);
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const int owner = __shfl_sync(ODB_FULL_MASK, src, 4 * j);
+                        const uint32_t w = __shfl_sync(ODB_FULL_MASK, m, 4 * j);
+                        if (owner == lane) mword[k] = w;
+                    }
+                    sb = rest;
                 }
             }
-        }
-        // A11: one integer atomic per warp per tile when the whole warp stayed in one slot
-        const int64_t slot0 = __shfl_sync(ODB_FULL_MASK, acc_slot, 0);
-        const bool same = __all_sync(ODB_FULL_MASK, acc_slot == slot0);
-        if (same) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                // the following aligned vector: from the right-hand neighbour when it loaded it
+                int4 n;
+                n.x = __shfl_down_sync(ODB_FULL_MASK, v0[k].x, 1);
+                n.y = __shfl_down_sync(ODB_FULL_MASK, v0[k].y, 1);
+                n.z = __shfl_down_sync(ODB_FULL_MASK, v0[k].z, 1);
+                n.w = __shfl_down_sync(ODB_FULL_MASK, v0[k].w, 1);
+                // neighbour in the same row and loaded <=> its vector is the one after ours
+                const uint32_t tag = ld[k] ? q[k] : 0xFFFFFFFFu;
+                const uint32_t ntag = __shfl_down_sync(ODB_FULL_MASK, tag, 1);
+                if (fast[k]) {
+                    const int64_t g = r[k].tok + t[k];
+                    const bool from_nb = lane < 31 && ntag == q[k];
+                    if (!from_nb) {
+                        const int64_t qn = (g >> 2) + 1;
+                        const bool need = ld[k] && (qn << 2) < r[k].tok + r[k].len;
+                        n = need ? __ldg(tok4 + qn) : make_int4(0, 0, 0, 0);
+                    }
+                    // x[j] = word (skew + j) of the 8-word window v0 | n
+                    int32_t w[8] = {v0[k].x, v0[k].y, v0[k].z, v0[k].w, n.x, n.y, n.z, n.w};
+                    const int sk = (int)g & 3;
+                    if (sk & 1) {
+#pragma unroll
+                        for (int j = 0; j < 7; ++j) w[j] = w[j + 1];
+                    }
+                    if (sk & 2) {
+#pragma unroll
+                        for (int j = 0; j < 5; ++j) w[j] = w[j + 2];
+                    }
+                    const int32_t x[5] = {w[0], w[1], w[2], w[3], w[4]};
+                    emit_vector<SHIFT>(A, r[k], (int64_t)q[k], t[k], x, a0 + (int64_t)(k * 32 + lane) * 4, mword[k], acc);
+                }
+            }
+            // mask: lane l holds the words of vectors k*32 + l; lane l stores vectors 4l .. 4l+3
+#pragma unroll
+            for (int k = 0; k < 4; ++k) sm[k * 32 + lane] = mword[k];
+            __syncwarp();
+            const int4 mv = *reinterpret_cast<const int4 *>(sm + 4 * lane);
+            __syncwarp();
+            __stcs(reinterpret_cast<int4 *>(A.mask + a0) + lane, mv);
             const int tot = __reduce_add_sync(ODB_FULL_MASK, acc);
-            if (lane == 0 && tot != 0) atomicAdd(&A.grp_valid[slot0], tot);
-        } else if (acc) {
-            atomicAdd(&A.grp_valid[acc_slot], acc);
+            if (lane == 0 && tot != 0) atomicAdd(&A.grp_valid[s], tot);
+        } else {
+            // ---------------- boundary chunk: generic per-vector path ----------------
+            int64_t off_n = A.grp_offset[s + 1];
+            int64_t acc_slot = -1;
+#pragma unroll 1
+            for (int k = 0; k < 4; ++k) {
+                const int64_t a = a0 + (int64_t)(k * 32 + lane) * 4;
+                if (a >= A.total_elems) break;
+                bool moved = false;
+                while (a >= off_n) {
+                    ++s;
+                    off_s = off_n;
+                    off_n = A.grp_offset[s + 1];
+                    moved = true;
+                }
+                if (moved) {
+                    W = (uint32_t)A.grp_width[s];
+                    area = (uint32_t)A.grp_count[s] * W;
+                    sp_s = A.grp_sample_ptr[s];
+                }
+                const uint32_t e = (uint32_t)(a - off_s);
+                if (e >= area) continue;  // alignment gap: never written
+                if (s != acc_slot) {
+                    if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
+                    acc = 0;
+                    acc_slot = s;
+                }
+                const uint32_t b = e / W;
+                const uint32_t t = e - b * W;
+                uint32_t mw;
+                int nvalid = 4;
+                if (t + 4 <= W) {
+                    const int64_t q = sp_s + b;
+                    const RowRegs r = load_row(A.rows, q);
+                    const int32_t *tp = A.tokens + r.tok + t;
+                    const int nreal = max(0, min(5, r.len - (int)t));
+                    int32_t x[5];
+#pragma unroll
+                    for (int j = 0; j < 5; ++j) x[j] = (j < nreal) ? __ldg(tp + j) : A.pad_id;
+                    emit_vector<SHIFT>(A, r, q, (int)t, x, a, mw, acc);
+                } else {
+                    mw = straddle_vector<SHIFT>(A, a, e, W, area, sp_s, acc);
+                    nvalid = (int)min(4u, area - e);
+                }
+                if (nvalid == 4) {
+                    __stcs(reinterpret_cast<unsigned int *>(A.mask + a), mw);
+                } else {
+                    for (int j = 0; j < nvalid; ++j) A.mask[a + j] = (uint8_t)(mw >> (8 * j));
+                }
+            }
+            if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
         }
     }
 }
@@ -238,11 +428,12 @@ cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64
     return cudaSuccess;
 }
 
-cudaError_t launch_tile_slots(odb_ctx *c, int64_t n_tiles, cudaStream_t st) {
+cudaError_t launch_chunk_table(odb_ctx *c, int64_t n_chunks, cudaStream_t st) {
     const int64_t n_slots = (int64_t)c->prm.n_ranks * c->n_steps;
-    if (n_slots == 0 || n_tiles == 0) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>((n_slots + 255) / 256, (int64_t)c->sm_count * 8);
-    k_tile_slots<<<blocks, 256, 0, st>>>(n_slots, c->grp_offset.p, c->tile_slot.p);
+    if (n_slots == 0 || n_chunks == 0) return cudaSuccess;
+    int blocks = (int)std::min<int64_t>((n_chunks + 255) / 256, (int64_t)c->sm_count * 16);
+    k_chunk_table<<<blocks, 256, 0, st>>>(n_chunks, n_slots, c->grp_offset.p, c->grp_count.p, c->grp_width.p,
+                                          c->grp_sample_ptr.p, c->chunks.p);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
@@ -250,14 +441,17 @@ cudaError_t launch_tile_slots(odb_ctx *c, int64_t n_tiles, cudaStream_t st) {
 cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st) {
     const int64_t n_tiles = args.tile_hi - args.tile_lo;
     if (n_tiles <= 0) return cudaSuccess;
-    static int occ = 0;
-    if (occ == 0) {
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_collate_v1, kColThreads, 0);
+    static int occ[2] = {0, 0};
+    const int sh = args.shift_labels ? 1 : 0;
+    if (occ[sh] == 0) {
+        cudaError_t e = sh ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[sh], k_collate<true>, kColThreads, 0)
+                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[sh], k_collate<false>, kColThreads, 0);
         if (e != cudaSuccess) return e;
-        if (occ < 1) occ = 1;
+        if (occ[sh] < 1) occ[sh] = 1;
     }
-    int blocks = (int)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * occ);
-    k_collate_v1<<<blocks, kColThreads, 0, st>>>(args);
+    int blocks = (int)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * occ[sh]);
+    if (sh) k_collate<true><<<blocks, kColThreads, 0, st>>>(args);
+    else k_collate<false><<<blocks, kColThreads, 0, st>>>(args);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

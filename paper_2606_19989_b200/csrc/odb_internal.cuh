@@ -21,7 +21,8 @@ constexpr int kSortThreads = 512;
 constexpr int kMergeThreads = 256;
 constexpr int kRankThreads = 1024;  // one CTA per rank for A2..A8
 constexpr int kColThreads = 256;    // collate CTA (A10)
-constexpr int kColTile = 4096;      // padded elements per collate tile (multiple of 8 warps * 128)
+constexpr int kColTile = 4096;      // arena elements per collate tile (one CTA iteration)
+constexpr int kColChunk = 512;      // arena elements per warp per tile (4 vectors per lane)
 
 // Per-round status record: written by the round's kernels, copied to pinned host memory (A7).
 struct RoundRec {
@@ -51,6 +52,17 @@ struct __align__(16) RowDesc {
     int32_t lo0, hi0, lo1, hi1;
 };
 
+// Where a 512-element chunk of the arenas starts: its slot's geometry and the (row, column) of the
+// chunk's first element.  32 bytes, two 16-byte loads.
+struct __align__(16) ChunkRec {
+    int64_t off_s;   // grp_offset of the slot
+    int32_t slot;
+    uint32_t W;      // grp_width
+    uint32_t area;   // count * width
+    uint32_t sp_s;   // grp_sample_ptr of the slot (index of its first row)
+    uint32_t b0, t0; // row / column of the chunk's first element (when it lies inside the block)
+};
+
 struct CollateArgs {
     const int32_t *tokens;
     const RowDesc *rows;
@@ -61,7 +73,7 @@ struct CollateArgs {
     const int64_t *grp_sample_ptr;  // n_slots + 1
     const int32_t *grp_count;
     const int32_t *grp_width;
-    const int32_t *tile_slot;  // first slot overlapping each tile
+    const ChunkRec *chunks;
     int32_t *ids;
     int32_t *labels;
     int32_t *pos;
@@ -167,7 +179,7 @@ struct odb_ctx {
     odb::DevBuf<int64_t> left_ptr, step_valid;
     odb::DevBuf<odb::RowDesc> rows;
     odb::DevBuf<int64_t> row_sp;
-    odb::DevBuf<int32_t> tile_slot;
+    odb::DevBuf<odb::ChunkRec> chunks;
 
     // device staging for odb_run_host
     odb::DevBuf<int32_t> hs_lengths, hs_tokens, hs_span_lo, hs_span_hi, hs_ids, hs_labels, hs_pos;
@@ -186,7 +198,7 @@ cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st);     // A9 + tables + l
 // ---- launchers implemented in odb_collate.cu -------------------------------------------------
 cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
                             const int32_t *d_span_lo, const int32_t *d_span_hi, cudaStream_t st);
-cudaError_t launch_tile_slots(odb_ctx *c, int64_t n_tiles, cudaStream_t st);
+cudaError_t launch_chunk_table(odb_ctx *c, int64_t n_chunks, cudaStream_t st);
 cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st);
 cudaError_t launch_step_valid(odb_ctx *c, int64_t *d_step_valid, cudaStream_t st);
 }  // namespace odb
