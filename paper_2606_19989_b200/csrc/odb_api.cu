@@ -76,6 +76,7 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->S);
     cudaFree(c->d_rec);
     cudaFree(c->d_tot);
+    cudaFree(c->d_tile_counter);
     if (c->h_rec) cudaFreeHost(c->h_rec);
     if (c->h_tot) cudaFreeHost(c->h_tot);
     c->st_count.release();
@@ -179,6 +180,7 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->S, R);
     if (e == cudaSuccess) e = dev_alloc(&c->d_rec, 1);
     if (e == cudaSuccess) e = dev_alloc(&c->d_tot, 1);
+    if (e == cudaSuccess) e = dev_alloc(&c->d_tile_counter, 1);
     if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_rec, sizeof(RoundRec));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_tot, sizeof(PlanTotals));
     for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
@@ -464,6 +466,7 @@ static int collate_ranks(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_s
     A.pos = o->d_position_ids;
     A.mask = o->d_attention_mask;
     A.grp_valid = c->grp_valid.p;
+    A.tile_counter = c->d_tile_counter;
     A.total_elems = h_rank_off[r_hi];
     // tiles are arena-aligned; a rank boundary inside a tile is handled by processing the boundary
     // tile in the launch that owns its first element (offsets are multiples of 16, tiles of 4096)

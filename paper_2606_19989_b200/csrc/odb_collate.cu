@@ -89,24 +89,25 @@ __global__ void k_chunk_table(int64_t n_chunks, int64_t n_slots, const int64_t *
 //
 // The four arenas are treated as flat arrays.  A tile is kColTile = 4096 consecutive arena elements;
 // each of a CTA's 8 warps owns a CHUNK of 512 consecutive elements.  Block offsets are multiples of
-// 16, so 4-element vectors (one int4 per int32 arena) and 16-element groups (one int4 of the uint8
-// mask) never straddle two slots.
+// 16, so a UNIT of 16 consecutive, 16-aligned elements never straddles two slots.
 //
 //   interior chunk (all 512 elements inside one slot's [count x width] block; > 95 % of the chunks
-//   of the BASELINE.json configs): lane l owns the vectors k*32 + l, k = 0..3, so every store
-//   instruction of the warp writes 512 contiguous bytes.  Tokens are fetched with 16-byte ALIGNED
-//   loads: a row's tokens start at an arbitrary 4-byte offset, so the lane loads the aligned vector
-//   that holds its first token and takes the following vector from its right-hand neighbour by
-//   shuffle (or loads it when the neighbour is in another row); the 5 tokens t..t+4 it needs (4
-//   ids + the shifted label of the last) are selected by the skew.  Real / masked / valid flags are
-//   4-bit sets built with range arithmetic, not per-element compares.  The mask bytes are transposed
-//   through 512 B of shared memory per warp so that each lane stores ONE int4 covering 16 elements.
-//   Vectors that cross a row end (one per row) are handled by the warp together, one element per
+//   of the BASELINE.json configs): lane l owns unit l = elements [16 l, 16 l + 16) of the chunk and
+//   writes them with two 256-bit stores per int32 arena (STG.256: each lane fills whole 32-byte
+//   sectors) and one 16-byte store of the uint8 mask.  Tokens are fetched with four 16-byte ALIGNED
+//   loads: a row's tokens start at an arbitrary 4-byte offset, so the lane loads the aligned vectors
+//   that cover its first 16 tokens and takes the following vector (it holds the shifted label of the
+//   last element) from its right-hand neighbour by shuffle, or loads it when the neighbour is in
+//   another row; the 17 tokens t..t+16 are then picked by the skew (0..3 words).  Real / masked /
+//   valid flags are 16-bit sets built with range arithmetic, not per-element compares, and units
+//   that are all real / all valid / all ignored skip the per-element selects.
+//   Units that cross a row end (one per row) are handled by the warp together, one element per
 //   lane, while the aligned loads are in flight.
 //
 //   boundary chunk (slot change, alignment gap, block end, end of arena): the per-vector generic
-//   path (scalar loads, 4-byte mask stores).
+//   path (4-element vectors, scalar loads, 4-byte mask stores).
 //
+// Work distribution: persistent CTAs take runs of kColGrab tiles from an atomic counter.
 // A11: valid-token counts are integer sums: warp reduce, one atomicAdd per chunk and slot.
 // ---------------------------------------------------------------------------------------------
 struct RowRegs {
@@ -128,24 +129,38 @@ __device__ __forceinline__ RowRegs load_row(const RowDesc *__restrict__ rows, in
     return r;
 }
 
-__device__ __forceinline__ int clamp04(int v) { return min(max(v, 0), 4); }
+__device__ __forceinline__ void st256(int32_t *p, const int32_t (&v)[16], int o) {
+    asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(v[o]), "r"(v[o + 1]), "r"(v[o + 2]),
+                 "r"(v[o + 3]), "r"(v[o + 4]), "r"(v[o + 5]), "r"(v[o + 6]), "r"(v[o + 7])
+                 : "memory");
+}
 
-// bits j in [0, 4) with lo <= c0 + j < hi
+template <int N>
+__device__ __forceinline__ int clamp0(int v) {
+    return min(max(v, 0), N);
+}
+
+// bits j in [0, N) with lo <= c0 + j < hi
+template <int N>
 __device__ __forceinline__ uint32_t range_bits(int lo, int hi, int c0) {
-    const uint32_t below_hi = (1u << clamp04(hi - c0)) - 1u;
-    const uint32_t below_lo = (1u << clamp04(lo - c0)) - 1u;
+    const uint32_t below_hi = (1u << clamp0<N>(hi - c0)) - 1u;
+    const uint32_t below_lo = (1u << clamp0<N>(lo - c0)) - 1u;
     return below_hi & ~below_lo;
 }
 
-// bits j in [0, 4) whose position c0 + j lies in a masked span of the row
+// bits j in [0, N) whose position c0 + j lies in a masked span of the row
+template <int N>
 __device__ __forceinline__ uint32_t masked_bits(const RowRegs &r, int c0, const CollateArgs &A, int64_t q) {
-    uint32_t m = range_bits(r.lo0, r.hi0, c0) | range_bits(r.lo1, r.hi1, c0);
+    uint32_t m = range_bits<N>(r.lo0, r.hi0, c0) | range_bits<N>(r.lo1, r.hi1, c0);
     if (r.nspan > 2) {  // rare: walk the CSR
         const int64_t sp = A.row_sp[q];
-        for (int j = 2; j < r.nspan; ++j) m |= range_bits(A.span_lo[sp + j], A.span_hi[sp + j], c0);
+        for (int j = 2; j < r.nspan; ++j) m |= range_bits<N>(A.span_lo[sp + j], A.span_hi[sp + j], c0);
     }
     return m;
 }
+
+// bit j -> byte j (4 bits -> 4 bytes of 0 / 1)
+__device__ __forceinline__ uint32_t spread4(uint32_t bits) { return ((bits & 15u) * 0x00204081u) & 0x01010101u; }
 
 // one output element (row r, column c)
 template <bool SHIFT>
@@ -157,17 +172,16 @@ __device__ __forceinline__ void one_element(const CollateArgs &A, const RowRegs 
     pos = real ? c : 0;
     m = real ? 1u : 0u;
     if (SHIFT) {
-        const bool ok = (c + 1 < r.len) && !(masked_bits(r, c + 1, A, q) & 1u);
+        const bool ok = (c + 1 < r.len) && !(masked_bits<1>(r, c + 1, A, q) & 1u);
         lab = ok ? __ldg(tp + c + 1) : A.ignore_index;
     } else {
-        const bool ok = real && !(masked_bits(r, c, A, q) & 1u);
+        const bool ok = real && !(masked_bits<1>(r, c, A, q) & 1u);
         lab = ok ? id : A.ignore_index;
     }
 }
 
-// 4 consecutive elements starting at block element e, which may cross row ends (and, when
-// `area` < e + 4, the end of the block): element by element.  Returns the mask bytes; counts valid
-// labels into acc.  Boundary chunks only.
+// Boundary chunks: 4 consecutive elements starting at block element e, which may cross row ends
+// (and, when `area` < e + 4, the end of the block): element by element.  Returns the mask bytes.
 template <bool SHIFT>
 __device__ __forceinline__ uint32_t straddle_vector(const CollateArgs &A, int64_t a, uint32_t e, uint32_t W, uint32_t area,
                                                     int64_t sp_s, int &acc) {
@@ -192,15 +206,14 @@ __device__ __forceinline__ uint32_t straddle_vector(const CollateArgs &A, int64_
     return mw;
 }
 
-// A vector inside one row: ids / labels / position ids / mask word from the 5 tokens
-// x[0..4] = tokens t .. t+4 of the row (anything beyond the sample).
+// Boundary chunks: a 4-element vector inside one row from the 5 tokens x[0..4] = tokens t .. t+4.
 template <bool SHIFT>
 __device__ __forceinline__ void emit_vector(const CollateArgs &A, const RowRegs &r, int64_t q, int t, const int32_t (&x)[5],
                                             int64_t a, uint32_t &mword, int &acc) {
-    const int nreal = clamp04(r.len - t);  // elements t .. t+3 that are real tokens
-    uint32_t ok;                            // elements whose label carries a loss term
-    if (SHIFT) ok = ((1u << clamp04(r.len - 1 - t)) - 1u) & ~masked_bits(r, t + 1, A, q);
-    else ok = ((1u << nreal) - 1u) & ~masked_bits(r, t, A, q);
+    const int nreal = clamp0<4>(r.len - t);  // elements t .. t+3 that are real tokens
+    uint32_t ok;                              // elements whose label carries a loss term
+    if (SHIFT) ok = ((1u << clamp0<4>(r.len - 1 - t)) - 1u) & ~masked_bits<4>(r, t + 1, A, q);
+    else ok = ((1u << nreal) - 1u) & ~masked_bits<4>(r, t, A, q);
     acc += __popc(ok);
     const int4 oid = make_int4(nreal > 0 ? x[0] : A.pad_id, nreal > 1 ? x[1] : A.pad_id, nreal > 2 ? x[2] : A.pad_id,
                                nreal > 3 ? x[3] : A.pad_id);
@@ -210,195 +223,227 @@ __device__ __forceinline__ void emit_vector(const CollateArgs &A, const RowRegs 
     __stcs(reinterpret_cast<int4 *>(A.ids + a), oid);
     __stcs(reinterpret_cast<int4 *>(A.labels + a), olab);
     __stcs(reinterpret_cast<int4 *>(A.pos + a), opos);
-    mword = (((1u << nreal) - 1u) * 0x00204081u) & 0x01010101u;  // bit j -> byte j
+    mword = spread4((1u << nreal) - 1u);
+}
+
+// Interior chunks: a 16-element unit inside one row from the 17 tokens x[0..16] = tokens t .. t+16
+// (anything beyond the sample).  Returns the 16 mask bytes.
+template <bool SHIFT>
+__device__ __forceinline__ int4 emit_unit(const CollateArgs &A, const RowRegs &r, int64_t q, int t, const int32_t (&x)[17],
+                                          int64_t a, int &acc) {
+    const int nreal = clamp0<16>(r.len - t);  // elements t .. t+15 that are real tokens
+    const uint32_t real = (1u << nreal) - 1u;
+    uint32_t ok;  // elements whose label carries a loss term
+    if (SHIFT) ok = ((1u << clamp0<16>(r.len - 1 - t)) - 1u) & ~masked_bits<16>(r, t + 1, A, q);
+    else ok = real & ~masked_bits<16>(r, t, A, q);
+    acc += __popc(ok);
+    int32_t o[16];
+    // input_ids
+    if (nreal == 16) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) o[j] = x[j];
+    } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) o[j] = j < nreal ? x[j] : A.pad_id;
+    }
+    st256(A.ids + a, o, 0);
+    st256(A.ids + a + 8, o, 8);
+    // position_ids
+#pragma unroll
+    for (int j = 0; j < 16; ++j) o[j] = j < nreal ? t + j : 0;
+    st256(A.pos + a, o, 0);
+    st256(A.pos + a + 8, o, 8);
+    // labels
+    if (ok == 0xFFFFu) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) o[j] = x[j + (SHIFT ? 1 : 0)];
+    } else if (ok == 0u) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) o[j] = A.ignore_index;
+    } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) o[j] = ((ok >> j) & 1u) ? x[j + (SHIFT ? 1 : 0)] : A.ignore_index;
+    }
+    st256(A.labels + a, o, 0);
+    st256(A.labels + a + 8, o, 8);
+    return make_int4((int)spread4(real), (int)spread4(real >> 4), (int)spread4(real >> 8), (int)spread4(real >> 12));
 }
 
 template <bool SHIFT>
 __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A) {
-    __shared__ __align__(16) uint32_t s_mask[kColThreads / 32][128];
+    __shared__ long long s_grab;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     constexpr int kWarps = kColThreads / 32;
-    static_assert(kColChunk == 512 && kColTile == kWarps * kColChunk, "a chunk is 4 vectors per lane");
-    uint32_t *sm = s_mask[warp];
+    static_assert(kColChunk == 512 && kColTile == kWarps * kColChunk, "a chunk is one 16-element unit per lane");
     const int4 *tok4 = reinterpret_cast<const int4 *>(A.tokens);
-    for (int64_t tile = A.tile_lo + blockIdx.x; tile < A.tile_hi; tile += gridDim.x) {
-        const int64_t chunk = tile * kWarps + warp;
-        const int64_t a0 = chunk * kColChunk;
-        if (a0 >= A.total_elems) continue;
-        const int4 *cp = reinterpret_cast<const int4 *>(A.chunks + chunk);
-        const int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
-        int64_t off_s = (int64_t)(((uint64_t)(uint32_t)c0.y << 32) | (uint32_t)c0.x);
-        int64_t s = c0.z;
-        uint32_t W = (uint32_t)c0.w, area = (uint32_t)c1.x;
-        int64_t sp_s = (int64_t)(uint32_t)c1.y;
-        const int64_t e0 = a0 - off_s;
-        int acc = 0;
-        if (e0 + kColChunk <= (int64_t)area) {
-            // ---------------- interior chunk ----------------
-            const uint32_t b0 = (uint32_t)c1.z, t0 = (uint32_t)c1.w;
-            const bool wide = W >= (uint32_t)kColChunk;            // then t0 + x < 2 W: quotient 0 or 1
-            const uint32_t M = (W >= 2u && !wide) ? 0xFFFFFFFFu / W + 1u : 0u;  // ceil(2^32 / W); exact for n < 1024
-            uint32_t q[4];
-            int t[4];
-            bool fast[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const uint32_t n = t0 + (uint32_t)(k * 32 + lane) * 4u;  // column if the row never ended
+    for (;;) {
+        __syncthreads();  // everyone has read the previous s_grab
+        if (threadIdx.x == 0) s_grab = (long long)atomicAdd(A.tile_counter, (unsigned long long)kColGrab);
+        __syncthreads();
+        const int64_t tile_begin = A.tile_lo + s_grab;
+        if (tile_begin >= A.tile_hi) break;
+        const int64_t tile_end = min(tile_begin + kColGrab, A.tile_hi);
+#pragma unroll 1
+        for (int64_t tile = tile_begin; tile < tile_end; ++tile) {
+            const int64_t chunk = tile * kWarps + warp;
+            const int64_t a0 = chunk * kColChunk;
+            if (a0 >= A.total_elems) break;
+            const int4 *cp = reinterpret_cast<const int4 *>(A.chunks + chunk);
+            const int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
+            int64_t off_s = (int64_t)(((uint64_t)(uint32_t)c0.y << 32) | (uint32_t)c0.x);
+            int64_t s = c0.z;
+            uint32_t W = (uint32_t)c0.w, area = (uint32_t)c1.x;
+            int64_t sp_s = (int64_t)(uint32_t)c1.y;
+            const int64_t e0 = a0 - off_s;
+            int acc = 0;
+            if (e0 + kColChunk <= (int64_t)area) {
+                // ---------------- interior chunk: lane = one 16-element unit ----------------
+                const uint32_t b0 = (uint32_t)c1.z, t0 = (uint32_t)c1.w;
+                const bool wide = W >= (uint32_t)kColChunk;  // then t0 + 16 l < 2 W: the row index grows by 0 or 1
+                // ceil(2^32 / W): floor(n / W) == umulhi(n, M) for n < 1024 and 2 <= W < 512
+                const uint32_t M = (W >= 2u && !wide) ? 0xFFFFFFFFu / W + 1u : 0u;
+                const uint32_t n = t0 + 16u * (uint32_t)lane;  // column if the row never ended
                 const uint32_t d = wide ? (n >= W ? 1u : 0u) : (W >= 2u ? __umulhi(n, M) : n);
-                t[k] = (int)(n - d * W);
-                q[k] = (uint32_t)sp_s + b0 + d;  // samples_emitted < 2^31
-                fast[k] = (uint32_t)t[k] + 4u <= W;
-            }
-            RowRegs r[4];
+                const int t = (int)(n - d * W);
+                const uint32_t q = (uint32_t)sp_s + b0 + d;  // samples_emitted < 2^31
+                const bool fast = (uint32_t)t + 16u <= W;
+                const RowRegs r = load_row(A.rows, (int64_t)q);
+                const int64_t g = r.tok + t;            // index of the unit's first token in d_tokens
+                const int64_t qv = g >> 2;              // aligned vector that holds it
+                const int64_t send = r.tok + r.len;     // one past the sample's last token
+                const bool ld = fast && t < r.len;
+                int4 v[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) r[k] = load_row(A.rows, (int64_t)q[k]);
-            int4 v0[4];
-            bool ld[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                ld[k] = fast[k] && t[k] < r[k].len;
-                v0[k] = ld[k] ? __ldg(tok4 + ((r[k].tok + t[k]) >> 2)) : make_int4(0, 0, 0, 0);
-            }
-            uint32_t mword[4];
-            // vectors that cross a row end (one per row of the block: rare, but a dependent chain of
-            // row-descriptor and token loads): the warp handles them together, one element per lane,
-            // while the aligned loads above are in flight
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                mword[k] = 0;
-                uint32_t sb = __ballot_sync(ODB_FULL_MASK, !fast[k]);
-                while (sb) {  // warp-uniform; up to 8 straddling vectors per pass, 4 lanes each
-                    uint32_t rest = sb;
-                    int src = -1;
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int l = rest ? __ffs(rest) - 1 : -1;
-                        if (l >= 0) rest &= rest - 1;
-                        if ((lane >> 2) == j) src = l;
-                    }
+                for (int i = 0; i < 4; ++i)
+                    v[i] = (fast && ((qv + i) << 2) < send) ? __ldg(tok4 + qv + i) : make_int4(0, 0, 0, 0);
+                // Units that cross a row end (one per row of the block: rare, but a dependent chain
+                // of row-descriptor and token loads): the warp handles two of them per pass, one
+                // element per lane, while the aligned loads above are in flight.
+                int4 mv = make_int4(0, 0, 0, 0);
+                uint32_t sb = __ballot_sync(ODB_FULL_MASK, !fast);
+                while (sb) {  // warp-uniform
+                    const int l0 = __ffs(sb) - 1;
+                    sb &= sb - 1;
+                    const int l1 = sb ? __ffs(sb) - 1 : -1;
+                    if (sb) sb &= sb - 1;
+                    const int src = lane < 16 ? l0 : l1;
                     uint32_t m = 0;
                     if (src >= 0) {
-                        const int j = lane & 3;
-                        const uint32_t ee = (uint32_t)e0 + (uint32_t)(k * 32 + src) * 4u + (uint32_t)j;
+                        const int j = lane & 15;
+                        const uint32_t ee = (uint32_t)e0 + 16u * (uint32_t)src + (uint32_t)j;
                         const uint32_t bb = ee / W;
                         const int c = (int)(ee - bb * W);
                         const int64_t qq = sp_s + bb;
                         const RowRegs rr = load_row(A.rows, qq);
                         int32_t id, lb, ps;
                         one_element<SHIFT>(A, rr, qq, c, id, lb, ps, m);
-                        const int64_t aa = a0 + (int64_t)(k * 32 + src) * 4 + j;
+                        const int64_t aa = a0 + 16 * src + j;
                         A.ids[aa] = id;
                         A.labels[aa] = lb;
                         A.pos[aa] = ps;
                         acc += (lb != A.ignore_index) ? 1 : 0;
-                        m <<= 8 * j;
+                        m <<= 8 * (j & 3);
                     }
-                    // combine the 4 mask bytes of each quad and hand the word to the owning lane
+                    // quad w of each half-warp assembles mask word w of its unit; hand the 4 words to the owner
                     m |= __shfl_xor_sync(ODB_FULL_MASK, m, 1);
                     m |= __shfl_xor_sync(ODB_FULL_MASK, m, 2);
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const int owner = __shfl_sync(ODB_FULL_MASK, src, 4 * j);
-                        const uint32_t w = __shfl_sync(ODB_FULL_MASK, m, 4 * j);
-                        if (owner == lane) mword[k] = w;
-                    }
-                    sb = rest;
+                    const uint32_t w0 = __shfl_sync(ODB_FULL_MASK, m, 0), w1 = __shfl_sync(ODB_FULL_MASK, m, 4);
+                    const uint32_t w2 = __shfl_sync(ODB_FULL_MASK, m, 8), w3 = __shfl_sync(ODB_FULL_MASK, m, 12);
+                    const uint32_t u0 = __shfl_sync(ODB_FULL_MASK, m, 16), u1 = __shfl_sync(ODB_FULL_MASK, m, 20);
+                    const uint32_t u2 = __shfl_sync(ODB_FULL_MASK, m, 24), u3 = __shfl_sync(ODB_FULL_MASK, m, 28);
+                    if (lane == l0) mv = make_int4((int)w0, (int)w1, (int)w2, (int)w3);
+                    if (lane == l1) mv = make_int4((int)u0, (int)u1, (int)u2, (int)u3);
                 }
-            }
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                // the following aligned vector: from the right-hand neighbour when it loaded it
-                int4 n;
-                n.x = __shfl_down_sync(ODB_FULL_MASK, v0[k].x, 1);
-                n.y = __shfl_down_sync(ODB_FULL_MASK, v0[k].y, 1);
-                n.z = __shfl_down_sync(ODB_FULL_MASK, v0[k].z, 1);
-                n.w = __shfl_down_sync(ODB_FULL_MASK, v0[k].w, 1);
-                // neighbour in the same row and loaded <=> its vector is the one after ours
-                const uint32_t tag = ld[k] ? q[k] : 0xFFFFFFFFu;
+                // the vector after our four: the right-hand neighbour's first, when it is in the same
+                // row and loaded it
+                int4 nb;
+                nb.x = __shfl_down_sync(ODB_FULL_MASK, v[0].x, 1);
+                nb.y = __shfl_down_sync(ODB_FULL_MASK, v[0].y, 1);
+                nb.z = __shfl_down_sync(ODB_FULL_MASK, v[0].z, 1);
+                nb.w = __shfl_down_sync(ODB_FULL_MASK, v[0].w, 1);
+                const uint32_t tag = ld ? q : 0xFFFFFFFFu;
                 const uint32_t ntag = __shfl_down_sync(ODB_FULL_MASK, tag, 1);
-                if (fast[k]) {
-                    const int64_t g = r[k].tok + t[k];
-                    const bool from_nb = lane < 31 && ntag == q[k];
-                    if (!from_nb) {
-                        const int64_t qn = (g >> 2) + 1;
-                        const bool need = ld[k] && (qn << 2) < r[k].tok + r[k].len;
-                        n = need ? __ldg(tok4 + qn) : make_int4(0, 0, 0, 0);
-                    }
-                    // x[j] = word (skew + j) of the 8-word window v0 | n
-                    int32_t w[8] = {v0[k].x, v0[k].y, v0[k].z, v0[k].w, n.x, n.y, n.z, n.w};
-                    const int sk = (int)g & 3;
-                    if (sk & 1) {
+                if (fast) {
+                    if (!(lane < 31 && ntag == q))
+                        nb = (ld && ((qv + 4) << 2) < send) ? __ldg(tok4 + qv + 4) : make_int4(0, 0, 0, 0);
+                    const int32_t w[20] = {v[0].x, v[0].y, v[0].z, v[0].w, v[1].x, v[1].y, v[1].z, v[1].w, v[2].x, v[2].y,
+                                           v[2].z, v[2].w, v[3].x, v[3].y, v[3].z, v[3].w, nb.x,   nb.y,   nb.z,   nb.w};
+                    int32_t x[17];
+                    switch ((int)g & 3) {  // the skew is the same for every unit of a row
+                    case 0:
 #pragma unroll
-                        for (int j = 0; j < 7; ++j) w[j] = w[j + 1];
-                    }
-                    if (sk & 2) {
+                        for (int j = 0; j < 17; ++j) x[j] = w[j];
+                        break;
+                    case 1:
 #pragma unroll
-                        for (int j = 0; j < 5; ++j) w[j] = w[j + 2];
+                        for (int j = 0; j < 17; ++j) x[j] = w[j + 1];
+                        break;
+                    case 2:
+#pragma unroll
+                        for (int j = 0; j < 17; ++j) x[j] = w[j + 2];
+                        break;
+                    default:
+#pragma unroll
+                        for (int j = 0; j < 17; ++j) x[j] = w[j + 3];
+                        break;
                     }
-                    const int32_t x[5] = {w[0], w[1], w[2], w[3], w[4]};
-                    emit_vector<SHIFT>(A, r[k], (int64_t)q[k], t[k], x, a0 + (int64_t)(k * 32 + lane) * 4, mword[k], acc);
+                    mv = emit_unit<SHIFT>(A, r, (int64_t)q, t, x, a0 + 16 * lane, acc);
                 }
-            }
-            // mask: lane l holds the words of vectors k*32 + l; lane l stores vectors 4l .. 4l+3
-#pragma unroll
-            for (int k = 0; k < 4; ++k) sm[k * 32 + lane] = mword[k];
-            __syncwarp();
-            const int4 mv = *reinterpret_cast<const int4 *>(sm + 4 * lane);
-            __syncwarp();
-            __stcs(reinterpret_cast<int4 *>(A.mask + a0) + lane, mv);
-            const int tot = __reduce_add_sync(ODB_FULL_MASK, acc);
-            if (lane == 0 && tot != 0) atomicAdd(&A.grp_valid[s], tot);
-        } else {
-            // ---------------- boundary chunk: generic per-vector path ----------------
-            int64_t off_n = A.grp_offset[s + 1];
-            int64_t acc_slot = -1;
+                *reinterpret_cast<int4 *>(A.mask + a0 + 16 * lane) = mv;
+                const int tot = __reduce_add_sync(ODB_FULL_MASK, acc);
+                if (lane == 0 && tot != 0) atomicAdd(&A.grp_valid[s], tot);
+            } else {
+                // ---------------- boundary chunk: generic per-vector path ----------------
+                int64_t off_n = A.grp_offset[s + 1];
+                int64_t acc_slot = -1;
 #pragma unroll 1
-            for (int k = 0; k < 4; ++k) {
-                const int64_t a = a0 + (int64_t)(k * 32 + lane) * 4;
-                if (a >= A.total_elems) break;
-                bool moved = false;
-                while (a >= off_n) {
-                    ++s;
-                    off_s = off_n;
-                    off_n = A.grp_offset[s + 1];
-                    moved = true;
-                }
-                if (moved) {
-                    W = (uint32_t)A.grp_width[s];
-                    area = (uint32_t)A.grp_count[s] * W;
-                    sp_s = A.grp_sample_ptr[s];
-                }
-                const uint32_t e = (uint32_t)(a - off_s);
-                if (e >= area) continue;  // alignment gap: never written
-                if (s != acc_slot) {
-                    if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
-                    acc = 0;
-                    acc_slot = s;
-                }
-                const uint32_t b = e / W;
-                const uint32_t t = e - b * W;
-                uint32_t mw;
-                int nvalid = 4;
-                if (t + 4 <= W) {
-                    const int64_t q = sp_s + b;
-                    const RowRegs r = load_row(A.rows, q);
-                    const int32_t *tp = A.tokens + r.tok + t;
-                    const int nreal = max(0, min(5, r.len - (int)t));
-                    int32_t x[5];
+                for (int k = 0; k < 4; ++k) {
+                    const int64_t a = a0 + (int64_t)(k * 32 + lane) * 4;
+                    if (a >= A.total_elems) break;
+                    bool moved = false;
+                    while (a >= off_n) {
+                        ++s;
+                        off_s = off_n;
+                        off_n = A.grp_offset[s + 1];
+                        moved = true;
+                    }
+                    if (moved) {
+                        W = (uint32_t)A.grp_width[s];
+                        area = (uint32_t)A.grp_count[s] * W;
+                        sp_s = A.grp_sample_ptr[s];
+                    }
+                    const uint32_t e = (uint32_t)(a - off_s);
+                    if (e >= area) continue;  // alignment gap: never written
+                    if (s != acc_slot) {
+                        if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
+                        acc = 0;
+                        acc_slot = s;
+                    }
+                    const uint32_t b = e / W;
+                    const uint32_t t = e - b * W;
+                    uint32_t mw;
+                    int nvalid = 4;
+                    if (t + 4 <= W) {
+                        const int64_t q = sp_s + b;
+                        const RowRegs r = load_row(A.rows, q);
+                        const int32_t *tp = A.tokens + r.tok + t;
+                        const int nreal = max(0, min(5, r.len - (int)t));
+                        int32_t x[5];
 #pragma unroll
-                    for (int j = 0; j < 5; ++j) x[j] = (j < nreal) ? __ldg(tp + j) : A.pad_id;
-                    emit_vector<SHIFT>(A, r, q, (int)t, x, a, mw, acc);
-                } else {
-                    mw = straddle_vector<SHIFT>(A, a, e, W, area, sp_s, acc);
-                    nvalid = (int)min(4u, area - e);
+                        for (int j = 0; j < 5; ++j) x[j] = (j < nreal) ? __ldg(tp + j) : A.pad_id;
+                        emit_vector<SHIFT>(A, r, q, (int)t, x, a, mw, acc);
+                    } else {
+                        mw = straddle_vector<SHIFT>(A, a, e, W, area, sp_s, acc);
+                        nvalid = (int)min(4u, area - e);
+                    }
+                    if (nvalid == 4) {
+                        __stcs(reinterpret_cast<unsigned int *>(A.mask + a), mw);
+                    } else {
+                        for (int j = 0; j < nvalid; ++j) A.mask[a + j] = (uint8_t)(mw >> (8 * j));
+                    }
                 }
-                if (nvalid == 4) {
-                    __stcs(reinterpret_cast<unsigned int *>(A.mask + a), mw);
-                } else {
-                    for (int j = 0; j < nvalid; ++j) A.mask[a + j] = (uint8_t)(mw >> (8 * j));
-                }
+                if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
             }
-            if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
         }
     }
 }
@@ -449,7 +494,9 @@ cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st)
         if (e != cudaSuccess) return e;
         if (occ[sh] < 1) occ[sh] = 1;
     }
-    int blocks = (int)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * occ[sh]);
+    int blocks = (int)std::min<int64_t>((n_tiles + kColGrab - 1) / kColGrab, (int64_t)c->sm_count * occ[sh]);
+    cudaError_t em = cudaMemsetAsync(args.tile_counter, 0, sizeof(unsigned long long), st);
+    if (em != cudaSuccess) return em;
     if (sh) k_collate<true><<<blocks, kColThreads, 0, st>>>(args);
     else k_collate<false><<<blocks, kColThreads, 0, st>>>(args);
     ODB_LAUNCH_CHECK(c);

@@ -22,7 +22,8 @@ constexpr int kMergeThreads = 256;
 constexpr int kRankThreads = 1024;  // one CTA per rank for A2..A8
 constexpr int kColThreads = 256;    // collate CTA (A10)
 constexpr int kColTile = 4096;      // arena elements per collate tile (one CTA iteration)
-constexpr int kColChunk = 512;      // arena elements per warp per tile (4 vectors per lane)
+constexpr int kColChunk = 512;      // arena elements per warp per tile (one 16-element unit per lane)
+constexpr int kColGrab = 16;        // tiles a CTA takes from the work counter at a time
 
 // Per-round status record: written by the round's kernels, copied to pinned host memory (A7).
 struct RoundRec {
@@ -79,6 +80,7 @@ struct CollateArgs {
     int32_t *pos;
     uint8_t *mask;
     int32_t *grp_valid;
+    unsigned long long *tile_counter;  // work counter of the launch (zeroed before it)
     int64_t total_elems;
     int64_t tile_lo, tile_hi;  // tiles [tile_lo, tile_hi) are processed by this launch
     int32_t pad_id, ignore_index, shift_labels;
@@ -167,6 +169,7 @@ struct odb_ctx {
     odb::RoundRec *h_rec = nullptr;  // pinned
     odb::PlanTotals *d_tot = nullptr;
     odb::PlanTotals *h_tot = nullptr;  // pinned
+    unsigned long long *d_tile_counter = nullptr;
 
     // step-major staging tables [step * R + r], growable
     odb::DevBuf<int32_t> st_count, st_width, st_idoff, st_round, step_samples;
