@@ -12,6 +12,7 @@ from .gen import (  # noqa: F401
     config5_cells,
     make_workload,
     protocol_workload,
+    custom_workload,
     audit_distribution,
     AUDIT_KINDS,
     token_ids,

@@ -326,6 +326,14 @@ def protocol_workload(kind: str, seed: int = 0, **over) -> Workload:
     return _assemble(kind, per, spans, 7000 + seed, params)
 
 
+def custom_workload(name: str, per_rank_lengths, seed: int = 0, **params) -> Workload:
+    """A workload from explicit per-rank length arrays (prompt spans drawn with the usual rule)."""
+    rng = np.random.default_rng(2000 + seed)
+    per = [np.asarray(x, dtype=np.int64) for x in per_rank_lengths]
+    spans = [_prompt_only(rng, p) for p in per]
+    return _assemble(name, per, spans, 9000 + seed, params)
+
+
 def describe(wl: Workload) -> dict:
     """Realised descriptors the paper uses for workloads: mean, CV, max, f_s."""
     l = wl.lengths.astype(np.float64)

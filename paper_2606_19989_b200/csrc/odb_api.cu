@@ -60,9 +60,8 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->jA);
     cudaFree(c->jB);
     cudaFree(c->mark);
-    cudaFree(c->flag);
     cudaFree(c->posflag);
-    cudaFree(c->emitted);
+    cudaFree(c->emit_pos);
     cudaFree(c->gpos);
     cudaFree(c->agpos);
     cudaFree(c->agcnt);
@@ -81,7 +80,7 @@ static void free_all(odb_ctx *c) {
     if (c->h_tot) cudaFreeHost(c->h_tot);
     c->st_count.release();
     c->st_width.release();
-    c->st_idoff.release();
+    c->st_real.release();
     c->st_round.release();
     c->step_samples.release();
     c->grp_count.release();
@@ -89,7 +88,7 @@ static void free_all(odb_ctx *c) {
     c->grp_round.release();
     c->grp_valid.release();
     c->grp_real.release();
-    c->grp_idoff.release();
+    c->scan_state.release();
     c->grp_offset.release();
     c->grp_sample_ptr.release();
     c->grp_sample_ids.release();
@@ -164,9 +163,8 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->jA, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->jB, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->mark, N + R);
-    if (e == cudaSuccess) e = dev_alloc(&c->flag, N);
     if (e == cudaSuccess) e = dev_alloc(&c->posflag, N);
-    if (e == cudaSuccess) e = dev_alloc(&c->emitted, N);
+    if (e == cudaSuccess) e = dev_alloc(&c->emit_pos, N);
     if (e == cudaSuccess) e = dev_alloc(&c->gpos, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->agpos, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->agcnt, N + R);
@@ -260,15 +258,7 @@ static int begin_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank
     c->d_lengths = d_lengths;
     CU(c, cudaSetDevice(c->device));
     CU(c, cudaMemcpyAsync(c->d_rank_ptr, c->h_rank_ptr.data(), (R + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
-    CU(c, cudaMemsetAsync(c->n_left, 0, R * sizeof(int32_t), st));
-    CU(c, cudaMemsetAsync(c->fetch_pos, 0, R * sizeof(int32_t), st));
-    CU(c, cudaMemsetAsync(c->emit_cur, 0, R * sizeof(int32_t), st));
-    CU(c, cudaMemsetAsync(c->G, 0, R * sizeof(int32_t), st));
-    CU(c, cudaMemsetAsync(c->S, 0, R * sizeof(int32_t), st));
-    CU(c, cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st));
-    if (c->n_total > 0) CU(c, cudaMemsetAsync(c->emitted, 0, (size_t)c->n_total, st));
-    if (c->step_samples.p) CU(c, cudaMemsetAsync(c->step_samples.p, 0, c->step_samples.cap * sizeof(int32_t), st));
-    CU(c, launch_validate_lengths(c, st));
+    CU(c, launch_begin(c, st));  // rank state, emit positions, step totals, length validation
     c->n_finished = 0;
     for (int r = 0; r < R; ++r)
         if (h_rank_ptr[r + 1] == h_rank_ptr[r]) c->n_finished++;
@@ -318,12 +308,11 @@ int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_
         const size_t used = (size_t)c->n_steps * R;
         CU(c, grow_preserve(c->st_count, (size_t)want * R, used, st));
         CU(c, grow_preserve(c->st_width, (size_t)want * R, used, st));
-        CU(c, grow_preserve(c->st_idoff, (size_t)want * R, used, st));
+        CU(c, grow_preserve(c->st_real, (size_t)want * R, used, st));
         CU(c, grow_preserve(c->st_round, (size_t)want * R, used, st));
         CU(c, grow_preserve(c->step_samples, (size_t)want, (size_t)c->n_steps, st));
         c->step_cap = want;
     }
-    CU(c, cudaMemsetAsync(&c->d_rec->n_finished, 0, sizeof(int32_t), st));
     CU(c, launch_round_form(c, st));
     c->state = 1;
     c->last_T = -1;
@@ -404,7 +393,6 @@ int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
     CU(c, c->grp_round.ensure(n_slots + 1));
     CU(c, c->grp_valid.ensure(n_slots + 1));
     CU(c, c->grp_real.ensure(n_slots + 1));
-    CU(c, c->grp_idoff.ensure(n_slots + 1));
     CU(c, c->grp_offset.ensure(n_slots + 1));
     CU(c, c->grp_sample_ptr.ensure(n_slots + 1));
     CU(c, c->grp_sample_ids.ensure((size_t)c->n_total + 1));
@@ -495,8 +483,7 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
     const int64_t n_chunks = (I.total_elems + kColChunk - 1) / kColChunk;
     CU(c, c->chunks.ensure((size_t)n_chunks + 1));
     CU(c, launch_row_desc(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st));
-    CU(c, launch_chunk_table(c, n_chunks, st));
-    if (n_slots) CU(c, cudaMemsetAsync(c->grp_valid.p, 0, n_slots * sizeof(int32_t), st));
+    CU(c, launch_chunk_table(c, st));
     // ev[1]..ev[2] brackets the collate kernel alone; the pre/post work is ev[0]..ev[1] / ev[2]..ev[3]
     if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
     std::vector<int64_t> rank_off(2);
@@ -508,20 +495,34 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
         if (rc != ODB_OK) return rc;
     }
     if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
-    CU(c, launch_step_valid(c, c->step_valid.p, st));
-    // tables
-    CU(c, copy_tab(o->d_grp_count, c->grp_count.p, n_slots, st));
-    CU(c, copy_tab(o->d_grp_width, c->grp_width.p, n_slots, st));
-    CU(c, copy_tab(o->d_grp_round, c->grp_round.p, n_slots, st));
-    CU(c, copy_tab(o->d_grp_valid_tokens, c->grp_valid.p, n_slots, st));
-    CU(c, copy_tab(o->d_grp_real_tokens, c->grp_real.p, n_slots, st));
-    CU(c, copy_tab(o->d_grp_offset, c->grp_offset.p, n_slots, st));
-    CU(c, copy_tab(o->d_grp_sample_ptr, c->grp_sample_ptr.p, n_slots + 1, st));
-    CU(c, copy_tab(o->d_grp_sample_ids, c->grp_sample_ids.p, (size_t)I.samples_emitted, st));
-    CU(c, copy_tab(o->d_step_samples, c->step_samples.p, (size_t)I.n_steps, st));
-    CU(c, copy_tab(o->d_step_valid_tokens, c->step_valid.p, (size_t)I.n_steps, st));
-    CU(c, copy_tab(o->d_left_ptr, c->left_ptr.p, (size_t)R + 1, st));
-    CU(c, copy_tab(o->d_left_ids, c->left_out.p, (size_t)I.samples_left, st));
+    {  // step totals + every table copy in one launch
+        PostArgs P;
+        memset(&P, 0, sizeof(P));
+        P.R = R;
+        P.n_steps = I.n_steps;
+        P.grp_valid = c->grp_valid.p;
+        P.step_valid = c->step_valid.p;
+        P.user_step_valid = o->d_step_valid_tokens;
+        auto job = [&](void *dst, const void *src, size_t n, size_t elem) {
+            if (!dst || n == 0) return;
+            P.job[P.n_jobs].dst = dst;
+            P.job[P.n_jobs].src = src;
+            P.job[P.n_jobs].words = (int64_t)(n * elem / 4);
+            P.n_jobs++;
+        };
+        job(o->d_grp_count, c->grp_count.p, n_slots, 4);
+        job(o->d_grp_width, c->grp_width.p, n_slots, 4);
+        job(o->d_grp_round, c->grp_round.p, n_slots, 4);
+        job(o->d_grp_valid_tokens, c->grp_valid.p, n_slots, 4);
+        job(o->d_grp_real_tokens, c->grp_real.p, n_slots, 4);
+        job(o->d_grp_offset, c->grp_offset.p, n_slots, 8);
+        job(o->d_grp_sample_ptr, c->grp_sample_ptr.p, n_slots + 1, 8);
+        job(o->d_grp_sample_ids, c->grp_sample_ids.p, (size_t)I.samples_emitted, 4);
+        job(o->d_step_samples, c->step_samples.p, (size_t)I.n_steps, 4);
+        job(o->d_left_ptr, c->left_ptr.p, (size_t)R + 1, 8);
+        job(o->d_left_ids, c->left_out.p, (size_t)I.samples_left, 4);
+        CU(c, launch_post(c, P, st));
+    }
     if (c->timing) {
         CU(c, cudaEventRecord(c->ev[3], st));
         c->ev_valid = true;
@@ -689,7 +690,6 @@ int64_t odb_debug_read(odb_ctx *c, int what, void *h_dst, int64_t max_bytes) {
     case 0: src = c->G; bytes = (int64_t)R * 4; break;
     case 1: src = c->S; bytes = (int64_t)R * 4; break;
     case 2: src = c->sorted; bytes = c->n_total * 8; break;
-    case 3: src = c->flag; bytes = c->n_total; break;
     default: return -1;
     }
     if (!src) return -1;

@@ -16,72 +16,42 @@ namespace odb {
     } while (0)
 
 // ---------------------------------------------------------------------------------------------
-// row descriptors: one warp per slot walks the slot's rows
+// row descriptors: one thread per sample (coalesced reads of sample_ptr / lengths / span CSR); the
+// row index of an emitted sample is its rank's first row + its position in the rank's emit region.
+// Also clears what the collate kernel accumulates into: grp_valid and the tile counter.
+// grid = (ceil(max n_r / 256), R)
 // ---------------------------------------------------------------------------------------------
-__global__ void k_row_desc(int R, int n_steps, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ len,
+__global__ void k_row_desc(int n_steps, int64_t n_slots, const int64_t *__restrict__ rank_ptr,
+                           const int32_t *__restrict__ len, const int32_t *__restrict__ emit_pos,
                            const int64_t *__restrict__ sample_ptr, const int64_t *__restrict__ span_ptr,
                            const int32_t *__restrict__ span_lo, const int32_t *__restrict__ span_hi,
-                           const int32_t *__restrict__ grp_count, const int64_t *__restrict__ grp_sample_ptr,
-                           const int32_t *__restrict__ grp_sample_ids, RowDesc *__restrict__ rows,
-                           int64_t *__restrict__ row_sp) {
-    const int lane = threadIdx.x & 31;
-    const int64_t n_slots = (int64_t)R * n_steps;
-    const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
-    for (int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; s < n_slots; s += warps) {
-        const int r = (int)(s / n_steps);
-        const int64_t base = rank_ptr[r];
-        const int c = grp_count[s];
-        const int64_t q0 = grp_sample_ptr[s];
-        for (int j = lane; j < c; j += 32) {
-            const int64_t g = base + grp_sample_ids[q0 + j];
-            RowDesc d;
-            d.tok = sample_ptr[g];
-            d.len = len[g];
-            const int64_t sp = span_ptr ? span_ptr[g] : 0;
-            const int ns = span_ptr ? (int)(span_ptr[g + 1] - sp) : 0;
-            d.nspan = ns;
-            d.lo0 = ns > 0 ? span_lo[sp] : 0;
-            d.hi0 = ns > 0 ? span_hi[sp] : 0;
-            d.lo1 = ns > 1 ? span_lo[sp + 1] : 0;
-            d.hi1 = ns > 1 ? span_hi[sp + 1] : 0;
-            rows[q0 + j] = d;
-            row_sp[q0 + j] = sp;
-        }
-    }
-}
-
-// Chunk table: chunk c = arena elements [512 c, 512 c + 512).  One thread per chunk finds the slot
-// that holds the chunk's first element (binary search in grp_offset; among equal offsets -- IDLE
-// slots have no elements -- the last one) and stores everything the collate kernel needs to start
-// on the chunk with ONE 32-byte load: the slot's geometry and (row, column) of the first element.
-__global__ void k_chunk_table(int64_t n_chunks, int64_t n_slots, const int64_t *__restrict__ grp_offset,
-                              const int32_t *__restrict__ grp_count, const int32_t *__restrict__ grp_width,
-                              const int64_t *__restrict__ grp_sample_ptr, ChunkRec *__restrict__ chunks) {
-    for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c < n_chunks; c += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t a0 = c * kColChunk;
-        int64_t lo = 0, hi = n_slots;  // last s in [0, n_slots) with grp_offset[s] <= a0
-        while (hi - lo > 1) {
-            const int64_t m = (lo + hi) >> 1;
-            if (__ldg(grp_offset + m) <= a0) lo = m;
-            else hi = m;
-        }
-        const int64_t s = lo;
-        ChunkRec r;
-        r.off_s = grp_offset[s];
-        r.slot = (int32_t)s;
-        r.W = (uint32_t)grp_width[s];
-        r.area = (uint32_t)grp_count[s] * r.W;
-        r.sp_s = (uint32_t)grp_sample_ptr[s];
-        const uint64_t e0 = (uint64_t)(a0 - r.off_s);
-        if (r.W > 0 && e0 < r.area) {
-            r.b0 = (uint32_t)(e0 / r.W);
-            r.t0 = (uint32_t)(e0 - (uint64_t)r.b0 * r.W);
-        } else {
-            r.b0 = 0;
-            r.t0 = 0;
-        }
-        chunks[c] = r;
-    }
+                           const int64_t *__restrict__ grp_sample_ptr, RowDesc *__restrict__ rows,
+                           int64_t *__restrict__ row_sp, int32_t *__restrict__ grp_valid,
+                           unsigned long long *__restrict__ tile_counter) {
+    const int r = blockIdx.y;
+    const int64_t lin = ((int64_t)r * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
+    for (int64_t s = lin; s < n_slots; s += (int64_t)gridDim.x * gridDim.y * blockDim.x) grp_valid[s] = 0;
+    if (lin == 0) *tile_counter = 0ull;
+    const int64_t base = rank_ptr[r];
+    const int n_r = (int)(rank_ptr[r + 1] - base);
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_r) return;
+    const int64_t g = base + i;
+    const int p = emit_pos[g];
+    if (p < 0) return;
+    const int64_t q = grp_sample_ptr[(int64_t)r * n_steps] + p;
+    RowDesc d;
+    d.tok = sample_ptr[g];
+    d.len = len[g];
+    const int64_t sp = span_ptr ? span_ptr[g] : 0;
+    const int ns = span_ptr ? (int)(span_ptr[g + 1] - sp) : 0;
+    d.nspan = ns;
+    d.lo0 = ns > 0 ? span_lo[sp] : 0;
+    d.hi0 = ns > 0 ? span_hi[sp] : 0;
+    d.lo1 = ns > 1 ? span_lo[sp + 1] : 0;
+    d.hi1 = ns > 1 ? span_hi[sp + 1] : 0;
+    rows[q] = d;
+    row_sp[q] = sp;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -448,12 +418,21 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
     }
 }
 
-// step_valid_tokens[k] = sum over ranks of grp_valid_tokens[r][k]  (Eq. 2's T_tok per step)
-__global__ void k_step_valid(int R, int n_steps, const int32_t *__restrict__ grp_valid, int64_t *__restrict__ step_valid) {
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_steps; k += gridDim.x * blockDim.x) {
+// After the collate kernel, one launch: step_valid_tokens[k] = sum over ranks of grp_valid_tokens[r][k]
+// (Eq. 2's T_tok per step), written to the library's table and the caller's, and the copies of the
+// plan tables into the caller's buffers (4-byte words).
+__global__ void k_post(const PostArgs A) {
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k = tid; k < A.n_steps; k += nth) {
         long long s = 0;
-        for (int r = 0; r < R; ++r) s += grp_valid[(int64_t)r * n_steps + k];
-        step_valid[k] = s;
+        for (int r = 0; r < A.R; ++r) s += A.grp_valid[(int64_t)r * A.n_steps + k];
+        A.step_valid[k] = s;
+        if (A.user_step_valid) A.user_step_valid[k] = s;
+    }
+    for (int j = 0; j < A.n_jobs; ++j) {
+        const uint32_t *__restrict__ src = reinterpret_cast<const uint32_t *>(A.job[j].src);
+        uint32_t *__restrict__ dst = reinterpret_cast<uint32_t *>(A.job[j].dst);
+        for (int64_t i = tid; i < A.job[j].words; i += nth) dst[i] = src[i];
     }
 }
 
@@ -464,21 +443,10 @@ cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64
                             const int32_t *d_span_lo, const int32_t *d_span_hi, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const int64_t n_slots = (int64_t)R * c->n_steps;
-    if (n_slots == 0) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>((n_slots * 32 + 255) / 256, (int64_t)c->sm_count * 8);
-    k_row_desc<<<blocks, 256, 0, st>>>(R, c->n_steps, c->d_rank_ptr, c->d_lengths, d_sample_ptr, d_span_ptr, d_span_lo,
-                                       d_span_hi, c->grp_count.p, c->grp_sample_ptr.p, c->grp_sample_ids.p, c->rows.p,
-                                       c->row_sp.p);
-    ODB_LAUNCH_CHECK(c);
-    return cudaSuccess;
-}
-
-cudaError_t launch_chunk_table(odb_ctx *c, int64_t n_chunks, cudaStream_t st) {
-    const int64_t n_slots = (int64_t)c->prm.n_ranks * c->n_steps;
-    if (n_slots == 0 || n_chunks == 0) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>((n_chunks + 255) / 256, (int64_t)c->sm_count * 16);
-    k_chunk_table<<<blocks, 256, 0, st>>>(n_chunks, n_slots, c->grp_offset.p, c->grp_count.p, c->grp_width.p,
-                                          c->grp_sample_ptr.p, c->chunks.p);
+    const int gx = std::max((c->max_nr + 255) / 256, 1);
+    k_row_desc<<<dim3(gx, R), 256, 0, st>>>(c->n_steps, n_slots, c->d_rank_ptr, c->d_lengths, c->emit_pos, d_sample_ptr,
+                                            d_span_ptr, d_span_lo, d_span_hi, c->grp_sample_ptr.p, c->rows.p, c->row_sp.p,
+                                            c->grp_valid.p, c->d_tile_counter);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
@@ -486,27 +454,26 @@ cudaError_t launch_chunk_table(odb_ctx *c, int64_t n_chunks, cudaStream_t st) {
 cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st) {
     const int64_t n_tiles = args.tile_hi - args.tile_lo;
     if (n_tiles <= 0) return cudaSuccess;
-    static int occ[2] = {0, 0};
     const int sh = args.shift_labels ? 1 : 0;
-    if (occ[sh] == 0) {
-        cudaError_t e = sh ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[sh], k_collate<true>, kColThreads, 0)
-                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ[sh], k_collate<false>, kColThreads, 0);
+    if (c->col_occ[sh] == 0) {
+        cudaError_t e = sh ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->col_occ[sh], k_collate<true>, kColThreads, 0)
+                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->col_occ[sh], k_collate<false>, kColThreads, 0);
         if (e != cudaSuccess) return e;
-        if (occ[sh] < 1) occ[sh] = 1;
+        if (c->col_occ[sh] < 1) c->col_occ[sh] = 1;
     }
-    int blocks = (int)std::min<int64_t>((n_tiles + kColGrab - 1) / kColGrab, (int64_t)c->sm_count * occ[sh]);
-    cudaError_t em = cudaMemsetAsync(args.tile_counter, 0, sizeof(unsigned long long), st);
-    if (em != cudaSuccess) return em;
+    int blocks = (int)std::min<int64_t>((n_tiles + kColGrab - 1) / kColGrab, (int64_t)c->sm_count * c->col_occ[sh]);
     if (sh) k_collate<true><<<blocks, kColThreads, 0, st>>>(args);
     else k_collate<false><<<blocks, kColThreads, 0, st>>>(args);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
 
-cudaError_t launch_step_valid(odb_ctx *c, int64_t *d_step_valid, cudaStream_t st) {
-    if (c->n_steps == 0) return cudaSuccess;
-    int blocks = std::min((c->n_steps + 255) / 256, c->sm_count * 4);
-    k_step_valid<<<blocks, 256, 0, st>>>(c->prm.n_ranks, c->n_steps, c->grp_valid.p, d_step_valid);
+cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st) {
+    int64_t work = args.n_steps;
+    for (int j = 0; j < args.n_jobs; ++j) work = std::max(work, args.job[j].words);
+    if (work == 0) return cudaSuccess;
+    int blocks = (int)std::min<int64_t>((work + 255) / 256, (int64_t)c->sm_count * 8);
+    k_post<<<blocks, 256, 0, st>>>(args);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

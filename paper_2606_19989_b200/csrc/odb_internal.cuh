@@ -20,6 +20,11 @@ constexpr int kSortChunk = 4096;    // keys sorted in shared memory by one CTA (
 constexpr int kSortThreads = 512;
 constexpr int kMergeThreads = 256;
 constexpr int kRankThreads = 1024;  // one CTA per rank for A2..A8
+constexpr size_t kFormSmemLimit = 231424;  // dynamic shared memory of k_form_groups_smem (227 KB - static)
+constexpr int kAlignSmemKeys = 8192;       // overflow sort keys kept in shared memory by k_align
+constexpr int kFinThreads = 512;           // k_fin_scan: tile = kFinThreads * kFinItems slots
+constexpr int kFinItems = 4;
+constexpr int kFinTile = kFinThreads * kFinItems;
 constexpr int kColThreads = 256;    // collate CTA (A10)
 constexpr int kColTile = 4096;      // arena elements per collate tile (one CTA iteration)
 constexpr int kColChunk = 512;      // arena elements per warp per tile (one 16-element unit per lane)
@@ -43,6 +48,15 @@ struct PlanTotals {
     int64_t padded_elems;
     unsigned long long real_tokens;
     int64_t samples_left;
+};
+
+// State of one tile of the slot scan (decoupled look-back): flag 0 = nothing, 1 = agg valid,
+// 2 = inc (inclusive prefix) valid.
+struct __align__(16) ScanTile {
+    long long agg[4];
+    long long inc[4];
+    int flag;
+    int pad_[3];
 };
 
 // One emitted row (sample) as the collate kernel wants it: 32 bytes, two 16-byte loads.
@@ -84,6 +98,21 @@ struct CollateArgs {
     int64_t total_elems;
     int64_t tile_lo, tile_hi;  // tiles [tile_lo, tile_hi) are processed by this launch
     int32_t pad_id, ignore_index, shift_labels;
+};
+
+// k_post: table copies (4-byte words) + the per-step valid-token totals
+struct CopyJob {
+    void *dst;
+    const void *src;
+    int64_t words;
+};
+struct PostArgs {
+    CopyJob job[12];
+    int n_jobs;
+    int R, n_steps;
+    const int32_t *grp_valid;
+    int64_t *step_valid;
+    int64_t *user_step_valid;
 };
 
 // growable device buffer (cudaMalloc on growth only)
@@ -131,6 +160,8 @@ struct odb_ctx {
     bool ev_valid = false;
     cudaEvent_t ev_status = nullptr;
     cudaStream_t last_stream = nullptr;
+    int col_occ[2] = {0, 0};  // resident collate CTAs per SM (shift 0 / 1)
+    bool attr_form = false, attr_align = false;  // cudaFuncSetAttribute done on this device
 
     // inputs fixed by the first odb_form_groups after create / reset
     const int32_t *d_lengths = nullptr;
@@ -158,9 +189,8 @@ struct odb_ctx {
     uint64_t *ovf = nullptr;            // 2*n_max + 2 (overflow sort keys)
     int32_t *jA = nullptr, *jB = nullptr;  // n_max + R
     uint8_t *mark = nullptr;            // n_max + R
-    uint8_t *flag = nullptr;            // n_max
     uint8_t *posflag = nullptr;         // n_max
-    uint8_t *emitted = nullptr;         // n_max
+    int32_t *emit_pos = nullptr;        // n_max: index in the rank's emit region, -1 = not emitted
     int32_t *gpos = nullptr;            // n_max + R
     int32_t *agpos = nullptr, *agcnt = nullptr, *agoff = nullptr;  // n_max + R
     int32_t *left_ids = nullptr, *emit_ids = nullptr;              // n_max
@@ -172,11 +202,12 @@ struct odb_ctx {
     unsigned long long *d_tile_counter = nullptr;
 
     // step-major staging tables [step * R + r], growable
-    odb::DevBuf<int32_t> st_count, st_width, st_idoff, st_round, step_samples;
+    odb::DevBuf<int32_t> st_count, st_width, st_real, st_round, step_samples;
     int64_t step_cap = 0;
 
     // rank-major plan tables built by odb_plan_query
-    odb::DevBuf<int32_t> grp_count, grp_width, grp_round, grp_valid, grp_real, grp_idoff;
+    odb::DevBuf<int32_t> grp_count, grp_width, grp_round, grp_valid, grp_real;
+    odb::DevBuf<unsigned char> scan_state;
     odb::DevBuf<int64_t> grp_offset, grp_sample_ptr;
     odb::DevBuf<int32_t> grp_sample_ids, left_out;
     odb::DevBuf<int64_t> left_ptr, step_valid;
@@ -194,14 +225,14 @@ struct odb_ctx {
 
 namespace odb {
 // ---- launchers implemented in odb_plan.cu ----------------------------------------------------
-cudaError_t launch_validate_lengths(odb_ctx *c, cudaStream_t st);
+cudaError_t launch_begin(odb_ctx *c, cudaStream_t st);  // per-run state reset + length validation
 cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st);   // A0..A3
 cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commit
 cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st);     // A9 + tables + leftovers
 // ---- launchers implemented in odb_collate.cu -------------------------------------------------
 cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
                             const int32_t *d_span_lo, const int32_t *d_span_hi, cudaStream_t st);
-cudaError_t launch_chunk_table(odb_ctx *c, int64_t n_chunks, cudaStream_t st);
+cudaError_t launch_chunk_table(odb_ctx *c, cudaStream_t st);
 cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st);
-cudaError_t launch_step_valid(odb_ctx *c, int64_t *d_step_valid, cudaStream_t st);
+cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st);
 }  // namespace odb

@@ -96,12 +96,29 @@ __device__ __forceinline__ int window_size(int n_left, int fetch_pos, int n_r, i
 }
 
 // ---------------------------------------------------------------------------------------------
-// length validation (len >= 1), once per run
+// start of a run: clear the per-rank state, mark every sample un-emitted, zero the step totals and
+// validate the lengths (len >= 1) -- one launch.  rec was zeroed by the caller.
 // ---------------------------------------------------------------------------------------------
-__global__ void k_validate_lengths(const int32_t *__restrict__ len, int64_t n, RoundRec *rec) {
+__global__ void k_begin(const int32_t *__restrict__ len, int64_t n, int R, int32_t *__restrict__ n_left,
+                        int32_t *__restrict__ fetch_pos, int32_t *__restrict__ emit_cur, int32_t *__restrict__ G,
+                        int32_t *__restrict__ S, int32_t *__restrict__ emit_pos, int32_t *__restrict__ step_samples,
+                        int64_t step_cap, RoundRec *rec) {
     int bad = 0;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        if (len[i] < 1) bad = 1;
+    const int64_t bound = max(n, max((int64_t)R, step_cap));
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < bound; i += (int64_t)gridDim.x * blockDim.x) {
+        if (i < R) {
+            n_left[i] = 0;
+            fetch_pos[i] = 0;
+            emit_cur[i] = 0;
+            G[i] = 0;
+            S[i] = 0;
+        }
+        if (i < n) {
+            emit_pos[i] = -1;
+            if (len[i] < 1) bad = 1;
+        }
+        if (i < step_cap) step_samples[i] = 0;
+    }
     if (__syncthreads_or(bad) && threadIdx.x == 0) rec->bad_length = 1;
 }
 
@@ -113,14 +130,17 @@ __global__ void k_validate_lengths(const int32_t *__restrict__ len, int64_t n, R
 __global__ void __launch_bounds__(kSortThreads)
 k_chunk_sort(const int32_t *__restrict__ len, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ n_left,
              const int32_t *__restrict__ fetch_pos, const int32_t *__restrict__ left_ids, int buffer_size,
-             uint64_t *__restrict__ keys_out, int32_t *__restrict__ S_out) {
+             uint64_t *__restrict__ keys_out, int32_t *__restrict__ S_out, RoundRec *rec) {
     __shared__ uint64_t sk[kSortChunk];
     const int r = blockIdx.y;
     const int64_t base = rank_ptr[r];
     const int n_r = (int)(rank_ptr[r + 1] - base);
     const int nl = n_left[r], fp = fetch_pos[r];
     const int S = window_size(nl, fp, n_r, buffer_size);
-    if (blockIdx.x == 0 && threadIdx.x == 0) S_out[r] = S;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        S_out[r] = S;
+        if (r == 0) rec->n_finished = 0;  // counted again by this round's commit
+    }
     const int c0 = blockIdx.x * kSortChunk;
     if (c0 >= S) return;
     const int cnt = min(kSortChunk, S - c0);
@@ -182,12 +202,102 @@ k_merge_pass(const uint64_t *__restrict__ src, uint64_t *__restrict__ dst, const
 //              after B(l) samples, l = the last sample of the previous group).
 //   MAXFIT:    x = ascending position; J[x] = largest e <= S with (e - x) * slen[e-1] <= L, >= x+1.
 // Round p marks next^(k + 2^p)(0) for every marked next^k(0) and squares the jump array, so after
-// ceil(log2 G) + 1 rounds exactly the orbit of 0 is marked.
+// ceil(log2 G) + 1 rounds exactly the orbit of 0 is marked.  Output: ascending start positions
+// gpos[0..G] (gpos[G] = S) and G_r.  A THRESHOLD mark at chase x > 0 is the ascending start S - x.
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int successor(const uint64_t *__restrict__ k, int x, int S, uint32_t budget, int rule) {
+    if (x == S) return S;
+    if (rule == ODB_RULE_THRESHOLD) {
+        if (x == 0) return 1;
+        const uint32_t l = key_len(k[S - x]);  // v[x-1] = ascending position S-1-(x-1)
+        uint32_t q = budget / (l > 0u ? l : 1u);  // Eq. 1 floor; budget < 2^31
+        if (q < 1u) q = 1u;
+        const uint32_t jj = (uint32_t)x + q;  // < 2^32
+        return (int)(jj < (uint32_t)S ? jj : (uint32_t)S);
+    }
+    int lo = x + 1, hi = S;  // the singleton [x, x+1) is always accepted (U10)
+    while (lo < hi) {
+        const int m = (lo + hi + 1) >> 1;
+        if ((long long)(m - x) * (long long)key_len(k[m - 1]) <= (long long)budget) lo = m;
+        else hi = m - 1;
+    }
+    return lo;
+}
+
+// Shared-memory version (windows of up to kFormSmemMaxS samples): the jump arrays are uint16 pairs
+// of buffers and the marks a bit set, all in the CTA's shared memory, so a round costs shared-memory
+// latency instead of L2 round trips.
+__global__ void __launch_bounds__(kRankThreads)
+k_form_groups_smem(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr,
+                   const int32_t *__restrict__ S_arr, uint32_t budget, int rule, int32_t *__restrict__ gpos,
+                   int32_t *__restrict__ G_out) {
+    extern __shared__ __align__(16) unsigned char fg_smem[];
+    __shared__ int s_scan[34];
+    const int r = blockIdx.x;
+    const int S = S_arr[r];
+    if (S == 0) {
+        if (threadIdx.x == 0) G_out[r] = 0;
+        return;
+    }
+    const int64_t base = rank_ptr[r];
+    const uint64_t *k = keys + base;
+    const int n1 = S + 1;
+    const int n1p = (n1 + 7) & ~7;
+    const int words = (n1 + 31) >> 5;
+    uint16_t *cur = reinterpret_cast<uint16_t *>(fg_smem);
+    uint16_t *nxt = cur + n1p;
+    uint32_t *mk = reinterpret_cast<uint32_t *>(nxt + n1p);
+    for (int w = threadIdx.x; w < words; w += blockDim.x) mk[w] = (w == 0) ? 1u : 0u;  // x = 0 is a start
+    for (int x = threadIdx.x; x <= S; x += blockDim.x) cur[x] = (uint16_t)successor(k, x, S, budget, rule);
+    __syncthreads();
+    while (true) {
+        int changed = 0;
+        for (int x = threadIdx.x; x <= S; x += blockDim.x) {
+            const int j = cur[x];
+            nxt[x] = cur[j];  // cur[S] == S
+            if (j < S && ((mk[x >> 5] >> (x & 31)) & 1u) && !((mk[j >> 5] >> (j & 31)) & 1u)) {
+                atomicOr(&mk[j >> 5], 1u << (j & 31));
+                changed = 1;
+            }
+        }
+        if (!__syncthreads_or(changed)) break;
+        uint16_t *t = cur;
+        cur = nxt;
+        nxt = t;
+    }
+    // marks live on x in [0, S); G = their number
+    int part = 0;
+    for (int w = threadIdx.x; w < words; w += blockDim.x) part += __popc(mk[w]);
+    int G;
+    (void)block_excl_scan<int>(part, s_scan, G);
+    int32_t *gp = gpos + base + r;
+    int carry = 0;
+    for (int w0 = 0; w0 < words; w0 += blockDim.x) {
+        const int w = w0 + threadIdx.x;
+        uint32_t bits = w < words ? mk[w] : 0u;
+        int tot;
+        int i = block_excl_scan<int>(__popc(bits), s_scan, tot) + carry;
+        while (bits) {
+            const int x = (w << 5) + __ffs(bits) - 1;
+            bits &= bits - 1;
+            if (rule == ODB_RULE_THRESHOLD) gp[G - i] = S - x;  // i-th mark (ascending x) -> start S - x
+            else gp[i] = x;
+            ++i;
+        }
+        carry += tot;
+    }
+    if (threadIdx.x == 0) {
+        if (rule == ODB_RULE_THRESHOLD) gp[0] = 0;
+        else gp[G] = S;
+        G_out[r] = G;
+    }
+}
+
+// Global-memory version for windows that do not fit the shared-memory one.
 __global__ void __launch_bounds__(kRankThreads)
 k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
-              long long budget, int rule, int32_t *jA, int32_t *jB, uint8_t *mark, uint8_t *__restrict__ flag,
-              int32_t *__restrict__ gpos, int32_t *__restrict__ G_out) {
+              uint32_t budget, int rule, int32_t *jA, int32_t *jB, uint8_t *mark, int32_t *__restrict__ gpos,
+              int32_t *__restrict__ G_out) {
     __shared__ int s_scan[34];
     const int r = blockIdx.x;
     const int S = S_arr[r];
@@ -201,29 +311,7 @@ k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ ran
     int32_t *cur = jA + jb, *nxt = jB + jb;
     uint8_t *mk = mark + jb;
     for (int x = threadIdx.x; x <= S; x += blockDim.x) {
-        int j;
-        if (x == S) {
-            j = S;
-        } else if (rule == ODB_RULE_THRESHOLD) {
-            if (x == 0) {
-                j = 1;
-            } else {
-                long long l = (long long)key_len(k[S - x]);  // v[x-1] = ascending position S-1-(x-1)
-                long long q = budget / (l > 0 ? l : 1);
-                if (q < 1) q = 1;
-                long long jj = (long long)x + q;
-                j = (int)(jj < (long long)S ? jj : (long long)S);
-            }
-        } else {
-            int lo = x + 1, hi = S;  // the singleton [x, x+1) is always accepted (U10)
-            while (lo < hi) {
-                int m = (lo + hi + 1) >> 1;
-                if ((long long)(m - x) * (long long)key_len(k[m - 1]) <= budget) lo = m;
-                else hi = m - 1;
-            }
-            j = lo;
-        }
-        cur[x] = j;
+        cur[x] = successor(k, x, S, budget, rule);
         mk[x] = (x == 0) ? 1 : 0;
     }
     __syncthreads();
@@ -242,16 +330,9 @@ k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ ran
         cur = nxt;
         nxt = t;
     }
-    // start flags in ascending coordinates; compact the start positions
-    uint8_t *fl = flag + base;
     int32_t *gp = gpos + jb;
     int G = block_compact(
-        S, s_scan,
-        [&](int a) {
-            bool f = (rule == ODB_RULE_THRESHOLD) ? (a == 0 || mk[S - a] != 0) : (mk[a] != 0);
-            fl[a] = f ? 1 : 0;
-            return f;
-        },
+        S, s_scan, [&](int a) { return (rule == ODB_RULE_THRESHOLD) ? (a == 0 || mk[S - a] != 0) : (mk[a] != 0); },
         [&](int a, int kidx) { gp[kidx] = a; });
     if (threadIdx.x == 0) {
         gp[G] = S;
@@ -260,16 +341,22 @@ k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ ran
 }
 
 // ---------------------------------------------------------------------------------------------
-// A4 + A5 + A6: T_grp (Eq. 3), split (the d rightmost non-start positions become starts, which is
-// what Alg. 1's backward scan produces), overflow (sort groups by
-// (count desc, index asc), keep the first T).  Output per rank: aligned groups in emit order as
+// A4 + A5 + A6: T_grp (Eq. 3), split, overflow.  Output per rank: aligned groups in emit order as
 // (agpos[k], agcnt[k]) over the sorted window, k < T.  Adds the counts into step_samples (A8a).
+//
+// Split closed form: Alg. 1's backward scan pops the last row of the rightmost
+// multi-sample group until G_r = T, i.e. it turns the d = T - G_r rightmost NON-START positions of
+// the sorted window into starts.  With ns(j) = (S - gpos[j]) - (G_r - j) = non-start positions in
+// groups j.., group j gives up k_j = min(d, ns(j)) - min(d, ns(j+1)) rows, and its head moves to
+// list index h_j = j + d - min(d, ns(j)); its k_j singletons follow it.  No scan needed.
+//
+// Overflow: sort groups by (count desc, index asc), keep the first T (shared memory when G_r fits).
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kRankThreads)
 k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr, const int32_t *__restrict__ G_arr, int R,
-        int slot_capacity, const uint8_t *__restrict__ flag, const int32_t *__restrict__ gpos, int32_t *__restrict__ agpos,
-        int32_t *__restrict__ agcnt, uint64_t *ovf, int32_t *step_samples, int step_base, RoundRec *rec) {
-    __shared__ int s_scan[34];
+        int slot_capacity, const int32_t *__restrict__ gpos, int32_t *__restrict__ agpos, int32_t *__restrict__ agcnt,
+        uint64_t *ovf, int32_t *step_samples, int step_base, RoundRec *rec) {
+    extern __shared__ __align__(16) unsigned char al_smem[];
     __shared__ int s_maxG, s_minS;
     const int r = blockIdx.x;
     if (threadIdx.x == 0) {
@@ -300,33 +387,40 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
     int32_t *ap = agpos + jb, *ac = agcnt + jb;
     if (Gr <= T) {
         const int d = T - Gr;
-        const uint8_t *fl = flag + base;
-        int carry_old = 0, carry_new = 0;
-        for (int b0 = 0; b0 < S; b0 += blockDim.x) {
-            int a = b0 + threadIdx.x;
-            int f = (a < S) ? fl[a] : 0;
-            int tot_old, tot_new;
-            int ex_old = block_excl_scan<int>(f, s_scan, tot_old) + carry_old;
-            int nf = 0;
-            if (a < S) {
-                int nonstarts_right = (S - a) - (Gr - ex_old);  // non-start positions in [a, S)
-                nf = (f || nonstarts_right <= d) ? 1 : 0;
+        const int lane = threadIdx.x & 31;
+        for (int j0 = (threadIdx.x >> 5) << 5; j0 < Gr; j0 += blockDim.x) {  // warp-uniform trip count
+            const int j = j0 + lane;
+            int p = 0, pn = 0, kj = 0, h = 0;
+            if (j < Gr) {
+                p = gp[j];
+                pn = gp[j + 1];
+                const int conv_from = min(d, (S - p) - (Gr - j));
+                const int conv_after = min(d, (S - pn) - (Gr - 1 - j));
+                kj = conv_from - conv_after;
+                h = j + d - conv_from;
+                const int c = pn - p - kj;
+                ap[h] = p;
+                ac[h] = c;
+                atomicAdd(&step_samples[step_base + h], c);
             }
-            int ex_new = block_excl_scan<int>(nf, s_scan, tot_new) + carry_new;
-            if (nf) ap[ex_new] = a;
-            carry_old += tot_old;
-            carry_new += tot_new;
+            uint32_t sp = __ballot_sync(ODB_FULL_MASK, kj > 0);
+            while (sp) {  // expand the singletons of the (few) groups that split
+                const int src = __ffs(sp) - 1;
+                sp &= sp - 1;
+                const int kk = __shfl_sync(ODB_FULL_MASK, kj, src);
+                const int hh = __shfl_sync(ODB_FULL_MASK, h, src);
+                const int pe = __shfl_sync(ODB_FULL_MASK, pn, src);
+                for (int i = lane; i < kk; i += 32) {
+                    ap[hh + 1 + i] = pe - kk + i;
+                    ac[hh + 1 + i] = 1;
+                    atomicAdd(&step_samples[step_base + hh + 1 + i], 1);
+                }
+            }
         }
         if (threadIdx.x == 0) ap[T] = S;
-        __syncthreads();
-        for (int k = threadIdx.x; k < T; k += blockDim.x) {
-            int c = ap[k + 1] - ap[k];
-            ac[k] = c;
-            atomicAdd(&step_samples[step_base + k], c);
-        }
     } else {
-        uint64_t *ok = ovf + 2 * base;
         const int n2 = next_pow2(Gr);
+        uint64_t *ok = (n2 <= kAlignSmemKeys) ? reinterpret_cast<uint64_t *>(al_smem) : ovf + 2 * base;
         for (int j = threadIdx.x; j < n2; j += blockDim.x) {
             uint64_t key = ~0ull;
             if (j < Gr) key = ((uint64_t)(uint32_t)(S - (gp[j + 1] - gp[j])) << 32) | (uint32_t)j;
@@ -346,16 +440,17 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
 
 // ---------------------------------------------------------------------------------------------
 // A7 + A8a: commit the round.  Finds the quota cut k* (non-join), writes the step-major staging
-// tables, appends the emitted ids to the rank's emit region, compacts the leftovers, advances the
-// rank state and counts the ranks that will be finished next round.
+// tables, appends the emitted ids to the rank's emit region (recording every sample's emit
+// position), compacts the leftovers, advances the rank state and counts the ranks that will be
+// finished next round.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kRankThreads)
 k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
          const int32_t *__restrict__ G_arr, int R, const int32_t *__restrict__ agpos, const int32_t *__restrict__ agcnt,
          int32_t *__restrict__ agoff, const int32_t *__restrict__ step_samples, int step_base, int round, int join_mode,
          long long quota, long long emitted_before, int32_t *__restrict__ st_count, int32_t *__restrict__ st_width,
-         int32_t *__restrict__ st_idoff, int32_t *__restrict__ st_round, uint8_t *__restrict__ posflag,
-         int32_t *__restrict__ emit_ids, uint8_t *__restrict__ emitted, int32_t *__restrict__ left_ids, int32_t *n_left,
+         int32_t *__restrict__ st_real, int32_t *__restrict__ st_round, uint8_t *__restrict__ posflag,
+         int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
          int32_t *fetch_pos, int32_t *emit_cur, RoundRec *rec) {
     __shared__ int s_scan[34];
     __shared__ long long s_scan64[34];
@@ -403,7 +498,7 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
             int64_t idx = (int64_t)(step_base + k) * R + r;
             st_count[idx] = 0;
             st_width[idx] = 0;
-            st_idoff[idx] = 0;
+            st_real[idx] = 0;
             st_round[idx] = round;
         }
         if (threadIdx.x == 0) atomicAdd(&rec->n_finished, 1);
@@ -415,7 +510,10 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
     int32_t *ao = agoff + jb;
     uint8_t *pf = posflag + base;
     const int cur = emit_cur[r];
-    for (int a = threadIdx.x; a < S; a += blockDim.x) pf[a] = 0;
+    // every sample of the window is emitted unless groups were dropped (overflow) or cut (quota)
+    const bool all_emitted = (Gr <= T) && (T_emit == T);
+    if (!all_emitted)
+        for (int a = threadIdx.x; a < S; a += blockDim.x) pf[a] = 0;
     int carry = 0;
     for (int b0 = 0; b0 < T_emit; b0 += blockDim.x) {
         int k = b0 + threadIdx.x;
@@ -427,7 +525,6 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
             int p = ap[k];
             st_count[idx] = c;
             st_width[idx] = (int32_t)key_len(k_[p + c - 1]);  // rows ascending: the last row is the longest
-            st_idoff[idx] = cur + ex;
             st_round[idx] = round;
             ao[k] = cur + ex;
         }
@@ -435,22 +532,30 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
     }
     const int emitted_r = carry;
     __syncthreads();
-    {  // copy ids: one warp per group
+    {  // copy ids and sum the lengths: one warp per group
         const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
         for (int k = w; k < T_emit; k += nw) {
-            int p = ap[k], c = ac[k], o = ao[k];
+            const int p = ap[k], c = ac[k], o = ao[k];
+            uint32_t sum = 0;  // count * max_len <= budget < 2^31, or a singleton
             for (int j = lane; j < c; j += 32) {
-                int id = key_id(k_[p + j]);
+                const uint64_t key = k_[p + j];
+                const int id = key_id(key);
+                sum += key_len(key);
                 emit_ids[base + o + j] = id;
-                emitted[base + id] = 1;
-                pf[p + j] = 1;
+                emit_pos[base + id] = o + j;
+                if (!all_emitted) pf[p + j] = 1;
             }
+            sum = __reduce_add_sync(ODB_FULL_MASK, sum);
+            if (lane == 0) st_real[(int64_t)(step_base + k) * R + r] = (int32_t)sum;
         }
     }
-    __syncthreads();
-    int32_t *lf = left_ids + base;
-    int n_left_new = block_compact(
-        S, s_scan, [&](int a) { return pf[a] == 0; }, [&](int a, int kidx) { lf[kidx] = key_id(k_[a]); });
+    int n_left_new = 0;
+    if (!all_emitted) {
+        __syncthreads();
+        int32_t *lf = left_ids + base;
+        n_left_new = block_compact(
+            S, s_scan, [&](int a) { return pf[a] == 0; }, [&](int a, int kidx) { lf[kidx] = key_id(k_[a]); });
+    }
     if (threadIdx.x == 0) {
         int nl_old = n_left[r], fp = fetch_pos[r];
         int fp_new = fp + (S - nl_old);
@@ -462,126 +567,194 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
 }
 
 // ---------------------------------------------------------------------------------------------
-// A9 and the rank-major plan tables
+// A9 and the rank-major plan tables.
+//
+// k_fin_scan: one pass over the slots in rank-major order s = r * n_steps + k.  Tiles of kFinTile
+// slots take a ticket (so every predecessor tile is running or done), transpose the step-major
+// staging tables, and scan four int64 quantities with decoupled look-back: the 16-aligned block
+// area (-> grp_offset), the sample count (-> grp_sample_ptr), count*width and the real tokens
+// (-> totals).
 // ---------------------------------------------------------------------------------------------
-__global__ void k_fin_slots(int R, int n_steps, const int32_t *__restrict__ st_count, const int32_t *__restrict__ st_width,
-                            const int32_t *__restrict__ st_idoff, const int32_t *__restrict__ st_round,
-                            int32_t *__restrict__ grp_count, int32_t *__restrict__ grp_width, int32_t *__restrict__ grp_round,
-                            int32_t *__restrict__ grp_idoff, int64_t *__restrict__ grp_offset,
-                            int64_t *__restrict__ grp_sample_ptr) {
-    const int64_t n_slots = (int64_t)R * n_steps;
-    for (int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; s < n_slots; s += (int64_t)gridDim.x * blockDim.x) {
-        int r = (int)(s / n_steps);
-        int k = (int)(s - (int64_t)r * n_steps);
-        int64_t src = (int64_t)k * R + r;
-        int c = st_count[src], w = st_width[src];
-        grp_count[s] = c;
-        grp_width[s] = w;
-        grp_round[s] = st_round[src];
-        grp_idoff[s] = st_idoff[src];
-        int64_t area = (int64_t)c * (int64_t)w;
-        grp_offset[s] = (area + 15) / 16 * 16;  // scanned in place by k_scan_slots
-        grp_sample_ptr[s] = c;
-    }
+__device__ __forceinline__ int ld_flag(const int *p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_flag(int *p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// In-place exclusive scans of grp_offset and grp_sample_ptr (n + 1 entries each) by one CTA, and the
-// sum of count*width.  8 consecutive items per thread per iteration.
-__global__ void __launch_bounds__(1024)
-k_scan_slots(int64_t n, int64_t *grp_offset, int64_t *grp_sample_ptr, const int32_t *__restrict__ grp_count,
-             const int32_t *__restrict__ grp_width, PlanTotals *tot) {
+__global__ void __launch_bounds__(kFinThreads)
+k_fin_scan(int R, int n_steps, const int32_t *__restrict__ st_count, const int32_t *__restrict__ st_width,
+           const int32_t *__restrict__ st_real, const int32_t *__restrict__ st_round, int32_t *__restrict__ grp_count,
+           int32_t *__restrict__ grp_width, int32_t *__restrict__ grp_round, int32_t *__restrict__ grp_real,
+           int64_t *__restrict__ grp_offset, int64_t *__restrict__ grp_sample_ptr, ScanTile *tiles, unsigned int *ticket,
+           PlanTotals *tot) {
     __shared__ long long s_scan64[34];
-    constexpr int ITEMS = 8;
-    long long carry_o = 0, carry_p = 0, area_sum = 0;
-    for (int64_t b0 = 0; b0 < n; b0 += (int64_t)blockDim.x * ITEMS) {
-        int64_t i0 = b0 + (int64_t)threadIdx.x * ITEMS;
-        long long vo[ITEMS], vp[ITEMS];
-        long long so = 0, sp = 0;
-#pragma unroll
-        for (int j = 0; j < ITEMS; ++j) {
-            int64_t i = i0 + j;
-            vo[j] = (i < n) ? grp_offset[i] : 0;
-            vp[j] = (i < n) ? grp_sample_ptr[i] : 0;
-            if (i < n) area_sum += (long long)grp_count[i] * (long long)grp_width[i];
-            so += vo[j];
-            sp += vp[j];
-        }
-        long long to, tp;
-        long long eo = block_excl_scan<long long>(so, s_scan64, to) + carry_o;
-        long long ep = block_excl_scan<long long>(sp, s_scan64, tp) + carry_p;
-#pragma unroll
-        for (int j = 0; j < ITEMS; ++j) {
-            int64_t i = i0 + j;
-            if (i < n) {
-                grp_offset[i] = eo;
-                grp_sample_ptr[i] = ep;
-            }
-            eo += vo[j];
-            ep += vp[j];
-        }
-        carry_o += to;
-        carry_p += tp;
-    }
-    long long ta;
-    (void)block_excl_scan<long long>(area_sum, s_scan64, ta);
-    if (threadIdx.x == 0) {
-        grp_offset[n] = carry_o;
-        grp_sample_ptr[n] = carry_p;
-        tot->total_elems = carry_o;
-        tot->samples_emitted = carry_p;
-        tot->padded_elems = ta;
-    }
-}
-
-// One warp per slot: gather the slot's sample ids in row order and sum their lengths.
-__global__ void k_gather_ids(int R, int n_steps, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ len,
-                             const int32_t *__restrict__ emit_ids, const int32_t *__restrict__ grp_idoff,
-                             const int32_t *__restrict__ grp_count, const int64_t *__restrict__ grp_sample_ptr,
-                             int32_t *__restrict__ grp_sample_ids, int32_t *__restrict__ grp_real, PlanTotals *tot) {
-    const int lane = threadIdx.x & 31;
+    __shared__ long long s_base[4];
+    __shared__ int s_tile;
+    if (threadIdx.x == 0) s_tile = (int)atomicAdd(ticket, 1u);
+    __syncthreads();
+    const int tile = s_tile;
     const int64_t n_slots = (int64_t)R * n_steps;
-    const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
-    unsigned long long local = 0;
-    for (int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; s < n_slots; s += warps) {
-        int r = (int)(s / n_steps);
-        int64_t base = rank_ptr[r];
-        int c = grp_count[s];
-        int o = grp_idoff[s];
-        int64_t q0 = grp_sample_ptr[s];
-        long long sum = 0;
-        for (int j = lane; j < c; j += 32) {
-            int id = emit_ids[base + o + j];
-            grp_sample_ids[q0 + j] = id;
-            sum += len[base + id];
-        }
+    const int64_t s0 = (int64_t)tile * kFinTile + (int64_t)threadIdx.x * kFinItems;
+    long long v[4][kFinItems];
+    long long sum[4] = {0, 0, 0, 0};
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) sum += __shfl_xor_sync(ODB_FULL_MASK, sum, d);
-        if (lane == 0) {
-            grp_real[s] = (int32_t)sum;
-            local += (unsigned long long)sum;
+    for (int i = 0; i < kFinItems; ++i) {
+        const int64_t s = s0 + i;
+        long long c = 0, w = 0, re = 0;
+        if (s < n_slots) {
+            const int r = (int)(s / n_steps);
+            const int k = (int)(s - (int64_t)r * n_steps);
+            const int64_t src = (int64_t)k * R + r;
+            c = st_count[src];
+            w = st_width[src];
+            re = st_real[src];
+            grp_count[s] = (int32_t)c;
+            grp_width[s] = (int32_t)w;
+            grp_real[s] = (int32_t)re;
+            grp_round[s] = st_round[src];
+        }
+        const long long area = c * w;
+        v[0][i] = (area + 15) / 16 * 16;
+        v[1][i] = c;
+        v[2][i] = area;
+        v[3][i] = re;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) sum[q] += v[q][i];
+    }
+    long long ex[4], total[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) ex[q] = block_excl_scan<long long>(sum[q], s_scan64, total[q]);
+    ScanTile *me = tiles + tile;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            me->agg[q] = total[q];
+            if (tile == 0) me->inc[q] = total[q];
+        }
+        st_flag(&me->flag, tile == 0 ? 2 : 1);
+        if (tile == 0) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) s_base[q] = 0;
         }
     }
-    if (lane == 0 && local) atomicAdd(&tot->real_tokens, local);
+    if (tile > 0 && threadIdx.x < 32) {  // warp 0 looks back over up to 32 predecessors at a time
+        const int lane = threadIdx.x;
+        long long acc[4] = {0, 0, 0, 0};
+        int t = tile - 1;
+        while (true) {
+            const int tt = t - lane;
+            int f = 2;  // tiles before the first count as "inclusive prefix 0"
+            long long x[4] = {0, 0, 0, 0};
+            if (tt >= 0) {
+                do {
+                    f = ld_flag(&tiles[tt].flag);
+                } while (f == 0);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) x[q] = (f == 2) ? __ldcg(&tiles[tt].inc[q]) : __ldcg(&tiles[tt].agg[q]);
+            }
+            const uint32_t done = __ballot_sync(ODB_FULL_MASK, f == 2);
+            const int first = __ffs(done) - 1;  // nearest tile with an inclusive prefix (done != 0 once tt < 0)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                long long y = (done == 0 || lane <= first) ? x[q] : 0;
+#pragma unroll
+                for (int dlt = 16; dlt > 0; dlt >>= 1) y += __shfl_xor_sync(ODB_FULL_MASK, y, dlt);
+                acc[q] += y;
+            }
+            if (done) break;
+            t -= 32;
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                s_base[q] = acc[q];
+                me->inc[q] = acc[q] + total[q];
+            }
+            st_flag(&me->flag, 2);
+        }
+    }
+    __syncthreads();
+    long long run_o = s_base[0] + ex[0], run_p = s_base[1] + ex[1];
+#pragma unroll
+    for (int i = 0; i < kFinItems; ++i) {
+        const int64_t s = s0 + i;
+        if (s < n_slots) {
+            grp_offset[s] = run_o;
+            grp_sample_ptr[s] = run_p;
+        }
+        run_o += v[0][i];
+        run_p += v[1][i];
+    }
+    const int64_t n_tiles = (n_slots + kFinTile - 1) / kFinTile;
+    if (threadIdx.x == 0 && (int64_t)tile == max(n_tiles, (int64_t)1) - 1) {
+        grp_offset[n_slots] = s_base[0] + total[0];
+        grp_sample_ptr[n_slots] = s_base[1] + total[1];
+        tot->total_elems = s_base[0] + total[0];
+        tot->samples_emitted = s_base[1] + total[1];
+        tot->padded_elems = s_base[2] + total[2];
+        tot->real_tokens = (unsigned long long)(s_base[3] + total[3]);
+    }
 }
 
-// Un-emitted local ids per rank, ascending (Lemma 1: buffer + sampler-pending).
+// Chunk table (A10's work list): chunk c = arena elements [512 c, 512 c + 512).  A slot owns the
+// chunks whose first element lies in its 16-aligned region [grp_offset[s], grp_offset[s+1]) (IDLE
+// slots own none); one warp per slot writes 32-byte records with everything the collate kernel
+// needs to start on the chunk: the slot's geometry and (row, column) of the chunk's first element.
+__global__ void k_chunk_table(int64_t n_slots, const int64_t *__restrict__ grp_offset, const int32_t *__restrict__ grp_count,
+                              const int32_t *__restrict__ grp_width, const int64_t *__restrict__ grp_sample_ptr,
+                              ChunkRec *__restrict__ chunks) {
+    const int lane = threadIdx.x & 31;
+    const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; s < n_slots; s += warps) {
+        const int64_t o = grp_offset[s], on = grp_offset[s + 1];
+        const int64_t c_lo = (o + kColChunk - 1) / kColChunk, c_hi = (on + kColChunk - 1) / kColChunk;
+        if (c_lo >= c_hi) continue;
+        ChunkRec rec;
+        rec.off_s = o;
+        rec.slot = (int32_t)s;
+        rec.W = (uint32_t)grp_width[s];
+        rec.area = (uint32_t)grp_count[s] * rec.W;
+        rec.sp_s = (uint32_t)grp_sample_ptr[s];
+        for (int64_t c = c_lo + lane; c < c_hi; c += 32) {
+            const uint32_t e0 = (uint32_t)(c * kColChunk - o);  // < area: no multiple of 16 lies in the alignment gap
+            rec.b0 = rec.W ? e0 / rec.W : 0u;
+            rec.t0 = e0 - rec.b0 * rec.W;
+            chunks[c] = rec;
+        }
+    }
+}
+
+// Per rank: the slot CSR's ids are the rank's emit region (slots of a rank are in emit order), and
+// the un-emitted local ids, ascending (Lemma 1: buffer + sampler-pending).
 __global__ void __launch_bounds__(kRankThreads)
-k_leftovers(int R, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ emit_cur,
-            const uint8_t *__restrict__ emitted, int64_t *__restrict__ left_ptr, int32_t *__restrict__ left_out,
-            PlanTotals *tot) {
+k_ids_left(int R, int n_steps, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ emit_cur,
+           const int32_t *__restrict__ emit_ids, const int32_t *__restrict__ emit_pos,
+           const int64_t *__restrict__ grp_sample_ptr, int32_t *__restrict__ grp_sample_ids, int64_t *__restrict__ left_ptr,
+           int32_t *__restrict__ left_out, PlanTotals *tot) {
     __shared__ int s_scan[34];
     __shared__ long long s_scan64[34];
     const int r = blockIdx.x;
+    const int64_t base = rank_ptr[r];
+    const int n_r = (int)(rank_ptr[r + 1] - base);
+    const int ec = emit_cur[r];
+    if (ec > 0) {
+        const int64_t q0 = grp_sample_ptr[(int64_t)r * n_steps];
+        for (int j = threadIdx.x; j < ec; j += blockDim.x) grp_sample_ids[q0 + j] = emit_ids[base + j];
+    }
     long long part = 0;
     for (int q = threadIdx.x; q < r; q += blockDim.x) part += (rank_ptr[q + 1] - rank_ptr[q]) - emit_cur[q];
     long long lbase;
     (void)block_excl_scan<long long>(part, s_scan64, lbase);
-    const int64_t base = rank_ptr[r];
-    const int n_r = (int)(rank_ptr[r + 1] - base);
-    const uint8_t *em = emitted + base;
-    int32_t *out = left_out + lbase;
-    int cnt = block_compact(
-        n_r, s_scan, [&](int i) { return em[i] == 0; }, [&](int i, int kidx) { out[kidx] = i; });
+    const int cnt = n_r - ec;
+    if (cnt > 0) {
+        const int32_t *ep = emit_pos + base;
+        int32_t *out = left_out + lbase;
+        (void)block_compact(
+            n_r, s_scan, [&](int i) { return ep[i] < 0; }, [&](int i, int kidx) { out[kidx] = i; });
+    }
     if (threadIdx.x == 0) {
         left_ptr[r] = lbase;
         if (r == R - 1) {
@@ -601,10 +774,15 @@ k_leftovers(int R, const int64_t *__restrict__ rank_ptr, const int32_t *__restri
         if (e_ != cudaSuccess) return e_;         \
     } while (0)
 
-cudaError_t launch_validate_lengths(odb_ctx *c, cudaStream_t st) {
-    if (c->n_total == 0) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>((c->n_total + 1023) / 1024, (int64_t)c->sm_count * 4);
-    k_validate_lengths<<<blocks, 256, 0, st>>>(c->d_lengths, c->n_total, c->d_rec);
+cudaError_t launch_begin(odb_ctx *c, cudaStream_t st) {
+    const int R = c->prm.n_ranks;
+    cudaError_t e = cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st);
+    if (e != cudaSuccess) return e;
+    const int64_t step_cap = c->step_samples.p ? (int64_t)c->step_samples.cap : 0;
+    const int64_t bound = std::max<int64_t>(std::max<int64_t>(c->n_total, R), step_cap);
+    int blocks = (int)std::min<int64_t>((bound + 1023) / 1024, (int64_t)c->sm_count * 4);
+    k_begin<<<std::max(blocks, 1), 256, 0, st>>>(c->d_lengths, c->n_total, R, c->n_left, c->fetch_pos, c->emit_cur, c->G,
+                                                c->S, c->emit_pos, c->step_samples.p, step_cap, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
@@ -615,13 +793,19 @@ static int max_window_bound(const odb_ctx *c) {
     return (int)m;
 }
 
+static size_t form_smem_bytes(int maxS) {
+    const size_t n1p = ((size_t)maxS + 1 + 7) & ~(size_t)7;
+    const size_t words = ((size_t)maxS + 1 + 31) >> 5;
+    return 4 * n1p + 4 * words;
+}
+
 cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const int maxS = max_window_bound(c);
     if (maxS == 0) return cudaSuccess;
     const int chunks = (maxS + kSortChunk - 1) / kSortChunk;
     k_chunk_sort<<<dim3(chunks, R), kSortThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos, c->left_ids,
-                                                          c->prm.buffer_size, c->keyA, c->S);
+                                                          c->prm.buffer_size, c->keyA, c->S, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     uint64_t *src = c->keyA, *dst = c->keyB;
     for (int64_t w = kSortChunk; w < maxS; w *= 2) {
@@ -633,22 +817,40 @@ cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st) {
         dst = t;
     }
     c->sorted = src;
-    k_form_groups<<<R, kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, (long long)c->prm.budget, c->prm.rule, c->jA,
-                                              c->jB, c->mark, c->flag, c->gpos, c->G);
+    const size_t smem = form_smem_bytes(maxS);
+    if (smem <= kFormSmemLimit && maxS <= 65534) {
+        if (!c->attr_form) {
+            cudaError_t e = cudaFuncSetAttribute(k_form_groups_smem, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)kFormSmemLimit);
+            if (e != cudaSuccess) return e;
+            c->attr_form = true;
+        }
+        k_form_groups_smem<<<R, kRankThreads, smem, st>>>(c->sorted, c->d_rank_ptr, c->S, (uint32_t)c->prm.budget,
+                                                          c->prm.rule, c->gpos, c->G);
+    } else {
+        k_form_groups<<<R, kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, (uint32_t)c->prm.budget, c->prm.rule, c->jA,
+                                                  c->jB, c->mark, c->gpos, c->G);
+    }
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
 
 cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
-    k_align<<<R, kRankThreads, 0, st>>>(c->d_rank_ptr, c->S, c->G, R, c->prm.slot_capacity, c->flag, c->gpos, c->agpos,
-                                        c->agcnt, c->ovf, c->step_samples.p, c->n_steps, c->d_rec);
+    const size_t al_smem = (size_t)kAlignSmemKeys * sizeof(uint64_t);
+    if (!c->attr_align) {
+        cudaError_t e = cudaFuncSetAttribute(k_align, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)al_smem);
+        if (e != cudaSuccess) return e;
+        c->attr_align = true;
+    }
+    k_align<<<R, kRankThreads, al_smem, st>>>(c->d_rank_ptr, c->S, c->G, R, c->prm.slot_capacity, c->gpos, c->agpos,
+                                              c->agcnt, c->ovf, c->step_samples.p, c->n_steps, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     k_commit<<<R, kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, c->G, R, c->agpos, c->agcnt, c->agoff,
                                          c->step_samples.p, c->n_steps, c->round, c->prm.join_mode,
                                          (long long)c->prm.sample_quota,
                                          (long long)c->prm.emitted_so_far + (long long)c->samples_emitted, c->st_count.p,
-                                         c->st_width.p, c->st_idoff.p, c->st_round.p, c->posflag, c->emit_ids, c->emitted,
+                                         c->st_width.p, c->st_real.p, c->st_round.p, c->posflag, c->emit_ids, c->emit_pos,
                                          c->left_ids, c->n_left, c->fetch_pos, c->emit_cur, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
@@ -657,27 +859,30 @@ cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st) {
 cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const int64_t n_slots = (int64_t)R * c->n_steps;
-    cudaError_t e = cudaMemsetAsync(c->d_tot, 0, sizeof(PlanTotals), st);
+    const int64_t n_tiles = std::max<int64_t>((n_slots + kFinTile - 1) / kFinTile, 1);
+    cudaError_t e = c->scan_state.ensure((size_t)n_tiles * sizeof(ScanTile) + 64);
     if (e != cudaSuccess) return e;
-    if (n_slots > 0) {
-        int blocks = (int)std::min<int64_t>((n_slots + 255) / 256, (int64_t)c->sm_count * 8);
-        k_fin_slots<<<blocks, 256, 0, st>>>(R, c->n_steps, c->st_count.p, c->st_width.p, c->st_idoff.p, c->st_round.p,
-                                            c->grp_count.p, c->grp_width.p, c->grp_round.p, c->grp_idoff.p,
-                                            c->grp_offset.p, c->grp_sample_ptr.p);
-        ODB_LAUNCH_CHECK(c);
-    }
-    k_scan_slots<<<1, 1024, 0, st>>>(n_slots, c->grp_offset.p, c->grp_sample_ptr.p, c->grp_count.p, c->grp_width.p,
-                                     c->d_tot);
+    // [0, 64): ticket; then the tile states.  d_tot is rewritten in full by the kernels below.
+    e = cudaMemsetAsync(c->scan_state.p, 0, (size_t)n_tiles * sizeof(ScanTile) + 64, st);
+    if (e != cudaSuccess) return e;
+    k_fin_scan<<<(int)n_tiles, kFinThreads, 0, st>>>(R, c->n_steps, c->st_count.p, c->st_width.p, c->st_real.p,
+                                                    c->st_round.p, c->grp_count.p, c->grp_width.p, c->grp_round.p,
+                                                    c->grp_real.p, c->grp_offset.p, c->grp_sample_ptr.p,
+                                                    reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
+                                                    reinterpret_cast<unsigned int *>(c->scan_state.p), c->d_tot);
     ODB_LAUNCH_CHECK(c);
-    if (n_slots > 0) {
-        int blocks = (int)std::min<int64_t>((n_slots * 32 + 255) / 256, (int64_t)c->sm_count * 8);
-        k_gather_ids<<<blocks, 256, 0, st>>>(R, c->n_steps, c->d_rank_ptr, c->d_lengths, c->emit_ids, c->grp_idoff.p,
-                                             c->grp_count.p, c->grp_sample_ptr.p, c->grp_sample_ids.p, c->grp_real.p,
-                                             c->d_tot);
-        ODB_LAUNCH_CHECK(c);
-    }
-    k_leftovers<<<R, kRankThreads, 0, st>>>(R, c->d_rank_ptr, c->emit_cur, c->emitted, c->left_ptr.p, c->left_out.p,
-                                            c->d_tot);
+    k_ids_left<<<R, kRankThreads, 0, st>>>(R, c->n_steps, c->d_rank_ptr, c->emit_cur, c->emit_ids, c->emit_pos,
+                                           c->grp_sample_ptr.p, c->grp_sample_ids.p, c->left_ptr.p, c->left_out.p, c->d_tot);
+    ODB_LAUNCH_CHECK(c);
+    return cudaSuccess;
+}
+
+cudaError_t launch_chunk_table(odb_ctx *c, cudaStream_t st) {
+    const int64_t n_slots = (int64_t)c->prm.n_ranks * c->n_steps;
+    if (n_slots == 0) return cudaSuccess;
+    int blocks = (int)std::min<int64_t>((n_slots * 32 + 255) / 256, (int64_t)c->sm_count * 16);
+    k_chunk_table<<<blocks, 256, 0, st>>>(n_slots, c->grp_offset.p, c->grp_count.p, c->grp_width.p, c->grp_sample_ptr.p,
+                                          c->chunks.p);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

@@ -160,6 +160,27 @@ def test_degenerate_cases(P, oracle):
     assert info.n_steps == 0 and info.total_elems == 0 and info.stop_reason == 0
 
 
+@pytest.mark.parametrize("rule", [0, 1])
+def test_large_window_global_memory_planner(P, oracle, rule):
+    """A window of more than ~56 K samples does not fit the shared-memory list-ranking kernel: the
+    global-memory version runs (rank 0), next to ranks that split heavily to reach its group count."""
+    wl = I.make_workload(0, n_ranks=3, n_per_rank=70_000, budget=1024, rule=rule)
+    plan = _sampled_parity(oracle, wl, n_sample=24)
+    assert plan.n_steps > 1000 and wl.n_samples == 210_000
+
+
+def test_heavy_split_unequal_group_counts(P, oracle):
+    """One rank forms thousands of groups, another a handful of big ones: the split closed form turns
+    thousands of rows of a few groups into singletons (Alg. 1)."""
+    rng = np.random.default_rng(11)
+    a = rng.integers(900, 1024, 6000)          # ~1 sample per group at budget 1024
+    b = rng.integers(1, 4, 6000)               # hundreds of samples per group
+    c = rng.integers(1, 1024, 6000)
+    wl = I.custom_workload("heavy_split", [a, b, c], 17, budget=1024, rule=0, join_mode=1)
+    plan, info, out = _full_parity(oracle, wl)
+    assert plan.n_steps >= 5000
+
+
 def test_bad_length_is_reported(P):
     import torch
     wl = I.make_workload(0)
