@@ -112,7 +112,11 @@ static void free_all(odb_ctx *c) {
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     if (c->ev_status) cudaEventDestroy(c->ev_status);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
     if (c->copy_ev) cudaEventDestroy(c->copy_ev);
+    for (cudaEvent_t e : c->tok_ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->col_ev) cudaEventDestroy(e);
+    if (c->h_rank_off) cudaFreeHost(c->h_rank_off);
 }
 
 extern "C" {
@@ -178,7 +182,7 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->S, R);
     if (e == cudaSuccess) e = dev_alloc(&c->d_rec, 1);
     if (e == cudaSuccess) e = dev_alloc(&c->d_tot, 1);
-    if (e == cudaSuccess) e = dev_alloc(&c->d_tile_counter, 1);
+    if (e == cudaSuccess) e = dev_alloc(&c->d_tile_counter, R + 1);  // one work counter per pipelined launch
     if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_rec, sizeof(RoundRec));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_tot, sizeof(PlanTotals));
     for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
@@ -434,9 +438,11 @@ static int check_capacity(const odb_ctx *c, const odb_outputs *o) {
     return ODB_OK;
 }
 
-// collate slots of ranks [r_lo, r_hi) (rank-major slots are contiguous in the arenas)
-static int collate_ranks(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_span_lo, const int32_t *d_span_hi,
-                         const odb_outputs *o, int r_lo, int r_hi, const std::vector<int64_t> &h_rank_off,
+// One collate launch over the arena elements [elem_lo, elem_hi) (both multiples of 16: slot offsets).
+// Tiles are arena-aligned; a tile that straddles elem_lo / elem_hi is visited by both neighbouring
+// launches, each writing only its own elements.  `counter` is this launch's zeroed work counter.
+static int collate_range(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_span_lo, const int32_t *d_span_hi,
+                         const odb_outputs *o, int64_t elem_lo, int64_t elem_hi, unsigned long long *counter,
                          cudaStream_t st) {
     CollateArgs A;
     A.tokens = d_tokens;
@@ -454,13 +460,11 @@ static int collate_ranks(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_s
     A.pos = o->d_position_ids;
     A.mask = o->d_attention_mask;
     A.grp_valid = c->grp_valid.p;
-    A.tile_counter = c->d_tile_counter;
-    A.total_elems = h_rank_off[r_hi];
-    // tiles are arena-aligned; a rank boundary inside a tile is handled by processing the boundary
-    // tile in the launch that owns its first element (offsets are multiples of 16, tiles of 4096)
-    A.tile_lo = (h_rank_off[r_lo] + kColTile - 1) / kColTile;
-    if (r_lo == 0) A.tile_lo = 0;
-    A.tile_hi = (h_rank_off[r_hi] + kColTile - 1) / kColTile;
+    A.tile_counter = counter;
+    A.total_elems = elem_hi;
+    A.elem_lo = elem_lo;
+    A.tile_lo = elem_lo / kColTile;
+    A.tile_hi = (elem_hi + kColTile - 1) / kColTile;
     A.pad_id = c->prm.pad_id;
     A.ignore_index = c->prm.ignore_index;
     A.shift_labels = c->prm.shift_labels;
@@ -486,12 +490,8 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
     CU(c, launch_chunk_table(c, st));
     // ev[1]..ev[2] brackets the collate kernel alone; the pre/post work is ev[0]..ev[1] / ev[2]..ev[3]
     if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
-    std::vector<int64_t> rank_off(2);
-    rank_off[0] = 0;
-    rank_off[1] = I.total_elems;
-    {
-        // whole arena in one launch: pretend one "rank" spanning everything
-        int rc = collate_ranks(c, d_tokens, d_span_lo, d_span_hi, o, 0, 1, rank_off, st);
+    {  // whole arena in one launch
+        int rc = collate_range(c, d_tokens, d_span_lo, d_span_hi, o, 0, I.total_elems, c->d_tile_counter, st);
         if (rc != ODB_OK) return rc;
     }
     if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
@@ -584,7 +584,6 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     if (N > 0 && (!h_lengths || !h_sample_ptr || !h_tokens)) return ODB_ERR_INVALID_ARG;
     const int64_t n_tok = N > 0 ? h_sample_ptr[N] : 0;
     const int64_t n_span = (h_span_ptr && N > 0) ? h_span_ptr[N] : 0;
-    // inputs host -> device (lengths first: planning needs nothing else)
     CU(c, c->hs_lengths.ensure((size_t)N + 1));
     CU(c, c->hs_sample_ptr.ensure((size_t)N + 1));
     CU(c, c->hs_span_ptr.ensure((size_t)N + 1));
@@ -593,12 +592,23 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     CU(c, c->hs_tokens.ensure((size_t)n_tok + 4));
     if (!c->copy_stream) {
         CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        CU(c, cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
         CU(c, cudaEventCreateWithFlags(&c->copy_ev, cudaEventDisableTiming));
+        CU(c, cudaMallocHost((void **)&c->h_rank_off, (size_t)(R + 1) * sizeof(int64_t)));
+        c->tok_ev.assign((size_t)R, nullptr);
+        c->col_ev.assign((size_t)R, nullptr);
+        for (int r = 0; r < R; ++r) {
+            CU(c, cudaEventCreateWithFlags(&c->tok_ev[r], cudaEventDisableTiming));
+            CU(c, cudaEventCreateWithFlags(&c->col_ev[r], cudaEventDisableTiming));
+        }
     }
+    // Inputs host -> device.  Lengths first, on the compute stream: planning needs nothing else.  The
+    // CSR arrays and then the tokens, RANK BY RANK (an event per rank), go on the copy stream and
+    // overlap the planning kernels, the collate launches of earlier ranks and the result copies.
     if (N > 0) CU(c, cudaMemcpyAsync(c->hs_lengths.p, h_lengths, (size_t)N * 4, cudaMemcpyHostToDevice, st));
-    // tokens and the CSR arrays go on the copy stream, overlapping the planning kernels
     CU(c, cudaEventRecord(c->copy_ev, st));
-    CU(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev, 0));
+    CU(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev, 0));  // orders this call after the previous one's reads
+    CU(c, cudaStreamWaitEvent(c->d2h_stream, c->copy_ev, 0));
     if (N > 0) {
         CU(c, cudaMemcpyAsync(c->hs_sample_ptr.p, h_sample_ptr, (size_t)(N + 1) * 8, cudaMemcpyHostToDevice, c->copy_stream));
         if (h_span_ptr) {
@@ -608,34 +618,43 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
                 CU(c, cudaMemcpyAsync(c->hs_span_hi.p, h_span_hi, (size_t)n_span * 4, cudaMemcpyHostToDevice, c->copy_stream));
             }
         }
-        if (n_tok) CU(c, cudaMemcpyAsync(c->hs_tokens.p, h_tokens, (size_t)n_tok * 4, cudaMemcpyHostToDevice, c->copy_stream));
     }
-    CU(c, cudaEventRecord(c->copy_ev, c->copy_stream));
+    CU(c, cudaEventRecord(c->copy_ev, c->copy_stream));  // CSR arrays landed
+    for (int r = 0; r < R; ++r) {
+        if (N > 0) {
+            const int64_t t0 = h_sample_ptr[h_rank_ptr[r]], t1 = h_sample_ptr[h_rank_ptr[r + 1]];
+            if (t1 > t0)
+                CU(c, cudaMemcpyAsync(c->hs_tokens.p + t0, h_tokens + t0, (size_t)(t1 - t0) * 4, cudaMemcpyHostToDevice,
+                                      c->copy_stream));
+        }
+        CU(c, cudaEventRecord(c->tok_ev[r], c->copy_stream));
+    }
+    auto drain = [&]() {
+        cudaStreamSynchronize(c->copy_stream);
+        cudaStreamSynchronize(c->d2h_stream);
+        cudaStreamSynchronize(st);
+    };
     int rc = run_rounds(c, c->hs_lengths.p, h_rank_ptr, h_out, st);
     if (rc != ODB_OK) {
-        cudaStreamSynchronize(c->copy_stream);
+        drain();
         return rc;
     }
     const odb_plan_info I = *h_out;
-    // host capacities
-    rc = ODB_OK;
-    {
-        odb_outputs chk = *ho;
-        const odb_plan_info &J = I;
-        if (J.total_elems > 0 && (!chk.d_input_ids || !chk.d_labels || !chk.d_position_ids || !chk.d_attention_mask))
+    {  // host capacities
+        const bool any_slot_tab = ho->d_grp_count || ho->d_grp_width || ho->d_grp_round || ho->d_grp_valid_tokens ||
+                                  ho->d_grp_real_tokens || ho->d_grp_offset || ho->d_grp_sample_ptr;
+        if (I.total_elems > 0 && (!ho->d_input_ids || !ho->d_labels || !ho->d_position_ids || !ho->d_attention_mask))
             rc = ODB_ERR_INVALID_ARG;
-        else if (J.total_elems > chk.arena_capacity)
+        else if (I.total_elems > ho->arena_capacity)
             rc = ODB_ERR_CAPACITY;
-        const bool any_slot_tab = chk.d_grp_count || chk.d_grp_width || chk.d_grp_round || chk.d_grp_valid_tokens ||
-                                  chk.d_grp_real_tokens || chk.d_grp_offset || chk.d_grp_sample_ptr;
-        if (rc == ODB_OK && any_slot_tab && chk.slot_capacity_alloc < J.n_slots) rc = ODB_ERR_CAPACITY;
-        if (rc == ODB_OK && chk.d_grp_sample_ids && chk.ids_capacity < J.samples_emitted) rc = ODB_ERR_CAPACITY;
-        if (rc == ODB_OK && (chk.d_step_samples || chk.d_step_valid_tokens) && chk.step_capacity_alloc < J.n_steps)
+        if (rc == ODB_OK && any_slot_tab && ho->slot_capacity_alloc < I.n_slots) rc = ODB_ERR_CAPACITY;
+        if (rc == ODB_OK && ho->d_grp_sample_ids && ho->ids_capacity < I.samples_emitted) rc = ODB_ERR_CAPACITY;
+        if (rc == ODB_OK && (ho->d_step_samples || ho->d_step_valid_tokens) && ho->step_capacity_alloc < I.n_steps)
             rc = ODB_ERR_CAPACITY;
-        if (rc == ODB_OK && chk.d_left_ids && chk.left_capacity < J.samples_left) rc = ODB_ERR_CAPACITY;
+        if (rc == ODB_OK && ho->d_left_ids && ho->left_capacity < I.samples_left) rc = ODB_ERR_CAPACITY;
     }
     if (rc != ODB_OK) {
-        cudaStreamSynchronize(c->copy_stream);
+        drain();
         return rc;
     }
     const size_t E = (size_t)I.total_elems;
@@ -650,21 +669,62 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     dev.d_position_ids = c->hs_pos.p;
     dev.d_attention_mask = c->hs_mask.p;
     dev.arena_capacity = (int64_t)E;
-    CU(c, cudaStreamWaitEvent(st, c->copy_ev, 0));  // tokens have landed
-    c->ev_valid = c->timing != 0;
-    rc = collate_impl(c, c->hs_tokens.p, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p,
-                      c->hs_span_hi.p, &dev, st);
-    if (rc != ODB_OK) return rc;
-    // results device -> host
     const size_t n_slots = (size_t)I.n_slots;
+    c->ev_valid = c->timing != 0;  // ev[0] was recorded by run_rounds
+    if (E > 0) {
+        CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
+        CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
+        CU(c, c->chunks.ensure((size_t)((I.total_elems + kColChunk - 1) / kColChunk) + 1));
+        CU(c, cudaStreamWaitEvent(st, c->copy_ev, 0));  // sample_ptr / spans have landed
+        CU(c, launch_row_desc(c, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p,
+                              c->hs_span_hi.p, st));
+        CU(c, launch_chunk_table(c, st));
+        CU(c, cudaMemsetAsync(c->d_tile_counter, 0, (size_t)(R + 1) * sizeof(unsigned long long), st));
+        // arena offset of every rank's first slot (slots are rank-major): R+1 strided int64
+        CU(c, cudaMemcpy2DAsync(c->h_rank_off, 8, c->grp_offset.p, (size_t)I.n_steps * 8, 8, (size_t)R + 1,
+                                cudaMemcpyDeviceToHost, st));
+        CU(c, cudaStreamSynchronize(st));
+        if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
+        // The pipeline: rank r's slots are collated as soon as its tokens have landed, and its slice of
+        // the four arenas goes back on the device -> host stream while later ranks are still being
+        // uploaded and collated (both directions of the host link busy at once).
+        for (int r = 0; r < R; ++r) {
+            const int64_t lo = c->h_rank_off[r], hi = c->h_rank_off[r + 1];
+            if (hi <= lo) continue;
+            CU(c, cudaStreamWaitEvent(st, c->tok_ev[r], 0));
+            rc = collate_range(c, c->hs_tokens.p, c->hs_span_lo.p, c->hs_span_hi.p, &dev, lo, hi, c->d_tile_counter + r, st);
+            if (rc != ODB_OK) {
+                drain();
+                return rc;
+            }
+            CU(c, cudaEventRecord(c->col_ev[r], st));
+            CU(c, cudaStreamWaitEvent(c->d2h_stream, c->col_ev[r], 0));
+            const size_t n = (size_t)(hi - lo);
+            CU(c, cudaMemcpyAsync(ho->d_input_ids + lo, c->hs_ids.p + lo, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
+            CU(c, cudaMemcpyAsync(ho->d_labels + lo, c->hs_labels.p + lo, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
+            CU(c, cudaMemcpyAsync(ho->d_position_ids + lo, c->hs_pos.p + lo, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
+            CU(c, cudaMemcpyAsync(ho->d_attention_mask + lo, c->hs_mask.p + lo, n, cudaMemcpyDeviceToHost, c->d2h_stream));
+        }
+        if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
+    } else if (c->timing) {
+        CU(c, cudaEventRecord(c->ev[1], st));
+        CU(c, cudaEventRecord(c->ev[2], st));
+    }
+    {  // step totals (Eq. 2's T_tok per step)
+        PostArgs P;
+        memset(&P, 0, sizeof(P));
+        P.R = R;
+        P.n_steps = I.n_steps;
+        P.grp_valid = c->grp_valid.p;
+        P.step_valid = c->step_valid.p;
+        CU(c, launch_post(c, P, st));
+    }
+    if (c->timing) CU(c, cudaEventRecord(c->ev[3], st));
+    // tables device -> host (small) on the compute stream
     auto d2h = [&](void *dst, const void *src, size_t bytes) -> cudaError_t {
         if (!dst || bytes == 0) return cudaSuccess;
         return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
     };
-    CU(c, d2h(ho->d_input_ids, c->hs_ids.p, E * 4));
-    CU(c, d2h(ho->d_labels, c->hs_labels.p, E * 4));
-    CU(c, d2h(ho->d_position_ids, c->hs_pos.p, E * 4));
-    CU(c, d2h(ho->d_attention_mask, c->hs_mask.p, E));
     CU(c, d2h(ho->d_grp_count, c->grp_count.p, n_slots * 4));
     CU(c, d2h(ho->d_grp_width, c->grp_width.p, n_slots * 4));
     CU(c, d2h(ho->d_grp_round, c->grp_round.p, n_slots * 4));
@@ -678,6 +738,8 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     CU(c, d2h(ho->d_left_ptr, c->left_ptr.p, (size_t)(R + 1) * 8));
     CU(c, d2h(ho->d_left_ids, c->left_out.p, (size_t)I.samples_left * 4));
     CU(c, cudaStreamSynchronize(st));
+    CU(c, cudaStreamSynchronize(c->d2h_stream));
+    CU(c, cudaStreamSynchronize(c->copy_stream));
     return ODB_OK;
 }
 

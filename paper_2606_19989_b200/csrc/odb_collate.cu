@@ -258,6 +258,7 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
             const int64_t chunk = tile * kWarps + warp;
             const int64_t a0 = chunk * kColChunk;
             if (a0 >= A.total_elems) break;
+            if (a0 + kColChunk <= A.elem_lo) continue;  // another launch's elements (odb_run_host pipelines ranks)
             const int4 *cp = reinterpret_cast<const int4 *>(A.chunks + chunk);
             const int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
             int64_t off_s = (int64_t)(((uint64_t)(uint32_t)c0.y << 32) | (uint32_t)c0.x);
@@ -370,6 +371,7 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
                 for (int k = 0; k < 4; ++k) {
                     const int64_t a = a0 + (int64_t)(k * 32 + lane) * 4;
                     if (a >= A.total_elems) break;
+                    if (a < A.elem_lo) continue;
                     bool moved = false;
                     while (a >= off_n) {
                         ++s;

@@ -95,8 +95,9 @@ struct CollateArgs {
     uint8_t *mask;
     int32_t *grp_valid;
     unsigned long long *tile_counter;  // work counter of the launch (zeroed before it)
-    int64_t total_elems;
-    int64_t tile_lo, tile_hi;  // tiles [tile_lo, tile_hi) are processed by this launch
+    int64_t total_elems;       // arena elements [elem_lo, total_elems) are written by this launch
+    int64_t elem_lo;
+    int64_t tile_lo, tile_hi;  // tiles [tile_lo, tile_hi) are visited by this launch
     int32_t pad_id, ignore_index, shift_labels;
 };
 
@@ -219,8 +220,11 @@ struct odb_ctx {
     odb::DevBuf<int32_t> hs_lengths, hs_tokens, hs_span_lo, hs_span_hi, hs_ids, hs_labels, hs_pos;
     odb::DevBuf<int64_t> hs_sample_ptr, hs_span_ptr;
     odb::DevBuf<uint8_t> hs_mask;
-    cudaStream_t copy_stream = nullptr;
+    cudaStream_t copy_stream = nullptr;  // host -> device
+    cudaStream_t d2h_stream = nullptr;   // device -> host
     cudaEvent_t copy_ev = nullptr;
+    std::vector<cudaEvent_t> tok_ev, col_ev;  // per rank: tokens landed / slots collated
+    int64_t *h_rank_off = nullptr;            // pinned, R+1: arena offset of each rank's first slot
 };
 
 namespace odb {

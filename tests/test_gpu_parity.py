@@ -223,27 +223,64 @@ def test_run_to_run_determinism(P):
         assert torch.equal(a.table(name), b.table(name))
 
 
-def test_run_host_end_to_end(P, oracle):
-    """odb_run_host: HOST buffers in, HOST buffers out (the e2e leg bench.py times)."""
+def _run_host_case(P, oracle, wl, ctx=None):
     import torch
-    wl = I.make_workload(1)
     plan, ref = oracle.run_workload(wl)
-    toks = torch.from_numpy(wl.tokens()).pin_memory()
-    pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
-    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+    toks_np = wl.tokens()
+    toks = torch.from_numpy(toks_np if len(toks_np) else np.zeros(1, np.int32)).pin_memory()
+    pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a) if len(a) else np.zeros(1, a.dtype)).to(dt).pin_memory()
+    own = ctx is None
+    ctx = ctx or P.Odb(Par.gpu_params(wl), max(wl.n_samples, 1))
+    try:
         out = P.OutputBuffers(wl.n_ranks, plan.total_elems, plan.n_slots, plan.samples_emitted, plan.n_steps,
                               plan.samples_left, "cpu", fill=Par.SENTINEL)
         info = P.odb_run_host(ctx.h, pin(wl.lengths, torch.int32), wl.rank_ptr, toks, pin(wl.sample_ptr, torch.int64),
                               pin(wl.span_ptr, torch.int64), pin(wl.span_lo, torch.int32), pin(wl.span_hi, torch.int32),
                               out.struct)
+    finally:
+        if own:
+            ctx.close()
     Par.compare_plan(plan, info, out)
     E = plan.total_elems
-    # the host copy is one flat memcpy of each arena, so gap bytes carry whatever the device staging
-    # held; compare blocks only
+    # each rank's slice of an arena is one flat memcpy, so gap bytes carry whatever the device
+    # staging held; compare blocks only
     inblk = np.zeros(E, dtype=bool)
     for s in range(plan.n_slots):
         o = int(plan.grp_offset[s])
         inblk[o:o + int(plan.grp_count[s]) * int(plan.grp_width[s])] = True
     for name in ("input_ids", "labels", "position_ids", "attention_mask"):
         assert np.array_equal(getattr(out, name)[:E].numpy()[inblk], ref[name][:E][inblk]), name
+        tail = getattr(out, name)[E:].numpy().view(np.uint8)
+        assert (tail == Par.SENTINEL).all(), name + ": wrote past total_elems"
     assert np.array_equal(out.table("grp_valid_tokens").numpy(), ref["grp_valid_tokens"])
+    assert np.array_equal(out.table("step_valid_tokens").numpy(), ref["step_valid_tokens"])
+
+
+@pytest.mark.parametrize("case", ["config2", "tiny", "tiny_maxfit", "unequal", "empty_rank", "overflow_nonjoin",
+                                  "config4_slice_nonjoin"])
+def test_run_host_end_to_end(P, oracle, case):
+    """odb_run_host: HOST buffers in, HOST buffers out (the e2e leg bench.py times).  Tokens go up
+    and results come back rank by rank, one collate launch per rank: rank boundaries fall inside
+    collate tiles and chunks, some ranks own no slot elements at all."""
+    if case == "config2":
+        wl = I.make_workload(1)
+    elif case == "tiny":
+        wl = I.make_workload(0)
+    elif case == "tiny_maxfit":
+        wl = I.make_workload(0, rule=1)
+    elif case == "overflow_nonjoin":
+        wl = I.protocol_workload("overflow_multiround", 1, join_mode=0)
+        wl.params["sample_quota"] = int(0.6 * wl.n_samples)
+    elif case == "config4_slice_nonjoin":
+        wl = I.make_workload(3, n_ranks=5, n_per_rank=700, join_mode=0)
+    else:
+        wl = I.protocol_workload(case, 2)
+    _run_host_case(P, oracle, wl)
+
+
+def test_run_host_reuses_context(P, oracle):
+    """Two odb_run_host calls on one context (staging buffers, events and counters are reused)."""
+    wl = I.make_workload(1, n_ranks=3, n_per_rank=300)
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        _run_host_case(P, oracle, wl, ctx)
+        _run_host_case(P, oracle, wl, ctx)
