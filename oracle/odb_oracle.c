@@ -50,6 +50,7 @@ static void ivec_push(ivec *a, int32_t x) {
 typedef struct {
     int32_t *ids;
     int32_t n;
+    int32_t orig; /* index of the candidate group (pre-alignment list) this group's samples came from */
 } group;
 
 typedef struct {
@@ -71,6 +72,7 @@ static void gvec_push(gvec *a, group x) { gvec_insert(a, a->n, x); }
 static group group_make(const int32_t *ids, int32_t n) {
     group g;
     g.n = n;
+    g.orig = -1;
     g.ids = (int32_t *)malloc((size_t)(n > 0 ? n : 1) * sizeof(int32_t));
     if (n > 0) memcpy(g.ids, ids, (size_t)n * sizeof(int32_t));
     return g;
@@ -82,6 +84,7 @@ typedef struct {
     int32_t count;
     int32_t width;
     int32_t round;
+    int32_t origin; /* step index of the first slot of this rank cut from the same candidate group */
 } slot;
 
 typedef struct {
@@ -182,7 +185,9 @@ static void align_split(gvec *G, int64_t T) {
         if (j < 0) break; /* no group with >= 2 samples (cannot happen when T <= S_r) */
         int32_t s = G->g[j].ids[G->g[j].n - 1];
         G->g[j].n -= 1;
-        gvec_insert(G, j + 1, group_make(&s, 1));
+        group single = group_make(&s, 1);
+        single.orig = G->g[j].orig; /* the singleton still belongs to its candidate group (loss scaling, App. B) */
+        gvec_insert(G, j + 1, single);
     }
 }
 
@@ -417,6 +422,7 @@ oracle_plan *oracle_plan_run(int32_t R, int64_t budget, int32_t rule, int32_t jo
             else
                 group_maxfit_asc(len_r, buf[r].v, (int32_t)buf[r].n, budget, &cand[r]);
             Gn[r] = cand[r].n; /* pre-alignment candidate count (U23) */
+            for (int64_t j = 0; j < cand[r].n; ++j) cand[r].g[j].orig = (int32_t)j;
         }
         /* Eq. 3 */
         int64_t T = oracle_target_groups(Gn, Sn, R, slot_capacity);
@@ -433,6 +439,7 @@ oracle_plan *oracle_plan_run(int32_t R, int64_t budget, int32_t rule, int32_t jo
         /* emit step k = 0..T-1 (U26); finished ranks emit IDLE slots (U14) */
         int quota_hit = 0;
         int64_t k_emit = T;
+        const int64_t step_base = p->step_samples.n; /* steps emitted by earlier rounds */
         for (int64_t k = 0; k < T; ++k) {
             int64_t e_k = 0;
             for (int32_t r = 0; r < R; ++r) {
@@ -442,8 +449,12 @@ oracle_plan *oracle_plan_run(int32_t R, int64_t budget, int32_t rule, int32_t jo
                     s.ids = (int32_t *)malloc(sizeof(int32_t));
                     s.count = 0;
                     s.width = 0;
+                    s.origin = (int32_t)(step_base + k);
                 } else {
                     group g = cand[r].g[k];
+                    int64_t k0 = 0;
+                    while (cand[r].g[k0].orig != g.orig) k0++; /* first aligned group cut from the same candidate */
+                    s.origin = (int32_t)(step_base + k0);
                     s.ids = g.ids; /* ownership moves to the slot */
                     s.count = g.n;
                     s.width = 0;
@@ -578,6 +589,56 @@ void oracle_plan_tables(const oracle_plan *p, int32_t *grp_count, int32_t *grp_w
     if (left_ptr) left_ptr[p->R] = lq;
     if (round_T)
         for (int64_t a = 0; a < p->round_T.n; ++a) round_T[a] = p->round_T.v[a];
+}
+
+/* per-slot origin (n_slots, rank-major): see `slot.origin` */
+void oracle_plan_origin(const oracle_plan *p, int32_t *grp_origin) {
+    for (int32_t r = 0; r < p->R; ++r)
+        for (int64_t k = 0; k < p->n_steps; ++k) grp_origin[(int64_t)r * p->n_steps + k] = p->slots[r].s[k].origin;
+}
+
+/*
+ * Loss-scaling weights w_{r,k} per slot (rank-major [R][n_steps]), fp64; DDP prescales rank r's mean loss
+ * of step k by W * w_{r,k} (section 2.3 "Loss scaling" P:60-65; App. B; the three modes P:738).
+ *   mode 1 sample-level:        w = n_{r,k} / N_k,           N_k = sum_r n_{r,k}            (P:65, P:738 (1))
+ *   mode 3 exact token-level:   w = t_{r,k} / T_tok,k,       T_tok,k = sum_r t_{r,k}        (Eq. 2)
+ *          with t = the POST-alignment valid-token count of the slot.
+ *   mode 2 approximate token-level: t_adj = n_adj * tbar, tbar = t_orig / n_orig of the PRE-alignment
+ *          candidate group the slot was cut from (P:283, P:738 (2); reading U27); w = t_adj / sum_r t_adj.
+ * A step whose denominator is 0 gets weight 0 on every rank.  Sums run over ranks in the order r = 0..R-1.
+ * count/valid/origin: the per-slot tables (origin = step index of the first slot cut from the same candidate).
+ */
+void oracle_loss_weights(int32_t mode, int32_t R, int64_t n_steps, const int32_t *count, const int32_t *valid,
+                         const int32_t *origin, double *w) {
+    for (int64_t k = 0; k < n_steps; ++k) {
+        double denom = 0.0;
+        for (int32_t r = 0; r < R; ++r) {
+            int64_t s = (int64_t)r * n_steps + k;
+            double num;
+            if (mode == 1) {
+                num = (double)count[s];
+            } else if (mode == 3) {
+                num = (double)valid[s];
+            } else {
+                int64_t t_orig = 0, n_orig = 0;
+                for (int64_t k2 = 0; k2 < n_steps; ++k2) { /* every slot of this rank cut from the same candidate */
+                    int64_t s2 = (int64_t)r * n_steps + k2;
+                    if (origin[s2] == origin[s]) {
+                        t_orig += valid[s2];
+                        n_orig += count[s2];
+                    }
+                }
+                double tbar = n_orig > 0 ? (double)t_orig / (double)n_orig : 0.0;
+                num = (double)count[s] * tbar;
+            }
+            w[s] = num;
+            denom = denom + num;
+        }
+        for (int32_t r = 0; r < R; ++r) {
+            int64_t s = (int64_t)r * n_steps + k;
+            w[s] = denom > 0.0 ? w[s] / denom : 0.0;
+        }
+    }
 }
 
 /* is token position t of a sample inside one of its masked spans [lo,hi)?  linear scan */

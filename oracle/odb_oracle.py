@@ -30,7 +30,7 @@ def build(force: bool = False) -> str:
     """Compile the oracle with gcc (-O2, single-threaded).  Returns the library path."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-std=c99", "-shared", "-fPIC", "-Wall", "-o", tmp, _SRC])
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-std=c99", "-shared", "-fPIC", "-Wall", "-o", tmp, _SRC])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -72,6 +72,10 @@ def lib():
         L.oracle_collate_all.restype = None
         L.oracle_collate_all.argtypes = [vp, pi32, pi64, pi64, pi32, pi32, i32, i32, i32, pi32, pu8, pi32, pi32,
                                          pi32, pi64]
+        L.oracle_plan_origin.restype = None
+        L.oracle_plan_origin.argtypes = [vp, pi32]
+        L.oracle_loss_weights.restype = None
+        L.oracle_loss_weights.argtypes = [i32, i32, i64, pi32, pi32, pi32, ctypes.POINTER(ctypes.c_double)]
         _lib = L
     return _lib
 
@@ -123,6 +127,22 @@ def target_group_size(budget: int, l: int) -> int:
     return int(lib().oracle_target_group_size(int(budget), int(l)))
 
 
+SCALE_SAMPLE = 1
+SCALE_TOKEN_APPROX = 2
+SCALE_TOKEN_EXACT = 3
+
+
+def loss_weights(mode: int, R: int, n_steps: int, count, valid, origin) -> np.ndarray:
+    """w[r, k] (fp64) of the three loss-scaling modes; tables are rank-major."""
+    count = np.ascontiguousarray(count, dtype=np.int32)
+    valid = np.ascontiguousarray(valid, dtype=np.int32)
+    origin = np.ascontiguousarray(origin, dtype=np.int32)
+    w = np.zeros(max(R * n_steps, 1), dtype=np.float64)
+    lib().oracle_loss_weights(int(mode), int(R), int(n_steps), _p(count, ctypes.c_int32), _p(valid, ctypes.c_int32),
+                              _p(origin, ctypes.c_int32), w.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    return w[:R * n_steps].reshape(R, n_steps)
+
+
 # ---------------------------------------------------------------------------------------
 # whole plan / collation
 # ---------------------------------------------------------------------------------------
@@ -163,13 +183,15 @@ class OraclePlan:
         self.left_ptr = np.zeros(self.R + 1, np.int64)
         self.left_ids = np.zeros(max(self.samples_left, 1), np.int32)
         self.round_T = np.zeros(max(n_emit_rounds, 1), np.int32)
+        self.grp_origin = np.zeros(ns, np.int32)
+        lib().oracle_plan_origin(self._h, _p(self.grp_origin, ctypes.c_int32))
         i32, i64 = ctypes.c_int32, ctypes.c_int64
         lib().oracle_plan_tables(self._h, _p(self.grp_count, i32), _p(self.grp_width, i32), _p(self.grp_round, i32),
                                  _p(self.grp_offset, i64), _p(self.grp_real_tokens, i32),
                                  _p(self.grp_sample_ptr, i64), _p(self.grp_sample_ids, i32),
                                  _p(self.step_samples, i32), _p(self.left_ptr, i64), _p(self.left_ids, i32),
                                  _p(self.round_T, i32))
-        for name in ("grp_count", "grp_width", "grp_round", "grp_offset", "grp_real_tokens"):
+        for name in ("grp_count", "grp_width", "grp_round", "grp_offset", "grp_real_tokens", "grp_origin"):
             setattr(self, name, getattr(self, name)[:self.n_slots])
         self.grp_sample_ids = self.grp_sample_ids[:self.samples_emitted]
         self.step_samples = self.step_samples[:self.n_steps]
