@@ -67,6 +67,11 @@ enum {
     ODB_RULE_THRESHOLD = 0, /* paper section 2.2: threshold carry-over greedy (default) */
     ODB_RULE_MAXFIT_ASC = 1 /* App. I: longest ascending run with count*max_len <= budget */
 };
+enum { /* loss-scaling modes (section 2.3; App. B) */
+    ODB_SCALE_SAMPLE = 1,       /* w = n_{r,k} / N_k */
+    ODB_SCALE_TOKEN_APPROX = 2, /* w from t_adj = n_adj * (t_orig / n_orig) of the slot's candidate group */
+    ODB_SCALE_TOKEN_EXACT = 3   /* Eq. 2: w = t_{r,k} / T_tok,k from post-alignment valid-token counts (default) */
+};
 enum {
     ODB_STOP_ALL_FINISHED = 0, /* join: every rank drained (Thm 1) */
     ODB_STOP_LOGICAL = 1,      /* non-join: some rank advertised "finished" */
@@ -112,6 +117,8 @@ typedef struct { /* device outputs, caller-allocated; any table pointer may be N
     int32_t *d_grp_round;
     int32_t *d_grp_valid_tokens; /* #{labels != ignore_index} in the slot (Eq. 2's t_{r,k}) */
     int32_t *d_grp_real_tokens;  /* sum of the slot's sample lengths */
+    int32_t *d_grp_origin;       /* step index of the first slot of the same rank cut from the same pre-alignment
+                                    candidate group (== own step unless the slot is a split singleton; App. B) */
     int64_t *d_grp_offset;
     int64_t *d_grp_sample_ptr;
     int64_t slot_capacity_alloc; /* slots available in the per-slot tables */
@@ -173,6 +180,15 @@ ODB_API int odb_run(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_ran
 ODB_API int odb_run_host(odb_ctx *ctx, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
                  const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
                  const int32_t *h_span_hi, const odb_outputs *h_out_bufs, odb_plan_info *h_out, void *stream);
+
+/* Loss-scaling weights (section 2.3 "Loss scaling", Eq. 2; modes P:738): d_weights[r * n_steps + k]
+ * = w_{r,k} in fp64, one per slot; rank r prescales its mean loss of step k by W * w_{r,k} so that DDP's
+ * average equals the per-token reference loss (Eq. 2).  Every quotient, product and sum is one IEEE fp64
+ * operation, sums over ranks run in the order r = 0..R-1, a step whose denominator is 0 gets weight 0:
+ * results are bit-identical to the CPU oracle.  Requires a completed odb_collate / odb_run on this
+ * context (valid-token counts; ODB_ERR_STATE otherwise).  d_weights: device, n_slots doubles, caller-owned.
+ * Asynchronous on `stream`. */
+ODB_API int odb_loss_weights(odb_ctx *ctx, int mode, double *d_weights, void *stream);
 
 /* Device times of the last odb_run / odb_collate on this context, in milliseconds, measured with
  * CUDA events on the launching stream: ms[0] = planning (all rounds, plan query, row descriptors and

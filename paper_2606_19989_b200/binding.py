@@ -45,7 +45,7 @@ class odb_outputs(ctypes.Structure):
     _fields_ = [("d_input_ids", _vp), ("d_labels", _vp), ("d_position_ids", _vp), ("d_attention_mask", _vp),
                 ("arena_capacity", _i64),
                 ("d_grp_count", _vp), ("d_grp_width", _vp), ("d_grp_round", _vp), ("d_grp_valid_tokens", _vp),
-                ("d_grp_real_tokens", _vp), ("d_grp_offset", _vp), ("d_grp_sample_ptr", _vp),
+                ("d_grp_real_tokens", _vp), ("d_grp_origin", _vp), ("d_grp_offset", _vp), ("d_grp_sample_ptr", _vp),
                 ("slot_capacity_alloc", _i64),
                 ("d_grp_sample_ids", _vp), ("ids_capacity", _i64),
                 ("d_step_samples", _vp), ("d_step_valid_tokens", _vp), ("step_capacity_alloc", _i64),
@@ -81,6 +81,7 @@ SYMBOLS = {
     "odb_collate": (_i32, [_vp, _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _vp]),
     "odb_run": (_i32, [_vp, _vp, _P(_i64), _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _P(odb_plan_info), _vp]),
     "odb_run_host": (_i32, [_vp, _vp, _P(_i64), _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _P(odb_plan_info), _vp]),
+    "odb_loss_weights": (_i32, [_vp, _i32, _vp, _vp]),
     "odb_set_timing": (_i32, [_vp, _i32]),
     "odb_get_timing": (_i32, [_vp, _P(ctypes.c_float)]),
     "odb_kernel_launches": (_i64, [_vp]),
@@ -242,6 +243,14 @@ def odb_run_host(ctx: int, h_lengths, h_rank_ptr, h_tokens, h_sample_ptr, h_span
     return info
 
 
+ODB_SCALE_SAMPLE, ODB_SCALE_TOKEN_APPROX, ODB_SCALE_TOKEN_EXACT = 1, 2, 3
+
+
+def odb_loss_weights(ctx: int, mode: int, d_weights, stream=None) -> None:
+    """w[r * n_steps + k] (fp64, device) of loss-scaling ``mode`` for the plan last collated on ``ctx``."""
+    _check(load().odb_loss_weights(ctx, int(mode), _ptr(d_weights), _stream(stream)), "odb_loss_weights", ctx)
+
+
 def odb_set_timing(ctx: int, enable: bool) -> None:
     _check(load().odb_set_timing(ctx, 1 if enable else 0), "odb_set_timing", ctx)
 
@@ -276,7 +285,8 @@ odb_status_string = status_string
 # ---- memory plumbing (torch allocations only; no arithmetic) ---------------------------------
 _TABLES = (  # name, torch dtype name, size key
     ("grp_count", "int32", "slots"), ("grp_width", "int32", "slots"), ("grp_round", "int32", "slots"),
-    ("grp_valid_tokens", "int32", "slots"), ("grp_real_tokens", "int32", "slots"), ("grp_offset", "int64", "slots"),
+    ("grp_valid_tokens", "int32", "slots"), ("grp_real_tokens", "int32", "slots"), ("grp_origin", "int32", "slots"),
+    ("grp_offset", "int64", "slots"),
     ("grp_sample_ptr", "int64", "slots1"), ("grp_sample_ids", "int32", "ids"),
     ("step_samples", "int32", "steps"), ("step_valid_tokens", "int64", "steps"),
     ("left_ptr", "int64", "ranks1"), ("left_ids", "int32", "left"),

@@ -66,6 +66,7 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->agpos);
     cudaFree(c->agcnt);
     cudaFree(c->agoff);
+    cudaFree(c->agorg);
     cudaFree(c->left_ids);
     cudaFree(c->emit_ids);
     cudaFree(c->n_left);
@@ -82,12 +83,14 @@ static void free_all(odb_ctx *c) {
     c->st_width.release();
     c->st_real.release();
     c->st_round.release();
+    c->st_origin.release();
     c->step_samples.release();
     c->grp_count.release();
     c->grp_width.release();
     c->grp_round.release();
     c->grp_valid.release();
     c->grp_real.release();
+    c->grp_origin.release();
     c->scan_state.release();
     c->grp_offset.release();
     c->grp_sample_ptr.release();
@@ -173,6 +176,7 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->agpos, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->agcnt, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->agoff, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->agorg, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->left_ids, N);
     if (e == cudaSuccess) e = dev_alloc(&c->emit_ids, N);
     if (e == cudaSuccess) e = dev_alloc(&c->n_left, R);
@@ -217,6 +221,7 @@ int odb_reset(odb_ctx *c) {
     c->last_T = 0;
     c->stop_reason = 0;
     c->info_valid = false;
+    c->collated = false;
     c->d_lengths = nullptr;
     c->ev_valid = false;
     return ODB_OK;
@@ -314,6 +319,7 @@ int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_
         CU(c, grow_preserve(c->st_width, (size_t)want * R, used, st));
         CU(c, grow_preserve(c->st_real, (size_t)want * R, used, st));
         CU(c, grow_preserve(c->st_round, (size_t)want * R, used, st));
+        CU(c, grow_preserve(c->st_origin, (size_t)want * R, used, st));
         CU(c, grow_preserve(c->step_samples, (size_t)want, (size_t)c->n_steps, st));
         c->step_cap = want;
     }
@@ -397,6 +403,7 @@ int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
     CU(c, c->grp_round.ensure(n_slots + 1));
     CU(c, c->grp_valid.ensure(n_slots + 1));
     CU(c, c->grp_real.ensure(n_slots + 1));
+    CU(c, c->grp_origin.ensure(n_slots + 1));
     CU(c, c->grp_offset.ensure(n_slots + 1));
     CU(c, c->grp_sample_ptr.ensure(n_slots + 1));
     CU(c, c->grp_sample_ids.ensure((size_t)c->n_total + 1));
@@ -430,7 +437,7 @@ static int check_capacity(const odb_ctx *c, const odb_outputs *o) {
         if (o->arena_capacity < I.total_elems) return ODB_ERR_CAPACITY;
     }
     const bool any_slot_tab = o->d_grp_count || o->d_grp_width || o->d_grp_round || o->d_grp_valid_tokens ||
-                              o->d_grp_real_tokens || o->d_grp_offset || o->d_grp_sample_ptr;
+                              o->d_grp_real_tokens || o->d_grp_origin || o->d_grp_offset || o->d_grp_sample_ptr;
     if (any_slot_tab && o->slot_capacity_alloc < I.n_slots) return ODB_ERR_CAPACITY;
     if (o->d_grp_sample_ids && o->ids_capacity < I.samples_emitted) return ODB_ERR_CAPACITY;
     if ((o->d_step_samples || o->d_step_valid_tokens) && o->step_capacity_alloc < I.n_steps) return ODB_ERR_CAPACITY;
@@ -515,6 +522,7 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
         job(o->d_grp_round, c->grp_round.p, n_slots, 4);
         job(o->d_grp_valid_tokens, c->grp_valid.p, n_slots, 4);
         job(o->d_grp_real_tokens, c->grp_real.p, n_slots, 4);
+        job(o->d_grp_origin, c->grp_origin.p, n_slots, 4);
         job(o->d_grp_offset, c->grp_offset.p, n_slots, 8);
         job(o->d_grp_sample_ptr, c->grp_sample_ptr.p, n_slots + 1, 8);
         job(o->d_grp_sample_ids, c->grp_sample_ids.p, (size_t)I.samples_emitted, 4);
@@ -527,6 +535,7 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
         CU(c, cudaEventRecord(c->ev[3], st));
         c->ev_valid = true;
     }
+    c->collated = true;
     return ODB_OK;
 }
 
@@ -642,7 +651,7 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     const odb_plan_info I = *h_out;
     {  // host capacities
         const bool any_slot_tab = ho->d_grp_count || ho->d_grp_width || ho->d_grp_round || ho->d_grp_valid_tokens ||
-                                  ho->d_grp_real_tokens || ho->d_grp_offset || ho->d_grp_sample_ptr;
+                                  ho->d_grp_real_tokens || ho->d_grp_origin || ho->d_grp_offset || ho->d_grp_sample_ptr;
         if (I.total_elems > 0 && (!ho->d_input_ids || !ho->d_labels || !ho->d_position_ids || !ho->d_attention_mask))
             rc = ODB_ERR_INVALID_ARG;
         else if (I.total_elems > ho->arena_capacity)
@@ -720,6 +729,7 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
         CU(c, launch_post(c, P, st));
     }
     if (c->timing) CU(c, cudaEventRecord(c->ev[3], st));
+    c->collated = true;
     // tables device -> host (small) on the compute stream
     auto d2h = [&](void *dst, const void *src, size_t bytes) -> cudaError_t {
         if (!dst || bytes == 0) return cudaSuccess;
@@ -730,6 +740,7 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     CU(c, d2h(ho->d_grp_round, c->grp_round.p, n_slots * 4));
     CU(c, d2h(ho->d_grp_valid_tokens, c->grp_valid.p, n_slots * 4));
     CU(c, d2h(ho->d_grp_real_tokens, c->grp_real.p, n_slots * 4));
+    CU(c, d2h(ho->d_grp_origin, c->grp_origin.p, n_slots * 4));
     CU(c, d2h(ho->d_grp_offset, c->grp_offset.p, n_slots * 8));
     CU(c, d2h(ho->d_grp_sample_ptr, c->grp_sample_ptr.p, (n_slots + 1) * 8));
     CU(c, d2h(ho->d_grp_sample_ids, c->grp_sample_ids.p, (size_t)I.samples_emitted * 4));
@@ -740,6 +751,17 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     CU(c, cudaStreamSynchronize(st));
     CU(c, cudaStreamSynchronize(c->d2h_stream));
     CU(c, cudaStreamSynchronize(c->copy_stream));
+    return ODB_OK;
+}
+
+int odb_loss_weights(odb_ctx *c, int mode, double *d_weights, void *stream) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (mode != ODB_SCALE_SAMPLE && mode != ODB_SCALE_TOKEN_APPROX && mode != ODB_SCALE_TOKEN_EXACT)
+        return ODB_ERR_INVALID_ARG;
+    if (c->state != 5 || !c->collated) return ODB_ERR_STATE;
+    if (c->info.n_slots > 0 && !d_weights) return ODB_ERR_INVALID_ARG;
+    CU(c, cudaSetDevice(c->device));
+    CU(c, launch_loss_weights(c, mode, d_weights, (cudaStream_t)stream));
     return ODB_OK;
 }
 

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "odb.h"
@@ -108,7 +109,7 @@ struct CopyJob {
     int64_t words;
 };
 struct PostArgs {
-    CopyJob job[12];
+    CopyJob job[16];
     int n_jobs;
     int R, n_steps;
     const int32_t *grp_valid;
@@ -193,7 +194,7 @@ struct odb_ctx {
     uint8_t *posflag = nullptr;         // n_max
     int32_t *emit_pos = nullptr;        // n_max: index in the rank's emit region, -1 = not emitted
     int32_t *gpos = nullptr;            // n_max + R
-    int32_t *agpos = nullptr, *agcnt = nullptr, *agoff = nullptr;  // n_max + R
+    int32_t *agpos = nullptr, *agcnt = nullptr, *agoff = nullptr, *agorg = nullptr;  // n_max + R
     int32_t *left_ids = nullptr, *emit_ids = nullptr;              // n_max
     int32_t *n_left = nullptr, *fetch_pos = nullptr, *emit_cur = nullptr, *G = nullptr, *S = nullptr;  // R
     odb::RoundRec *d_rec = nullptr;
@@ -203,11 +204,12 @@ struct odb_ctx {
     unsigned long long *d_tile_counter = nullptr;
 
     // step-major staging tables [step * R + r], growable
-    odb::DevBuf<int32_t> st_count, st_width, st_real, st_round, step_samples;
+    odb::DevBuf<int32_t> st_count, st_width, st_real, st_round, st_origin, step_samples;
     int64_t step_cap = 0;
 
     // rank-major plan tables built by odb_plan_query
-    odb::DevBuf<int32_t> grp_count, grp_width, grp_round, grp_valid, grp_real;
+    odb::DevBuf<int32_t> grp_count, grp_width, grp_round, grp_valid, grp_real, grp_origin;
+    bool collated = false;  // grp_valid holds the counts of a completed collate
     odb::DevBuf<unsigned char> scan_state;
     odb::DevBuf<int64_t> grp_offset, grp_sample_ptr;
     odb::DevBuf<int32_t> grp_sample_ids, left_out;
@@ -239,4 +241,6 @@ cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64
 cudaError_t launch_chunk_table(odb_ctx *c, cudaStream_t st);
 cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st);
 cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st);
+// ---- odb_scale.cu ------------------------------------------------------------------------------
+cudaError_t launch_loss_weights(odb_ctx *c, int mode, double *d_weights, cudaStream_t st);
 }  // namespace odb

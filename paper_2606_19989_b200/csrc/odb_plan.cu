@@ -355,7 +355,7 @@ k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ ran
 __global__ void __launch_bounds__(kRankThreads)
 k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr, const int32_t *__restrict__ G_arr, int R,
         int slot_capacity, const int32_t *__restrict__ gpos, int32_t *__restrict__ agpos, int32_t *__restrict__ agcnt,
-        uint64_t *ovf, int32_t *step_samples, int step_base, RoundRec *rec) {
+        int32_t *__restrict__ agorg, uint64_t *ovf, int32_t *step_samples, int step_base, RoundRec *rec) {
     extern __shared__ __align__(16) unsigned char al_smem[];
     __shared__ int s_maxG, s_minS;
     const int r = blockIdx.x;
@@ -384,7 +384,7 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
     const int64_t base = rank_ptr[r];
     const int64_t jb = base + r;
     const int32_t *gp = gpos + jb;
-    int32_t *ap = agpos + jb, *ac = agcnt + jb;
+    int32_t *ap = agpos + jb, *ac = agcnt + jb, *ag = agorg + jb;  // ag: list index of the candidate's head
     if (Gr <= T) {
         const int d = T - Gr;
         const int lane = threadIdx.x & 31;
@@ -401,6 +401,7 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
                 const int c = pn - p - kj;
                 ap[h] = p;
                 ac[h] = c;
+                ag[h] = h;
                 atomicAdd(&step_samples[step_base + h], c);
             }
             uint32_t sp = __ballot_sync(ODB_FULL_MASK, kj > 0);
@@ -413,6 +414,7 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
                 for (int i = lane; i < kk; i += 32) {
                     ap[hh + 1 + i] = pe - kk + i;
                     ac[hh + 1 + i] = 1;
+                    ag[hh + 1 + i] = hh;  // cut from the candidate group whose head sits at hh
                     atomicAdd(&step_samples[step_base + hh + 1 + i], 1);
                 }
             }
@@ -433,6 +435,7 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
             int p = gp[j], c = gp[j + 1] - p;
             ap[k] = p;
             ac[k] = c;
+            ag[k] = k;
             atomicAdd(&step_samples[step_base + k], c);
         }
     }
@@ -447,9 +450,10 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
 __global__ void __launch_bounds__(kRankThreads)
 k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
          const int32_t *__restrict__ G_arr, int R, const int32_t *__restrict__ agpos, const int32_t *__restrict__ agcnt,
-         int32_t *__restrict__ agoff, const int32_t *__restrict__ step_samples, int step_base, int round, int join_mode,
+         const int32_t *__restrict__ agorg, int32_t *__restrict__ agoff, const int32_t *__restrict__ step_samples, int step_base, int round, int join_mode,
          long long quota, long long emitted_before, int32_t *__restrict__ st_count, int32_t *__restrict__ st_width,
-         int32_t *__restrict__ st_real, int32_t *__restrict__ st_round, uint8_t *__restrict__ posflag,
+         int32_t *__restrict__ st_real, int32_t *__restrict__ st_round, int32_t *__restrict__ st_origin,
+         uint8_t *__restrict__ posflag,
          int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
          int32_t *fetch_pos, int32_t *emit_cur, RoundRec *rec) {
     __shared__ int s_scan[34];
@@ -500,6 +504,7 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
             st_width[idx] = 0;
             st_real[idx] = 0;
             st_round[idx] = round;
+            st_origin[idx] = step_base + k;
         }
         if (threadIdx.x == 0) atomicAdd(&rec->n_finished, 1);
         return;
@@ -526,6 +531,7 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
             st_count[idx] = c;
             st_width[idx] = (int32_t)key_len(k_[p + c - 1]);  // rows ascending: the last row is the longest
             st_round[idx] = round;
+            st_origin[idx] = step_base + agorg[jb + k];
             ao[k] = cur + ex;
         }
         carry += tot;
@@ -586,8 +592,9 @@ __device__ __forceinline__ void st_flag(int *p, int v) {
 
 __global__ void __launch_bounds__(kFinThreads)
 k_fin_scan(int R, int n_steps, const int32_t *__restrict__ st_count, const int32_t *__restrict__ st_width,
-           const int32_t *__restrict__ st_real, const int32_t *__restrict__ st_round, int32_t *__restrict__ grp_count,
-           int32_t *__restrict__ grp_width, int32_t *__restrict__ grp_round, int32_t *__restrict__ grp_real,
+           const int32_t *__restrict__ st_real, const int32_t *__restrict__ st_round,
+           const int32_t *__restrict__ st_origin, int32_t *__restrict__ grp_count, int32_t *__restrict__ grp_width,
+           int32_t *__restrict__ grp_round, int32_t *__restrict__ grp_real, int32_t *__restrict__ grp_origin,
            int64_t *__restrict__ grp_offset, int64_t *__restrict__ grp_sample_ptr, ScanTile *tiles, unsigned int *ticket,
            PlanTotals *tot) {
     __shared__ long long s_scan64[34];
@@ -615,6 +622,7 @@ k_fin_scan(int R, int n_steps, const int32_t *__restrict__ st_count, const int32
             grp_width[s] = (int32_t)w;
             grp_real[s] = (int32_t)re;
             grp_round[s] = st_round[src];
+            grp_origin[s] = st_origin[src];
         }
         const long long area = c * w;
         v[0][i] = (area + 15) / 16 * 16;
@@ -844,13 +852,13 @@ cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st) {
         c->attr_align = true;
     }
     k_align<<<R, kRankThreads, al_smem, st>>>(c->d_rank_ptr, c->S, c->G, R, c->prm.slot_capacity, c->gpos, c->agpos,
-                                              c->agcnt, c->ovf, c->step_samples.p, c->n_steps, c->d_rec);
+                                              c->agcnt, c->agorg, c->ovf, c->step_samples.p, c->n_steps, c->d_rec);
     ODB_LAUNCH_CHECK(c);
-    k_commit<<<R, kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, c->G, R, c->agpos, c->agcnt, c->agoff,
+    k_commit<<<R, kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, c->G, R, c->agpos, c->agcnt, c->agorg, c->agoff,
                                          c->step_samples.p, c->n_steps, c->round, c->prm.join_mode,
                                          (long long)c->prm.sample_quota,
                                          (long long)c->prm.emitted_so_far + (long long)c->samples_emitted, c->st_count.p,
-                                         c->st_width.p, c->st_real.p, c->st_round.p, c->posflag, c->emit_ids, c->emit_pos,
+                                         c->st_width.p, c->st_real.p, c->st_round.p, c->st_origin.p, c->posflag, c->emit_ids, c->emit_pos,
                                          c->left_ids, c->n_left, c->fetch_pos, c->emit_cur, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
@@ -866,8 +874,8 @@ cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st) {
     e = cudaMemsetAsync(c->scan_state.p, 0, (size_t)n_tiles * sizeof(ScanTile) + 64, st);
     if (e != cudaSuccess) return e;
     k_fin_scan<<<(int)n_tiles, kFinThreads, 0, st>>>(R, c->n_steps, c->st_count.p, c->st_width.p, c->st_real.p,
-                                                    c->st_round.p, c->grp_count.p, c->grp_width.p, c->grp_round.p,
-                                                    c->grp_real.p, c->grp_offset.p, c->grp_sample_ptr.p,
+                                                    c->st_round.p, c->st_origin.p, c->grp_count.p, c->grp_width.p,
+                                                    c->grp_round.p, c->grp_real.p, c->grp_origin.p, c->grp_offset.p, c->grp_sample_ptr.p,
                                                     reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
                                                     reinterpret_cast<unsigned int *>(c->scan_state.p), c->d_tot);
     ODB_LAUNCH_CHECK(c);

@@ -9,7 +9,7 @@ import odb_inputs as I
 SENTINEL = 0x5A
 PLAN_SCALARS = ("n_rounds", "n_steps", "stop_reason", "n_slots", "total_elems", "samples_emitted", "samples_left",
                 "real_tokens", "padded_elems")
-SLOT_TABLES = ("grp_count", "grp_width", "grp_round", "grp_offset", "grp_real_tokens", "grp_sample_ptr")
+SLOT_TABLES = ("grp_count", "grp_width", "grp_round", "grp_offset", "grp_real_tokens", "grp_origin", "grp_sample_ptr")
 
 
 class DeviceWorkload:

@@ -284,3 +284,46 @@ def test_run_host_reuses_context(P, oracle):
     with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
         _run_host_case(P, oracle, wl, ctx)
         _run_host_case(P, oracle, wl, ctx)
+
+
+# ---- loss-scaling weights --------------------------------------------------
+@pytest.mark.parametrize("case", ["tiny", "config2", "unequal", "empty_rank", "overflow_multiround",
+                                  "config4_slice_nonjoin", "heavy_split"])
+def test_loss_weights_bit_exact(P, oracle, case):
+    """odb_loss_weights vs the oracle, all three modes (Eq. 2; App. B).
+    Tolerance: ZERO ulps in fp64 -- both sides perform the same sequence of single correctly rounded
+    IEEE operations (int -> double conversions are exact below 2^53, one division for tbar, one
+    product, a left-to-right sum over ranks, one division; no FMA contraction on either side)."""
+    import torch
+    if case == "tiny":
+        wl = I.make_workload(0)
+    elif case == "config2":
+        wl = I.make_workload(1)
+    elif case == "config4_slice_nonjoin":
+        wl = I.make_workload(3, n_ranks=5, n_per_rank=700, join_mode=0)
+    elif case == "heavy_split":
+        rng = np.random.default_rng(11)
+        wl = I.custom_workload("heavy_split", [rng.integers(8, 64, size=40), rng.integers(900, 1000, size=300),
+                                               rng.integers(8, 2000, size=200)], seed=5, budget=4096)
+    else:
+        wl = I.protocol_workload(case, 6)
+    plan, ref = oracle.run_workload(wl)
+    dw = Par.DeviceWorkload(wl)
+    R, K = wl.n_ranks, plan.n_steps
+    with P.Odb(Par.gpu_params(wl), max(wl.n_samples, 1)) as ctx:
+        info = ctx.plan(dw.lengths, wl.rank_ptr)
+        out = P.OutputBuffers.for_plan(R, info, dw.device)
+        w = torch.full((max(R * K, 1),), float("nan"), dtype=torch.float64, device=dw.device)
+        with pytest.raises(P.OdbError):  # no collate yet: no valid-token counts
+            P.odb_loss_weights(ctx.h, P.ODB_SCALE_TOKEN_EXACT, w)
+        P.odb_collate(ctx.h, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out.struct)
+        assert np.array_equal(out.table("grp_origin").cpu().numpy(), plan.grp_origin)
+        for mode in (P.ODB_SCALE_SAMPLE, P.ODB_SCALE_TOKEN_APPROX, P.ODB_SCALE_TOKEN_EXACT):
+            w.fill_(float("nan"))
+            P.odb_loss_weights(ctx.h, mode, w)
+            torch.cuda.synchronize()
+            want = oracle.loss_weights(mode, R, K, plan.grp_count, ref["grp_valid_tokens"], plan.grp_origin)
+            got = w[:R * K].cpu().numpy().reshape(R, K)
+            assert np.array_equal(got.view(np.uint64), want.view(np.uint64)), (case, mode, np.abs(got - want).max())
+        with pytest.raises(P.OdbError):
+            P.odb_loss_weights(ctx.h, 7, w)
