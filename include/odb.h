@@ -190,6 +190,51 @@ ODB_API int odb_run_host(odb_ctx *ctx, const int32_t *h_lengths, const int64_t *
  * Asynchronous on `stream`. */
 ODB_API int odb_loss_weights(odb_ctx *ctx, int mode, double *d_weights, void *stream);
 
+/* The two halves of odb_loss_weights, for a job whose ranks live in several processes: numerators of
+ * the local slots (d_num: n_slots doubles); after the caller has gathered the numerators of all ranks
+ * into d_num_world (rank-major [world_ranks][n_steps]; rows [rank_offset, rank_offset + n_ranks) are this
+ * context's), odb_loss_normalize sums each step's column in the order r = 0..world_ranks-1 and writes the
+ * local weights (d_weights may alias the local rows of d_num_world). */
+ODB_API int odb_loss_numerators(odb_ctx *ctx, int mode, double *d_num, void *stream);
+ODB_API int odb_loss_normalize(odb_ctx *ctx, const double *d_num_world, int32_t world_ranks, int32_t rank_offset,
+                               double *d_weights, void *stream);
+
+/* ---- ranks spread over several processes / GPUs -------------------------------
+ * The paper runs one rank per process and exchanges, once per round, every rank's status and group
+ * counts with ONE unconditional all_gather (section 2.3; message layout P:250; deadlock-freedom
+ * Lemma 3), then evaluates Eq. 3 and the termination predicates on that shared tensor.  Here a
+ * context holds n_ranks consecutive ranks of a job of world_ranks ranks (equal n_ranks in every
+ * process); the library never communicates: it exposes the device buffers, the CALLER runs the
+ * collectives (torch.distributed over NCCL / NVLink) between the calls:
+ *
+ *   odb_dist_config(ctx, world_ranks, rank_offset, world_max_window)      once per run (resets the ctx)
+ *   per round:
+ *     odb_form_groups(...)         local windows, groups; packs (G_r, S_r) pairs into d_summary_local
+ *     all_gather(d_summary_world <- d_summary_local)                       [collective 1, 8 bytes per rank]
+ *     odb_align(...)               Eq. 3 and the termination predicates from d_summary_world; split / overflow
+ *     all_reduce(SUM, d_step_samples_round[0 .. step_window))              [collective 2, global e_k, P:347]
+ *     odb_commit(...)              quota cut on the global totals, staging tables, leftovers
+ *     odb_round_status(...)        identical on every process
+ *   odb_plan_query / odb_collate   local slots only
+ *   all_reduce(SUM, the caller's out->d_step_valid_tokens[0 .. n_steps))   [Eq. 2's T_tok per step]
+ *
+ * world_max_window = max over ALL ranks of the job of min(n_r, buffer_size or n_r): bounds T_grp of a
+ * round (a process whose ranks are all finished still emits T IDLE slots).  odb_plan_info then counts
+ * the local ranks only, except n_rounds / n_steps / stop_reason, which are global.  In this mode
+ * odb_run / odb_run_host return ODB_ERR_STATE. */
+typedef struct {
+    int32_t *d_summary_local;      /* 2 * n_ranks int32: (G_r, S_r) per local rank */
+    int32_t *d_summary_world;      /* 2 * world_ranks int32 */
+    int32_t summary_local_count, summary_world_count;
+    int32_t *d_step_samples_round; /* valid between odb_form_groups and odb_commit of a round */
+    int32_t step_window;
+    int32_t reserved;
+} odb_dist_bufs;
+ODB_API int odb_dist_config(odb_ctx *ctx, int32_t world_ranks, int32_t rank_offset, int32_t world_max_window);
+ODB_API int odb_dist_buffers(odb_ctx *ctx, odb_dist_bufs *out);
+/* Distributed mode only (ODB_ERR_STATE otherwise): second half of odb_align, after collective 2. */
+ODB_API int odb_commit(odb_ctx *ctx, void *stream);
+
 /* Device times of the last odb_run / odb_collate on this context, in milliseconds, measured with
  * CUDA events on the launching stream: ms[0] = planning (all rounds, plan query, row descriptors and
  * the tile table), ms[1] = the collate kernel alone, ms[2] = what follows it (step totals, table

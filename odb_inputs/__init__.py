@@ -18,4 +18,5 @@ from .gen import (  # noqa: F401
     token_ids,
     tokens_for_samples,
     describe,
+    split_ranks,
 )

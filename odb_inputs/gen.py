@@ -68,7 +68,7 @@ def tokens_for_samples(wl: "Workload", global_sample_ids: Sequence[int]):
         off[1:] = np.cumsum(lens)[:-1]
     toks = np.empty(int(lens.sum()), dtype=np.int32)
     for k, g in enumerate(ids):
-        toks[off[k]: off[k] + lens[k]] = token_ids(wl.token_seed, int(wl.sample_ptr[g]), int(lens[k]))
+        toks[off[k]: off[k] + lens[k]] = token_ids(wl.token_seed, wl.token_start + int(wl.sample_ptr[g]), int(lens[k]))
     return toks, off
 
 
@@ -87,6 +87,7 @@ class Workload:
     span_hi: np.ndarray       # int32
     token_seed: int
     params: Dict[str, int] = field(default_factory=dict)
+    token_start: int = 0      # global ragged-buffer index of this workload's first token (split_ranks)
 
     @property
     def n_samples(self) -> int:
@@ -98,7 +99,7 @@ class Workload:
 
     def tokens(self) -> np.ndarray:
         """Full ragged int32 token buffer (only call when it fits in host RAM)."""
-        return token_ids(self.token_seed, 0, self.n_tokens)
+        return token_ids(self.token_seed, self.token_start, self.n_tokens)
 
 
 _DEFAULT_PARAMS = dict(
@@ -332,6 +333,25 @@ def custom_workload(name: str, per_rank_lengths, seed: int = 0, **params) -> Wor
     per = [np.asarray(x, dtype=np.int64) for x in per_rank_lengths]
     spans = [_prompt_only(rng, p) for p in per]
     return _assemble(name, per, spans, 9000 + seed, params)
+
+
+def split_ranks(wl: Workload, n_parts: int):
+    """The same job held by ``n_parts`` processes: part p gets the consecutive ranks
+    [p*R/n_parts, (p+1)*R/n_parts) with their samples, spans and (same hash indices) tokens.  Pure slicing."""
+    R = wl.n_ranks
+    assert R % n_parts == 0
+    rl = R // n_parts
+    parts = []
+    for p in range(n_parts):
+        g0, g1 = int(wl.rank_ptr[p * rl]), int(wl.rank_ptr[(p + 1) * rl])
+        sp0, sp1 = int(wl.span_ptr[g0]), int(wl.span_ptr[g1])
+        parts.append(Workload("%s[part %d/%d]" % (wl.name, p, n_parts), rl,
+                              (wl.rank_ptr[p * rl:(p + 1) * rl + 1] - g0).copy(), wl.lengths[g0:g1].copy(),
+                              (wl.sample_ptr[g0:g1 + 1] - wl.sample_ptr[g0]).copy(),
+                              (wl.span_ptr[g0:g1 + 1] - sp0).copy(), wl.span_lo[sp0:sp1].copy(),
+                              wl.span_hi[sp0:sp1].copy(), wl.token_seed, dict(wl.params),
+                              wl.token_start + int(wl.sample_ptr[g0])))
+    return parts
 
 
 def describe(wl: Workload) -> dict:

@@ -52,6 +52,11 @@ class odb_outputs(ctypes.Structure):
                 ("d_left_ptr", _vp), ("d_left_ids", _vp), ("left_capacity", _i64)]
 
 
+class odb_dist_bufs(ctypes.Structure):
+    _fields_ = [("d_summary_local", _vp), ("d_summary_world", _vp), ("summary_local_count", _i32),
+                ("summary_world_count", _i32), ("d_step_samples_round", _vp), ("step_window", _i32), ("reserved", _i32)]
+
+
 class OdbLibraryError(RuntimeError):
     """libodb.so is missing / unloadable.  There is no fallback path."""
 
@@ -82,6 +87,11 @@ SYMBOLS = {
     "odb_run": (_i32, [_vp, _vp, _P(_i64), _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _P(odb_plan_info), _vp]),
     "odb_run_host": (_i32, [_vp, _vp, _P(_i64), _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _P(odb_plan_info), _vp]),
     "odb_loss_weights": (_i32, [_vp, _i32, _vp, _vp]),
+    "odb_loss_numerators": (_i32, [_vp, _i32, _vp, _vp]),
+    "odb_loss_normalize": (_i32, [_vp, _vp, _i32, _i32, _vp, _vp]),
+    "odb_dist_config": (_i32, [_vp, _i32, _i32, _i32]),
+    "odb_dist_buffers": (_i32, [_vp, _P(odb_dist_bufs)]),
+    "odb_commit": (_i32, [_vp, _vp]),
     "odb_set_timing": (_i32, [_vp, _i32]),
     "odb_get_timing": (_i32, [_vp, _P(ctypes.c_float)]),
     "odb_kernel_launches": (_i64, [_vp]),
@@ -249,6 +259,29 @@ ODB_SCALE_SAMPLE, ODB_SCALE_TOKEN_APPROX, ODB_SCALE_TOKEN_EXACT = 1, 2, 3
 def odb_loss_weights(ctx: int, mode: int, d_weights, stream=None) -> None:
     """w[r * n_steps + k] (fp64, device) of loss-scaling ``mode`` for the plan last collated on ``ctx``."""
     _check(load().odb_loss_weights(ctx, int(mode), _ptr(d_weights), _stream(stream)), "odb_loss_weights", ctx)
+
+
+def odb_loss_numerators(ctx: int, mode: int, d_num, stream=None) -> None:
+    _check(load().odb_loss_numerators(ctx, int(mode), _ptr(d_num), _stream(stream)), "odb_loss_numerators", ctx)
+
+
+def odb_loss_normalize(ctx: int, d_num_world, world_ranks: int, rank_offset: int, d_weights, stream=None) -> None:
+    _check(load().odb_loss_normalize(ctx, _ptr(d_num_world), int(world_ranks), int(rank_offset), _ptr(d_weights),
+                                     _stream(stream)), "odb_loss_normalize", ctx)
+
+
+def odb_dist_config(ctx: int, world_ranks: int, rank_offset: int, world_max_window: int) -> None:
+    _check(load().odb_dist_config(ctx, int(world_ranks), int(rank_offset), int(world_max_window)), "odb_dist_config", ctx)
+
+
+def odb_dist_buffers(ctx: int) -> odb_dist_bufs:
+    b = odb_dist_bufs()
+    _check(load().odb_dist_buffers(ctx, ctypes.byref(b)), "odb_dist_buffers", ctx)
+    return b
+
+
+def odb_commit(ctx: int, stream=None) -> None:
+    _check(load().odb_commit(ctx, _stream(stream)), "odb_commit", ctx)
 
 
 def odb_set_timing(ctx: int, enable: bool) -> None:

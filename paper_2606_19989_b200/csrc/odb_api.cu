@@ -77,6 +77,8 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->d_rec);
     cudaFree(c->d_tot);
     cudaFree(c->d_tile_counter);
+    cudaFree(c->gs_local);
+    cudaFree(c->gs_world);
     if (c->h_rec) cudaFreeHost(c->h_rec);
     if (c->h_tot) cudaFreeHost(c->h_tot);
     c->st_count.release();
@@ -299,7 +301,8 @@ int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_
         return ODB_ERR_STATE;
     }
     CU(c, cudaSetDevice(c->device));
-    if (check_terminated(c)) {
+    // distributed mode: termination is decided on the device from the gathered world summary (k_align)
+    if (!c->world_ranks && check_terminated(c)) {
         // the terminal check round: nothing to form; odb_align / odb_round_status report done
         c->state = 1;
         c->last_T = 0;
@@ -307,7 +310,7 @@ int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_
     }
     const int R = c->prm.n_ranks;
     // make room for this round's steps: T <= the largest window, and <= slot_capacity
-    int64_t bound = c->max_nr;
+    int64_t bound = c->world_ranks ? std::max<int64_t>(c->max_nr, c->world_max_window) : c->max_nr;
     if (c->prm.buffer_size > 0) bound = std::min<int64_t>(bound, c->prm.buffer_size);
     if (c->prm.slot_capacity > 0) bound = std::min<int64_t>(bound, c->prm.slot_capacity);
     bound = std::max<int64_t>(bound, 1);
@@ -323,7 +326,9 @@ int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_
         CU(c, grow_preserve(c->step_samples, (size_t)want, (size_t)c->n_steps, st));
         c->step_cap = want;
     }
+    c->round_window = (int32_t)bound;
     CU(c, launch_round_form(c, st));
+    if (c->world_ranks) CU(c, launch_pack_summary(c, st));
     c->state = 1;
     c->last_T = -1;
     return ODB_OK;
@@ -338,10 +343,69 @@ int odb_align(odb_ctx *c, void *stream) {
         c->state = 2;
         return ODB_OK;
     }
+    if (c->world_ranks) {  // the caller all_reduces the round's step_samples window, then odb_commit
+        CU(c, launch_align_only(c, st));
+        c->state = 6;
+        return ODB_OK;
+    }
     CU(c, launch_round_align(c, st));
     CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, st));
     CU(c, cudaEventRecord(c->ev_status, st));
     c->state = 2;
+    return ODB_OK;
+}
+
+int odb_commit(odb_ctx *c, void *stream) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (c->state != 6) return ODB_ERR_STATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(c, cudaSetDevice(c->device));
+    CU(c, launch_commit_only(c, st));
+    CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, st));
+    CU(c, cudaEventRecord(c->ev_status, st));
+    c->state = 2;
+    return ODB_OK;
+}
+
+int odb_dist_config(odb_ctx *c, int32_t world_ranks, int32_t rank_offset, int32_t world_max_window) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (c->state != 0 && c->state != 4 && c->state != 5) return ODB_ERR_STATE;  // not in the middle of a run
+    const int R = c->prm.n_ranks;
+    if (world_ranks == 0) {  // back to single-process mode
+        c->world_ranks = 0;
+        c->rank_offset = 0;
+        c->world_max_window = 0;
+        return ODB_OK;
+    }
+    if (world_ranks < R || world_ranks > 65535 || rank_offset < 0 || rank_offset + R > world_ranks || world_max_window < 0)
+        return ODB_ERR_INVALID_ARG;
+    CU(c, cudaSetDevice(c->device));
+    if (!c->gs_local) CU(c, dev_alloc(&c->gs_local, 2 * (size_t)R));
+    if (c->gs_world_cap < world_ranks) {
+        if (c->gs_world) cudaFree(c->gs_world);
+        c->gs_world = nullptr;
+        CU(c, dev_alloc(&c->gs_world, 2 * (size_t)world_ranks));
+        c->gs_world_cap = world_ranks;
+    }
+    c->world_ranks = world_ranks;
+    c->rank_offset = rank_offset;
+    c->world_max_window = world_max_window;
+    odb_reset(c);
+    return ODB_OK;
+}
+
+int odb_dist_buffers(odb_ctx *c, odb_dist_bufs *out) {
+    if (!c || !out) return ODB_ERR_INVALID_ARG;
+    if (!c->world_ranks) return ODB_ERR_STATE;
+    memset(out, 0, sizeof(*out));
+    out->d_summary_local = c->gs_local;
+    out->d_summary_world = c->gs_world;
+    out->summary_local_count = 2 * c->prm.n_ranks;
+    out->summary_world_count = 2 * c->world_ranks;
+    if (c->state == 1 || c->state == 6) {  // inside a round: the window of step totals this round may touch
+        out->d_step_samples_round = c->step_samples.p + c->n_steps;
+        out->step_window = c->round_window;
+    }
     return ODB_OK;
 }
 
@@ -368,6 +432,15 @@ int odb_round_status(odb_ctx *c, int32_t *h_done, int32_t *h_T) {
     if (rec.bad_length) {
         c->state = 0;
         return ODB_ERR_BAD_LENGTH;
+    }
+    if (rec.done) {  // distributed mode: the gathered status said "terminated"; nothing was emitted
+        c->stop_reason = c->prm.join_mode ? ODB_STOP_ALL_FINISHED : ODB_STOP_LOGICAL;
+        c->n_rounds = c->round + 1;
+        c->last_T = 0;
+        c->state = 4;
+        if (h_done) *h_done = 1;
+        if (h_T) *h_T = 0;
+        return ODB_OK;
     }
     c->last_T = rec.T;
     c->n_steps += rec.T_emit;
@@ -571,6 +644,7 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
             const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo, const int32_t *d_span_hi,
             const odb_outputs *o, odb_plan_info *h_out, void *stream) {
     if (!c || !o || !h_out) return ODB_ERR_INVALID_ARG;
+    if (c->world_ranks) return ODB_ERR_STATE;  // the caller drives the rounds and their collectives
     cudaStream_t st = (cudaStream_t)stream;
     int rc = run_rounds(c, d_lengths, h_rank_ptr, h_out, st);
     if (rc != ODB_OK) return rc;
@@ -585,6 +659,7 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
                  const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
                  const int32_t *h_span_hi, const odb_outputs *ho, odb_plan_info *h_out, void *stream) {
     if (!c || !ho || !h_out || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
+    if (c->world_ranks) return ODB_ERR_STATE;
     cudaStream_t st = (cudaStream_t)stream;
     CU(c, cudaSetDevice(c->device));
     const int R = c->prm.n_ranks;
@@ -762,6 +837,29 @@ int odb_loss_weights(odb_ctx *c, int mode, double *d_weights, void *stream) {
     if (c->info.n_slots > 0 && !d_weights) return ODB_ERR_INVALID_ARG;
     CU(c, cudaSetDevice(c->device));
     CU(c, launch_loss_weights(c, mode, d_weights, (cudaStream_t)stream));
+    return ODB_OK;
+}
+
+int odb_loss_numerators(odb_ctx *c, int mode, double *d_num, void *stream) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (mode != ODB_SCALE_SAMPLE && mode != ODB_SCALE_TOKEN_APPROX && mode != ODB_SCALE_TOKEN_EXACT)
+        return ODB_ERR_INVALID_ARG;
+    if (c->state != 5 || !c->collated) return ODB_ERR_STATE;
+    if (c->info.n_slots > 0 && !d_num) return ODB_ERR_INVALID_ARG;
+    CU(c, cudaSetDevice(c->device));
+    CU(c, launch_loss_numerators(c, mode, d_num, (cudaStream_t)stream));
+    return ODB_OK;
+}
+
+int odb_loss_normalize(odb_ctx *c, const double *d_num_world, int32_t world_ranks, int32_t rank_offset, double *d_weights,
+                       void *stream) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (c->state != 5 || !c->collated) return ODB_ERR_STATE;
+    if (world_ranks < c->prm.n_ranks || rank_offset < 0 || rank_offset + c->prm.n_ranks > world_ranks)
+        return ODB_ERR_INVALID_ARG;
+    if (c->info.n_slots > 0 && (!d_num_world || !d_weights)) return ODB_ERR_INVALID_ARG;
+    CU(c, cudaSetDevice(c->device));
+    CU(c, launch_loss_normalize(c, d_num_world, world_ranks, rank_offset, d_weights, (cudaStream_t)stream));
     return ODB_OK;
 }
 

@@ -38,7 +38,7 @@ struct RoundRec {
     int32_t quota_hit;   // 1 if the non-join sample quota was reached in this round
     int32_t n_finished;  // ranks that will be "finished" (status -1) at the start of the next round
     int32_t bad_length;  // some length < 1 was seen
-    int32_t pad_;
+    int32_t done;        // distributed mode: the world summary of this round says "terminated" (no emission)
     int64_t emitted_round;  // samples emitted in this round over all ranks
 };
 
@@ -171,8 +171,15 @@ struct odb_ctx {
     int64_t n_total = 0;
     int32_t max_nr = 0;
 
+    // distributed layout (odb_dist_config): this context holds ranks [rank_offset, rank_offset + R) of
+    // world_ranks; 0 = single-process mode
+    int32_t world_ranks = 0, rank_offset = 0, world_max_window = 0, gs_world_cap = 0;
+    int32_t round_window = 0;  // step totals this round may touch: step_samples[n_steps .. n_steps + round_window)
+    int32_t *gs_local = nullptr;  // 2 R: (G_r, S_r) pairs of the local ranks, input of the all_gather
+    int32_t *gs_world = nullptr;  // 2 world_ranks: the gathered pairs
+
     // state machine: 0 = fresh, 1 = groups formed, 2 = aligned (status pending), 3 = status read,
-    // 4 = terminated, 5 = plan queried
+    // 4 = terminated, 5 = plan queried, 6 = aligned but not committed (distributed mode)
     int state = 0;
     int32_t round = 0;     // rounds fully processed (emitting rounds)
     int32_t n_rounds = 0;  // including the terminal check once terminated
@@ -233,7 +240,10 @@ namespace odb {
 // ---- launchers implemented in odb_plan.cu ----------------------------------------------------
 cudaError_t launch_begin(odb_ctx *c, cudaStream_t st);  // per-run state reset + length validation
 cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st);   // A0..A3
-cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commit
+cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commit (single-process mode)
+cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: (G_r, S_r) pairs for the all_gather
+cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
+cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce
 cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st);     // A9 + tables + leftovers
 // ---- launchers implemented in odb_collate.cu -------------------------------------------------
 cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
@@ -243,4 +253,7 @@ cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st)
 cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st);
 // ---- odb_scale.cu ------------------------------------------------------------------------------
 cudaError_t launch_loss_weights(odb_ctx *c, int mode, double *d_weights, cudaStream_t st);
+cudaError_t launch_loss_numerators(odb_ctx *c, int mode, double *d_num, cudaStream_t st);
+cudaError_t launch_loss_normalize(odb_ctx *c, const double *d_num_world, int world_ranks, int rank_offset,
+                                  double *d_weights, cudaStream_t st);
 }  // namespace odb

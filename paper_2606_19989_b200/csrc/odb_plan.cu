@@ -354,25 +354,41 @@ k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ ran
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kRankThreads)
 k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr, const int32_t *__restrict__ G_arr, int R,
-        int slot_capacity, const int32_t *__restrict__ gpos, int32_t *__restrict__ agpos, int32_t *__restrict__ agcnt,
+        const int32_t *__restrict__ gs_world, int world_ranks, int join_mode, int slot_capacity, const int32_t *__restrict__ gpos, int32_t *__restrict__ agpos, int32_t *__restrict__ agcnt,
         int32_t *__restrict__ agorg, uint64_t *ovf, int32_t *step_samples, int step_base, RoundRec *rec) {
     extern __shared__ __align__(16) unsigned char al_smem[];
-    __shared__ int s_maxG, s_minS;
+    __shared__ int s_maxG, s_minS, s_nfin;
     const int r = blockIdx.x;
     if (threadIdx.x == 0) {
         s_maxG = 0;
         s_minS = 0x7fffffff;
+        s_nfin = 0;
     }
     __syncthreads();
-    for (int q = threadIdx.x; q < R; q += blockDim.x) {
-        int g = G_arr[q];
+    // the reduction runs over every rank of the job: the local tables, or -- distributed mode -- the
+    // all_gathered (G, S) pairs of all world_ranks ranks (the paper's per-round all_gather)
+    const int nq = gs_world ? world_ranks : R;
+    for (int q = threadIdx.x; q < nq; q += blockDim.x) {
+        const int g = gs_world ? gs_world[2 * q] : G_arr[q];
+        const int sq = gs_world ? gs_world[2 * q + 1] : S_arr[q];
         if (g > 0) {  // active set A = {r : G_r > 0}
             atomicMax(&s_maxG, g);
-            int sq = S_arr[q];
             if (sq > 0) atomicMin(&s_minS, sq);
         }
+        if (sq == 0) atomicAdd(&s_nfin, 1);  // status -1 "finished"
     }
     __syncthreads();
+    if (gs_world) {
+        // termination predicates on the status every process holds identically (Thm 3 proof P:341)
+        const bool done = join_mode ? (s_nfin == world_ranks) : (s_nfin > 0);
+        if (done) {
+            if (r == 0 && threadIdx.x == 0) {
+                rec->T = 0;
+                rec->done = 1;
+            }
+            return;
+        }
+    }
     int T = s_maxG;
     if (slot_capacity > 0 && T > slot_capacity) T = slot_capacity;  // C+min (same C on every rank)
     if (T > s_minS) T = s_minS;                                     // S+min
@@ -460,6 +476,14 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
     __shared__ long long s_scan64[34];
     __shared__ int s_found;
     const int r = blockIdx.x;
+    if (rec->done) {  // distributed mode: this round was the terminal check
+        if (r == 0 && threadIdx.x == 0) {
+            rec->T_emit = 0;
+            rec->quota_hit = 0;
+            rec->emitted_round = 0;
+        }
+        return;
+    }
     const int T = rec->T;
     int T_emit = T, quota_hit = 0;
     if (!join_mode && quota > 0) {
@@ -843,7 +867,7 @@ cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st) {
     return cudaSuccess;
 }
 
-cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st) {
+static cudaError_t launch_align_kernel(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const size_t al_smem = (size_t)kAlignSmemKeys * sizeof(uint64_t);
     if (!c->attr_align) {
@@ -851,15 +875,49 @@ cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st) {
         if (e != cudaSuccess) return e;
         c->attr_align = true;
     }
-    k_align<<<R, kRankThreads, al_smem, st>>>(c->d_rank_ptr, c->S, c->G, R, c->prm.slot_capacity, c->gpos, c->agpos,
+    k_align<<<R, kRankThreads, al_smem, st>>>(c->d_rank_ptr, c->S, c->G, R, c->world_ranks ? c->gs_world : nullptr,
+                                              c->world_ranks, c->prm.join_mode, c->prm.slot_capacity, c->gpos, c->agpos,
                                               c->agcnt, c->agorg, c->ovf, c->step_samples.p, c->n_steps, c->d_rec);
     ODB_LAUNCH_CHECK(c);
+    return cudaSuccess;
+}
+
+static cudaError_t launch_commit_kernel(odb_ctx *c, cudaStream_t st) {
+    const int R = c->prm.n_ranks;
     k_commit<<<R, kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, c->G, R, c->agpos, c->agcnt, c->agorg, c->agoff,
                                          c->step_samples.p, c->n_steps, c->round, c->prm.join_mode,
                                          (long long)c->prm.sample_quota,
                                          (long long)c->prm.emitted_so_far + (long long)c->samples_emitted, c->st_count.p,
-                                         c->st_width.p, c->st_real.p, c->st_round.p, c->st_origin.p, c->posflag, c->emit_ids, c->emit_pos,
-                                         c->left_ids, c->n_left, c->fetch_pos, c->emit_cur, c->d_rec);
+                                         c->st_width.p, c->st_real.p, c->st_round.p, c->st_origin.p, c->posflag,
+                                         c->emit_ids, c->emit_pos, c->left_ids, c->n_left, c->fetch_pos, c->emit_cur,
+                                         c->d_rec);
+    ODB_LAUNCH_CHECK(c);
+    return cudaSuccess;
+}
+
+cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st) {
+    cudaError_t e = launch_align_kernel(c, st);
+    if (e != cudaSuccess) return e;
+    return launch_commit_kernel(c, st);
+}
+
+cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st) { return launch_align_kernel(c, st); }
+cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st) { return launch_commit_kernel(c, st); }
+
+// distributed mode: the local ranks' (G_r, S_r) pairs, the message of the per-round all_gather
+__global__ void k_pack_summary(int R, const int32_t *__restrict__ G, const int32_t *__restrict__ S, int32_t *__restrict__ gs,
+                               RoundRec *rec) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < R) {
+        gs[2 * q] = G[q];
+        gs[2 * q + 1] = S[q];
+    }
+    if (q == 0) rec->done = 0;
+}
+
+cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
+    const int R = c->prm.n_ranks;
+    k_pack_summary<<<(R + 127) / 128, 128, 0, st>>>(R, c->G, c->S, c->gs_local, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

@@ -37,31 +37,44 @@ __global__ void k_loss_num(int mode, int R, int n_steps, const int32_t *__restri
     }
 }
 
-// pass 2, one thread per step: denominator = sum over ranks in rank order, then the quotients
-__global__ void k_loss_norm(int R, int n_steps, double *__restrict__ w) {
+// pass 2, one thread per step: denominator = sum over ALL ranks of the job in rank order, then the
+// quotients of the local ranks.  num_world is rank-major [world_ranks][n_steps]; the local ranks are
+// rows [rank_offset, rank_offset + R).  w may alias the local rows of num_world.
+__global__ void k_loss_norm(int R, int world_ranks, int rank_offset, int n_steps, const double *num_world, double *w) {
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_steps; k += gridDim.x * blockDim.x) {
         double denom = 0.0;
-        for (int r = 0; r < R; ++r) denom = __dadd_rn(denom, w[(int64_t)r * n_steps + k]);
+        for (int q = 0; q < world_ranks; ++q) denom = __dadd_rn(denom, num_world[(int64_t)q * n_steps + k]);
         for (int r = 0; r < R; ++r) {
-            const int64_t s = (int64_t)r * n_steps + k;
-            w[s] = denom > 0.0 ? __ddiv_rn(w[s], denom) : 0.0;
+            const double num = num_world[(int64_t)(rank_offset + r) * n_steps + k];
+            w[(int64_t)r * n_steps + k] = denom > 0.0 ? __ddiv_rn(num, denom) : 0.0;
         }
     }
 }
 
-cudaError_t launch_loss_weights(odb_ctx *c, int mode, double *d_weights, cudaStream_t st) {
+cudaError_t launch_loss_numerators(odb_ctx *c, int mode, double *d_num, cudaStream_t st) {
     const int R = c->prm.n_ranks, n_steps = c->n_steps;
     const int64_t n_slots = (int64_t)R * n_steps;
     if (n_slots == 0) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>((n_slots + 255) / 256, (int64_t)c->sm_count * 8);
-    k_loss_num<<<blocks, 256, 0, st>>>(mode, R, n_steps, c->grp_count.p, c->grp_valid.p, c->grp_origin.p, d_weights);
-    c->launches++;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    blocks = (int)std::min<int64_t>(((int64_t)n_steps + 127) / 128, (int64_t)c->sm_count * 8);
-    k_loss_norm<<<blocks, 128, 0, st>>>(R, n_steps, d_weights);
+    const int blocks = (int)std::min<int64_t>((n_slots + 255) / 256, (int64_t)c->sm_count * 8);
+    k_loss_num<<<blocks, 256, 0, st>>>(mode, R, n_steps, c->grp_count.p, c->grp_valid.p, c->grp_origin.p, d_num);
     c->launches++;
     return cudaGetLastError();
+}
+
+cudaError_t launch_loss_normalize(odb_ctx *c, const double *d_num_world, int world_ranks, int rank_offset,
+                                  double *d_weights, cudaStream_t st) {
+    const int R = c->prm.n_ranks, n_steps = c->n_steps;
+    if ((int64_t)R * n_steps == 0) return cudaSuccess;
+    const int blocks = (int)std::min<int64_t>(((int64_t)n_steps + 127) / 128, (int64_t)c->sm_count * 8);
+    k_loss_norm<<<blocks, 128, 0, st>>>(R, world_ranks, rank_offset, n_steps, d_num_world, d_weights);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_loss_weights(odb_ctx *c, int mode, double *d_weights, cudaStream_t st) {
+    cudaError_t e = launch_loss_numerators(c, mode, d_weights, st);
+    if (e != cudaSuccess) return e;
+    return launch_loss_normalize(c, d_weights, c->prm.n_ranks, 0, d_weights, st);  // in place: world = local
 }
 
 }  // namespace odb

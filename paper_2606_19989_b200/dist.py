@@ -1,0 +1,240 @@
+"""Ranks spread over several processes / GPUs: the host-side protocol driver.
+
+The paper runs one rank per process and exchanges, once per round, every rank's status and group counts
+with ONE unconditional all_gather on a dedicated channel (section 2.3; message layout
+P:250; deadlock-freedom Lemma 3), then evaluates Eq. 3 and the termination predicates
+on the shared tensor.  Here every process holds ``n_ranks`` consecutive virtual ranks of the job on its
+own GPU; per round it runs
+
+    odb_form_groups -> all_gather (G_r, S_r) -> odb_align -> all_reduce step totals -> odb_commit
+
+with the collectives issued by THIS module through ``torch.distributed`` (NCCL over NVLink on GPUs) on
+device buffers the library exposes (``odb_dist_buffers``).  Every step of the method itself runs in the
+kernels of libodb; this module only sequences calls and collectives (plumbing).
+
+The protocol is written as a generator that yields one request per collective, so that the same code
+is driven (a) by ``torch.distributed`` (``run``), one process per GPU, and (b) in lock step for several
+engines inside one process (``run_lockstep``), which is how a single GPU checks the multi-process path
+bit for bit against the oracle without ranks ever waiting on one another.
+
+Every process issues the same collectives in the same order whatever its data (no data-dependent early
+exit before a collective): the deadlock-freedom argument of Lemma 3.
+"""
+from __future__ import annotations
+
+from typing import Generator, List, Sequence, Tuple
+
+import numpy as np
+
+from . import binding as B
+
+
+# ---- collective requests yielded by the protocol ----------------------------------------------
+#   ("max_int", value)                 -> the driver sends back max over processes (int)
+#   ("all_gather", out, inp)           -> out = concatenation over processes of inp (tensors)
+#   ("all_reduce_sum", t)              -> t = elementwise sum over processes, in place (tensor)
+Request = Tuple
+
+
+class _DevArray:
+    """A raw device pointer as something ``torch.as_tensor`` can wrap (no copy)."""
+
+    def __init__(self, ptr: int, count: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (int(count),), "typestr": typestr, "data": (int(ptr), False),
+                                         "version": 3, "strides": None}
+
+
+def _wrap(ptr: int, count: int, typestr: str, device):
+    import torch
+    if count <= 0 or not ptr:
+        return torch.zeros(0, dtype=torch.int32 if typestr == "<i4" else torch.int64, device=device)
+    return torch.as_tensor(_DevArray(ptr, count, typestr), device=device)
+
+
+class CudaEngine:
+    """The local half of the protocol on one GPU: a thin holder of an ``Odb`` context in distributed
+    mode plus torch views of the buffers the collectives work on."""
+
+    def __init__(self, params: B.odb_params, max_samples_total: int, d_lengths, h_rank_ptr, device: int = 0,
+                 stream=None):
+        self.ctx = B.Odb(params, max_samples_total, device)
+        self.params = params
+        self.d_lengths = d_lengths
+        self.h_rank_ptr = np.ascontiguousarray(h_rank_ptr, dtype=np.int64)
+        self.device = "cuda:%d" % device
+        self.stream = stream
+        self.n_ranks = int(params.n_ranks)
+
+    def close(self):
+        self.ctx.close()
+
+    # window bound of the local ranks: max_r min(n_r, buffer_size or n_r)
+    def local_max_window(self) -> int:
+        n = np.diff(self.h_rank_ptr)
+        m = int(n.max()) if len(n) else 0
+        bs = int(self.params.buffer_size)
+        return min(m, bs) if bs > 0 else m
+
+    def dist_config(self, world_ranks: int, rank_offset: int, world_max_window: int):
+        B.odb_dist_config(self.ctx.h, world_ranks, rank_offset, world_max_window)
+
+    def form_groups(self):
+        B.odb_form_groups(self.ctx.h, self.d_lengths, self.h_rank_ptr, self.stream)
+
+    def summary(self):
+        b = B.odb_dist_buffers(self.ctx.h)
+        return (_wrap(b.d_summary_world, b.summary_world_count, "<i4", self.device),
+                _wrap(b.d_summary_local, b.summary_local_count, "<i4", self.device))
+
+    def align(self):
+        B.odb_align(self.ctx.h, self.stream)
+
+    def step_samples_window(self):
+        b = B.odb_dist_buffers(self.ctx.h)
+        return _wrap(b.d_step_samples_round, b.step_window, "<i4", self.device)
+
+    def commit(self):
+        B.odb_commit(self.ctx.h, self.stream)
+
+    def round_status(self):
+        return B.odb_round_status(self.ctx.h)
+
+    def plan_query(self):
+        return B.odb_plan_query(self.ctx.h)
+
+    def collate(self, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, out: B.OutputBuffers):
+        B.odb_collate(self.ctx.h, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, out.struct, self.stream)
+
+    def loss_numerators(self, mode: int, d_num):
+        B.odb_loss_numerators(self.ctx.h, mode, d_num, self.stream)
+
+    def loss_normalize(self, d_num_world, world_ranks: int, rank_offset: int, d_weights):
+        B.odb_loss_normalize(self.ctx.h, d_num_world, world_ranks, rank_offset, d_weights, self.stream)
+
+
+# ---- the protocol ------------------------------------------------------------------------------
+def plan_protocol(engine, world_ranks: int, rank_offset: int) -> Generator[Request, object, tuple]:
+    """Round loop of one process.  Returns (plan info of the local ranks, [T_grp of every emitting round])."""
+    wmax = yield ("max_int", int(engine.local_max_window()))
+    engine.dist_config(world_ranks, rank_offset, int(wmax))
+    round_T: List[int] = []
+    while True:
+        engine.form_groups()
+        world, local = engine.summary()
+        yield ("all_gather", world, local)                 # the per-round metadata exchange
+        engine.align()                                      # Eq. 3 + termination predicates on the shared tensor
+        yield ("all_reduce_sum", engine.step_samples_window())   # global e_k (trainer-side count)
+        engine.commit()
+        done, T = engine.round_status()
+        if T > 0:
+            round_T.append(T)
+        if done:
+            break
+    return engine.plan_query(), round_T
+
+
+def step_valid_protocol(step_valid_tokens) -> Generator[Request, object, None]:
+    """After the local collate: T_tok per step over ALL ranks (Eq. 2)."""
+    yield ("all_reduce_sum", step_valid_tokens)
+
+
+def loss_weights_protocol(engine, mode: int, world_ranks: int, rank_offset: int, num_local, num_world,
+                          weights) -> Generator[Request, object, None]:
+    """w_{r,k} of the local slots; denominators run over all ranks of the job in rank order, so the
+    result is bit-identical to a single-process evaluation (see odb_loss_normalize)."""
+    engine.loss_numerators(mode, num_local)
+    yield ("all_gather", num_world, num_local)
+    engine.loss_normalize(num_world, world_ranks, rank_offset, weights)
+
+
+# ---- drivers -----------------------------------------------------------------------------------
+class TorchCollectives:
+    """``torch.distributed`` (NCCL for CUDA tensors, gloo for CPU tensors)."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist = dist
+        self.group = group
+        self.world_size = dist.get_world_size(group)
+        self.rank = dist.get_rank(group)
+
+    def max_int(self, v: int, device="cpu") -> int:
+        import torch
+        t = torch.tensor([int(v)], dtype=torch.int64, device=device)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
+        return int(t.item())
+
+    def all_gather(self, out, inp):
+        if inp.numel() == 0:
+            return
+        self.dist.all_gather_into_tensor(out, inp, group=self.group)
+
+    def all_reduce_sum(self, t):
+        if t.numel() == 0:
+            return
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
+
+
+def run(gen: Generator, coll: TorchCollectives, device="cpu"):
+    """Drive one protocol generator with real collectives.  Returns the generator's return value."""
+    reply = None
+    try:
+        while True:
+            req = gen.send(reply)
+            reply = None
+            if req[0] == "max_int":
+                reply = coll.max_int(req[1], device)
+            elif req[0] == "all_gather":
+                coll.all_gather(req[1], req[2])
+            elif req[0] == "all_reduce_sum":
+                coll.all_reduce_sum(req[1])
+            else:
+                raise ValueError("unknown request %r" % (req[0],))
+    except StopIteration as e:
+        return e.value
+
+
+def run_lockstep(gens: Sequence[Generator]):
+    """Drive the generators of several processes-in-one in lock step: all are advanced to their next
+    collective, the collective is performed among their tensors by plain copies / sums, then all are
+    resumed.  Nothing ever waits on a kernel of another engine.  Returns the list of return values."""
+    import torch
+    n = len(gens)
+    replies = [None] * n
+    results = [None] * n
+    live = [True] * n
+    while any(live):
+        reqs = [None] * n
+        for i, g in enumerate(gens):
+            if not live[i]:
+                continue
+            try:
+                reqs[i] = g.send(replies[i])
+            except StopIteration as e:
+                results[i] = e.value
+                live[i] = False
+        active = [r for r in reqs if r is not None]
+        if not active:
+            break
+        if len(active) != n or len({r[0] for r in active}) != 1:
+            raise RuntimeError("processes diverged: %r" % ([r and r[0] for r in reqs],))  # Lemma 3 would be violated
+        kind = active[0][0]
+        replies = [None] * n
+        if kind == "max_int":
+            m = max(r[1] for r in reqs)
+            replies = [m] * n
+        elif kind == "all_gather":
+            cat = torch.cat([r[2].reshape(-1) for r in reqs]) if reqs[0][2].numel() else None
+            for r in reqs:
+                if cat is not None:
+                    r[1].reshape(-1)[:cat.numel()].copy_(cat)
+        elif kind == "all_reduce_sum":
+            if reqs[0][1].numel():
+                tot = reqs[0][1].clone()
+                for r in reqs[1:]:
+                    tot += r[1]
+                for r in reqs:
+                    r[1].copy_(tot)
+        else:
+            raise ValueError(kind)
+    return results

@@ -1,0 +1,113 @@
+"""A CPU stand-in for ``paper_2606_19989_b200.dist.CudaEngine`` built from the ORACLE's pieces
+(group_window, target_groups, align_list), used only by the world_size-2 gloo tests: it lets the
+protocol driver of dist.py (the product's host-side logic: sequencing, collectives, termination on
+the shared status) run on a box without a GPU.  Test infrastructure; never imported by the package."""
+from types import SimpleNamespace
+
+import numpy as np
+import torch
+
+
+class OracleEngine:
+    def __init__(self, oracle, wl):
+        self.o = oracle
+        self.wl = wl
+        self.p = wl.params
+        self.R = wl.n_ranks
+        self.lens = [wl.lengths[wl.rank_ptr[r]:wl.rank_ptr[r + 1]] for r in range(self.R)]
+
+    def local_max_window(self):
+        m = max((len(x) for x in self.lens), default=0)
+        bs = self.p["buffer_size"]
+        return min(m, bs) if bs > 0 else m
+
+    def dist_config(self, world_ranks, rank_offset, world_max_window):
+        self.W, self.off = world_ranks, rank_offset
+        bs, C = self.p["buffer_size"], self.p["slot_capacity"]
+        b = world_max_window
+        if C > 0:
+            b = min(b, C)
+        self.bound = max(b, 1)
+        self.buf = [[] for _ in range(self.R)]
+        self.pos = [0] * self.R
+        self.slots = [[] for _ in range(self.R)]
+        self.step_samples = []
+        self.s_emit = 0
+        self.round = 0
+        self.stop = None
+        self.world = torch.zeros(2 * world_ranks, dtype=torch.int32)
+        self.local = torch.zeros(2 * self.R, dtype=torch.int32)
+
+    def form_groups(self):
+        bs = self.p["buffer_size"]
+        self.cand = []
+        for r in range(self.R):
+            n_r = len(self.lens[r])
+            while (bs == 0 or len(self.buf[r]) < bs) and self.pos[r] < n_r:
+                self.buf[r].append(self.pos[r])
+                self.pos[r] += 1
+            S = len(self.buf[r])
+            g = self.o.group_window(self.p["rule"], self.p["budget"], self.lens[r], np.array(self.buf[r], np.int32)) if S else []
+            self.cand.append(g)
+            self.local[2 * r], self.local[2 * r + 1] = len(g), S
+        self.window = torch.zeros(self.bound, dtype=torch.int32)
+        self.done = False
+        self.T = 0
+
+    def summary(self):
+        return self.world, self.local
+
+    def align(self):
+        G, S = self.world[0::2].numpy().astype(np.int64), self.world[1::2].numpy().astype(np.int64)
+        n_fin = int((S == 0).sum())
+        self.done = (n_fin == self.W) if self.p["join_mode"] else (n_fin > 0)
+        if self.done:
+            return
+        self.T = self.o.target_groups(G, S, self.p["slot_capacity"])
+        self.aligned = []
+        for r in range(self.R):
+            if not self.cand[r]:
+                self.aligned.append(None)
+                continue
+            al, back = self.o.align_list(self.cand[r], self.T)
+            self.buf[r] = list(back)
+            self.aligned.append(al)
+            for k, g in enumerate(al):
+                self.window[k] += len(g)
+
+    def step_samples_window(self):
+        return self.window
+
+    def commit(self):
+        if self.done:
+            self.stop = 0 if self.p["join_mode"] else 1
+            self.round += 1
+            return
+        e = self.window[:self.T].tolist()      # global after the all_reduce
+        T_emit, Q = self.T, self.p["sample_quota"]
+        if not self.p["join_mode"] and Q > 0:
+            run = self.p["emitted_so_far"] + self.s_emit
+            for k in range(self.T):
+                run += e[k]
+                if run >= Q:
+                    T_emit = k + 1
+                    self.stop = 2
+                    break
+        for r in range(self.R):
+            for k in range(T_emit):
+                self.slots[r].append(list(self.aligned[r][k]) if self.aligned[r] is not None else [])
+            if self.aligned[r] is not None:
+                for k in range(T_emit, self.T):
+                    self.buf[r].extend(self.aligned[r][k])
+        self.step_samples.extend(e[:T_emit])
+        self.s_emit += sum(e[:T_emit])
+        self.round += 1
+
+    def round_status(self):
+        if self.done:
+            return 1, 0
+        return (1 if self.stop == 2 else 0), self.T
+
+    def plan_query(self):
+        return SimpleNamespace(n_rounds=self.round, n_steps=len(self.step_samples), stop_reason=self.stop,
+                               slots=self.slots, step_samples=list(self.step_samples))

@@ -31,7 +31,7 @@ class DeviceWorkload:
         if tokens_from_host is not None:
             self.tokens[:n_tok].copy_(torch.from_numpy(tokens_from_host))
         else:
-            P.odb_synth_tokens(self.tokens, 0, n_tok, wl.token_seed, I.VOCAB)
+            P.odb_synth_tokens(self.tokens, wl.token_start, n_tok, wl.token_seed, I.VOCAB)
         torch.cuda.synchronize()
 
 

@@ -1,0 +1,94 @@
+"""world_size-2 gloo test of the multi-process protocol driver (paper_2606_19989_b200/dist.py) on CPU:
+two real processes, real torch.distributed collectives; the local engine is the oracle-backed stand-in
+of tests/_oracle_engine.py (the CUDA engine needs a GPU: tests/test_gpu_dist.py).  Each process must
+end with the slots the whole-job oracle gives to its ranks, the global step totals, and the same
+termination as everyone else (Lemma 3: predicates computed from the same gathered tensor)."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+CASES = ["tiny", "unequal", "empty_rank", "overflow_multiround", "overflow_nonjoin_quota", "nonjoin_logical",
+         "one_process_idle"]
+
+
+def _case(name):
+    import odb_inputs as I
+    if name == "tiny":
+        return I.make_workload(0)
+    if name == "overflow_nonjoin_quota":
+        wl = I.protocol_workload("overflow_multiround", 3, join_mode=0)
+        wl.params["sample_quota"] = int(0.6 * wl.n_samples)
+        return wl
+    if name == "nonjoin_logical":
+        return I.protocol_workload("unequal", 5, join_mode=0, buffer_size=32)
+    if name == "one_process_idle":   # every rank of the second process is empty from the start
+        rng = np.random.default_rng(1)
+        return I.custom_workload("one_process_idle", [rng.integers(8, 300, 50), rng.integers(8, 300, 70), [], []],
+                                 seed=3, budget=1024, buffer_size=16)
+    return I.protocol_workload(name, 2)
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import odb_inputs as I
+    from oracle import odb_oracle
+    from paper_2606_19989_b200 import dist as D
+    from tests._oracle_engine import OracleEngine
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
+    try:
+        coll = D.TorchCollectives()
+        for name in CASES:
+            wl = _case(name)
+            rl = wl.n_ranks // world
+            part = I.split_ranks(wl, world)[rank]
+            eng = OracleEngine(odb_oracle, part)
+            info, round_T = D.run(D.plan_protocol(eng, wl.n_ranks, rank * rl), coll)
+            q.put((name, rank, info.n_rounds, info.n_steps, info.stop_reason, info.slots, info.step_samples, round_T))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_process_gloo_protocol_matches_whole_job_oracle():
+    import torch.multiprocessing as mp
+    sys.path.insert(0, ROOT)
+    from oracle import odb_oracle
+    odb_oracle.build()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = {}
+    for _ in range(2 * len(CASES)):
+        item = q.get(timeout=240)
+        got[(item[0], item[1])] = item[2:]
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    for name in CASES:
+        wl = _case(name)
+        plan, _ = odb_oracle.run_workload(wl, collate=False)
+        rl = wl.n_ranks // 2
+        for rank in range(2):
+            n_rounds, n_steps, stop, slots, step_samples, round_T = got[(name, rank)]
+            assert (n_rounds, n_steps, stop) == (plan.n_rounds, plan.n_steps, plan.stop_reason), (name, rank)
+            assert round_T == plan.round_T.tolist(), (name, rank)
+            assert step_samples == plan.step_samples.tolist(), (name, rank)
+            for j in range(rl):
+                assert slots[j] == plan.groups_of_rank(rank * rl + j), (name, rank, j)

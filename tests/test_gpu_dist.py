@@ -1,0 +1,169 @@
+"""The multi-process path on ONE GPU: the R ranks of a job are split over 2 or 4
+contexts ("processes"), each driven by the very protocol generator a torch.distributed run uses
+(paper_2606_19989_b200/dist.py), in lock step -- all contexts are advanced to their next collective,
+the collective is done by plain tensor copies / sums, all are resumed, so no kernel ever waits on
+another context.  Every process's slots, arenas, step totals and loss weights must equal, bit for
+bit, the oracle's result for the WHOLE job restricted to that process's ranks."""
+import numpy as np
+import pytest
+
+import odb_inputs as I
+from tests import _parity as Par
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2606_19989_b200 as P
+    P.load()
+    return P
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    from oracle import odb_oracle
+    odb_oracle.build()
+    return odb_oracle
+
+
+def _case(name):
+    if name == "tiny":
+        return I.make_workload(0)
+    if name == "config2_slice":
+        return I.make_workload(1, n_ranks=4, n_per_rank=600)
+    if name == "config4_slice_nonjoin":
+        return I.make_workload(3, n_ranks=4, n_per_rank=700, join_mode=0)
+    if name == "overflow_nonjoin_quota":
+        wl = I.protocol_workload("overflow_multiround", 3, join_mode=0)
+        wl.params["sample_quota"] = int(0.6 * wl.n_samples)
+        return wl
+    if name == "maxfit_overflow":
+        return I.protocol_workload("overflow_multiround", 5, rule=1)
+    return I.protocol_workload(name, 2)
+
+
+@pytest.mark.parametrize("n_proc", [2, 4])
+@pytest.mark.parametrize("name", ["tiny", "config2_slice", "unequal", "empty_rank", "overflow_multiround",
+                                  "overflow_nonjoin_quota", "maxfit_overflow", "config4_slice_nonjoin",
+                                  "audit:bimodal"])
+def test_lockstep_processes_match_whole_job_oracle(P, oracle, name, n_proc):
+    import torch
+    from paper_2606_19989_b200 import dist as D
+    wl = _case(name)
+    if wl.n_ranks % n_proc:
+        pytest.skip("ranks do not split evenly")
+    plan, ref = oracle.run_workload(wl)
+    R, K = wl.n_ranks, plan.n_steps
+    rl = R // n_proc
+    parts = I.split_ranks(wl, n_proc)
+    dws = [Par.DeviceWorkload(w) for w in parts]
+    engines = [D.CudaEngine(Par.gpu_params(w), max(w.n_samples, 1), dw.lengths, w.rank_ptr) for w, dw in zip(parts, dws)]
+    try:
+        res = D.run_lockstep([D.plan_protocol(e, R, p * rl) for p, e in enumerate(engines)])
+        outs = []
+        for p, (e, w, dw) in enumerate(zip(engines, parts, dws)):
+            info, round_T = res[p]
+            assert round_T == plan.round_T.tolist()
+            assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason)
+            out = P.OutputBuffers.for_plan(rl, info, dw.device, fill=Par.SENTINEL)
+            e.collate(dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out)
+            outs.append((info, out))
+        D.run_lockstep([D.step_valid_protocol(out.table("step_valid_tokens")) for _, out in outs])
+        torch.cuda.synchronize()
+        for p, (info, out) in enumerate(outs):
+            s0, s1 = p * rl * K, (p + 1) * rl * K
+            off0 = int(plan.grp_offset[s0]) if s0 < plan.n_slots else plan.total_elems
+            off1 = int(plan.grp_offset[s1]) if s1 < plan.n_slots else plan.total_elems
+            q0, q1 = int(plan.grp_sample_ptr[s0]), int(plan.grp_sample_ptr[s1])
+            assert int(info.total_elems) == off1 - off0 and int(info.samples_emitted) == q1 - q0
+            for name_ in ("grp_count", "grp_width", "grp_round", "grp_real_tokens", "grp_origin"):
+                assert np.array_equal(out.table(name_).cpu().numpy(), getattr(plan, name_)[s0:s1]), name_
+            assert np.array_equal(out.table("grp_offset").cpu().numpy(), plan.grp_offset[s0:s1] - off0)
+            assert np.array_equal(out.table("grp_sample_ptr").cpu().numpy(), plan.grp_sample_ptr[s0:s1 + 1] - q0)
+            assert np.array_equal(out.table("grp_sample_ids").cpu().numpy(), plan.grp_sample_ids[q0:q1])
+            assert np.array_equal(out.table("grp_valid_tokens").cpu().numpy(), ref["grp_valid_tokens"][s0:s1])
+            # global per-step tables: identical on every process
+            assert np.array_equal(out.table("step_samples").cpu().numpy(), plan.step_samples)
+            assert np.array_equal(out.table("step_valid_tokens").cpu().numpy(), ref["step_valid_tokens"])
+            l0, l1 = int(plan.left_ptr[p * rl]), int(plan.left_ptr[(p + 1) * rl])
+            assert np.array_equal(out.table("left_ptr").cpu().numpy(), plan.left_ptr[p * rl:(p + 1) * rl + 1] - l0)
+            assert np.array_equal(out.table("left_ids").cpu().numpy(), plan.left_ids[l0:l1])
+            E = off1 - off0
+            for name_ in ("input_ids", "labels", "position_ids", "attention_mask"):
+                assert np.array_equal(getattr(out, name_)[:E].cpu().numpy(), ref[name_][off0:off1]), name_
+        # loss weights: denominators over all ranks of the job, bit-identical to the single-process oracle
+        for mode in (P.ODB_SCALE_SAMPLE, P.ODB_SCALE_TOKEN_APPROX, P.ODB_SCALE_TOKEN_EXACT):
+            want = oracle.loss_weights(mode, R, K, plan.grp_count, ref["grp_valid_tokens"], plan.grp_origin)
+            bufs = []
+            for p, e in enumerate(engines):
+                num_local = torch.zeros(max(rl * K, 1), dtype=torch.float64, device="cuda:0")[:rl * K]
+                num_world = torch.zeros(max(R * K, 1), dtype=torch.float64, device="cuda:0")[:R * K]
+                w = torch.full((max(rl * K, 1),), float("nan"), dtype=torch.float64, device="cuda:0")[:rl * K]
+                bufs.append((num_local, num_world, w))
+            D.run_lockstep([D.loss_weights_protocol(e, mode, R, p * rl, *bufs[p]) for p, e in enumerate(engines)])
+            torch.cuda.synchronize()
+            for p in range(n_proc):
+                got = bufs[p][2].cpu().numpy().reshape(rl, K)
+                assert np.array_equal(got.view(np.uint64), want[p * rl:(p + 1) * rl].view(np.uint64)), (mode, p)
+    finally:
+        for e in engines:
+            e.close()
+
+
+def test_single_process_nccl_world(P, oracle):
+    """The torch.distributed driver itself (NCCL, world_size 1 -- the box has one GPU): the protocol
+    with real collectives on the library's device buffers equals the oracle."""
+    import os
+    import torch
+    import torch.distributed as dist
+    from paper_2606_19989_b200 import dist as D
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29731")
+    created = False
+    if not dist.is_initialized():
+        torch.cuda.set_device(0)
+        dist.init_process_group("nccl", rank=0, world_size=1)
+        created = True
+    try:
+        wl = I.protocol_workload("overflow_multiround", 7)
+        plan, ref = oracle.run_workload(wl)
+        dw = Par.DeviceWorkload(wl)
+        e = D.CudaEngine(Par.gpu_params(wl), wl.n_samples, dw.lengths, wl.rank_ptr)
+        try:
+            coll = D.TorchCollectives()
+            info, round_T = D.run(D.plan_protocol(e, wl.n_ranks, 0), coll, device="cuda:0")
+            out = P.OutputBuffers.for_plan(wl.n_ranks, info, dw.device, fill=Par.SENTINEL)
+            e.collate(dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out)
+            D.run(D.step_valid_protocol(out.table("step_valid_tokens")), coll, device="cuda:0")
+            torch.cuda.synchronize()
+            assert round_T == plan.round_T.tolist()
+            Par.compare_plan(plan, info, out)
+            Par.compare_full(plan, ref, info, out)
+        finally:
+            e.close()
+    finally:
+        if created:
+            dist.destroy_process_group()
+
+
+def test_dist_mode_errors(P):
+    wl = I.make_workload(0)
+    dw = Par.DeviceWorkload(wl)
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        with pytest.raises(P.OdbError):
+            P.odb_commit(ctx.h)                       # not in distributed mode
+        with pytest.raises(P.OdbError):
+            P.odb_dist_buffers(ctx.h)
+        with pytest.raises(P.OdbError):
+            P.odb_dist_config(ctx.h, 1, 0, 64)        # world smaller than the local ranks
+        P.odb_dist_config(ctx.h, 4, 2, 64)
+        empty = P.OutputBuffers(wl.n_ranks, 0, 0, 0, 0, 0, dw.device)
+        with pytest.raises(P.OdbError):               # the caller drives the rounds in this mode
+            P.odb_run(ctx.h, dw.lengths, wl.rank_ptr, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi,
+                      empty.struct)
+        P.odb_dist_config(ctx.h, 0, 0, 0)             # back to single-process mode
+        Par.run_gpu(wl, dw, staged=False)
