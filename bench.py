@@ -52,6 +52,9 @@ def parse_args():
     ap.add_argument("--rule", type=int, default=0)
     ap.add_argument("--join", type=int, default=1)
     ap.add_argument("--sweep", action="store_true", help="also time the nine config-5 cells (extra key 'sweep')")
+    ap.add_argument("--shard-ranks", action="store_true",
+                    help="SURVEY.md 8(f) F1: split the job's virtual ranks over the N GPUs (strong scaling; per-round "
+                         "all_gather + all_reduce over NCCL) instead of N independent replicas")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -429,6 +432,102 @@ def run_ours(args):
         print(json.dumps(result), flush=True)
 
 
+def run_sharded(args):
+    """--shard-ranks: ONE job whose R virtual ranks are split over the N GPUs (R/N consecutive ranks per
+    process), driven by the protocol of paper_2606_19989_b200/dist.py: per round one all_gather of the
+    (G_r, S_r) pairs and one all_reduce of the step totals over NCCL, then the local collate and the
+    all_reduce of the per-step valid-token totals.  Strong scaling: value = the job's samples / time."""
+    import torch
+    import torch.distributed as dist
+    import paper_2606_19989_b200 as P
+    from paper_2606_19989_b200 import dist as D
+    P.load()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = "cuda:%d" % local
+    if world == 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29577")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device(device))
+    else:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    wl_all = make_wl(args)
+    if wl_all.n_ranks % world:
+        raise SystemExit("--shard-ranks needs the rank count (%d) to be a multiple of --gpus" % wl_all.n_ranks)
+    rl = wl_all.n_ranks // world
+    wl = I.split_ranks(wl_all, world)[rank]
+    t = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).to(device)
+    lengths, sample_ptr, span_ptr = t(wl.lengths, torch.int32), t(wl.sample_ptr, torch.int64), t(wl.span_ptr, torch.int64)
+    z = torch.zeros(1, dtype=torch.int32, device=device)
+    span_lo = t(wl.span_lo, torch.int32) if len(wl.span_lo) else z
+    span_hi = t(wl.span_hi, torch.int32) if len(wl.span_hi) else z
+    tokens = torch.empty(wl.n_tokens + 16, dtype=torch.int32, device=device)
+    P.odb_synth_tokens(tokens, wl.token_start, wl.n_tokens, wl.token_seed, I.VOCAB)
+    coll = D.TorchCollectives()
+    eng = D.CudaEngine(gpu_params(P, wl), max(wl.n_samples, 1), lengths, wl.rank_ptr, device=local)
+    P.odb_set_timing(eng.ctx.h, True)
+    info, _ = D.run(D.plan_protocol(eng, wl_all.n_ranks, rank * rl), coll, device)
+    out = P.OutputBuffers.for_plan(rl, info, device)
+
+    def one():
+        info, _ = D.run(D.plan_protocol(eng, wl_all.n_ranks, rank * rl), coll, device)
+        eng.collate(tokens, sample_ptr, span_ptr, span_lo, span_hi, out)
+        D.run(D.step_valid_protocol(out.table("step_valid_tokens")), coll, device)
+        return info
+
+    for _ in range(args.warmup):
+        one()
+    torch.cuda.synchronize()
+    dist.barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = P.odb_kernel_launches(eng.ctx.h)
+    col = 0.0
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(args.steps):
+        info = one()
+        col += P.odb_get_timing(eng.ctx.h)[1]
+    ev1.record()
+    torch.cuda.synchronize()
+    dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = P.odb_kernel_launches(eng.ctx.h) - l0
+    tt = torch.tensor([ev0.elapsed_time(ev1) / max(args.steps, 1), col / max(args.steps, 1)], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms, col_ms = float(tt[0]), float(tt[1])
+    tot = torch.tensor([int(info.samples_emitted), int(info.real_tokens), int(info.padded_elems)], dtype=torch.int64, device=device)
+    loc = tot.clone()
+    dist.all_reduce(tot)
+    n_samples, n_tok, n_pad = (int(x) for x in tot.tolist())
+    peak, peak_src = measured_peak()
+    ab_local = algorithmic_bytes(int(loc[1]), int(loc[2]))
+    achieved = ab_local / (col_ms * 1e-3) / 1e9
+    eng.close()
+    dist.barrier()
+    dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": n_samples / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "int32", "data": "synthetic",
+            "config": {"workload": workload_name(args, wl_all), "rule": RULE_NAMES[args.rule], "join_mode": args.join,
+                       "samples": n_samples, "real_tokens": n_tok, "padded_elems": n_pad, "n_steps": int(info.n_steps),
+                       "n_rounds": int(info.n_rounds),
+                       "parallelism": "virtual ranks sharded over %d GPU(s), %d per GPU; per round all_gather(G,S) + "
+                                      "all_reduce(step totals) over NCCL" % (world, rl),
+                       "l2": "no flush: inputs and outputs are far larger than the 126 MB L2"},
+            "tokens_per_s": n_tok / (ms * 1e-3), "stage_ms": {"collate_kernel": col_ms},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "k_collate (rank 0's share)", "algorithmic_bytes": ab_local,
+                         "kernel_ms": col_ms, "peak_source": peak_src},
+            "gpu_launches": int(launches), "clocks": clocks, "e2e": None, "cpu_baseline": None}), flush=True)
+
+
 def run_sweep(P, args, device, peak):
     """The nine (CV, budget) cells of configs[4], both rules: samples/s, tokens/s, collate GB/s."""
     import torch
@@ -459,6 +558,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard_ranks:
+        run_sharded(args)
     else:
         run_ours(args)
 

@@ -8,3 +8,4 @@ from .binding import (  # noqa: F401
     Odb, OdbError, OdbLibraryError, OutputBuffers, SYMBOLS, library_path, load, make_params,
     odb_outputs, odb_params, odb_plan_info, status_string,
 )
+from .batches import StepBatches  # noqa: F401,E402

@@ -1,0 +1,66 @@
+"""Step-wise view of a collated plan: what a training loop iterates over (adapter).
+
+The paper's main-process iterator "pops batches from the output queue and transparently skips
+IDLE_DATA sentinels" (section 2.1); every rank sees the same number of steps (P:40,
+reading U26: step k = slot k of every rank).  Here a collated plan already sits in four flat arenas;
+this module only builds zero-copy ``[count, width]`` tensor VIEWS of them, per step and rank, and
+leaves out IDLE slots.  No arithmetic of the method happens here (plumbing).
+"""
+from __future__ import annotations
+
+from typing import Dict, Iterator, List, Optional
+
+
+class StepBatches:
+    """``for step in StepBatches(out, info, n_ranks): step[r] -> batch dict or None (IDLE)``.
+
+    ``out`` is an ``OutputBuffers`` filled by odb_collate / odb_run (device or pinned host).  The
+    per-slot tables are read back once (a few KB).  ``weights`` (optional) is the fp64 tensor written
+    by odb_loss_weights: each batch then carries its ``loss_weight`` w_{r,k} (Eq. 2).
+    """
+
+    def __init__(self, out, info, n_ranks: int, weights=None):
+        self.out = out
+        self.n_ranks = int(n_ranks)
+        self.n_steps = int(info.n_steps)
+        tab = lambda name: out.table(name).cpu().tolist()
+        self._count = tab("grp_count")
+        self._width = tab("grp_width")
+        self._offset = tab("grp_offset")
+        self._valid = tab("grp_valid_tokens")
+        self._round = tab("grp_round")
+        self._sptr = tab("grp_sample_ptr")
+        self._step_valid = tab("step_valid_tokens")
+        self._step_samples = tab("step_samples")
+        self._weights = weights
+
+    def __len__(self) -> int:
+        return self.n_steps
+
+    def batch(self, rank: int, step: int) -> Optional[Dict]:
+        """The batch rank ``rank`` trains on at step ``step``; None for an IDLE slot."""
+        s = rank * self.n_steps + step
+        c, w = self._count[s], self._width[s]
+        if c == 0:
+            return None
+        o = self._offset[s]
+        view = lambda t: t[o:o + c * w].view(c, w)
+        b = dict(input_ids=view(self.out.input_ids), attention_mask=view(self.out.attention_mask),
+                 position_ids=view(self.out.position_ids), labels=view(self.out.labels),
+                 sample_ids=self.out.grp_sample_ids[self._sptr[s]:self._sptr[s + 1]], valid_tokens=self._valid[s],
+                 step_valid_tokens=self._step_valid[step], step_samples=self._step_samples[step],
+                 round=self._round[s], rank=rank, step=step)
+        if self._weights is not None:
+            b["loss_weight"] = self._weights[s]
+        return b
+
+    def __iter__(self) -> Iterator[List[Optional[Dict]]]:
+        for k in range(self.n_steps):
+            yield [self.batch(r, k) for r in range(self.n_ranks)]
+
+    def rank_iter(self, rank: int) -> Iterator[Dict]:
+        """What one rank's training loop sees: its real batches in step order, IDLE slots skipped."""
+        for k in range(self.n_steps):
+            b = self.batch(rank, k)
+            if b is not None:
+                yield b

@@ -327,3 +327,38 @@ def test_loss_weights_bit_exact(P, oracle, case):
             assert np.array_equal(got.view(np.uint64), want.view(np.uint64)), (case, mode, np.abs(got - want).max())
         with pytest.raises(P.OdbError):
             P.odb_loss_weights(ctx.h, 7, w)
+
+
+def test_step_batches_views(P, oracle):
+    """StepBatches: zero-copy [count, width] views per step and rank, IDLE slots skipped, against
+    the oracle's per-slot collation; the join-mode identity contract seen through the iterator (Thm 1)."""
+    import torch
+    wl = I.protocol_workload("empty_rank", 3)
+    plan, ref = oracle.run_workload(wl)
+    dw = Par.DeviceWorkload(wl)
+    info, out, _ = Par.run_gpu(wl, dw, staged=False)
+    sb = P.StepBatches(out, info, wl.n_ranks)
+    assert len(sb) == plan.n_steps
+    toks = wl.tokens()
+    seen = [[] for _ in range(wl.n_ranks)]
+    n_idle = 0
+    for k, step in enumerate(sb):
+        assert len(step) == wl.n_ranks
+        for r, b in enumerate(step):
+            s = r * plan.n_steps + k
+            if plan.grp_count[s] == 0:
+                assert b is None
+                n_idle += 1
+                continue
+            want = plan.collate_slot(s, toks, wl.sample_ptr[:-1], wl.span_ptr, wl.span_lo, wl.span_hi)
+            for name in ("input_ids", "attention_mask", "position_ids", "labels"):
+                assert b[name].shape == want[name].shape
+                assert b[name].data_ptr() == getattr(out, name).data_ptr() + int(plan.grp_offset[s]) * b[name].element_size()
+                assert np.array_equal(b[name].cpu().numpy(), want[name]), (name, r, k)
+            assert b["valid_tokens"] == want["valid"] and b["step_samples"] == int(plan.step_samples[k])
+            seen[r].extend(b["sample_ids"].cpu().tolist())
+    assert n_idle > 0
+    for r in range(wl.n_ranks):   # every id exactly once per rank (Thm 1 P:46)
+        n_r = int(wl.rank_ptr[r + 1] - wl.rank_ptr[r])
+        assert sorted(seen[r]) == list(range(n_r))
+        assert sum(1 for _ in sb.rank_iter(r)) == int((plan.grp_count.reshape(wl.n_ranks, -1)[r] > 0).sum())
