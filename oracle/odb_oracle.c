@@ -348,9 +348,30 @@ void oracle_plan_free(oracle_plan *p) {
  * C.3 the round loop (section 2.1; section 2.3; Alg. 1; App. C.1 with Q_r = {}).
  * Returns NULL with *err = 2 when some length < 1, *err = 1 on bad arguments.
  */
+oracle_plan *oracle_plan_run_sched(int32_t R, int64_t budget, int32_t rule, int32_t join_mode, int64_t sample_quota,
+                                   int64_t emitted_so_far, int32_t buffer_size, int32_t slot_capacity,
+                                   const int32_t *lengths, const int64_t *rank_ptr, const int64_t *avail_sched,
+                                   int32_t n_sched, int32_t *err);
+
 oracle_plan *oracle_plan_run(int32_t R, int64_t budget, int32_t rule, int32_t join_mode, int64_t sample_quota,
                              int64_t emitted_so_far, int32_t buffer_size, int32_t slot_capacity,
                              const int32_t *lengths, const int64_t *rank_ptr, int32_t *err) {
+    return oracle_plan_run_sched(R, budget, rule, join_mode, sample_quota, emitted_so_far, buffer_size, slot_capacity,
+                                 lengths, rank_ptr, NULL, 0, err);
+}
+
+/*
+ * The round loop with an ARRIVAL SCHEDULE (the asynchronous side of App. C.1: a sampler view sits in the
+ * worker queue Q_r until the workers deliver it): in round j < n_sched only the first avail_sched[j*R + r]
+ * views of rank r's stream have arrived and may be drained into B_r; from round n_sched on everything has.
+ * A rank whose buffer is empty while views are still pending advertises n_groups = 0 ("insufficient data",
+ * P:52), is not finished, and gets IDLE slots like any rank outside A; a round in which no rank has a group
+ * is a SKIP round (no emission; Lemma 2: skip rounds are finite because the schedule is).
+ */
+oracle_plan *oracle_plan_run_sched(int32_t R, int64_t budget, int32_t rule, int32_t join_mode, int64_t sample_quota,
+                                   int64_t emitted_so_far, int32_t buffer_size, int32_t slot_capacity,
+                                   const int32_t *lengths, const int64_t *rank_ptr, const int64_t *avail_sched,
+                                   int32_t n_sched, int32_t *err) {
     *err = 0;
     if (R < 1 || budget < 1 || (rule != 0 && rule != 1) || buffer_size < 0 || slot_capacity < 0) {
         *err = 1;
@@ -392,9 +413,14 @@ oracle_plan *oracle_plan_run(int32_t R, int64_t budget, int32_t rule, int32_t jo
         int32_t n_finished = 0;
         for (int32_t r = 0; r < R; ++r) {
             int64_t n_r = rank_ptr[r + 1] - rank_ptr[r];
-            while ((buffer_size == 0 || buf[r].n < buffer_size) && pos[r] < n_r) ivec_push(&buf[r], (int32_t)pos[r]++);
+            int64_t arrived = n_r; /* views of R_r the workers have delivered so far */
+            if (avail_sched && round < n_sched && avail_sched[(int64_t)round * R + r] < n_r)
+                arrived = avail_sched[(int64_t)round * R + r] > 0 ? avail_sched[(int64_t)round * R + r] : 0;
+            while ((buffer_size == 0 || buf[r].n < buffer_size) && pos[r] < arrived) ivec_push(&buf[r], (int32_t)pos[r]++);
             Sn[r] = buf[r].n;
-            if (Sn[r] == 0) n_finished++; /* status -1 "finished" (U12) */
+            /* status -1 "finished": nothing buffered and nothing pending; an empty buffer with views
+             * still pending is status 0 "insufficient data" (unreachable without a schedule; U12) */
+            if (Sn[r] == 0 && pos[r] == n_r) n_finished++;
         }
         /* termination predicates computed from the shared status (Thm 3 proof P:341) */
         if (join_mode && n_finished == R) {
@@ -423,6 +449,14 @@ oracle_plan *oracle_plan_run(int32_t R, int64_t budget, int32_t rule, int32_t jo
                 group_maxfit_asc(len_r, buf[r].v, (int32_t)buf[r].n, budget, &cand[r]);
             Gn[r] = cand[r].n; /* pre-alignment candidate count (U23) */
             for (int64_t j = 0; j < cand[r].n; ++j) cand[r].g[j].orig = (int32_t)j;
+        }
+        /* skip round: no rank produced a group (all "insufficient data" or finished): nothing is emitted */
+        int any_active = 0;
+        for (int32_t r = 0; r < R; ++r)
+            if (Gn[r] > 0) any_active = 1;
+        if (!any_active) {
+            round++;
+            continue;
         }
         /* Eq. 3 */
         int64_t T = oracle_target_groups(Gn, Sn, R, slot_capacity);

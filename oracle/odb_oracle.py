@@ -61,6 +61,8 @@ def lib():
         L.oracle_target_group_size.argtypes = [i64, i64]
         L.oracle_plan_run.restype = vp
         L.oracle_plan_run.argtypes = [i32, i64, i32, i32, i64, i64, i32, i32, pi32, pi64, pi32]
+        L.oracle_plan_run_sched.restype = vp
+        L.oracle_plan_run_sched.argtypes = [i32, i64, i32, i32, i64, i64, i32, i32, pi32, pi64, pi64, i32, pi32]
         L.oracle_plan_free.restype = None
         L.oracle_plan_free.argtypes = [vp]
         L.oracle_plan_scalar.restype = i64
@@ -150,16 +152,24 @@ class OraclePlan:
     """Result of the round loop (grouping + alignment) for R ranks; owns the C object."""
 
     def __init__(self, lengths, rank_ptr, *, budget, rule=0, join_mode=1, sample_quota=0, emitted_so_far=0,
-                 buffer_size=0, slot_capacity=0, **_ignored):
+                 buffer_size=0, slot_capacity=0, avail_schedule=None, **_ignored):
         self.lengths = np.ascontiguousarray(lengths, dtype=np.int32)
         self.rank_ptr = np.ascontiguousarray(rank_ptr, dtype=np.int64)
         self.R = len(self.rank_ptr) - 1
         err = ctypes.c_int32(0)
         lens = self.lengths if len(self.lengths) else np.zeros(1, dtype=np.int32)
-        self._h = lib().oracle_plan_run(self.R, int(budget), int(rule), int(join_mode), int(sample_quota),
-                                        int(emitted_so_far), int(buffer_size), int(slot_capacity),
-                                        _p(lens, ctypes.c_int32), _p(self.rank_ptr, ctypes.c_int64),
-                                        ctypes.byref(err))
+        if avail_schedule is None:
+            self._h = lib().oracle_plan_run(self.R, int(budget), int(rule), int(join_mode), int(sample_quota),
+                                            int(emitted_so_far), int(buffer_size), int(slot_capacity),
+                                            _p(lens, ctypes.c_int32), _p(self.rank_ptr, ctypes.c_int64),
+                                            ctypes.byref(err))
+        else:  # [n_sched, R]: views of each rank that have arrived by round j (see oracle_plan_run_sched)
+            sched = np.ascontiguousarray(avail_schedule, dtype=np.int64).reshape(-1, self.R)
+            sp = sched if sched.size else np.zeros(1, np.int64)
+            self._h = lib().oracle_plan_run_sched(self.R, int(budget), int(rule), int(join_mode), int(sample_quota),
+                                                  int(emitted_so_far), int(buffer_size), int(slot_capacity),
+                                                  _p(lens, ctypes.c_int32), _p(self.rank_ptr, ctypes.c_int64),
+                                                  _p(sp, ctypes.c_int64), int(sched.shape[0]), ctypes.byref(err))
         self.err = err.value
         if not self._h:
             raise ValueError("oracle_plan_run failed with status %d" % self.err)
@@ -262,10 +272,10 @@ class OraclePlan:
                     grp_valid_tokens=gv[:self.n_slots], step_valid_tokens=sv[:self.n_steps])
 
 
-def run_workload(wl, tokens=None, *, collate: bool = True):
+def run_workload(wl, tokens=None, *, collate: bool = True, avail_schedule=None):
     """Plan (and optionally collate) an ``odb_inputs.Workload``.  Returns (plan, outputs-or-None)."""
     p = wl.params
-    plan = OraclePlan(wl.lengths, wl.rank_ptr, **p)
+    plan = OraclePlan(wl.lengths, wl.rank_ptr, avail_schedule=avail_schedule, **p)
     if not collate:
         return plan, None
     if tokens is None:

@@ -88,13 +88,15 @@ def test_config4_highcv_longtail(P, oracle, rule, join):
         assert plan.stop_reason == 2 and Q <= plan.samples_emitted <= Q + int(plan.step_samples.max())
 
 
-@pytest.mark.parametrize("cv,budget", [(1.0, 65536), (2.5, 16384), (0.3, 262144)])
+@pytest.mark.parametrize("cv,budget", I.config5_cells())
 def test_config5_sweep_cells(P, oracle, cv, budget):
+    """All nine (CV, budget) cells of BASELINE.json configs[4] at full size (32 x 32768 samples, ~2.1e9 tokens)."""
     _sampled_parity(oracle, I.make_workload(4, cv=cv, budget=budget), n_sample=24)
 
 
-def test_config5_maxfit(P, oracle):
-    _sampled_parity(oracle, I.make_workload(4, cv=1.0, budget=65536, rule=1), n_sample=16)
+@pytest.mark.parametrize("cv,budget", [(1.0, 65536), (2.5, 16384), (0.3, 262144)])
+def test_config5_maxfit(P, oracle, cv, budget):
+    _sampled_parity(oracle, I.make_workload(4, cv=cv, budget=budget, rule=1), n_sample=16)
 
 
 # ---- protocol tests (multi-round, overflow, IDLE, empty ranks, quota) --------------------------
