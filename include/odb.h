@@ -148,6 +148,17 @@ ODB_API int odb_reset(odb_ctx *ctx);
  * h_rank_ptr[R] <= max_samples_total) for the following rounds.  Asynchronous. */
 ODB_API int odb_form_groups(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, void *stream);
 
+/* Arrival state of the streams (the asynchronous side of App. C.1: a sampler view sits in the
+ * worker queue until the workers deliver it).  h_arrived[r] = how many views of rank r's stream (in
+ * sampler order) have arrived so far; only those can be drained into the window by the next
+ * odb_form_groups.  A rank whose window is empty while views are pending advertises n_groups = 0
+ * ("insufficient data"): it is not finished and gets IDLE slots; a round in which no rank has a
+ * group is a skip round (T_grp = 0, nothing emitted; Lemma 2) -- the caller must let arrivals
+ * progress, or the loop never terminates.  NULL = everything has arrived (the default after create /
+ * reset, and what odb_run uses).  Values must not decrease.  Call between rounds only (before the first
+ * odb_form_groups or after odb_round_status; ODB_ERR_STATE otherwise).  h_arrived: host, n_ranks entries. */
+ODB_API int odb_set_available(odb_ctx *ctx, const int64_t *h_arrived, void *stream);
+
 /* Second half (section 2.3, Alg. 1): T_grp by an on-device reduction over the R ranks, split /
  * overflow, IDLE slots, step totals, the non-join quota cut, leftovers.  Asynchronous. */
 ODB_API int odb_align(odb_ctx *ctx, void *stream);

@@ -81,6 +81,7 @@ SYMBOLS = {
     "odb_reset": (_i32, [_vp]),
     "odb_form_groups": (_i32, [_vp, _vp, _P(_i64), _vp]),
     "odb_align": (_i32, [_vp, _vp]),
+    "odb_set_available": (_i32, [_vp, _P(_i64), _vp]),
     "odb_round_status": (_i32, [_vp, _P(_i32), _P(_i32)]),
     "odb_plan_query": (_i32, [_vp, _P(odb_plan_info)]),
     "odb_collate": (_i32, [_vp, _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _vp]),
@@ -198,6 +199,16 @@ def odb_form_groups(ctx: int, d_lengths, h_rank_ptr, stream=None) -> None:
     rp = _host_i64(h_rank_ptr)
     _check(load().odb_form_groups(ctx, _ptr(d_lengths), rp.ctypes.data_as(_P(_i64)), _stream(stream)),
            "odb_form_groups", ctx)
+
+
+def odb_set_available(ctx: int, h_arrived, stream=None) -> None:
+    """Views of each rank's stream that have arrived so far (None = everything)."""
+    if h_arrived is None:
+        rc = load().odb_set_available(ctx, None, _stream(stream))
+    else:
+        a = _host_i64(h_arrived)
+        rc = load().odb_set_available(ctx, a.ctypes.data_as(_P(_i64)), _stream(stream))
+    _check(rc, "odb_set_available", ctx)
 
 
 def odb_align(ctx: int, stream=None) -> None:
@@ -408,12 +419,18 @@ class Odb:
         except Exception:
             pass
 
-    def plan(self, d_lengths, h_rank_ptr, stream=None) -> odb_plan_info:
-        """The round loop (odb_form_groups / odb_align / odb_round_status until done) + odb_plan_query."""
+    def plan(self, d_lengths, h_rank_ptr, stream=None, avail_schedule=None) -> odb_plan_info:
+        """The round loop (odb_form_groups / odb_align / odb_round_status until done) + odb_plan_query.
+        ``avail_schedule[j][r]`` (optional) = views of rank r that have arrived by round j; after the
+        schedule everything has (odb_set_available)."""
         odb_reset(self.h)
         done = 0
         self.round_T = []
+        j = 0
         while not done:
+            if avail_schedule is not None:
+                odb_set_available(self.h, avail_schedule[j] if j < len(avail_schedule) else None, stream)
+                j += 1
             odb_form_groups(self.h, d_lengths, h_rank_ptr, stream)
             odb_align(self.h, stream)
             done, T = odb_round_status(self.h)

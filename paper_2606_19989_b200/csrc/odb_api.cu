@@ -74,6 +74,8 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->emit_cur);
     cudaFree(c->G);
     cudaFree(c->S);
+    cudaFree(c->F);
+    cudaFree(c->d_arrived);
     cudaFree(c->d_rec);
     cudaFree(c->d_tot);
     cudaFree(c->d_tile_counter);
@@ -186,6 +188,8 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->emit_cur, R);
     if (e == cudaSuccess) e = dev_alloc(&c->G, R);
     if (e == cudaSuccess) e = dev_alloc(&c->S, R);
+    if (e == cudaSuccess) e = dev_alloc(&c->F, R);
+    if (e == cudaSuccess) e = dev_alloc(&c->d_arrived, R);
     if (e == cudaSuccess) e = dev_alloc(&c->d_rec, 1);
     if (e == cudaSuccess) e = dev_alloc(&c->d_tot, 1);
     if (e == cudaSuccess) e = dev_alloc(&c->d_tile_counter, R + 1);  // one work counter per pipelined launch
@@ -224,6 +228,7 @@ int odb_reset(odb_ctx *c) {
     c->stop_reason = 0;
     c->info_valid = false;
     c->collated = false;
+    c->arrived_set = false;
     c->d_lengths = nullptr;
     c->ev_valid = false;
     return ODB_OK;
@@ -269,6 +274,8 @@ static int begin_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank
     c->d_lengths = d_lengths;
     CU(c, cudaSetDevice(c->device));
     CU(c, cudaMemcpyAsync(c->d_rank_ptr, c->h_rank_ptr.data(), (R + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    if (!c->arrived_set) c->h_arrived.assign((size_t)R, 0x7fffffff);  // everything has arrived
+    CU(c, cudaMemcpyAsync(c->d_arrived, c->h_arrived.data(), (size_t)R * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(c, launch_begin(c, st));  // rank state, emit positions, step totals, length validation
     c->n_finished = 0;
     for (int r = 0; r < R; ++r)
@@ -331,6 +338,24 @@ int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_
     if (c->world_ranks) CU(c, launch_pack_summary(c, st));
     c->state = 1;
     c->last_T = -1;
+    return ODB_OK;
+}
+
+int odb_set_available(odb_ctx *c, const int64_t *h_arrived, void *stream) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (c->state != 0 && c->state != 3) return ODB_ERR_STATE;  // between rounds only
+    const int R = c->prm.n_ranks;
+    c->h_arrived.resize((size_t)R);
+    for (int r = 0; r < R; ++r) {
+        const int64_t a = h_arrived ? h_arrived[r] : 0x7fffffffll;
+        c->h_arrived[r] = (int32_t)std::min<int64_t>(std::max<int64_t>(a, 0), 0x7fffffffll);
+    }
+    c->arrived_set = true;
+    if (c->state == 3) {  // mid-run: the next odb_form_groups reads the device copy
+        CU(c, cudaSetDevice(c->device));
+        CU(c, cudaMemcpyAsync(c->d_arrived, c->h_arrived.data(), (size_t)R * sizeof(int32_t), cudaMemcpyHostToDevice,
+                              (cudaStream_t)stream));
+    }
     return ODB_OK;
 }
 

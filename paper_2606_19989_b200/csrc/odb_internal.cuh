@@ -204,6 +204,10 @@ struct odb_ctx {
     int32_t *agpos = nullptr, *agcnt = nullptr, *agoff = nullptr, *agorg = nullptr;  // n_max + R
     int32_t *left_ids = nullptr, *emit_ids = nullptr;              // n_max
     int32_t *n_left = nullptr, *fetch_pos = nullptr, *emit_cur = nullptr, *G = nullptr, *S = nullptr;  // R
+    int32_t *F = nullptr;          // R: 1 = the rank is finished (status -1)
+    int32_t *d_arrived = nullptr;  // R: views of the rank's stream that have arrived (odb_set_available)
+    std::vector<int32_t> h_arrived;
+    bool arrived_set = false;
     odb::RoundRec *d_rec = nullptr;
     odb::RoundRec *h_rec = nullptr;  // pinned
     odb::PlanTotals *d_tot = nullptr;

@@ -89,8 +89,8 @@ __device__ __forceinline__ void block_bitonic(uint64_t *k, int n2) {
 }
 
 // window size of rank r this round: leftovers + un-fetched samples, capped by buffer_size (A0)
-__device__ __forceinline__ int window_size(int n_left, int fetch_pos, int n_r, int buffer_size) {
-    long long avail = (long long)n_left + (long long)(n_r - fetch_pos);
+__device__ __forceinline__ int window_size(int n_left, int fetch_pos, int n_arrived, int buffer_size) {
+    long long avail = (long long)n_left + (long long)max(n_arrived - fetch_pos, 0);
     if (buffer_size > 0 && avail > buffer_size) avail = buffer_size;
     return (int)avail;
 }
@@ -101,8 +101,8 @@ __device__ __forceinline__ int window_size(int n_left, int fetch_pos, int n_r, i
 // ---------------------------------------------------------------------------------------------
 __global__ void k_begin(const int32_t *__restrict__ len, int64_t n, int R, int32_t *__restrict__ n_left,
                         int32_t *__restrict__ fetch_pos, int32_t *__restrict__ emit_cur, int32_t *__restrict__ G,
-                        int32_t *__restrict__ S, int32_t *__restrict__ emit_pos, int32_t *__restrict__ step_samples,
-                        int64_t step_cap, RoundRec *rec) {
+                        int32_t *__restrict__ S, int32_t *__restrict__ F, int32_t *__restrict__ emit_pos,
+                        int32_t *__restrict__ step_samples, int64_t step_cap, RoundRec *rec) {
     int bad = 0;
     const int64_t bound = max(n, max((int64_t)R, step_cap));
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < bound; i += (int64_t)gridDim.x * blockDim.x) {
@@ -112,6 +112,7 @@ __global__ void k_begin(const int32_t *__restrict__ len, int64_t n, int R, int32
             emit_cur[i] = 0;
             G[i] = 0;
             S[i] = 0;
+            F[i] = 0;
         }
         if (i < n) {
             emit_pos[i] = -1;
@@ -129,16 +130,19 @@ __global__ void k_begin(const int32_t *__restrict__ len, int64_t n, int R, int32
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kSortThreads)
 k_chunk_sort(const int32_t *__restrict__ len, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ n_left,
-             const int32_t *__restrict__ fetch_pos, const int32_t *__restrict__ left_ids, int buffer_size,
-             uint64_t *__restrict__ keys_out, int32_t *__restrict__ S_out, RoundRec *rec) {
+             const int32_t *__restrict__ fetch_pos, const int32_t *__restrict__ left_ids,
+             const int32_t *__restrict__ arrived, int buffer_size, uint64_t *__restrict__ keys_out,
+             int32_t *__restrict__ S_out, int32_t *__restrict__ F_out, RoundRec *rec) {
     __shared__ uint64_t sk[kSortChunk];
     const int r = blockIdx.y;
     const int64_t base = rank_ptr[r];
     const int n_r = (int)(rank_ptr[r + 1] - base);
     const int nl = n_left[r], fp = fetch_pos[r];
-    const int S = window_size(nl, fp, n_r, buffer_size);
+    // only the views the workers have delivered so far can be drained (App. C.1; odb_set_available)
+    const int S = window_size(nl, fp, min(n_r, arrived[r]), buffer_size);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         S_out[r] = S;
+        F_out[r] = (S == 0 && fp >= n_r) ? 1 : 0;  // status -1 "finished"; S == 0 with views pending is status 0
         if (r == 0) rec->n_finished = 0;  // counted again by this round's commit
     }
     const int c0 = blockIdx.x * kSortChunk;
@@ -375,7 +379,7 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
             atomicMax(&s_maxG, g);
             if (sq > 0) atomicMin(&s_minS, sq);
         }
-        if (sq == 0) atomicAdd(&s_nfin, 1);  // status -1 "finished"
+        if (sq < 0) atomicAdd(&s_nfin, 1);  // status -1 "finished", encoded by k_pack_summary
     }
     __syncthreads();
     if (gs_world) {
@@ -393,6 +397,7 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
     if (slot_capacity > 0 && T > slot_capacity) T = slot_capacity;  // C+min (same C on every rank)
     if (T > s_minS) T = s_minS;                                     // S+min
     if (T < 1) T = 1;
+    if (s_maxG == 0) T = 0;  // A is empty: a skip round, nothing is emitted (Lemma 2)
     if (r == 0 && threadIdx.x == 0) rec->T = T;
     const int Gr = G_arr[r];
     if (Gr == 0) return;  // finished rank: IDLE slots are written by the commit kernel
@@ -530,7 +535,8 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
             st_round[idx] = round;
             st_origin[idx] = step_base + k;
         }
-        if (threadIdx.x == 0) atomicAdd(&rec->n_finished, 1);
+        // finished (nothing buffered, nothing pending) or merely waiting for the workers (status 0)?
+        if (threadIdx.x == 0 && n_left[r] == 0 && fetch_pos[r] >= n_r) atomicAdd(&rec->n_finished, 1);
         return;
     }
     const int64_t jb = base + r;
@@ -814,7 +820,7 @@ cudaError_t launch_begin(odb_ctx *c, cudaStream_t st) {
     const int64_t bound = std::max<int64_t>(std::max<int64_t>(c->n_total, R), step_cap);
     int blocks = (int)std::min<int64_t>((bound + 1023) / 1024, (int64_t)c->sm_count * 4);
     k_begin<<<std::max(blocks, 1), 256, 0, st>>>(c->d_lengths, c->n_total, R, c->n_left, c->fetch_pos, c->emit_cur, c->G,
-                                                c->S, c->emit_pos, c->step_samples.p, step_cap, c->d_rec);
+                                                c->S, c->F, c->emit_pos, c->step_samples.p, step_cap, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
@@ -837,7 +843,7 @@ cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st) {
     if (maxS == 0) return cudaSuccess;
     const int chunks = (maxS + kSortChunk - 1) / kSortChunk;
     k_chunk_sort<<<dim3(chunks, R), kSortThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos, c->left_ids,
-                                                          c->prm.buffer_size, c->keyA, c->S, c->d_rec);
+                                                          c->d_arrived, c->prm.buffer_size, c->keyA, c->S, c->F, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     uint64_t *src = c->keyA, *dst = c->keyB;
     for (int64_t w = kSortChunk; w < maxS; w *= 2) {
@@ -905,19 +911,19 @@ cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st) { return launch_align
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st) { return launch_commit_kernel(c, st); }
 
 // distributed mode: the local ranks' (G_r, S_r) pairs, the message of the per-round all_gather
-__global__ void k_pack_summary(int R, const int32_t *__restrict__ G, const int32_t *__restrict__ S, int32_t *__restrict__ gs,
-                               RoundRec *rec) {
+__global__ void k_pack_summary(int R, const int32_t *__restrict__ G, const int32_t *__restrict__ S,
+                               const int32_t *__restrict__ F, int32_t *__restrict__ gs, RoundRec *rec) {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q < R) {
         gs[2 * q] = G[q];
-        gs[2 * q + 1] = S[q];
+        gs[2 * q + 1] = F[q] ? -1 : S[q];  // -1 = "finished"; 0 = "insufficient data"
     }
     if (q == 0) rec->done = 0;
 }
 
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
-    k_pack_summary<<<(R + 127) / 128, 128, 0, st>>>(R, c->G, c->S, c->gs_local, c->d_rec);
+    k_pack_summary<<<(R + 127) / 128, 128, 0, st>>>(R, c->G, c->S, c->F, c->gs_local, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

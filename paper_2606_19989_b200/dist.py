@@ -78,6 +78,9 @@ class CudaEngine:
     def dist_config(self, world_ranks: int, rank_offset: int, world_max_window: int):
         B.odb_dist_config(self.ctx.h, world_ranks, rank_offset, world_max_window)
 
+    def set_available(self, h_arrived):
+        B.odb_set_available(self.ctx.h, h_arrived, self.stream)
+
     def form_groups(self):
         B.odb_form_groups(self.ctx.h, self.d_lengths, self.h_rank_ptr, self.stream)
 
@@ -113,12 +116,17 @@ class CudaEngine:
 
 
 # ---- the protocol ------------------------------------------------------------------------------
-def plan_protocol(engine, world_ranks: int, rank_offset: int) -> Generator[Request, object, tuple]:
-    """Round loop of one process.  Returns (plan info of the local ranks, [T_grp of every emitting round])."""
+def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=None) -> Generator[Request, object, tuple]:
+    """Round loop of one process.  Returns (plan info of the local ranks, [T_grp of every emitting round]).
+    ``avail_schedule[j]`` (optional): arrived views of the LOCAL ranks at round j (odb_set_available)."""
     wmax = yield ("max_int", int(engine.local_max_window()))
     engine.dist_config(world_ranks, rank_offset, int(wmax))
     round_T: List[int] = []
+    j = 0
     while True:
+        if avail_schedule is not None:
+            engine.set_available(avail_schedule[j] if j < len(avail_schedule) else None)
+            j += 1
         engine.form_groups()
         world, local = engine.summary()
         yield ("all_gather", world, local)                 # the per-round metadata exchange (P:52)

@@ -49,7 +49,8 @@ class OracleEngine:
             S = len(self.buf[r])
             g = self.o.group_window(self.p["rule"], self.p["budget"], self.lens[r], np.array(self.buf[r], np.int32)) if S else []
             self.cand.append(g)
-            self.local[2 * r], self.local[2 * r + 1] = len(g), S
+            # S encoded as -1 when the rank is finished (nothing buffered, nothing pending), as k_pack_summary does
+            self.local[2 * r], self.local[2 * r + 1] = len(g), (-1 if (S == 0 and self.pos[r] == n_r) else S)
         self.window = torch.zeros(self.bound, dtype=torch.int32)
         self.done = False
         self.T = 0
@@ -59,7 +60,7 @@ class OracleEngine:
 
     def align(self):
         G, S = self.world[0::2].numpy().astype(np.int64), self.world[1::2].numpy().astype(np.int64)
-        n_fin = int((S == 0).sum())
+        n_fin = int((S < 0).sum())
         self.done = (n_fin == self.W) if self.p["join_mode"] else (n_fin > 0)
         if self.done:
             return

@@ -44,7 +44,7 @@ def gpu_params(wl):
                          ignore_index=p["ignore_index"], shift_labels=p["shift_labels"])
 
 
-def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL):
+def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL, avail_schedule=None):
     """Returns (info, OutputBuffers, round_T).  staged=True uses form_groups/align/round_status/
     plan_query/collate; staged=False uses odb_run (two calls: the first sizes the outputs)."""
     import torch
@@ -52,7 +52,7 @@ def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL):
     dw = dw or DeviceWorkload(wl)
     with P.Odb(gpu_params(wl), max(wl.n_samples, 1)) as ctx:
         if staged:
-            info = ctx.plan(dw.lengths, wl.rank_ptr)
+            info = ctx.plan(dw.lengths, wl.rank_ptr, avail_schedule=avail_schedule)
             round_T = list(ctx.round_T)
             out = P.OutputBuffers.for_plan(wl.n_ranks, info, dw.device, fill=fill)
             P.odb_collate(ctx.h, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out.struct)

@@ -114,6 +114,43 @@ def test_lockstep_processes_match_whole_job_oracle(P, oracle, name, n_proc):
             e.close()
 
 
+def test_lockstep_with_arrival_schedule(P, oracle):
+    """Status 0 / -1 travel through the gathered summary (S encoded as -1 when finished): two contexts with
+    a random arrival schedule equal the whole-job oracle run with the same schedule."""
+    import torch
+    from paper_2606_19989_b200 import dist as D
+    from tests.test_oracle_arrival import _random_schedule
+    for seed, join in ((0, 1), (1, 1), (2, 0), (3, 1)):
+        wl = I.protocol_workload("unequal" if seed % 2 else "overflow_multiround", seed, join_mode=join)
+        rng = np.random.default_rng(50 + seed)
+        sched = _random_schedule(rng, wl, 7)
+        plan, _ = oracle.run_workload(wl, collate=False, avail_schedule=sched)
+        R, K = wl.n_ranks, plan.n_steps
+        rl = R // 2
+        parts = I.split_ranks(wl, 2)
+        dws = [Par.DeviceWorkload(w) for w in parts]
+        engines = [D.CudaEngine(Par.gpu_params(w), max(w.n_samples, 1), dw.lengths, w.rank_ptr) for w, dw in zip(parts, dws)]
+        try:
+            res = D.run_lockstep([D.plan_protocol(e, R, p * rl, [row[p * rl:(p + 1) * rl] for row in sched])
+                                  for p, e in enumerate(engines)])
+            for p, (e, dw) in enumerate(zip(engines, dws)):
+                info, round_T = res[p]
+                assert round_T == plan.round_T.tolist()
+                assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason)
+                out = P.OutputBuffers.for_plan(rl, info, dw.device)
+                e.collate(dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out)
+                torch.cuda.synchronize()
+                s0, s1 = p * rl * K, (p + 1) * rl * K
+                q0, q1 = int(plan.grp_sample_ptr[s0]), int(plan.grp_sample_ptr[s1])
+                assert np.array_equal(out.table("grp_count").cpu().numpy(), plan.grp_count[s0:s1])
+                assert np.array_equal(out.table("grp_round").cpu().numpy(), plan.grp_round[s0:s1])
+                assert np.array_equal(out.table("grp_sample_ids").cpu().numpy(), plan.grp_sample_ids[q0:q1])
+                assert np.array_equal(out.table("step_samples").cpu().numpy(), plan.step_samples)
+        finally:
+            for e in engines:
+                e.close()
+
+
 def test_single_process_nccl_world(P, oracle):
     """The torch.distributed driver itself (NCCL, world_size 1 -- the box has one GPU): the protocol
     with real collectives on the library's device buffers equals the oracle."""

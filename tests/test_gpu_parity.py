@@ -364,3 +364,50 @@ def test_step_batches_views(P, oracle):
         n_r = int(wl.rank_ptr[r + 1] - wl.rank_ptr[r])
         assert sorted(seen[r]) == list(range(n_r))
         assert sum(1 for _ in sb.rank_iter(r)) == int((plan.grp_count.reshape(wl.n_ranks, -1)[r] > 0).sum())
+
+
+# ---- arrival schedules: status 0 "insufficient data", skip rounds (App. C.1) ---------------
+def _sched_parity(oracle, wl, sched):
+    plan, ref = oracle.run_workload(wl, avail_schedule=sched)
+    info, out, round_T = Par.run_gpu(wl, staged=True, avail_schedule=sched)
+    Par.compare_plan(plan, info, out, round_T)
+    Par.compare_full(plan, ref, info, out)
+    return plan
+
+
+def test_arrival_fixture_e8(P, oracle):
+    from tests import _golden as G
+    g = G.load("e8_arrival.txt")
+    per_rank = [G.ints(x) for x in g["rank_lengths"].split("|")]
+    for join, key in ((1, "case1_schedule"), (0, "case1_schedule"), (1, "case3_schedule")):
+        wl = I.custom_workload("e8", per_rank, seed=1, budget=int(g["budget"]), join_mode=join)
+        plan = _sched_parity(oracle, wl, [G.ints(g[key])])
+        if key == "case3_schedule":
+            assert plan.n_rounds == 3 and plan.round_T.tolist() == [3]     # one skip round, one emitting, terminal
+
+
+def test_arrival_random_schedules(P, oracle):
+    from tests.test_oracle_arrival import _random_schedule
+    for seed in range(60):
+        rng = np.random.default_rng(1000 + seed)
+        wl = I.protocol_workload("fuzz", seed)
+        sched = _random_schedule(rng, wl, int(rng.integers(1, 12)))
+        try:
+            _sched_parity(oracle, wl, sched)
+        except AssertionError as e:
+            raise AssertionError("seed %d params %r sched %r: %s" % (seed, wl.params, sched.tolist(), e))
+    for kind in ("overflow_multiround", "unequal", "empty_rank"):
+        for rule in (0, 1):
+            rng = np.random.default_rng(7)
+            wl = I.protocol_workload(kind, 3, rule=rule)
+            _sched_parity(oracle, wl, _random_schedule(rng, wl, 9))
+
+
+def test_set_available_state_errors(P):
+    wl = I.make_workload(0)
+    dw = Par.DeviceWorkload(wl)
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        P.odb_set_available(ctx.h, [3, 5])
+        P.odb_form_groups(ctx.h, dw.lengths, wl.rank_ptr)
+        with pytest.raises(P.OdbError):       # inside a round
+            P.odb_set_available(ctx.h, [10, 10])
