@@ -486,8 +486,11 @@ oracle_plan *oracle_plan_run_sched(int32_t R, int64_t budget, int32_t rule, int3
                     s.origin = (int32_t)(step_base + k);
                 } else {
                     group g = cand[r].g[k];
-                    int64_t k0 = 0;
-                    while (cand[r].g[k0].orig != g.orig) k0++; /* first aligned group cut from the same candidate */
+                    /* first aligned group cut from the same candidate: such groups are adjacent (a split
+                     * singleton is inserted right after the group it came from, U5; groups kept by overflow
+                     * are distinct candidates), so walk back over the run */
+                    int64_t k0 = k;
+                    while (k0 > 0 && cand[r].g[k0 - 1].orig == g.orig) k0--;
                     s.origin = (int32_t)(step_base + k0);
                     s.ids = g.ids; /* ownership moves to the slot */
                     s.count = g.n;

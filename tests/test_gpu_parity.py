@@ -411,3 +411,51 @@ def test_set_available_state_errors(P):
         P.odb_form_groups(ctx.h, dw.lengths, wl.rank_ptr)
         with pytest.raises(P.OdbError):       # inside a round
             P.odb_set_available(ctx.h, [10, 10])
+
+
+# ---- maximum sizes ------------------------------------------------------------------------------
+def _big_slot_parity(oracle, wl, slots):
+    """Plan tables in full, the listed (large) slots element by element, any-size properties on the device."""
+    plan, _ = oracle.run_workload(wl, collate=False)
+    info, out, _ = Par.run_gpu(wl, staged=False)
+    Par.compare_plan(plan, info, out)
+    Par.compare_sampled_slots(wl, plan, out, slots(plan))
+    Par.device_self_consistency(info, out, wl.params["ignore_index"])
+    return plan
+
+
+def test_max_sizes_two_million_sample_windows(P, oracle):
+    """Two ranks, one window of 2 M samples each (sort: 9 merge passes; list ranking in global memory;
+    ~870 K steps, 1.7 M slots: the slot scan runs over hundreds of tiles), a few hundred splits."""
+    rng = np.random.default_rng(21)
+    wl = I.custom_workload("big_windows", [rng.integers(1, 41, 2_000_000), rng.integers(1, 41, 2_000_000)], 3,
+                           budget=64)
+    plan = _sampled_parity(oracle, wl, n_sample=32)
+    assert plan.n_steps > 500_000
+
+
+def test_max_sizes_many_ranks(P, oracle):
+    """4096 ranks x 0..96 samples, 26 rounds: the cross-rank reduction and the rank-major tables at a large R."""
+    rng = np.random.default_rng(22)
+    per = [rng.integers(8, 600, int(rng.integers(0, 97))) for _ in range(4096)]
+    wl = I.custom_workload("many_ranks", per, 4, budget=2048, buffer_size=32)
+    plan = _sampled_parity(oracle, wl, n_sample=32)
+    assert plan.n_rounds > 2
+
+
+def test_max_sizes_huge_budget(P, oracle):
+    """Budget 2^31 - 1: one group of 599,999 rows x 64 columns (3.8e7 elements; the longest sample is a
+    singleton, App. D step 1)."""
+    rng = np.random.default_rng(23)
+    wl = I.custom_workload("huge_budget", [rng.integers(1, 65, 600_000), rng.integers(1, 65, 1000)], 5,
+                           budget=2**31 - 1)
+    plan = _big_slot_parity(oracle, wl, lambda p: range(p.n_slots))
+    assert plan.n_steps == 2 and int(plan.grp_count.max()) == 599_999
+
+
+def test_max_sizes_huge_singleton(P, oracle):
+    """An over-budget singleton of 1.2e8 tokens (U10) under budget 1000: a one-row block 1.2e8 wide."""
+    wl = I.custom_workload("huge_singleton", [np.array([120_000_000, 7, 300, 300]), np.array([5, 6, 7, 8])], 6,
+                           budget=1000)
+    plan = _big_slot_parity(oracle, wl, lambda p: range(p.n_slots))
+    assert int(plan.grp_width.max()) == 120_000_000
