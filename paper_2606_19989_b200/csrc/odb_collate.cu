@@ -51,7 +51,7 @@ __global__ void k_row_desc(int n_steps, int64_t n_slots, const int64_t *__restri
     d.lo1 = ns > 1 ? span_lo[sp + 1] : 0;
     d.hi1 = ns > 1 ? span_hi[sp + 1] : 0;
     rows[q] = d;
-    row_sp[q] = sp;
+    if (ns > 2) row_sp[q] = sp;  // only read on the CSR path (more than two spans): skip the scattered 8-byte store
 }
 
 // ---------------------------------------------------------------------------------------------

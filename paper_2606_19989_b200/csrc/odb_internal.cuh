@@ -21,6 +21,7 @@ constexpr int kSortChunk = 4096;    // keys sorted in shared memory by one CTA (
 constexpr int kSortThreads = 512;
 constexpr int kMergeThreads = 256;
 constexpr int kRankThreads = 1024;  // one CTA per rank for A2..A8
+constexpr int kCommitParts = 4;     // CTAs per rank that share k_commit's scan-free fast path
 constexpr size_t kFormSmemLimit = 231424;  // dynamic shared memory of k_form_groups_smem (227 KB - static)
 constexpr int kAlignSmemKeys = 8192;       // overflow sort keys kept in shared memory by k_align
 constexpr int kFinThreads = 512;           // k_fin_scan: tile = kFinThreads * kFinItems slots
@@ -205,6 +206,7 @@ struct odb_ctx {
     int32_t *left_ids = nullptr, *emit_ids = nullptr;              // n_max
     int32_t *n_left = nullptr, *fetch_pos = nullptr, *emit_cur = nullptr, *G = nullptr, *S = nullptr;  // R
     int32_t *F = nullptr;          // R: 1 = the rank is finished (status -1)
+    int32_t *emit_snap = nullptr;  // R: emit_cur as seen by k_align (read by every CTA of k_commit)
     int32_t *d_arrived = nullptr;  // R: views of the rank's stream that have arrived (odb_set_available)
     std::vector<int32_t> h_arrived;
     bool arrived_set = false;

@@ -359,7 +359,8 @@ k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ ran
 __global__ void __launch_bounds__(kRankThreads)
 k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr, const int32_t *__restrict__ G_arr, int R,
         const int32_t *__restrict__ gs_world, int world_ranks, int join_mode, int slot_capacity, const int32_t *__restrict__ gpos, int32_t *__restrict__ agpos, int32_t *__restrict__ agcnt,
-        int32_t *__restrict__ agorg, uint64_t *ovf, int32_t *step_samples, int step_base, RoundRec *rec) {
+        int32_t *__restrict__ agorg, uint64_t *ovf, int32_t *step_samples, int step_base,
+        const int32_t *__restrict__ emit_cur, int32_t *__restrict__ emit_snap, RoundRec *rec) {
     extern __shared__ __align__(16) unsigned char al_smem[];
     __shared__ int s_maxG, s_minS, s_nfin;
     const int r = blockIdx.x;
@@ -401,6 +402,8 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
     if (r == 0 && threadIdx.x == 0) rec->T = T;
     const int Gr = G_arr[r];
     if (Gr == 0) return;  // finished rank: IDLE slots are written by the commit kernel
+    // k_commit runs several CTAs per rank and one of them advances emit_cur: they all read this snapshot
+    if (threadIdx.x == 0) emit_snap[r] = emit_cur[r];
     const int S = S_arr[r];
     const int64_t base = rank_ptr[r];
     const int64_t jb = base + r;
@@ -476,12 +479,16 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
          int32_t *__restrict__ st_real, int32_t *__restrict__ st_round, int32_t *__restrict__ st_origin,
          uint8_t *__restrict__ posflag,
          int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
-         int32_t *fetch_pos, int32_t *emit_cur, RoundRec *rec) {
+         int32_t *fetch_pos, int32_t *emit_cur, const int32_t *__restrict__ emit_snap, RoundRec *rec) {
     __shared__ int s_scan[34];
     __shared__ long long s_scan64[34];
     __shared__ int s_found;
     const int r = blockIdx.x;
+    // gridDim.y CTAs per rank share the fast path below; everything that needs a rank-wide scan, and all
+    // state updates, is done by part 0 alone
+    const int part = blockIdx.y, nparts = gridDim.y;
     if (rec->done) {  // distributed mode: this round was the terminal check
+        if (part != 0) return;
         if (r == 0 && threadIdx.x == 0) {
             rec->T_emit = 0;
             rec->quota_hit = 0;
@@ -511,11 +518,11 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
         }
         __syncthreads();
     }
-    if (r == 0) {  // round totals for the host
-        long long part = 0;
-        for (int k = threadIdx.x; k < T_emit; k += blockDim.x) part += step_samples[step_base + k];
+    if (r == 0 && part == 0) {  // round totals for the host
+        long long acc = 0;
+        for (int k = threadIdx.x; k < T_emit; k += blockDim.x) acc += step_samples[step_base + k];
         long long tot;
-        (void)block_excl_scan<long long>(part, s_scan64, tot);
+        (void)block_excl_scan<long long>(acc, s_scan64, tot);
         if (threadIdx.x == 0) {
             rec->T_emit = T_emit;
             rec->quota_hit = quota_hit;
@@ -527,6 +534,7 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
     const int64_t base = rank_ptr[r];
     const int n_r = (int)(rank_ptr[r + 1] - base);
     if (Gr == 0) {  // finished rank: IDLE slots (U14)
+        if (part != 0) return;
         for (int k = threadIdx.x; k < T_emit; k += blockDim.x) {
             int64_t idx = (int64_t)(step_base + k) * R + r;
             st_count[idx] = 0;
@@ -544,42 +552,81 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
     const int32_t *ap = agpos + jb, *ac = agcnt + jb;
     int32_t *ao = agoff + jb;
     uint8_t *pf = posflag + base;
-    const int cur = emit_cur[r];
+    const int cur = emit_snap[r];  // emit_cur[r] as k_align saw it (part 0 advances emit_cur below)
     // every sample of the window is emitted unless groups were dropped (overflow) or cut (quota)
     const bool all_emitted = (Gr <= T) && (T_emit == T);
-    if (!all_emitted)
-        for (int a = threadIdx.x; a < S; a += blockDim.x) pf[a] = 0;
-    int carry = 0;
-    for (int b0 = 0; b0 < T_emit; b0 += blockDim.x) {
-        int k = b0 + threadIdx.x;
-        int c = (k < T_emit) ? ac[k] : 0;
-        int tot;
-        int ex = block_excl_scan<int>(c, s_scan, tot) + carry;
-        if (k < T_emit) {
-            int64_t idx = (int64_t)(step_base + k) * R + r;
-            int p = ap[k];
+    int emitted_r;
+    if (all_emitted) {
+        // Fast path (no overflow, no quota cut): the aligned groups are consecutive runs of the sorted
+        // window in order, so the emit order IS the sorted order -- one coalesced pass over the samples,
+        // then one thread per group for the tables (short groups sum their lengths there; long ones are
+        // summed by a warp each).
+        const int tid = part * blockDim.x + threadIdx.x, nth = nparts * blockDim.x;
+#pragma unroll 4
+        for (int a = tid; a < S; a += nth) {
+            const int id = key_id(k_[a]);
+            emit_ids[base + cur + a] = id;
+            emit_pos[base + id] = cur + a;
+        }
+        for (int k = tid; k < T_emit; k += nth) {
+            const int p = ap[k], c = ac[k];
+            const int64_t idx = (int64_t)(step_base + k) * R + r;
             st_count[idx] = c;
             st_width[idx] = (int32_t)key_len(k_[p + c - 1]);  // rows ascending: the last row is the longest
             st_round[idx] = round;
             st_origin[idx] = step_base + agorg[jb + k];
-            ao[k] = cur + ex;
+            if (c <= 32) {
+                uint32_t sum = 0;  // count * max_len <= budget < 2^31, or a singleton
+                for (int j = 0; j < c; ++j) sum += key_len(k_[p + j]);
+                st_real[idx] = (int32_t)sum;
+            }
         }
-        carry += tot;
-    }
-    const int emitted_r = carry;
-    __syncthreads();
-    {  // copy ids and sum the lengths: one warp per group
+        const int lane = threadIdx.x & 31, w = tid >> 5, nw = nth >> 5;
+        for (int k = w; k < T_emit; k += nw) {
+            const int c = ac[k];
+            if (c <= 32) continue;
+            const int p = ap[k];
+            uint32_t sum = 0;
+            for (int j = lane; j < c; j += 32) sum += key_len(k_[p + j]);
+            sum = __reduce_add_sync(ODB_FULL_MASK, sum);
+            if (lane == 0) st_real[(int64_t)(step_base + k) * R + r] = (int32_t)sum;
+        }
+        emitted_r = S;
+        if (part != 0) return;
+    } else {
+        if (part != 0) return;
+        for (int a = threadIdx.x; a < S; a += blockDim.x) pf[a] = 0;
+        int carry = 0;
+        for (int b0 = 0; b0 < T_emit; b0 += blockDim.x) {
+            int k = b0 + threadIdx.x;
+            int c = (k < T_emit) ? ac[k] : 0;
+            int tot;
+            int ex = block_excl_scan<int>(c, s_scan, tot) + carry;
+            if (k < T_emit) {
+                int64_t idx = (int64_t)(step_base + k) * R + r;
+                int p = ap[k];
+                st_count[idx] = c;
+                st_width[idx] = (int32_t)key_len(k_[p + c - 1]);
+                st_round[idx] = round;
+                st_origin[idx] = step_base + agorg[jb + k];
+                ao[k] = cur + ex;
+            }
+            carry += tot;
+        }
+        emitted_r = carry;
+        __syncthreads();
+        // copy ids and sum the lengths: one warp per group
         const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
         for (int k = w; k < T_emit; k += nw) {
             const int p = ap[k], c = ac[k], o = ao[k];
-            uint32_t sum = 0;  // count * max_len <= budget < 2^31, or a singleton
+            uint32_t sum = 0;
             for (int j = lane; j < c; j += 32) {
                 const uint64_t key = k_[p + j];
                 const int id = key_id(key);
                 sum += key_len(key);
                 emit_ids[base + o + j] = id;
                 emit_pos[base + id] = o + j;
-                if (!all_emitted) pf[p + j] = 1;
+                pf[p + j] = 1;
             }
             sum = __reduce_add_sync(ODB_FULL_MASK, sum);
             if (lane == 0) st_real[(int64_t)(step_base + k) * R + r] = (int32_t)sum;
@@ -883,20 +930,21 @@ static cudaError_t launch_align_kernel(odb_ctx *c, cudaStream_t st) {
     }
     k_align<<<R, kRankThreads, al_smem, st>>>(c->d_rank_ptr, c->S, c->G, R, c->world_ranks ? c->gs_world : nullptr,
                                               c->world_ranks, c->prm.join_mode, c->prm.slot_capacity, c->gpos, c->agpos,
-                                              c->agcnt, c->agorg, c->ovf, c->step_samples.p, c->n_steps, c->d_rec);
+                                              c->agcnt, c->agorg, c->ovf, c->step_samples.p, c->n_steps, c->emit_cur, c->emit_snap,
+                                              c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
 
 static cudaError_t launch_commit_kernel(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
-    k_commit<<<R, kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, c->G, R, c->agpos, c->agcnt, c->agorg, c->agoff,
+    k_commit<<<dim3(R, kCommitParts), kRankThreads, 0, st>>>(c->sorted, c->d_rank_ptr, c->S, c->G, R, c->agpos, c->agcnt, c->agorg, c->agoff,
                                          c->step_samples.p, c->n_steps, c->round, c->prm.join_mode,
                                          (long long)c->prm.sample_quota,
                                          (long long)c->prm.emitted_so_far + (long long)c->samples_emitted, c->st_count.p,
                                          c->st_width.p, c->st_real.p, c->st_round.p, c->st_origin.p, c->posflag,
                                          c->emit_ids, c->emit_pos, c->left_ids, c->n_left, c->fetch_pos, c->emit_cur,
-                                         c->d_rec);
+                                         c->emit_snap, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
