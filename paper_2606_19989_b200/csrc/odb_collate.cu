@@ -99,8 +99,9 @@ __device__ __forceinline__ RowRegs load_row(const RowDesc *__restrict__ rows, in
     return r;
 }
 
+// 256-bit streaming store (.cs: the arenas are written once and not re-read by this kernel)
 __device__ __forceinline__ void st256(int32_t *p, const int32_t (&v)[16], int o) {
-    asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(v[o]), "r"(v[o + 1]), "r"(v[o + 2]),
+    asm volatile("st.global.cs.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(v[o]), "r"(v[o + 1]), "r"(v[o + 2]),
                  "r"(v[o + 3]), "r"(v[o + 4]), "r"(v[o + 5]), "r"(v[o + 6]), "r"(v[o + 7])
                  : "memory");
 }
@@ -360,7 +361,7 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
                     }
                     mv = emit_unit<SHIFT>(A, r, (int64_t)q, t, x, a0 + 16 * lane, acc);
                 }
-                *reinterpret_cast<int4 *>(A.mask + a0 + 16 * lane) = mv;
+                __stcs(reinterpret_cast<int4 *>(A.mask + a0 + 16 * lane), mv);
                 const int tot = __reduce_add_sync(ODB_FULL_MASK, acc);
                 if (lane == 0 && tot != 0) atomicAdd(&A.grp_valid[s], tot);
             } else {

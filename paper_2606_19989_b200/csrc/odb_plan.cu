@@ -1000,7 +1000,7 @@ cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st) {
 cudaError_t launch_chunk_table(odb_ctx *c, cudaStream_t st) {
     const int64_t n_slots = (int64_t)c->prm.n_ranks * c->n_steps;
     if (n_slots == 0) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>((n_slots * 32 + 255) / 256, (int64_t)c->sm_count * 16);
+    int blocks = (int)std::min<int64_t>((n_slots * 32 + 255) / 256, (int64_t)c->sm_count * 64);
     k_chunk_table<<<blocks, 256, 0, st>>>(n_slots, c->grp_offset.p, c->grp_count.p, c->grp_width.p, c->grp_sample_ptr.p,
                                           c->chunks.p);
     ODB_LAUNCH_CHECK(c);
