@@ -396,15 +396,26 @@ k_form_groups_smem(const uint64_t *__restrict__ keys, const int64_t *__restrict_
     uint16_t *nxt = cur + n1p;
     uint32_t *mk = reinterpret_cast<uint32_t *>(nxt + n1p);
     for (int w = threadIdx.x; w < words; w += blockDim.x) mk[w] = (w == 0) ? 1u : 0u;  // x = 0 is a start
-    for (int x = threadIdx.x; x <= S; x += blockDim.x) cur[x] = (uint16_t)successor(k, x, S, budget, rule);
+    // entries (S, n1p) are padding: they jump to S like S itself, so pairs can be processed blindly
+    for (int x = threadIdx.x; x < n1p; x += blockDim.x)
+        cur[x] = (uint16_t)(x <= S ? successor(k, x, S, budget, rule) : S);
     __syncthreads();
     while (true) {
         int changed = 0;
-        for (int x = threadIdx.x; x <= S; x += blockDim.x) {
-            const int j = cur[x];
-            nxt[x] = cur[j];  // cur[S] == S
-            if (j < S && ((mk[x >> 5] >> (x & 31)) & 1u) && !((mk[j >> 5] >> (j & 31)) & 1u)) {
-                atomicOr(&mk[j >> 5], 1u << (j & 31));
+        // two positions per thread and iteration: one 32-bit load / store for the pair's jump entries
+        const uint32_t *cur2 = reinterpret_cast<const uint32_t *>(cur);
+        uint32_t *nxt2 = reinterpret_cast<uint32_t *>(nxt);
+        for (int p = threadIdx.x; 2 * p <= S; p += blockDim.x) {
+            const uint32_t v = cur2[p];
+            const int j0 = (int)(v & 0xffffu), j1 = (int)(v >> 16);
+            nxt2[p] = (uint32_t)cur[j0] | ((uint32_t)cur[j1] << 16);  // cur[S] == S
+            const uint32_t mw = mk[p >> 4] >> ((2 * p) & 31);          // marks of x = 2p (bit 0) and 2p + 1 (bit 1)
+            if ((mw & 1u) && j0 < S && !((mk[j0 >> 5] >> (j0 & 31)) & 1u)) {
+                atomicOr(&mk[j0 >> 5], 1u << (j0 & 31));
+                changed = 1;
+            }
+            if ((mw & 2u) && j1 < S && !((mk[j1 >> 5] >> (j1 & 31)) & 1u)) {
+                atomicOr(&mk[j1 >> 5], 1u << (j1 & 31));
                 changed = 1;
             }
         }
