@@ -682,7 +682,7 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
     return rc;
 }
 
-int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
+static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
                  const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
                  const int32_t *h_span_hi, const odb_outputs *ho, odb_plan_info *h_out, void *stream) {
     if (!c || !ho || !h_out || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
@@ -854,6 +854,21 @@ int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr
     CU(c, cudaStreamSynchronize(c->d2h_stream));
     CU(c, cudaStreamSynchronize(c->copy_stream));
     return ODB_OK;
+}
+
+int odb_run_host(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
+                 const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
+                 const int32_t *h_span_hi, const odb_outputs *ho, odb_plan_info *h_out, void *stream) {
+    const int rc = run_host_impl(c, h_lengths, h_rank_ptr, h_tokens, h_sample_ptr, h_span_ptr, h_span_lo, h_span_hi, ho,
+                                 h_out, stream);
+    if (rc != ODB_OK && c) {
+        // whatever failed, no copy may still be running on the caller's host buffers when we return
+        if (c->copy_stream) cudaStreamSynchronize(c->copy_stream);
+        if (c->d2h_stream) cudaStreamSynchronize(c->d2h_stream);
+        cudaStreamSynchronize((cudaStream_t)stream);
+        (void)cudaGetLastError();
+    }
+    return rc;
 }
 
 int odb_loss_weights(odb_ctx *c, int mode, double *d_weights, void *stream) {

@@ -111,8 +111,14 @@ def test_protocol(P, oracle, kind, rule, join):
     _full_parity(oracle, wl)
 
 
+@pytest.mark.parametrize("kind", ["audit:" + k for k in I.AUDIT_KINDS])
+def test_protocol_audit_whole_window(P, oracle, kind):
+    """The audit distributions with the buffer holding the whole stream (buffer 1000)."""
+    _full_parity(oracle, I.protocol_workload(kind, 1, buffer_size=1000))
+
+
 def test_protocol_fuzz(P, oracle):
-    for seed in range(150):
+    for seed in range(500):
         wl = I.protocol_workload("fuzz", seed)
         try:
             _full_parity(oracle, wl, staged=bool(seed & 1))
