@@ -382,6 +382,7 @@ def run_ours(args):
                        "pad_frac": 1.0 - n_tok / max(int(info.padded_elems), 1), "n_steps": int(info.n_steps),
                        "n_slots": int(info.n_slots), "n_rounds": int(info.n_rounds),
                        "length_mean": desc["mean"], "length_cv": desc["cv"], "length_max": desc["max"],
+                       "f_s": desc["f_s"],   # Pr[l < L_max / 4], the paper's short-sample fraction
                        "parallelism": "replicas only (virtual ranks live on one GPU; no inter-GPU collective)",
                        "l2": "no flush: every step reads %.1f GB of tokens and writes %.1f GB of outputs, both far "
                              "larger than the 126 MB L2" % (4 * n_tok / 1e9, 13 * int(info.padded_elems) / 1e9)},
