@@ -119,6 +119,9 @@ static void free_all(odb_ctx *c) {
     for (int i = 0; i < 4; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     if (c->ev_status) cudaEventDestroy(c->ev_status);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
     if (c->copy_ev) cudaEventDestroy(c->copy_ev);
@@ -521,12 +524,32 @@ int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
     I.n_slots = (int64_t)n_slots;
     I.total_elems = c->h_tot->total_elems;
     I.samples_emitted = c->h_tot->samples_emitted;
-    I.samples_left = c->h_tot->samples_left;
+    I.samples_left = c->n_total - c->h_tot->samples_emitted;  // Lemma 1: emitted + un-emitted = all
     I.real_tokens = (int64_t)c->h_tot->real_tokens;
     I.padded_elems = c->h_tot->padded_elems;
     c->info_valid = true;
     c->state = 5;
     *h_out = I;
+    return ODB_OK;
+}
+
+// Collate preparation.  The row descriptors run on the caller's stream; the chunk table and the id /
+// leftover tables (independent of them, and of each other's outputs) run beside them on an auxiliary
+// stream and are joined before anything that follows on `st`.
+static int launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
+                       const int32_t *d_span_hi, cudaStream_t st) {
+    if (!c->aux_stream) {
+        CU(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+        CU(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+        CU(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    }
+    CU(c, cudaEventRecord(c->ev_fork, st));
+    CU(c, cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
+    CU(c, launch_chunk_table(c, c->aux_stream));
+    CU(c, launch_ids_left(c, c->aux_stream));
+    CU(c, cudaEventRecord(c->ev_join, c->aux_stream));
+    CU(c, launch_row_desc(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st));
+    CU(c, cudaStreamWaitEvent(st, c->ev_join, 0));
     return ODB_OK;
 }
 
@@ -593,8 +616,10 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
     CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
     const int64_t n_chunks = (I.total_elems + kColChunk - 1) / kColChunk;
     CU(c, c->chunks.ensure((size_t)n_chunks + 1));
-    CU(c, launch_row_desc(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st));
-    CU(c, launch_chunk_table(c, st));
+    {
+        int rc = launch_prep(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st);
+        if (rc != ODB_OK) return rc;
+    }
     // ev[1]..ev[2] brackets the collate kernel alone; the pre/post work is ev[0]..ev[1] / ev[2]..ev[3]
     if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
     {  // whole arena in one launch
@@ -787,9 +812,9 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
         CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
         CU(c, c->chunks.ensure((size_t)((I.total_elems + kColChunk - 1) / kColChunk) + 1));
         CU(c, cudaStreamWaitEvent(st, c->copy_ev, 0));  // sample_ptr / spans have landed
-        CU(c, launch_row_desc(c, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p,
-                              c->hs_span_hi.p, st));
-        CU(c, launch_chunk_table(c, st));
+        rc = launch_prep(c, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p,
+                         c->hs_span_hi.p, st);
+        if (rc != ODB_OK) return rc;
         CU(c, cudaMemsetAsync(c->d_tile_counter, 0, (size_t)(R + 1) * sizeof(unsigned long long), st));
         // arena offset of every rank's first slot (slots are rank-major): R+1 strided int64
         CU(c, cudaMemcpy2DAsync(c->h_rank_off, 8, c->grp_offset.p, (size_t)I.n_steps * 8, 8, (size_t)R + 1,
@@ -817,9 +842,12 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
             CU(c, cudaMemcpyAsync(ho->d_attention_mask + lo, c->hs_mask.p + lo, n, cudaMemcpyDeviceToHost, c->d2h_stream));
         }
         if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
-    } else if (c->timing) {
-        CU(c, cudaEventRecord(c->ev[1], st));
-        CU(c, cudaEventRecord(c->ev[2], st));
+    } else {
+        CU(c, launch_ids_left(c, st));  // nothing to collate, but the leftover table is still owed
+        if (c->timing) {
+            CU(c, cudaEventRecord(c->ev[1], st));
+            CU(c, cudaEventRecord(c->ev[2], st));
+        }
     }
     {  // step totals (Eq. 2's T_tok per step)
         PostArgs P;

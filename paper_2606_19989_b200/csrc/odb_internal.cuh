@@ -235,6 +235,8 @@ struct odb_ctx {
     odb::DevBuf<int32_t> hs_lengths, hs_tokens, hs_span_lo, hs_span_hi, hs_ids, hs_labels, hs_pos;
     odb::DevBuf<int64_t> hs_sample_ptr, hs_span_ptr;
     odb::DevBuf<uint8_t> hs_mask;
+    cudaStream_t aux_stream = nullptr;   // collate preparation: chunk table + id tables beside the row descriptors
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     cudaStream_t copy_stream = nullptr;  // host -> device
     cudaStream_t d2h_stream = nullptr;   // device -> host
     cudaEvent_t copy_ev = nullptr;
@@ -250,7 +252,8 @@ cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commi
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: (G_r, S_r) pairs for the all_gather
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce
-cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st);     // A9 + tables + leftovers
+cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st);     // A9: rank-major tables, offsets, totals
+cudaError_t launch_ids_left(odb_ctx *c, cudaStream_t st);     // slot CSR ids + leftover CSR
 // ---- launchers implemented in odb_collate.cu -------------------------------------------------
 cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
                             const int32_t *d_span_lo, const int32_t *d_span_hi, cudaStream_t st);

@@ -1152,6 +1152,13 @@ cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st) {
                                                     reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
                                                     reinterpret_cast<unsigned int *>(c->scan_state.p), c->d_tot);
     ODB_LAUNCH_CHECK(c);
+    return cudaSuccess;
+}
+
+// the slot CSR's ids and the leftover CSR: only the caller's tables need them, so this runs beside the
+// collate preparation (odb_api.cu: launch_prep), not in front of the plan-size read-back
+cudaError_t launch_ids_left(odb_ctx *c, cudaStream_t st) {
+    const int R = c->prm.n_ranks;
     k_ids_left<<<R, kRankThreads, 0, st>>>(R, c->n_steps, c->d_rank_ptr, c->emit_cur, c->emit_ids, c->emit_pos,
                                            c->grp_sample_ptr.p, c->grp_sample_ids.p, c->left_ptr.p, c->left_out.p, c->d_tot);
     ODB_LAUNCH_CHECK(c);
