@@ -37,13 +37,18 @@ class OracleEngine:
         self.stop = None
         self.world = torch.zeros(2 * world_ranks, dtype=torch.int32)
         self.local = torch.zeros(2 * self.R, dtype=torch.int32)
+        self.arrived = None
+
+    def set_available(self, h_arrived):
+        self.arrived = None if h_arrived is None else [int(x) for x in h_arrived]
 
     def form_groups(self):
         bs = self.p["buffer_size"]
         self.cand = []
         for r in range(self.R):
             n_r = len(self.lens[r])
-            while (bs == 0 or len(self.buf[r]) < bs) and self.pos[r] < n_r:
+            lim = n_r if self.arrived is None else max(0, min(n_r, self.arrived[r]))
+            while (bs == 0 or len(self.buf[r]) < bs) and self.pos[r] < lim:
                 self.buf[r].append(self.pos[r])
                 self.pos[r] += 1
             S = len(self.buf[r])
@@ -64,7 +69,11 @@ class OracleEngine:
         self.done = (n_fin == self.W) if self.p["join_mode"] else (n_fin > 0)
         if self.done:
             return
-        self.T = self.o.target_groups(G, S, self.p["slot_capacity"])
+        if not (G > 0).any():      # skip round: nobody has a group (all "insufficient data" or finished)
+            self.T = 0
+            self.aligned = [None] * self.R
+            return
+        self.T = self.o.target_groups(G, np.maximum(S, 0), self.p["slot_capacity"])
         self.aligned = []
         for r in range(self.R):
             if not self.cand[r]:

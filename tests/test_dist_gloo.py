@@ -92,3 +92,34 @@ def test_two_process_gloo_protocol_matches_whole_job_oracle():
             assert step_samples == plan.step_samples.tolist(), (name, rank)
             for j in range(rl):
                 assert slots[j] == plan.groups_of_rank(rank * rl + j), (name, rank, j)
+
+
+@pytest.mark.parametrize("n_proc", [2, 4])
+def test_lockstep_driver_with_oracle_engines(n_proc):
+    """The same protocol generator driven in lock step inside one process (dist.run_lockstep, the driver the
+    single-GPU tests use), with oracle-backed engines: 2 and 4 "processes", with and without an arrival
+    schedule (status 0 / -1 through the gathered summary, skip rounds)."""
+    sys.path.insert(0, ROOT)
+    import odb_inputs as I
+    from oracle import odb_oracle
+    from paper_2606_19989_b200 import dist as D
+    from tests._oracle_engine import OracleEngine
+    from tests.test_oracle_arrival import _random_schedule
+    odb_oracle.build()
+    for name in ("unequal", "empty_rank", "overflow_multiround", "overflow_nonjoin_quota", "audit:longtail"):
+        for with_sched in (False, True):
+            wl = _case(name) if not name.startswith("audit") else I.protocol_workload(name, 2)
+            if wl.n_ranks % n_proc:
+                continue
+            sched = _random_schedule(np.random.default_rng(5), wl, 8) if with_sched else None
+            plan, _ = odb_oracle.run_workload(wl, collate=False, avail_schedule=sched)
+            rl = wl.n_ranks // n_proc
+            engines = [OracleEngine(odb_oracle, part) for part in I.split_ranks(wl, n_proc)]
+            res = D.run_lockstep([D.plan_protocol(e, wl.n_ranks, p * rl,
+                                                  None if sched is None else [row[p * rl:(p + 1) * rl] for row in sched])
+                                  for p, e in enumerate(engines)])
+            for p, (info, round_T) in enumerate(res):
+                assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason), name
+                assert round_T == plan.round_T.tolist() and info.step_samples == plan.step_samples.tolist()
+                for j in range(rl):
+                    assert info.slots[j] == plan.groups_of_rank(p * rl + j), (name, with_sched, p, j)
