@@ -465,3 +465,16 @@ def test_max_sizes_huge_singleton(P, oracle):
                            budget=1000)
     plan = _big_slot_parity(oracle, wl, lambda p: range(p.n_slots))
     assert int(plan.grp_width.max()) == 120_000_000
+
+
+def test_quota_fixture_e9(P, oracle):
+    """The hand-worked quota cases of tests/golden/e9_quota.txt through the CUDA path."""
+    from tests import _golden as G
+    g = G.load("e9_quota.txt")
+    per_rank = [G.ints(x) for x in g["rank_lengths"].split("|")]
+    for q, carried in ((5, 0), (4, 0), (8, 0), (5, 3), (100, 0)):
+        wl = I.custom_workload("e9", per_rank, seed=2, budget=int(g["budget"]), join_mode=0, sample_quota=q,
+                               emitted_so_far=carried)
+        plan, info, out = _full_parity(oracle, wl)
+        if (q, carried) == (5, 0):
+            assert plan.samples_emitted == int(g["samples_emitted"]) and plan.stop_reason == int(g["stop"])

@@ -559,3 +559,24 @@ def test_token_hash_reference_values():
         want = [(((mix64(seed * 0x9E3779B97F4A7C15 + start + j) >> 32) * I.VOCAB) >> 32) for j in range(64)]
         assert got.tolist() == want
         assert got.min() >= 0 and got.max() < I.VOCAB
+
+
+def test_e9_quota_fixture(oracle):
+    g = G.load("e9_quota.txt")
+    per_rank = [G.ints(x) for x in g["rank_lengths"].split("|")]
+    lens = np.array([x for r in per_rank for x in r], np.int32)
+    rp = np.array([0, 4, 8], np.int64)
+    p = oracle.OraclePlan(lens, rp, budget=int(g["budget"]), join_mode=0, sample_quota=int(g["quota"]))
+    assert p.groups_of_rank(0) == G.groups(g["groups_a"]) and p.groups_of_rank(1) == G.groups(g["groups_b"])
+    assert p.left_ids[p.left_ptr[0]:p.left_ptr[1]].tolist() == G.ints(g["left_a"])
+    assert p.left_ids[p.left_ptr[1]:p.left_ptr[2]].tolist() == G.ints(g["left_b"])
+    assert p.samples_emitted == int(g["samples_emitted"]) and p.stop_reason == int(g["stop"])
+    assert p.n_rounds == int(g["n_rounds"])
+    for q, key in ((4, "quota4_steps"), (8, "quota8_steps")):
+        p = oracle.OraclePlan(lens, rp, budget=int(g["budget"]), join_mode=0, sample_quota=q)
+        assert p.n_steps == int(g[key]) and p.stop_reason == oracle.STOP_QUOTA
+    p = oracle.OraclePlan(lens, rp, budget=int(g["budget"]), join_mode=0, sample_quota=5, emitted_so_far=3)
+    assert p.n_steps == int(g["carried3_quota5_steps"])
+    # join mode ignores the quota
+    p = oracle.OraclePlan(lens, rp, budget=int(g["budget"]), join_mode=1, sample_quota=5)
+    assert p.n_steps == 3 and p.stop_reason == oracle.STOP_ALL_FINISHED
