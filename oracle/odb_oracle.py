@@ -211,7 +211,10 @@ class OraclePlan:
     def __del__(self):
         h = getattr(self, "_h", None)
         if h:
-            lib().oracle_plan_free(h)
+            try:
+                lib().oracle_plan_free(h)
+            except Exception:  # interpreter shutdown: module globals are already gone
+                pass
             self._h = None
 
     def slot_ids(self, r: int, k: int):

@@ -74,7 +74,6 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->emit_cur);
     cudaFree(c->G);
     cudaFree(c->S);
-    cudaFree(c->F);
     cudaFree(c->emit_snap);
     cudaFree(c->d_arrived);
     cudaFree(c->d_rec);
@@ -192,7 +191,6 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->emit_cur, R);
     if (e == cudaSuccess) e = dev_alloc(&c->G, R);
     if (e == cudaSuccess) e = dev_alloc(&c->S, R);
-    if (e == cudaSuccess) e = dev_alloc(&c->F, R);
     if (e == cudaSuccess) e = dev_alloc(&c->emit_snap, R);
     if (e == cudaSuccess) e = dev_alloc(&c->d_arrived, R);
     if (e == cudaSuccess) e = dev_alloc(&c->d_rec, 1);

@@ -205,7 +205,6 @@ struct odb_ctx {
     int32_t *agpos = nullptr, *agcnt = nullptr, *agoff = nullptr, *agorg = nullptr;  // n_max + R
     int32_t *left_ids = nullptr, *emit_ids = nullptr;              // n_max
     int32_t *n_left = nullptr, *fetch_pos = nullptr, *emit_cur = nullptr, *G = nullptr, *S = nullptr;  // R
-    int32_t *F = nullptr;          // R: 1 = the rank is finished (status -1)
     int32_t *emit_snap = nullptr;  // R: emit_cur as seen by k_align (read by every CTA of k_commit)
     int32_t *d_arrived = nullptr;  // R: views of the rank's stream that have arrived (odb_set_available)
     std::vector<int32_t> h_arrived;

@@ -101,7 +101,7 @@ __device__ __forceinline__ int window_size(int n_left, int fetch_pos, int n_arri
 // ---------------------------------------------------------------------------------------------
 __global__ void k_begin(const int32_t *__restrict__ len, int64_t n, int R, int32_t *__restrict__ n_left,
                         int32_t *__restrict__ fetch_pos, int32_t *__restrict__ emit_cur, int32_t *__restrict__ G,
-                        int32_t *__restrict__ S, int32_t *__restrict__ F, int32_t *__restrict__ emit_pos,
+                        int32_t *__restrict__ S, int32_t *__restrict__ emit_pos,
                         int32_t *__restrict__ step_samples, int64_t step_cap, RoundRec *rec) {
     int bad = 0;
     const int64_t bound = max(n, max((int64_t)R, step_cap));
@@ -112,7 +112,6 @@ __global__ void k_begin(const int32_t *__restrict__ len, int64_t n, int R, int32
             emit_cur[i] = 0;
             G[i] = 0;
             S[i] = 0;
-            F[i] = 0;
         }
         if (i < n) {
             emit_pos[i] = -1;
@@ -132,7 +131,7 @@ __global__ void __launch_bounds__(kSortThreads)
 k_chunk_sort(const int32_t *__restrict__ len, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ n_left,
              const int32_t *__restrict__ fetch_pos, const int32_t *__restrict__ left_ids,
              const int32_t *__restrict__ arrived, int buffer_size, uint64_t *__restrict__ keys_out,
-             int32_t *__restrict__ S_out, int32_t *__restrict__ F_out, RoundRec *rec) {
+             int32_t *__restrict__ S_out, RoundRec *rec) {
     __shared__ uint64_t sk[kSortChunk];
     const int r = blockIdx.y;
     const int64_t base = rank_ptr[r];
@@ -142,7 +141,6 @@ k_chunk_sort(const int32_t *__restrict__ len, const int64_t *__restrict__ rank_p
     const int S = window_size(nl, fp, min(n_r, arrived[r]), buffer_size);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         S_out[r] = S;
-        F_out[r] = (S == 0 && fp >= n_r) ? 1 : 0;  // status -1 "finished"; S == 0 with views pending is status 0
         if (r == 0) rec->n_finished = 0;  // counted again by this round's commit
     }
     const int c0 = blockIdx.x * kSortChunk;
@@ -212,7 +210,7 @@ __global__ void __launch_bounds__(kSortRegThreads)
 k_chunk_sort_reg(const int32_t *__restrict__ len, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ n_left,
                  const int32_t *__restrict__ fetch_pos, const int32_t *__restrict__ left_ids,
                  const int32_t *__restrict__ arrived, int buffer_size, uint64_t *__restrict__ keys_out,
-                 int32_t *__restrict__ S_out, int32_t *__restrict__ F_out, RoundRec *rec) {
+                 int32_t *__restrict__ S_out, RoundRec *rec) {
     __shared__ uint64_t sk[kSortChunk + kSortChunk / 16];
     const int r_ = blockIdx.y;
     const int64_t base = rank_ptr[r_];
@@ -221,7 +219,6 @@ k_chunk_sort_reg(const int32_t *__restrict__ len, const int64_t *__restrict__ ra
     const int S = window_size(nl, fp, min(n_r, arrived[r_]), buffer_size);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         S_out[r_] = S;
-        F_out[r_] = (S == 0 && fp >= n_r) ? 1 : 0;
         if (r_ == 0) rec->n_finished = 0;
     }
     const int c0 = blockIdx.x * kSortChunk;
@@ -1022,7 +1019,7 @@ cudaError_t launch_begin(odb_ctx *c, cudaStream_t st) {
     const int64_t bound = std::max<int64_t>(std::max<int64_t>(c->n_total, R), step_cap);
     int blocks = (int)std::min<int64_t>((bound + 1023) / 1024, (int64_t)c->sm_count * 4);
     k_begin<<<std::max(blocks, 1), 256, 0, st>>>(c->d_lengths, c->n_total, R, c->n_left, c->fetch_pos, c->emit_cur, c->G,
-                                                c->S, c->F, c->emit_pos, c->step_samples.p, step_cap, c->d_rec);
+                                                c->S, c->emit_pos, c->step_samples.p, step_cap, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
@@ -1047,11 +1044,11 @@ cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st) {
     if (maxS > kSortChunk / 2)  // full-size chunks: the register-blocked network; small windows: the shared-memory one
         k_chunk_sort_reg<<<dim3(chunks, R), kSortRegThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos,
                                                                      c->left_ids, c->d_arrived, c->prm.buffer_size,
-                                                                     c->keyA, c->S, c->F, c->d_rec);
+                                                                     c->keyA, c->S, c->d_rec);
     else
         k_chunk_sort<<<dim3(chunks, R), kSortThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos,
                                                               c->left_ids, c->d_arrived, c->prm.buffer_size, c->keyA, c->S,
-                                                              c->F, c->d_rec);
+                                                              c->d_rec);
     ODB_LAUNCH_CHECK(c);
     uint64_t *src = c->keyA, *dst = c->keyB;
     for (int64_t w = kSortChunk; w < maxS; w *= 2) {
@@ -1121,18 +1118,24 @@ cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st) { return launch_comm
 
 // distributed mode: the local ranks' (G_r, S_r) pairs, the message of the per-round all_gather
 __global__ void k_pack_summary(int R, const int32_t *__restrict__ G, const int32_t *__restrict__ S,
-                               const int32_t *__restrict__ F, int32_t *__restrict__ gs, RoundRec *rec) {
+                               const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ fetch_pos,
+                               int32_t *__restrict__ gs, RoundRec *rec) {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q < R) {
+        // status -1 "finished": nothing buffered and nothing pending; an empty window with views still
+        // pending is status 0 "insufficient data".  Computed here, not in the sort kernel, because a
+        // process whose ranks hold no sample at all never launches the sort.
+        const int n_r = (int)(rank_ptr[q + 1] - rank_ptr[q]);
+        const bool fin = S[q] == 0 && fetch_pos[q] >= n_r;
         gs[2 * q] = G[q];
-        gs[2 * q + 1] = F[q] ? -1 : S[q];  // -1 = "finished"; 0 = "insufficient data"
+        gs[2 * q + 1] = fin ? -1 : S[q];
     }
     if (q == 0) rec->done = 0;
 }
 
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
-    k_pack_summary<<<(R + 127) / 128, 128, 0, st>>>(R, c->G, c->S, c->F, c->gs_local, c->d_rec);
+    k_pack_summary<<<(R + 127) / 128, 128, 0, st>>>(R, c->G, c->S, c->d_rank_ptr, c->fetch_pos, c->gs_local, c->d_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

@@ -41,6 +41,12 @@ def _case(name):
         wl = I.protocol_workload("overflow_multiround", 3, join_mode=0)
         wl.params["sample_quota"] = int(0.6 * wl.n_samples)
         return wl
+    if name.startswith("sampleless_process"):   # one process whose ranks hold no sample at all (soak seed 25)
+        rng = np.random.default_rng(25)
+        per = [[], rng.integers(1, 1500, 43), rng.integers(1, 1500, 58), rng.integers(1, 100, 20)]
+        join = 0 if name.endswith("nonjoin") else 1
+        return I.custom_workload(name, per, 25, budget=4096, buffer_size=64, slot_capacity=17, join_mode=join,
+                                 sample_quota=0 if join else 42)
     if name == "maxfit_overflow":
         return I.protocol_workload("overflow_multiround", 5, rule=1)
     return I.protocol_workload(name, 2)
@@ -49,7 +55,7 @@ def _case(name):
 @pytest.mark.parametrize("n_proc", [2, 4])
 @pytest.mark.parametrize("name", ["tiny", "config2_slice", "unequal", "empty_rank", "overflow_multiround",
                                   "overflow_nonjoin_quota", "maxfit_overflow", "config4_slice_nonjoin",
-                                  "audit:bimodal"])
+                                  "audit:bimodal", "sampleless_process_join", "sampleless_process_nonjoin"])
 def test_lockstep_processes_match_whole_job_oracle(P, oracle, name, n_proc):
     import torch
     from paper_2606_19989_b200 import dist as D
