@@ -167,3 +167,20 @@ def device_self_consistency(info, out, ignore_index=-100):
     assert int(real.sum()) == int(info.real_tokens)
     sv = out.table("grp_valid_tokens").to(torch.int64).view(-1, n_steps).sum(0)
     assert torch.equal(sv, out.table("step_valid_tokens"))
+
+
+def wide_fuzz_case(seed, max_ranks=8, max_n=300):
+    """A random job wider than ``protocol_workload("fuzz")``: up to 8 ranks x 300 samples, lengths up to
+    3000, budgets 16 .. 100000, every flag; returns (workload, arrival schedule or None)."""
+    from tests.test_oracle_arrival import _random_schedule
+    rng = np.random.default_rng(900_000 + seed)
+    R = int(rng.integers(1, max_ranks + 1))
+    per = [rng.integers(1, int(rng.choice([8, 100, 3000])) + 1, int(rng.integers(0, max_n + 1))) for _ in range(R)]
+    wl = I.custom_workload("wide_fuzz", per, seed, budget=int(rng.choice([16, 300, 4096, 100000])),
+                           buffer_size=int(rng.choice([0, 1, 7, 64, 300])), slot_capacity=int(rng.choice([0, 1, 3, 17])),
+                           rule=int(rng.integers(0, 2)), join_mode=int(rng.integers(0, 2)),
+                           shift_labels=int(rng.integers(0, 2)))
+    if not wl.params["join_mode"] and rng.uniform() < 0.6:
+        wl.params["sample_quota"] = int(rng.integers(1, max(2, wl.n_samples + 1)))
+    sched = _random_schedule(rng, wl, int(rng.integers(1, 10))) if seed % 2 == 0 else None
+    return wl, sched

@@ -210,3 +210,50 @@ def test_dist_mode_errors(P):
                       empty.struct)
         P.odb_dist_config(ctx.h, 0, 0, 0)             # back to single-process mode
         Par.run_gpu(wl, dw, staged=False)
+
+
+def test_lockstep_wide_fuzz(P, oracle):
+    """120 random jobs split over 2-4 contexts (ranks with no samples, processes with no samples, quota,
+    overflow, arrival schedules): every context equals the whole-job oracle."""
+    import torch
+    from paper_2606_19989_b200 import dist as D
+    for seed in range(120):
+        rng = np.random.default_rng(seed)
+        n_proc = int(rng.choice([2, 3, 4]))
+        rl = int(rng.integers(1, 4))
+        R = n_proc * rl
+        wl, sched = None, None
+        for s2 in range(50):   # a generated job with exactly R ranks
+            wl, sched = Par.wide_fuzz_case(1000 * seed + s2, max_ranks=12, max_n=150)
+            if wl.n_ranks == R:
+                break
+        if wl.n_ranks != R:
+            continue
+        plan, ref = oracle.run_workload(wl, avail_schedule=sched)
+        K = plan.n_steps
+        parts = I.split_ranks(wl, n_proc)
+        dws = [Par.DeviceWorkload(w) for w in parts]
+        engines = [D.CudaEngine(Par.gpu_params(w), max(w.n_samples, 1), dw.lengths, w.rank_ptr) for w, dw in zip(parts, dws)]
+        try:
+            res = D.run_lockstep([D.plan_protocol(e, R, p * rl, None if sched is None else [row[p * rl:(p + 1) * rl] for row in sched])
+                                  for p, e in enumerate(engines)])
+            for p, (e, dw) in enumerate(zip(engines, dws)):
+                info, round_T = res[p]
+                assert round_T == plan.round_T.tolist(), seed
+                assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason), seed
+                out = P.OutputBuffers.for_plan(rl, info, dw.device, fill=Par.SENTINEL)
+                e.collate(dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out)
+                torch.cuda.synchronize()
+                s0, s1 = p * rl * K, (p + 1) * rl * K
+                off0 = int(plan.grp_offset[s0]) if s0 < plan.n_slots else plan.total_elems
+                off1 = int(plan.grp_offset[s1]) if s1 < plan.n_slots else plan.total_elems
+                q0, q1 = int(plan.grp_sample_ptr[s0]), int(plan.grp_sample_ptr[s1])
+                assert np.array_equal(out.table("grp_count").cpu().numpy(), plan.grp_count[s0:s1]), seed
+                assert np.array_equal(out.table("grp_sample_ids").cpu().numpy(), plan.grp_sample_ids[q0:q1]), seed
+                assert np.array_equal(out.table("step_samples").cpu().numpy(), plan.step_samples), seed
+                E = off1 - off0
+                for nm in ("input_ids", "labels"):
+                    assert np.array_equal(getattr(out, nm)[:E].cpu().numpy(), ref[nm][off0:off1]), (seed, nm)
+        finally:
+            for e in engines:
+                e.close()

@@ -478,3 +478,18 @@ def test_quota_fixture_e9(P, oracle):
         plan, info, out = _full_parity(oracle, wl)
         if (q, carried) == (5, 0):
             assert plan.samples_emitted == int(g["samples_emitted"]) and plan.stop_reason == int(g["stop"])
+
+
+def test_wide_fuzz(P, oracle):
+    """300 random jobs (up to 8 ranks x 300 samples, all flags, half of them with an arrival schedule):
+    plan tables and arenas bit for bit.  (A scratch soak of the same generators ran 86,000 single-context,
+    20,000 lock-step multi-context and 4,000 odb_run_host cases at the end of round 1.)"""
+    for seed in range(300):
+        wl, sched = Par.wide_fuzz_case(seed)
+        try:
+            plan, ref = oracle.run_workload(wl, avail_schedule=sched)
+            info, out, round_T = Par.run_gpu(wl, staged=True, avail_schedule=sched)
+            Par.compare_plan(plan, info, out, round_T)
+            Par.compare_full(plan, ref, info, out)
+        except AssertionError as e:
+            raise AssertionError("wide fuzz seed %d params %r: %s" % (seed, wl.params, e))
