@@ -6,8 +6,10 @@ sort, greedy successor, list ranking, cross-rank reduction, split/overflow, step
 collation with valid-token counts) through ``odb_run`` over one batch of synthetic input that is
 already resident in HBM.  Default workload = BASELINE.json configs[4] (the throughput sweep, the
 largest config, on which north_star states its target), cell CV=1.0 / budget=65536, paper rule
-(THRESHOLD), join mode.  ``--sweep`` adds the nine (CV, budget) cells; ``--config k`` picks another
-BASELINE.json config.
+(THRESHOLD), join mode.  The default run also times the nine (CV, budget) cells of configs[4] and configs[1..3] (key
+``sweep``; ``--no-sweep`` skips it, ``--sweep`` adds the MAXFIT_ASC rule) and the paper's operating point, a
+1024-sample grouping buffer per rank (key ``paper_operating_point``); ``--config k`` picks another
+BASELINE.json config, ``--buffer-size`` another window.
 
 Prints ONE JSON line (rank 0).  Extra objects: ``roofline`` (collate kernel, CUDA events on the
 launching stream inside the timed region), ``e2e`` (odb_run_host with pinned HOST buffers, copies
@@ -17,6 +19,8 @@ box's host cores), ``clocks`` (nvidia-smi sampled during the timed region).
 ``--impl reference`` times the CPU oracle instead (rank 0 only), per the tier contract.
 Multi-GPU: the path does not shard across GPUs (north_star: virtual ranks on ONE GPU, no inter-GPU
 collectives) -> "replicas only": N independent replicas, max-over-ranks time, value = N x units / t.
+``--gpus N`` without a torchrun environment starts the N processes itself (one per GPU, NCCL rendezvous on
+127.0.0.1) and fails loudly when the box has fewer than N devices; under torchrun WORLD_SIZE must equal N.
 """
 from __future__ import annotations
 
@@ -51,7 +55,9 @@ def parse_args():
     ap.add_argument("--budget", type=int, default=None)
     ap.add_argument("--rule", type=int, default=0)
     ap.add_argument("--join", type=int, default=1)
-    ap.add_argument("--sweep", action="store_true", help="also time the nine config-5 cells (extra key 'sweep')")
+    ap.add_argument("--buffer-size", type=int, default=None, help="per-round window per rank (0 = whole stream)")
+    ap.add_argument("--sweep", action="store_true", help="the sweep also runs the MAXFIT_ASC rule on every cell")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the sweep cells and the paper operating point")
     ap.add_argument("--shard-ranks", action="store_true",
                     help="SURVEY.md 8(f) F1: split the job's virtual ranks over the N GPUs (strong scaling; per-round "
                          "all_gather + all_reduce over NCCL) instead of N independent replicas")
@@ -77,7 +83,10 @@ def make_wl(args, **over):
     if args.config == 4:
         kw["cv"] = args.cv
     kw.update(over)
-    return I.make_workload(args.config, **kw)
+    wl = I.make_workload(args.config, **kw)
+    if args.buffer_size is not None:
+        wl.params["buffer_size"] = args.buffer_size
+    return wl
 
 
 def algorithmic_bytes(real_tokens, padded_elems):
@@ -147,7 +156,8 @@ def measured_peak():
 
 
 def ncu_traffic(workload_key):
-    """dram bytes per collate launch from the committed ncu --set full summary (profiles/), or None."""
+    """dram bytes per collate launch from the committed ncu --set full summary (profiles/), keyed by cell, or
+    None: a cell that has no capture of the committed kernel reports null, never another cell's constant."""
     p = os.path.join(ROOT, "profiles", "collate_traffic.txt")
     try:
         with open(p) as f:
@@ -280,18 +290,22 @@ def time_device(P, ctx, wl, din, out, steps, warmup, barrier):
     barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = P.odb_kernel_launches(ctx.h)
-    stage = np.zeros(3)
     torch.cuda.synchronize()
     ev0.record()
     for _ in range(steps):
         info = one()
-        stage += np.asarray(P.odb_get_timing(ctx.h))     # waits for this step's last event (no extra work)
     ev1.record()
     torch.cuda.synchronize()
     barrier()
     ms = ev0.elapsed_time(ev1) / max(steps, 1)
     launches = (P.odb_kernel_launches(ctx.h) - l0) / max(steps, 1)
-    stage /= max(steps, 1)
+    # per-step stage events, recorded by the library on the launching stream INSIDE the timed region and read
+    # here, after it (the library keeps the last 64 runs' events)
+    n_read = min(steps, 64)
+    stage = np.zeros(3)
+    for back in range(n_read):
+        stage += np.asarray(P.odb_get_timing_at(ctx.h, back))
+    stage /= max(n_read, 1)
     return ms, float(stage[1]), float(stage[0]), float(stage[2]), launches, info
 
 
@@ -327,6 +341,16 @@ def time_e2e(P, ctx, wl, din, info, steps, device):
     return dt, int(h2d), int(d2h)
 
 
+def check_world(args, world):
+    """The printed n_gpus is the world size; it must be what --gpus asked for."""
+    import torch
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d" % (args.gpus, world))
+    if torch.cuda.device_count() < int(os.environ.get("LOCAL_RANK", "0")) + 1:
+        raise SystemExit("bench.py: LOCAL_RANK %s has no CUDA device (%d visible)" % (
+            os.environ.get("LOCAL_RANK", "0"), torch.cuda.device_count()))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -337,6 +361,7 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    check_world(args, world)
     torch.cuda.set_device(local)
     device = "cuda:%d" % local
     if world > 1:
@@ -372,7 +397,9 @@ def run_ours(args):
         abytes = algorithmic_bytes(info.real_tokens, info.padded_elems)
         peak, peak_src = measured_peak()
         achieved = abytes / (col_ms_max * 1e-3) / 1e9
-        wkey = "config%d_cv%g_L%d_rule%d" % (args.config, args.cv, wl.params["budget"], args.rule)
+        wkey = cell_key(args.config, args.cv if args.config == 4 else 0, wl.params["budget"], args.rule,
+                        wl.params["buffer_size"])
+        traffic = ncu_traffic(wkey)
         result = {
             "metric": METRIC, "value": world * n_samples / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
@@ -390,14 +417,32 @@ def run_ours(args):
             "hbm_gbs_whole_step": abytes / (ms * 1e-3) / 1e9,
             "stage_ms": {"planning": plan_ms, "collate_kernel": col_ms, "post": post_ms},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": ncu_traffic(wkey), "kernel": "k_collate", "algorithmic_bytes": abytes,
+                         "traffic": traffic, "traffic_over_algorithmic": traffic / abytes if traffic else None,
+                         "traffic_source": ("profiles/collate_traffic.txt key %s (ncu --set full capture of this "
+                                            "cell)" % wkey) if traffic else "no ncu capture of this cell",
+                         "kernel": "k_collate", "algorithmic_bytes": abytes,
                          "kernel_ms": col_ms_max, "peak_source": peak_src,
                          "frac_of_nominal_8180": achieved / 8180.0},
             "gpu_launches": int(round(launches * args.steps)),
             "clocks": clocks,
         }
-        if args.sweep and args.config == 4 and world == 1:
-            result["sweep"] = run_sweep(P, args, device, peak)
+        result["stage_ms"]["planning_share"] = plan_ms / ms
+        result["launches_per_step"] = launches
+        if not args.no_sweep and world == 1:
+            rows = run_sweep(P, args, device, peak)
+            result["sweep"] = rows
+            big = [r for r in rows if r["workload"].startswith("configs[4]") and r["frac"] is not None]
+            small = [r for r in rows if not r["workload"].startswith("configs[4]") and r["frac"] is not None]
+            if big:
+                w = min(big, key=lambda r: r["frac"])
+                result["roofline"]["worst_cell"] = {"workload": w["workload"], "rule": w["rule"], "frac": w["frac"],
+                                                    "whole_step_frac": w["whole_step_frac"]}
+            if small:
+                w = min(small, key=lambda r: r["frac"])
+                result["roofline"]["worst_small_config"] = {"workload": w["workload"], "rule": w["rule"],
+                                                            "frac": w["frac"], "ms_per_step": w["ms_per_step"],
+                                                            "note": "sub-millisecond steps: launch latency, not HBM, bounds them"}
+            result["paper_operating_point"] = paper_operating_point(P, device, peak)
         # ---- e2e through the C ABI with HOST buffers (odb_run_host) -------------------------
         if not args.no_e2e:
             need = 4 * wl.n_tokens + 13 * int(info.total_elems)
@@ -446,6 +491,7 @@ def run_sharded(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    check_world(args, world)
     torch.cuda.set_device(local)
     device = "cuda:%d" % local
     if world == 1:
@@ -529,36 +575,119 @@ def run_sharded(args):
             "gpu_launches": int(launches), "clocks": clocks, "e2e": None, "cpu_baseline": None}), flush=True)
 
 
-def run_sweep(P, args, device, peak):
-    """The nine (CV, budget) cells of configs[4], both rules: samples/s, tokens/s, collate GB/s."""
+def cell_key(config, cv, budget, rule, buffer_size=0):
+    k = "config%d_cv%g_L%d_rule%d" % (config, cv, budget, rule)
+    return k + ("_buf%d" % buffer_size if buffer_size else "")
+
+
+def measure_workload(P, wl, device, steps, warmup):
+    """One workload through odb_run on `device` (own context, inputs and outputs); returns a row dict."""
     import torch
+    din = DeviceInputs(wl, device, P)
+    with P.Odb(gpu_params(P, wl), max(wl.n_samples, 1), device=int(device.split(":")[1])) as ctx:
+        P.odb_set_timing(ctx.h, True)
+        info = ctx.plan(din.lengths, wl.rank_ptr)
+        out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
+        ms, col_ms, plan_ms, post_ms, launches, info = time_device(P, ctx, wl, din, out, steps, warmup, lambda: None)
+        del out
+    del din
+    torch.cuda.empty_cache()
+    ab = algorithmic_bytes(info.real_tokens, info.padded_elems)
+    n_rounds = int(info.n_rounds)
+    return {"rule": RULE_NAMES[wl.params["rule"]], "join_mode": wl.params["join_mode"],
+            "buffer_size": wl.params["buffer_size"], "ms_per_step": ms,
+            "samples_per_s": int(info.samples_emitted) / (ms * 1e-3),
+            "tokens_per_s": int(info.real_tokens) / (ms * 1e-3),
+            "planning_ms": plan_ms, "collate_ms": col_ms, "post_ms": post_ms,
+            "planning_share": plan_ms / max(ms, 1e-9), "collate_gbs": ab / (col_ms * 1e-3) / 1e9 if col_ms > 0 else None,
+            "whole_step_gbs": ab / (ms * 1e-3) / 1e9, "algorithmic_bytes": ab,
+            "n_steps": int(info.n_steps), "n_rounds": n_rounds, "launches_per_step": launches,
+            "planning_ms_per_round": plan_ms / max(n_rounds, 1),
+            "pad_frac": 1.0 - int(info.real_tokens) / max(int(info.padded_elems), 1)}
+
+
+def run_sweep(P, args, device, peak):
+    """The nine (CV, budget) cells of configs[4] (rule THRESHOLD; --sweep adds MAXFIT_ASC) and configs[1..3]
+    (configs[3] in join and non-join mode): per-row collate fraction of the measured peak."""
     rows = []
+    rules = (0, 1) if args.sweep else (0,)
+
+    def add(name, key, wl):
+        row = measure_workload(P, wl, device, 5, 3)
+        row["workload"] = name
+        row["frac"] = row["collate_gbs"] / peak if row["collate_gbs"] else None
+        row["whole_step_frac"] = row["whole_step_gbs"] / peak
+        row["traffic"] = ncu_traffic(key)
+        rows.append(row)
+
     for cv, L in I.config5_cells():
-        for rule in (0, 1):
-            wl = I.make_workload(4, cv=cv, budget=L, rule=rule)
-            din = DeviceInputs(wl, device, P)
-            with P.Odb(gpu_params(P, wl), wl.n_samples, device=int(device.split(":")[1])) as ctx:
-                P.odb_set_timing(ctx.h, True)
-                info = ctx.plan(din.lengths, wl.rank_ptr)
-                out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
-                ms, col_ms, plan_ms, post_ms, _, info = time_device(P, ctx, wl, din, out, 5, 3, lambda: None)
-                ab = algorithmic_bytes(info.real_tokens, info.padded_elems)
-                rows.append({"cv": cv, "budget": L, "rule": RULE_NAMES[rule], "ms_per_step": ms,
-                             "samples_per_s": int(info.samples_emitted) / (ms * 1e-3),
-                             "tokens_per_s": int(info.real_tokens) / (ms * 1e-3), "collate_ms": col_ms,
-                             "planning_ms": plan_ms, "collate_gbs": ab / (col_ms * 1e-3) / 1e9,
-                             "frac": ab / (col_ms * 1e-3) / 1e9 / peak, "n_steps": int(info.n_steps),
-                             "pad_frac": 1.0 - int(info.real_tokens) / max(int(info.padded_elems), 1)})
-                del out
-            del din
-            torch.cuda.empty_cache()
+        for rule in rules:
+            add("configs[4] CV %g L %d" % (cv, L), cell_key(4, cv, L, rule), I.make_workload(4, cv=cv, budget=L, rule=rule))
+    for idx in (1, 2, 3):
+        c = I.bj_config(idx)
+        for rule in rules:
+            add("configs[%d] %s" % (idx, c["name"]), cell_key(idx, 0, c["budget"], rule), I.make_workload(idx, rule=rule))
+    add("configs[3] highcv_longtail non-join (quota)", "config3_nonjoin", I.make_workload(3, join_mode=0))
     return rows
+
+
+def paper_operating_point(P, device, peak):
+    """The paper's operating point: a 1024-sample grouping buffer per rank, i.e. tens of protocol rounds
+    per rank stream, on the configs[4] recipe (CV 1.0, budget 65536)."""
+    wl = I.make_workload(4, cv=1.0, budget=65536)
+    wl.params["buffer_size"] = 1024
+    row = measure_workload(P, wl, device, 5, 3)
+    row["workload"] = "configs[4] CV 1 L 65536, buffer_size 1024 (P:28)"
+    row["frac"] = row["collate_gbs"] / peak if row["collate_gbs"] else None
+    row["whole_step_frac"] = row["whole_step_gbs"] / peak
+    return row
+
+
+# --------------------------------------------------------------------------------------------
+# --gpus N without torchrun: start the N processes ourselves
+# --------------------------------------------------------------------------------------------
+def launcher_envs(n, port, base_env):
+    """Environment of each of the n worker processes (rank i on GPU i, rendezvous on 127.0.0.1)."""
+    envs = []
+    for i in range(n):
+        e = dict(base_env)
+        e.update(RANK=str(i), LOCAL_RANK=str(i), WORLD_SIZE=str(n), LOCAL_WORLD_SIZE=str(n),
+                 MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        e.setdefault("NCCL_DEBUG", "INFO")            # communicator lines (rank counts) stay visible in stderr
+        e.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        envs.append(e)
+    return envs
+
+
+def free_port():
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
+def self_launch(args):
+    """One process per GPU; rank 0 prints the JSON line on our stdout.  Exits non-zero when the box has fewer
+    than --gpus CUDA devices (never a silent N=1 number)."""
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < args.gpus:
+        sys.stderr.write("bench.py: --gpus %d but this box has %d CUDA device(s); refusing to report an N=%d number "
+                         "from fewer GPUs\n" % (args.gpus, have, args.gpus))
+        sys.exit(2)
+    envs = launcher_envs(args.gpus, free_port(), os.environ)
+    procs = [subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=e,
+                              stdout=(None if i == 0 else subprocess.DEVNULL)) for i, e in enumerate(envs)]
+    rcs = [p.wait() for p in procs]
+    sys.exit(max(abs(rc) for rc in rcs))
 
 
 def main():
     args = parse_args()
     if args.impl == "reference":
-        run_reference(args)
+        run_reference(args)       # rank 0 alone runs it, whatever --gpus says
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        self_launch(args)
     elif args.shard_ranks:
         run_sharded(args)
     else:

@@ -252,6 +252,10 @@ ODB_API int odb_commit(odb_ctx *ctx, void *stream);
  * copies).  Synchronises.  Enabled by odb_set_timing(ctx, 1); off by default. */
 ODB_API int odb_set_timing(odb_ctx *ctx, int enable);
 ODB_API int odb_get_timing(odb_ctx *ctx, float *ms3);
+/* The same for the timed run `back` runs before the latest one (0 = the latest, up to 63): the events of
+ * the last 64 runs are kept, so a benchmark can enqueue many runs back to back and read their stage times
+ * afterwards instead of waiting on every run.  ODB_ERR_STATE if that run does not exist (any more). */
+ODB_API int odb_get_timing_at(odb_ctx *ctx, int back, float *ms3);
 /* Number of kernels this context has launched since odb_create (diagnostics / bench accounting). */
 ODB_API int64_t odb_kernel_launches(const odb_ctx *ctx);
 

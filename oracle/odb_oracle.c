@@ -744,3 +744,22 @@ void oracle_collate_all(const oracle_plan *p, const int32_t *tokens, const int64
         if (step_valid_tokens) step_valid_tokens[s % (p->n_steps > 0 ? p->n_steps : 1)] += v;
     }
 }
+
+/* The loop of oracle_collate_all restricted to the slots [slot_lo, slot_hi) (one rank's slots, say),
+ * written into buffers whose element 0 is arena element elem_base: the full-size parity tests compare
+ * rank by rank so that neither side holds 28 GB on the host.  No arithmetic of its own: every element
+ * comes from oracle_collate_slot.  grp_valid_tokens: slot_hi - slot_lo entries. */
+void oracle_collate_range(const oracle_plan *p, int64_t slot_lo, int64_t slot_hi, int64_t elem_base,
+                          const int32_t *tokens, const int64_t *tok_start, const int64_t *span_ptr,
+                          const int32_t *span_lo, const int32_t *span_hi, int32_t pad_id, int32_t ignore_index,
+                          int32_t shift_labels, int32_t *input_ids, uint8_t *attention_mask, int32_t *position_ids,
+                          int32_t *labels, int32_t *grp_valid_tokens) {
+    for (int64_t s = slot_lo; s < slot_hi; ++s) {
+        int64_t off = p->grp_offset[s] - elem_base;
+        int64_t v = oracle_collate_slot(p, s, tokens, tok_start, span_ptr, span_lo, span_hi, pad_id, ignore_index,
+                                        shift_labels, input_ids ? input_ids + off : NULL,
+                                        attention_mask ? attention_mask + off : NULL,
+                                        position_ids ? position_ids + off : NULL, labels ? labels + off : NULL);
+        if (grp_valid_tokens) grp_valid_tokens[s - slot_lo] = (int32_t)v;
+    }
+}

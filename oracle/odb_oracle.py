@@ -74,6 +74,9 @@ def lib():
         L.oracle_collate_all.restype = None
         L.oracle_collate_all.argtypes = [vp, pi32, pi64, pi64, pi32, pi32, i32, i32, i32, pi32, pu8, pi32, pi32,
                                          pi32, pi64]
+        L.oracle_collate_range.restype = None
+        L.oracle_collate_range.argtypes = [vp, i64, i64, i64, pi32, pi64, pi64, pi32, pi32, i32, i32, i32, pi32, pu8,
+                                           pi32, pi32, pi32]
         L.oracle_plan_origin.restype = None
         L.oracle_plan_origin.argtypes = [vp, pi32]
         L.oracle_loss_weights.restype = None
@@ -273,6 +276,34 @@ class OraclePlan:
                                  _p(mask, ctypes.c_uint8), _p(pos, i32), _p(lab, i32), _p(gv, i32), _p(sv, i64))
         return dict(input_ids=ids, attention_mask=mask, position_ids=pos, labels=lab,
                     grp_valid_tokens=gv[:self.n_slots], step_valid_tokens=sv[:self.n_steps])
+
+
+def collate_rank(plan: "OraclePlan", r: int, tokens, tok_start, span_ptr, span_lo, span_hi, *, pad_id=0,
+                 ignore_index=-100, shift_labels=1, sentinel: int = 0x5A) -> Dict[str, np.ndarray]:
+    """Rank r's slots into flat buffers that start at the rank's first arena element (gaps keep the sentinel).
+    ``tokens`` / ``tok_start`` need to cover rank r's samples only (tok_start is indexed by global sample id).
+    Thread-safe (the collation routines only read the plan)."""
+    K = plan.n_steps
+    s0, s1 = r * K, (r + 1) * K
+    e0 = int(plan.grp_offset[s0]) if s0 < plan.n_slots else plan.total_elems
+    e1 = int(plan.grp_offset[s1]) if s1 < plan.n_slots else plan.total_elems
+    n = max(e1 - e0, 1)
+    s32 = np.int32(sentinel | (sentinel << 8) | (sentinel << 16) | (sentinel << 24))
+    ids, pos, lab = np.full(n, s32, np.int32), np.full(n, s32, np.int32), np.full(n, s32, np.int32)
+    mask = np.full(n, sentinel, np.uint8)
+    gv = np.zeros(max(K, 1), np.int32)
+    i32, i64 = ctypes.c_int32, ctypes.c_int64
+    tokens = np.ascontiguousarray(tokens, dtype=np.int32)
+    tok_start = np.ascontiguousarray(tok_start, dtype=np.int64)
+    lib().oracle_collate_range(plan._h, s0, s1, e0, _p(tokens, i32), _p(tok_start, i64),
+                               _p(np.ascontiguousarray(span_ptr, dtype=np.int64), i64),
+                               _p(np.ascontiguousarray(span_lo, dtype=np.int32), i32),
+                               _p(np.ascontiguousarray(span_hi, dtype=np.int32), i32), pad_id, ignore_index,
+                               shift_labels, _p(ids, i32), _p(mask, ctypes.c_uint8), _p(pos, i32), _p(lab, i32),
+                               _p(gv, i32))
+    m = e1 - e0
+    return dict(elem_lo=e0, elem_hi=e1, input_ids=ids[:m], attention_mask=mask[:m], position_ids=pos[:m],
+                labels=lab[:m], grp_valid_tokens=gv[:K])
 
 
 def run_workload(wl, tokens=None, *, collate: bool = True, avail_schedule=None):

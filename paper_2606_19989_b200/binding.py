@@ -95,6 +95,7 @@ SYMBOLS = {
     "odb_commit": (_i32, [_vp, _vp]),
     "odb_set_timing": (_i32, [_vp, _i32]),
     "odb_get_timing": (_i32, [_vp, _P(ctypes.c_float)]),
+    "odb_get_timing_at": (_i32, [_vp, _i32, _P(ctypes.c_float)]),
     "odb_kernel_launches": (_i64, [_vp]),
     "odb_debug_read": (_i64, [_vp, _i32, _vp, _i64]),
     "odb_synth_tokens": (_i32, [_vp, _i64, _i64, ctypes.c_uint64, _i32, _vp]),
@@ -303,6 +304,13 @@ def odb_get_timing(ctx: int):
     """(planning ms, collate-kernel ms, post ms) of the last odb_run / odb_collate."""
     ms = (ctypes.c_float * 3)()
     _check(load().odb_get_timing(ctx, ms), "odb_get_timing", ctx)
+    return float(ms[0]), float(ms[1]), float(ms[2])
+
+
+def odb_get_timing_at(ctx: int, back: int):
+    """The same for the timed run ``back`` runs before the latest one (the last 64 runs are kept)."""
+    ms = (ctypes.c_float * 3)()
+    _check(load().odb_get_timing_at(ctx, int(back), ms), "odb_get_timing_at", ctx)
     return float(ms[0]), float(ms[1]), float(ms[2])
 
 

@@ -115,8 +115,7 @@ static void free_all(odb_ctx *c) {
     c->hs_sample_ptr.release();
     c->hs_span_ptr.release();
     c->hs_mask.release();
-    for (int i = 0; i < 4; ++i)
-        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (cudaEvent_t e : c->evring) cudaEventDestroy(e);
     if (c->ev_status) cudaEventDestroy(c->ev_status);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
@@ -198,7 +197,6 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->d_tile_counter, R + 1);  // one work counter per pipelined launch
     if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_rec, sizeof(RoundRec));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_tot, sizeof(PlanTotals));
-    for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_status, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
@@ -233,29 +231,46 @@ int odb_reset(odb_ctx *c) {
     c->collated = false;
     c->arrived_set = false;
     c->d_lengths = nullptr;
-    c->ev_valid = false;
     return ODB_OK;
 }
 
 int odb_set_timing(odb_ctx *c, int enable) {
     if (!c) return ODB_ERR_INVALID_ARG;
+    if (enable && c->evring.empty()) {
+        CU(c, cudaSetDevice(c->device));
+        c->evring.assign((size_t)4 * kTimingRing, nullptr);
+        for (cudaEvent_t &e : c->evring) CU(c, cudaEventCreate(&e));
+    }
     c->timing = enable ? 1 : 0;
+    c->ev_seq = 0;
+    c->ev = c->evring.empty() ? nullptr : c->evring.data();
     c->ev_valid = false;
     return ODB_OK;
 }
 
-int odb_get_timing(odb_ctx *c, float *ms3) {
-    if (!c || !ms3) return ODB_ERR_INVALID_ARG;
-    if (!c->timing || !c->ev_valid) return ODB_ERR_STATE;
-    CU(c, cudaEventSynchronize(c->ev[3]));
+// the timed run `back` runs before the latest one (0 = the latest)
+int odb_get_timing_at(odb_ctx *c, int back, float *ms3) {
+    if (!c || !ms3 || back < 0) return ODB_ERR_INVALID_ARG;
+    if (!c->timing || back >= kTimingRing || (int64_t)back >= c->ev_seq) return ODB_ERR_STATE;
+    cudaEvent_t *ev = c->evring.data() + 4 * (size_t)((c->ev_seq - 1 - back) % kTimingRing);
+    CU(c, cudaEventSynchronize(ev[3]));
     float plan = 0.f, col = 0.f, all = 0.f;
-    CU(c, cudaEventElapsedTime(&plan, c->ev[0], c->ev[1]));
-    CU(c, cudaEventElapsedTime(&col, c->ev[1], c->ev[2]));
-    CU(c, cudaEventElapsedTime(&all, c->ev[2], c->ev[3]));
+    CU(c, cudaEventElapsedTime(&plan, ev[0], ev[1]));
+    CU(c, cudaEventElapsedTime(&col, ev[1], ev[2]));
+    CU(c, cudaEventElapsedTime(&all, ev[2], ev[3]));
     ms3[0] = plan;
     ms3[1] = col;
     ms3[2] = all;
     return ODB_OK;
+}
+
+int odb_get_timing(odb_ctx *c, float *ms3) { return odb_get_timing_at(c, 0, ms3); }
+
+// the quadruple a run that starts now records into; timing_done() closes it
+static void timing_begin(odb_ctx *c) { c->ev = c->evring.data() + 4 * (size_t)(c->ev_seq % kTimingRing); }
+static void timing_done(odb_ctx *c) {
+    c->ev_seq++;
+    c->ev_valid = true;
 }
 
 // first round after create / reset: bind inputs, clear the per-run device state
@@ -656,7 +671,7 @@ static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sa
     }
     if (c->timing) {
         CU(c, cudaEventRecord(c->ev[3], st));
-        c->ev_valid = true;
+        timing_done(c);
     }
     c->collated = true;
     return ODB_OK;
@@ -670,14 +685,20 @@ int odb_collate(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sample_ptr
     int rc = check_capacity(c, o);
     if (rc != ODB_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    if (c->timing) CU(c, cudaEventRecord(c->ev[0], st));
+    if (c->timing) {
+        timing_begin(c);
+        CU(c, cudaEventRecord(c->ev[0], st));
+    }
     return collate_impl(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
 }
 
 static int run_rounds(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out,
                       cudaStream_t st) {
     odb_reset(c);
-    if (c->timing) CU(c, cudaEventRecord(c->ev[0], st));
+    if (c->timing) {
+        timing_begin(c);
+        CU(c, cudaEventRecord(c->ev[0], st));
+    }
     int32_t done = 0, T = 0;
     while (!done) {
         int rc = odb_form_groups(c, d_lengths, h_rank_ptr, st);
@@ -700,7 +721,6 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
     if (rc != ODB_OK) return rc;
     rc = check_capacity(c, o);
     if (rc != ODB_OK) return rc;
-    c->ev_valid = c->timing != 0;  // ev[0] was recorded by run_rounds
     rc = collate_impl(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
     return rc;
 }
@@ -804,7 +824,6 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
     dev.d_attention_mask = c->hs_mask.p;
     dev.arena_capacity = (int64_t)E;
     const size_t n_slots = (size_t)I.n_slots;
-    c->ev_valid = c->timing != 0;  // ev[0] was recorded by run_rounds
     if (E > 0) {
         CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
         CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
@@ -856,7 +875,10 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
         P.step_valid = c->step_valid.p;
         CU(c, launch_post(c, P, st));
     }
-    if (c->timing) CU(c, cudaEventRecord(c->ev[3], st));
+    if (c->timing) {
+        CU(c, cudaEventRecord(c->ev[3], st));
+        timing_done(c);
+    }
     c->collated = true;
     // tables device -> host (small) on the compute stream
     auto d2h = [&](void *dst, const void *src, size_t bytes) -> cudaError_t {

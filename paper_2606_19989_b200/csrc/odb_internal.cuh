@@ -31,6 +31,7 @@ constexpr int kColThreads = 256;    // collate CTA (A10)
 constexpr int kColTile = 4096;      // arena elements per collate tile (one CTA iteration)
 constexpr int kColChunk = 512;      // arena elements per warp per tile (one 16-element unit per lane)
 constexpr int kColGrab = 16;        // tiles a CTA takes from the work counter at a time
+constexpr int kTimingRing = 64;     // timed runs whose stage events are kept (odb_get_timing_at)
 
 // Per-round status record: written by the round's kernels, copied to pinned host memory (A7).
 struct RoundRec {
@@ -159,7 +160,11 @@ struct odb_ctx {
     int last_cuda_error = 0;
     int64_t launches = 0;
     int timing = 0;
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    // timing: a ring of kTimingRing event quadruples, one per timed run, so that a caller can read the stage
+    // times of many back-to-back runs AFTER they have all been enqueued (no per-step wait)
+    std::vector<cudaEvent_t> evring;  // 4 * kTimingRing, created by odb_set_timing
+    int64_t ev_seq = 0;               // timed runs completed (ev[3] recorded) since odb_set_timing
+    cudaEvent_t *ev = nullptr;        // the current run's quadruple inside evring
     bool ev_valid = false;
     cudaEvent_t ev_status = nullptr;
     cudaStream_t last_stream = nullptr;

@@ -131,6 +131,60 @@ def compare_sampled_slots(wl, plan, out, slots):
             assert (gap == SENTINEL).all(), ("gap written", s)
 
 
+def compare_full_by_rank(oracle, wl, plan, out, n_threads=None):
+    """Every element of the four arenas, every slot, against the oracle -- rank by rank, so that neither side
+    holds the whole output on the host (SURVEY.md section 7 "Host memory for parity"; about 0.9 GB per rank on
+    configs[4]).  Per rank: its tokens are regenerated from the hash on the host, the oracle collates its slots
+    into sentinel-filled buffers (oracle_collate_range), and the device slice [grp_offset[r K], grp_offset[(r+1) K])
+    must equal them byte for byte -- blocks AND alignment gaps (which must still hold the sentinel)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    p = wl.params
+    K, R = plan.n_steps, wl.n_ranks
+    gv_dev = out.table("grp_valid_tokens").cpu().numpy()
+    if n_threads is None:
+        try:
+            n_threads = len(os.sched_getaffinity(0))
+        except AttributeError:
+            n_threads = os.cpu_count() or 1
+        n_threads = max(1, min(n_threads, 6, R))
+
+    def one_rank(r):
+        g0, g1 = int(wl.rank_ptr[r]), int(wl.rank_ptr[r + 1])
+        t0, t1 = int(wl.sample_ptr[g0]), int(wl.sample_ptr[g1])
+        toks = I.token_ids(wl.token_seed, wl.token_start + t0, t1 - t0)
+        tok_start = np.zeros(max(wl.n_samples, 1), dtype=np.int64)
+        tok_start[g0:g1] = wl.sample_ptr[g0:g1] - t0
+        ref = oracle.collate_rank(plan, r, toks if len(toks) else np.zeros(1, np.int32), tok_start, wl.span_ptr,
+                                  wl.span_lo, wl.span_hi, pad_id=p["pad_id"], ignore_index=p["ignore_index"],
+                                  shift_labels=p["shift_labels"], sentinel=SENTINEL)
+        e0, e1 = ref["elem_lo"], ref["elem_hi"]
+        for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+            g = getattr(out, name)[e0:e1].cpu().numpy()
+            o = ref[name]
+            if not np.array_equal(g, o):
+                bad = np.flatnonzero(g != o)
+                a = e0 + int(bad[0])
+                s = int(np.searchsorted(plan.grp_offset, a, side="right") - 1)
+                raise AssertionError("rank %d: %s differs at %d elements; first at arena element %d (slot %d, offset %d, "
+                                     "count %d, width %d): gpu %r oracle %r" % (
+                                         r, name, len(bad), a, s, plan.grp_offset[s], plan.grp_count[s],
+                                         plan.grp_width[s], g[bad[0]], o[bad[0]]))
+        assert np.array_equal(gv_dev[r * K:(r + 1) * K], ref["grp_valid_tokens"]), ("grp_valid_tokens", r)
+        return e1 - e0
+
+    with ThreadPoolExecutor(max_workers=n_threads) as ex:
+        done = sum(ex.map(one_rank, range(R)))
+    assert done == plan.total_elems          # the rank slices tile the arena
+    # tail guard: the 16 spare elements past total_elems were never written
+    E = plan.total_elems
+    for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+        tail = getattr(out, name)[E:].cpu().numpy().view(np.uint8)
+        assert (tail == SENTINEL).all(), name + ": wrote past total_elems"
+    sv = gv_dev.astype(np.int64).reshape(R, K).sum(0) if K else np.zeros(0, np.int64)
+    assert np.array_equal(out.table("step_valid_tokens").cpu().numpy(), sv)
+
+
 def device_self_consistency(info, out, ignore_index=-100):
     """Properties that hold at any size, checked on the device output itself: the valid-token table
     equals a recount of labels != ignore_index per slot; step totals are its column sums; the mask

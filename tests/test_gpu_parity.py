@@ -78,6 +78,35 @@ def _sampled_parity(oracle, wl, n_sample=48, seed=0):
     return plan
 
 
+def _full_size_elementwise(oracle, wl):
+    """Full-size run in the launch configuration bench.py times (odb_run, one collate launch over the whole
+    arena): plan tables in full, then ALL FOUR ARENAS OVER EVERY SLOT against the oracle, rank by rank."""
+    plan, _ = oracle.run_workload(wl, collate=False)
+    info, out, _ = Par.run_gpu(wl, staged=False)
+    Par.compare_plan(plan, info, out)
+    Par.compare_full_by_rank(oracle, wl, plan, out)
+    return plan
+
+
+@pytest.mark.parametrize("rule,join", [(0, 1), (0, 0), (1, 1)])
+def test_config4_full_size_every_element(P, oracle, rule, join):
+    """BASELINE.json configs[3] (16 x 16384, high-CV long tail) at full size, join and non-join (quota cut):
+    every element of input_ids / labels / position_ids / attention_mask of every slot."""
+    wl = I.make_workload(3, rule=rule, join_mode=join)
+    plan = _full_size_elementwise(oracle, wl)
+    if not join:
+        assert plan.stop_reason == 2 and plan.samples_left > 0
+
+
+@pytest.mark.parametrize("cv,budget", [(1.0, 65536), (2.5, 16384)])
+def test_config5_full_size_every_element(P, oracle, cv, budget):
+    """BASELINE.json configs[4] at full size (32 x 32768 samples, 2.1e9 tokens, 28 GB of outputs; element offsets
+    exceed 2^31): the cell bench.py is quoted on (CV 1.0 / L 65536) and the CV 2.5 / L 16384 cell (over-budget
+    singletons of up to ~270 K tokens), every element of every slot, rank by rank."""
+    plan = _full_size_elementwise(oracle, I.make_workload(4, cv=cv, budget=budget))
+    assert plan.total_elems > 2**31
+
+
 @pytest.mark.parametrize("rule", [0, 1])
 @pytest.mark.parametrize("join", [1, 0])
 def test_config4_highcv_longtail(P, oracle, rule, join):

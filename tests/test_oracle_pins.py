@@ -538,6 +538,30 @@ def test_collate_slot_equals_collate_all(oracle):
         assert out["grp_valid_tokens"][s] == o["valid"]
 
 
+def test_collate_rank_tiles_collate_all(oracle):
+    """collate_rank (the rank-by-rank form the full-size GPU parity tests use, with only the rank's own tokens
+    regenerated from the hash) concatenated over the ranks IS collate_all's arenas, gaps included."""
+    for wl in (I.protocol_workload("empty_rank", 1), I.protocol_workload("overflow_multiround", 2, join_mode=0),
+               I.make_workload(0)):
+        plan, out = oracle.run_workload(wl)
+        at = 0
+        for r in range(wl.n_ranks):
+            g0, g1 = int(wl.rank_ptr[r]), int(wl.rank_ptr[r + 1])
+            t0, t1 = int(wl.sample_ptr[g0]), int(wl.sample_ptr[g1])
+            toks = I.token_ids(wl.token_seed, wl.token_start + t0, t1 - t0)
+            tok_start = np.full(max(wl.n_samples, 1), -(1 << 40), dtype=np.int64)   # other ranks: never dereferenced
+            tok_start[g0:g1] = wl.sample_ptr[g0:g1] - t0
+            ref = oracle.collate_rank(plan, r, toks if len(toks) else np.zeros(1, np.int32), tok_start, wl.span_ptr,
+                                      wl.span_lo, wl.span_hi, shift_labels=wl.params["shift_labels"])
+            assert ref["elem_lo"] == at
+            at = ref["elem_hi"]
+            for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+                assert np.array_equal(ref[name], out[name][ref["elem_lo"]:ref["elem_hi"]]), (wl.name, r, name)
+            K = plan.n_steps
+            assert np.array_equal(ref["grp_valid_tokens"], out["grp_valid_tokens"][r * K:(r + 1) * K])
+        assert at == plan.total_elems
+
+
 # ---------------------------------------------------------------------------------------
 # input generator: counter-based token ids
 # ---------------------------------------------------------------------------------------
