@@ -44,13 +44,29 @@ struct RoundRec {
     int64_t emitted_round;  // samples emitted in this round over all ranks
 };
 
-// Totals produced by the finalize kernels.
-struct PlanTotals {
+// Sizes of the plan, DEVICE-RESIDENT: written by the planning kernels (the host uploads the first four
+// fields in the staged path, where it has read them round by round), read by every later kernel, so that
+// nothing after the round loop needs a size from the host.  A pinned host copy is filled by the slot scan.
+struct PlanDims {
+    int32_t n_steps;      // slots per rank
+    int32_t n_rounds;     // protocol rounds including the terminal check
+    int32_t stop_reason;  // ODB_STOP_*
+    int32_t complete;     // 1 = the protocol has terminated: the tables may be finalised and collated
+    int32_t err;          // ODB_ERR_CAPACITY flagged by the slot scan against the caller's capacities
+    int32_t bad_length;
+    int64_t n_slots;
     int64_t total_elems;
     int64_t samples_emitted;
     int64_t padded_elems;
     unsigned long long real_tokens;
     int64_t samples_left;
+};
+
+// The caller's output capacities, checked on the device by the slot scan (odb_run enqueues the collate
+// kernels before the host has seen the plan sizes).
+struct CapCheck {
+    int64_t arena, slots, ids, steps, left;  // < 0 = not checked
+    int64_t tiles;                           // capacity of the library's tile table
 };
 
 // State of one tile of the slot scan (decoupled look-back): flag 0 = nothing, 1 = agg valid,
@@ -70,15 +86,16 @@ struct __align__(16) RowDesc {
     int32_t lo0, hi0, lo1, hi1;
 };
 
-// Where a 512-element chunk of the arenas starts: its slot's geometry and the (row, column) of the
-// chunk's first element.  32 bytes, two 16-byte loads.
-struct __align__(16) ChunkRec {
+// Where a 4096-element tile of the arenas starts: the slot that holds the tile's first element (or the
+// alignment gap behind that slot's block) and its geometry.  32 bytes, two 16-byte loads; a warp derives
+// (row, column) of its own 512-element chunk from it with one division.
+struct __align__(16) TileRec {
     int64_t off_s;   // grp_offset of the slot
     int32_t slot;
     uint32_t W;      // grp_width
     uint32_t area;   // count * width
     uint32_t sp_s;   // grp_sample_ptr of the slot (index of its first row)
-    uint32_t b0, t0; // row / column of the chunk's first element (when it lies inside the block)
+    uint32_t pad_[2];
 };
 
 struct CollateArgs {
@@ -91,7 +108,8 @@ struct CollateArgs {
     const int64_t *grp_sample_ptr;  // n_slots + 1
     const int32_t *grp_count;
     const int32_t *grp_width;
-    const ChunkRec *chunks;
+    const TileRec *tiles;
+    const PlanDims *dims;  // non-NULL: the launch covers the whole arena, whose size is read on the device
     int32_t *ids;
     int32_t *labels;
     int32_t *pos;
@@ -102,6 +120,13 @@ struct CollateArgs {
     int64_t elem_lo;
     int64_t tile_lo, tile_hi;  // tiles [tile_lo, tile_hi) are visited by this launch
     int32_t pad_id, ignore_index, shift_labels;
+    // fused epilogue (whole-arena launches): the last CTA to finish sums the valid tokens per step
+    // (Eq. 2's T_tok) and copies grp_valid into the caller's table
+    unsigned int *done_counter;
+    int32_t R;
+    int64_t *step_valid;
+    int64_t *user_step_valid;
+    int32_t *user_grp_valid;
 };
 
 // k_post: table copies (4-byte words) + the per-step valid-token totals
@@ -113,7 +138,8 @@ struct CopyJob {
 struct PostArgs {
     CopyJob job[16];
     int n_jobs;
-    int R, n_steps;
+    int R;
+    const PlanDims *dims;
     const int32_t *grp_valid;
     int64_t *step_valid;
     int64_t *user_step_valid;
