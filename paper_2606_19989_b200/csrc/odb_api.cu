@@ -77,12 +77,15 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->emit_snap);
     cudaFree(c->d_arrived);
     cudaFree(c->d_rec);
-    cudaFree(c->d_tot);
+    cudaFree(c->d_dims);
+    cudaFree(c->d_done_ctr);
     cudaFree(c->d_tile_counter);
     cudaFree(c->gs_local);
     cudaFree(c->gs_world);
     if (c->h_rec) cudaFreeHost(c->h_rec);
-    if (c->h_tot) cudaFreeHost(c->h_tot);
+    if (c->h_dims) cudaFreeHost(c->h_dims);
+    if (c->h_dims_up) cudaFreeHost(c->h_dims_up);
+    if (c->ev_plan) cudaEventDestroy(c->ev_plan);
     c->st_count.release();
     c->st_width.release();
     c->st_real.release();
@@ -104,7 +107,7 @@ static void free_all(odb_ctx *c) {
     c->step_valid.release();
     c->rows.release();
     c->row_sp.release();
-    c->chunks.release();
+    c->tiles.release();
     c->hs_lengths.release();
     c->hs_tokens.release();
     c->hs_span_lo.release();
@@ -193,10 +196,16 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->emit_snap, R);
     if (e == cudaSuccess) e = dev_alloc(&c->d_arrived, R);
     if (e == cudaSuccess) e = dev_alloc(&c->d_rec, 1);
-    if (e == cudaSuccess) e = dev_alloc(&c->d_tot, 1);
+    if (e == cudaSuccess) e = dev_alloc(&c->d_dims, 1);
+    if (e == cudaSuccess) e = cudaMemset(c->d_dims, 0, sizeof(PlanDims));
+    if (e == cudaSuccess) e = dev_alloc(&c->d_done_ctr, 2);
+    if (e == cudaSuccess) e = cudaMemset(c->d_done_ctr, 0, 2 * sizeof(unsigned int));
     if (e == cudaSuccess) e = dev_alloc(&c->d_tile_counter, R + 1);  // one work counter per pipelined launch
     if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_rec, sizeof(RoundRec));
-    if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_tot, sizeof(PlanTotals));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_dims, sizeof(PlanDims));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_dims_up, sizeof(PlanDims));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&c->h_rank_off, (R + 1) * sizeof(int64_t));
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_plan, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_status, cudaEventDisableTiming);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
@@ -503,6 +512,40 @@ int odb_round_status(odb_ctx *c, int32_t *h_done, int32_t *h_T) {
     return ODB_OK;
 }
 
+// internal rank-major tables for a plan of at most n_slots slots / n_steps steps
+static int ensure_plan_tables(odb_ctx *c, size_t n_slots, size_t n_steps) {
+    const size_t R = (size_t)c->prm.n_ranks;
+    CU(c, c->grp_count.ensure(n_slots + 1));
+    CU(c, c->grp_width.ensure(n_slots + 1));
+    CU(c, c->grp_round.ensure(n_slots + 1));
+    CU(c, c->grp_valid.ensure(n_slots + 1));
+    CU(c, c->grp_real.ensure(n_slots + 1));
+    CU(c, c->grp_origin.ensure(n_slots + 1));
+    CU(c, c->grp_offset.ensure(n_slots + 1));
+    CU(c, c->grp_sample_ptr.ensure(n_slots + 1));
+    CU(c, c->grp_sample_ids.ensure((size_t)c->n_total + 1));
+    CU(c, c->left_out.ensure((size_t)c->n_total + 1));
+    CU(c, c->left_ptr.ensure(R + 1));
+    CU(c, c->step_valid.ensure(n_steps + 1));
+    return ODB_OK;
+}
+
+static void fill_info(odb_ctx *c) {
+    odb_plan_info &I = c->info;
+    const PlanDims &D = *c->h_dims;
+    I.n_rounds = c->n_rounds;
+    I.n_steps = c->n_steps;
+    I.stop_reason = c->stop_reason;
+    I.reserved = 0;
+    I.n_slots = (int64_t)c->prm.n_ranks * c->n_steps;
+    I.total_elems = D.total_elems;
+    I.samples_emitted = D.samples_emitted;
+    I.samples_left = c->n_total - D.samples_emitted;  // Lemma 1: emitted + un-emitted = all
+    I.real_tokens = (int64_t)D.real_tokens;
+    I.padded_elems = D.padded_elems;
+    c->info_valid = true;
+}
+
 int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
     if (!c || !h_out) return ODB_ERR_INVALID_ARG;
     if (c->state == 5 && c->info_valid) {
@@ -514,55 +557,25 @@ int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
     cudaStream_t st = c->last_stream;  // the stream of the last odb_form_groups / odb_align
     const int R = c->prm.n_ranks;
     const size_t n_slots = (size_t)R * (size_t)c->n_steps;
-    CU(c, c->grp_count.ensure(n_slots + 1));
-    CU(c, c->grp_width.ensure(n_slots + 1));
-    CU(c, c->grp_round.ensure(n_slots + 1));
-    CU(c, c->grp_valid.ensure(n_slots + 1));
-    CU(c, c->grp_real.ensure(n_slots + 1));
-    CU(c, c->grp_origin.ensure(n_slots + 1));
-    CU(c, c->grp_offset.ensure(n_slots + 1));
-    CU(c, c->grp_sample_ptr.ensure(n_slots + 1));
-    CU(c, c->grp_sample_ids.ensure((size_t)c->n_total + 1));
-    CU(c, c->left_out.ensure((size_t)c->n_total + 1));
-    CU(c, c->left_ptr.ensure((size_t)R + 1));
-    CU(c, c->step_valid.ensure((size_t)c->n_steps + 1));
-    CU(c, launch_finalize(c, st));
-    CU(c, cudaMemcpyAsync(c->h_tot, c->d_tot, sizeof(PlanTotals), cudaMemcpyDeviceToHost, st));
-    CU(c, cudaStreamSynchronize(st));
-    odb_plan_info &I = c->info;
-    I.n_rounds = c->n_rounds;
-    I.n_steps = c->n_steps;
-    I.stop_reason = c->stop_reason;
-    I.reserved = 0;
-    I.n_slots = (int64_t)n_slots;
-    I.total_elems = c->h_tot->total_elems;
-    I.samples_emitted = c->h_tot->samples_emitted;
-    I.samples_left = c->n_total - c->h_tot->samples_emitted;  // Lemma 1: emitted + un-emitted = all
-    I.real_tokens = (int64_t)c->h_tot->real_tokens;
-    I.padded_elems = c->h_tot->padded_elems;
-    c->info_valid = true;
-    c->state = 5;
-    *h_out = I;
-    return ODB_OK;
-}
-
-// Collate preparation.  The row descriptors run on the caller's stream; the chunk table and the id /
-// leftover tables (independent of them, and of each other's outputs) run beside them on an auxiliary
-// stream and are joined before anything that follows on `st`.
-static int launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
-                       const int32_t *d_span_hi, cudaStream_t st) {
-    if (!c->aux_stream) {
-        CU(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
-        CU(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
-        CU(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    {
+        int rc = ensure_plan_tables(c, n_slots, (size_t)c->n_steps);
+        if (rc != ODB_OK) return rc;
     }
-    CU(c, cudaEventRecord(c->ev_fork, st));
-    CU(c, cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
-    CU(c, launch_chunk_table(c, c->aux_stream));
-    CU(c, launch_ids_left(c, c->aux_stream));
-    CU(c, cudaEventRecord(c->ev_join, c->aux_stream));
-    CU(c, launch_row_desc(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st));
-    CU(c, cudaStreamWaitEvent(st, c->ev_join, 0));
+    // the host has followed the rounds: its sizes go up, every later kernel reads them on the device
+    PlanDims *U = c->h_dims_up;
+    memset(U, 0, sizeof(*U));
+    U->n_steps = c->n_steps;
+    U->n_rounds = c->n_rounds;
+    U->stop_reason = c->stop_reason;
+    U->complete = 1;
+    CU(c, cudaMemcpyAsync(c->d_dims, U, sizeof(PlanDims), cudaMemcpyHostToDevice, st));
+    CapCheck cap = {-1, -1, -1, -1, -1, -1};
+    CU(c, launch_finalize(c, (int64_t)n_slots, cap, c->h_rank_off, st));
+    CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
+    CU(c, cudaStreamSynchronize(st));
+    fill_info(c);
+    c->state = 5;
+    *h_out = c->info;
     return ODB_OK;
 }
 
@@ -581,13 +594,16 @@ static int check_capacity(const odb_ctx *c, const odb_outputs *o) {
     return ODB_OK;
 }
 
-// One collate launch over the arena elements [elem_lo, elem_hi) (both multiples of 16: slot offsets).
-// Tiles are arena-aligned; a tile that straddles elem_lo / elem_hi is visited by both neighbouring
-// launches, each writing only its own elements.  `counter` is this launch's zeroed work counter.
-static int collate_range(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_span_lo, const int32_t *d_span_hi,
-                         const odb_outputs *o, int64_t elem_lo, int64_t elem_hi, unsigned long long *counter,
-                         cudaStream_t st) {
+// One collate launch.  whole = false: the arena elements [elem_lo, elem_hi) (both multiples of 16: slot
+// offsets; tiles are arena-aligned, a tile that straddles elem_lo / elem_hi is visited by both neighbouring
+// launches, each writing only its own elements); `counter` is this launch's zeroed work counter.
+// whole = true: the whole arena, its extent read on the device from PlanDims (tile_bound = the most tiles
+// it can have, for the grid), with the fused epilogue (step totals, the caller's valid-token tables).
+static int collate_launch(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_span_lo, const int32_t *d_span_hi,
+                          const odb_outputs *o, bool whole, int64_t elem_lo, int64_t elem_hi, int64_t tile_bound,
+                          unsigned long long *counter, cudaStream_t st) {
     CollateArgs A;
+    memset(&A, 0, sizeof(A));
     A.tokens = d_tokens;
     A.rows = c->rows.p;
     A.row_sp = c->row_sp.p;
@@ -597,82 +613,80 @@ static int collate_range(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_s
     A.grp_sample_ptr = c->grp_sample_ptr.p;
     A.grp_count = c->grp_count.p;
     A.grp_width = c->grp_width.p;
-    A.chunks = c->chunks.p;
+    A.tiles = c->tiles.p;
+    A.dims = c->d_dims;
     A.ids = o->d_input_ids;
     A.labels = o->d_labels;
     A.pos = o->d_position_ids;
     A.mask = o->d_attention_mask;
     A.grp_valid = c->grp_valid.p;
     A.tile_counter = counter;
-    A.total_elems = elem_hi;
-    A.elem_lo = elem_lo;
-    A.tile_lo = elem_lo / kColTile;
-    A.tile_hi = (elem_hi + kColTile - 1) / kColTile;
     A.pad_id = c->prm.pad_id;
     A.ignore_index = c->prm.ignore_index;
     A.shift_labels = c->prm.shift_labels;
+    if (whole) {
+        A.total_elems = 0;  // read on the device
+        A.elem_lo = 0;
+        A.tile_lo = 0;
+        A.tile_hi = tile_bound;
+        A.done_counter = c->d_done_ctr + 1;
+        A.R = c->prm.n_ranks;
+        A.step_valid = c->step_valid.p;
+        A.user_step_valid = o->d_step_valid_tokens;
+        A.user_grp_valid = o->d_grp_valid_tokens;
+    } else {
+        A.total_elems = elem_hi;
+        A.elem_lo = elem_lo;
+        A.tile_lo = elem_lo / kColTile;
+        A.tile_hi = (elem_hi + kColTile - 1) / kColTile;
+    }
     CU(c, launch_collate(c, A, st));
+    return ODB_OK;
+}
+
+static int check_pointers(const int32_t *d_tokens, const odb_outputs *o) {
+    if (((uintptr_t)d_tokens & 15u) != 0) return ODB_ERR_INVALID_ARG;
+    if (((uintptr_t)o->d_input_ids & 15u) || ((uintptr_t)o->d_labels & 15u) || ((uintptr_t)o->d_position_ids & 15u) ||
+        ((uintptr_t)o->d_attention_mask & 15u))
+        return ODB_ERR_INVALID_ARG;
+    return ODB_OK;
+}
+
+// Everything behind the slot scan: collate preparation (one launch), the collate kernel over the whole
+// arena (with the step totals fused into its last CTA).  Nothing here needs a size from the host: the
+// kernels read PlanDims.  rows_bound / tile_bound size the library's row and tile tables.
+static int enqueue_collate(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
+                           const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *o, int64_t rows_bound,
+                           int64_t tile_bound, cudaStream_t st) {
+    CU(c, c->rows.ensure((size_t)rows_bound + 1));
+    CU(c, c->row_sp.ensure((size_t)rows_bound + 1));
+    CU(c, c->tiles.ensure((size_t)tile_bound + 2));
+    CU(c, launch_prep(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st));
+    // ev[1]..ev[2] brackets the collate kernel alone; what precedes it is ev[0]..ev[1]
+    if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
+    {
+        int rc = collate_launch(c, d_tokens, d_span_lo, d_span_hi, o, true, 0, 0, tile_bound, c->d_tile_counter, st);
+        if (rc != ODB_OK) return rc;
+    }
+    if (c->timing) {
+        CU(c, cudaEventRecord(c->ev[2], st));
+        CU(c, cudaEventRecord(c->ev[3], st));
+    }
     return ODB_OK;
 }
 
 static int collate_impl(odb_ctx *c, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
                         const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *o, cudaStream_t st) {
     const odb_plan_info &I = c->info;
-    const int R = c->prm.n_ranks;
-    const size_t n_slots = (size_t)I.n_slots;
     if (I.samples_emitted > 0 && (!d_tokens || !d_sample_ptr)) return ODB_ERR_INVALID_ARG;
-    if (((uintptr_t)d_tokens & 15u) != 0) return ODB_ERR_INVALID_ARG;
-    if (((uintptr_t)o->d_input_ids & 15u) || ((uintptr_t)o->d_labels & 15u) || ((uintptr_t)o->d_position_ids & 15u) ||
-        ((uintptr_t)o->d_attention_mask & 15u))
-        return ODB_ERR_INVALID_ARG;
-    CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
-    CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
-    const int64_t n_chunks = (I.total_elems + kColChunk - 1) / kColChunk;
-    CU(c, c->chunks.ensure((size_t)n_chunks + 1));
     {
-        int rc = launch_prep(c, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, st);
+        int rc = check_pointers(d_tokens, o);
         if (rc != ODB_OK) return rc;
     }
-    // ev[1]..ev[2] brackets the collate kernel alone; the pre/post work is ev[0]..ev[1] / ev[2]..ev[3]
-    if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
-    {  // whole arena in one launch
-        int rc = collate_range(c, d_tokens, d_span_lo, d_span_hi, o, 0, I.total_elems, c->d_tile_counter, st);
-        if (rc != ODB_OK) return rc;
-    }
-    if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
-    {  // step totals + every table copy in one launch
-        PostArgs P;
-        memset(&P, 0, sizeof(P));
-        P.R = R;
-        P.n_steps = I.n_steps;
-        P.grp_valid = c->grp_valid.p;
-        P.step_valid = c->step_valid.p;
-        P.user_step_valid = o->d_step_valid_tokens;
-        auto job = [&](void *dst, const void *src, size_t n, size_t elem) {
-            if (!dst || n == 0) return;
-            P.job[P.n_jobs].dst = dst;
-            P.job[P.n_jobs].src = src;
-            P.job[P.n_jobs].words = (int64_t)(n * elem / 4);
-            P.n_jobs++;
-        };
-        job(o->d_grp_count, c->grp_count.p, n_slots, 4);
-        job(o->d_grp_width, c->grp_width.p, n_slots, 4);
-        job(o->d_grp_round, c->grp_round.p, n_slots, 4);
-        job(o->d_grp_valid_tokens, c->grp_valid.p, n_slots, 4);
-        job(o->d_grp_real_tokens, c->grp_real.p, n_slots, 4);
-        job(o->d_grp_origin, c->grp_origin.p, n_slots, 4);
-        job(o->d_grp_offset, c->grp_offset.p, n_slots, 8);
-        job(o->d_grp_sample_ptr, c->grp_sample_ptr.p, n_slots + 1, 8);
-        job(o->d_grp_sample_ids, c->grp_sample_ids.p, (size_t)I.samples_emitted, 4);
-        job(o->d_step_samples, c->step_samples.p, (size_t)I.n_steps, 4);
-        job(o->d_left_ptr, c->left_ptr.p, (size_t)R + 1, 8);
-        job(o->d_left_ids, c->left_out.p, (size_t)I.samples_left, 4);
-        CU(c, launch_post(c, P, st));
-    }
-    if (c->timing) {
-        CU(c, cudaEventRecord(c->ev[3], st));
-        timing_done(c);
-    }
+    const int64_t n_tiles = (I.total_elems + kColTile - 1) / kColTile;
+    int rc = enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, I.samples_emitted, n_tiles, st);
+    if (rc != ODB_OK) return rc;
+    if (c->timing) timing_done(c);
     c->collated = true;
     return ODB_OK;
 }
@@ -714,15 +728,91 @@ static int run_rounds(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_ran
 int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
             const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo, const int32_t *d_span_hi,
             const odb_outputs *o, odb_plan_info *h_out, void *stream) {
-    if (!c || !o || !h_out) return ODB_ERR_INVALID_ARG;
+    if (!c || !o || !h_out || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
     if (c->world_ranks) return ODB_ERR_STATE;  // the caller drives the rounds and their collectives
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = run_rounds(c, d_lengths, h_rank_ptr, h_out, st);
+    const int R = c->prm.n_ranks;
+    // When every rank's whole stream fits its window and the output slots are unlimited, the protocol
+    // normally ends with the first round (equal group-count targets are reached by splitting; only unequal
+    // windows overflow).  Then NOTHING needs the host between the first kernel and the last: the round is
+    // closed on the device (k_commit), and the slot scan, the collate preparation and the collate kernel are
+    // enqueued behind it; they read the plan sizes from PlanDims and check the caller's capacities on the
+    // device.  The host waits only for the sizes (an event behind the slot scan), while the collate kernel
+    // is already running.  If the device says another round is due, those launches were no-ops and the
+    // staged loop below takes over.
+    int64_t max_nr = 0;
+    for (int r = 0; r < R; ++r) max_nr = std::max(max_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
+    const bool arenas = o->d_input_ids && o->d_labels && o->d_position_ids && o->d_attention_mask;
+    const bool speculate = (c->prm.buffer_size == 0 || c->prm.buffer_size >= max_nr) && c->prm.slot_capacity == 0 &&
+                           arenas && d_tokens && d_sample_ptr && check_pointers(d_tokens, o) == ODB_OK;
+    odb_reset(c);
+    CU(c, cudaSetDevice(c->device));
+    if (c->timing) {
+        timing_begin(c);
+        CU(c, cudaEventRecord(c->ev[0], st));
+    }
+    int32_t done = 0, T = 0;
+    int rc = odb_form_groups(c, d_lengths, h_rank_ptr, st);
+    if (rc != ODB_OK) return rc;
+    bool collate_enqueued = false;
+    if (speculate && c->last_T != 0) {  // an emitting round was formed
+        rc = odb_align(c, st);
+        if (rc != ODB_OK) return rc;
+        const int64_t steps_bound = c->round_window;  // T_grp <= the largest window
+        const int64_t slots_bound = (int64_t)R * steps_bound;
+        rc = ensure_plan_tables(c, (size_t)slots_bound, (size_t)steps_bound);
+        if (rc != ODB_OK) return rc;
+        const int64_t tile_bound = (std::max<int64_t>(o->arena_capacity, 0) + kColTile - 1) / kColTile;
+        CU(c, c->tiles.ensure((size_t)tile_bound + 2));
+        const bool any_slot_tab = o->d_grp_count || o->d_grp_width || o->d_grp_round || o->d_grp_valid_tokens ||
+                                  o->d_grp_real_tokens || o->d_grp_origin || o->d_grp_offset || o->d_grp_sample_ptr;
+        CapCheck cap;
+        cap.arena = std::max<int64_t>(o->arena_capacity, 0);
+        cap.slots = any_slot_tab ? o->slot_capacity_alloc : -1;
+        cap.ids = o->d_grp_sample_ids ? o->ids_capacity : -1;
+        cap.steps = (o->d_step_samples || o->d_step_valid_tokens) ? o->step_capacity_alloc : -1;
+        cap.left = o->d_left_ids ? o->left_capacity : -1;
+        cap.tiles = tile_bound;
+        CU(c, launch_finalize(c, slots_bound, cap, c->h_rank_off, st));
+        CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
+        CU(c, cudaEventRecord(c->ev_plan, st));
+        rc = enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, c->n_total, tile_bound, st);
+        if (rc != ODB_OK) return rc;
+        CU(c, cudaEventSynchronize(c->ev_plan));  // the sizes are here; the collate kernel is running
+        collate_enqueued = c->h_dims->complete != 0;
+        rc = odb_round_status(c, &done, &T);
+        if (rc != ODB_OK) return rc;
+    } else {
+        rc = odb_align(c, st);
+        if (rc != ODB_OK) return rc;
+        rc = odb_round_status(c, &done, &T);
+        if (rc != ODB_OK) return rc;
+    }
+    while (!done) {  // (after a speculated round that ended the protocol: the terminal check, no launch)
+        rc = odb_form_groups(c, d_lengths, h_rank_ptr, st);
+        if (rc != ODB_OK) return rc;
+        rc = odb_align(c, st);
+        if (rc != ODB_OK) return rc;
+        rc = odb_round_status(c, &done, &T);
+        if (rc != ODB_OK) return rc;
+    }
+    if (collate_enqueued) {
+        const PlanDims &D = *c->h_dims;
+        // the device closed the round with the predicates the host state machine has just applied
+        if (D.n_steps != c->n_steps || D.n_rounds != c->n_rounds || D.stop_reason != c->stop_reason) return ODB_ERR_STATE;
+        fill_info(c);
+        c->state = 5;
+        *h_out = c->info;
+        if (D.err) return D.err;  // ODB_ERR_CAPACITY: the kernels behind the slot scan wrote nothing
+        if (c->timing) timing_done(c);
+        c->collated = true;
+        return ODB_OK;
+    }
+    rc = odb_plan_query(c, h_out);
     if (rc != ODB_OK) return rc;
     rc = check_capacity(c, o);
     if (rc != ODB_OK) return rc;
-    rc = collate_impl(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
-    return rc;
+    return collate_impl(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
 }
 
 static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
@@ -748,7 +838,6 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
         CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
         CU(c, cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
         CU(c, cudaEventCreateWithFlags(&c->copy_ev, cudaEventDisableTiming));
-        CU(c, cudaMallocHost((void **)&c->h_rank_off, (size_t)(R + 1) * sizeof(int64_t)));
         c->tok_ev.assign((size_t)R, nullptr);
         c->col_ev.assign((size_t)R, nullptr);
         for (int r = 0; r < R; ++r) {
@@ -824,28 +913,26 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
     dev.d_attention_mask = c->hs_mask.p;
     dev.arena_capacity = (int64_t)E;
     const size_t n_slots = (size_t)I.n_slots;
+    CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
+    CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
+    CU(c, c->tiles.ensure((size_t)((I.total_elems + kColTile - 1) / kColTile) + 2));
+    CU(c, cudaStreamWaitEvent(st, c->copy_ev, 0));  // sample_ptr / spans have landed
+    // row descriptors, tile table, id / leftover tables, cleared counters: one launch
+    CU(c, launch_prep(c, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p, c->hs_span_hi.p,
+                      nullptr, st));
+    if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
     if (E > 0) {
-        CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
-        CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
-        CU(c, c->chunks.ensure((size_t)((I.total_elems + kColChunk - 1) / kColChunk) + 1));
-        CU(c, cudaStreamWaitEvent(st, c->copy_ev, 0));  // sample_ptr / spans have landed
-        rc = launch_prep(c, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p,
-                         c->hs_span_hi.p, st);
-        if (rc != ODB_OK) return rc;
-        CU(c, cudaMemsetAsync(c->d_tile_counter, 0, (size_t)(R + 1) * sizeof(unsigned long long), st));
-        // arena offset of every rank's first slot (slots are rank-major): R+1 strided int64
-        CU(c, cudaMemcpy2DAsync(c->h_rank_off, 8, c->grp_offset.p, (size_t)I.n_steps * 8, 8, (size_t)R + 1,
-                                cudaMemcpyDeviceToHost, st));
-        CU(c, cudaStreamSynchronize(st));
-        if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
         // The pipeline: rank r's slots are collated as soon as its tokens have landed, and its slice of
         // the four arenas goes back on the device -> host stream while later ranks are still being
-        // uploaded and collated (both directions of the host link busy at once).
+        // uploaded and collated (both directions of the host link busy at once).  The arena offset of
+        // every rank's first slot was written to pinned memory by the slot scan, together with the plan
+        // sizes the host has already waited for (odb_plan_query): no further synchronisation here.
         for (int r = 0; r < R; ++r) {
             const int64_t lo = c->h_rank_off[r], hi = c->h_rank_off[r + 1];
             if (hi <= lo) continue;
             CU(c, cudaStreamWaitEvent(st, c->tok_ev[r], 0));
-            rc = collate_range(c, c->hs_tokens.p, c->hs_span_lo.p, c->hs_span_hi.p, &dev, lo, hi, c->d_tile_counter + r, st);
+            rc = collate_launch(c, c->hs_tokens.p, c->hs_span_lo.p, c->hs_span_hi.p, &dev, false, lo, hi, 0,
+                                c->d_tile_counter + r, st);
             if (rc != ODB_OK) {
                 drain();
                 return rc;
@@ -858,19 +945,13 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
             CU(c, cudaMemcpyAsync(ho->d_position_ids + lo, c->hs_pos.p + lo, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
             CU(c, cudaMemcpyAsync(ho->d_attention_mask + lo, c->hs_mask.p + lo, n, cudaMemcpyDeviceToHost, c->d2h_stream));
         }
-        if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
-    } else {
-        CU(c, launch_ids_left(c, st));  // nothing to collate, but the leftover table is still owed
-        if (c->timing) {
-            CU(c, cudaEventRecord(c->ev[1], st));
-            CU(c, cudaEventRecord(c->ev[2], st));
-        }
     }
+    if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
     {  // step totals (Eq. 2's T_tok per step)
         PostArgs P;
         memset(&P, 0, sizeof(P));
         P.R = R;
-        P.n_steps = I.n_steps;
+        P.dims = c->d_dims;
         P.grp_valid = c->grp_valid.p;
         P.step_valid = c->step_valid.p;
         CU(c, launch_post(c, P, st));

@@ -4,7 +4,10 @@
 //
 // Paper: collate_fn P:28; pad to the group max P:416-420; valid tokens t_r of Eq. 2 P:60-63.
 // Tensor contract: BASELINE.json north_star (readings U16-U18).
+#include <cstring>
+
 #include "odb_internal.cuh"
+#include "odb_device.cuh"
 
 namespace odb {
 
@@ -16,42 +19,163 @@ namespace odb {
     } while (0)
 
 // ---------------------------------------------------------------------------------------------
-// row descriptors: one thread per sample (coalesced reads of sample_ptr / lengths / span CSR); the
-// row index of an emitted sample is its rank's first row + its position in the rank's emit region.
-// Also clears what the collate kernel accumulates into: grp_valid and the tile counter.
-// grid = (ceil(max n_r / 256), R)
+// Collate preparation, ONE launch with three roles told apart by the block index (all sizes come from
+// the device-resident PlanDims; the launch is skipped on the device when the plan is not complete or the
+// caller's capacities are too small):
+//
+//   rows   one thread per sample (coalesced reads of sample_ptr / lengths / span CSR): the 32-byte
+//          RowDesc of every emitted sample, stored at its rank's first row + its position in the rank's
+//          emit region;
+//   tiles  one warp per slot, a lane per 4096-element tile whose first element lies in the slot's
+//          16-aligned region [grp_offset[s], grp_offset[s+1]) (IDLE slots own none): the 32-byte TileRec
+//          the collate kernel starts a tile with.  These blocks also clear what the collate kernel
+//          accumulates into (grp_valid, the work counters) and copy the plan tables into the caller's;
+//   ids    one block per rank: the slot CSR's ids are the rank's emit region (slots of a rank are in
+//          emit order), and the un-emitted local ids, ascending (Lemma 1: buffer + sampler-pending).
 // ---------------------------------------------------------------------------------------------
-__global__ void k_row_desc(int n_steps, int64_t n_slots, const int64_t *__restrict__ rank_ptr,
-                           const int32_t *__restrict__ len, const int32_t *__restrict__ emit_pos,
-                           const int64_t *__restrict__ sample_ptr, const int64_t *__restrict__ span_ptr,
-                           const int32_t *__restrict__ span_lo, const int32_t *__restrict__ span_hi,
-                           const int64_t *__restrict__ grp_sample_ptr, RowDesc *__restrict__ rows,
-                           int64_t *__restrict__ row_sp, int32_t *__restrict__ grp_valid,
-                           unsigned long long *__restrict__ tile_counter) {
-    const int r = blockIdx.y;
-    const int64_t lin = ((int64_t)r * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
-    for (int64_t s = lin; s < n_slots; s += (int64_t)gridDim.x * gridDim.y * blockDim.x) grp_valid[s] = 0;
-    if (lin == 0) *tile_counter = 0ull;
-    const int64_t base = rank_ptr[r];
-    const int n_r = (int)(rank_ptr[r + 1] - base);
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+constexpr int kPrepThreads = 1024;
+
+struct PrepJob {
+    void *dst;
+    const void *src;
+    int kind;  // words to copy: 0 = n_slots, 1 = 2 n_slots, 2 = 2 (n_slots + 1), 3 = n_steps
+};
+
+struct PrepArgs {
+    const PlanDims *dims;
+    int R;
+    // rows
+    int rows_gx;  // blocks per rank
+    const int64_t *rank_ptr;
+    const int32_t *len;
+    const int32_t *emit_pos;
+    const int64_t *sample_ptr;
+    const int64_t *span_ptr;
+    const int32_t *span_lo;
+    const int32_t *span_hi;
+    const int64_t *grp_sample_ptr;
+    RowDesc *rows;
+    int64_t *row_sp;
+    // tiles
+    int tile_blocks;
+    const int64_t *grp_offset;
+    const int32_t *grp_count;
+    const int32_t *grp_width;
+    TileRec *tiles;
+    int32_t *grp_valid;
+    unsigned long long *tile_counter;
+    int n_counters;
+    PrepJob job[10];
+    int n_jobs;
+    // ids
+    const int32_t *emit_cur;
+    const int32_t *emit_ids;
+    int32_t *grp_sample_ids, *user_ids;
+    int64_t *left_ptr, *user_left_ptr;
+    int32_t *left_out, *user_left;
+};
+
+__device__ __forceinline__ void prep_rows(const PrepArgs &A, int n_steps, int b) {
+    const int r = b / A.rows_gx, bx = b - r * A.rows_gx;
+    const int64_t base = A.rank_ptr[r];
+    const int n_r = (int)(A.rank_ptr[r + 1] - base);
+    const int i = bx * kPrepThreads + threadIdx.x;
     if (i >= n_r) return;
     const int64_t g = base + i;
-    const int p = emit_pos[g];
+    const int p = A.emit_pos[g];
     if (p < 0) return;
-    const int64_t q = grp_sample_ptr[(int64_t)r * n_steps] + p;
+    const int64_t q = A.grp_sample_ptr[(int64_t)r * n_steps] + p;
     RowDesc d;
-    d.tok = sample_ptr[g];
-    d.len = len[g];
-    const int64_t sp = span_ptr ? span_ptr[g] : 0;
-    const int ns = span_ptr ? (int)(span_ptr[g + 1] - sp) : 0;
+    d.tok = A.sample_ptr[g];
+    d.len = A.len[g];
+    const int64_t sp = A.span_ptr ? A.span_ptr[g] : 0;
+    const int ns = A.span_ptr ? (int)(A.span_ptr[g + 1] - sp) : 0;
     d.nspan = ns;
-    d.lo0 = ns > 0 ? span_lo[sp] : 0;
-    d.hi0 = ns > 0 ? span_hi[sp] : 0;
-    d.lo1 = ns > 1 ? span_lo[sp + 1] : 0;
-    d.hi1 = ns > 1 ? span_hi[sp + 1] : 0;
-    rows[q] = d;
-    if (ns > 2) row_sp[q] = sp;  // only read on the CSR path (more than two spans): skip the scattered 8-byte store
+    d.lo0 = ns > 0 ? A.span_lo[sp] : 0;
+    d.hi0 = ns > 0 ? A.span_hi[sp] : 0;
+    d.lo1 = ns > 1 ? A.span_lo[sp + 1] : 0;
+    d.hi1 = ns > 1 ? A.span_hi[sp + 1] : 0;
+    A.rows[q] = d;
+    if (ns > 2) A.row_sp[q] = sp;  // only read on the CSR path (more than two spans): skip the scattered 8-byte store
+}
+
+__device__ __forceinline__ void prep_tiles(const PrepArgs &A, int n_steps, int64_t n_slots, int b) {
+    const int64_t tid = (int64_t)b * kPrepThreads + threadIdx.x, nth = (int64_t)A.tile_blocks * kPrepThreads;
+    for (int64_t s = tid; s < n_slots; s += nth) A.grp_valid[s] = 0;
+    if (tid < A.n_counters) A.tile_counter[tid] = 0ull;
+    const int lane = threadIdx.x & 31;
+    for (int64_t s = tid >> 5; s < n_slots; s += nth >> 5) {
+        const int64_t o = A.grp_offset[s], on = A.grp_offset[s + 1];
+        const int64_t t_lo = (o + kColTile - 1) / kColTile, t_hi = (on + kColTile - 1) / kColTile;
+        if (t_lo >= t_hi) continue;
+        TileRec rec;
+        rec.off_s = o;
+        rec.slot = (int32_t)s;
+        rec.W = (uint32_t)A.grp_width[s];
+        rec.area = (uint32_t)A.grp_count[s] * rec.W;
+        rec.sp_s = (uint32_t)A.grp_sample_ptr[s];
+        rec.pad_[0] = rec.pad_[1] = 0u;
+        for (int64_t t = t_lo + lane; t < t_hi; t += 32) A.tiles[t] = rec;
+    }
+    for (int j = 0; j < A.n_jobs; ++j) {
+        const int kind = A.job[j].kind;
+        const int64_t words = kind == 0 ? n_slots : kind == 1 ? 2 * n_slots : kind == 2 ? 2 * (n_slots + 1) : (int64_t)n_steps;
+        const uint32_t *__restrict__ src = reinterpret_cast<const uint32_t *>(A.job[j].src);
+        uint32_t *__restrict__ dst = reinterpret_cast<uint32_t *>(A.job[j].dst);
+        for (int64_t i = tid; i < words; i += nth) dst[i] = src[i];
+    }
+}
+
+__device__ __forceinline__ void prep_ids(const PrepArgs &A, int n_steps, int r) {
+    __shared__ int s_scan[34];
+    __shared__ long long s_scan64[34];
+    const int R = A.R;
+    const int64_t base = A.rank_ptr[r];
+    const int n_r = (int)(A.rank_ptr[r + 1] - base);
+    const int ec = A.emit_cur[r];
+    if (ec > 0) {
+        const int64_t q0 = A.grp_sample_ptr[(int64_t)r * n_steps];
+        for (int j = threadIdx.x; j < ec; j += blockDim.x) {
+            const int32_t id = A.emit_ids[base + j];
+            A.grp_sample_ids[q0 + j] = id;
+            if (A.user_ids) A.user_ids[q0 + j] = id;
+        }
+    }
+    long long part = 0;
+    for (int q = threadIdx.x; q < r; q += blockDim.x) part += (A.rank_ptr[q + 1] - A.rank_ptr[q]) - A.emit_cur[q];
+    long long lbase;
+    (void)block_excl_scan<long long>(part, s_scan64, lbase);
+    const int cnt = n_r - ec;
+    if (cnt > 0) {
+        const int32_t *ep = A.emit_pos + base;
+        int32_t *out = A.left_out + lbase;
+        int32_t *uout = A.user_left ? A.user_left + lbase : nullptr;
+        (void)block_compact(
+            n_r, s_scan, [&](int i) { return ep[i] < 0; },
+            [&](int i, int kidx) {
+                out[kidx] = i;
+                if (uout) uout[kidx] = i;
+            });
+    }
+    if (threadIdx.x == 0) {
+        A.left_ptr[r] = lbase;
+        if (A.user_left_ptr) A.user_left_ptr[r] = lbase;
+        if (r == R - 1) {
+            A.left_ptr[R] = lbase + cnt;
+            if (A.user_left_ptr) A.user_left_ptr[R] = lbase + cnt;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kPrepThreads) k_prep(const PrepArgs A) {
+    if (!A.dims->complete || A.dims->err) return;
+    const int n_steps = A.dims->n_steps;
+    const int64_t n_slots = (int64_t)A.R * n_steps;
+    const int b = blockIdx.x;
+    const int nb_rows = A.rows_gx * A.R;
+    if (b < nb_rows) prep_rows(A, n_steps, b);
+    else if (b < nb_rows + A.tile_blocks) prep_tiles(A, n_steps, n_slots, b - nb_rows);
+    else prep_ids(A, n_steps, b - nb_rows - A.tile_blocks);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -247,30 +371,60 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
     constexpr int kWarps = kColThreads / 32;
     static_assert(kColChunk == 512 && kColTile == kWarps * kColChunk, "a chunk is one 16-element unit per lane");
     const int4 *tok4 = reinterpret_cast<const int4 *>(A.tokens);
+    // a whole-arena launch reads its extent on the device (it may have been enqueued before the host saw
+    // the plan) and does nothing when the plan is not complete or the caller's buffers are too small
+    int64_t total_elems = A.total_elems, tile_hi = A.tile_hi;
+    if (A.done_counter) {
+        if (!A.dims->complete || A.dims->err) return;
+        total_elems = A.dims->total_elems;
+        tile_hi = (total_elems + kColTile - 1) / kColTile;
+    }
     for (;;) {
         __syncthreads();  // everyone has read the previous s_grab
         if (threadIdx.x == 0) s_grab = (long long)atomicAdd(A.tile_counter, (unsigned long long)kColGrab);
         __syncthreads();
         const int64_t tile_begin = A.tile_lo + s_grab;
-        if (tile_begin >= A.tile_hi) break;
-        const int64_t tile_end = min(tile_begin + kColGrab, A.tile_hi);
+        if (tile_begin >= tile_hi) break;
+        const int64_t tile_end = min(tile_begin + kColGrab, tile_hi);
 #pragma unroll 1
         for (int64_t tile = tile_begin; tile < tile_end; ++tile) {
             const int64_t chunk = tile * kWarps + warp;
             const int64_t a0 = chunk * kColChunk;
-            if (a0 >= A.total_elems) break;
+            if (a0 >= total_elems) break;
             if (a0 + kColChunk <= A.elem_lo) continue;  // another launch's elements (odb_run_host pipelines ranks)
-            const int4 *cp = reinterpret_cast<const int4 *>(A.chunks + chunk);
-            const int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
+            // the tile's record: the slot that holds the tile's first element, and its geometry
+            const int4 *tp = reinterpret_cast<const int4 *>(A.tiles + tile);
+            const int4 c0 = __ldg(tp), c1 = __ldg(tp + 1);
             int64_t off_s = (int64_t)(((uint64_t)(uint32_t)c0.y << 32) | (uint32_t)c0.x);
             int64_t s = c0.z;
             uint32_t W = (uint32_t)c0.w, area = (uint32_t)c1.x;
             int64_t sp_s = (int64_t)(uint32_t)c1.y;
+            if (a0 >= off_s + (((int64_t)area + 15) & ~15ll)) {
+                // this warp's chunk starts in a later slot of the tile: find the slot j >= s + 1 whose region
+                // [grp_offset[j], grp_offset[j + 1]) holds a0, 32 upper boundaries at a time (IDLE slots have
+                // empty regions and are skipped over)
+                int64_t cand = s + 1;
+                const int64_t n_slots = A.dims->n_slots;
+                for (;;) {  // warp-uniform
+                    const int64_t idx = cand + 1 + lane;
+                    const int64_t v = idx <= n_slots ? __ldg(A.grp_offset + idx) : 0x7fffffffffffffffll;
+                    const uint32_t gt = __ballot_sync(ODB_FULL_MASK, v > a0);
+                    if (gt) {
+                        s = cand + (__ffs(gt) - 1);
+                        break;
+                    }
+                    cand += 32;
+                }
+                off_s = __ldg(A.grp_offset + s);
+                W = (uint32_t)__ldg(A.grp_width + s);
+                area = (uint32_t)__ldg(A.grp_count + s) * W;
+                sp_s = __ldg(A.grp_sample_ptr + s);
+            }
             const int64_t e0 = a0 - off_s;
             int acc = 0;
             if (e0 + kColChunk <= (int64_t)area) {
                 // ---------------- interior chunk: lane = one 16-element unit ----------------
-                const uint32_t b0 = (uint32_t)c1.z, t0 = (uint32_t)c1.w;
+                const uint32_t b0 = (uint32_t)e0 / W, t0 = (uint32_t)e0 - b0 * W;  // row / column of the chunk's first element
                 const bool wide = W >= (uint32_t)kColChunk;  // then t0 + 16 l < 2 W: the row index grows by 0 or 1
                 // ceil(2^32 / W): floor(n / W) == umulhi(n, M) for n < 1024 and 2 <= W < 512
                 const uint32_t M = (W >= 2u && !wide) ? 0xFFFFFFFFu / W + 1u : 0u;
@@ -371,7 +525,7 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
 #pragma unroll 1
                 for (int k = 0; k < 4; ++k) {
                     const int64_t a = a0 + (int64_t)(k * 32 + lane) * 4;
-                    if (a >= A.total_elems) break;
+                    if (a >= total_elems) break;
                     if (a < A.elem_lo) continue;
                     bool moved = false;
                     while (a >= off_n) {
@@ -419,6 +573,31 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
             }
         }
     }
+    // Whole-arena launches: the last CTA to finish sums the valid tokens per step over the ranks (Eq. 2's
+    // T_tok per step) and hands the per-slot counts to the caller -- what used to be a separate launch.
+    if (A.done_counter) {
+        __shared__ int s_last;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            s_last = (atomicAdd(A.done_counter, 1u) == gridDim.x - 1u) ? 1 : 0;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const int n_steps = A.dims->n_steps;
+            const int64_t n_slots = A.dims->n_slots;
+            for (int k = threadIdx.x; k < n_steps; k += blockDim.x) {
+                long long t = 0;
+                for (int r = 0; r < A.R; ++r) t += __ldcg(A.grp_valid + (int64_t)r * n_steps + k);
+                A.step_valid[k] = t;
+                if (A.user_step_valid) A.user_step_valid[k] = t;
+            }
+            if (A.user_grp_valid)
+                for (int64_t q = threadIdx.x; q < n_slots; q += blockDim.x) A.user_grp_valid[q] = __ldcg(A.grp_valid + q);
+            if (threadIdx.x == 0) *A.done_counter = 0u;
+        }
+    }
 }
 
 // After the collate kernel, one launch: step_valid_tokens[k] = sum over ranks of grp_valid_tokens[r][k]
@@ -426,9 +605,10 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
 // plan tables into the caller's buffers (4-byte words).
 __global__ void k_post(const PostArgs A) {
     const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t k = tid; k < A.n_steps; k += nth) {
+    const int n_steps = A.dims->n_steps;
+    for (int64_t k = tid; k < n_steps; k += nth) {
         long long s = 0;
-        for (int r = 0; r < A.R; ++r) s += A.grp_valid[(int64_t)r * A.n_steps + k];
+        for (int r = 0; r < A.R; ++r) s += A.grp_valid[(int64_t)r * n_steps + k];
         A.step_valid[k] = s;
         if (A.user_step_valid) A.user_step_valid[k] = s;
     }
@@ -442,21 +622,69 @@ __global__ void k_post(const PostArgs A) {
 // ---------------------------------------------------------------------------------------------
 // host launchers
 // ---------------------------------------------------------------------------------------------
-cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
-                            const int32_t *d_span_lo, const int32_t *d_span_hi, cudaStream_t st) {
+cudaError_t launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
+                        const int32_t *d_span_hi, const odb_outputs *u, cudaStream_t st) {
     const int R = c->prm.n_ranks;
-    const int64_t n_slots = (int64_t)R * c->n_steps;
-    const int gx = std::max((c->max_nr + 255) / 256, 1);
-    k_row_desc<<<dim3(gx, R), 256, 0, st>>>(c->n_steps, n_slots, c->d_rank_ptr, c->d_lengths, c->emit_pos, d_sample_ptr,
-                                            d_span_ptr, d_span_lo, d_span_hi, c->grp_sample_ptr.p, c->rows.p, c->row_sp.p,
-                                            c->grp_valid.p, c->d_tile_counter);
+    PrepArgs A;
+    memset(&A, 0, sizeof(A));
+    A.dims = c->d_dims;
+    A.R = R;
+    A.rows_gx = std::max((c->max_nr + kPrepThreads - 1) / kPrepThreads, 1);
+    A.rank_ptr = c->d_rank_ptr;
+    A.len = c->d_lengths;
+    A.emit_pos = c->emit_pos;
+    A.sample_ptr = d_sample_ptr;
+    A.span_ptr = d_span_ptr;
+    A.span_lo = d_span_lo;
+    A.span_hi = d_span_hi;
+    A.grp_sample_ptr = c->grp_sample_ptr.p;
+    A.rows = c->rows.p;
+    A.row_sp = c->row_sp.p;
+    // one warp per slot; the bound on the slot count is what the tables were sized for
+    const int64_t slots_bound = (int64_t)c->grp_count.cap;
+    A.tile_blocks = (int)std::max<int64_t>(1, std::min<int64_t>((slots_bound * 32 + kPrepThreads - 1) / kPrepThreads,
+                                                                (int64_t)c->sm_count * 2));
+    A.grp_offset = c->grp_offset.p;
+    A.grp_count = c->grp_count.p;
+    A.grp_width = c->grp_width.p;
+    A.tiles = c->tiles.p;
+    A.grp_valid = c->grp_valid.p;
+    A.tile_counter = c->d_tile_counter;
+    A.n_counters = R + 1;
+    auto job = [&](void *dst, const void *src, int kind) {
+        if (!dst) return;
+        A.job[A.n_jobs].dst = dst;
+        A.job[A.n_jobs].src = src;
+        A.job[A.n_jobs].kind = kind;
+        A.n_jobs++;
+    };
+    if (u) {
+        job(u->d_grp_count, c->grp_count.p, 0);
+        job(u->d_grp_width, c->grp_width.p, 0);
+        job(u->d_grp_round, c->grp_round.p, 0);
+        job(u->d_grp_real_tokens, c->grp_real.p, 0);
+        job(u->d_grp_origin, c->grp_origin.p, 0);
+        job(u->d_grp_offset, c->grp_offset.p, 1);
+        job(u->d_grp_sample_ptr, c->grp_sample_ptr.p, 2);
+        job(u->d_step_samples, c->step_samples.p, 3);
+    }
+    A.emit_cur = c->emit_cur;
+    A.emit_ids = c->emit_ids;
+    A.grp_sample_ids = c->grp_sample_ids.p;
+    A.left_ptr = c->left_ptr.p;
+    A.left_out = c->left_out.p;
+    if (u) {
+        A.user_ids = u->d_grp_sample_ids;
+        A.user_left_ptr = u->d_left_ptr;
+        A.user_left = u->d_left_ids;
+    }
+    const int blocks = A.rows_gx * R + A.tile_blocks + R;
+    k_prep<<<blocks, kPrepThreads, 0, st>>>(A);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
 
 cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st) {
-    const int64_t n_tiles = args.tile_hi - args.tile_lo;
-    if (n_tiles <= 0) return cudaSuccess;
     const int sh = args.shift_labels ? 1 : 0;
     if (c->col_occ[sh] == 0) {
         cudaError_t e = sh ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->col_occ[sh], k_collate<true>, kColThreads, 0)
@@ -464,7 +692,11 @@ cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st)
         if (e != cudaSuccess) return e;
         if (c->col_occ[sh] < 1) c->col_occ[sh] = 1;
     }
-    int blocks = (int)std::min<int64_t>((n_tiles + kColGrab - 1) / kColGrab, (int64_t)c->sm_count * c->col_occ[sh]);
+    // tiles the launch can have to visit: known for a ranged launch, bounded by the caller's arena otherwise
+    const int64_t n_tiles = args.tile_hi - args.tile_lo;
+    if (n_tiles <= 0 && !args.done_counter) return cudaSuccess;
+    int blocks = (int)std::min<int64_t>(std::max<int64_t>((n_tiles + kColGrab - 1) / kColGrab, 1),
+                                        (int64_t)c->sm_count * c->col_occ[sh]);
     if (sh) k_collate<true><<<blocks, kColThreads, 0, st>>>(args);
     else k_collate<false><<<blocks, kColThreads, 0, st>>>(args);
     ODB_LAUNCH_CHECK(c);
@@ -472,7 +704,7 @@ cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st)
 }
 
 cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st) {
-    int64_t work = args.n_steps;
+    int64_t work = c->n_steps;
     for (int j = 0; j < args.n_jobs; ++j) work = std::max(work, args.job[j].words);
     if (work == 0) return cudaSuccess;
     int blocks = (int)std::min<int64_t>((work + 255) / 256, (int64_t)c->sm_count * 8);

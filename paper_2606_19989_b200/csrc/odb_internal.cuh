@@ -242,8 +242,11 @@ struct odb_ctx {
     bool arrived_set = false;
     odb::RoundRec *d_rec = nullptr;
     odb::RoundRec *h_rec = nullptr;  // pinned
-    odb::PlanTotals *d_tot = nullptr;
-    odb::PlanTotals *h_tot = nullptr;  // pinned
+    odb::PlanDims *d_dims = nullptr;
+    odb::PlanDims *h_dims = nullptr;     // pinned: the device's sizes, copied back behind the slot scan
+    odb::PlanDims *h_dims_up = nullptr;  // pinned: the host's sizes on their way up (staged path)
+    unsigned int *d_done_ctr = nullptr;  // 2: "last CTA" counters of k_commit / k_collate (self-resetting)
+    cudaEvent_t ev_plan = nullptr;       // recorded behind the slot scan's read-back
     unsigned long long *d_tile_counter = nullptr;
 
     // step-major staging tables [step * R + r], growable
@@ -259,7 +262,7 @@ struct odb_ctx {
     odb::DevBuf<int64_t> left_ptr, step_valid;
     odb::DevBuf<odb::RowDesc> rows;
     odb::DevBuf<int64_t> row_sp;
-    odb::DevBuf<odb::ChunkRec> chunks;
+    odb::DevBuf<odb::TileRec> tiles;
 
     // device staging for odb_run_host
     odb::DevBuf<int32_t> hs_lengths, hs_tokens, hs_span_lo, hs_span_hi, hs_ids, hs_labels, hs_pos;
@@ -282,12 +285,12 @@ cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commi
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: (G_r, S_r) pairs for the all_gather
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce
-cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st);     // A9: rank-major tables, offsets, totals
-cudaError_t launch_ids_left(odb_ctx *c, cudaStream_t st);     // slot CSR ids + leftover CSR
+// A9: rank-major tables, offsets, totals (sizes from the device-resident PlanDims)
+cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st);
 // ---- launchers implemented in odb_collate.cu -------------------------------------------------
-cudaError_t launch_row_desc(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
-                            const int32_t *d_span_lo, const int32_t *d_span_hi, cudaStream_t st);
-cudaError_t launch_chunk_table(odb_ctx *c, cudaStream_t st);
+// collate preparation in ONE launch: row descriptors, tile table, slot-id / leftover tables, table copies
+cudaError_t launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
+                        const int32_t *d_span_hi, const odb_outputs *user, cudaStream_t st);
 cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st);
 cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st);
 // ---- odb_scale.cu ------------------------------------------------------------------------------

@@ -5,6 +5,7 @@
 // Paper: /root/reference/PAPER.md (P:<line>).  Section 2.2 P:32-36 and Eq. 1 (grouping), Eq. 3
 // (target), Alg. 1 P:258-279 (split / overflow), P:28 (IDLE slots), Thm 2 P:48 + P:347 (quota).
 #include "odb_internal.cuh"
+#include "odb_device.cuh"
 
 namespace odb {
 
@@ -13,54 +14,6 @@ namespace odb {
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t key_len(uint64_t k) { return (uint32_t)(k >> 32); }
 __device__ __forceinline__ int32_t key_id(uint64_t k) { return (int32_t)(uint32_t)(k & 0xffffffffull); }
-
-template <class V>
-__device__ __forceinline__ V warp_incl_scan(V v) {
-    const int lane = threadIdx.x & 31;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        V n = __shfl_up_sync(ODB_FULL_MASK, v, d);
-        if (lane >= d) v += n;
-    }
-    return v;
-}
-
-// Exclusive scan of one value per thread over the CTA.  `s` is shared scratch of 34 V's.
-// Returns the exclusive prefix; `total` receives the CTA-wide sum.  Contains barriers: every
-// thread of the CTA must call it.
-template <class V>
-__device__ __forceinline__ V block_excl_scan(V v, V *s, V &total) {
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    V inc = warp_incl_scan(v);
-    if (lane == 31) s[w] = inc;
-    __syncthreads();
-    if (w == 0) {
-        V x = lane < nw ? s[lane] : (V)0;
-        V xi = warp_incl_scan(x);
-        s[lane] = xi - x;
-        if (lane == 31) s[32] = xi;
-    }
-    __syncthreads();
-    V r = inc - v + s[w];
-    total = s[32];
-    __syncthreads();
-    return r;
-}
-
-// Stream compaction over i in [0, n): emit(i, k) for the k-th i with pred(i).  Returns the count.
-template <class Pred, class Emit>
-__device__ __forceinline__ int block_compact(int n, int *s, Pred pred, Emit emit) {
-    int carry = 0;
-    for (int base = 0; base < n; base += blockDim.x) {
-        int i = base + threadIdx.x;
-        int f = (i < n && pred(i)) ? 1 : 0;
-        int tot;
-        int ex = block_excl_scan<int>(f, s, tot);
-        if (f) emit(i, carry + ex);
-        carry += tot;
-    }
-    return carry;
-}
 
 __device__ __forceinline__ int next_pow2(int n) {
     int p = 1;
@@ -623,8 +576,8 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
 // position), compacts the leftovers, advances the rank state and counts the ranks that will be
 // finished next round.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRankThreads)
-k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
+__device__ __forceinline__ void
+commit_body(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
          const int32_t *__restrict__ G_arr, int R, const int32_t *__restrict__ agpos, const int32_t *__restrict__ agcnt,
          const int32_t *__restrict__ agorg, int32_t *__restrict__ agoff, const int32_t *__restrict__ step_samples, int step_base, int round, int join_mode,
          long long quota, long long emitted_before, int32_t *__restrict__ st_count, int32_t *__restrict__ st_width,
@@ -801,6 +754,57 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
     }
 }
 
+// The kernel: the body above, then -- single-process mode -- the LAST CTA to finish closes the round on
+// the device: it evaluates the termination predicates on the status every rank shares (Thm 3 proof
+// P:341) exactly as the host state machine does, and writes the plan sizes into the device-resident
+// PlanDims, so that the kernels after the round loop (slot scan, collate preparation, collate) can be
+// enqueued behind this one without a host round trip: they read `complete` and skip if another round is due.
+__global__ void __launch_bounds__(kRankThreads)
+k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
+         const int32_t *__restrict__ G_arr, int R, const int32_t *__restrict__ agpos, const int32_t *__restrict__ agcnt,
+         const int32_t *__restrict__ agorg, int32_t *__restrict__ agoff, const int32_t *__restrict__ step_samples, int step_base, int round, int join_mode,
+         long long quota, long long emitted_before, int32_t *__restrict__ st_count, int32_t *__restrict__ st_width,
+         int32_t *__restrict__ st_real, int32_t *__restrict__ st_round, int32_t *__restrict__ st_origin,
+         uint8_t *__restrict__ posflag,
+         int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
+         int32_t *fetch_pos, int32_t *emit_cur, const int32_t *__restrict__ emit_snap, RoundRec *rec, PlanDims *dims,
+         unsigned int *done_ctr) {
+    commit_body(keys, rank_ptr, S_arr, G_arr, R, agpos, agcnt, agorg, agoff, step_samples, step_base, round, join_mode,
+                quota, emitted_before, st_count, st_width, st_real, st_round, st_origin, posflag, emit_ids, emit_pos,
+                left_ids, n_left, fetch_pos, emit_cur, emit_snap, rec);
+    if (!dims) return;  // distributed mode: the host decides from the gathered status
+    __shared__ int s_last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned int t = atomicAdd(done_ctr, 1u);
+        s_last = (t == gridDim.x * gridDim.y - 1u) ? 1 : 0;
+    }
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence();
+        const volatile RoundRec *vr = rec;
+        const int T_emit = vr->T_emit, quota_hit = vr->quota_hit, n_fin = vr->n_finished, bad = vr->bad_length;
+        int complete = 0, stop = 0, n_rounds = 0;
+        if (quota_hit) {  // Thm 2 / P:347: the trainer-side emitted-sample count reached the quota
+            complete = 1;
+            stop = ODB_STOP_QUOTA;
+            n_rounds = round + 1;
+        } else if (join_mode ? (n_fin == R) : (n_fin > 0)) {  // the next round is the terminal check
+            complete = 1;
+            stop = join_mode ? ODB_STOP_ALL_FINISHED : ODB_STOP_LOGICAL;
+            n_rounds = round + 2;
+        }
+        dims->n_steps = step_base + T_emit;
+        dims->n_rounds = n_rounds;
+        dims->stop_reason = stop;
+        dims->bad_length = bad;
+        dims->err = 0;
+        dims->complete = bad ? 0 : complete;
+        *done_ctr = 0u;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // A9 and the rank-major plan tables.
 //
@@ -810,193 +814,143 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
 // area (-> grp_offset), the sample count (-> grp_sample_ptr), count*width and the real tokens
 // (-> totals).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int ld_flag(const int *p) {
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_flag(int *p, int v) {
-    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
 __global__ void __launch_bounds__(kFinThreads)
-k_fin_scan(int R, int n_steps, const int32_t *__restrict__ st_count, const int32_t *__restrict__ st_width,
+k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const int32_t *__restrict__ st_width,
            const int32_t *__restrict__ st_real, const int32_t *__restrict__ st_round,
            const int32_t *__restrict__ st_origin, int32_t *__restrict__ grp_count, int32_t *__restrict__ grp_width,
            int32_t *__restrict__ grp_round, int32_t *__restrict__ grp_real, int32_t *__restrict__ grp_origin,
            int64_t *__restrict__ grp_offset, int64_t *__restrict__ grp_sample_ptr, ScanTile *tiles, unsigned int *ticket,
-           PlanTotals *tot) {
+           CapCheck cap, int64_t n_total, int64_t *rank_off) {
     __shared__ long long s_scan64[34];
     __shared__ long long s_base[4];
     __shared__ int s_tile;
-    if (threadIdx.x == 0) s_tile = (int)atomicAdd(ticket, 1u);
-    __syncthreads();
-    const int tile = s_tile;
+    if (!dims->complete) return;  // enqueued behind a round that did not terminate the protocol
+    const int n_steps = dims->n_steps;
     const int64_t n_slots = (int64_t)R * n_steps;
-    const int64_t s0 = (int64_t)tile * kFinTile + (int64_t)threadIdx.x * kFinItems;
-    long long v[4][kFinItems];
-    long long sum[4] = {0, 0, 0, 0};
+    const int64_t n_tiles = max((n_slots + kFinTile - 1) / kFinTile, (int64_t)1);
+    for (;;) {
+        __syncthreads();  // everyone has read the previous s_tile / s_base
+        if (threadIdx.x == 0) s_tile = (int)atomicAdd(ticket, 1u);
+        __syncthreads();
+        const int tile = s_tile;
+        if ((int64_t)tile >= n_tiles) break;
+        const int64_t s0 = (int64_t)tile * kFinTile + (int64_t)threadIdx.x * kFinItems;
+        long long v[4][kFinItems];
+        long long sum[4] = {0, 0, 0, 0};
 #pragma unroll
-    for (int i = 0; i < kFinItems; ++i) {
-        const int64_t s = s0 + i;
-        long long c = 0, w = 0, re = 0;
-        if (s < n_slots) {
-            const int r = (int)(s / n_steps);
-            const int k = (int)(s - (int64_t)r * n_steps);
-            const int64_t src = (int64_t)k * R + r;
-            c = st_count[src];
-            w = st_width[src];
-            re = st_real[src];
-            grp_count[s] = (int32_t)c;
-            grp_width[s] = (int32_t)w;
-            grp_real[s] = (int32_t)re;
-            grp_round[s] = st_round[src];
-            grp_origin[s] = st_origin[src];
-        }
-        const long long area = c * w;
-        v[0][i] = (area + 15) / 16 * 16;
-        v[1][i] = c;
-        v[2][i] = area;
-        v[3][i] = re;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) sum[q] += v[q][i];
-    }
-    long long ex[4], total[4];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) ex[q] = block_excl_scan<long long>(sum[q], s_scan64, total[q]);
-    ScanTile *me = tiles + tile;
-    if (threadIdx.x == 0) {
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            me->agg[q] = total[q];
-            if (tile == 0) me->inc[q] = total[q];
-        }
-        st_flag(&me->flag, tile == 0 ? 2 : 1);
-        if (tile == 0) {
-#pragma unroll
-            for (int q = 0; q < 4; ++q) s_base[q] = 0;
-        }
-    }
-    if (tile > 0 && threadIdx.x < 32) {  // warp 0 looks back over up to 32 predecessors at a time
-        const int lane = threadIdx.x;
-        long long acc[4] = {0, 0, 0, 0};
-        int t = tile - 1;
-        while (true) {
-            const int tt = t - lane;
-            int f = 2;  // tiles before the first count as "inclusive prefix 0"
-            long long x[4] = {0, 0, 0, 0};
-            if (tt >= 0) {
-                do {
-                    f = ld_flag(&tiles[tt].flag);
-                } while (f == 0);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) x[q] = (f == 2) ? __ldcg(&tiles[tt].inc[q]) : __ldcg(&tiles[tt].agg[q]);
+        for (int i = 0; i < kFinItems; ++i) {
+            const int64_t s = s0 + i;
+            long long c = 0, w = 0, re = 0;
+            if (s < n_slots) {
+                const int r = (int)(s / n_steps);
+                const int k = (int)(s - (int64_t)r * n_steps);
+                const int64_t src = (int64_t)k * R + r;
+                c = st_count[src];
+                w = st_width[src];
+                re = st_real[src];
+                grp_count[s] = (int32_t)c;
+                grp_width[s] = (int32_t)w;
+                grp_real[s] = (int32_t)re;
+                grp_round[s] = st_round[src];
+                grp_origin[s] = st_origin[src];
             }
-            const uint32_t done = __ballot_sync(ODB_FULL_MASK, f == 2);
-            const int first = __ffs(done) - 1;  // nearest tile with an inclusive prefix (done != 0 once tt < 0)
+            const long long area = c * w;
+            v[0][i] = (area + 15) / 16 * 16;
+            v[1][i] = c;
+            v[2][i] = area;
+            v[3][i] = re;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) sum[q] += v[q][i];
+        }
+        long long ex[4], total[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) ex[q] = block_excl_scan<long long>(sum[q], s_scan64, total[q]);
+        ScanTile *me = tiles + tile;
+        if (threadIdx.x == 0) {
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                long long y = (done == 0 || lane <= first) ? x[q] : 0;
-#pragma unroll
-                for (int dlt = 16; dlt > 0; dlt >>= 1) y += __shfl_xor_sync(ODB_FULL_MASK, y, dlt);
-                acc[q] += y;
+                me->agg[q] = total[q];
+                if (tile == 0) me->inc[q] = total[q];
             }
-            if (done) break;
-            t -= 32;
-        }
-        if (lane == 0) {
+            st_flag(&me->flag, tile == 0 ? 2 : 1);
+            if (tile == 0) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                s_base[q] = acc[q];
-                me->inc[q] = acc[q] + total[q];
+                for (int q = 0; q < 4; ++q) s_base[q] = 0;
             }
-            st_flag(&me->flag, 2);
         }
-    }
-    __syncthreads();
-    long long run_o = s_base[0] + ex[0], run_p = s_base[1] + ex[1];
+        if (tile > 0 && threadIdx.x < 32) {  // warp 0 looks back over up to 32 predecessors at a time
+            const int lane = threadIdx.x;
+            long long acc[4] = {0, 0, 0, 0};
+            int t = tile - 1;
+            while (true) {
+                const int tt = t - lane;
+                int f = 2;  // tiles before the first count as "inclusive prefix 0"
+                long long x[4] = {0, 0, 0, 0};
+                if (tt >= 0) {
+                    do {
+                        f = ld_flag(&tiles[tt].flag);
+                    } while (f == 0);
 #pragma unroll
-    for (int i = 0; i < kFinItems; ++i) {
-        const int64_t s = s0 + i;
-        if (s < n_slots) {
-            grp_offset[s] = run_o;
-            grp_sample_ptr[s] = run_p;
+                    for (int q = 0; q < 4; ++q) x[q] = (f == 2) ? __ldcg(&tiles[tt].inc[q]) : __ldcg(&tiles[tt].agg[q]);
+                }
+                const uint32_t done = __ballot_sync(ODB_FULL_MASK, f == 2);
+                const int first = __ffs(done) - 1;  // nearest tile with an inclusive prefix (done != 0 once tt < 0)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    long long y = (done == 0 || lane <= first) ? x[q] : 0;
+#pragma unroll
+                    for (int dlt = 16; dlt > 0; dlt >>= 1) y += __shfl_xor_sync(ODB_FULL_MASK, y, dlt);
+                    acc[q] += y;
+                }
+                if (done) break;
+                t -= 32;
+            }
+            if (lane == 0) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    s_base[q] = acc[q];
+                    me->inc[q] = acc[q] + total[q];
+                }
+                st_flag(&me->flag, 2);
+            }
         }
-        run_o += v[0][i];
-        run_p += v[1][i];
-    }
-    const int64_t n_tiles = (n_slots + kFinTile - 1) / kFinTile;
-    if (threadIdx.x == 0 && (int64_t)tile == max(n_tiles, (int64_t)1) - 1) {
-        grp_offset[n_slots] = s_base[0] + total[0];
-        grp_sample_ptr[n_slots] = s_base[1] + total[1];
-        tot->total_elems = s_base[0] + total[0];
-        tot->samples_emitted = s_base[1] + total[1];
-        tot->padded_elems = s_base[2] + total[2];
-        tot->real_tokens = (unsigned long long)(s_base[3] + total[3]);
-    }
-}
-
-// Chunk table (A10's work list): chunk c = arena elements [512 c, 512 c + 512).  A slot owns the
-// chunks whose first element lies in its 16-aligned region [grp_offset[s], grp_offset[s+1]) (IDLE
-// slots own none); one warp per slot writes 32-byte records with everything the collate kernel
-// needs to start on the chunk: the slot's geometry and (row, column) of the chunk's first element.
-__global__ void k_chunk_table(int64_t n_slots, const int64_t *__restrict__ grp_offset, const int32_t *__restrict__ grp_count,
-                              const int32_t *__restrict__ grp_width, const int64_t *__restrict__ grp_sample_ptr,
-                              ChunkRec *__restrict__ chunks) {
-    const int lane = threadIdx.x & 31;
-    const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
-    for (int64_t s = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; s < n_slots; s += warps) {
-        const int64_t o = grp_offset[s], on = grp_offset[s + 1];
-        const int64_t c_lo = (o + kColChunk - 1) / kColChunk, c_hi = (on + kColChunk - 1) / kColChunk;
-        if (c_lo >= c_hi) continue;
-        ChunkRec rec;
-        rec.off_s = o;
-        rec.slot = (int32_t)s;
-        rec.W = (uint32_t)grp_width[s];
-        rec.area = (uint32_t)grp_count[s] * rec.W;
-        rec.sp_s = (uint32_t)grp_sample_ptr[s];
-        for (int64_t c = c_lo + lane; c < c_hi; c += 32) {
-            const uint32_t e0 = (uint32_t)(c * kColChunk - o);  // < area: no multiple of 16 lies in the alignment gap
-            rec.b0 = rec.W ? e0 / rec.W : 0u;
-            rec.t0 = e0 - rec.b0 * rec.W;
-            chunks[c] = rec;
+        __syncthreads();
+        long long run_o = s_base[0] + ex[0], run_p = s_base[1] + ex[1];
+#pragma unroll
+        for (int i = 0; i < kFinItems; ++i) {
+            const int64_t s = s0 + i;
+            if (s < n_slots) {
+                grp_offset[s] = run_o;
+                grp_sample_ptr[s] = run_p;
+                if (rank_off && s % n_steps == 0) rank_off[s / n_steps] = run_o;  // arena offset of each rank's first slot
+            }
+            run_o += v[0][i];
+            run_p += v[1][i];
         }
-    }
-}
-
-// Per rank: the slot CSR's ids are the rank's emit region (slots of a rank are in emit order), and
-// the un-emitted local ids, ascending (Lemma 1: buffer + sampler-pending).
-__global__ void __launch_bounds__(kRankThreads)
-k_ids_left(int R, int n_steps, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ emit_cur,
-           const int32_t *__restrict__ emit_ids, const int32_t *__restrict__ emit_pos,
-           const int64_t *__restrict__ grp_sample_ptr, int32_t *__restrict__ grp_sample_ids, int64_t *__restrict__ left_ptr,
-           int32_t *__restrict__ left_out, PlanTotals *tot) {
-    __shared__ int s_scan[34];
-    __shared__ long long s_scan64[34];
-    const int r = blockIdx.x;
-    const int64_t base = rank_ptr[r];
-    const int n_r = (int)(rank_ptr[r + 1] - base);
-    const int ec = emit_cur[r];
-    if (ec > 0) {
-        const int64_t q0 = grp_sample_ptr[(int64_t)r * n_steps];
-        for (int j = threadIdx.x; j < ec; j += blockDim.x) grp_sample_ids[q0 + j] = emit_ids[base + j];
-    }
-    long long part = 0;
-    for (int q = threadIdx.x; q < r; q += blockDim.x) part += (rank_ptr[q + 1] - rank_ptr[q]) - emit_cur[q];
-    long long lbase;
-    (void)block_excl_scan<long long>(part, s_scan64, lbase);
-    const int cnt = n_r - ec;
-    if (cnt > 0) {
-        const int32_t *ep = emit_pos + base;
-        int32_t *out = left_out + lbase;
-        (void)block_compact(
-            n_r, s_scan, [&](int i) { return ep[i] < 0; }, [&](int i, int kidx) { out[kidx] = i; });
-    }
-    if (threadIdx.x == 0) {
-        left_ptr[r] = lbase;
-        if (r == R - 1) {
-            left_ptr[R] = lbase + cnt;
-            tot->samples_left = lbase + cnt;
+        if (threadIdx.x == 0 && (int64_t)tile == n_tiles - 1) {
+            const long long tot_e = s_base[0] + total[0], tot_s = s_base[1] + total[1];
+            grp_offset[n_slots] = tot_e;
+            grp_sample_ptr[n_slots] = tot_s;
+            if (rank_off) {
+                rank_off[R] = tot_e;
+                if (n_steps == 0)
+                    for (int r = 0; r < R; ++r) rank_off[r] = 0;
+            }
+            dims->n_slots = n_slots;
+            dims->total_elems = tot_e;
+            dims->samples_emitted = tot_s;
+            dims->padded_elems = s_base[2] + total[2];
+            dims->real_tokens = (unsigned long long)(s_base[3] + total[3]);
+            dims->samples_left = n_total - tot_s;  // Lemma 1: emitted + un-emitted = all
+            // the caller's capacities (odb_run enqueues the collate kernels before the host sees the sizes)
+            int err = 0;
+            if (cap.arena >= 0 && tot_e > cap.arena) err = ODB_ERR_CAPACITY;
+            if (cap.tiles >= 0 && (tot_e + kColTile - 1) / kColTile > cap.tiles) err = ODB_ERR_CAPACITY;
+            if (cap.slots >= 0 && n_slots > cap.slots) err = ODB_ERR_CAPACITY;
+            if (cap.ids >= 0 && tot_s > cap.ids) err = ODB_ERR_CAPACITY;
+            if (cap.steps >= 0 && n_steps > cap.steps) err = ODB_ERR_CAPACITY;
+            if (cap.left >= 0 && n_total - tot_s > cap.left) err = ODB_ERR_CAPACITY;
+            dims->err = err;
         }
     }
 }
@@ -1102,7 +1056,7 @@ static cudaError_t launch_commit_kernel(odb_ctx *c, cudaStream_t st) {
                                          (long long)c->prm.emitted_so_far + (long long)c->samples_emitted, c->st_count.p,
                                          c->st_width.p, c->st_real.p, c->st_round.p, c->st_origin.p, c->posflag,
                                          c->emit_ids, c->emit_pos, c->left_ids, c->n_left, c->fetch_pos, c->emit_cur,
-                                         c->emit_snap, c->d_rec);
+                                         c->emit_snap, c->d_rec, c->world_ranks ? nullptr : c->d_dims, c->d_done_ctr);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
@@ -1140,40 +1094,23 @@ cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
     return cudaSuccess;
 }
 
-cudaError_t launch_finalize(odb_ctx *c, cudaStream_t st) {
+// A9.  `slots_bound` >= the number of slots the plan can hold (the host may not have seen the plan yet);
+// the grid is persistent: tiles are taken by ticket.
+cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st) {
     const int R = c->prm.n_ranks;
-    const int64_t n_slots = (int64_t)R * c->n_steps;
-    const int64_t n_tiles = std::max<int64_t>((n_slots + kFinTile - 1) / kFinTile, 1);
+    const int64_t n_tiles = std::max<int64_t>((slots_bound + kFinTile - 1) / kFinTile, 1);
     cudaError_t e = c->scan_state.ensure((size_t)n_tiles * sizeof(ScanTile) + 64);
     if (e != cudaSuccess) return e;
-    // [0, 64): ticket; then the tile states.  d_tot is rewritten in full by the kernels below.
+    // [0, 64): ticket; then the tile states
     e = cudaMemsetAsync(c->scan_state.p, 0, (size_t)n_tiles * sizeof(ScanTile) + 64, st);
     if (e != cudaSuccess) return e;
-    k_fin_scan<<<(int)n_tiles, kFinThreads, 0, st>>>(R, c->n_steps, c->st_count.p, c->st_width.p, c->st_real.p,
-                                                    c->st_round.p, c->st_origin.p, c->grp_count.p, c->grp_width.p,
-                                                    c->grp_round.p, c->grp_real.p, c->grp_origin.p, c->grp_offset.p, c->grp_sample_ptr.p,
-                                                    reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
-                                                    reinterpret_cast<unsigned int *>(c->scan_state.p), c->d_tot);
-    ODB_LAUNCH_CHECK(c);
-    return cudaSuccess;
-}
-
-// the slot CSR's ids and the leftover CSR: only the caller's tables need them, so this runs beside the
-// collate preparation (odb_api.cu: launch_prep), not in front of the plan-size read-back
-cudaError_t launch_ids_left(odb_ctx *c, cudaStream_t st) {
-    const int R = c->prm.n_ranks;
-    k_ids_left<<<R, kRankThreads, 0, st>>>(R, c->n_steps, c->d_rank_ptr, c->emit_cur, c->emit_ids, c->emit_pos,
-                                           c->grp_sample_ptr.p, c->grp_sample_ids.p, c->left_ptr.p, c->left_out.p, c->d_tot);
-    ODB_LAUNCH_CHECK(c);
-    return cudaSuccess;
-}
-
-cudaError_t launch_chunk_table(odb_ctx *c, cudaStream_t st) {
-    const int64_t n_slots = (int64_t)c->prm.n_ranks * c->n_steps;
-    if (n_slots == 0) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>((n_slots * 32 + 255) / 256, (int64_t)c->sm_count * 64);
-    k_chunk_table<<<blocks, 256, 0, st>>>(n_slots, c->grp_offset.p, c->grp_count.p, c->grp_width.p, c->grp_sample_ptr.p,
-                                          c->chunks.p);
+    const int blocks = (int)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * 2);
+    k_fin_scan<<<blocks, kFinThreads, 0, st>>>(R, c->d_dims, c->st_count.p, c->st_width.p, c->st_real.p, c->st_round.p,
+                                               c->st_origin.p, c->grp_count.p, c->grp_width.p, c->grp_round.p,
+                                               c->grp_real.p, c->grp_origin.p, c->grp_offset.p, c->grp_sample_ptr.p,
+                                               reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
+                                               reinterpret_cast<unsigned int *>(c->scan_state.p), cap, c->n_total,
+                                               rank_off);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
