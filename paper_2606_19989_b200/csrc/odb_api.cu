@@ -239,6 +239,7 @@ int odb_reset(odb_ctx *c) {
     c->info_valid = false;
     c->collated = false;
     c->arrived_set = false;
+    c->begin_pending = false;
     c->d_lengths = nullptr;
     return ODB_OK;
 }
@@ -303,7 +304,9 @@ static int begin_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank
     CU(c, cudaMemcpyAsync(c->d_rank_ptr, c->h_rank_ptr.data(), (R + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
     if (!c->arrived_set) c->h_arrived.assign((size_t)R, 0x7fffffff);  // everything has arrived
     CU(c, cudaMemcpyAsync(c->d_arrived, c->h_arrived.data(), (size_t)R * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-    CU(c, launch_begin(c, st));  // rank state, emit positions, step totals, length validation
+    // rank state, emit positions, step totals, length validation: done by the first sort launch (or k_begin)
+    CU(c, cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st));
+    c->begin_pending = true;
     c->n_finished = 0;
     for (int r = 0; r < R; ++r)
         if (h_rank_ptr[r + 1] == h_rank_ptr[r]) c->n_finished++;
@@ -338,6 +341,7 @@ int odb_form_groups(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_
     // distributed mode: termination is decided on the device from the gathered world summary (k_align)
     if (!c->world_ranks && check_terminated(c)) {
         // the terminal check round: nothing to form; odb_align / odb_round_status report done
+        CU(c, flush_begin(c, st));
         c->state = 1;
         c->last_T = 0;
         return ODB_OK;
@@ -629,11 +633,7 @@ static int collate_launch(odb_ctx *c, const int32_t *d_tokens, const int32_t *d_
         A.elem_lo = 0;
         A.tile_lo = 0;
         A.tile_hi = tile_bound;
-        A.done_counter = c->d_done_ctr + 1;
-        A.R = c->prm.n_ranks;
-        A.step_valid = c->step_valid.p;
-        A.user_step_valid = o->d_step_valid_tokens;
-        A.user_grp_valid = o->d_grp_valid_tokens;
+        A.whole = 1;
     } else {
         A.total_elems = elem_hi;
         A.elem_lo = elem_lo;
@@ -668,10 +668,19 @@ static int enqueue_collate(odb_ctx *c, const int32_t *d_tokens, const int64_t *d
         int rc = collate_launch(c, d_tokens, d_span_lo, d_span_hi, o, true, 0, 0, tile_bound, c->d_tile_counter, st);
         if (rc != ODB_OK) return rc;
     }
-    if (c->timing) {
-        CU(c, cudaEventRecord(c->ev[2], st));
-        CU(c, cudaEventRecord(c->ev[3], st));
+    if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));
+    {  // step totals (Eq. 2's T_tok per step) + the caller's valid-token tables
+        PostArgs P;
+        memset(&P, 0, sizeof(P));
+        P.R = c->prm.n_ranks;
+        P.dims = c->d_dims;
+        P.grp_valid = c->grp_valid.p;
+        P.step_valid = c->step_valid.p;
+        P.user_step_valid = o->d_step_valid_tokens;
+        P.user_grp_valid = o->d_grp_valid_tokens;
+        CU(c, launch_post(c, P, st));
     }
+    if (c->timing) CU(c, cudaEventRecord(c->ev[3], st));
     return ODB_OK;
 }
 

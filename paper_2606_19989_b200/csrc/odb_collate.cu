@@ -374,7 +374,7 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
     // a whole-arena launch reads its extent on the device (it may have been enqueued before the host saw
     // the plan) and does nothing when the plan is not complete or the caller's buffers are too small
     int64_t total_elems = A.total_elems, tile_hi = A.tile_hi;
-    if (A.done_counter) {
+    if (A.whole) {
         if (!A.dims->complete || A.dims->err) return;
         total_elems = A.dims->total_elems;
         tile_hi = (total_elems + kColTile - 1) / kColTile;
@@ -573,50 +573,27 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
             }
         }
     }
-    // Whole-arena launches: the last CTA to finish sums the valid tokens per step over the ranks (Eq. 2's
-    // T_tok per step) and hands the per-slot counts to the caller -- what used to be a separate launch.
-    if (A.done_counter) {
-        __shared__ int s_last;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            __threadfence();
-            s_last = (atomicAdd(A.done_counter, 1u) == gridDim.x - 1u) ? 1 : 0;
-        }
-        __syncthreads();
-        if (s_last) {
-            __threadfence();
-            const int n_steps = A.dims->n_steps;
-            const int64_t n_slots = A.dims->n_slots;
-            for (int k = threadIdx.x; k < n_steps; k += blockDim.x) {
-                long long t = 0;
-                for (int r = 0; r < A.R; ++r) t += __ldcg(A.grp_valid + (int64_t)r * n_steps + k);
-                A.step_valid[k] = t;
-                if (A.user_step_valid) A.user_step_valid[k] = t;
-            }
-            if (A.user_grp_valid)
-                for (int64_t q = threadIdx.x; q < n_slots; q += blockDim.x) A.user_grp_valid[q] = __ldcg(A.grp_valid + q);
-            if (threadIdx.x == 0) *A.done_counter = 0u;
-        }
-    }
 }
 
 // After the collate kernel, one launch: step_valid_tokens[k] = sum over ranks of grp_valid_tokens[r][k]
-// (Eq. 2's T_tok per step), written to the library's table and the caller's, and the copies of the
-// plan tables into the caller's buffers (4-byte words).
+// (Eq. 2's T_tok per step), written to the library's table and the caller's, and the per-slot counts into
+// the caller's table.  Sizes from PlanDims; skipped when the plan is not complete / the capacities too small.
+// (Fusing this into the collate kernel's last CTA was tried: one CTA walking R x n_steps counts costs
+// 40-200 us on the configs[4] cells against 12 us for this launch.)
 __global__ void k_post(const PostArgs A) {
+    if (!A.dims->complete || A.dims->err) return;
     const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (int64_t)gridDim.x * blockDim.x;
     const int n_steps = A.dims->n_steps;
+    const int64_t n_slots = (int64_t)A.R * n_steps;
     for (int64_t k = tid; k < n_steps; k += nth) {
         long long s = 0;
+#pragma unroll 4
         for (int r = 0; r < A.R; ++r) s += A.grp_valid[(int64_t)r * n_steps + k];
         A.step_valid[k] = s;
         if (A.user_step_valid) A.user_step_valid[k] = s;
     }
-    for (int j = 0; j < A.n_jobs; ++j) {
-        const uint32_t *__restrict__ src = reinterpret_cast<const uint32_t *>(A.job[j].src);
-        uint32_t *__restrict__ dst = reinterpret_cast<uint32_t *>(A.job[j].dst);
-        for (int64_t i = tid; i < A.job[j].words; i += nth) dst[i] = src[i];
-    }
+    if (A.user_grp_valid)
+        for (int64_t i = tid; i < n_slots; i += nth) A.user_grp_valid[i] = A.grp_valid[i];
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -694,7 +671,7 @@ cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st)
     }
     // tiles the launch can have to visit: known for a ranged launch, bounded by the caller's arena otherwise
     const int64_t n_tiles = args.tile_hi - args.tile_lo;
-    if (n_tiles <= 0 && !args.done_counter) return cudaSuccess;
+    if (n_tiles <= 0 && !args.whole) return cudaSuccess;
     int blocks = (int)std::min<int64_t>(std::max<int64_t>((n_tiles + kColGrab - 1) / kColGrab, 1),
                                         (int64_t)c->sm_count * c->col_occ[sh]);
     if (sh) k_collate<true><<<blocks, kColThreads, 0, st>>>(args);
@@ -704,9 +681,8 @@ cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st)
 }
 
 cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st) {
-    int64_t work = c->n_steps;
-    for (int j = 0; j < args.n_jobs; ++j) work = std::max(work, args.job[j].words);
-    if (work == 0) return cudaSuccess;
+    // the grid is sized by what the tables can hold (the host may not have seen the plan yet)
+    const int64_t work = std::max<int64_t>((int64_t)c->grp_valid.cap, 1);
     int blocks = (int)std::min<int64_t>((work + 255) / 256, (int64_t)c->sm_count * 8);
     k_post<<<blocks, 256, 0, st>>>(args);
     ODB_LAUNCH_CHECK(c);

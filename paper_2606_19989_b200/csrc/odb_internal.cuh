@@ -120,29 +120,17 @@ struct CollateArgs {
     int64_t elem_lo;
     int64_t tile_lo, tile_hi;  // tiles [tile_lo, tile_hi) are visited by this launch
     int32_t pad_id, ignore_index, shift_labels;
-    // fused epilogue (whole-arena launches): the last CTA to finish sums the valid tokens per step
-    // (Eq. 2's T_tok) and copies grp_valid into the caller's table
-    unsigned int *done_counter;
-    int32_t R;
-    int64_t *step_valid;
-    int64_t *user_step_valid;
-    int32_t *user_grp_valid;
+    int32_t whole;  // 1: the launch covers the whole arena, extent read from dims (skipped if the plan is not usable)
 };
 
-// k_post: table copies (4-byte words) + the per-step valid-token totals
-struct CopyJob {
-    void *dst;
-    const void *src;
-    int64_t words;
-};
+// k_post: the per-step valid-token totals and the caller's valid-token tables
 struct PostArgs {
-    CopyJob job[16];
-    int n_jobs;
     int R;
     const PlanDims *dims;
     const int32_t *grp_valid;
     int64_t *step_valid;
     int64_t *user_step_valid;
+    int32_t *user_grp_valid;
 };
 
 // growable device buffer (cudaMalloc on growth only)
@@ -195,7 +183,9 @@ struct odb_ctx {
     cudaEvent_t ev_status = nullptr;
     cudaStream_t last_stream = nullptr;
     int col_occ[2] = {0, 0};  // resident collate CTAs per SM (shift 0 / 1)
-    bool attr_form = false, attr_align = false;  // cudaFuncSetAttribute done on this device
+    bool attr_form = false, attr_form_hier = false, attr_align = false, attr_sort = false;  // cudaFuncSetAttribute done
+    bool no_cluster_sort = false;  // the cluster sort could not be launched on this device: use the fallback
+    bool begin_pending = false;    // a run has started and its per-run device state is not cleared yet
 
     // inputs fixed by the first odb_form_groups after create / reset
     const int32_t *d_lengths = nullptr;
@@ -245,7 +235,7 @@ struct odb_ctx {
     odb::PlanDims *d_dims = nullptr;
     odb::PlanDims *h_dims = nullptr;     // pinned: the device's sizes, copied back behind the slot scan
     odb::PlanDims *h_dims_up = nullptr;  // pinned: the host's sizes on their way up (staged path)
-    unsigned int *d_done_ctr = nullptr;  // 2: "last CTA" counters of k_commit / k_collate (self-resetting)
+    unsigned int *d_done_ctr = nullptr;  // "last CTA" counter of k_commit (self-resetting)
     cudaEvent_t ev_plan = nullptr;       // recorded behind the slot scan's read-back
     unsigned long long *d_tile_counter = nullptr;
 
@@ -280,7 +270,10 @@ struct odb_ctx {
 namespace odb {
 // ---- launchers implemented in odb_plan.cu ----------------------------------------------------
 cudaError_t launch_begin(odb_ctx *c, cudaStream_t st);  // per-run state reset + length validation
+cudaError_t flush_begin(odb_ctx *c, cudaStream_t st);   // ... if no sort launch has done it
 cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st);   // A0..A3
+// A0 + A1 in one launch (odb_sort.cu): cluster merge sort; cudaErrorNotSupported for windows > 65536 keys
+cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st);
 cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commit (single-process mode)
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: (G_r, S_r) pairs for the all_gather
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary

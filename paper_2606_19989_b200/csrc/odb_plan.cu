@@ -402,6 +402,133 @@ k_form_groups_smem(const uint64_t *__restrict__ keys, const int64_t *__restrict_
     }
 }
 
+// Hierarchical version (windows of up to 32768 samples; the default): the successor is strictly increasing
+// (next[x] > x), so the orbit of 0 can be found with JUMP-OUT TABLES instead of pointer doubling over the
+// whole window.  Positions are cut into blocks of 32 and superblocks of 1024:
+//   out1[x] = the first element of x's chain that leaves x's block      (backward DP inside each block:
+//             one thread per block, 32 dependent steps);
+//   out2[x] = the first element of x's chain that leaves x's superblock (one warp per superblock walks its
+//             32 blocks from the last to the first, a lane per position: out2[x] = out1[x] if that is
+//             outside, else out2[out1[x]], already known);
+// then the orbit is expanded top-down: thread 0 chases out2 from 0 (at most 32 steps) and records where
+// the orbit enters each superblock; a thread per superblock chases out1 from there and records where it
+// enters each block; a thread per block chases next and builds the block's 32-bit mark word in a register.
+// About 5 x 32 dependent shared-memory steps in all, and O(S) work per phase whatever the group sizes --
+// against ceil(log2 G) + 1 passes over the whole window for pointer doubling (51 us -> see profiles/).
+// Arrays are uint16 (S <= 32768) with one spare entry per 32, so a thread per block walks without bank conflicts.
+__device__ __forceinline__ int fg_pad(int i) { return i + (i >> 5); }
+
+__global__ void __launch_bounds__(kRankThreads)
+k_form_groups_hier(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr,
+                   const int32_t *__restrict__ S_arr, uint32_t budget, int rule, int32_t *__restrict__ gpos,
+                   int32_t *__restrict__ G_out) {
+    extern __shared__ __align__(16) unsigned char fh_smem[];
+    __shared__ int s_scan[34];
+    __shared__ uint16_t s_e2[32];
+    const int r = blockIdx.x;
+    const int S = S_arr[r];
+    if (S == 0) {
+        if (threadIdx.x == 0) G_out[r] = 0;
+        return;
+    }
+    const int64_t base = rank_ptr[r];
+    const uint64_t *k = keys + base;
+    const int np = fg_pad(S) + 2;            // entries per array (even, so the arrays stay 4-byte aligned)
+    const int npe = (np + 1) & ~1;
+    const int nb1 = (S + 31) >> 5, nb2 = (S + 1023) >> 10;
+    uint16_t *nxt = reinterpret_cast<uint16_t *>(fh_smem);
+    uint16_t *out1 = nxt + npe;
+    uint16_t *out2 = out1 + npe;
+    uint16_t *e1 = out2 + npe;                                  // nb1 entries (padded to even)
+    uint32_t *mk = reinterpret_cast<uint32_t *>(e1 + ((nb1 + 1) & ~1));  // nb1 words
+    constexpr uint16_t kNone = 0xFFFFu;
+    for (int x = threadIdx.x; x < S; x += blockDim.x) nxt[fg_pad(x)] = (uint16_t)successor(k, x, S, budget, rule);
+    for (int b = threadIdx.x; b < nb1; b += blockDim.x) e1[b] = kNone;
+    if (threadIdx.x < 32) s_e2[threadIdx.x] = kNone;
+    __syncthreads();
+    // out1: one thread per block, from the block's last position down
+    for (int b = threadIdx.x; b < nb1; b += blockDim.x) {
+        const int lo = b << 5, end = min(S, lo + 32);
+        for (int i = end - 1; i >= lo; --i) {
+            const int j = nxt[fg_pad(i)];
+            out1[fg_pad(i)] = (uint16_t)(j >= end ? j : out1[fg_pad(j)]);
+        }
+    }
+    __syncthreads();
+    // out2: one warp per superblock, its blocks from the last to the first, a lane per position
+    {
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+        for (int sb = w; sb < nb2; sb += nw) {
+            const int slo = sb << 10, send = min(S, slo + 1024);
+            for (int blk = ((send - 1) >> 5); blk >= (slo >> 5); --blk) {
+                const int i = (blk << 5) + lane;
+                if (i < send) {
+                    const int j = out1[fg_pad(i)];
+                    out2[fg_pad(i)] = (uint16_t)(j >= send ? j : out2[fg_pad(j)]);
+                }
+                __syncwarp();
+            }
+        }
+    }
+    __syncthreads();
+    // top-down: where the orbit of 0 enters each superblock, each block, and its marks inside each block
+    if (threadIdx.x == 0) {
+        int x = 0;
+        while (x < S) {
+            s_e2[x >> 10] = (uint16_t)x;
+            x = out2[fg_pad(x)];
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < nb2 && s_e2[threadIdx.x] != kNone) {
+        const int send = min(S, ((int)threadIdx.x + 1) << 10);
+        int x = s_e2[threadIdx.x];
+        while (x < send) {
+            e1[x >> 5] = (uint16_t)x;
+            x = out1[fg_pad(x)];
+        }
+    }
+    __syncthreads();
+    int part = 0;
+    for (int b = threadIdx.x; b < nb1; b += blockDim.x) {
+        uint32_t word = 0u;
+        if (e1[b] != kNone) {
+            const int end = min(S, (b + 1) << 5);
+            int x = e1[b];
+            while (x < end) {
+                word |= 1u << (x & 31);
+                x = nxt[fg_pad(x)];
+            }
+        }
+        mk[b] = word;
+        part += __popc(word);
+    }
+    // marks live on chase coordinates x in [0, S); G = their number
+    int G;
+    (void)block_excl_scan<int>(part, s_scan, G);  // (its barriers also publish mk)
+    int32_t *gp = gpos + base + r;
+    int carry = 0;
+    for (int w0 = 0; w0 < nb1; w0 += blockDim.x) {
+        const int w = w0 + threadIdx.x;
+        uint32_t bits = w < nb1 ? mk[w] : 0u;
+        int tot;
+        int i = block_excl_scan<int>(__popc(bits), s_scan, tot) + carry;
+        while (bits) {
+            const int x = (w << 5) + __ffs(bits) - 1;
+            bits &= bits - 1;
+            if (rule == ODB_RULE_THRESHOLD) gp[G - i] = S - x;  // i-th mark (ascending x) -> start S - x
+            else gp[i] = x;
+            ++i;
+        }
+        carry += tot;
+    }
+    if (threadIdx.x == 0) {
+        if (rule == ODB_RULE_THRESHOLD) gp[0] = 0;
+        else gp[G] = S;
+        G_out[r] = G;
+    }
+}
+
 // Global-memory version for windows that do not fit the shared-memory one.
 __global__ void __launch_bounds__(kRankThreads)
 k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
@@ -966,9 +1093,7 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
     } while (0)
 
 cudaError_t launch_begin(odb_ctx *c, cudaStream_t st) {
-    const int R = c->prm.n_ranks;
-    cudaError_t e = cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st);
-    if (e != cudaSuccess) return e;
+    const int R = c->prm.n_ranks;  // (d_rec was zeroed when the run began)
     const int64_t step_cap = c->step_samples.p ? (int64_t)c->step_samples.cap : 0;
     const int64_t bound = std::max<int64_t>(std::max<int64_t>(c->n_total, R), step_cap);
     int blocks = (int)std::min<int64_t>((bound + 1023) / 1024, (int64_t)c->sm_count * 4);
@@ -984,38 +1109,76 @@ static int max_window_bound(const odb_ctx *c) {
     return (int)m;
 }
 
+static size_t form_hier_smem_bytes(int maxS) {
+    const size_t np = (size_t)maxS + ((size_t)maxS >> 5) + 2, npe = (np + 1) & ~(size_t)1;
+    const size_t nb1 = ((size_t)maxS + 31) >> 5;
+    return 3 * npe * 2 + ((nb1 + 1) & ~(size_t)1) * 2 + nb1 * 4 + 16;
+}
+
 static size_t form_smem_bytes(int maxS) {
     const size_t n1p = ((size_t)maxS + 1 + 7) & ~(size_t)7;
     const size_t words = ((size_t)maxS + 1 + 31) >> 5;
     return 4 * n1p + 4 * words;
 }
 
+// the per-run state reset, when no sort launch has done it (no window anywhere, or the fallback sort)
+cudaError_t flush_begin(odb_ctx *c, cudaStream_t st) {
+    if (!c->begin_pending) return cudaSuccess;
+    c->begin_pending = false;
+    return launch_begin(c, st);
+}
+
 cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const int maxS = max_window_bound(c);
-    if (maxS == 0) return cudaSuccess;
-    const int chunks = (maxS + kSortChunk - 1) / kSortChunk;
-    if (maxS > kSortChunk / 2)  // full-size chunks: the register-blocked network; small windows: the shared-memory one
-        k_chunk_sort_reg<<<dim3(chunks, R), kSortRegThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos,
-                                                                     c->left_ids, c->d_arrived, c->prm.buffer_size,
-                                                                     c->keyA, c->S, c->d_rec);
-    else
-        k_chunk_sort<<<dim3(chunks, R), kSortThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos,
-                                                              c->left_ids, c->d_arrived, c->prm.buffer_size, c->keyA, c->S,
-                                                              c->d_rec);
-    ODB_LAUNCH_CHECK(c);
-    uint64_t *src = c->keyA, *dst = c->keyB;
-    for (int64_t w = kSortChunk; w < maxS; w *= 2) {
-        int gx = (maxS + kMergeTile - 1) / kMergeTile;
-        k_merge_pass<<<dim3(gx, R), kMergeThreads, 0, st>>>(src, dst, c->d_rank_ptr, c->S, (int)w);
-        ODB_LAUNCH_CHECK(c);
-        uint64_t *t = src;
-        src = dst;
-        dst = t;
+    if (maxS == 0) return flush_begin(c, st);
+    // A0 + A1: one cluster launch (windows of up to 65536 keys); it also clears the per-run state in the
+    // first round.  Larger windows: chunk sorts + merge passes through global memory.
+    cudaError_t se = cudaErrorNotSupported;
+    if (!c->no_cluster_sort) {
+        se = launch_sort_window(c, maxS, c->begin_pending, st);
+        if (se == cudaSuccess) c->begin_pending = false;
+        else if (se != cudaErrorNotSupported) {  // e.g. a 16-CTA cluster the device will not schedule: fall back for good
+            (void)cudaGetLastError();
+            c->no_cluster_sort = true;
+        }
     }
-    c->sorted = src;
+    if (se != cudaSuccess) {
+        cudaError_t e = flush_begin(c, st);
+        if (e != cudaSuccess) return e;
+        const int chunks = (maxS + kSortChunk - 1) / kSortChunk;
+        if (maxS > kSortChunk / 2)  // full-size chunks: the register-blocked network; small windows: the shared-memory one
+            k_chunk_sort_reg<<<dim3(chunks, R), kSortRegThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos,
+                                                                         c->left_ids, c->d_arrived, c->prm.buffer_size,
+                                                                         c->keyA, c->S, c->d_rec);
+        else
+            k_chunk_sort<<<dim3(chunks, R), kSortThreads, 0, st>>>(c->d_lengths, c->d_rank_ptr, c->n_left, c->fetch_pos,
+                                                                  c->left_ids, c->d_arrived, c->prm.buffer_size, c->keyA, c->S,
+                                                                  c->d_rec);
+        ODB_LAUNCH_CHECK(c);
+        uint64_t *src = c->keyA, *dst = c->keyB;
+        for (int64_t w = kSortChunk; w < maxS; w *= 2) {
+            int gx = (maxS + kMergeTile - 1) / kMergeTile;
+            k_merge_pass<<<dim3(gx, R), kMergeThreads, 0, st>>>(src, dst, c->d_rank_ptr, c->S, (int)w);
+            ODB_LAUNCH_CHECK(c);
+            uint64_t *t = src;
+            src = dst;
+            dst = t;
+        }
+        c->sorted = src;
+    }
+    // A2 + A3
     const size_t smem = form_smem_bytes(maxS);
-    if (smem <= kFormSmemLimit && maxS <= 65534) {
+    if (maxS <= 32768) {
+        if (!c->attr_form_hier) {
+            cudaError_t e = cudaFuncSetAttribute(k_form_groups_hier, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)kFormSmemLimit);
+            if (e != cudaSuccess) return e;
+            c->attr_form_hier = true;
+        }
+        k_form_groups_hier<<<R, kRankThreads, form_hier_smem_bytes(maxS), st>>>(c->sorted, c->d_rank_ptr, c->S,
+                                                                               (uint32_t)c->prm.budget, c->prm.rule, c->gpos, c->G);
+    } else if (smem <= kFormSmemLimit && maxS <= 65534) {
         if (!c->attr_form) {
             cudaError_t e = cudaFuncSetAttribute(k_form_groups_smem, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                  (int)kFormSmemLimit);

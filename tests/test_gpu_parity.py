@@ -206,6 +206,18 @@ def test_large_window_global_memory_planner(P, oracle, rule):
     assert plan.n_steps > 1000 and wl.n_samples == 210_000
 
 
+@pytest.mark.parametrize("n", [4096, 4097, 9000, 20_000, 32_768, 33_000, 50_000, 65_536])
+@pytest.mark.parametrize("rule", [0, 1])
+def test_cluster_sort_window_sizes(P, oracle, n, rule):
+    """Windows that need a thread-block cluster of 1, 2, 4, 8 and 16 CTAs for the segmented sort (ragged last
+    chunks, a rank with a much smaller window beside them), and both list-ranking kernels behind it."""
+    rng = np.random.default_rng(n + rule)
+    per = [rng.integers(1, 3000, n), rng.integers(1, 3000, max(1, n // 3)), rng.integers(1, 40, n - 5)]
+    wl = I.custom_workload("cluster_sort", per, 31, budget=8192, rule=rule)
+    plan = _sampled_parity(oracle, wl, n_sample=16)
+    assert plan.samples_emitted == wl.n_samples
+
+
 def test_heavy_split_unequal_group_counts(P, oracle):
     """One rank forms thousands of groups, another a handful of big ones: the split closed form turns
     thousands of rows of a few groups into singletons (Alg. 1)."""
