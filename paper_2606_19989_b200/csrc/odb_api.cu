@@ -82,6 +82,7 @@ static void free_all(odb_ctx *c) {
     cudaFree(c->d_tile_counter);
     cudaFree(c->gs_local);
     cudaFree(c->gs_world);
+    cudaFree(c->gs_rounds);
     if (c->h_rec) cudaFreeHost(c->h_rec);
     if (c->h_dims) cudaFreeHost(c->h_dims);
     if (c->h_dims_up) cudaFreeHost(c->h_dims_up);
@@ -734,6 +735,34 @@ static int run_rounds(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_ran
     return odb_plan_query(c, h_out);
 }
 
+// Everything behind the round loop, enqueued BEFORE the host knows the plan: the slot scan (which checks the
+// caller's capacities on the device), the read-back of the plan sizes with an event behind it, the collate
+// preparation, the collate kernel and the step totals.  Every kernel reads PlanDims and does nothing unless
+// the plan is complete and fits.  steps_bound >= the number of steps the plan can have.
+static int enqueue_tail(odb_ctx *c, int64_t steps_bound, const int32_t *d_tokens, const int64_t *d_sample_ptr,
+                        const int64_t *d_span_ptr, const int32_t *d_span_lo, const int32_t *d_span_hi,
+                        const odb_outputs *o, cudaStream_t st) {
+    const int R = c->prm.n_ranks;
+    const int64_t slots_bound = (int64_t)R * steps_bound;
+    int rc = ensure_plan_tables(c, (size_t)slots_bound, (size_t)steps_bound);
+    if (rc != ODB_OK) return rc;
+    const int64_t tile_bound = (std::max<int64_t>(o->arena_capacity, 0) + kColTile - 1) / kColTile;
+    CU(c, c->tiles.ensure((size_t)tile_bound + 2));
+    const bool any_slot_tab = o->d_grp_count || o->d_grp_width || o->d_grp_round || o->d_grp_valid_tokens ||
+                              o->d_grp_real_tokens || o->d_grp_origin || o->d_grp_offset || o->d_grp_sample_ptr;
+    CapCheck cap;
+    cap.arena = std::max<int64_t>(o->arena_capacity, 0);
+    cap.slots = any_slot_tab ? o->slot_capacity_alloc : -1;
+    cap.ids = o->d_grp_sample_ids ? o->ids_capacity : -1;
+    cap.steps = (o->d_step_samples || o->d_step_valid_tokens) ? o->step_capacity_alloc : -1;
+    cap.left = o->d_left_ids ? o->left_capacity : -1;
+    cap.tiles = tile_bound;
+    CU(c, launch_finalize(c, slots_bound, cap, c->h_rank_off, st));
+    CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
+    CU(c, cudaEventRecord(c->ev_plan, st));
+    return enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, c->n_total, tile_bound, st);
+}
+
 int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
             const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo, const int32_t *d_span_hi,
             const odb_outputs *o, odb_plan_info *h_out, void *stream) {
@@ -741,19 +770,24 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
     if (c->world_ranks) return ODB_ERR_STATE;  // the caller drives the rounds and their collectives
     cudaStream_t st = (cudaStream_t)stream;
     const int R = c->prm.n_ranks;
-    // When every rank's whole stream fits its window and the output slots are unlimited, the protocol
-    // normally ends with the first round (equal group-count targets are reached by splitting; only unequal
-    // windows overflow).  Then NOTHING needs the host between the first kernel and the last: the round is
-    // closed on the device (k_commit), and the slot scan, the collate preparation and the collate kernel are
-    // enqueued behind it; they read the plan sizes from PlanDims and check the caller's capacities on the
-    // device.  The host waits only for the sizes (an event behind the slot scan), while the collate kernel
-    // is already running.  If the device says another round is due, those launches were no-ops and the
-    // staged loop below takes over.
+    // NOTHING needs the host between the first kernel and the last when
+    //  (A) the windows are small (<= 4096 samples: the paper's regime) and the R ranks fit the device:
+    //      ONE persistent kernel runs every protocol round (k_rounds), or
+    //  (B) every rank's whole stream fits its window and the output slots are unlimited: the protocol
+    //      normally ends with the first round (unequal group counts are levelled by splitting; only unequal
+    //      windows overflow), and k_commit closes the round on the device.
+    // The slot scan, the collate preparation and the collate kernel are enqueued behind the rounds; they read
+    // the plan sizes from PlanDims and check the caller's capacities on the device.  The host waits only for
+    // the sizes (an event behind the slot scan) while the collate kernel is already running.  If (B)'s first
+    // round does not end the protocol, those launches were no-ops and the staged loop below takes over.
     int64_t max_nr = 0;
     for (int r = 0; r < R; ++r) max_nr = std::max(max_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
+    const int64_t window = c->prm.buffer_size > 0 ? std::min<int64_t>(max_nr, c->prm.buffer_size) : max_nr;
     const bool arenas = o->d_input_ids && o->d_labels && o->d_position_ids && o->d_attention_mask;
-    const bool speculate = (c->prm.buffer_size == 0 || c->prm.buffer_size >= max_nr) && c->prm.slot_capacity == 0 &&
-                           arenas && d_tokens && d_sample_ptr && check_pointers(d_tokens, o) == ODB_OK;
+    const bool async_ok = arenas && d_tokens && d_sample_ptr && check_pointers(d_tokens, o) == ODB_OK && max_nr > 0;
+    const bool fused = async_ok && window <= kSortChunk && !c->no_rounds_kernel &&
+                       (int64_t)R * (max_nr + window + 64) <= (1ll << 27);
+    const bool speculate = async_ok && !fused && window >= max_nr && c->prm.slot_capacity == 0;
     odb_reset(c);
     CU(c, cudaSetDevice(c->device));
     if (c->timing) {
@@ -761,31 +795,61 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
         CU(c, cudaEventRecord(c->ev[0], st));
     }
     int32_t done = 0, T = 0;
-    int rc = odb_form_groups(c, d_lengths, h_rank_ptr, st);
+    int rc;
+    if (fused) {
+        c->last_stream = st;
+        rc = begin_run(c, d_lengths, h_rank_ptr, st);
+        if (rc != ODB_OK) return rc;
+        // room for every step the run can have: n_steps <= the longest stream (a rank that is active in every
+        // emitting round emits at least T samples per round), plus one round's window
+        const int64_t steps_bound = max_nr + window + 64;
+        if (steps_bound > c->step_cap) {
+            CU(c, grow_preserve(c->st_count, (size_t)steps_bound * R, 0, st));
+            CU(c, grow_preserve(c->st_width, (size_t)steps_bound * R, 0, st));
+            CU(c, grow_preserve(c->st_real, (size_t)steps_bound * R, 0, st));
+            CU(c, grow_preserve(c->st_round, (size_t)steps_bound * R, 0, st));
+            CU(c, grow_preserve(c->st_origin, (size_t)steps_bound * R, 0, st));
+            CU(c, grow_preserve(c->step_samples, (size_t)steps_bound, 0, st));
+            c->step_cap = steps_bound;
+        }
+        cudaError_t le = launch_rounds(c, st);
+        if (le == cudaSuccess) {
+            c->begin_pending = false;
+            rc = enqueue_tail(c, steps_bound, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
+            if (rc != ODB_OK) return rc;
+            CU(c, cudaEventSynchronize(c->ev_plan));  // the sizes are here; the collate kernel is running
+            const PlanDims &D = *c->h_dims;
+            if (D.bad_length) {
+                c->state = 0;
+                return ODB_ERR_BAD_LENGTH;
+            }
+            if (!D.complete) return D.err ? D.err : ODB_ERR_STATE;
+            c->n_steps = D.n_steps;
+            c->n_rounds = D.n_rounds;
+            c->round = D.n_rounds;
+            c->stop_reason = D.stop_reason;
+            c->samples_emitted = D.samples_emitted;
+            fill_info(c);
+            c->state = 5;
+            *h_out = c->info;
+            if (D.err) return D.err;  // ODB_ERR_CAPACITY: the kernels behind the slot scan wrote nothing
+            if (c->timing) timing_done(c);
+            c->collated = true;
+            return ODB_OK;
+        }
+        // the cooperative launch is not possible here (too many ranks for the device): drive the rounds from the host
+        (void)cudaGetLastError();
+        if (le != cudaErrorNotSupported) c->no_rounds_kernel = true;
+        odb_reset(c);
+    }
+    rc = odb_form_groups(c, d_lengths, h_rank_ptr, st);
     if (rc != ODB_OK) return rc;
     bool collate_enqueued = false;
     if (speculate && c->last_T != 0) {  // an emitting round was formed
         rc = odb_align(c, st);
         if (rc != ODB_OK) return rc;
-        const int64_t steps_bound = c->round_window;  // T_grp <= the largest window
-        const int64_t slots_bound = (int64_t)R * steps_bound;
-        rc = ensure_plan_tables(c, (size_t)slots_bound, (size_t)steps_bound);
-        if (rc != ODB_OK) return rc;
-        const int64_t tile_bound = (std::max<int64_t>(o->arena_capacity, 0) + kColTile - 1) / kColTile;
-        CU(c, c->tiles.ensure((size_t)tile_bound + 2));
-        const bool any_slot_tab = o->d_grp_count || o->d_grp_width || o->d_grp_round || o->d_grp_valid_tokens ||
-                                  o->d_grp_real_tokens || o->d_grp_origin || o->d_grp_offset || o->d_grp_sample_ptr;
-        CapCheck cap;
-        cap.arena = std::max<int64_t>(o->arena_capacity, 0);
-        cap.slots = any_slot_tab ? o->slot_capacity_alloc : -1;
-        cap.ids = o->d_grp_sample_ids ? o->ids_capacity : -1;
-        cap.steps = (o->d_step_samples || o->d_step_valid_tokens) ? o->step_capacity_alloc : -1;
-        cap.left = o->d_left_ids ? o->left_capacity : -1;
-        cap.tiles = tile_bound;
-        CU(c, launch_finalize(c, slots_bound, cap, c->h_rank_off, st));
-        CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
-        CU(c, cudaEventRecord(c->ev_plan, st));
-        rc = enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, c->n_total, tile_bound, st);
+        rc = enqueue_tail(c, c->round_window /* T_grp <= the largest window */, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo,
+                          d_span_hi, o, st);
         if (rc != ODB_OK) return rc;
         CU(c, cudaEventSynchronize(c->ev_plan));  // the sizes are here; the collate kernel is running
         collate_enqueued = c->h_dims->complete != 0;

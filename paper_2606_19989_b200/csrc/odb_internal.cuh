@@ -186,6 +186,9 @@ struct odb_ctx {
     bool attr_form = false, attr_form_hier = false, attr_align = false, attr_sort = false;  // cudaFuncSetAttribute done
     bool no_cluster_sort = false;  // the cluster sort could not be launched on this device: use the fallback
     bool begin_pending = false;    // a run has started and its per-run device state is not cleared yet
+    bool no_rounds_kernel = false; // the persistent round-loop kernel could not be launched on this device
+    int rounds_max_ctas = 0;       // resident CTAs of k_rounds on this device (0 = not asked yet, -1 = no cooperative launch)
+    int32_t *gs_rounds = nullptr;  // k_rounds: the double-buffered per-round summary + the grid-barrier counter
 
     // inputs fixed by the first odb_form_groups after create / reset
     const int32_t *d_lengths = nullptr;
@@ -275,6 +278,8 @@ cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st);   // A0..A3
 // A0 + A1 in one launch (odb_sort.cu): cluster merge sort; cudaErrorNotSupported for windows > 65536 keys
 cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st);
 cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commit (single-process mode)
+// every protocol round in one cooperative launch; cudaErrorNotSupported if R CTAs cannot be resident
+cudaError_t launch_rounds(odb_ctx *c, cudaStream_t st);
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: (G_r, S_r) pairs for the all_gather
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce

@@ -4,8 +4,11 @@
 //
 // Paper: /root/reference/PAPER.md (P:<line>).  Section 2.2 P:32-36 and Eq. 1 (grouping), Eq. 3
 // (target), Alg. 1 P:258-279 (split / overflow), P:28 (IDLE slots), Thm 2 P:48 + P:347 (quota).
+#include <cstring>
+
 #include "odb_internal.cuh"
 #include "odb_device.cuh"
+#include "odb_sort.cuh"
 
 namespace odb {
 
@@ -303,7 +306,7 @@ k_merge_pass(const uint64_t *__restrict__ src, uint64_t *__restrict__ dst, const
 // ceil(log2 G) + 1 rounds exactly the orbit of 0 is marked.  Output: ascending start positions
 // gpos[0..G] (gpos[G] = S) and G_r.  A THRESHOLD mark at chase x > 0 is the ascending start S - x.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int successor(const uint64_t *__restrict__ k, int x, int S, uint32_t budget, int rule) {
+__device__ __forceinline__ int successor(const uint64_t *k, int x, int S, uint32_t budget, int rule) {
     if (x == S) return S;
     if (rule == ODB_RULE_THRESHOLD) {
         if (x == 0) return 1;
@@ -418,21 +421,10 @@ k_form_groups_smem(const uint64_t *__restrict__ keys, const int64_t *__restrict_
 // Arrays are uint16 (S <= 32768) with one spare entry per 32, so a thread per block walks without bank conflicts.
 __device__ __forceinline__ int fg_pad(int i) { return i + (i >> 5); }
 
-__global__ void __launch_bounds__(kRankThreads)
-k_form_groups_hier(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr,
-                   const int32_t *__restrict__ S_arr, uint32_t budget, int rule, int32_t *__restrict__ gpos,
-                   int32_t *__restrict__ G_out) {
-    extern __shared__ __align__(16) unsigned char fh_smem[];
-    __shared__ int s_scan[34];
-    __shared__ uint16_t s_e2[32];
-    const int r = blockIdx.x;
-    const int S = S_arr[r];
-    if (S == 0) {
-        if (threadIdx.x == 0) G_out[r] = 0;
-        return;
-    }
-    const int64_t base = rank_ptr[r];
-    const uint64_t *k = keys + base;
+// (a device function: the persistent round-loop kernel calls it too, on keys it has just written itself)
+__device__ __forceinline__ int
+form_hier_body(const uint64_t *k, int S, uint32_t budget, int rule, int32_t *gp, unsigned char *fh_smem, int *s_scan,
+               uint16_t *s_e2) {
     const int np = fg_pad(S) + 2;            // entries per array (even, so the arrays stay 4-byte aligned)
     const int npe = (np + 1) & ~1;
     const int nb1 = (S + 31) >> 5, nb2 = (S + 1023) >> 10;
@@ -506,7 +498,6 @@ k_form_groups_hier(const uint64_t *__restrict__ keys, const int64_t *__restrict_
     // marks live on chase coordinates x in [0, S); G = their number
     int G;
     (void)block_excl_scan<int>(part, s_scan, G);  // (its barriers also publish mk)
-    int32_t *gp = gpos + base + r;
     int carry = 0;
     for (int w0 = 0; w0 < nb1; w0 += blockDim.x) {
         const int w = w0 + threadIdx.x;
@@ -525,8 +516,26 @@ k_form_groups_hier(const uint64_t *__restrict__ keys, const int64_t *__restrict_
     if (threadIdx.x == 0) {
         if (rule == ODB_RULE_THRESHOLD) gp[0] = 0;
         else gp[G] = S;
-        G_out[r] = G;
     }
+    return G;
+}
+
+__global__ void __launch_bounds__(kRankThreads)
+k_form_groups_hier(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr,
+                   const int32_t *__restrict__ S_arr, uint32_t budget, int rule, int32_t *__restrict__ gpos,
+                   int32_t *__restrict__ G_out) {
+    extern __shared__ __align__(16) unsigned char fh_smem[];
+    __shared__ int s_scan[34];
+    __shared__ uint16_t s_e2[32];
+    const int r = blockIdx.x;
+    const int S = S_arr[r];
+    if (S == 0) {
+        if (threadIdx.x == 0) G_out[r] = 0;
+        return;
+    }
+    const int64_t base = rank_ptr[r];
+    const int G = form_hier_body(keys + base, S, budget, rule, gpos + base + r, fh_smem, s_scan, s_e2);
+    if (threadIdx.x == 0) G_out[r] = G;
 }
 
 // Global-memory version for windows that do not fit the shared-memory one.
@@ -588,6 +597,77 @@ k_form_groups(const uint64_t *__restrict__ keys, const int64_t *__restrict__ ran
 //
 // Overflow: sort groups by (count desc, index asc), keep the first T (shared memory when G_r fits).
 // ---------------------------------------------------------------------------------------------
+// One rank's alignment to T (A5 / A6): aligned groups in emit order as (ap[k], ac[k]) over the sorted window,
+// ag[k] = list index of the head of the candidate group slot k was cut from; counts added into
+// step_tot[k] (= step_samples + step_base; integer atomics).  A device function: k_align and the persistent
+// round-loop kernel call it.  `ok` = scratch for the overflow sort (next_pow2(Gr) keys).
+__device__ __forceinline__ void align_body(int S, int Gr, int T, const int32_t *gp, int32_t *ap, int32_t *ac, int32_t *ag,
+                                           uint64_t *ok, int32_t *step_tot) {
+    if (Gr <= T) {
+        const int d = T - Gr;
+        const int lane = threadIdx.x & 31;
+        for (int j0 = (threadIdx.x >> 5) << 5; j0 < Gr; j0 += blockDim.x) {  // warp-uniform trip count
+            const int j = j0 + lane;
+            int p = 0, pn = 0, kj = 0, h = 0;
+            if (j < Gr) {
+                p = gp[j];
+                pn = gp[j + 1];
+                const int conv_from = min(d, (S - p) - (Gr - j));
+                const int conv_after = min(d, (S - pn) - (Gr - 1 - j));
+                kj = conv_from - conv_after;
+                h = j + d - conv_from;
+                const int c = pn - p - kj;
+                ap[h] = p;
+                ac[h] = c;
+                ag[h] = h;
+                atomicAdd(&step_tot[h], c);
+            }
+            uint32_t sp = __ballot_sync(ODB_FULL_MASK, kj > 0);
+            while (sp) {  // expand the singletons of the (few) groups that split
+                const int src = __ffs(sp) - 1;
+                sp &= sp - 1;
+                const int kk = __shfl_sync(ODB_FULL_MASK, kj, src);
+                const int hh = __shfl_sync(ODB_FULL_MASK, h, src);
+                const int pe = __shfl_sync(ODB_FULL_MASK, pn, src);
+                for (int i = lane; i < kk; i += 32) {
+                    ap[hh + 1 + i] = pe - kk + i;
+                    ac[hh + 1 + i] = 1;
+                    ag[hh + 1 + i] = hh;  // cut from the candidate group whose head sits at hh
+                    atomicAdd(&step_tot[hh + 1 + i], 1);
+                }
+            }
+        }
+        if (threadIdx.x == 0) ap[T] = S;
+    } else {
+        const int n2 = next_pow2(Gr);
+        for (int j = threadIdx.x; j < n2; j += blockDim.x) {
+            uint64_t key = ~0ull;
+            if (j < Gr) key = ((uint64_t)(uint32_t)(S - (gp[j + 1] - gp[j])) << 32) | (uint32_t)j;
+            ok[j] = key;
+        }
+        __syncthreads();
+        block_bitonic(ok, n2);
+        for (int k = threadIdx.x; k < T; k += blockDim.x) {
+            int j = key_id(ok[k]);
+            int p = gp[j], c = gp[j + 1] - p;
+            ap[k] = p;
+            ac[k] = c;
+            ag[k] = k;
+            atomicAdd(&step_tot[k], c);
+        }
+    }
+}
+
+// Eq. 3 from the reduced status of all ranks: T = max(min(max_A G, C+min, S+min), 1); 0 when A is empty
+__device__ __forceinline__ int target_groups(int maxG, int minS, int slot_capacity) {
+    int T = maxG;
+    if (slot_capacity > 0 && T > slot_capacity) T = slot_capacity;  // C+min (same C on every rank)
+    if (T > minS) T = minS;                                         // S+min
+    if (T < 1) T = 1;
+    if (maxG == 0) T = 0;  // A is empty: a skip round, nothing is emitted (Lemma 2)
+    return T;
+}
+
 __global__ void __launch_bounds__(kRankThreads)
 k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr, const int32_t *__restrict__ G_arr, int R,
         const int32_t *__restrict__ gs_world, int world_ranks, int join_mode, int slot_capacity, const int32_t *__restrict__ gpos, int32_t *__restrict__ agpos, int32_t *__restrict__ agcnt,
@@ -626,11 +706,7 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
             return;
         }
     }
-    int T = s_maxG;
-    if (slot_capacity > 0 && T > slot_capacity) T = slot_capacity;  // C+min (same C on every rank)
-    if (T > s_minS) T = s_minS;                                     // S+min
-    if (T < 1) T = 1;
-    if (s_maxG == 0) T = 0;  // A is empty: a skip round, nothing is emitted (Lemma 2)
+    const int T = target_groups(s_maxG, s_minS, slot_capacity);
     if (r == 0 && threadIdx.x == 0) rec->T = T;
     const int Gr = G_arr[r];
     if (Gr == 0) return;  // finished rank: IDLE slots are written by the commit kernel
@@ -639,62 +715,8 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
     const int S = S_arr[r];
     const int64_t base = rank_ptr[r];
     const int64_t jb = base + r;
-    const int32_t *gp = gpos + jb;
-    int32_t *ap = agpos + jb, *ac = agcnt + jb, *ag = agorg + jb;  // ag: list index of the candidate's head
-    if (Gr <= T) {
-        const int d = T - Gr;
-        const int lane = threadIdx.x & 31;
-        for (int j0 = (threadIdx.x >> 5) << 5; j0 < Gr; j0 += blockDim.x) {  // warp-uniform trip count
-            const int j = j0 + lane;
-            int p = 0, pn = 0, kj = 0, h = 0;
-            if (j < Gr) {
-                p = gp[j];
-                pn = gp[j + 1];
-                const int conv_from = min(d, (S - p) - (Gr - j));
-                const int conv_after = min(d, (S - pn) - (Gr - 1 - j));
-                kj = conv_from - conv_after;
-                h = j + d - conv_from;
-                const int c = pn - p - kj;
-                ap[h] = p;
-                ac[h] = c;
-                ag[h] = h;
-                atomicAdd(&step_samples[step_base + h], c);
-            }
-            uint32_t sp = __ballot_sync(ODB_FULL_MASK, kj > 0);
-            while (sp) {  // expand the singletons of the (few) groups that split
-                const int src = __ffs(sp) - 1;
-                sp &= sp - 1;
-                const int kk = __shfl_sync(ODB_FULL_MASK, kj, src);
-                const int hh = __shfl_sync(ODB_FULL_MASK, h, src);
-                const int pe = __shfl_sync(ODB_FULL_MASK, pn, src);
-                for (int i = lane; i < kk; i += 32) {
-                    ap[hh + 1 + i] = pe - kk + i;
-                    ac[hh + 1 + i] = 1;
-                    ag[hh + 1 + i] = hh;  // cut from the candidate group whose head sits at hh
-                    atomicAdd(&step_samples[step_base + hh + 1 + i], 1);
-                }
-            }
-        }
-        if (threadIdx.x == 0) ap[T] = S;
-    } else {
-        const int n2 = next_pow2(Gr);
-        uint64_t *ok = (n2 <= kAlignSmemKeys) ? reinterpret_cast<uint64_t *>(al_smem) : ovf + 2 * base;
-        for (int j = threadIdx.x; j < n2; j += blockDim.x) {
-            uint64_t key = ~0ull;
-            if (j < Gr) key = ((uint64_t)(uint32_t)(S - (gp[j + 1] - gp[j])) << 32) | (uint32_t)j;
-            ok[j] = key;
-        }
-        __syncthreads();
-        block_bitonic(ok, n2);
-        for (int k = threadIdx.x; k < T; k += blockDim.x) {
-            int j = key_id(ok[k]);
-            int p = gp[j], c = gp[j + 1] - p;
-            ap[k] = p;
-            ac[k] = c;
-            ag[k] = k;
-            atomicAdd(&step_samples[step_base + k], c);
-        }
-    }
+    uint64_t *ok = (next_pow2(Gr) <= kAlignSmemKeys) ? reinterpret_cast<uint64_t *>(al_smem) : ovf + 2 * base;
+    align_body(S, Gr, T, gpos + jb, agpos + jb, agcnt + jb, agorg + jb, ok, step_samples + step_base);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -704,21 +726,19 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
 // finished next round.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void
-commit_body(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
-         const int32_t *__restrict__ G_arr, int R, const int32_t *__restrict__ agpos, const int32_t *__restrict__ agcnt,
-         const int32_t *__restrict__ agorg, int32_t *__restrict__ agoff, const int32_t *__restrict__ step_samples, int step_base, int round, int join_mode,
-         long long quota, long long emitted_before, int32_t *__restrict__ st_count, int32_t *__restrict__ st_width,
-         int32_t *__restrict__ st_real, int32_t *__restrict__ st_round, int32_t *__restrict__ st_origin,
-         uint8_t *__restrict__ posflag,
-         int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
-         int32_t *fetch_pos, int32_t *emit_cur, const int32_t *__restrict__ emit_snap, RoundRec *rec) {
+commit_body(const int r, const uint64_t *keys, const int64_t *rank_ptr, const int32_t *S_arr,
+         const int32_t *G_arr, int R, const int32_t *agpos, const int32_t *agcnt,
+         const int32_t *agorg, int32_t *agoff, const int32_t *step_samples, int step_base, int round, int join_mode,
+         long long quota, long long emitted_before, int32_t *st_count, int32_t *st_width,
+         int32_t *st_real, int32_t *st_round, int32_t *st_origin,
+         uint8_t *posflag,
+         int32_t *emit_ids, int32_t *emit_pos, int32_t *left_ids, int32_t *n_left,
+         int32_t *fetch_pos, int32_t *emit_cur, const int32_t *emit_snap, RoundRec *rec, bool own_rec, int part, int nparts) {
     __shared__ int s_scan[34];
     __shared__ long long s_scan64[34];
     __shared__ int s_found;
-    const int r = blockIdx.x;
-    // gridDim.y CTAs per rank share the fast path below; everything that needs a rank-wide scan, and all
+    // nparts CTAs per rank share the fast path below; everything that needs a rank-wide scan, and all
     // state updates, is done by part 0 alone
-    const int part = blockIdx.y, nparts = gridDim.y;
     if (rec->done) {  // distributed mode: this round was the terminal check
         if (part != 0) return;
         if (r == 0 && threadIdx.x == 0) {
@@ -736,7 +756,7 @@ commit_body(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_
         long long carry = 0;
         for (int b0 = 0; b0 < T; b0 += blockDim.x) {
             int k = b0 + threadIdx.x;
-            long long v = (k < T) ? (long long)step_samples[step_base + k] : 0ll;
+            long long v = (k < T) ? (long long)__ldcg(&step_samples[step_base + k]) : 0ll;
             long long tot;
             long long ex = block_excl_scan<long long>(v, s_scan64, tot);
             if (k < T && emitted_before + carry + ex + v >= quota) atomicMin(&s_found, k);
@@ -750,9 +770,9 @@ commit_body(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_
         }
         __syncthreads();
     }
-    if (r == 0 && part == 0) {  // round totals for the host
+    if ((r == 0 || own_rec) && part == 0) {  // round totals for the host (or for this CTA, in the persistent round loop)
         long long acc = 0;
-        for (int k = threadIdx.x; k < T_emit; k += blockDim.x) acc += step_samples[step_base + k];
+        for (int k = threadIdx.x; k < T_emit; k += blockDim.x) acc += __ldcg(&step_samples[step_base + k]);
         long long tot;
         (void)block_excl_scan<long long>(acc, s_scan64, tot);
         if (threadIdx.x == 0) {
@@ -896,9 +916,9 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
          int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
          int32_t *fetch_pos, int32_t *emit_cur, const int32_t *__restrict__ emit_snap, RoundRec *rec, PlanDims *dims,
          unsigned int *done_ctr) {
-    commit_body(keys, rank_ptr, S_arr, G_arr, R, agpos, agcnt, agorg, agoff, step_samples, step_base, round, join_mode,
-                quota, emitted_before, st_count, st_width, st_real, st_round, st_origin, posflag, emit_ids, emit_pos,
-                left_ids, n_left, fetch_pos, emit_cur, emit_snap, rec);
+    commit_body(blockIdx.x, keys, rank_ptr, S_arr, G_arr, R, agpos, agcnt, agorg, agoff, step_samples, step_base, round,
+                join_mode, quota, emitted_before, st_count, st_width, st_real, st_round, st_origin, posflag, emit_ids,
+                emit_pos, left_ids, n_left, fetch_pos, emit_cur, emit_snap, rec, false, blockIdx.y, gridDim.y);
     if (!dims) return;  // distributed mode: the host decides from the gathered status
     __shared__ int s_last;
     __syncthreads();
@@ -929,6 +949,168 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
         dims->err = 0;
         dims->complete = bad ? 0 : complete;
         *done_ctr = 0u;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The whole round loop in ONE launch (A0 .. A8, every protocol round): the paper's operating point is a
+// grouping buffer of about a thousand samples per rank, i.e. tens of protocol rounds per rank stream,
+// each of them a few microseconds of work -- far less than a kernel launch plus a host round trip.
+// One persistent CTA per rank (cooperative launch: all R CTAs are resident) loops over the rounds:
+//   window fill + merge sort in shared memory (A0, A1) -> successor + jump-out tables (A2, A3) ->
+//   the rank's (G_r, S_r / "finished") goes into a double-buffered summary, GRID BARRIER -- the paper's one
+//   unconditional exchange per round (deadlock-freedom Lemma 3) -- every CTA evaluates Eq. 3 and
+//   the termination predicates on the same summary (Thm 3 proof P:341) -> split / overflow (A5, A6) ->
+//   [non-join with a quota: a second grid barrier, the global step totals are needed for the cut] ->
+//   commit (A7, A8a).
+// The device functions are the ones the per-round kernels use; per-round scratch lives in the same global
+// arrays (L2-resident).  Requirements (odb_api.cu checks them): windows of at most 4096 samples, R resident
+// CTAs, every view has arrived (no odb_set_available), single-process mode.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int *p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// all CTAs of the (cooperatively launched) grid; `target` = arrivals expected so far, counter zeroed by the host
+__device__ __forceinline__ void grid_barrier(unsigned int *ctr, unsigned int target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(ctr, 1u);
+        while (ld_acquire_u32(ctr) < target) {
+        }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+struct RoundsArgs {
+    SortArgs sort;  // window fill + sort inputs (first = 1: the per-run state is cleared in round 0)
+    int R;
+    uint32_t budget;
+    int rule, join_mode, slot_capacity;
+    long long quota, emitted_before;
+    int32_t *G, *S, *gpos, *agpos, *agcnt, *agorg, *agoff, *emit_snap;
+    int32_t *st_count, *st_width, *st_real, *st_round, *st_origin;
+    uint8_t *posflag;
+    int32_t *emit_ids, *left_ids_w;
+    int32_t *gs;  // [2][2 R]: the per-round summary, double-buffered by round parity
+    unsigned int *bar;
+    PlanDims *dims;
+};
+
+__global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
+    extern __shared__ __align__(16) unsigned char rd_smem[];  // kMsPadded keys: sort buffer, then form / overflow scratch
+    __shared__ int s_scan[34];
+    __shared__ uint16_t s_e2[32];
+    __shared__ int s_red[3];
+    __shared__ RoundRec s_rec;
+    uint64_t *X = reinterpret_cast<uint64_t *>(rd_smem);
+    const int r = blockIdx.x, t = threadIdx.x, R = A.R;
+    const SortArgs &SA = A.sort;
+    ms_first_round_init(SA, (int64_t)r * kMsThreads + t, (int64_t)gridDim.x * kMsThreads);
+    const int64_t base = SA.rank_ptr[r];
+    const int n_r = (int)(SA.rank_ptr[r + 1] - base);
+    const int64_t jb = base + r;
+    uint64_t *keys = SA.keys_out;
+    if (t == 0) {
+        SA.n_left[r] = 0;
+        SA.fetch_pos[r] = 0;
+        SA.emit_cur[r] = 0;
+    }
+    __syncthreads();
+    unsigned int n_bar = 0;
+    int n_steps = 0, n_rounds = 0, stop = 0, bad = 0;
+    long long emitted_before = A.emitted_before;
+    const bool quota_mode = !A.join_mode && A.quota > 0;
+    for (int round = 0;; ++round) {
+        // ---- A0 + A1: this rank's window, sorted ----
+        const int nl = SA.n_left[r], fp = SA.fetch_pos[r];
+        const int S = ms_window_size(nl, fp, n_r, SA.buffer_size);
+        int G = 0;
+        if (S > 0) {
+            uint64_t k[16];
+            ms_load_keys(SA, base, nl, fp, 0, S, k);
+            ms_sort_cta(k, X);
+            for (int i = t; i < S; i += kMsThreads) keys[base + i] = X[ms_pad(i)];
+            __syncthreads();
+            // ---- A2 + A3: candidate groups ----
+            G = form_hier_body(keys + base, S, A.budget, A.rule, A.gpos + jb, rd_smem, s_scan, s_e2);
+        }
+        // ---- the exchange: (G_r, S_r), S_r = -1 for "finished" (nothing buffered, nothing pending) ----
+        int32_t *gs = A.gs + (size_t)(round & 1) * 2 * R;
+        if (t == 0) {
+            A.G[r] = G;
+            A.S[r] = S;
+            __stcg(&gs[2 * r], G);
+            __stcg(&gs[2 * r + 1], S == 0 ? -1 : S);
+            s_red[0] = 0;
+            s_red[1] = 0x7fffffff;
+            s_red[2] = 0;
+        }
+        grid_barrier(A.bar, (unsigned int)R * (++n_bar));
+        for (int q = t; q < R; q += kMsThreads) {
+            const int g = __ldcg(&gs[2 * q]), sq = __ldcg(&gs[2 * q + 1]);
+            if (g > 0) {  // active set A = {r : G_r > 0}
+                atomicMax(&s_red[0], g);
+                if (sq > 0) atomicMin(&s_red[1], sq);
+            }
+            if (sq < 0) atomicAdd(&s_red[2], 1);
+        }
+        if (round == 0 && t == 0) bad = __ldcg(&SA.rec->bad_length);
+        bad = __syncthreads_or(bad);
+        if (bad) break;
+        const int n_fin = s_red[2];
+        // termination predicates, identical in every CTA (Thm 3 proof P:341)
+        if (A.join_mode ? (n_fin == R) : (n_fin > 0)) {
+            stop = A.join_mode ? ODB_STOP_ALL_FINISHED : ODB_STOP_LOGICAL;
+            n_rounds = round + 1;  // this round was the terminal check
+            break;
+        }
+        const int T = target_groups(s_red[0], s_red[1], A.slot_capacity);
+        __syncthreads();  // s_red is rewritten next round
+        if ((long long)n_steps + T > SA.step_cap) {  // cannot happen (n_steps <= the longest stream); never write past the tables
+            bad = 2;
+            break;
+        }
+        // ---- A4 .. A6: align to T ----
+        if (G > 0) {
+            if (t == 0) A.emit_snap[r] = SA.emit_cur[r];
+            align_body(S, G, T, A.gpos + jb, A.agpos + jb, A.agcnt + jb, A.agorg + jb, X, SA.step_samples + n_steps);
+        }
+        if (quota_mode) grid_barrier(A.bar, (unsigned int)R * (++n_bar));  // the global step totals are complete
+        if (t == 0) {
+            s_rec.T = T;
+            s_rec.done = 0;
+            s_rec.n_finished = 0;
+        }
+        __syncthreads();
+        // ---- A7 + A8a: commit ----
+        commit_body(r, keys, SA.rank_ptr, A.S, A.G, R, A.agpos, A.agcnt, A.agorg, A.agoff, SA.step_samples, n_steps, round,
+                    A.join_mode, A.quota, emitted_before, A.st_count, A.st_width, A.st_real, A.st_round, A.st_origin,
+                    A.posflag, A.emit_ids, SA.emit_pos, A.left_ids_w, SA.n_left, SA.fetch_pos, SA.emit_cur, A.emit_snap,
+                    &s_rec, true, 0, 1);
+        __syncthreads();
+        n_steps += s_rec.T_emit;
+        if (quota_mode) {
+            emitted_before += s_rec.emitted_round;
+            if (s_rec.quota_hit) {  // Thm 2 / P:347
+                stop = ODB_STOP_QUOTA;
+                n_rounds = round + 1;
+                break;
+            }
+        }
+        __syncthreads();  // s_rec is rewritten next round
+    }
+    if (r == 0 && t == 0) {
+        A.dims->n_steps = n_steps;
+        A.dims->n_rounds = n_rounds;
+        A.dims->stop_reason = stop;
+        A.dims->bad_length = bad == 1 ? 1 : 0;
+        A.dims->err = bad == 2 ? ODB_ERR_STATE : 0;
+        A.dims->complete = bad ? 0 : 1;
     }
 }
 
@@ -1254,6 +1436,80 @@ cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     k_pack_summary<<<(R + 127) / 128, 128, 0, st>>>(R, c->G, c->S, c->d_rank_ptr, c->fetch_pos, c->gs_local, c->d_rec);
     ODB_LAUNCH_CHECK(c);
+    return cudaSuccess;
+}
+
+// The whole round loop in one cooperative launch (k_rounds).  cudaErrorNotSupported when the R CTAs cannot
+// all be resident on this device (the caller then drives the rounds from the host).
+cudaError_t launch_rounds(odb_ctx *c, cudaStream_t st) {
+    const int R = c->prm.n_ranks;
+    const size_t smem = (size_t)kMsPadded * sizeof(uint64_t);
+    if (c->rounds_max_ctas == 0) {
+        int occ = 0, coop = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device);
+        if (e != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_rounds, kMsThreads, smem);
+        if (e != cudaSuccess) return e;
+        c->rounds_max_ctas = coop ? std::max(occ * c->sm_count, 1) : -1;
+    }
+    if (c->rounds_max_ctas < R) return cudaErrorNotSupported;
+    if (!c->gs_rounds) {
+        cudaError_t e = cudaMalloc((void **)&c->gs_rounds, (size_t)4 * R * sizeof(int32_t) + 64);
+        if (e != cudaSuccess) return e;
+    }
+    // the barrier counter lives behind the summary
+    unsigned int *bar = reinterpret_cast<unsigned int *>(c->gs_rounds + (size_t)4 * R);
+    cudaError_t e = cudaMemsetAsync(bar, 0, 64, st);
+    if (e != cudaSuccess) return e;
+    RoundsArgs A;
+    memset(&A, 0, sizeof(A));
+    A.sort.len = c->d_lengths;
+    A.sort.rank_ptr = c->d_rank_ptr;
+    A.sort.n_left = c->n_left;
+    A.sort.fetch_pos = c->fetch_pos;
+    A.sort.emit_cur = c->emit_cur;
+    A.sort.left_ids = c->left_ids;
+    A.sort.arrived = c->d_arrived;
+    A.sort.buffer_size = c->prm.buffer_size;
+    A.sort.keys_out = c->keyA;
+    A.sort.S_out = c->S;
+    A.sort.rec = c->d_rec;
+    A.sort.first = 1;
+    A.sort.n_total = c->n_total;
+    A.sort.emit_pos = c->emit_pos;
+    A.sort.step_samples = c->step_samples.p;
+    A.sort.step_cap = c->step_samples.p ? (int64_t)c->step_samples.cap : 0;
+    A.R = R;
+    A.budget = (uint32_t)c->prm.budget;
+    A.rule = c->prm.rule;
+    A.join_mode = c->prm.join_mode;
+    A.slot_capacity = c->prm.slot_capacity;
+    A.quota = (long long)c->prm.sample_quota;
+    A.emitted_before = (long long)c->prm.emitted_so_far;
+    A.G = c->G;
+    A.S = c->S;
+    A.gpos = c->gpos;
+    A.agpos = c->agpos;
+    A.agcnt = c->agcnt;
+    A.agorg = c->agorg;
+    A.agoff = c->agoff;
+    A.emit_snap = c->emit_snap;
+    A.st_count = c->st_count.p;
+    A.st_width = c->st_width.p;
+    A.st_real = c->st_real.p;
+    A.st_round = c->st_round.p;
+    A.st_origin = c->st_origin.p;
+    A.posflag = c->posflag;
+    A.emit_ids = c->emit_ids;
+    A.left_ids_w = c->left_ids;
+    A.gs = c->gs_rounds;
+    A.bar = bar;
+    A.dims = c->d_dims;
+    void *args[] = {(void *)&A};
+    e = cudaLaunchCooperativeKernel((const void *)k_rounds, dim3((unsigned)R), dim3(kMsThreads), args, smem, st);
+    if (e != cudaSuccess) return e;
+    c->launches++;
+    c->sorted = c->keyA;
     return cudaSuccess;
 }
 

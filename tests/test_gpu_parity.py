@@ -218,6 +218,39 @@ def test_cluster_sort_window_sizes(P, oracle, n, rule):
     assert plan.samples_emitted == wl.n_samples
 
 
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("join", [1, 0])
+def test_paper_operating_point_buffer_1024(P, oracle, rule, join):
+    """The paper's operating point: a 1024-sample grouping buffer per rank, tens of protocol rounds per
+    rank stream -- through odb_run, i.e. the persistent round-loop kernel (one launch for every round) --
+    on the configs[3] recipe (16 ranks x 16384 samples, high-CV long tail): plan tables in full, every element
+    of every slot."""
+    wl = I.make_workload(3, rule=rule, join_mode=join)
+    wl.params["buffer_size"] = 1024
+    plan = _full_size_elementwise(oracle, wl)
+    assert plan.n_rounds >= 16
+
+
+@pytest.mark.parametrize("buffer_size,slot_capacity", [(4096, 0), (1000, 7), (333, 0), (64, 3)])
+def test_round_loop_kernel_windows(P, oracle, buffer_size, slot_capacity):
+    """Persistent round-loop kernel: full 4096-key windows, ragged windows, overflow + recirculation through
+    finite slot capacity, unequal streams (IDLE slots while other ranks continue), both modes with a quota."""
+    rng = np.random.default_rng(buffer_size)
+    per = [rng.integers(1, 2000, 9000), rng.integers(1, 300, 5000), rng.integers(500, 4000, 2500), np.zeros(0, np.int64)]
+    for join in (1, 0):
+        wl = I.custom_workload("round_loop", per[: 3 + join], 41, budget=8192, buffer_size=buffer_size,
+                               slot_capacity=slot_capacity, join_mode=join)
+        if not join:
+            wl.params["sample_quota"] = int(0.7 * wl.n_samples)
+        plan, _ = oracle.run_workload(wl, collate=False)
+        info, out, _ = Par.run_gpu(wl, staged=False)
+        Par.compare_plan(plan, info, out)
+        Par.compare_full_by_rank(oracle, wl, plan, out)
+        # and the staged API (host-driven rounds) gives the same plan
+        info2, out2, _ = Par.run_gpu(wl, staged=True)
+        Par.compare_plan(plan, info2, out2)
+
+
 def test_heavy_split_unequal_group_counts(P, oracle):
     """One rank forms thousands of groups, another a handful of big ones: the split closed form turns
     thousands of rows of a few groups into singletons (Alg. 1)."""
