@@ -30,8 +30,7 @@ namespace odb {
 //          16-aligned region [grp_offset[s], grp_offset[s+1]) (IDLE slots own none): the 32-byte TileRec
 //          the collate kernel starts a tile with.  These blocks also clear what the collate kernel
 //          accumulates into (grp_valid, the work counters) and copy the plan tables into the caller's;
-//   ids    one block per rank: the slot CSR's ids are the rank's emit region (slots of a rank are in
-//          emit order), and the un-emitted local ids, ascending (Lemma 1: buffer + sampler-pending).
+//   ids    one block per rank: the un-emitted local ids, ascending (Lemma 1: buffer + sampler-pending).
 // ---------------------------------------------------------------------------------------------
 constexpr int kPrepThreads = 1024;
 
@@ -82,9 +81,16 @@ __device__ __forceinline__ void prep_rows(const PrepArgs &A, int n_steps, int b)
     const int i = bx * kPrepThreads + threadIdx.x;
     if (i >= n_r) return;
     const int64_t g = base + i;
+    const int64_t q0 = A.grp_sample_ptr[(int64_t)r * n_steps];
+    // the slot CSR's ids are the rank's emit region (slots of a rank are in emit order): entry i of it
+    if (i < A.emit_cur[r]) {
+        const int32_t id = A.emit_ids[g];
+        A.grp_sample_ids[q0 + i] = id;
+        if (A.user_ids) A.user_ids[q0 + i] = id;
+    }
     const int p = A.emit_pos[g];
     if (p < 0) return;
-    const int64_t q = A.grp_sample_ptr[(int64_t)r * n_steps] + p;
+    const int64_t q = q0 + p;
     RowDesc d;
     d.tok = A.sample_ptr[g];
     d.len = A.len[g];
@@ -132,15 +138,7 @@ __device__ __forceinline__ void prep_ids(const PrepArgs &A, int n_steps, int r) 
     const int R = A.R;
     const int64_t base = A.rank_ptr[r];
     const int n_r = (int)(A.rank_ptr[r + 1] - base);
-    const int ec = A.emit_cur[r];
-    if (ec > 0) {
-        const int64_t q0 = A.grp_sample_ptr[(int64_t)r * n_steps];
-        for (int j = threadIdx.x; j < ec; j += blockDim.x) {
-            const int32_t id = A.emit_ids[base + j];
-            A.grp_sample_ids[q0 + j] = id;
-            if (A.user_ids) A.user_ids[q0 + j] = id;
-        }
-    }
+    const int ec = A.emit_cur[r];  // (the slot CSR's ids are copied by the row threads)
     long long part = 0;
     for (int q = threadIdx.x; q < r; q += blockDim.x) part += (A.rank_ptr[q + 1] - A.rank_ptr[q]) - A.emit_cur[q];
     long long lbase;

@@ -448,7 +448,8 @@ form_hier_body(const uint64_t *k, int S, uint32_t budget, int rule, int32_t *gp,
     }
     __syncthreads();
     // out2: one warp per superblock, its blocks from the last to the first, a lane per position
-    {
+    // (a window of one superblock needs none: the orbit enters it at 0)
+    if (nb2 > 1) {
         const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
         for (int sb = w; sb < nb2; sb += nw) {
             const int slo = sb << 10, send = min(S, slo + 1024);
@@ -466,10 +467,12 @@ form_hier_body(const uint64_t *k, int S, uint32_t budget, int rule, int32_t *gp,
     // top-down: where the orbit of 0 enters each superblock, each block, and its marks inside each block
     if (threadIdx.x == 0) {
         int x = 0;
-        while (x < S) {
-            s_e2[x >> 10] = (uint16_t)x;
-            x = out2[fg_pad(x)];
-        }
+        if (nb2 == 1) s_e2[0] = 0;
+        else
+            while (x < S) {
+                s_e2[x >> 10] = (uint16_t)x;
+                x = out2[fg_pad(x)];
+            }
     }
     __syncthreads();
     if (threadIdx.x < nb2 && s_e2[threadIdx.x] != kNone) {
@@ -1031,9 +1034,10 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
         const int S = ms_window_size(nl, fp, n_r, SA.buffer_size);
         int G = 0;
         if (S > 0) {
-            uint64_t k[16];
-            ms_load_keys(SA, base, nl, fp, 0, S, k);
-            ms_sort_cta(k, X);
+            uint64_t k[kMsItems];
+            const int n_keys = ms_active_keys(S);
+            ms_load_keys(SA, base, nl, fp, 0, S, n_keys, k);
+            ms_sort_cta(k, X, n_keys);
             for (int i = t; i < S; i += kMsThreads) keys[base + i] = X[ms_pad(i)];
             __syncthreads();
             // ---- A2 + A3: candidate groups ----

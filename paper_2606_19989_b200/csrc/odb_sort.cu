@@ -2,8 +2,8 @@
 // (length, local id) (paper section 2.2 P:36 "sorted ascending"; reading U1).  sm_100a only.
 //
 // A rank's window of up to CL * 4096 keys is sorted by a thread-block CLUSTER of CL CTAs (CL = 1, 2, 4, 8
-// or 16): each CTA merge-sorts 4096 keys in its shared memory (16 keys per thread: a register sorting
-// network, then eight merge-path levels), then log2(CL) cross-CTA levels merge runs that live in the
+// or 16): each CTA merge-sorts 4096 keys in its shared memory (1024 threads x 4 keys: a register sorting
+// network, then ten merge-path levels with 4-step serial merges), then log2(CL) cross-CTA levels merge runs that live in the
 // shared memory of neighbouring CTAs, read through distributed shared memory (DSMEM): a CTA cuts its
 // 4096-key output tile out of the two runs with merge-path searches over DSMEM, stages the two input
 // pieces locally with coalesced DSMEM loads, merges them from local shared memory, and the cluster
@@ -22,7 +22,7 @@ namespace odb {
     } while (0)
 
 // grid = (CL, R), cluster (CL, 1, 1).  Dynamic shared memory: X (and Y when CL > 1), kMsPadded keys each.
-__global__ void __launch_bounds__(kMsThreads, 2) k_sort_window(const SortArgs A, int CL) {
+__global__ void __launch_bounds__(kMsThreads) k_sort_window(const SortArgs A, int CL) {
     extern __shared__ __align__(16) unsigned char ms_smem[];
     uint64_t *X = reinterpret_cast<uint64_t *>(ms_smem);
     uint64_t *Y = X + kMsPadded;
@@ -47,9 +47,11 @@ __global__ void __launch_bounds__(kMsThreads, 2) k_sort_window(const SortArgs A,
     if (S == 0) return;  // the whole cluster leaves
     const int c0 = c * kMsChunk;
     const int cnt = max(0, min(kMsChunk, S - c0));
-    uint64_t k[16];
-    ms_load_keys(A, base, nl, fp, c0, cnt, k);
-    ms_sort_cta(k, X);
+    uint64_t k[kMsItems];
+    // (a lone CTA sorts only as many keys as its window needs; in a cluster every CTA sorts a full chunk)
+    const int n_keys = CL == 1 ? ms_active_keys(cnt) : kMsChunk;
+    ms_load_keys(A, base, nl, fp, c0, cnt, n_keys, k);
+    ms_sort_cta(k, X, n_keys);
     uint64_t *out = A.keys_out + base;
     if (CL == 1) {
         for (int i = t; i < cnt; i += kMsThreads) out[i] = X[ms_pad(i)];
@@ -72,12 +74,12 @@ __global__ void __launch_bounds__(kMsThreads, 2) k_sort_window(const SortArgs A,
         for (int i = t; i < kMsChunk; i += kMsThreads)
             Y[ms_pad(i)] = i < la ? ms_run_key(x_addr, p0, a0 + i) : ms_run_key(x_addr, p0 + m, b0 + (i - la));
         __syncthreads();
-        const int ai = ms_path_local(Y, 0, la, la, kMsChunk - la, 16 * t);
-        ms_merge16(Y, ai, la, la + (16 * t - ai), kMsChunk, k);
+        const int ai = ms_path_local(Y, 0, la, la, kMsChunk - la, kMsItems * t);
+        ms_merge_items(Y, ai, la, la + (kMsItems * t - ai), kMsChunk, k);
         (void)b1;
         cluster_sync_all();  // every CTA has read what it needs from the others' X
 #pragma unroll
-        for (int q = 0; q < 16; ++q) X[ms_pad(16 * t + q)] = k[q];
+        for (int q = 0; q < kMsItems; ++q) X[ms_pad(kMsItems * t + q)] = k[q];
         __syncthreads();
     }
     for (int i = t; i < cnt; i += kMsThreads) out[c0 + i] = X[ms_pad(i)];

@@ -7,13 +7,13 @@
 
 namespace odb {
 
-constexpr int kMsThreads = 256;
-constexpr int kMsItems = 16;
+constexpr int kMsThreads = 1024;
+constexpr int kMsItems = 4;                      // keys per thread: short serial merges, many threads to hide latency
 constexpr int kMsChunk = kMsThreads * kMsItems;  // 4096 keys per CTA
 static_assert(kMsChunk == kSortChunk, "one CTA sorts one chunk");
-constexpr int kMsPadded = kMsChunk + kMsChunk / 16;  // one spare key per 16: conflict-free 16-key runs
+constexpr int kMsPadded = kMsChunk + kMsChunk / kMsItems;  // one spare key per thread run: conflict-free stores
 
-__device__ __forceinline__ int ms_pad(int i) { return i + (i >> 4); }
+__device__ __forceinline__ int ms_pad(int i) { return i + (i >> 2); }
 
 // ---- cluster / DSMEM primitives (PTX; no cooperative-groups dependency) --------------------------
 __device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -38,15 +38,15 @@ __device__ __forceinline__ void ms_cmp_xchg(uint64_t &lo, uint64_t &hi, bool asc
     hi = b;
 }
 
-// ascending sort of 16 keys in registers: the bitonic network (10 stages, 80 compare-exchanges)
-__device__ __forceinline__ void ms_sort16(uint64_t (&k)[16]) {
+// ascending sort of this thread's keys in registers: the bitonic network
+__device__ __forceinline__ void ms_sort_items(uint64_t (&k)[kMsItems]) {
 #pragma unroll
-    for (int kk = 2; kk <= 16; kk <<= 1) {
+    for (int kk = 2; kk <= kMsItems; kk <<= 1) {
 #pragma unroll
         for (int j = kk >> 1; j > 0; j >>= 1) {
 #pragma unroll
-            for (int r = 0; r < 16; ++r)
-                if ((r & j) == 0) ms_cmp_xchg(k[r], k[r | j], kk == 16 || (r & kk) == 0);
+            for (int r = 0; r < kMsItems; ++r)
+                if ((r & j) == 0) ms_cmp_xchg(k[r], k[r | j], kk == kMsItems || (r & kk) == 0);
         }
     }
 }
@@ -62,43 +62,59 @@ __device__ __forceinline__ int ms_path_local(const uint64_t *X, int a0, int na, 
     return lo;
 }
 
-// 16 outputs of merge(X[a.. a_end), X[b.. b_end)) starting at the split (ai, bi), into registers
-__device__ __forceinline__ void ms_merge16(const uint64_t *X, int ai, int a_end, int bi, int b_end, uint64_t (&out)[16]) {
+// kMsItems outputs of merge(X[a.. a_end), X[b.. b_end)) starting at the split (ai, bi), into registers
+__device__ __forceinline__ void ms_merge_items(const uint64_t *X, int ai, int a_end, int bi, int b_end,
+                                               uint64_t (&out)[kMsItems]) {
     uint64_t ka = ai < a_end ? X[ms_pad(ai)] : ~0ull;
     uint64_t kb = bi < b_end ? X[ms_pad(bi)] : ~0ull;
 #pragma unroll
-    for (int q = 0; q < 16; ++q) {
+    for (int q = 0; q < kMsItems; ++q) {
         // keys are unique (the id is part of the key), padding keys (~0) sort last: ties are irrelevant
         const bool take_a = (bi >= b_end) || (ai < a_end && ka < kb);
         out[q] = take_a ? ka : kb;
-        if (take_a) {
-            ++ai;
-            ka = ai < a_end ? X[ms_pad(ai)] : ~0ull;
-        } else {
-            ++bi;
-            kb = bi < b_end ? X[ms_pad(bi)] : ~0ull;
+        if (q + 1 < kMsItems) {
+            if (take_a) {
+                ++ai;
+                ka = ai < a_end ? X[ms_pad(ai)] : ~0ull;
+            } else {
+                ++bi;
+                kb = bi < b_end ? X[ms_pad(bi)] : ~0ull;
+            }
         }
     }
 }
 
-// The CTA-local part: 16 keys per thread (any assignment) -> X holds the 4096 keys ascending (padded layout).
-// All kMsThreads threads must call it.
-__device__ __forceinline__ void ms_sort_cta(uint64_t (&k)[16], uint64_t *X) {
-    const int t = threadIdx.x;
-    ms_sort16(k);
+// Keys in play for a window of S keys: a power of two, at least one warp's worth, at most the chunk.
+__device__ __forceinline__ int ms_active_keys(int S) {
+    int n = 32 * kMsItems;
+    while (n < S) n <<= 1;
+    return min(n, kMsChunk);
+}
+
+// The CTA-local part: the first n_keys / kMsItems threads hold kMsItems keys each (any assignment) -> X holds
+// the n_keys keys ascending (padded layout).  n_keys = ms_active_keys(.).  All kMsThreads threads must call it.
+__device__ __forceinline__ void ms_sort_cta(uint64_t (&k)[kMsItems], uint64_t *X, int n_keys) {
+    const int o = kMsItems * (int)threadIdx.x;
+    const bool active = o < n_keys;
+    if (active) {
+        ms_sort_items(k);
 #pragma unroll
-    for (int q = 0; q < 16; ++q) X[ms_pad(16 * t + q)] = k[q];
+        for (int q = 0; q < kMsItems; ++q) X[ms_pad(o + q)] = k[q];
+    }
     __syncthreads();
 #pragma unroll 1
-    for (int w = 16; w < kMsChunk; w <<= 1) {  // runs of w keys are merged pairwise; thread t owns outputs [16 t, 16 t + 16)
-        const int o = 16 * t;
-        const int ps = o & ~(2 * w - 1);  // first key of the pair of runs
-        const int d = o - ps;
-        const int ai = ms_path_local(X, ps, w, ps + w, w, d);
-        ms_merge16(X, ps + ai, ps + w, ps + w + (d - ai), ps + 2 * w, k);
+    for (int w = kMsItems; w < n_keys; w <<= 1) {  // runs of w keys are merged pairwise; a thread owns kMsItems outputs
+        if (active) {
+            const int ps = o & ~(2 * w - 1);  // first key of the pair of runs
+            const int d = o - ps;
+            const int ai = ms_path_local(X, ps, w, ps + w, w, d);
+            ms_merge_items(X, ps + ai, ps + w, ps + w + (d - ai), ps + 2 * w, k);
+        }
         __syncthreads();  // every read of this level is done
+        if (active) {
 #pragma unroll
-        for (int q = 0; q < 16; ++q) X[ms_pad(o + q)] = k[q];
+            for (int q = 0; q < kMsItems; ++q) X[ms_pad(o + q)] = k[q];
+        }
         __syncthreads();
     }
 }
@@ -159,15 +175,16 @@ __device__ __forceinline__ void ms_first_round_init(const SortArgs &A, int64_t m
     if (__syncthreads_or(bad) && threadIdx.x == 0) A.rec->bad_length = 1;
 }
 
-// this thread's 16 keys of the chunk [c0, c0 + cnt) of rank r's window (any assignment will do: coalesced)
-__device__ __forceinline__ void ms_load_keys(const SortArgs &A, int64_t base, int nl, int fp, int c0, int cnt,
-                                             uint64_t (&k)[16]) {
-    const int t = threadIdx.x;
+// the keys of the chunk [c0, c0 + cnt) of rank r's window, kMsItems per thread on the first n_keys / kMsItems
+// threads (any assignment will do: coalesced); positions beyond cnt are padding that sorts to the end
+__device__ __forceinline__ void ms_load_keys(const SortArgs &A, int64_t base, int nl, int fp, int c0, int cnt, int n_keys,
+                                             uint64_t (&k)[kMsItems]) {
+    const int t = threadIdx.x, na = n_keys / kMsItems;
 #pragma unroll
-    for (int q = 0; q < 16; ++q) {
-        const int e = q * kMsThreads + t;
-        uint64_t key = ~0ull;  // padding sorts to the end
-        if (e < cnt) {
+    for (int q = 0; q < kMsItems; ++q) {
+        const int e = q * na + t;
+        uint64_t key = ~0ull;
+        if (t < na && e < cnt) {
             const int w = c0 + e;
             const int id = w < nl ? A.left_ids[base + w] : fp + (w - nl);
             const int l = A.len[base + id];
