@@ -434,7 +434,30 @@ form_hier_body(const uint64_t *k, int S, uint32_t budget, int rule, int32_t *gp,
     uint16_t *e1 = out2 + npe;                                  // nb1 entries (padded to even)
     uint32_t *mk = reinterpret_cast<uint32_t *>(e1 + ((nb1 + 1) & ~1));  // nb1 words
     constexpr uint16_t kNone = 0xFFFFu;
-    for (int x = threadIdx.x; x < S; x += blockDim.x) nxt[fg_pad(x)] = (uint16_t)successor(k, x, S, budget, rule);
+    if (rule == ODB_RULE_THRESHOLD) {
+        // J[x] = min(S, x + B(len(v[x-1]))), B from Eq. 1; eight independent (coalesced) key loads in flight per
+        // thread: a load per iteration would serialise on the L2 latency
+        for (int x0 = threadIdx.x; x0 < S; x0 += 8 * blockDim.x) {
+            uint32_t l[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int x = x0 + u * blockDim.x;
+                l[u] = (x > 0 && x < S) ? key_len(k[S - x]) : 1u;
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int x = x0 + u * blockDim.x;
+                if (x < S) {
+                    uint32_t q = budget / (l[u] > 0u ? l[u] : 1u);  // Eq. 1 floor; budget < 2^31
+                    if (q < 1u) q = 1u;
+                    const uint32_t jj = (uint32_t)x + q;
+                    nxt[fg_pad(x)] = (uint16_t)(x == 0 ? 1u : (jj < (uint32_t)S ? jj : (uint32_t)S));
+                }
+            }
+        }
+    } else {
+        for (int x = threadIdx.x; x < S; x += blockDim.x) nxt[fg_pad(x)] = (uint16_t)successor(k, x, S, budget, rule);
+    }
     for (int b = threadIdx.x; b < nb1; b += blockDim.x) e1[b] = kNone;
     if (threadIdx.x < 32) s_e2[threadIdx.x] = kNone;
     __syncthreads();
@@ -728,15 +751,23 @@ k_align(const int64_t *__restrict__ rank_ptr, const int32_t *__restrict__ S_arr,
 // position), compacts the leftovers, advances the rank state and counts the ranks that will be
 // finished next round.
 // ---------------------------------------------------------------------------------------------
+// one rank's slices of the per-round scratch: global memory (per-round kernels) or shared memory (k_rounds)
+struct RankView {
+    const uint64_t *k;                 // the sorted window
+    const int32_t *ap, *ac, *ag;       // aligned groups: start position, count, origin
+    int32_t *ao;                       // their emit offsets (slow path)
+    uint8_t *pf;                       // "emitted" flags over window positions (slow path)
+    int S, Gr, cur, n_r;               // window size, candidate groups, emit cursor before this round, stream length
+    int64_t base;                      // first global sample of the rank
+    int32_t *n_left, *fetch_pos, *emit_cur;  // the rank's state words
+};
+
 __device__ __forceinline__ void
-commit_body(const int r, const uint64_t *keys, const int64_t *rank_ptr, const int32_t *S_arr,
-         const int32_t *G_arr, int R, const int32_t *agpos, const int32_t *agcnt,
-         const int32_t *agorg, int32_t *agoff, const int32_t *step_samples, int step_base, int round, int join_mode,
-         long long quota, long long emitted_before, int32_t *st_count, int32_t *st_width,
-         int32_t *st_real, int32_t *st_round, int32_t *st_origin,
-         uint8_t *posflag,
-         int32_t *emit_ids, int32_t *emit_pos, int32_t *left_ids, int32_t *n_left,
-         int32_t *fetch_pos, int32_t *emit_cur, const int32_t *emit_snap, RoundRec *rec, bool own_rec, int part, int nparts) {
+commit_body(const int r, const int R, const RankView V, const int32_t *step_samples, int step_base, int round, int join_mode,
+            long long quota, long long emitted_before, int32_t *st_count, int32_t *st_width, int32_t *st_real,
+            int32_t *st_round, int32_t *st_origin, int32_t *emit_ids, int32_t *emit_pos, int32_t *left_ids, RoundRec *rec,
+            bool own_rec, int part, int nparts) {
+
     __shared__ int s_scan[34];
     __shared__ long long s_scan64[34];
     __shared__ int s_found;
@@ -784,10 +815,8 @@ commit_body(const int r, const uint64_t *keys, const int64_t *rank_ptr, const in
             rec->emitted_round = tot;
         }
     }
-    const int Gr = G_arr[r];
-    const int S = S_arr[r];
-    const int64_t base = rank_ptr[r];
-    const int n_r = (int)(rank_ptr[r + 1] - base);
+    const int Gr = V.Gr, S = V.S, n_r = V.n_r;
+    const int64_t base = V.base;
     if (Gr == 0) {  // finished rank: IDLE slots (U14)
         if (part != 0) return;
         for (int k = threadIdx.x; k < T_emit; k += blockDim.x) {
@@ -799,15 +828,14 @@ commit_body(const int r, const uint64_t *keys, const int64_t *rank_ptr, const in
             st_origin[idx] = step_base + k;
         }
         // finished (nothing buffered, nothing pending) or merely waiting for the workers (status 0)?
-        if (threadIdx.x == 0 && n_left[r] == 0 && fetch_pos[r] >= n_r) atomicAdd(&rec->n_finished, 1);
+        if (threadIdx.x == 0 && *V.n_left == 0 && *V.fetch_pos >= n_r) atomicAdd(&rec->n_finished, 1);
         return;
     }
-    const int64_t jb = base + r;
-    const uint64_t *k_ = keys + base;
-    const int32_t *ap = agpos + jb, *ac = agcnt + jb;
-    int32_t *ao = agoff + jb;
-    uint8_t *pf = posflag + base;
-    const int cur = emit_snap[r];  // emit_cur[r] as k_align saw it (part 0 advances emit_cur below)
+    const uint64_t *k_ = V.k;
+    const int32_t *ap = V.ap, *ac = V.ac;
+    int32_t *ao = V.ao;
+    uint8_t *pf = V.pf;
+    const int cur = V.cur;  // emit_cur[r] as k_align saw it (part 0 advances emit_cur below)
     // every sample of the window is emitted unless groups were dropped (overflow) or cut (quota)
     const bool all_emitted = (Gr <= T) && (T_emit == T);
     int emitted_r;
@@ -829,7 +857,7 @@ commit_body(const int r, const uint64_t *keys, const int64_t *rank_ptr, const in
             st_count[idx] = c;
             st_width[idx] = (int32_t)key_len(k_[p + c - 1]);  // rows ascending: the last row is the longest
             st_round[idx] = round;
-            st_origin[idx] = step_base + agorg[jb + k];
+            st_origin[idx] = step_base + V.ag[k];
             if (c <= 32) {
                 uint32_t sum = 0;  // count * max_len <= budget < 2^31, or a singleton
                 for (int j = 0; j < c; ++j) sum += key_len(k_[p + j]);
@@ -863,7 +891,7 @@ commit_body(const int r, const uint64_t *keys, const int64_t *rank_ptr, const in
                 st_count[idx] = c;
                 st_width[idx] = (int32_t)key_len(k_[p + c - 1]);
                 st_round[idx] = round;
-                st_origin[idx] = step_base + agorg[jb + k];
+                st_origin[idx] = step_base + V.ag[k];
                 ao[k] = cur + ex;
             }
             carry += tot;
@@ -895,11 +923,11 @@ commit_body(const int r, const uint64_t *keys, const int64_t *rank_ptr, const in
             S, s_scan, [&](int a) { return pf[a] == 0; }, [&](int a, int kidx) { lf[kidx] = key_id(k_[a]); });
     }
     if (threadIdx.x == 0) {
-        int nl_old = n_left[r], fp = fetch_pos[r];
+        int nl_old = *V.n_left, fp = *V.fetch_pos;
         int fp_new = fp + (S - nl_old);
-        emit_cur[r] = cur + emitted_r;
-        n_left[r] = n_left_new;
-        fetch_pos[r] = fp_new;
+        *V.emit_cur = cur + emitted_r;
+        *V.n_left = n_left_new;
+        *V.fetch_pos = fp_new;
         if (n_left_new + (n_r - fp_new) == 0) atomicAdd(&rec->n_finished, 1);
     }
 }
@@ -919,9 +947,27 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
          int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
          int32_t *fetch_pos, int32_t *emit_cur, const int32_t *__restrict__ emit_snap, RoundRec *rec, PlanDims *dims,
          unsigned int *done_ctr) {
-    commit_body(blockIdx.x, keys, rank_ptr, S_arr, G_arr, R, agpos, agcnt, agorg, agoff, step_samples, step_base, round,
-                join_mode, quota, emitted_before, st_count, st_width, st_real, st_round, st_origin, posflag, emit_ids,
-                emit_pos, left_ids, n_left, fetch_pos, emit_cur, emit_snap, rec, false, blockIdx.y, gridDim.y);
+    {
+        const int r = blockIdx.x;
+        RankView V;
+        V.base = rank_ptr[r];
+        const int64_t jb = V.base + r;
+        V.k = keys + V.base;
+        V.ap = agpos + jb;
+        V.ac = agcnt + jb;
+        V.ag = agorg + jb;
+        V.ao = agoff + jb;
+        V.pf = posflag + V.base;
+        V.S = S_arr[r];
+        V.Gr = G_arr[r];
+        V.cur = emit_snap[r];
+        V.n_r = (int)(rank_ptr[r + 1] - V.base);
+        V.n_left = n_left + r;
+        V.fetch_pos = fetch_pos + r;
+        V.emit_cur = emit_cur + r;
+        commit_body(r, R, V, step_samples, step_base, round, join_mode, quota, emitted_before, st_count, st_width, st_real,
+                    st_round, st_origin, emit_ids, emit_pos, left_ids, rec, false, blockIdx.y, gridDim.y);
+    }
     if (!dims) return;  // distributed mode: the host decides from the gathered status
     __shared__ int s_last;
     __syncthreads();
@@ -1004,25 +1050,28 @@ struct RoundsArgs {
     PlanDims *dims;
 };
 
+// dynamic shared memory of k_rounds: the sort buffer (also scratch of the list ranking and of the overflow
+// sort), the sorted window, and the round's group tables
+constexpr size_t kRoundsSmem = (size_t)kMsPadded * 8 + (size_t)kMsChunk * 8 + 4 * (size_t)(kMsChunk + 4) * 4;
+
 __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
-    extern __shared__ __align__(16) unsigned char rd_smem[];  // kMsPadded keys: sort buffer, then form / overflow scratch
+    extern __shared__ __align__(16) unsigned char rd_smem[];
     __shared__ int s_scan[34];
     __shared__ uint16_t s_e2[32];
     __shared__ int s_red[3];
+    __shared__ int s_state[3];  // n_left, fetch_pos, emit_cur of this rank
     __shared__ RoundRec s_rec;
-    uint64_t *X = reinterpret_cast<uint64_t *>(rd_smem);
+    uint64_t *X = reinterpret_cast<uint64_t *>(rd_smem);  // kMsPadded keys
+    uint64_t *K = X + kMsPadded;                          // the sorted window, kMsChunk keys
+    int32_t *s_gp = reinterpret_cast<int32_t *>(K + kMsChunk);
+    int32_t *s_ap = s_gp + (kMsChunk + 4), *s_ac = s_ap + (kMsChunk + 4), *s_ag = s_ac + (kMsChunk + 4);
     const int r = blockIdx.x, t = threadIdx.x, R = A.R;
     const SortArgs &SA = A.sort;
     ms_first_round_init(SA, (int64_t)r * kMsThreads + t, (int64_t)gridDim.x * kMsThreads);
     const int64_t base = SA.rank_ptr[r];
     const int n_r = (int)(SA.rank_ptr[r + 1] - base);
     const int64_t jb = base + r;
-    uint64_t *keys = SA.keys_out;
-    if (t == 0) {
-        SA.n_left[r] = 0;
-        SA.fetch_pos[r] = 0;
-        SA.emit_cur[r] = 0;
-    }
+    if (t < 3) s_state[t] = 0;
     __syncthreads();
     unsigned int n_bar = 0;
     int n_steps = 0, n_rounds = 0, stop = 0, bad = 0;
@@ -1030,7 +1079,7 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
     const bool quota_mode = !A.join_mode && A.quota > 0;
     for (int round = 0;; ++round) {
         // ---- A0 + A1: this rank's window, sorted ----
-        const int nl = SA.n_left[r], fp = SA.fetch_pos[r];
+        const int nl = s_state[0], fp = s_state[1], cur = s_state[2];
         const int S = ms_window_size(nl, fp, n_r, SA.buffer_size);
         int G = 0;
         if (S > 0) {
@@ -1038,16 +1087,14 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
             const int n_keys = ms_active_keys(S);
             ms_load_keys(SA, base, nl, fp, 0, S, n_keys, k);
             ms_sort_cta(k, X, n_keys);
-            for (int i = t; i < S; i += kMsThreads) keys[base + i] = X[ms_pad(i)];
+            for (int i = t; i < S; i += kMsThreads) K[i] = X[ms_pad(i)];
             __syncthreads();
             // ---- A2 + A3: candidate groups ----
-            G = form_hier_body(keys + base, S, A.budget, A.rule, A.gpos + jb, rd_smem, s_scan, s_e2);
+            G = form_hier_body(K, S, A.budget, A.rule, s_gp, rd_smem, s_scan, s_e2);
         }
         // ---- the exchange: (G_r, S_r), S_r = -1 for "finished" (nothing buffered, nothing pending) ----
         int32_t *gs = A.gs + (size_t)(round & 1) * 2 * R;
         if (t == 0) {
-            A.G[r] = G;
-            A.S[r] = S;
             __stcg(&gs[2 * r], G);
             __stcg(&gs[2 * r + 1], S == 0 ? -1 : S);
             s_red[0] = 0;
@@ -1080,10 +1127,7 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
             break;
         }
         // ---- A4 .. A6: align to T ----
-        if (G > 0) {
-            if (t == 0) A.emit_snap[r] = SA.emit_cur[r];
-            align_body(S, G, T, A.gpos + jb, A.agpos + jb, A.agcnt + jb, A.agorg + jb, X, SA.step_samples + n_steps);
-        }
+        if (G > 0) align_body(S, G, T, s_gp, s_ap, s_ac, s_ag, X, SA.step_samples + n_steps);
         if (quota_mode) grid_barrier(A.bar, (unsigned int)R * (++n_bar));  // the global step totals are complete
         if (t == 0) {
             s_rec.T = T;
@@ -1092,10 +1136,23 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
         }
         __syncthreads();
         // ---- A7 + A8a: commit ----
-        commit_body(r, keys, SA.rank_ptr, A.S, A.G, R, A.agpos, A.agcnt, A.agorg, A.agoff, SA.step_samples, n_steps, round,
-                    A.join_mode, A.quota, emitted_before, A.st_count, A.st_width, A.st_real, A.st_round, A.st_origin,
-                    A.posflag, A.emit_ids, SA.emit_pos, A.left_ids_w, SA.n_left, SA.fetch_pos, SA.emit_cur, A.emit_snap,
-                    &s_rec, true, 0, 1);
+        RankView V;
+        V.k = K;
+        V.ap = s_ap;
+        V.ac = s_ac;
+        V.ag = s_ag;
+        V.ao = A.agoff + jb;
+        V.pf = A.posflag + base;
+        V.S = S;
+        V.Gr = G;
+        V.cur = cur;
+        V.n_r = n_r;
+        V.base = base;
+        V.n_left = &s_state[0];
+        V.fetch_pos = &s_state[1];
+        V.emit_cur = &s_state[2];
+        commit_body(r, R, V, SA.step_samples, n_steps, round, A.join_mode, A.quota, emitted_before, A.st_count, A.st_width,
+                    A.st_real, A.st_round, A.st_origin, A.emit_ids, SA.emit_pos, A.left_ids_w, &s_rec, true, 0, 1);
         __syncthreads();
         n_steps += s_rec.T_emit;
         if (quota_mode) {
@@ -1108,13 +1165,18 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
         }
         __syncthreads();  // s_rec is rewritten next round
     }
-    if (r == 0 && t == 0) {
-        A.dims->n_steps = n_steps;
-        A.dims->n_rounds = n_rounds;
-        A.dims->stop_reason = stop;
-        A.dims->bad_length = bad == 1 ? 1 : 0;
-        A.dims->err = bad == 2 ? ODB_ERR_STATE : 0;
-        A.dims->complete = bad ? 0 : 1;
+    if (t == 0) {  // the rank's final state, for the kernels behind the round loop
+        SA.n_left[r] = s_state[0];
+        SA.fetch_pos[r] = s_state[1];
+        SA.emit_cur[r] = s_state[2];
+        if (r == 0) {
+            A.dims->n_steps = n_steps;
+            A.dims->n_rounds = n_rounds;
+            A.dims->stop_reason = stop;
+            A.dims->bad_length = bad == 1 ? 1 : 0;
+            A.dims->err = bad == 2 ? ODB_ERR_STATE : 0;
+            A.dims->complete = bad ? 0 : 1;
+        }
     }
 }
 
@@ -1447,9 +1509,11 @@ cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
 // all be resident on this device (the caller then drives the rounds from the host).
 cudaError_t launch_rounds(odb_ctx *c, cudaStream_t st) {
     const int R = c->prm.n_ranks;
-    const size_t smem = (size_t)kMsPadded * sizeof(uint64_t);
+    const size_t smem = kRoundsSmem;
     if (c->rounds_max_ctas == 0) {
         int occ = 0, coop = 0;
+        cudaError_t ae = cudaFuncSetAttribute(k_rounds, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ae != cudaSuccess) return ae;
         cudaError_t e = cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device);
         if (e != cudaSuccess) return e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_rounds, kMsThreads, smem);

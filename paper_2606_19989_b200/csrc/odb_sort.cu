@@ -65,7 +65,10 @@ __global__ void __launch_bounds__(kMsThreads) k_sort_window(const SortArgs A, in
         const int p0 = c & ~(2 * m - 1);  // first CTA of the pair of runs
         const int na = m * kMsChunk, nb = m * kMsChunk;
         const int d0 = (c - p0) * kMsChunk, d1 = d0 + kMsChunk;
-        if (t == 0 || t == 32) s_cut[t >> 5] = ms_path_remote(x_addr, p0, na, p0 + m, nb, t ? d1 : d0);
+        if (t < 64) {  // warp 0: the cut of the tile's first diagonal, warp 1: of its last
+            const int cut = ms_path_remote(x_addr, p0, na, p0 + m, nb, t < 32 ? d0 : d1);
+            if ((t & 31) == 0) s_cut[t >> 5] = cut;
+        }
         __syncthreads();
         const int a0 = s_cut[0], a1 = s_cut[1];
         const int b0 = d0 - a0, b1 = d1 - a1;

@@ -110,12 +110,16 @@ __device__ __forceinline__ void ms_sort_cta(uint64_t (&k)[kMsItems], uint64_t *X
             const int ai = ms_path_local(X, ps, w, ps + w, w, d);
             ms_merge_items(X, ps + ai, ps + w, ps + w + (d - ai), ps + 2 * w, k);
         }
-        __syncthreads();  // every read of this level is done
+        // (while a pair of runs lies inside one warp's 32 * kMsItems keys, the warp's own barrier is enough)
+        const bool in_warp = 2 * w <= 32 * kMsItems;
+        if (in_warp) __syncwarp();
+        else __syncthreads();  // every read of this level is done
         if (active) {
 #pragma unroll
             for (int q = 0; q < kMsItems; ++q) X[ms_pad(o + q)] = k[q];
         }
-        __syncthreads();
+        if (in_warp && 4 * w <= 32 * kMsItems) __syncwarp();
+        else __syncthreads();
     }
 }
 
@@ -124,12 +128,20 @@ __device__ __forceinline__ uint64_t ms_run_key(uint32_t x_addr, int cta0, int i)
     return ld_dsmem_u64(cluster_map(x_addr + 8u * (uint32_t)ms_pad(i & (kMsChunk - 1)), (uint32_t)(cta0 + (i >> 12))));
 }
 
+// Merge-path cut over DSMEM by ONE WARP: 32 probes per round split [lo, hi) into 33 parts (the predicate
+// "a[mid] < b[d - 1 - mid]" is true below the answer and false from it on), so runs of 32768 keys need three
+// rounds of two remote loads instead of fifteen dependent ones.  All 32 lanes must call it; all return the cut.
 __device__ __forceinline__ int ms_path_remote(uint32_t x_addr, int ctaA, int na, int ctaB, int nb, int d) {
+    const int lane = threadIdx.x & 31;
     int lo = max(0, d - nb), hi = min(d, na);
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if (ms_run_key(x_addr, ctaA, mid) < ms_run_key(x_addr, ctaB, d - 1 - mid)) lo = mid + 1;
-        else hi = mid;
+    while (lo < hi) {  // warp-uniform
+        const int mid = lo + (int)(((long long)(hi - lo) * (lane + 1)) / 33);  // in [lo, hi), non-decreasing in lane
+        const bool below = ms_run_key(x_addr, ctaA, mid) < ms_run_key(x_addr, ctaB, d - 1 - mid);
+        const int p = __popc(__ballot_sync(ODB_FULL_MASK, below));  // the probes below the answer are the first p lanes
+        const int lo_n = __shfl_sync(ODB_FULL_MASK, mid, max(p - 1, 0)) + 1;
+        const int hi_n = __shfl_sync(ODB_FULL_MASK, mid, min(p, 31));
+        if (p > 0) lo = lo_n;
+        if (p < 32) hi = hi_n;
     }
     return lo;
 }
