@@ -61,6 +61,9 @@ def parse_args():
     ap.add_argument("--shard-ranks", action="store_true",
                     help="SURVEY.md 8(f) F1: split the job's virtual ranks over the N GPUs (strong scaling; per-round "
                          "all_gather + all_reduce over NCCL) instead of N independent replicas")
+    ap.add_argument("--pipeline", type=int, default=0,
+                    help="measure N contexts driven round-robin on N streams (planning of one step beside the collate "
+                         "kernel of another); extra key 'pipelined'")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -427,6 +430,32 @@ def run_ours(args):
             "clocks": clocks,
         }
         result["stage_ms"]["planning_share"] = plan_ms / ms
+        if not args.no_sweep and world == 1:
+            # the store-side ceiling for this kernel's byte mix, and the bulk-store form of the kernel beside the adopted one
+            del out
+            torch.cuda.empty_cache()
+            mc = mix_ceiling(P, device)
+            best = max(mc["mix_stg256"], mc["mix_bulk_store"])
+            result["roofline"]["mix_ceiling"] = mc
+            result["roofline"]["mix_ceiling_gbs"] = best
+            result["roofline"]["frac_of_mix_ceiling"] = achieved / best
+            out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
+            P.odb_set_option(ctx.h, P.ODB_OPT_COLLATE_BULK_STORES, 1)
+            _, col_b, _, _, _, _ = time_device(P, ctx, wl, din, out, 5, 3, barrier)
+            P.odb_set_option(ctx.h, P.ODB_OPT_COLLATE_BULK_STORES, 0)
+            result["roofline"]["bulk_store_variant"] = {"kernel_ms": col_b, "achieved": abytes / (col_b * 1e-3) / 1e9,
+                                                        "vs_adopted": col_b / col_ms_max,
+                                                        "note": "k_collate<., BULK=true>: interior chunks staged in shared "
+                                                                "memory, cp.async.bulk stores; not adopted unless faster"}
+        if args.pipeline > 1 and world == 1:
+            del out
+            torch.cuda.empty_cache()
+            pms = time_pipelined(P, wl, device, args.pipeline, args.steps, args.warmup)
+            result["pipelined"] = {"contexts": args.pipeline, "ms_per_step": pms, "vs_single_context": pms / ms,
+                                   "samples_per_s": n_samples / (pms * 1e-3),
+                                   "hbm_gbs_whole_step": abytes / (pms * 1e-3) / 1e9,
+                                   "whole_step_frac": abytes / (pms * 1e-3) / 1e9 / peak}
+            out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
         result["launches_per_step"] = launches
         if not args.no_sweep and world == 1:
             rows = run_sweep(P, args, device, peak)
@@ -573,6 +602,77 @@ def run_sharded(args):
                          "traffic": None, "kernel": "k_collate (rank 0's share)", "algorithmic_bytes": ab_local,
                          "kernel_ms": col_ms, "peak_source": peak_src},
             "gpu_launches": int(launches), "clocks": clocks, "e2e": None, "cpu_baseline": None}), flush=True)
+
+
+def time_pipelined(P, wl, device, n_ctx, steps, warmup):
+    """n_ctx contexts (own scratch, own outputs, own stream), the same resident inputs, odb_run called round-robin:
+    while one context's collate kernel runs, the next context's planning kernels are already enqueued on another
+    stream (odb_run returns as soon as the plan sizes are known).  Device time per step over all contexts."""
+    import torch
+    local = int(device.split(":")[1])
+    din = DeviceInputs(wl, device, P)
+    ctxs, outs, streams = [], [], []
+    try:
+        for i in range(n_ctx):
+            c = P.Odb(gpu_params(P, wl), max(wl.n_samples, 1), device=local)
+            info = c.plan(din.lengths, wl.rank_ptr)
+            ctxs.append(c)
+            outs.append(P.OutputBuffers.for_plan(wl.n_ranks, info, device))
+            streams.append(torch.cuda.Stream(device=device))
+        torch.cuda.synchronize()
+
+        def one(i):
+            with torch.cuda.stream(streams[i]):
+                return P.odb_run(ctxs[i].h, din.lengths, wl.rank_ptr, din.tokens, din.sample_ptr, din.span_ptr, din.span_lo,
+                                 din.span_hi, outs[i].struct, stream=streams[i])
+
+        for k in range(warmup * n_ctx):
+            one(k % n_ctx)
+        torch.cuda.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for s_ in streams:
+            s_.wait_event(ev0)
+        for k in range(steps * n_ctx):
+            one(k % n_ctx)
+        cur = torch.cuda.current_stream()
+        for s_ in streams:
+            cur.wait_stream(s_)
+        ev1.record()
+        torch.cuda.synchronize()
+        return ev0.elapsed_time(ev1) / (steps * n_ctx)
+    finally:
+        for c in ctxs:
+            c.close()
+        del outs, din
+        torch.cuda.empty_cache()
+
+
+def mix_ceiling(P, device, n_elems=1 << 29):
+    """What the collate kernel's byte mix (4 B read + 13 B written per element) reaches with trivial indexing on this
+    device, in the two store forms the kernel can use, next to a pure-store stream and a copy (odb_probe_bandwidth)."""
+    import torch
+    src = torch.empty(n_elems, dtype=torch.int32, device=device)
+    o = [torch.empty(n_elems, dtype=torch.int32, device=device) for _ in range(3)]
+    m = torch.empty(n_elems, dtype=torch.uint8, device=device)
+    src.zero_()
+    names = {0: "mix_stg256", 1: "mix_bulk_store", 2: "store_only_stg256", 3: "store_only_bulk_store", 4: "copy_4r_4w"}
+    bytes_per = {0: 17, 1: 17, 2: 13, 3: 13, 4: 8}
+    out = {"n_elems": n_elems, "unit": "GB/s"}
+    for kind, name in names.items():
+        ms = P.odb_probe_bandwidth(kind, src, o[0], o[1], o[2], m, n_elems, reps=5)
+        out[name] = bytes_per[kind] * n_elems / (ms * 1e-3) / 1e9
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    o[0].zero_()
+    ev0.record()
+    for _ in range(5):
+        o[0].zero_()
+    ev1.record()
+    torch.cuda.synchronize()
+    out["memset_torch_zero"] = 5 * 4 * n_elems / (ev0.elapsed_time(ev1) * 1e-3) / 1e9
+    del src, o, m
+    torch.cuda.empty_cache()
+    return out
 
 
 def cell_key(config, cv, budget, rule, buffer_size=0):

@@ -256,6 +256,23 @@ ODB_API int odb_get_timing(odb_ctx *ctx, float *ms3);
  * the last 64 runs are kept, so a benchmark can enqueue many runs back to back and read their stage times
  * afterwards instead of waiting on every run.  ODB_ERR_STATE if that run does not exist (any more). */
 ODB_API int odb_get_timing_at(odb_ctx *ctx, int back, float *ms3);
+/* Tuning / measurement switches.  ODB_OPT_COLLATE_BULK_STORES (value 0 / 1, default 0): the collate kernel stages
+ * the interior chunks of each arena in shared memory and stores them with bulk asynchronous copies
+ * (cp.async.bulk.global.shared::cta, the store side of BASELINE.json's "TMA bulk copies") instead of 256-bit
+ * streaming stores from registers.  Same results bit for bit; the measured comparison is in profiles/.
+ * ODB_ERR_INVALID_ARG for an unknown option. */
+enum { ODB_OPT_COLLATE_BULK_STORES = 1 };
+ODB_API int odb_set_option(odb_ctx *ctx, int option, int64_t value);
+
+/* Bandwidth probes (measurement utility, not part of the method): the collate kernel's byte mix -- 4 bytes read
+ * and 13 written per element -- with trivial indexing.  kind 0: the mix with 256-bit streaming stores; 1: the mix
+ * with bulk stores from shared memory; 2 / 3: the 13 bytes of stores alone in the two forms; 4: a copy (4 bytes
+ * read, 4 written).  d_in: n_elems int32 (kinds 0, 1, 4); d_out0..2: n_elems int32, d_out3: n_elems bytes (kind 4
+ * writes d_out0 only); all 16-byte aligned; n_elems is rounded down to a multiple of 512.  Runs 1 + reps launches
+ * on `stream` and writes the average milliseconds per launch to *h_ms.  Synchronises. */
+ODB_API int odb_probe_bandwidth(int kind, const int32_t *d_in, int32_t *d_out0, int32_t *d_out1, int32_t *d_out2,
+                                uint8_t *d_out3, int64_t n_elems, int reps, void *stream, float *h_ms);
+
 /* Number of kernels this context has launched since odb_create (diagnostics / bench accounting). */
 ODB_API int64_t odb_kernel_launches(const odb_ctx *ctx);
 

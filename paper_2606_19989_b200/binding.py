@@ -96,6 +96,8 @@ SYMBOLS = {
     "odb_set_timing": (_i32, [_vp, _i32]),
     "odb_get_timing": (_i32, [_vp, _P(ctypes.c_float)]),
     "odb_get_timing_at": (_i32, [_vp, _i32, _P(ctypes.c_float)]),
+    "odb_set_option": (_i32, [_vp, _i32, _i64]),
+    "odb_probe_bandwidth": (_i32, [_i32, _vp, _vp, _vp, _vp, _vp, _i64, _i32, _vp, _P(ctypes.c_float)]),
     "odb_kernel_launches": (_i64, [_vp]),
     "odb_debug_read": (_i64, [_vp, _i32, _vp, _i64]),
     "odb_synth_tokens": (_i32, [_vp, _i64, _i64, ctypes.c_uint64, _i32, _vp]),
@@ -312,6 +314,21 @@ def odb_get_timing_at(ctx: int, back: int):
     ms = (ctypes.c_float * 3)()
     _check(load().odb_get_timing_at(ctx, int(back), ms), "odb_get_timing_at", ctx)
     return float(ms[0]), float(ms[1]), float(ms[2])
+
+
+ODB_OPT_COLLATE_BULK_STORES = 1
+
+
+def odb_set_option(ctx: int, option: int, value: int) -> None:
+    _check(load().odb_set_option(ctx, int(option), int(value)), "odb_set_option", ctx)
+
+
+def odb_probe_bandwidth(kind: int, d_in, d_out0, d_out1, d_out2, d_out3, n_elems: int, reps: int = 5, stream=None) -> float:
+    """Average milliseconds per launch of bandwidth probe ``kind`` (include/odb.h)."""
+    ms = ctypes.c_float(0.0)
+    _check(load().odb_probe_bandwidth(int(kind), _ptr(d_in), _ptr(d_out0), _ptr(d_out1), _ptr(d_out2), _ptr(d_out3),
+                                      int(n_elems), int(reps), _stream(stream), ctypes.byref(ms)), "odb_probe_bandwidth")
+    return float(ms.value)
 
 
 def odb_kernel_launches(ctx: int) -> int:

@@ -245,6 +245,14 @@ int odb_reset(odb_ctx *c) {
     return ODB_OK;
 }
 
+int odb_set_option(odb_ctx *c, int option, int64_t value) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    switch (option) {
+    case ODB_OPT_COLLATE_BULK_STORES: c->collate_bulk = value != 0; return ODB_OK;
+    default: return ODB_ERR_INVALID_ARG;
+    }
+}
+
 int odb_set_timing(odb_ctx *c, int enable) {
     if (!c) return ODB_ERR_INVALID_ARG;
     if (enable && c->evring.empty()) {

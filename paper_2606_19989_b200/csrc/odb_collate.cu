@@ -319,11 +319,38 @@ __device__ __forceinline__ void emit_vector(const CollateArgs &A, const RowRegs 
     mword = spread4((1u << nreal) - 1u);
 }
 
+// ---- bulk (TMA) stores from shared memory: the alternative store form of the interior chunks ----
+constexpr int kColStage = 3 * kColChunk * 4 + kColChunk;  // one warp's staging buffer: ids | labels | pos | mask
+__device__ __forceinline__ void bulk_store(void *gdst, const void *ssrc, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst),
+                 "r"((uint32_t)__cvta_generic_to_shared(ssrc)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// 16 consecutive int32 of a unit: two 256-bit streaming stores to the arena, or four 16-byte stores to the
+// warp's staging buffer
+template <bool BULK>
+__device__ __forceinline__ void put16(int32_t *p, const int32_t (&o)[16]) {
+    if (BULK) {
+        int4 *q = reinterpret_cast<int4 *>(p);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) q[i] = make_int4(o[4 * i], o[4 * i + 1], o[4 * i + 2], o[4 * i + 3]);
+    } else {
+        st256(p, o, 0);
+        st256(p + 8, o, 8);
+    }
+}
+
 // Interior chunks: a 16-element unit inside one row from the 17 tokens x[0..16] = tokens t .. t+16
-// (anything beyond the sample).  Returns the 16 mask bytes.
-template <bool SHIFT>
+// (anything beyond the sample), written at d_ids / d_lab / d_pos (the arenas, or the staging buffer).
+// Returns the 16 mask bytes.
+template <bool SHIFT, bool BULK>
 __device__ __forceinline__ int4 emit_unit(const CollateArgs &A, const RowRegs &r, int64_t q, int t, const int32_t (&x)[17],
-                                          int64_t a, int &acc) {
+                                          int32_t *d_ids, int32_t *d_lab, int32_t *d_pos, int &acc) {
     const int nreal = clamp0<16>(r.len - t);  // elements t .. t+15 that are real tokens
     const uint32_t real = (1u << nreal) - 1u;
     uint32_t ok;  // elements whose label carries a loss term
@@ -339,13 +366,11 @@ __device__ __forceinline__ int4 emit_unit(const CollateArgs &A, const RowRegs &r
 #pragma unroll
         for (int j = 0; j < 16; ++j) o[j] = j < nreal ? x[j] : A.pad_id;
     }
-    st256(A.ids + a, o, 0);
-    st256(A.ids + a + 8, o, 8);
+    put16<BULK>(d_ids, o);
     // position_ids
 #pragma unroll
     for (int j = 0; j < 16; ++j) o[j] = j < nreal ? t + j : 0;
-    st256(A.pos + a, o, 0);
-    st256(A.pos + a + 8, o, 8);
+    put16<BULK>(d_pos, o);
     // labels
     if (ok == 0xFFFFu) {
 #pragma unroll
@@ -357,15 +382,22 @@ __device__ __forceinline__ int4 emit_unit(const CollateArgs &A, const RowRegs &r
 #pragma unroll
         for (int j = 0; j < 16; ++j) o[j] = ((ok >> j) & 1u) ? x[j + (SHIFT ? 1 : 0)] : A.ignore_index;
     }
-    st256(A.labels + a, o, 0);
-    st256(A.labels + a + 8, o, 8);
+    put16<BULK>(d_lab, o);
     return make_int4((int)spread4(real), (int)spread4(real >> 4), (int)spread4(real >> 8), (int)spread4(real >> 12));
 }
 
-template <bool SHIFT>
+// BULK = false: the interior chunks leave the registers with 256-bit streaming stores (the adopted form);
+// BULK = true: they are staged in shared memory (one 6.5 KB buffer per warp) and leave with four bulk (TMA)
+// stores per chunk, one per arena (BASELINE.json's sketch of the store side; measured in profiles/r02_*).
+template <bool SHIFT, bool BULK>
 __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A) {
+    extern __shared__ __align__(128) unsigned char col_smem[];
     __shared__ long long s_grab;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // this warp's staging buffer (BULK only)
+    int32_t *const s_ids = reinterpret_cast<int32_t *>(col_smem + (BULK ? (size_t)warp * kColStage : 0));
+    int32_t *const s_lab = s_ids + kColChunk, *const s_pos = s_lab + kColChunk;
+    uint8_t *const s_msk = reinterpret_cast<uint8_t *>(s_pos + kColChunk);
     constexpr int kWarps = kColThreads / 32;
     static_assert(kColChunk == 512 && kColTile == kWarps * kColChunk, "a chunk is one 16-element unit per lane");
     const int4 *tok4 = reinterpret_cast<const int4 *>(A.tokens);
@@ -436,6 +468,10 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
                 const int64_t qv = g >> 2;              // aligned vector that holds it
                 const int64_t send = r.tok + r.len;     // one past the sample's last token
                 const bool ld = fast && t < r.len;
+                if (BULK) {  // the previous chunk's bulk stores have read the staging buffer
+                    if (lane == 0) bulk_wait_read();
+                    __syncwarp();
+                }
                 int4 v[4];
 #pragma unroll
                 for (int i = 0; i < 4; ++i)
@@ -461,10 +497,16 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
                         const RowRegs rr = load_row(A.rows, qq);
                         int32_t id, lb, ps;
                         one_element<SHIFT>(A, rr, qq, c, id, lb, ps, m);
-                        const int64_t aa = a0 + 16 * src + j;
-                        A.ids[aa] = id;
-                        A.labels[aa] = lb;
-                        A.pos[aa] = ps;
+                        if (BULK) {
+                            s_ids[16 * src + j] = id;
+                            s_lab[16 * src + j] = lb;
+                            s_pos[16 * src + j] = ps;
+                        } else {
+                            const int64_t aa = a0 + 16 * src + j;
+                            A.ids[aa] = id;
+                            A.labels[aa] = lb;
+                            A.pos[aa] = ps;
+                        }
                         acc += (lb != A.ignore_index) ? 1 : 0;
                         m <<= 8 * (j & 3);
                     }
@@ -511,9 +553,24 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
                         for (int j = 0; j < 17; ++j) x[j] = w[j + 3];
                         break;
                     }
-                    mv = emit_unit<SHIFT>(A, r, (int64_t)q, t, x, a0 + 16 * lane, acc);
+                    if (BULK) mv = emit_unit<SHIFT, true>(A, r, (int64_t)q, t, x, s_ids + 16 * lane, s_lab + 16 * lane, s_pos + 16 * lane, acc);
+                    else mv = emit_unit<SHIFT, false>(A, r, (int64_t)q, t, x, A.ids + a0 + 16 * lane, A.labels + a0 + 16 * lane,
+                                                      A.pos + a0 + 16 * lane, acc);
                 }
-                __stcs(reinterpret_cast<int4 *>(A.mask + a0 + 16 * lane), mv);
+                if (BULK) {
+                    reinterpret_cast<int4 *>(s_msk)[lane] = mv;
+                    fence_async_smem();  // the generic-proxy writes above, before the async proxy reads them
+                    __syncwarp();
+                    if (lane == 0) {
+                        bulk_store(A.ids + a0, s_ids, kColChunk * 4);
+                        bulk_store(A.labels + a0, s_lab, kColChunk * 4);
+                        bulk_store(A.pos + a0, s_pos, kColChunk * 4);
+                        bulk_store(A.mask + a0, s_msk, kColChunk);
+                        bulk_commit();
+                    }
+                } else {
+                    __stcs(reinterpret_cast<int4 *>(A.mask + a0 + 16 * lane), mv);
+                }
                 const int tot = __reduce_add_sync(ODB_FULL_MASK, acc);
                 if (lane == 0 && tot != 0) atomicAdd(&A.grp_valid[s], tot);
             } else {
@@ -570,6 +627,10 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
                 if (acc) atomicAdd(&A.grp_valid[acc_slot], acc);
             }
         }
+    }
+    if (BULK) {  // the staging buffers must outlive the bulk stores that read them
+        if (lane == 0) bulk_wait_all();
+        __syncwarp();
     }
 }
 
@@ -659,23 +720,33 @@ cudaError_t launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *
     return cudaSuccess;
 }
 
-cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st) {
-    const int sh = args.shift_labels ? 1 : 0;
-    if (c->col_occ[sh] == 0) {
-        cudaError_t e = sh ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->col_occ[sh], k_collate<true>, kColThreads, 0)
-                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->col_occ[sh], k_collate<false>, kColThreads, 0);
+template <bool SHIFT, bool BULK>
+static cudaError_t launch_collate_t(odb_ctx *c, const CollateArgs &args, cudaStream_t st) {
+    const int v = (SHIFT ? 1 : 0) + (BULK ? 2 : 0);
+    const size_t smem = BULK ? (size_t)(kColThreads / 32) * kColStage : 0;
+    if (c->col_occ[v] == 0) {
+        if (BULK) {
+            cudaError_t e = cudaFuncSetAttribute(k_collate<SHIFT, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->col_occ[v], k_collate<SHIFT, BULK>, kColThreads, smem);
         if (e != cudaSuccess) return e;
-        if (c->col_occ[sh] < 1) c->col_occ[sh] = 1;
+        if (c->col_occ[v] < 1) c->col_occ[v] = 1;
     }
     // tiles the launch can have to visit: known for a ranged launch, bounded by the caller's arena otherwise
     const int64_t n_tiles = args.tile_hi - args.tile_lo;
     if (n_tiles <= 0 && !args.whole) return cudaSuccess;
-    int blocks = (int)std::min<int64_t>(std::max<int64_t>((n_tiles + kColGrab - 1) / kColGrab, 1),
-                                        (int64_t)c->sm_count * c->col_occ[sh]);
-    if (sh) k_collate<true><<<blocks, kColThreads, 0, st>>>(args);
-    else k_collate<false><<<blocks, kColThreads, 0, st>>>(args);
+    const int blocks = (int)std::min<int64_t>(std::max<int64_t>((n_tiles + kColGrab - 1) / kColGrab, 1),
+                                              (int64_t)c->sm_count * c->col_occ[v]);
+    k_collate<SHIFT, BULK><<<blocks, kColThreads, smem, st>>>(args);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
+}
+
+cudaError_t launch_collate(odb_ctx *c, const CollateArgs &args, cudaStream_t st) {
+    const bool sh = args.shift_labels != 0;
+    if (c->collate_bulk) return sh ? launch_collate_t<true, true>(c, args, st) : launch_collate_t<false, true>(c, args, st);
+    return sh ? launch_collate_t<true, false>(c, args, st) : launch_collate_t<false, false>(c, args, st);
 }
 
 cudaError_t launch_post(odb_ctx *c, const PostArgs &args, cudaStream_t st) {

@@ -44,13 +44,15 @@ def gpu_params(wl):
                          ignore_index=p["ignore_index"], shift_labels=p["shift_labels"])
 
 
-def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL, avail_schedule=None):
+def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL, avail_schedule=None, bulk_stores=False):
     """Returns (info, OutputBuffers, round_T).  staged=True uses form_groups/align/round_status/
     plan_query/collate; staged=False uses odb_run (two calls: the first sizes the outputs)."""
     import torch
     import paper_2606_19989_b200 as P
     dw = dw or DeviceWorkload(wl)
     with P.Odb(gpu_params(wl), max(wl.n_samples, 1)) as ctx:
+        if bulk_stores:
+            P.odb_set_option(ctx.h, P.ODB_OPT_COLLATE_BULK_STORES, 1)
         if staged:
             info = ctx.plan(dw.lengths, wl.rank_ptr, avail_schedule=avail_schedule)
             round_T = list(ctx.round_T)

@@ -251,6 +251,45 @@ def test_round_loop_kernel_windows(P, oracle, buffer_size, slot_capacity):
         Par.compare_plan(plan, info2, out2)
 
 
+@pytest.mark.parametrize("staged", [True, False])
+def test_collate_bulk_store_variant(P, oracle, staged):
+    """ODB_OPT_COLLATE_BULK_STORES: the interior chunks leave through shared memory and bulk asynchronous stores
+    instead of 256-bit register stores -- the same bytes (configs[1], configs[2] in both label modes, the
+    many-span path, fuzz)."""
+    for wl in (I.make_workload(1), I.make_workload(2), I.make_workload(2, rule=1), I.protocol_workload("unequal", 4)):
+        for shift in (1, 0):
+            wl.params["shift_labels"] = shift
+            plan, ref = oracle.run_workload(wl)
+            info, out, _ = Par.run_gpu(wl, staged=staged, bulk_stores=True)
+            Par.compare_plan(plan, info, out)
+            Par.compare_full(plan, ref, info, out)
+    for seed in range(60):
+        wl, sched = Par.wide_fuzz_case(seed)
+        plan, ref = oracle.run_workload(wl)
+        info, out, _ = Par.run_gpu(wl, staged=staged, bulk_stores=True)
+        Par.compare_plan(plan, info, out)
+        Par.compare_full(plan, ref, info, out)
+
+
+def test_bandwidth_probes_run(P):
+    """The mix-ceiling probes of bench.py: every kind runs, and the stores land where they should."""
+    import torch
+    n = 1 << 22
+    src = torch.arange(n, dtype=torch.int32, device="cuda:0")
+    o = [torch.full((n,), -1, dtype=torch.int32, device="cuda:0") for _ in range(3)]
+    m = torch.full((n,), 7, dtype=torch.uint8, device="cuda:0")
+    for kind in range(5):
+        for t in o:
+            t.fill_(-1)
+        ms = P.odb_probe_bandwidth(kind, src, o[0], o[1], o[2], m, n, reps=2)
+        torch.cuda.synchronize()
+        assert ms > 0
+        if kind in (0, 1, 4):
+            assert torch.equal(o[0], src)
+        if kind in (0, 1):
+            assert torch.equal(o[1], src ^ 0x55)
+
+
 def test_heavy_split_unequal_group_counts(P, oracle):
     """One rank forms thousands of groups, another a handful of big ones: the split closed form turns
     thousands of rows of a few groups into singletons (Alg. 1)."""
