@@ -31,14 +31,27 @@ __device__ __forceinline__ void pb_fence_async() { asm volatile("fence.proxy.asy
 template <int KIND>
 __global__ void __launch_bounds__(kPbThreads, 3)
 k_probe(const int32_t *__restrict__ in, int32_t *__restrict__ o0, int32_t *__restrict__ o1, int32_t *__restrict__ o2,
-        uint8_t *__restrict__ o3, int64_t n_chunks) {
+        uint8_t *__restrict__ o3, int64_t n_chunks, unsigned long long *counter) {
     extern __shared__ __align__(128) unsigned char pb_smem[];
     constexpr bool kBulk = (KIND == 1 || KIND == 3);
     constexpr bool kRead = (KIND == 0 || KIND == 1 || KIND == 4);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t warps = (int64_t)gridDim.x * (kPbThreads / 32);
     unsigned char *stage = pb_smem + (size_t)warp * kPbStage;
-    for (int64_t c = (int64_t)blockIdx.x * (kPbThreads / 32) + warp; c < n_chunks; c += warps) {
+    // the work distribution of k_collate: persistent CTAs take runs of 16 tiles (8 chunks each) from a counter
+    __shared__ long long s_grab;
+    constexpr int kWarps = kPbThreads / 32, kGrab = 16;
+    const int64_t n_tiles = (n_chunks + kWarps - 1) / kWarps;
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_grab = (long long)atomicAdd(counter, (unsigned long long)kGrab);
+        __syncthreads();
+        const int64_t t0 = s_grab;
+        if (t0 >= n_tiles) break;
+        const int64_t t1 = min(t0 + kGrab, n_tiles);
+#pragma unroll 1
+    for (int64_t tile = t0; tile < t1; ++tile) {
+        const int64_t c = tile * kWarps + warp;
+        if (c >= n_chunks) break;
         const int64_t a = c * kPbChunk + 16 * lane;
         int32_t x[16];
         if (kRead) {
@@ -100,6 +113,7 @@ k_probe(const int32_t *__restrict__ in, int32_t *__restrict__ o0, int32_t *__res
         }
         }
     }
+    }
     if (kBulk) {
         if (lane == 0) pb_bulk_wait_all();
         __syncwarp();
@@ -108,14 +122,16 @@ k_probe(const int32_t *__restrict__ in, int32_t *__restrict__ o0, int32_t *__res
 
 template <int KIND>
 static cudaError_t run_probe(const int32_t *in, int32_t *o0, int32_t *o1, int32_t *o2, uint8_t *o3, int64_t n_chunks,
-                             int blocks, cudaStream_t st) {
+                             int blocks, unsigned long long *counter, cudaStream_t st) {
     constexpr bool kBulk = (KIND == 1 || KIND == 3);
     const size_t smem = kBulk ? (size_t)(kPbThreads / 32) * kPbStage : 0;
     if (kBulk) {
         cudaError_t e = cudaFuncSetAttribute(k_probe<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    k_probe<KIND><<<blocks, kPbThreads, smem, st>>>(in, o0, o1, o2, o3, n_chunks);
+    cudaError_t e = cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    k_probe<KIND><<<blocks, kPbThreads, smem, st>>>(in, o0, o1, o2, o3, n_chunks, counter);
     return cudaGetLastError();
 }
 
@@ -135,18 +151,20 @@ extern "C" int odb_probe_bandwidth(int kind, const int32_t *d_in, int32_t *d_out
     if (cudaGetDevice(&dev) != cudaSuccess) return ODB_ERR_CUDA;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const int64_t n_chunks = n_elems / kPbChunk;
-    const int blocks = (int)std::min<int64_t>((n_chunks + 7) / 8, (int64_t)sms * 3);
+    const int blocks = (int)std::min<int64_t>((n_chunks + 127) / 128, (int64_t)sms * 3);
     cudaEvent_t e0, e1;
+    unsigned long long *counter = nullptr;
+    if (cudaMalloc((void **)&counter, sizeof(unsigned long long)) != cudaSuccess) return ODB_ERR_CUDA;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return ODB_ERR_CUDA;
     cudaError_t e = cudaSuccess;
     for (int i = 0; i <= reps && e == cudaSuccess; ++i) {  // rep 0 is a warm-up
         if (i == 1) cudaEventRecord(e0, st);
         switch (kind) {
-        case 0: e = run_probe<0>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, st); break;
-        case 1: e = run_probe<1>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, st); break;
-        case 2: e = run_probe<2>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, st); break;
-        case 3: e = run_probe<3>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, st); break;
-        default: e = run_probe<4>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, st); break;
+        case 0: e = run_probe<0>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, counter, st); break;
+        case 1: e = run_probe<1>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, counter, st); break;
+        case 2: e = run_probe<2>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, counter, st); break;
+        case 3: e = run_probe<3>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, counter, st); break;
+        default: e = run_probe<4>(d_in, d_out0, d_out1, d_out2, d_out3, n_chunks, blocks, counter, st); break;
         }
     }
     cudaEventRecord(e1, st);
@@ -155,6 +173,7 @@ extern "C" int odb_probe_bandwidth(int kind, const int32_t *d_in, int32_t *d_out
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
+    cudaFree(counter);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
         return ODB_ERR_CUDA;
