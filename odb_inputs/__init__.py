@@ -19,4 +19,5 @@ from .gen import (  # noqa: F401
     tokens_for_samples,
     describe,
     split_ranks,
+    offline_workload,
 )

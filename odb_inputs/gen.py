@@ -335,6 +335,20 @@ def custom_workload(name: str, per_rank_lengths, seed: int = 0, **params) -> Wor
     return _assemble(name, per, spans, 9000 + seed, params)
 
 
+def offline_workload(n_ranks: int, seed: int = 0, *, n: int = 4096, mean: float = 512.0, cv: float = 1.0,
+                     budget: int = 16384) -> Workload:
+    """A GLOBAL pool of n samples for the offline comparators (F4: GMT / BMT / HFG): one
+    length array for the whole job (rank_ptr = [0, n]) plus the random draws those planners consume, as inputs:
+    ``perm`` (the epoch-seeded shuffle) and ``shuffle_key`` (one 31-bit key per potential batch)."""
+    rng = np.random.default_rng(5000 + seed)
+    lens = np.maximum(np.rint(_lognormal(rng, mean, cv, n)), 1).astype(np.int64)
+    wl = _assemble("offline_pool", [lens], [_prompt_only(rng, lens)], 11000 + seed, dict(budget=budget, rule=1))
+    wl.perm = rng.permutation(n).astype(np.int32)
+    wl.shuffle_key = rng.integers(0, 2**31 - 1, max(n, 1)).astype(np.int32)
+    wl.world = int(n_ranks)
+    return wl
+
+
 def split_ranks(wl: Workload, n_parts: int):
     """The same job held by ``n_parts`` processes: part p gets the consecutive ranks
     [p*R/n_parts, (p+1)*R/n_parts) with their samples, spans and (same hash indices) tokens.  Pure slicing."""

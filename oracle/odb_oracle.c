@@ -763,3 +763,181 @@ void oracle_collate_range(const oracle_plan *p, int64_t slot_lo, int64_t slot_hi
         if (grp_valid_tokens) grp_valid_tokens[s - slot_lo] = (int32_t)v;
     }
 }
+
+/* ========================================================================================= */
+/* the paper's OFFLINE comparators as planners (App. I; App. J).
+ * They see a GLOBAL scalar length array (the "oracle cache"), build one global batch list that every rank
+ * computes identically, and hand batches to the W ranks by striding; a slot's ids are therefore GLOBAL
+ * sample ids (the plan's rank_ptr is all zeros).  Random numbers are inputs: `perm` (the epoch-seeded
+ * shuffle, a permutation of 0..N-1) and `shuffle_key` (one non-negative key per potential batch index; the
+ * batch shuffle orders batches by (key, index)).
+ *
+ *   GMT (planner 0): "ascending-length sort plus greedy packing against a max-token budget", feasibility on
+ *       padded area max_i l_i * |b| <= budget, "singleton overflows allowed".
+ *   BMT (planner 1): "epoch-seeded shuffle, sample-count buckets, within-bucket length sort, greedy packing,
+ *       then batch shuffle".  Readings (U30): a bucket = `size` consecutive entries of the
+ *       shuffled order (the last one ragged); the within-bucket sort is ascending by (length, position in the
+ *       shuffled order); packing never crosses a bucket boundary.
+ *   both: "The list is then padded to a multiple of the world size by wrap-around repetition of the leading
+ *       batches and assigned to ranks by striding": G batches -> n_steps = ceil(G / W), slot (r, k) =
+ *       batch (k W + r) mod G.
+ *   HFG (planner 2): "samples a random permutation, partitions it into megabatches, sorts each megabatch by the
+ *       oracle post-tokenization length, concatenates the megabatches, pads the index list to a multiple of
+ *       world size, and stride-shards it across ranks ... keeps a fixed batch size".  Readings (U31):
+ *       the megabatch sort is DESCENDING (the HuggingFace group_by_length convention the paper names), ties by
+ *       descending position in the permutation (= the reverse of the ascending (length, position) order);
+ *       padding repeats the leading indices; rank r's list is every W-th index from r; its steps are runs of
+ *       `batch_size` consecutive entries (the last one ragged), rows in list order.
+ * Slot width = the longest sample of the slot (pad to max).  round = 0, origin = own step,
+ * stop_reason = ALL_FINISHED, n_rounds = 1. */
+static void offline_finish(oracle_plan *p, int32_t *err) {
+    int32_t R = p->R;
+    p->n_steps = (int32_t)p->slots[0].n;
+    for (int32_t r = 1; r < R; ++r)
+        if (p->slots[r].n != p->n_steps) *err = 5;
+    p->n_slots = (int64_t)R * p->n_steps;
+    p->grp_offset = (int64_t *)malloc((size_t)(p->n_slots > 0 ? p->n_slots : 1) * sizeof(int64_t));
+    int64_t off = 0;
+    for (int32_t r = 0; r < R; ++r)
+        for (int64_t k = 0; k < p->n_steps; ++k) {
+            slot *s = &p->slots[r].s[k];
+            s->width = 0;
+            for (int32_t a = 0; a < s->count; ++a)
+                if (p->lengths[s->ids[a]] > s->width) s->width = p->lengths[s->ids[a]];
+            int64_t area = (int64_t)s->count * (int64_t)s->width;
+            p->grp_offset[(int64_t)r * p->n_steps + k] = off;
+            off += (area + 15) / 16 * 16;
+            p->padded_elems += area;
+            p->samples_emitted += s->count;
+            for (int32_t a = 0; a < s->count; ++a) p->real_tokens += p->lengths[s->ids[a]];
+        }
+    p->total_elems = off;
+    for (int64_t k = 0; k < p->n_steps; ++k) {
+        int64_t e = 0;
+        for (int32_t r = 0; r < R; ++r) e += p->slots[r].s[k].count;
+        ivec_push(&p->step_samples, (int32_t)e);
+    }
+    p->n_rounds = 1;
+    p->stop_reason = ORACLE_STOP_ALL_FINISHED;
+}
+
+static const int32_t *g_key_ptr; /* batch shuffle keys (single-threaded) */
+static int cmp_key_index(const void *pa, const void *pb) {
+    int32_t a = *(const int32_t *)pa, b = *(const int32_t *)pb;
+    if (g_key_ptr[a] != g_key_ptr[b]) return g_key_ptr[a] < g_key_ptr[b] ? -1 : 1;
+    return a < b ? -1 : (a > b ? 1 : 0);
+}
+
+oracle_plan *oracle_offline_plan(int32_t planner, int32_t W, int64_t budget, const int32_t *len, int64_t N,
+                                 const int32_t *perm, const int32_t *shuffle_key, int32_t size, int32_t batch_size,
+                                 int32_t *err) {
+    *err = 0;
+    if (W < 1 || N < 0 || planner < 0 || planner > 2 || (planner != 0 && !perm && N > 0) ||
+        (planner == 1 && (!shuffle_key || size < 1)) || (planner == 2 && (size < 1 || batch_size < 1)) ||
+        (planner != 2 && budget < 1)) {
+        *err = 1;
+        return NULL;
+    }
+    for (int64_t i = 0; i < N; ++i)
+        if (len[i] < 1) {
+            *err = 2;
+            return NULL;
+        }
+    oracle_plan *p = (oracle_plan *)calloc(1, sizeof(oracle_plan));
+    p->R = W;
+    p->budget = budget;
+    p->rule = ORACLE_RULE_MAXFIT_ASC;
+    p->join_mode = 1;
+    p->rank_ptr = (int64_t *)calloc((size_t)W + 1, sizeof(int64_t)); /* all zeros: slot ids are global ids */
+    p->lengths = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+    if (N > 0) memcpy(p->lengths, len, (size_t)N * sizeof(int32_t));
+    p->slots = (svec *)calloc((size_t)W, sizeof(svec));
+    p->left = (ivec *)calloc((size_t)W, sizeof(ivec));
+    if (planner == 2) {
+        /* HFG: per-megabatch descending sort of the permutation, concatenated */
+        int32_t *L = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+        int32_t *plen = (int32_t *)malloc((size_t)(size > 0 ? size : 1) * sizeof(int32_t));
+        int32_t *loc = (int32_t *)malloc((size_t)(size > 0 ? size : 1) * sizeof(int32_t));
+        for (int64_t m0 = 0; m0 < N; m0 += size) {
+            int32_t n = (int32_t)((N - m0 < size) ? (N - m0) : size);
+            for (int32_t a = 0; a < n; ++a) {
+                plen[a] = len[perm[m0 + a]];
+                loc[a] = a;
+            }
+            g_sort_len = plen;
+            qsort(loc, (size_t)n, sizeof(int32_t), cmp_len_id); /* ascending (length, position) ... */
+            for (int32_t a = 0; a < n; ++a) L[m0 + a] = perm[m0 + loc[n - 1 - a]]; /* ... read backwards */
+        }
+        int64_t n_per = (N + W - 1) / W; /* the index list padded to a multiple of W, one stride per rank */
+        for (int32_t r = 0; r < W; ++r)
+            for (int64_t i0 = 0; i0 < n_per; i0 += batch_size) {
+                int64_t n = (n_per - i0 < batch_size) ? (n_per - i0) : batch_size;
+                slot s;
+                memset(&s, 0, sizeof(s));
+                s.ids = (int32_t *)malloc((size_t)n * sizeof(int32_t));
+                s.count = (int32_t)n;
+                s.origin = (int32_t)(i0 / batch_size);
+                for (int64_t a = 0; a < n; ++a) s.ids[a] = L[((i0 + a) * W + r) % N]; /* wrap-around padding */
+                svec_push(&p->slots[r], s);
+            }
+        free(L);
+        free(plen);
+        free(loc);
+    } else {
+        gvec batches;
+        memset(&batches, 0, sizeof(batches));
+        if (planner == 0) {
+            int32_t *order = (int32_t *)malloc((size_t)(N > 0 ? N : 1) * sizeof(int32_t));
+            for (int64_t i = 0; i < N; ++i) order[i] = (int32_t)i;
+            g_sort_len = len;
+            qsort(order, (size_t)N, sizeof(int32_t), cmp_len_id);
+            group_maxfit_asc(len, order, (int32_t)N, budget, &batches);
+            free(order);
+        } else {
+            int32_t *plen = (int32_t *)malloc((size_t)size * sizeof(int32_t));
+            int32_t *loc = (int32_t *)malloc((size_t)size * sizeof(int32_t));
+            int32_t *ord = (int32_t *)malloc((size_t)size * sizeof(int32_t));
+            gvec pre;
+            memset(&pre, 0, sizeof(pre));
+            for (int64_t b0 = 0; b0 < N; b0 += size) {
+                int32_t n = (int32_t)((N - b0 < size) ? (N - b0) : size);
+                for (int32_t a = 0; a < n; ++a) {
+                    plen[a] = len[perm[b0 + a]];
+                    loc[a] = a;
+                }
+                g_sort_len = plen;
+                qsort(loc, (size_t)n, sizeof(int32_t), cmp_len_id);
+                for (int32_t a = 0; a < n; ++a) ord[a] = perm[b0 + loc[a]];
+                group_maxfit_asc(len, ord, n, budget, &pre); /* packing never leaves the bucket */
+            }
+            /* batch shuffle: order by (key, index) */
+            int32_t *idx = (int32_t *)malloc((size_t)(pre.n > 0 ? pre.n : 1) * sizeof(int32_t));
+            for (int64_t j = 0; j < pre.n; ++j) idx[j] = (int32_t)j;
+            g_key_ptr = shuffle_key;
+            qsort(idx, (size_t)pre.n, sizeof(int32_t), cmp_key_index);
+            for (int64_t j = 0; j < pre.n; ++j) gvec_push(&batches, pre.g[idx[j]]);
+            free(idx);
+            free(pre.g);
+            free(plen);
+            free(loc);
+            free(ord);
+        }
+        /* wrap-around repetition of the leading batches to a multiple of W, then striding */
+        int64_t G = batches.n, n_steps = (G + W - 1) / W;
+        for (int32_t r = 0; r < W; ++r)
+            for (int64_t k = 0; k < n_steps; ++k) {
+                const group *g = &batches.g[(k * W + r) % G];
+                slot s;
+                memset(&s, 0, sizeof(s));
+                s.ids = (int32_t *)malloc((size_t)(g->n > 0 ? g->n : 1) * sizeof(int32_t));
+                memcpy(s.ids, g->ids, (size_t)g->n * sizeof(int32_t));
+                s.count = g->n;
+                s.origin = (int32_t)k;
+                svec_push(&p->slots[r], s);
+            }
+        for (int64_t j = 0; j < G; ++j) free(batches.g[j].ids);
+        free(batches.g);
+    }
+    offline_finish(p, err);
+    return p;
+}

@@ -63,6 +63,8 @@ def lib():
         L.oracle_plan_run.argtypes = [i32, i64, i32, i32, i64, i64, i32, i32, pi32, pi64, pi32]
         L.oracle_plan_run_sched.restype = vp
         L.oracle_plan_run_sched.argtypes = [i32, i64, i32, i32, i64, i64, i32, i32, pi32, pi64, pi64, i32, pi32]
+        L.oracle_offline_plan.restype = vp
+        L.oracle_offline_plan.argtypes = [i32, i32, i64, pi32, i64, pi32, pi32, i32, i32, pi32]
         L.oracle_plan_free.restype = None
         L.oracle_plan_free.argtypes = [vp]
         L.oracle_plan_scalar.restype = i64
@@ -174,8 +176,33 @@ class OraclePlan:
                                                   _p(lens, ctypes.c_int32), _p(self.rank_ptr, ctypes.c_int64),
                                                   _p(sp, ctypes.c_int64), int(sched.shape[0]), ctypes.byref(err))
         self.err = err.value
+        self._load()
+
+    PLANNER_GMT, PLANNER_BMT, PLANNER_HFG = 0, 1, 2
+
+    @classmethod
+    def offline(cls, planner: int, lengths, n_ranks: int, *, budget: int = 1, perm=None, shuffle_key=None, size: int = 0,
+                batch_size: int = 0) -> "OraclePlan":
+        """The paper's offline comparators as planners (App. I; App. J): GMT (0), BMT (1), HFG (2) over a
+        GLOBAL length array; slot ids are global sample ids.  ``perm`` / ``shuffle_key``: the random draws, as inputs."""
+        self = cls.__new__(cls)
+        self.lengths = np.ascontiguousarray(lengths, dtype=np.int32)
+        self.R = int(n_ranks)
+        self.rank_ptr = np.zeros(self.R + 1, dtype=np.int64)
+        err = ctypes.c_int32(0)
+        lens = self.lengths if len(self.lengths) else np.zeros(1, dtype=np.int32)
+        pm = None if perm is None else np.ascontiguousarray(perm, dtype=np.int32)
+        sk = None if shuffle_key is None else np.ascontiguousarray(shuffle_key, dtype=np.int32)
+        self._h = lib().oracle_offline_plan(int(planner), self.R, int(budget), _p(lens, ctypes.c_int32), len(self.lengths),
+                                            _p(pm, ctypes.c_int32), _p(sk, ctypes.c_int32), int(size), int(batch_size),
+                                            ctypes.byref(err))
+        self.err = err.value
+        self._load()
+        return self
+
+    def _load(self):
         if not self._h:
-            raise ValueError("oracle_plan_run failed with status %d" % self.err)
+            raise ValueError("the oracle planner failed with status %d" % self.err)
         if self.err:
             raise AssertionError("oracle: ranks hold different slot counts")
         sc = lambda w: int(lib().oracle_plan_scalar(self._h, w))
