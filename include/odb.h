@@ -256,6 +256,37 @@ ODB_API int odb_get_timing(odb_ctx *ctx, float *ms3);
  * the last 64 runs are kept, so a benchmark can enqueue many runs back to back and read their stage times
  * afterwards instead of waiting on every run.  ODB_ERR_STATE if that run does not exist (any more). */
 ODB_API int odb_get_timing_at(odb_ctx *ctx, int back, float *ms3);
+/* ---- the paper's offline comparators as planners ---------------------------------
+ * GMT and BMT (App. I) and HFG (App. J) build their batches from a GLOBAL scalar length array (the
+ * paper's "oracle cache"), not from per-rank streams; every rank computes the same list and takes its share by
+ * striding.  odb_offline_plan plans such a job for the context's n_ranks = W ranks and budget (padded-area
+ * feasibility max_i l_i * |b| <= budget, over-budget singletons allowed); afterwards odb_plan_query /
+ * odb_collate / odb_loss_weights work as for an ODB plan, with these differences: a slot's ids
+ * (d_grp_sample_ids) are GLOBAL sample ids; d_sample_ptr / d_span_ptr of odb_collate are indexed by global
+ * sample id; a sample may sit in two slots (wrap-around repetition); there are no leftovers; n_rounds = 1.
+ *   GMT: ascending (length, id) sort of all samples, greedy packing; the batch list is padded to a multiple of W
+ *        by repeating its leading batches (at most W - 1) and batch j goes to rank j mod W, step j div W.
+ *   BMT: the shuffled order d_perm is cut into buckets of `size` samples, each bucket is sorted by (length,
+ *        position in the shuffled order) and packed on its own, the batches are then ordered by (d_shuffle_key[j],
+ *        j), j = the batch's index before the shuffle; padding and striding as GMT.
+ *   HFG: d_perm is cut into megabatches of `size` samples, each sorted by length DESCENDING (the reverse of the
+ *        ascending (length, position) order), concatenated, padded to a multiple of W with its leading entries;
+ *        rank r takes every W-th index from r, and steps are runs of `batch_size` consecutive entries.
+ * The random draws are inputs: d_perm = a permutation of 0 .. n_samples - 1, d_shuffle_key = n_samples keys in
+ * [0, 2^31) (device pointers, caller-owned, must stay valid until odb_collate).  Synchronises (an offline
+ * planner: the host sizes the batch tables).  ODB_ERR_BAD_LENGTH if some length < 1. */
+enum { ODB_PLANNER_GMT = 0, ODB_PLANNER_BMT = 1, ODB_PLANNER_HFG = 2 };
+typedef struct {
+    int32_t planner;    /* ODB_PLANNER_* */
+    int32_t size;       /* BMT: samples per bucket; HFG: samples per megabatch */
+    int32_t batch_size; /* HFG: the fixed batch size */
+    int32_t reserved;
+    const int32_t *d_perm;        /* BMT, HFG */
+    const int32_t *d_shuffle_key; /* BMT */
+} odb_offline_params;
+ODB_API int odb_offline_plan(odb_ctx *ctx, const odb_offline_params *params, const int32_t *d_lengths, int64_t n_samples,
+                             void *stream);
+
 /* Tuning / measurement switches.  ODB_OPT_COLLATE_BULK_STORES (value 0 / 1, default 0): the collate kernel stages
  * the interior chunks of each arena in shared memory and stores them with bulk asynchronous copies
  * (cp.async.bulk.global.shared::cta, the store side of BASELINE.json's "TMA bulk copies") instead of 256-bit

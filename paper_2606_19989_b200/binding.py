@@ -57,6 +57,14 @@ class odb_dist_bufs(ctypes.Structure):
                 ("summary_world_count", _i32), ("d_step_samples_round", _vp), ("step_window", _i32), ("reserved", _i32)]
 
 
+class odb_offline_params(ctypes.Structure):
+    _fields_ = [("planner", _i32), ("size", _i32), ("batch_size", _i32), ("reserved", _i32), ("d_perm", _vp),
+                ("d_shuffle_key", _vp)]
+
+
+ODB_PLANNER_GMT, ODB_PLANNER_BMT, ODB_PLANNER_HFG = 0, 1, 2
+
+
 class OdbLibraryError(RuntimeError):
     """libodb.so is missing / unloadable.  There is no fallback path."""
 
@@ -96,6 +104,7 @@ SYMBOLS = {
     "odb_set_timing": (_i32, [_vp, _i32]),
     "odb_get_timing": (_i32, [_vp, _P(ctypes.c_float)]),
     "odb_get_timing_at": (_i32, [_vp, _i32, _P(ctypes.c_float)]),
+    "odb_offline_plan": (_i32, [_vp, _P(odb_offline_params), _vp, _i64, _vp]),
     "odb_set_option": (_i32, [_vp, _i32, _i64]),
     "odb_probe_bandwidth": (_i32, [_i32, _vp, _vp, _vp, _vp, _vp, _i64, _i32, _vp, _P(ctypes.c_float)]),
     "odb_kernel_launches": (_i64, [_vp]),
@@ -314,6 +323,16 @@ def odb_get_timing_at(ctx: int, back: int):
     ms = (ctypes.c_float * 3)()
     _check(load().odb_get_timing_at(ctx, int(back), ms), "odb_get_timing_at", ctx)
     return float(ms[0]), float(ms[1]), float(ms[2])
+
+
+def odb_offline_plan(ctx: int, planner: int, d_lengths, n_samples: int, *, d_perm=None, d_shuffle_key=None, size: int = 0,
+                     batch_size: int = 0, stream=None) -> None:
+    """Plan with one of the paper's offline comparators (GMT / BMT / HFG; include/odb.h); then odb_plan_query /
+    odb_collate as usual.  The caller keeps d_perm / d_shuffle_key alive until the collate call."""
+    prm = odb_offline_params(planner=int(planner), size=int(size), batch_size=int(batch_size), reserved=0,
+                             d_perm=_ptr(d_perm), d_shuffle_key=_ptr(d_shuffle_key))
+    _check(load().odb_offline_plan(ctx, ctypes.byref(prm), _ptr(d_lengths), int(n_samples), _stream(stream)),
+           "odb_offline_plan", ctx)
 
 
 ODB_OPT_COLLATE_BULK_STORES = 1

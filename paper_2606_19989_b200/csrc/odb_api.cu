@@ -241,7 +241,57 @@ int odb_reset(odb_ctx *c) {
     c->collated = false;
     c->arrived_set = false;
     c->begin_pending = false;
+    c->offline = false;
+    c->offline_perm = nullptr;
     c->d_lengths = nullptr;
+    return ODB_OK;
+}
+
+int odb_offline_plan(odb_ctx *c, const odb_offline_params *P, const int32_t *d_lengths, int64_t n_samples, void *stream) {
+    if (!c || !P) return ODB_ERR_INVALID_ARG;
+    if (c->world_ranks) return ODB_ERR_STATE;
+    if (n_samples < 0 || n_samples > c->n_max || (n_samples > 0 && !d_lengths)) return ODB_ERR_INVALID_ARG;
+    if (P->planner != ODB_PLANNER_GMT && P->planner != ODB_PLANNER_BMT && P->planner != ODB_PLANNER_HFG)
+        return ODB_ERR_INVALID_ARG;
+    if (P->planner != ODB_PLANNER_GMT && (P->size < 1 || (n_samples > 0 && !P->d_perm))) return ODB_ERR_INVALID_ARG;
+    if (P->planner == ODB_PLANNER_BMT && n_samples > 0 && !P->d_shuffle_key) return ODB_ERR_INVALID_ARG;
+    if (P->planner == ODB_PLANNER_HFG && P->batch_size < 1) return ODB_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(c, cudaSetDevice(c->device));
+    odb_reset(c);
+    c->last_stream = st;
+    c->offline = true;
+    c->offline_planner = P->planner;
+    c->offline_bs = P->batch_size;
+    c->offline_perm = P->planner == ODB_PLANNER_GMT ? nullptr : P->d_perm;
+    c->d_lengths = d_lengths;
+    c->n_total = n_samples;
+    c->max_nr = (int32_t)std::min<int64_t>(n_samples, 0x7fffffff);
+    c->h_rank_ptr.assign((size_t)c->prm.n_ranks + 1, 0);
+    CU(c, offline_build(c, P, d_lengths, n_samples, st));
+    {  // bad lengths
+        CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, st));
+        CU(c, cudaStreamSynchronize(st));
+        if (c->h_rec->bad_length) {
+            odb_reset(c);
+            return ODB_ERR_BAD_LENGTH;
+        }
+    }
+    const int64_t W = c->prm.n_ranks;
+    int64_t n_steps;
+    if (P->planner == ODB_PLANNER_HFG) {
+        const int64_t n_per = (n_samples + W - 1) / W;
+        n_steps = (n_per + P->batch_size - 1) / P->batch_size;
+    } else {
+        n_steps = (c->offline_G + W - 1) / W;
+    }
+    if (n_steps > 0x7fffffff / std::max<int64_t>(W, 1)) return ODB_ERR_INVALID_ARG;
+    c->n_steps = (int32_t)n_steps;
+    c->n_rounds = 1;
+    c->round = 1;
+    c->stop_reason = ODB_STOP_ALL_FINISHED;
+    CU(c, offline_slots(c, st));
+    c->state = 4;
     return ODB_OK;
 }
 
@@ -553,7 +603,7 @@ static void fill_info(odb_ctx *c) {
     I.n_slots = (int64_t)c->prm.n_ranks * c->n_steps;
     I.total_elems = D.total_elems;
     I.samples_emitted = D.samples_emitted;
-    I.samples_left = c->n_total - D.samples_emitted;  // Lemma 1: emitted + un-emitted = all
+    I.samples_left = D.samples_left;  // Lemma 1: emitted + un-emitted = all (0 for an offline plan)
     I.real_tokens = (int64_t)D.real_tokens;
     I.padded_elems = D.padded_elems;
     c->info_valid = true;
@@ -587,6 +637,11 @@ int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
     CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
     CU(c, cudaStreamSynchronize(st));
     fill_info(c);
+    if (c->offline) {  // the slot CSR's (global) ids: wrap-around repetition can emit a sample twice
+        CU(c, c->grp_sample_ids.ensure((size_t)c->info.samples_emitted + 1));
+        CU(c, launch_offline_ids(c, st));
+        CU(c, cudaMemsetAsync(c->left_ptr.p, 0, ((size_t)R + 1) * sizeof(int64_t), st));
+    }
     c->state = 5;
     *h_out = c->info;
     return ODB_OK;

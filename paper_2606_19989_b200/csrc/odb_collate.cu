@@ -37,13 +37,14 @@ constexpr int kPrepThreads = 1024;
 struct PrepJob {
     void *dst;
     const void *src;
-    int kind;  // words to copy: 0 = n_slots, 1 = 2 n_slots, 2 = 2 (n_slots + 1), 3 = n_steps
+    int kind;  // words to copy: 0 = n_slots, 1 = 2 n_slots, 2 = 2 (n_slots + 1), 3 = n_steps, 4 = samples_emitted, 5 = 2 (R + 1)
 };
 
 struct PrepArgs {
     const PlanDims *dims;
     int R;
     // rows
+    int offline_row_blocks;  // > 0: an offline plan (global ids): one thread per emitted ROW, that many blocks
     int rows_gx;  // blocks per rank
     const int64_t *rank_ptr;
     const int32_t *len;
@@ -105,6 +106,28 @@ __device__ __forceinline__ void prep_rows(const PrepArgs &A, int n_steps, int b)
     if (ns > 2) A.row_sp[q] = sp;  // only read on the CSR path (more than two spans): skip the scattered 8-byte store
 }
 
+// offline plans (F4): the slot CSR holds GLOBAL sample ids and a sample may be emitted twice, so the row
+// descriptors are gathered in emit order: one thread per emitted row
+__device__ __forceinline__ void prep_rows_offline(const PrepArgs &A, int b) {
+    const int64_t n_rows = A.dims->samples_emitted;
+    for (int64_t q = (int64_t)b * kPrepThreads + threadIdx.x; q < n_rows; q += (int64_t)A.offline_row_blocks * kPrepThreads) {
+        const int64_t g = A.grp_sample_ids[q];
+        if (A.user_ids) A.user_ids[q] = (int32_t)g;
+        RowDesc d;
+        d.tok = A.sample_ptr[g];
+        d.len = A.len[g];
+        const int64_t sp = A.span_ptr ? A.span_ptr[g] : 0;
+        const int ns = A.span_ptr ? (int)(A.span_ptr[g + 1] - sp) : 0;
+        d.nspan = ns;
+        d.lo0 = ns > 0 ? A.span_lo[sp] : 0;
+        d.hi0 = ns > 0 ? A.span_hi[sp] : 0;
+        d.lo1 = ns > 1 ? A.span_lo[sp + 1] : 0;
+        d.hi1 = ns > 1 ? A.span_hi[sp + 1] : 0;
+        A.rows[q] = d;
+        if (ns > 2) A.row_sp[q] = sp;
+    }
+}
+
 __device__ __forceinline__ void prep_tiles(const PrepArgs &A, int n_steps, int64_t n_slots, int b) {
     const int64_t tid = (int64_t)b * kPrepThreads + threadIdx.x, nth = (int64_t)A.tile_blocks * kPrepThreads;
     for (int64_t s = tid; s < n_slots; s += nth) A.grp_valid[s] = 0;
@@ -125,7 +148,12 @@ __device__ __forceinline__ void prep_tiles(const PrepArgs &A, int n_steps, int64
     }
     for (int j = 0; j < A.n_jobs; ++j) {
         const int kind = A.job[j].kind;
-        const int64_t words = kind == 0 ? n_slots : kind == 1 ? 2 * n_slots : kind == 2 ? 2 * (n_slots + 1) : (int64_t)n_steps;
+        const int64_t words = kind == 0   ? n_slots
+                              : kind == 1 ? 2 * n_slots
+                              : kind == 2 ? 2 * (n_slots + 1)
+                              : kind == 3 ? (int64_t)n_steps
+                              : kind == 4 ? A.dims->samples_emitted
+                                          : 2 * ((int64_t)A.R + 1);
         const uint32_t *__restrict__ src = reinterpret_cast<const uint32_t *>(A.job[j].src);
         uint32_t *__restrict__ dst = reinterpret_cast<uint32_t *>(A.job[j].dst);
         for (int64_t i = tid; i < words; i += nth) dst[i] = src[i];
@@ -170,10 +198,15 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(const PrepArgs A) {
     const int n_steps = A.dims->n_steps;
     const int64_t n_slots = (int64_t)A.R * n_steps;
     const int b = blockIdx.x;
-    const int nb_rows = A.rows_gx * A.R;
-    if (b < nb_rows) prep_rows(A, n_steps, b);
-    else if (b < nb_rows + A.tile_blocks) prep_tiles(A, n_steps, n_slots, b - nb_rows);
-    else prep_ids(A, n_steps, b - nb_rows - A.tile_blocks);
+    const int nb_rows = A.offline_row_blocks > 0 ? A.offline_row_blocks : A.rows_gx * A.R;
+    if (b < nb_rows) {
+        if (A.offline_row_blocks > 0) prep_rows_offline(A, b);
+        else prep_rows(A, n_steps, b);
+    } else if (b < nb_rows + A.tile_blocks) {
+        prep_tiles(A, n_steps, n_slots, b - nb_rows);
+    } else {
+        prep_ids(A, n_steps, b - nb_rows - A.tile_blocks);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -714,7 +747,19 @@ cudaError_t launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *
         A.user_left_ptr = u->d_left_ptr;
         A.user_left = u->d_left_ids;
     }
-    const int blocks = A.rows_gx * R + A.tile_blocks + R;
+    int blocks = A.rows_gx * R + A.tile_blocks + R;
+    if (c->offline) {  // rows in emit order; no leftovers (left_ptr was zeroed by odb_plan_query)
+        const int64_t n_rows = std::max<int64_t>(c->info.samples_emitted, 1);
+        A.offline_row_blocks = (int)std::min<int64_t>((n_rows + kPrepThreads - 1) / kPrepThreads, (int64_t)c->sm_count * 8);
+        A.user_ids = u ? u->d_grp_sample_ids : nullptr;
+        if (u && u->d_left_ptr) {
+            A.job[A.n_jobs].dst = u->d_left_ptr;
+            A.job[A.n_jobs].src = c->left_ptr.p;
+            A.job[A.n_jobs].kind = 5;
+            A.n_jobs++;
+        }
+        blocks = A.offline_row_blocks + A.tile_blocks;
+    }
     k_prep<<<blocks, kPrepThreads, 0, st>>>(A);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;

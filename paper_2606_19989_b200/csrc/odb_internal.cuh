@@ -258,6 +258,19 @@ struct odb_ctx {
     odb::DevBuf<int64_t> row_sp;
     odb::DevBuf<odb::TileRec> tiles;
 
+    // offline planners (odb_offline.cu): the plan's slots hold GLOBAL sample ids
+    bool offline = false;
+    int offline_planner = 0, offline_size = 0, offline_bs = 0;
+    int64_t offline_G = 0;             // batches in the global list (GMT / BMT)
+    const int32_t *offline_perm = nullptr;
+    odb::DevBuf<int64_t> of_seg_ptr;   // nseg + 1
+    odb::DevBuf<int32_t> of_seg_i32;   // 5 x nseg: zeros (n_left), zeros (fetch_pos), zeros (emit_cur), "all arrived", S; then G, boff (nseg + 1)
+    odb::DevBuf<int32_t> of_plen;      // N: lengths in list order; later the batch-shuffle keys
+    odb::DevBuf<int32_t> of_gpos;      // N + nseg + 1
+    odb::DevBuf<int32_t> of_bstart, of_bcnt, of_border;  // per batch: first position in the sorted keys, count; the shuffled order
+    odb::DevBuf<uint64_t> of_keyA, of_keyB;               // the batch shuffle's sort buffers
+    uint64_t *of_sorted = nullptr;
+
     // device staging for odb_run_host
     odb::DevBuf<int32_t> hs_lengths, hs_tokens, hs_span_lo, hs_span_hi, hs_ids, hs_labels, hs_pos;
     odb::DevBuf<int64_t> hs_sample_ptr, hs_span_ptr;
@@ -286,6 +299,18 @@ cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: 
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce
 // A9: rank-major tables, offsets, totals (sizes from the device-resident PlanDims)
 cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st);
+// ---- segment-level pieces shared with the offline planners (odb_offline.cu) -------------------------
+struct SortArgs;
+cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A, int64_t nseg, int maxS, cudaStream_t st);
+cudaError_t sort_segments_any(odb_ctx *c, const SortArgs &A, int64_t nseg, int maxS, uint64_t *keyB, uint64_t **sorted,
+                              cudaStream_t st);
+cudaError_t form_segments_maxfit(odb_ctx *c, const uint64_t *sorted, const int64_t *seg_ptr, const int32_t *S_arr,
+                                 int64_t nseg, int maxS, int32_t *jA, int32_t *jB, uint8_t *mark, int32_t *gpos,
+                                 int32_t *G_out, cudaStream_t st);
+// ---- odb_offline.cu -------------------------------------------------------------------------------
+cudaError_t offline_build(odb_ctx *c, const odb_offline_params *P, const int32_t *d_lengths, int64_t N, cudaStream_t st);
+cudaError_t offline_slots(odb_ctx *c, cudaStream_t st);
+cudaError_t launch_offline_ids(odb_ctx *c, cudaStream_t st);
 // ---- launchers implemented in odb_collate.cu -------------------------------------------------
 // collate preparation in ONE launch: row descriptors, tile table, slot-id / leftover tables, table copies
 cudaError_t launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,

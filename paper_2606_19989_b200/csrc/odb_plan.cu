@@ -1316,7 +1316,8 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
             dims->samples_emitted = tot_s;
             dims->padded_elems = s_base[2] + total[2];
             dims->real_tokens = (unsigned long long)(s_base[3] + total[3]);
-            dims->samples_left = n_total - tot_s;  // Lemma 1: emitted + un-emitted = all
+            // Lemma 1: emitted + un-emitted = all (n_total < 0: an offline plan, no leftovers)
+            dims->samples_left = n_total >= 0 ? n_total - tot_s : 0;
             // the caller's capacities (odb_run enqueues the collate kernels before the host sees the sizes)
             int err = 0;
             if (cap.arena >= 0 && tot_e > cap.arena) err = ODB_ERR_CAPACITY;
@@ -1324,7 +1325,7 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
             if (cap.slots >= 0 && n_slots > cap.slots) err = ODB_ERR_CAPACITY;
             if (cap.ids >= 0 && tot_s > cap.ids) err = ODB_ERR_CAPACITY;
             if (cap.steps >= 0 && n_steps > cap.steps) err = ODB_ERR_CAPACITY;
-            if (cap.left >= 0 && n_total - tot_s > cap.left) err = ODB_ERR_CAPACITY;
+            if (cap.left >= 0 && n_total >= 0 && n_total - tot_s > cap.left) err = ODB_ERR_CAPACITY;
             dims->err = err;
         }
     }
@@ -1367,6 +1368,65 @@ static size_t form_smem_bytes(int maxS) {
     const size_t n1p = ((size_t)maxS + 1 + 7) & ~(size_t)7;
     const size_t words = ((size_t)maxS + 1 + 31) >> 5;
     return 4 * n1p + 4 * words;
+}
+
+// Segmented sort of arbitrary segments (used by the offline planners): the cluster sort when every segment has
+// at most 65536 keys, else chunk sorts + merge passes through global memory.  A.keys_out / keyB: ping-pong buffers;
+// *sorted receives the buffer that holds the result.  A.first must be 0 on the fallback path (no state reset there).
+cudaError_t sort_segments_any(odb_ctx *c, const SortArgs &A, int64_t nseg, int maxS, uint64_t *keyB, uint64_t **sorted,
+                              cudaStream_t st) {
+    *sorted = A.keys_out;
+    if (maxS == 0 || nseg == 0) return cudaSuccess;
+    cudaError_t se = c->no_cluster_sort ? cudaErrorNotSupported : launch_sort_segments(c, A, nseg, maxS, st);
+    if (se == cudaSuccess) return cudaSuccess;
+    if (se != cudaErrorNotSupported) {
+        (void)cudaGetLastError();
+        c->no_cluster_sort = true;
+    }
+    if (nseg > 65535) return cudaErrorInvalidValue;  // (large segments and that many of them do not occur together)
+    const int chunks = (maxS + kSortChunk - 1) / kSortChunk;
+    k_chunk_sort_reg<<<dim3(chunks, (unsigned)nseg), kSortRegThreads, 0, st>>>(A.len, A.rank_ptr, A.n_left, A.fetch_pos,
+                                                                             A.left_ids, A.arrived, A.buffer_size,
+                                                                             A.keys_out, A.S_out, c->d_rec);
+    ODB_LAUNCH_CHECK(c);
+    uint64_t *src = A.keys_out, *dst = keyB;
+    for (int64_t w = kSortChunk; w < maxS; w *= 2) {
+        const int gx = (maxS + kMergeTile - 1) / kMergeTile;
+        k_merge_pass<<<dim3(gx, (unsigned)nseg), kMergeThreads, 0, st>>>(src, dst, A.rank_ptr, A.S_out, (int)w);
+        ODB_LAUNCH_CHECK(c);
+        uint64_t *t = src;
+        src = dst;
+        dst = t;
+    }
+    *sorted = src;
+    return cudaSuccess;
+}
+
+// A2 + A3 over arbitrary segments with the padded-area rule (the offline planners' greedy packing, App. I)
+cudaError_t form_segments_maxfit(odb_ctx *c, const uint64_t *sorted, const int64_t *seg_ptr, const int32_t *S_arr,
+                                 int64_t nseg, int maxS, int32_t *jA, int32_t *jB, uint8_t *mark, int32_t *gpos,
+                                 int32_t *G_out, cudaStream_t st) {
+    if (nseg == 0 || maxS == 0) return cudaSuccess;
+    const uint32_t budget = (uint32_t)c->prm.budget;
+    {
+        const unsigned ns = (unsigned)nseg;  // (gridDim.x holds 2^31 - 1 blocks)
+        const int64_t s0 = 0;
+        if (maxS <= 32768) {
+            if (!c->attr_form_hier) {
+                cudaError_t e = cudaFuncSetAttribute(k_form_groups_hier, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                     (int)kFormSmemLimit);
+                if (e != cudaSuccess) return e;
+                c->attr_form_hier = true;
+            }
+            k_form_groups_hier<<<ns, kRankThreads, form_hier_smem_bytes(maxS), st>>>(sorted, seg_ptr + s0, S_arr + s0, budget,
+                                                                                    ODB_RULE_MAXFIT_ASC, gpos, G_out + s0);
+        } else {
+            k_form_groups<<<ns, kRankThreads, 0, st>>>(sorted, seg_ptr + s0, S_arr + s0, budget, ODB_RULE_MAXFIT_ASC, jA, jB,
+                                                       mark, gpos, G_out + s0);
+        }
+        ODB_LAUNCH_CHECK(c);
+    }
+    return cudaSuccess;
 }
 
 // the per-run state reset, when no sort launch has done it (no window anywhere, or the fallback sort)
@@ -1596,8 +1656,8 @@ cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap
                                                c->st_origin.p, c->grp_count.p, c->grp_width.p, c->grp_round.p,
                                                c->grp_real.p, c->grp_origin.p, c->grp_offset.p, c->grp_sample_ptr.p,
                                                reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
-                                               reinterpret_cast<unsigned int *>(c->scan_state.p), cap, c->n_total,
-                                               rank_off);
+                                               reinterpret_cast<unsigned int *>(c->scan_state.p), cap,
+                                               c->offline ? (int64_t)-1 : c->n_total, rank_off);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(kMsThreads) k_sort_window(const SortArgs A, in
             A.fetch_pos[r_] = 0;
             A.emit_cur[r_] = 0;
         }
-        if (r_ == 0) A.rec->n_finished = 0;  // counted again by this round's commit
+        if (r_ == 0 && A.rec) A.rec->n_finished = 0;  // counted again by this round's commit
     }
     if (S == 0) return;  // the whole cluster leaves
     const int c0 = c * kMsChunk;
@@ -89,9 +89,10 @@ __global__ void __launch_bounds__(kMsThreads) k_sort_window(const SortArgs A, in
     cluster_sync_all();  // nobody leaves while a neighbour may still read its shared memory (none does; cheap insurance)
 }
 
-// Launches the cluster sort for windows of up to 16 * 4096 keys.  Returns cudaErrorNotSupported when the
-// window is larger (the caller falls back to chunk sorts + global merge passes).
-cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st) {
+// Launches the cluster sort for `nseg` segments (rank windows; buckets / megabatches of the offline planners)
+// of up to 16 * 4096 keys each.  Returns cudaErrorNotSupported when a segment can be larger (the caller falls
+// back to chunk sorts + global merge passes).
+cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A0, int64_t nseg, int maxS, cudaStream_t st) {
     const int chunks = (maxS + kMsChunk - 1) / kMsChunk;
     int CL = 1;
     while (CL < chunks) CL <<= 1;
@@ -105,6 +106,42 @@ cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st
         if (e != cudaSuccess) return e;
         c->attr_sort = true;
     }
+    for (int64_t s0 = 0; s0 < nseg; s0 += 65535) {  // gridDim.y is limited to 65535
+        const unsigned ns = (unsigned)std::min<int64_t>(nseg - s0, 65535);
+        SortArgs A = A0;
+        A.rank_ptr += s0;
+        A.n_left += s0;
+        A.fetch_pos += s0;
+        A.emit_cur += s0;
+        A.arrived += s0;
+        A.S_out += s0;
+        if (s0 > 0) A.first = 0;  // (the per-run state is cleared by the first batch of segments)
+        if (CL == 1) {  // no cluster needed: a plain launch (the attribute path costs a few microseconds per launch)
+            k_sort_window<<<dim3(1, ns), kMsThreads, smem, st>>>(A, 1);
+            ODB_LAUNCH_CHECK(c);
+            continue;
+        }
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3((unsigned)CL, ns, 1);
+        cfg.blockDim = dim3(kMsThreads, 1, 1);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)CL;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        cudaError_t e = cudaLaunchKernelEx(&cfg, k_sort_window, A, CL);
+        if (e != cudaSuccess) return e;
+        c->launches++;
+    }
+    return cudaSuccess;
+}
+
+cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st) {
     SortArgs A;
     A.len = c->d_lengths;
     A.rank_ptr = c->d_rank_ptr;
@@ -122,30 +159,9 @@ cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st
     A.emit_pos = c->emit_pos;
     A.step_samples = c->step_samples.p;
     A.step_cap = c->step_samples.p ? (int64_t)c->step_samples.cap : 0;
-    if (CL == 1) {  // no cluster needed: a plain launch (the attribute path costs a few microseconds per launch)
-        k_sort_window<<<dim3(1, (unsigned)c->prm.n_ranks), kMsThreads, smem, st>>>(A, 1);
-        ODB_LAUNCH_CHECK(c);
-        c->sorted = c->keyA;
-        return cudaSuccess;
-    }
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = dim3((unsigned)CL, (unsigned)c->prm.n_ranks, 1);
-    cfg.blockDim = dim3(kMsThreads, 1, 1);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)CL;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, k_sort_window, A, CL);
-    if (e != cudaSuccess) return e;
-    c->launches++;
-    c->sorted = c->keyA;
-    return cudaSuccess;
+    cudaError_t e = launch_sort_segments(c, A, c->prm.n_ranks, maxS, st);
+    if (e == cudaSuccess) c->sorted = c->keyA;
+    return e;
 }
 
 }  // namespace odb
