@@ -203,7 +203,6 @@ cudaError_t launch_offline_ids(odb_ctx *c, cudaStream_t st) {
 
 // Builds the plan up to the step-major staging tables; *h_G receives the number of batches (GMT / BMT).
 cudaError_t offline_build(odb_ctx *c, const odb_offline_params *P, const int32_t *d_lengths, int64_t N, cudaStream_t st) {
-    const int W = c->prm.n_ranks;
     const int64_t size = P->planner == ODB_PLANNER_GMT ? std::max<int64_t>(N, 1) : P->size;
     const int64_t nseg = N == 0 ? 0 : (N + size - 1) / size;
     const int maxS = (int)std::min<int64_t>(size, N);
@@ -220,7 +219,9 @@ cudaError_t offline_build(odb_ctx *c, const odb_offline_params *P, const int32_t
     int32_t *S = tab + 4 * nseg, *G = tab + 5 * nseg, *boff = tab + 6 * nseg;
     {
         const int blocks = (int)std::min<int64_t>((N + 255) / 256, (int64_t)c->sm_count * 8);
-        k_of_gather<<<blocks, 256, 0, st>>>(d_lengths, P->d_perm, N, c->of_plen.p, c->d_rec);
+        // (GMT works on the samples in their own order; BMT / HFG on the shuffled order)
+        k_of_gather<<<blocks, 256, 0, st>>>(d_lengths, P->planner == ODB_PLANNER_GMT ? nullptr : P->d_perm, N, c->of_plen.p,
+                                            c->d_rec);
         ODB_LAUNCH_CHECK(c);
         const int b2 = (int)std::min<int64_t>((nseg + 256) / 256, (int64_t)c->sm_count * 8);
         k_of_segments<<<b2, 256, 0, st>>>(N, size, nseg, c->of_seg_ptr.p, tab);

@@ -105,7 +105,7 @@ def compare_full(plan, oracle_out, info, out):
     assert np.array_equal(out.table("step_valid_tokens").cpu().numpy(), oracle_out["step_valid_tokens"])
 
 
-def compare_sampled_slots(wl, plan, out, slots):
+def compare_sampled_slots(wl, plan, out, slots, global_ids=False):
     """Collate the listed slots one by one with the oracle (tokens regenerated from the hash for just
     their samples) and compare with the GPU arenas; also the slot's valid-token count."""
     p = wl.params
@@ -114,7 +114,9 @@ def compare_sampled_slots(wl, plan, out, slots):
         s = int(s)
         r = s // plan.n_steps
         c, w, off = int(plan.grp_count[s]), int(plan.grp_width[s]), int(plan.grp_offset[s])
-        ids = plan.grp_sample_ids[plan.grp_sample_ptr[s]:plan.grp_sample_ptr[s + 1]].astype(np.int64) + wl.rank_ptr[r]
+        ids = plan.grp_sample_ids[plan.grp_sample_ptr[s]:plan.grp_sample_ptr[s + 1]].astype(np.int64)
+        if not global_ids:      # (an offline plan's slots hold global sample ids already)
+            ids = ids + wl.rank_ptr[r]
         toks, toff = I.tokens_for_samples(wl, ids)
         tok_start = np.zeros(max(wl.n_samples, 1), dtype=np.int64)
         tok_start[ids] = toff

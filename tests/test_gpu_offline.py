@@ -67,7 +67,7 @@ def test_offline_gmt_large_pool(P, oracle):
     Par.compare_plan(plan, info, out)
     rng = np.random.default_rng(0)
     pick = sorted(set(rng.integers(0, plan.n_slots, 24).tolist()) | {0, plan.n_slots - 1})
-    Par.compare_sampled_slots(wl, plan, out, pick)
+    Par.compare_sampled_slots(wl, plan, out, pick, global_ids=True)
     Par.device_self_consistency(info, out)
 
 
@@ -82,7 +82,7 @@ def test_offline_bad_length_and_reuse(P, oracle):
         assert ei.value.status == P.ODB_ERR_BAD_LENGTH
     # an ODB run on a context that planned offline before (and back): the offline state does not leak
     dw = Par.DeviceWorkload(wl)
-    with P.Odb(P.make_params(1, 2048), 300) as ctx:
+    with P.Odb(Par.gpu_params(wl), 300) as ctx:
         P.odb_offline_plan(ctx.h, 0, dw.lengths, 300)
         a = P.odb_plan_query(ctx.h)
         info = ctx.plan(dw.lengths, wl.rank_ptr)
