@@ -472,6 +472,7 @@ def run_ours(args):
                                                             "frac": w["frac"], "ms_per_step": w["ms_per_step"],
                                                             "note": "sub-millisecond steps: launch latency, not HBM, bounds them"}
             result["paper_operating_point"] = paper_operating_point(P, device, peak)
+            result["comparators"] = comparators(P, device)
         # ---- e2e through the C ABI with HOST buffers (odb_run_host) -------------------------
         if not args.no_e2e:
             need = 4 * wl.n_tokens + 13 * int(info.total_elems)
@@ -673,6 +674,62 @@ def mix_ceiling(P, device, n_elems=1 << 29):
     del src, o, m
     torch.cuda.empty_cache()
     return out
+
+
+def comparators(P, device):
+    """Shape statistics of ODB beside the paper's offline comparators as planners (F4: GMT / BMT; HFG)
+    on the synthetic configs: samples per update (global), padding fraction, steps -- the quantities of the paper's
+    Tables 13 / 14.  Planning only (lengths; no token is touched).  The offline planners see the pooled
+    lengths of all ranks; HFG's fixed batch size is the largest one whose padded area fits the budget for the longest
+    sample (its "full-epoch-safe" batch size), its megabatch = 50 batches per rank (the HuggingFace default),
+    BMT buckets hold 4096 samples."""
+    import torch
+    local = int(device.split(":")[1])
+    rows = []
+    for idx in (1, 2, 3):
+        wl = I.make_workload(idx)
+        W, N, budget = wl.n_ranks, wl.n_samples, wl.params["budget"]
+        d_len = torch.from_numpy(wl.lengths).to(device)
+        rng = np.random.default_rng(600 + idx)
+        d_perm = torch.from_numpy(rng.permutation(N).astype(np.int32)).to(device)
+        d_key = torch.from_numpy(rng.integers(0, 2**31 - 1, N).astype(np.int32)).to(device)
+        bs = max(1, budget // int(wl.lengths.max()))
+
+        def row(method, info, ms):
+            rows.append({"workload": "configs[%d] %s" % (idx, I.bj_config(idx)["name"]), "method": method,
+                         "samples_per_update": int(info.samples_emitted) / max(int(info.n_steps), 1),
+                         "real_tokens_per_update": int(info.real_tokens) / max(int(info.n_steps), 1),
+                         "pad_frac": 1.0 - int(info.real_tokens) / max(int(info.padded_elems), 1),
+                         "n_steps": int(info.n_steps), "samples_emitted": int(info.samples_emitted), "plan_ms": ms})
+
+        def timed(fn):
+            fn()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            info = fn()
+            torch.cuda.synchronize()
+            return info, (time.perf_counter() - t0) * 1e3
+
+        with P.Odb(gpu_params(P, wl), N, device=local) as ctx:
+            info, ms = timed(lambda: ctx.plan(d_len, wl.rank_ptr))
+            row("ODB (rule THRESHOLD, whole-stream window)", info, ms)
+        wl1k = I.make_workload(idx)
+        wl1k.params["buffer_size"] = 1024
+        with P.Odb(gpu_params(P, wl1k), N, device=local) as ctx:
+            info, ms = timed(lambda: ctx.plan(d_len, wl.rank_ptr))
+            row("ODB (rule THRESHOLD, buffer 1024)", info, ms)
+        prm = P.make_params(W, budget, rule=P.ODB_RULE_MAXFIT_ASC)
+        for name, planner, kw in (("GMT-oracle", P.ODB_PLANNER_GMT, {}),
+                                  ("BMT-oracle (bucket 4096)", P.ODB_PLANNER_BMT, dict(d_perm=d_perm, d_shuffle_key=d_key, size=4096)),
+                                  ("HFG-oracle (bs %d, megabatch %d)" % (bs, bs * W * 50), P.ODB_PLANNER_HFG,
+                                   dict(d_perm=d_perm, size=bs * W * 50, batch_size=bs))):
+            with P.Odb(prm, N, device=local) as ctx:
+                def fn():
+                    P.odb_offline_plan(ctx.h, planner, d_len, N, **kw)
+                    return P.odb_plan_query(ctx.h)
+                info, ms = timed(fn)
+                row(name, info, ms)
+    return rows
 
 
 def cell_key(config, cv, budget, rule, buffer_size=0):

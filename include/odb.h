@@ -186,8 +186,10 @@ ODB_API int odb_run(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_ran
 
 /* End-to-end variant with HOST buffers (pinned memory recommended): copies lengths, sample_ptr,
  * spans and tokens host->device, runs the whole path, copies the four arenas and every non-NULL
- * table of `h_out_bufs` (same struct, HOST pointers) back, rank by rank so that copies overlap the
- * collate kernel.  Synchronises before returning.  n_spans = h_span_ptr[N]. */
+ * table of `h_out_bufs` (same struct, HOST pointers) back.  The device memory it uses does not grow
+ * with the job: tokens pass through a ring of three rank-sized buffers, the arenas through a ring of
+ * three fixed-size pieces (ODB_OPT_HOST_STAGING_ELEMS), uploads, collate launches and downloads overlapping
+ * on three streams.  Synchronises before returning.  n_spans = h_span_ptr[N]. */
 ODB_API int odb_run_host(odb_ctx *ctx, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
                  const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
                  const int32_t *h_span_hi, const odb_outputs *h_out_bufs, odb_plan_info *h_out, void *stream);
@@ -291,8 +293,10 @@ ODB_API int odb_offline_plan(odb_ctx *ctx, const odb_offline_params *params, con
  * the interior chunks of each arena in shared memory and stores them with bulk asynchronous copies
  * (cp.async.bulk.global.shared::cta, the store side of BASELINE.json's "TMA bulk copies") instead of 256-bit
  * streaming stores from registers.  Same results bit for bit; the measured comparison is in profiles/.
+ * ODB_OPT_HOST_STAGING_ELEMS (value >= 1, default 2^25): arena elements per device staging piece of odb_run_host
+ * (three pieces of 13 bytes per element are held; rounded down to a multiple of 4096, at least 4096).
  * ODB_ERR_INVALID_ARG for an unknown option. */
-enum { ODB_OPT_COLLATE_BULK_STORES = 1 };
+enum { ODB_OPT_COLLATE_BULK_STORES = 1, ODB_OPT_HOST_STAGING_ELEMS = 2 };
 ODB_API int odb_set_option(odb_ctx *ctx, int option, int64_t value);
 
 /* Bandwidth probes (measurement utility, not part of the method): the collate kernel's byte mix -- 4 bytes read

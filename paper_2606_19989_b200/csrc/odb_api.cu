@@ -127,8 +127,8 @@ static void free_all(odb_ctx *c) {
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
     if (c->copy_ev) cudaEventDestroy(c->copy_ev);
-    for (cudaEvent_t e : c->tok_ev) cudaEventDestroy(e);
-    for (cudaEvent_t e : c->col_ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    c->piece_ctr.release();
     if (c->h_rank_off) cudaFreeHost(c->h_rank_off);
 }
 
@@ -299,6 +299,10 @@ int odb_set_option(odb_ctx *c, int option, int64_t value) {
     if (!c) return ODB_ERR_INVALID_ARG;
     switch (option) {
     case ODB_OPT_COLLATE_BULK_STORES: c->collate_bulk = value != 0; return ODB_OK;
+    case ODB_OPT_HOST_STAGING_ELEMS:
+        if (value < 1) return ODB_ERR_INVALID_ARG;
+        c->host_staging_elems = value;
+        return ODB_OK;
     default: return ODB_ERR_INVALID_ARG;
     }
 }
@@ -951,6 +955,28 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
     return collate_impl(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
 }
 
+// a pool of timing-less events (odb_run_host orders its three streams with one event per token load and two
+// per output piece)
+static cudaError_t pool_event(odb_ctx *c, size_t i, cudaEvent_t *out) {
+    while (c->ev_pool.size() <= i) {
+        cudaEvent_t e = nullptr;
+        cudaError_t rc = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+        if (rc != cudaSuccess) return rc;
+        c->ev_pool.push_back(e);
+    }
+    *out = c->ev_pool[i];
+    return cudaSuccess;
+}
+
+// Device memory of odb_run_host does NOT grow with the job: the tokens go through a ring of three rank-sized
+// buffers, the four arenas through a ring of three fixed-size pieces (host_staging_elems elements each), so a job
+// whose inputs and outputs exceed the device memory still runs.  Three streams: lengths go up first on the compute
+// stream (planning needs nothing else); the CSR arrays and then the tokens go up RANK BY RANK on the copy stream
+// (a ring slot is reused once the rank that held it has been collated); a rank's slots are collated piece by piece
+// as soon as its tokens have landed (a piece = a tile-aligned range of arena elements inside the rank's range; a
+// tile that straddles a rank boundary is visited by both neighbouring launches, each writing only its own
+// elements), and every piece goes down on the third stream while later pieces are collated and later ranks
+// uploaded: both directions of the host link are busy at once.
 static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_rank_ptr, const int32_t *h_tokens,
                  const int64_t *h_sample_ptr, const int64_t *h_span_ptr, const int32_t *h_span_lo,
                  const int32_t *h_span_hi, const odb_outputs *ho, odb_plan_info *h_out, void *stream) {
@@ -962,28 +988,34 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
     const int64_t N = h_rank_ptr[R];
     if (N < 0 || N > c->n_max) return ODB_ERR_INVALID_ARG;
     if (N > 0 && (!h_lengths || !h_sample_ptr || !h_tokens)) return ODB_ERR_INVALID_ARG;
-    const int64_t n_tok = N > 0 ? h_sample_ptr[N] : 0;
     const int64_t n_span = (h_span_ptr && N > 0) ? h_span_ptr[N] : 0;
+    int64_t max_rank_tok = 0;
+    for (int r = 0; r < R && N > 0; ++r)
+        max_rank_tok = std::max(max_rank_tok, h_sample_ptr[h_rank_ptr[r + 1]] - h_sample_ptr[h_rank_ptr[r]]);
+    constexpr int kRing = 3;
+    const size_t tok_slot = ((size_t)max_rank_tok + 8 + 3) & ~(size_t)3;  // ints per ring slot (16-byte multiples)
+    const int64_t piece = std::max<int64_t>(kColTile, (c->host_staging_elems / kColTile) * kColTile);
     CU(c, c->hs_lengths.ensure((size_t)N + 1));
     CU(c, c->hs_sample_ptr.ensure((size_t)N + 1));
     CU(c, c->hs_span_ptr.ensure((size_t)N + 1));
     CU(c, c->hs_span_lo.ensure((size_t)n_span + 1));
     CU(c, c->hs_span_hi.ensure((size_t)n_span + 1));
-    CU(c, c->hs_tokens.ensure((size_t)n_tok + 4));
+    CU(c, c->hs_tokens.ensure(kRing * tok_slot + 16));
+    CU(c, c->hs_ids.ensure(kRing * (size_t)piece + 16));
+    CU(c, c->hs_labels.ensure(kRing * (size_t)piece + 16));
+    CU(c, c->hs_pos.ensure(kRing * (size_t)piece + 16));
+    CU(c, c->hs_mask.ensure(kRing * (size_t)piece + 16));
     if (!c->copy_stream) {
         CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
         CU(c, cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
         CU(c, cudaEventCreateWithFlags(&c->copy_ev, cudaEventDisableTiming));
-        c->tok_ev.assign((size_t)R, nullptr);
-        c->col_ev.assign((size_t)R, nullptr);
-        for (int r = 0; r < R; ++r) {
-            CU(c, cudaEventCreateWithFlags(&c->tok_ev[r], cudaEventDisableTiming));
-            CU(c, cudaEventCreateWithFlags(&c->col_ev[r], cudaEventDisableTiming));
-        }
     }
-    // Inputs host -> device.  Lengths first, on the compute stream: planning needs nothing else.  The
-    // CSR arrays and then the tokens, RANK BY RANK (an event per rank), go on the copy stream and
-    // overlap the planning kernels, the collate launches of earlier ranks and the result copies.
+    // events: [0, R) tokens of rank r landed; [R, 2R) rank r collated; then two per piece (collated, copied back)
+    auto drain = [&]() {
+        cudaStreamSynchronize(c->copy_stream);
+        cudaStreamSynchronize(c->d2h_stream);
+        cudaStreamSynchronize(st);
+    };
     if (N > 0) CU(c, cudaMemcpyAsync(c->hs_lengths.p, h_lengths, (size_t)N * 4, cudaMemcpyHostToDevice, st));
     CU(c, cudaEventRecord(c->copy_ev, st));
     CU(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev, 0));  // orders this call after the previous one's reads
@@ -999,20 +1031,33 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
         }
     }
     CU(c, cudaEventRecord(c->copy_ev, c->copy_stream));  // CSR arrays landed
-    for (int r = 0; r < R; ++r) {
+    // the first ring's worth of tokens can go up while the plan is being made
+    auto upload_rank = [&](int r) -> int {
+        cudaEvent_t ev;
+        if (r >= kRing) {  // the slot is free once the rank that held it has been collated
+            CU(c, pool_event(c, (size_t)R + (size_t)(r - kRing), &ev));
+            CU(c, cudaStreamWaitEvent(c->copy_stream, ev, 0));
+        }
         if (N > 0) {
             const int64_t t0 = h_sample_ptr[h_rank_ptr[r]], t1 = h_sample_ptr[h_rank_ptr[r + 1]];
+            // placed so that (slot + (t0 & 3)) - t0 is 16-byte aligned: the kernel's aligned vector loads see the same
+            // skew as in the caller's buffer
+            int32_t *dst = c->hs_tokens.p + (size_t)(r % kRing) * tok_slot + (size_t)(t0 & 3);
             if (t1 > t0)
-                CU(c, cudaMemcpyAsync(c->hs_tokens.p + t0, h_tokens + t0, (size_t)(t1 - t0) * 4, cudaMemcpyHostToDevice,
-                                      c->copy_stream));
+                CU(c, cudaMemcpyAsync(dst, h_tokens + t0, (size_t)(t1 - t0) * 4, cudaMemcpyHostToDevice, c->copy_stream));
         }
-        CU(c, cudaEventRecord(c->tok_ev[r], c->copy_stream));
-    }
-    auto drain = [&]() {
-        cudaStreamSynchronize(c->copy_stream);
-        cudaStreamSynchronize(c->d2h_stream);
-        cudaStreamSynchronize(st);
+        CU(c, pool_event(c, (size_t)r, &ev));
+        CU(c, cudaEventRecord(ev, c->copy_stream));
+        return ODB_OK;
     };
+    int uploaded = 0;
+    for (; uploaded < std::min(R, kRing); ++uploaded) {
+        int urc = upload_rank(uploaded);
+        if (urc != ODB_OK) {
+            drain();
+            return urc;
+        }
+    }
     int rc = run_rounds(c, c->hs_lengths.p, h_rank_ptr, h_out, st);
     if (rc != ODB_OK) {
         drain();
@@ -1036,50 +1081,74 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
         drain();
         return rc;
     }
-    const size_t E = (size_t)I.total_elems;
-    CU(c, c->hs_ids.ensure(E + 16));
-    CU(c, c->hs_labels.ensure(E + 16));
-    CU(c, c->hs_pos.ensure(E + 16));
-    CU(c, c->hs_mask.ensure(E + 16));
-    odb_outputs dev;
-    memset(&dev, 0, sizeof(dev));
-    dev.d_input_ids = c->hs_ids.p;
-    dev.d_labels = c->hs_labels.p;
-    dev.d_position_ids = c->hs_pos.p;
-    dev.d_attention_mask = c->hs_mask.p;
-    dev.arena_capacity = (int64_t)E;
     const size_t n_slots = (size_t)I.n_slots;
     CU(c, c->rows.ensure((size_t)I.samples_emitted + 1));
     CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
     CU(c, c->tiles.ensure((size_t)((I.total_elems + kColTile - 1) / kColTile) + 2));
+    // pieces: every rank's arena range [lo, hi) cut at tile-aligned positions, at most `piece` elements each
+    int64_t n_pieces = 0;
+    for (int r = 0; r < R; ++r) {
+        const int64_t lo = c->h_rank_off[r], hi = c->h_rank_off[r + 1];
+        for (int64_t cur = lo; cur < hi; ++n_pieces) cur = std::min(hi, (cur / kColTile) * kColTile + piece);
+    }
+    CU(c, c->piece_ctr.ensure((size_t)n_pieces + 1));
+    CU(c, cudaMemsetAsync(c->piece_ctr.p, 0, ((size_t)n_pieces + 1) * sizeof(unsigned long long), st));
     CU(c, cudaStreamWaitEvent(st, c->copy_ev, 0));  // sample_ptr / spans have landed
-    // row descriptors, tile table, id / leftover tables, cleared counters: one launch
+    // row descriptors, tile table, id / leftover tables: one launch
     CU(c, launch_prep(c, c->hs_sample_ptr.p, h_span_ptr ? c->hs_span_ptr.p : nullptr, c->hs_span_lo.p, c->hs_span_hi.p,
                       nullptr, st));
     if (c->timing) CU(c, cudaEventRecord(c->ev[1], st));
-    if (E > 0) {
-        // The pipeline: rank r's slots are collated as soon as its tokens have landed, and its slice of
-        // the four arenas goes back on the device -> host stream while later ranks are still being
-        // uploaded and collated (both directions of the host link busy at once).  The arena offset of
-        // every rank's first slot was written to pinned memory by the slot scan, together with the plan
-        // sizes the host has already waited for (odb_plan_query): no further synchronisation here.
-        for (int r = 0; r < R; ++r) {
-            const int64_t lo = c->h_rank_off[r], hi = c->h_rank_off[r + 1];
-            if (hi <= lo) continue;
-            CU(c, cudaStreamWaitEvent(st, c->tok_ev[r], 0));
-            rc = collate_launch(c, c->hs_tokens.p, c->hs_span_lo.p, c->hs_span_hi.p, &dev, false, lo, hi, 0,
-                                c->d_tile_counter + r, st);
-            if (rc != ODB_OK) {
-                drain();
-                return rc;
+    int64_t pi = 0;
+    const size_t ev_piece0 = 2 * (size_t)R;
+    for (int r = 0; r < R; ++r) {
+        const int64_t lo = c->h_rank_off[r], hi = c->h_rank_off[r + 1];
+        cudaEvent_t ev;
+        if (hi > lo) {
+            CU(c, pool_event(c, (size_t)r, &ev));
+            CU(c, cudaStreamWaitEvent(st, ev, 0));  // the rank's tokens have landed
+            const int64_t t0 = N > 0 ? h_sample_ptr[h_rank_ptr[r]] : 0;
+            const int32_t *tok_base = c->hs_tokens.p + (size_t)(r % kRing) * tok_slot + (size_t)(t0 & 3) - t0;
+            for (int64_t cur = lo; cur < hi;) {
+                const int64_t end = std::min(hi, (cur / kColTile) * kColTile + piece);
+                const size_t slot = (size_t)(pi % kRing) * (size_t)piece;
+                if (pi >= kRing) {  // the staging piece is free once its previous contents have been copied back
+                    CU(c, pool_event(c, ev_piece0 + 2 * (size_t)(pi - kRing) + 1, &ev));
+                    CU(c, cudaStreamWaitEvent(st, ev, 0));
+                }
+                odb_outputs dev;
+                memset(&dev, 0, sizeof(dev));
+                // arena element a of this piece lives at staging element a - cur (cur is a multiple of 16)
+                dev.d_input_ids = c->hs_ids.p + slot - cur;
+                dev.d_labels = c->hs_labels.p + slot - cur;
+                dev.d_position_ids = c->hs_pos.p + slot - cur;
+                dev.d_attention_mask = c->hs_mask.p + slot - cur;
+                rc = collate_launch(c, tok_base, c->hs_span_lo.p, c->hs_span_hi.p, &dev, false, cur, end, 0, c->piece_ctr.p + pi, st);
+                if (rc != ODB_OK) {
+                    drain();
+                    return rc;
+                }
+                CU(c, pool_event(c, ev_piece0 + 2 * (size_t)pi, &ev));
+                CU(c, cudaEventRecord(ev, st));
+                CU(c, cudaStreamWaitEvent(c->d2h_stream, ev, 0));
+                const size_t n = (size_t)(end - cur);
+                CU(c, cudaMemcpyAsync(ho->d_input_ids + cur, c->hs_ids.p + slot, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
+                CU(c, cudaMemcpyAsync(ho->d_labels + cur, c->hs_labels.p + slot, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
+                CU(c, cudaMemcpyAsync(ho->d_position_ids + cur, c->hs_pos.p + slot, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
+                CU(c, cudaMemcpyAsync(ho->d_attention_mask + cur, c->hs_mask.p + slot, n, cudaMemcpyDeviceToHost, c->d2h_stream));
+                CU(c, pool_event(c, ev_piece0 + 2 * (size_t)pi + 1, &ev));
+                CU(c, cudaEventRecord(ev, c->d2h_stream));
+                cur = end;
+                ++pi;
             }
-            CU(c, cudaEventRecord(c->col_ev[r], st));
-            CU(c, cudaStreamWaitEvent(c->d2h_stream, c->col_ev[r], 0));
-            const size_t n = (size_t)(hi - lo);
-            CU(c, cudaMemcpyAsync(ho->d_input_ids + lo, c->hs_ids.p + lo, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
-            CU(c, cudaMemcpyAsync(ho->d_labels + lo, c->hs_labels.p + lo, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
-            CU(c, cudaMemcpyAsync(ho->d_position_ids + lo, c->hs_pos.p + lo, n * 4, cudaMemcpyDeviceToHost, c->d2h_stream));
-            CU(c, cudaMemcpyAsync(ho->d_attention_mask + lo, c->hs_mask.p + lo, n, cudaMemcpyDeviceToHost, c->d2h_stream));
+        }
+        CU(c, pool_event(c, (size_t)R + (size_t)r, &ev));
+        CU(c, cudaEventRecord(ev, st));  // rank r is collated: its token slot may be reused
+        if (uploaded < R) {
+            int urc = upload_rank(uploaded++);
+            if (urc != ODB_OK) {
+                drain();
+                return urc;
+            }
         }
     }
     if (c->timing) CU(c, cudaEventRecord(c->ev[2], st));

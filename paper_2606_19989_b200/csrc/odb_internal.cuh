@@ -280,7 +280,9 @@ struct odb_ctx {
     cudaStream_t copy_stream = nullptr;  // host -> device
     cudaStream_t d2h_stream = nullptr;   // device -> host
     cudaEvent_t copy_ev = nullptr;
-    std::vector<cudaEvent_t> tok_ev, col_ev;  // per rank: tokens landed / slots collated
+    std::vector<cudaEvent_t> ev_pool;         // odb_run_host: tokens landed / rank collated / piece collated / piece copied
+    odb::DevBuf<unsigned long long> piece_ctr;  // one work counter per output piece
+    int64_t host_staging_elems = 1ll << 25;   // arena elements per staging piece (ODB_OPT_HOST_STAGING_ELEMS)
     int64_t *h_rank_off = nullptr;            // pinned, R+1: arena offset of each rank's first slot
 };
 

@@ -344,7 +344,7 @@ def test_run_to_run_determinism(P):
         assert torch.equal(a.table(name), b.table(name))
 
 
-def _run_host_case(P, oracle, wl, ctx=None):
+def _run_host_case(P, oracle, wl, ctx=None, staging_elems=None):
     import torch
     plan, ref = oracle.run_workload(wl)
     toks_np = wl.tokens()
@@ -352,6 +352,8 @@ def _run_host_case(P, oracle, wl, ctx=None):
     pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a) if len(a) else np.zeros(1, a.dtype)).to(dt).pin_memory()
     own = ctx is None
     ctx = ctx or P.Odb(Par.gpu_params(wl), max(wl.n_samples, 1))
+    if staging_elems:
+        P.odb_set_option(ctx.h, P.ODB_OPT_HOST_STAGING_ELEMS, staging_elems)
     try:
         out = P.OutputBuffers(wl.n_ranks, plan.total_elems, plan.n_slots, plan.samples_emitted, plan.n_steps,
                               plan.samples_left, "cpu", fill=Par.SENTINEL)
@@ -397,6 +399,17 @@ def test_run_host_end_to_end(P, oracle, case):
     else:
         wl = I.protocol_workload(case, 2)
     _run_host_case(P, oracle, wl)
+
+
+@pytest.mark.parametrize("staging", [4096, 8192, 40_000, 1 << 20])
+def test_run_host_streams_through_fixed_size_staging(P, oracle, staging):
+    """The arenas are far larger than the device staging of odb_run_host (three pieces of `staging` elements; the
+    tokens go through a ring of three rank-sized buffers): 8 ranks -> the token ring wraps, hundreds of pieces."""
+    _run_host_case(P, oracle, I.make_workload(1), staging_elems=staging)
+    wl = I.protocol_workload("overflow_multiround", 5, join_mode=0)
+    wl.params["sample_quota"] = int(0.7 * wl.n_samples)
+    _run_host_case(P, oracle, wl, staging_elems=staging)
+    _run_host_case(P, oracle, I.protocol_workload("empty_rank", 2), staging_elems=staging)
 
 
 def test_run_host_reuses_context(P, oracle):
