@@ -24,7 +24,10 @@
  *   - Samples are laid out rank-major: rank r owns samples h_rank_ptr[r] .. h_rank_ptr[r+1]-1 in
  *     sampler order; a "local id" is the index inside the rank.
  *   - d_sample_ptr[g] .. d_sample_ptr[g+1] are the token offsets of global sample g in d_tokens and
- *     must equal the prefix sum of d_lengths.  d_tokens must be 16-byte aligned.
+ *     must equal the prefix sum of d_lengths.  d_tokens must be 16-byte aligned, and READABLE up to the
+ *     next multiple of 4 int32 past its last token: the collate kernel fetches tokens with aligned 16-byte
+ *     loads, so the vector that holds the last token is read whole (the extra words are discarded).
+ *     odb_run_host pads its own staging; callers of odb_collate / odb_run allocate round_up(n_tokens, 4).
  *   - Masked spans (labels -> ignore_index) are CSR per sample: spans d_span_ptr[g] .. d_span_ptr[g+1]-1,
  *     half-open [lo,hi) token positions, sorted and disjoint.
  *   - Every call returns an ODB_* status (0 = OK).  No exceptions, no abort, nothing printed.

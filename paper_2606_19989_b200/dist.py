@@ -118,22 +118,56 @@ class CudaEngine:
 # ---- the protocol ------------------------------------------------------------------------------
 def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=None) -> Generator[Request, object, tuple]:
     """Round loop of one process.  Returns (plan info of the local ranks, [T_grp of every emitting round]).
-    ``avail_schedule[j]`` (optional): arrived views of the LOCAL ranks at round j (odb_set_available)."""
+    ``avail_schedule[j]`` (optional): arrived views of the LOCAL ranks at round j (odb_set_available).
+
+    A process whose engine reports an error (a bad length, an invalid argument, a CUDA error) does NOT leave the
+    protocol on its own -- its peers would wait for ever in the next collective.  It stops calling its engine,
+    keeps issuing the round's collectives with buffers of the agreed sizes, and every round ends with a MAX
+    exchange of the error status: all processes then raise together (Lemma 3's "same collectives in the same
+    order whatever the data", extended to failures)."""
+    import torch
+    err = [0]
+    exc = [None]
+
+    def call(fn, *a):
+        if err[0]:
+            return None
+        try:
+            return fn(*a)
+        except B.OdbError as e:
+            err[0] = int(e.status) or B.ODB_ERR_STATE
+            exc[0] = e
+            return None
+
     wmax = yield ("max_int", int(engine.local_max_window()))
-    engine.dist_config(world_ranks, rank_offset, int(wmax))
+    call(engine.dist_config, world_ranks, rank_offset, int(wmax))
+    # the step-total window of a round has the same size in every process: T_grp <= the largest window of the job
+    cap = int(getattr(engine.params, "slot_capacity", 0) or 0)
+    window = max(1, min(int(wmax), cap) if cap > 0 else int(wmax))
+    dev = getattr(engine, "device", "cpu")
     round_T: List[int] = []
     j = 0
     while True:
         if avail_schedule is not None:
-            engine.set_available(avail_schedule[j] if j < len(avail_schedule) else None)
+            call(engine.set_available, avail_schedule[j] if j < len(avail_schedule) else None)
             j += 1
-        engine.form_groups()
-        world, local = engine.summary()
-        yield ("all_gather", world, local)                 # the per-round metadata exchange (P:52)
-        engine.align()                                      # Eq. 3 + termination predicates on the shared tensor
-        yield ("all_reduce_sum", engine.step_samples_window())   # global e_k (trainer-side count, P:347)
-        engine.commit()
-        done, T = engine.round_status()
+        call(engine.form_groups)
+        bufs = call(engine.summary)
+        if bufs is None:  # (the engine failed: stand-ins of the agreed sizes keep the collective well-formed)
+            bufs = (torch.zeros(2 * world_ranks, dtype=torch.int32, device=dev),
+                    torch.zeros(2 * engine.n_ranks, dtype=torch.int32, device=dev))
+        yield ("all_gather", bufs[0], bufs[1])              # the per-round metadata exchange
+        call(engine.align)                                  # Eq. 3 + termination predicates on the shared tensor
+        win = call(engine.step_samples_window)
+        if win is None or win.numel() != window:
+            win = torch.zeros(window, dtype=torch.int32, device=dev) if err[0] else win
+        yield ("all_reduce_sum", win)                       # global e_k (trainer-side count)
+        call(engine.commit)
+        st = call(engine.round_status)
+        worst = yield ("max_int", int(err[0]))              # does every process still stand?
+        if worst:
+            raise exc[0] if exc[0] is not None else B.OdbError(int(worst), "plan_protocol (a peer process failed)")
+        done, T = st
         if T > 0:
             round_T.append(T)
         if done:

@@ -13,7 +13,10 @@ class OracleEngine:
         self.o = oracle
         self.wl = wl
         self.p = wl.params
-        self.R = wl.n_ranks
+        self.params = SimpleNamespace(**wl.params)
+        self.R = self.n_ranks = wl.n_ranks
+        self.device = "cpu"
+        self.fail_at_round = None      # tests: raise an engine error in form_groups of that round
         self.lens = [wl.lengths[wl.rank_ptr[r]:wl.rank_ptr[r + 1]] for r in range(self.R)]
 
     def local_max_window(self):
@@ -43,6 +46,9 @@ class OracleEngine:
         self.arrived = None if h_arrived is None else [int(x) for x in h_arrived]
 
     def form_groups(self):
+        if self.fail_at_round is not None and self.round == self.fail_at_round:
+            from paper_2606_19989_b200 import binding as B
+            raise B.OdbError(B.ODB_ERR_BAD_LENGTH, "OracleEngine.form_groups (injected failure)")
         bs = self.p["buffer_size"]
         self.cand = []
         for r in range(self.R):

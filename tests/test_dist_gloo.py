@@ -63,6 +63,48 @@ def _worker(rank, world, port, q):
         dist.destroy_process_group()
 
 
+def _failing_worker(rank, world, port, q, fail_round):
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    import odb_inputs as I
+    from oracle import odb_oracle
+    from paper_2606_19989_b200 import dist as D
+    from paper_2606_19989_b200 import binding as B
+    from tests._oracle_engine import OracleEngine
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
+    try:
+        wl = _case("overflow_multiround")
+        rl = wl.n_ranks // world
+        eng = OracleEngine(odb_oracle, I.split_ranks(wl, world)[rank])
+        if rank == 1:
+            eng.fail_at_round = fail_round
+        try:
+            D.run(D.plan_protocol(eng, wl.n_ranks, rank * rl), D.TorchCollectives())
+            q.put((rank, "finished", 0))
+        except B.OdbError as e:
+            q.put((rank, "raised", int(e.status)))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("fail_round", [0, 3])
+def test_a_failing_process_takes_its_peers_down_instead_of_hanging_them(fail_round):
+    """One process's engine fails (a bad length, say) in some round: every process issues that round's collectives
+    and then raises, together (the MAX exchange of the error status at the end of every round)."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_failing_worker, args=(r, 2, port, q, fail_round)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = dict((item[0], item[1:]) for item in (q.get(timeout=120) for _ in range(2)))
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert got[0] == ("raised", 2) and got[1] == ("raised", 2)     # ODB_ERR_BAD_LENGTH on both
+
+
 def test_two_process_gloo_protocol_matches_whole_job_oracle():
     import torch.multiprocessing as mp
     sys.path.insert(0, ROOT)
