@@ -316,7 +316,8 @@ ODB_API int64_t odb_kernel_launches(const odb_ctx *ctx);
 
 /* Diagnostics: copy an internal device table to the host (synchronises).  `what`: 0 = G_r (int32[R])
  * of the last round, 1 = S_r (int32[R]), 2 = sorted keys of the last round ((len<<32)|id, uint64[N],
- * rank regions at h_rank_ptr).  Returns bytes copied or < 0. */
+ * rank regions at h_rank_ptr), 3 = views emitted so far per rank (int32[R]; valid between rounds of the staged calls).
+ * Returns bytes copied or < 0. */
 ODB_API int64_t odb_debug_read(odb_ctx *ctx, int what, void *h_dst, int64_t max_bytes);
 
 /* Synthetic-input utility (benchmarks / tests; not part of the method): d_tokens[j] for j in

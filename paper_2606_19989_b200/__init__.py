@@ -9,3 +9,4 @@ from .binding import (  # noqa: F401
     odb_outputs, odb_params, odb_plan_info, status_string,
 )
 from .batches import StepBatches  # noqa: F401,E402
+from .stream import WorkerPool, plan_online  # noqa: F401,E402

@@ -1248,6 +1248,7 @@ int64_t odb_debug_read(odb_ctx *c, int what, void *h_dst, int64_t max_bytes) {
     case 0: src = c->G; bytes = (int64_t)R * 4; break;
     case 1: src = c->S; bytes = (int64_t)R * 4; break;
     case 2: src = c->sorted; bytes = c->n_total * 8; break;
+    case 3: src = c->emit_cur; bytes = (int64_t)R * 4; break;
     default: return -1;
     }
     if (!src) return -1;

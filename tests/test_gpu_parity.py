@@ -535,6 +535,30 @@ def test_arrival_random_schedules(P, oracle):
             _sched_parity(oracle, wl, _random_schedule(rng, wl, 9))
 
 
+@pytest.mark.parametrize("latency,rate", [(0, None), (2, None), (3, 50)])
+def test_online_run_against_worker_pool_model(P, oracle, latency, rate):
+    """plan_online: the protocol rounds against the worker-pool model (outstanding-depth envelope D = max(pf * nw,
+    buffer_size); skip rounds while nothing has been delivered, Lemma 2) -- the plan and the arenas are the
+    oracle's under the arrival schedule the run saw, and the envelope holds in every round."""
+    for kind in ("overflow_multiround", "empty_rank", "unequal"):
+        wl = I.protocol_workload(kind, 7)
+        n = np.diff(wl.rank_ptr)
+        bs = wl.params["buffer_size"] or int(n.max())
+        pool = P.WorkerPool.from_loader(n, prefetch_factor=4, num_workers=2, buffer_size=bs, latency=latency, rate=rate)
+        dw = Par.DeviceWorkload(wl)
+        with P.Odb(Par.gpu_params(wl), max(wl.n_samples, 1)) as ctx:
+            info, log = P.plan_online(ctx, dw.lengths, wl.rank_ptr, pool)
+            out = P.OutputBuffers.for_plan(wl.n_ranks, info, dw.device, fill=Par.SENTINEL)
+            P.odb_collate(ctx.h, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out.struct)
+        sched = np.array([e["arrived"] for e in log])
+        plan, ref = oracle.run_workload(wl, avail_schedule=sched)
+        Par.compare_plan(plan, info, out, [e["T"] for e in log if e["T"] > 0])
+        Par.compare_full(plan, ref, info, out)
+        assert all((e["outstanding"] <= pool.depth).all() for e in log)
+        if latency:
+            assert log[0]["T"] == 0 and not (log[0]["arrived"] > 0).any()      # a skip round: nothing delivered yet
+
+
 def test_set_available_state_errors(P):
     wl = I.make_workload(0)
     dw = Par.DeviceWorkload(wl)
