@@ -64,6 +64,10 @@ def parse_args():
     ap.add_argument("--pipeline", type=int, default=0,
                     help="measure N contexts driven round-robin on N streams (planning of one step beside the collate "
                          "kernel of another); extra key 'pipelined'")
+    ap.add_argument("--host-staging-elems", type=int, default=None,
+                    help="arena elements per device staging piece of odb_run_host (ODB_OPT_HOST_STAGING_ELEMS)")
+    ap.add_argument("--collate-bulk", action="store_true",
+                    help="time the bulk-store (cp.async.bulk) form of the collate kernel instead of the adopted one")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -387,6 +391,8 @@ def run_ours(args):
     result = {}
     with P.Odb(gpu_params(P, wl), max(wl.n_samples, 1), device=local) as ctx:
         P.odb_set_timing(ctx.h, True)
+        if args.collate_bulk:
+            P.odb_set_option(ctx.h, P.ODB_OPT_COLLATE_BULK_STORES, 1)
         info = ctx.plan(din.lengths, wl.rank_ptr)
         out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
         sampler = ClockSampler(local)
@@ -488,11 +494,16 @@ def run_ours(args):
                 del out
                 torch.cuda.empty_cache()
                 barrier()
+                if args.host_staging_elems:
+                    P.odb_set_option(ctx.h, P.ODB_OPT_HOST_STAGING_ELEMS, args.host_staging_elems)
                 dt, h2d, d2h = time_e2e(P, ctx, wl, din, info, args.e2e_steps, device)
                 dt = max_over_ranks(dt)
                 result["e2e"] = {"value": world * n_samples / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                                  "d2h_bytes_per_step": d2h, "ms_per_step": dt * 1e3, "steps": args.e2e_steps,
                                  "tokens_per_s": world * n_tok / dt, "pcie_gbs": (h2d + d2h) / dt / 1e9,
+                                 "d2h_gbs": d2h / dt / 1e9, "h2d_gbs_if_alone": h2d / dt / 1e9,
+                                 "device_staging": "token ring 3 x one rank, output ring 3 x %d elements (13 B each)" % (
+                                     args.host_staging_elems or (1 << 25)),
                                  "api": "odb_run_host (pinned host buffers in and out)"}
     del din
     torch.cuda.empty_cache()
