@@ -808,6 +808,7 @@ def paper_operating_point(P, device, peak):
     row["workload"] = "configs[4] CV 1 L 65536, buffer_size 1024 (P:28)"
     row["frac"] = row["collate_gbs"] / peak if row["collate_gbs"] else None
     row["whole_step_frac"] = row["whole_step_gbs"] / peak
+    row["traffic"] = ncu_traffic(cell_key(4, 1.0, 65536, 0, 1024))
     return row
 
 
