@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(const PrepArgs A) {
 //   boundary chunk (slot change, alignment gap, block end, end of arena): the per-vector generic
 //   path (4-element vectors, scalar loads, 4-byte mask stores).
 //
-// Work distribution: persistent CTAs take runs of kColGrab tiles from an atomic counter.
+// Work distribution: persistent CTAs take runs of up to kColGrab tiles from an atomic counter.
 // A11: valid-token counts are integer sums: warp reduce, one atomicAdd per chunk and slot.
 // ---------------------------------------------------------------------------------------------
 struct RowRegs {
@@ -442,13 +442,18 @@ __global__ void __launch_bounds__(kColThreads, 3) k_collate(const CollateArgs A)
         total_elems = A.dims->total_elems;
         tile_hi = (total_elems + kColTile - 1) / kColTile;
     }
+    // tiles taken from the work counter at a time: kColGrab when there is plenty of work (the measured optimum on the
+    // large configs), fewer when the launch holds only a few runs per CTA, so that small launches do not end with
+    // half of the CTAs idle (configs[1] has 1.2 runs of 16 per CTA)
+    const int64_t n_tiles_all = tile_hi - A.tile_lo;
+    const int grab = (int)max((int64_t)1, min((int64_t)kColGrab, n_tiles_all / ((int64_t)gridDim.x * 8)));
     for (;;) {
         __syncthreads();  // everyone has read the previous s_grab
-        if (threadIdx.x == 0) s_grab = (long long)atomicAdd(A.tile_counter, (unsigned long long)kColGrab);
+        if (threadIdx.x == 0) s_grab = (long long)atomicAdd(A.tile_counter, (unsigned long long)grab);
         __syncthreads();
         const int64_t tile_begin = A.tile_lo + s_grab;
         if (tile_begin >= tile_hi) break;
-        const int64_t tile_end = min(tile_begin + kColGrab, tile_hi);
+        const int64_t tile_end = min(tile_begin + grab, tile_hi);
 #pragma unroll 1
         for (int64_t tile = tile_begin; tile < tile_end; ++tile) {
             const int64_t chunk = tile * kWarps + warp;

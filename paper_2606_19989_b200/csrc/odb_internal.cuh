@@ -25,7 +25,7 @@ constexpr int kCommitParts = 4;     // CTAs per rank that share k_commit's scan-
 constexpr size_t kFormSmemLimit = 231424;  // dynamic shared memory of k_form_groups_smem (227 KB - static)
 constexpr int kAlignSmemKeys = 8192;       // overflow sort keys kept in shared memory by k_align
 constexpr int kFinThreads = 512;           // k_fin_scan: tile = kFinThreads * kFinItems slots
-constexpr int kFinItems = 4;
+constexpr int kFinItems = 1;
 constexpr int kFinTile = kFinThreads * kFinItems;
 constexpr int kColThreads = 256;    // collate CTA (A10)
 constexpr int kColTile = 4096;      // arena elements per collate tile (one CTA iteration)

@@ -98,12 +98,12 @@ def test_config4_full_size_every_element(P, oracle, rule, join):
         assert plan.stop_reason == 2 and plan.samples_left > 0
 
 
-@pytest.mark.parametrize("cv,budget", [(1.0, 65536), (2.5, 16384)])
-def test_config5_full_size_every_element(P, oracle, cv, budget):
+@pytest.mark.parametrize("cv,budget,rule", [(1.0, 65536, 0), (2.5, 16384, 0), (0.3, 262144, 0), (1.0, 65536, 1)])
+def test_config5_full_size_every_element(P, oracle, cv, budget, rule):
     """BASELINE.json configs[4] at full size (32 x 32768 samples, 2.1e9 tokens, 28 GB of outputs; element offsets
     exceed 2^31): the cell bench.py is quoted on (CV 1.0 / L 65536) and the CV 2.5 / L 16384 cell (over-budget
     singletons of up to ~270 K tokens), every element of every slot, rank by rank."""
-    plan = _full_size_elementwise(oracle, I.make_workload(4, cv=cv, budget=budget))
+    plan = _full_size_elementwise(oracle, I.make_workload(4, cv=cv, budget=budget, rule=rule))
     assert plan.total_elems > 2**31
 
 
