@@ -298,8 +298,13 @@ ODB_API int odb_offline_plan(odb_ctx *ctx, const odb_offline_params *params, con
  * streaming stores from registers.  Same results bit for bit; the measured comparison is in profiles/.
  * ODB_OPT_HOST_STAGING_ELEMS (value >= 1, default 2^25): arena elements per device staging piece of odb_run_host
  * (three pieces of 13 bytes per element are held; rounded down to a multiple of 4096, at least 4096).
+ * ODB_OPT_ROUND_PARALLEL (value 0 / 1, default 1): with a grouping buffer of 8 .. 4096 samples (the paper's
+ * operating point) odb_run forms and commits the protocol rounds round-parallel -- a round depends on its
+ * predecessors only through the leftovers, and there are none until a round overflows -- and the
+ * sequential round loop resumes at the first round that does; 0 = every round in the sequential loop.  Same
+ * results bit for bit.
  * ODB_ERR_INVALID_ARG for an unknown option. */
-enum { ODB_OPT_COLLATE_BULK_STORES = 1, ODB_OPT_HOST_STAGING_ELEMS = 2 };
+enum { ODB_OPT_COLLATE_BULK_STORES = 1, ODB_OPT_HOST_STAGING_ELEMS = 2, ODB_OPT_ROUND_PARALLEL = 3 };
 ODB_API int odb_set_option(odb_ctx *ctx, int option, int64_t value);
 
 /* Bandwidth probes (measurement utility, not part of the method): the collate kernel's byte mix -- 4 bytes read
@@ -316,7 +321,9 @@ ODB_API int64_t odb_kernel_launches(const odb_ctx *ctx);
 
 /* Diagnostics: copy an internal device table to the host (synchronises).  `what`: 0 = G_r (int32[R])
  * of the last round, 1 = S_r (int32[R]), 2 = sorted keys of the last round ((len<<32)|id, uint64[N],
- * rank regions at h_rank_ptr), 3 = views emitted so far per rank (int32[R]; valid between rounds of the staged calls).
+ * rank regions at h_rank_ptr), 3 = views emitted so far per rank (int32[R]; valid between rounds of the staged calls),
+ * 4 = the record of the round-parallel planner of the last odb_run (int32[4]: rounds it committed, steps they emit,
+ * 1 if it ended the protocol, 0; < 0 is returned when that run did not use it).
  * Returns bytes copied or < 0. */
 ODB_API int64_t odb_debug_read(odb_ctx *ctx, int what, void *h_dst, int64_t max_bytes);
 

@@ -129,6 +129,7 @@ static void free_all(odb_ctx *c) {
     if (c->copy_ev) cudaEventDestroy(c->copy_ev);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     c->piece_ctr.release();
+    c->spec_tab.release();
     if (c->h_rank_off) cudaFreeHost(c->h_rank_off);
 }
 
@@ -182,11 +183,11 @@ int odb_create(const odb_params *p, int device, int64_t max_samples_total, odb_c
     if (e == cudaSuccess) e = dev_alloc(&c->mark, N + R);
     if (e == cudaSuccess) e = dev_alloc(&c->posflag, N);
     if (e == cudaSuccess) e = dev_alloc(&c->emit_pos, N);
-    if (e == cudaSuccess) e = dev_alloc(&c->gpos, N + R);
-    if (e == cudaSuccess) e = dev_alloc(&c->agpos, N + R);
-    if (e == cudaSuccess) e = dev_alloc(&c->agcnt, N + R);
-    if (e == cudaSuccess) e = dev_alloc(&c->agoff, N + R);
-    if (e == cudaSuccess) e = dev_alloc(&c->agorg, N + R);
+    if (e == cudaSuccess) e = dev_alloc(&c->gpos, plan_table_entries(N, R));
+    if (e == cudaSuccess) e = dev_alloc(&c->agpos, plan_table_entries(N, R));
+    if (e == cudaSuccess) e = dev_alloc(&c->agcnt, plan_table_entries(N, R));
+    if (e == cudaSuccess) e = dev_alloc(&c->agoff, plan_table_entries(N, R));
+    if (e == cudaSuccess) e = dev_alloc(&c->agorg, plan_table_entries(N, R));
     if (e == cudaSuccess) e = dev_alloc(&c->left_ids, N);
     if (e == cudaSuccess) e = dev_alloc(&c->emit_ids, N);
     if (e == cudaSuccess) e = dev_alloc(&c->n_left, R);
@@ -244,6 +245,7 @@ int odb_reset(odb_ctx *c) {
     c->offline = false;
     c->offline_perm = nullptr;
     c->d_lengths = nullptr;
+    c->spec_used = false;
     return ODB_OK;
 }
 
@@ -299,6 +301,7 @@ int odb_set_option(odb_ctx *c, int option, int64_t value) {
     if (!c) return ODB_ERR_INVALID_ARG;
     switch (option) {
     case ODB_OPT_COLLATE_BULK_STORES: c->collate_bulk = value != 0; return ODB_OK;
+    case ODB_OPT_ROUND_PARALLEL: c->round_parallel = value != 0; return ODB_OK;
     case ODB_OPT_HOST_STAGING_ELEMS:
         if (value < 1) return ODB_ERR_INVALID_ARG;
         c->host_staging_elems = value;
@@ -879,8 +882,19 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
             CU(c, grow_preserve(c->step_samples, (size_t)steps_bound, 0, st));
             c->step_cap = steps_bound;
         }
-        cudaError_t le = launch_rounds(c, st);
+        // rounds that are certainly not the terminal check (join: some stream still holds views; non-join: every
+        // stream does): formed and committed round-parallel as long as no round overflows (odb_plan.cu)
+        int64_t spec_rounds = 0;
+        if (c->round_parallel && c->prm.buffer_size >= kSpecMinWindow && (c->prm.join_mode || c->prm.sample_quota <= 0)) {
+            const int64_t B = c->prm.buffer_size;
+            int64_t min_nr = max_nr;
+            for (int r = 0; r < R; ++r) min_nr = std::min(min_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
+            spec_rounds = ((c->prm.join_mode ? max_nr : min_nr) + B - 1) / B;
+            if (spec_rounds < 2 || spec_rounds > kSpecMaxRounds) spec_rounds = 0;
+        }
+        cudaError_t le = launch_rounds(c, (int)spec_rounds, st);
         if (le == cudaSuccess) {
+            c->spec_used = spec_rounds > 0;
             c->begin_pending = false;
             rc = enqueue_tail(c, steps_bound, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
             if (rc != ODB_OK) return rc;
@@ -1249,6 +1263,7 @@ int64_t odb_debug_read(odb_ctx *c, int what, void *h_dst, int64_t max_bytes) {
     case 1: src = c->S; bytes = (int64_t)R * 4; break;
     case 2: src = c->sorted; bytes = c->n_total * 8; break;
     case 3: src = c->emit_cur; bytes = (int64_t)R * 4; break;
+    case 4: src = c->spec_used ? c->spec_tab.p : nullptr; bytes = 16; break;
     default: return -1;
     }
     if (!src) return -1;

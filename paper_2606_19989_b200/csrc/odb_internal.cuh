@@ -62,6 +62,16 @@ struct PlanDims {
     int64_t samples_left;
 };
 
+// Result of the speculative, round-parallel planner (k_spec_form): the protocol rounds [0, j_star) have been
+// formed under the assumption "no leftovers so far", which holds as long as no round overflows; round j_star
+// is the first that does (the sequential round loop resumes there) or the terminal check (complete = 1).
+struct SpecRec {
+    int32_t j_star;    // rounds committed by k_spec_commit
+    int32_t n_steps;   // steps those rounds emit (sum of their T)
+    int32_t complete;  // 1 = round j_star is the terminal check: the protocol is over
+    int32_t pad_;
+};
+
 // The caller's output capacities, checked on the device by the slot scan (odb_run enqueues the collate
 // kernels before the host has seen the plan sizes).
 struct CapCheck {
@@ -190,6 +200,10 @@ struct odb_ctx {
     bool no_rounds_kernel = false; // the persistent round-loop kernel could not be launched on this device
     int rounds_max_ctas = 0;       // resident CTAs of k_rounds on this device (0 = not asked yet, -1 = no cooperative launch)
     int32_t *gs_rounds = nullptr;  // k_rounds: the double-buffered per-round summary + the grid-barrier counter
+    odb::DevBuf<int32_t> spec_tab;  // round-parallel planner: SpecRec, per-round T / step base / arrival counters, G table
+    int spec_occ = 0;               // k_spec_form's shared-memory attribute is set
+    bool round_parallel = true;     // odb_set_option(ODB_OPT_ROUND_PARALLEL)
+    bool spec_used = false;         // the last run went through the round-parallel planner (spec_tab holds its SpecRec)
 
     // inputs fixed by the first odb_form_groups after create / reset
     const int32_t *d_lengths = nullptr;
@@ -295,7 +309,14 @@ cudaError_t launch_round_form(odb_ctx *c, cudaStream_t st);   // A0..A3
 cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st);
 cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commit (single-process mode)
 // every protocol round in one cooperative launch; cudaErrorNotSupported if R CTAs cannot be resident
-cudaError_t launch_rounds(odb_ctx *c, cudaStream_t st);
+// `spec_rounds` > 0: the rounds [0, spec_rounds) are first formed and committed round-parallel (k_spec_form /
+// k_spec_commit) and the persistent kernel resumes where that speculation stops
+cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st);
+// scratch entries per rank-sized table (gpos, agpos, ...): every (rank, round) window of the round-parallel
+// planner owns S + 1 entries
+inline size_t plan_table_entries(size_t N, size_t R) { return N + N / 8 + 2 * R + 64; }
+constexpr int kSpecMinWindow = 8;       // smallest buffer_size the round-parallel planner takes
+constexpr int kSpecMaxRounds = 65535;   // (gridDim.y)
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: (G_r, S_r) pairs for the all_gather
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce

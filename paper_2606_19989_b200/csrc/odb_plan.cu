@@ -1048,6 +1048,7 @@ struct RoundsArgs {
     int32_t *gs;  // [2][2 R]: the per-round summary, double-buffered by round parity
     unsigned int *bar;
     PlanDims *dims;
+    const SpecRec *spec;  // non-NULL: the rounds [0, spec->j_star) were committed by the round-parallel planner
 };
 
 // dynamic shared memory of k_rounds: the sort buffer (also scratch of the list ranking and of the overflow
@@ -1067,17 +1068,33 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
     int32_t *s_ap = s_gp + (kMsChunk + 4), *s_ac = s_ap + (kMsChunk + 4), *s_ag = s_ac + (kMsChunk + 4);
     const int r = blockIdx.x, t = threadIdx.x, R = A.R;
     const SortArgs &SA = A.sort;
-    ms_first_round_init(SA, (int64_t)r * kMsThreads + t, (int64_t)gridDim.x * kMsThreads);
+    if (SA.first) ms_first_round_init(SA, (int64_t)r * kMsThreads + t, (int64_t)gridDim.x * kMsThreads);
     const int64_t base = SA.rank_ptr[r];
     const int n_r = (int)(SA.rank_ptr[r + 1] - base);
     const int64_t jb = base + r;
-    if (t < 3) s_state[t] = 0;
-    __syncthreads();
     unsigned int n_bar = 0;
-    int n_steps = 0, n_rounds = 0, stop = 0, bad = 0;
+    int n_steps = 0, n_rounds = 0, stop = 0, bad = 0, round0 = 0;
+    bool run_loop = true;
+    if (t < 3) s_state[t] = 0;
+    if (A.spec) {
+        // resume behind the round-parallel planner: no leftovers so far, every rank has fetched round0 windows
+        round0 = __ldcg(&A.spec->j_star);
+        n_steps = __ldcg(&A.spec->n_steps);
+        const int fp0 = (int)min((long long)round0 * SA.buffer_size, (long long)n_r);
+        if (t == 1 || t == 2) s_state[t] = fp0;  // fetch_pos, emit_cur
+        if (t == 0) bad = __ldcg(&SA.rec->bad_length);
+        bad = __syncthreads_or(bad);
+        if (bad) run_loop = false;
+        else if (__ldcg(&A.spec->complete)) {  // round0 is the terminal check
+            stop = A.join_mode ? ODB_STOP_ALL_FINISHED : ODB_STOP_LOGICAL;
+            n_rounds = round0 + 1;
+            run_loop = false;
+        }
+    }
+    __syncthreads();
     long long emitted_before = A.emitted_before;
     const bool quota_mode = !A.join_mode && A.quota > 0;
-    for (int round = 0;; ++round) {
+    for (int round = round0; run_loop; ++round) {
         // ---- A0 + A1: this rank's window, sorted ----
         const int nl = s_state[0], fp = s_state[1], cur = s_state[2];
         const int S = ms_window_size(nl, fp, n_r, SA.buffer_size);
@@ -1110,7 +1127,7 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
             }
             if (sq < 0) atomicAdd(&s_red[2], 1);
         }
-        if (round == 0 && t == 0) bad = __ldcg(&SA.rec->bad_length);
+        if (round == 0 && t == 0) bad = __ldcg(&SA.rec->bad_length);  // (a resumed run has checked it above)
         bad = __syncthreads_or(bad);
         if (bad) break;
         const int n_fin = s_red[2];
@@ -1178,6 +1195,179 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
             A.dims->complete = bad ? 0 : 1;
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The protocol rounds ROUND-PARALLEL (A0 .. A8 for every round at once).  The round loop above keeps one CTA per
+// rank busy and leaves the other SMs idle; at the paper's operating point (a 1024-sample grouping buffer,
+// P:28) a rank stream is tens of rounds.  But a round only depends on its predecessors through the leftovers
+// ("returned to the buffer") -- and there are none as long as no round overflows: splitting (T >= G_r)
+// emits every sample of the window (Lemma 1).  Under that assumption round j of rank r drains exactly the
+// views [j B, (j + 1) B) of its stream, so ALL windows of ALL rounds can be sorted and grouped at once:
+//   k_spec_form    one CTA per (rank, round): window fill + sort + candidate groups (the device functions of the
+//                  round loop); the last CTA of a round to arrive evaluates Eq. 3 on the round's (G_r, S_r) and
+//                  checks the assumption for the NEXT round (nobody overflows: max_A G_r <= min(C+min, S+min));
+//                  the last CTA of the launch finds j* = the first round that breaks it and scans the step bases;
+//   k_spec_commit  one CTA per (rank, round < j*): split + commit (align_body / commit_body as they are);
+//   k_rounds       resumes at round j* with the state those rounds leave behind (or only records the plan sizes
+//                  when j* is the terminal check).
+// The rounds that are terminal checks are known on the host (join: the first round in which every stream is
+// drained; non-join without a quota: the first in which one is), so the grid holds only non-terminal rounds.
+// Not used with a sample quota (the cut needs the running emitted count), with arrival schedules, or in
+// distributed mode.  Results are those of the sequential loop by construction; tests compare both with the oracle.
+// ---------------------------------------------------------------------------------------------
+struct SpecArgs {
+    SortArgs sort;
+    int R, n_rounds;
+    uint32_t budget;
+    int rule, join_mode, slot_capacity;
+    int x_keys;  // padded sort keys the shared-memory layout reserves
+    int32_t *gpos, *agpos, *agcnt, *agorg;
+    int32_t *st_count, *st_width, *st_real, *st_round, *st_origin;
+    int32_t *emit_ids, *left_ids_w;
+    SpecRec *rec;
+    int32_t *T_tab, *sb_tab, *G_tab;
+    unsigned int *ctr;  // [0, n_rounds): arrivals per round; [kSpecMaxRounds]: rounds closed (all self-resetting)
+};
+
+// first scratch entry of window (r, j): every non-empty window of S samples owns S + 1 entries
+__device__ __forceinline__ int64_t spec_off(int64_t base, int B, int r, int j) {
+    return base + (base + B - 1) / B + r + (int64_t)j * (B + 1);
+}
+
+__global__ void __launch_bounds__(kMsThreads) k_spec_form(const SpecArgs A) {
+    extern __shared__ __align__(16) unsigned char sp_smem[];
+    __shared__ int s_scan[34];
+    __shared__ uint16_t s_e2[32];
+    __shared__ int s_red[2];
+    __shared__ int s_flag;
+    const SortArgs &SA = A.sort;
+    const int r = blockIdx.x, j = blockIdx.y, t = threadIdx.x, R = A.R, B = SA.buffer_size;
+    ms_first_round_init(SA, ((int64_t)j * R + r) * blockDim.x + t, (int64_t)gridDim.x * gridDim.y * blockDim.x);
+    const int64_t base = SA.rank_ptr[r];
+    const int n_r = (int)(SA.rank_ptr[r + 1] - base);
+    const int fp = (int)min((long long)j * B, (long long)n_r);
+    const int S = min(B, n_r - fp);
+    int G = 0;
+    if (S > 0) {
+        uint64_t *X = reinterpret_cast<uint64_t *>(sp_smem);
+        uint64_t *K = X + A.x_keys;
+        int32_t *gp = reinterpret_cast<int32_t *>(K + B);
+        uint64_t k[kMsItems];
+        const int n_keys = ms_active_keys(S);
+        ms_load_keys(SA, base, 0, fp, 0, S, n_keys, k);
+        ms_sort_cta(k, X, n_keys);
+        uint64_t *out = SA.keys_out + base + fp;
+        for (int i = t; i < S; i += blockDim.x) {
+            const uint64_t key = X[ms_pad(i)];
+            K[i] = key;
+            out[i] = key;
+        }
+        __syncthreads();
+        G = form_hier_body(K, S, A.budget, A.rule, gp, sp_smem, s_scan, s_e2);
+        __syncthreads();
+        int32_t *gpo = A.gpos + spec_off(base, B, r, j);
+        for (int i = t; i <= G; i += blockDim.x) gpo[i] = gp[i];
+    }
+    if (t == 0) __stcg(&A.G_tab[(int64_t)j * R + r], G);
+    // ---- the last CTA of round j to arrive: Eq. 3 and the no-overflow check ----
+    __threadfence();
+    __syncthreads();
+    if (t == 0) {
+        s_flag = atomicAdd(&A.ctr[j], 1u) == (unsigned int)(R - 1);
+        s_red[0] = 0;
+        s_red[1] = 0x7fffffff;
+    }
+    __syncthreads();
+    if (!s_flag) return;
+    __threadfence();
+    for (int q = t; q < R; q += blockDim.x) {
+        const int g = __ldcg(&A.G_tab[(int64_t)j * R + q]);
+        if (g > 0) {  // active set A = {r : G_r > 0}; its windows are non-empty
+            const int64_t bq = SA.rank_ptr[q];
+            const int nq = (int)(SA.rank_ptr[q + 1] - bq);
+            const int sq = min(B, nq - (int)min((long long)j * B, (long long)nq));
+            atomicMax(&s_red[0], g);
+            atomicMin(&s_red[1], sq);
+        }
+    }
+    __syncthreads();
+    if (t == 0) {
+        const int maxG = s_red[0];
+        const int T = target_groups(maxG, s_red[1], A.slot_capacity);
+        // every rank splits up to T (or idles): nothing is dropped, the next round starts without leftovers
+        __stcg(&A.T_tab[j], T == maxG ? T : -1);
+        A.ctr[j] = 0u;
+        __threadfence();
+        s_flag = atomicAdd(&A.ctr[kSpecMaxRounds], 1u) == (unsigned int)(A.n_rounds - 1);
+        s_red[0] = A.n_rounds;
+    }
+    __syncthreads();
+    if (!s_flag) return;
+    // ---- the last CTA of the launch: j* and the step bases ----
+    __threadfence();
+    for (int q = t; q < A.n_rounds; q += blockDim.x)
+        if (__ldcg(&A.T_tab[q]) < 0) atomicMin(&s_red[0], q);
+    __syncthreads();
+    const int js = s_red[0];
+    int carry = 0;
+    for (int q0 = 0; q0 < js; q0 += blockDim.x) {
+        const int q = q0 + t;
+        const int v = q < js ? __ldcg(&A.T_tab[q]) : 0;
+        int tot;
+        const int ex = block_excl_scan<int>(v, s_scan, tot);
+        if (q < js) A.sb_tab[q] = carry + ex;
+        carry += tot;
+    }
+    if (t == 0) {
+        A.rec->j_star = js;
+        A.rec->n_steps = carry;
+        A.rec->complete = js == A.n_rounds ? 1 : 0;
+        A.rec->pad_ = 0;
+        A.ctr[kSpecMaxRounds] = 0u;
+    }
+}
+
+__global__ void __launch_bounds__(kMsThreads) k_spec_commit(const SpecArgs A) {
+    __shared__ RoundRec s_rec;
+    __shared__ int s_state[3];
+    const SortArgs &SA = A.sort;
+    const int r = blockIdx.x, j = blockIdx.y, t = threadIdx.x, R = A.R, B = SA.buffer_size;
+    if (j >= A.rec->j_star) return;
+    const int T = A.T_tab[j], sb = A.sb_tab[j], G = A.G_tab[(int64_t)j * R + r];
+    const int64_t base = SA.rank_ptr[r];
+    const int n_r = (int)(SA.rank_ptr[r + 1] - base);
+    const int fp = (int)min((long long)j * B, (long long)n_r);
+    const int S = min(B, n_r - fp);
+    const int64_t off = spec_off(base, B, r, j);
+    if (t == 0) {
+        s_rec.T = T;
+        s_rec.done = 0;
+        s_rec.n_finished = 0;
+        s_state[0] = 0;
+        s_state[1] = fp;
+        s_state[2] = fp;
+    }
+    // A5: split up to T (G <= T in every committed round: the overflow branch is never taken)
+    if (G > 0) align_body(S, G, T, A.gpos + off, A.agpos + off, A.agcnt + off, A.agorg + off, nullptr, SA.step_samples + sb);
+    __syncthreads();
+    RankView V;
+    V.k = SA.keys_out + base + fp;
+    V.ap = A.agpos + off;
+    V.ac = A.agcnt + off;
+    V.ag = A.agorg + off;
+    V.ao = nullptr;
+    V.pf = nullptr;
+    V.S = S;
+    V.Gr = G;
+    V.cur = fp;
+    V.n_r = n_r;
+    V.base = base;
+    V.n_left = &s_state[0];
+    V.fetch_pos = &s_state[1];
+    V.emit_cur = &s_state[2];
+    commit_body(r, R, V, SA.step_samples, sb, j, A.join_mode, 0ll, 0ll, A.st_count, A.st_width, A.st_real, A.st_round,
+                A.st_origin, A.emit_ids, SA.emit_pos, A.left_ids_w, &s_rec, true, 0, 1);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1567,7 +1757,13 @@ cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
 
 // The whole round loop in one cooperative launch (k_rounds).  cudaErrorNotSupported when the R CTAs cannot
 // all be resident on this device (the caller then drives the rounds from the host).
-cudaError_t launch_rounds(odb_ctx *c, cudaStream_t st) {
+static int host_active_keys(int S) {
+    int n = 32 * kMsItems;
+    while (n < S) n <<= 1;
+    return std::min(n, kMsChunk);
+}
+
+cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const size_t smem = kRoundsSmem;
     if (c->rounds_max_ctas == 0) {
@@ -1633,6 +1829,56 @@ cudaError_t launch_rounds(odb_ctx *c, cudaStream_t st) {
     A.gs = c->gs_rounds;
     A.bar = bar;
     A.dims = c->d_dims;
+    A.spec = nullptr;
+    if (spec_rounds > 0) {
+        // the rounds [0, spec_rounds) round-parallel; k_rounds resumes where the speculation stops
+        const int B = c->prm.buffer_size;
+        const int n_keys = host_active_keys(B);
+        const int threads = std::max(n_keys / kMsItems, 128);
+        const size_t x_keys = (size_t)n_keys + n_keys / kMsItems;
+        const size_t x_bytes = std::max(x_keys * 8, (form_hier_smem_bytes(B) + 15) & ~(size_t)15);
+        const size_t sp_smem = x_bytes + (size_t)B * 8 + ((size_t)B + 4) * 4;
+        if (!c->spec_occ) {
+            cudaError_t ae = cudaFuncSetAttribute(k_spec_form, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(96 * 1024));
+            if (ae != cudaSuccess) return ae;
+            c->spec_occ = 1;
+        }
+        const size_t tab_fixed = 4 + (size_t)kSpecMaxRounds + 1;
+        e = c->spec_tab.ensure(tab_fixed + 2 * ((size_t)kSpecMaxRounds + 1) + (size_t)spec_rounds * R, true, st);
+        if (e != cudaSuccess) return e;
+        SpecArgs P;
+        memset(&P, 0, sizeof(P));
+        P.sort = A.sort;
+        P.R = R;
+        P.n_rounds = spec_rounds;
+        P.budget = A.budget;
+        P.rule = A.rule;
+        P.join_mode = A.join_mode;
+        P.slot_capacity = A.slot_capacity;
+        P.x_keys = (int)(x_bytes / 8);
+        P.gpos = c->gpos;
+        P.agpos = c->agpos;
+        P.agcnt = c->agcnt;
+        P.agorg = c->agorg;
+        P.st_count = A.st_count;
+        P.st_width = A.st_width;
+        P.st_real = A.st_real;
+        P.st_round = A.st_round;
+        P.st_origin = A.st_origin;
+        P.emit_ids = c->emit_ids;
+        P.left_ids_w = c->left_ids;
+        P.rec = reinterpret_cast<SpecRec *>(c->spec_tab.p);
+        P.ctr = reinterpret_cast<unsigned int *>(c->spec_tab.p + 4);
+        P.T_tab = c->spec_tab.p + tab_fixed;
+        P.sb_tab = P.T_tab + kSpecMaxRounds + 1;
+        P.G_tab = P.sb_tab + kSpecMaxRounds + 1;
+        k_spec_form<<<dim3((unsigned)R, (unsigned)spec_rounds), threads, sp_smem, st>>>(P);
+        ODB_LAUNCH_CHECK(c);
+        k_spec_commit<<<dim3((unsigned)R, (unsigned)spec_rounds), threads, 0, st>>>(P);
+        ODB_LAUNCH_CHECK(c);
+        A.sort.first = 0;
+        A.spec = P.rec;
+    }
     void *args[] = {(void *)&A};
     e = cudaLaunchCooperativeKernel((const void *)k_rounds, dim3((unsigned)R), dim3(kMsThreads), args, smem, st);
     if (e != cudaSuccess) return e;

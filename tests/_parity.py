@@ -44,15 +44,20 @@ def gpu_params(wl):
                          ignore_index=p["ignore_index"], shift_labels=p["shift_labels"])
 
 
-def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL, avail_schedule=None, bulk_stores=False):
+def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL, avail_schedule=None, bulk_stores=False, options=None,
+            spec_rec=None):
     """Returns (info, OutputBuffers, round_T).  staged=True uses form_groups/align/round_status/
-    plan_query/collate; staged=False uses odb_run (two calls: the first sizes the outputs)."""
+    plan_query/collate; staged=False uses odb_run (two calls: the first sizes the outputs).
+    options: {ODB_OPT_*: value}; spec_rec: a list that receives the round-parallel planner's record of the last
+    odb_run ([rounds committed, steps, ended the protocol, 0]) or None when that run did not use it."""
     import torch
     import paper_2606_19989_b200 as P
     dw = dw or DeviceWorkload(wl)
     with P.Odb(gpu_params(wl), max(wl.n_samples, 1)) as ctx:
         if bulk_stores:
             P.odb_set_option(ctx.h, P.ODB_OPT_COLLATE_BULK_STORES, 1)
+        for opt, val in (options or {}).items():
+            P.odb_set_option(ctx.h, opt, val)
         if staged:
             info = ctx.plan(dw.lengths, wl.rank_ptr, avail_schedule=avail_schedule)
             round_T = list(ctx.round_T)
@@ -66,6 +71,9 @@ def run_gpu(wl, dw=None, *, staged=True, fill=SENTINEL, avail_schedule=None, bul
             info = P.odb_run(ctx.h, dw.lengths, wl.rank_ptr, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo,
                              dw.span_hi, out.struct)
             round_T = None
+            if spec_rec is not None:
+                rec = np.zeros(4, dtype=np.int32)
+                spec_rec.append(rec if P.odb_debug_read(ctx.h, 4, rec) == 16 else None)
         torch.cuda.synchronize()
     return info, out, round_T
 

@@ -251,6 +251,63 @@ def test_round_loop_kernel_windows(P, oracle, buffer_size, slot_capacity):
         Par.compare_plan(plan, info2, out2)
 
 
+def _stream_lengths(rng, n, hi=3000):
+    return rng.integers(1, hi, n)
+
+
+@pytest.mark.parametrize("rule", [0, 1])
+@pytest.mark.parametrize("case", ["equal", "ragged_tail", "short_rank", "nonjoin", "capacity", "tiny_buffer", "full_chunk"])
+def test_round_parallel_planner(P, oracle, case, rule):
+    """The round-parallel planner (k_spec_form / k_spec_commit, ODB_OPT_ROUND_PARALLEL): every round that starts
+    without leftovers is formed at once, the sequential loop resumes at the first round that overflows.  Equal
+    streams (the whole run is round-parallel), ragged tails (the last windows differ: S+min caps T, the tail is
+    sequential), a rank that finishes early (IDLE slots beside round-parallel rounds), non-join without a quota
+    (the terminal round is the first in which a stream is drained), finite slot capacity (overflow in round 0:
+    nothing is committed round-parallel), an 8-sample buffer and full 4096-key windows.  Plan tables in full and
+    every element of every slot against the oracle; the sequential loop (option off) gives the same."""
+    rng = np.random.default_rng(7 + rule)
+    kw = dict(budget=8192, rule=rule, join_mode=1)
+    if case == "equal":
+        per, kw["buffer_size"] = [_stream_lengths(rng, 6000) for _ in range(5)], 500
+        expect = ("all", 12)
+    elif case == "ragged_tail":
+        per, kw["buffer_size"] = [_stream_lengths(rng, n) for n in (5000, 5013, 4990, 5100)], 1000
+        expect = ("some", None)  # (4 or 5 rounds: the 13-sample window of the last round caps T below the others' counts)
+    elif case == "short_rank":
+        per, kw["buffer_size"] = [_stream_lengths(rng, n) for n in (4096, 1024, 4096, 0)], 1024
+        expect = ("all", 4)
+    elif case == "nonjoin":
+        per, kw["buffer_size"], kw["join_mode"] = [_stream_lengths(rng, n) for n in (3000, 2048, 2600)], 256, 0
+        expect = ("all", 8)
+    elif case == "capacity":
+        per, kw["buffer_size"], kw["slot_capacity"] = [_stream_lengths(rng, 3000, 200) for _ in range(3)], 512, 3
+        expect = ("some", 0)
+    elif case == "tiny_buffer":
+        per, kw["buffer_size"] = [_stream_lengths(rng, 400, 9000) for _ in range(6)], 8
+        expect = ("all", 50)
+    else:
+        per, kw["buffer_size"] = [_stream_lengths(rng, 3 * 4096) for _ in range(3)], 4096
+        expect = ("all", 3)
+    wl = I.custom_workload("round_parallel_" + case, per, 77, **kw)
+    plan, _ = oracle.run_workload(wl, collate=False)
+    rec = []
+    info, out, _ = Par.run_gpu(wl, staged=False, spec_rec=rec)
+    Par.compare_plan(plan, info, out)
+    Par.compare_full_by_rank(oracle, wl, plan, out)
+    assert rec[0] is not None, "the round-parallel planner did not run"
+    committed, steps, ended = int(rec[0][0]), int(rec[0][1]), int(rec[0][2])
+    if expect[0] == "all":
+        assert ended == 1 and committed == expect[1] == plan.n_rounds - 1 and steps == plan.n_steps
+    else:
+        assert ended == 0 and committed < plan.n_rounds - 1
+        assert committed == expect[1] if expect[1] is not None else committed >= 4
+    # the sequential loop alone
+    rec2 = []
+    info2, out2, _ = Par.run_gpu(wl, staged=False, options={P.ODB_OPT_ROUND_PARALLEL: 0}, spec_rec=rec2)
+    assert rec2[0] is None
+    Par.compare_plan(plan, info2, out2)
+
+
 @pytest.mark.parametrize("staged", [True, False])
 def test_collate_bulk_store_variant(P, oracle, staged):
     """ODB_OPT_COLLATE_BULK_STORES: the interior chunks leave through shared memory and bulk asynchronous stores
