@@ -748,11 +748,13 @@ def cell_key(config, cv, budget, rule, buffer_size=0):
     return k + ("_buf%d" % buffer_size if buffer_size else "")
 
 
-def measure_workload(P, wl, device, steps, warmup):
+def measure_workload(P, wl, device, steps, warmup, options=None):
     """One workload through odb_run on `device` (own context, inputs and outputs); returns a row dict."""
     import torch
     din = DeviceInputs(wl, device, P)
     with P.Odb(gpu_params(P, wl), max(wl.n_samples, 1), device=int(device.split(":")[1])) as ctx:
+        for opt, val in (options or {}).items():
+            P.odb_set_option(ctx.h, opt, val)
         P.odb_set_timing(ctx.h, True)
         info = ctx.plan(din.lengths, wl.rank_ptr)
         out = P.OutputBuffers.for_plan(wl.n_ranks, info, device)
@@ -809,6 +811,11 @@ def paper_operating_point(P, device, peak):
     row["frac"] = row["collate_gbs"] / peak if row["collate_gbs"] else None
     row["whole_step_frac"] = row["whole_step_gbs"] / peak
     row["traffic"] = ncu_traffic(cell_key(4, 1.0, 65536, 0, 1024))
+    row["planner"] = "round-parallel (k_spec_form / k_spec_commit; k_rounds resumes at the first round that overflows)"
+    # the same job with every round in the sequential device-side loop (ODB_OPT_ROUND_PARALLEL = 0)
+    seq = measure_workload(P, wl, device, 5, 3, options={P.ODB_OPT_ROUND_PARALLEL: 0})
+    row["sequential_round_loop"] = {k: seq[k] for k in ("ms_per_step", "planning_ms", "planning_ms_per_round",
+                                                        "launches_per_step")}
     return row
 
 

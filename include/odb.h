@@ -180,6 +180,33 @@ ODB_API int odb_plan_query(odb_ctx *ctx, odb_plan_info *h_out);
 ODB_API int odb_collate(odb_ctx *ctx, const int32_t *d_tokens, const int64_t *d_sample_ptr, const int64_t *d_span_ptr,
                 const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *out, void *stream);
 
+/* The whole plan without collation: reset, every protocol round until termination (on the device where odb_run
+ * would run them there: the round-parallel planner and the persistent round loop for grouping buffers of at most
+ * 4096 samples; host-driven rounds otherwise), the slot scan.  Synchronises for the plan sizes (*h_out);
+ * afterwards the context is where odb_plan_query leaves it: odb_collate, odb_collate_steps and odb_loss_weights
+ * may follow. */
+ODB_API int odb_plan(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out, void *stream);
+
+/* Streaming output (section 2.3: a round's aligned groups go to the trainer while the next window is being
+ * grouped): collate the steps [step_lo, step_hi) of the plan SO FAR as a self-contained plan into `out` -- slots
+ * s' = r * n + (k - step_lo), n = step_hi - step_lo, block offsets from 0 (the exclusive scan of
+ * round_up(count * width, 16) over s'), every table of `out` indexed by s' (d_grp_origin keeps plan-wide step
+ * indices, d_grp_round plan-wide rounds, d_grp_sample_ids rank-local ids, d_step_samples / d_step_valid_tokens the
+ * n steps of the range; no leftover tables).  Allowed between rounds of the staged calls (after odb_round_status:
+ * the steps emitted so far) and after termination (odb_plan / odb_plan_query / odb_run); the context's state and the
+ * full plan's tables are untouched, so a trainer can pull a long plan through output buffers of bounded size, or
+ * take every round's batches as soon as the round is committed.  *h_out describes the range (n_steps = n, n_slots,
+ * total_elems, samples_emitted, real_tokens, padded_elems; n_rounds / stop_reason of the plan so far).  Waits only
+ * for those sizes; the collate kernel is then running on `stream`.  The library keeps TWO sets of range tables and
+ * alternates between them, so two ranges can be in flight at once (double buffering: a call reuses the tables of
+ * the call before the previous one and must be ordered behind it -- same stream, or that call's work complete).
+ * Null arenas: a sizing call (ODB_ERR_CAPACITY with *h_out filled unless the range is empty).  ODB_ERR_CAPACITY
+ * (nothing written) if an arena or table of `out` is too small; ODB_ERR_STATE for offline plans and distributed
+ * mode. */
+ODB_API int odb_collate_steps(odb_ctx *ctx, int32_t step_lo, int32_t step_hi, const int32_t *d_tokens,
+                              const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
+                              const int32_t *d_span_hi, const odb_outputs *out, odb_plan_info *h_out, void *stream);
+
 /* Everything: reset, the round loop until termination, plan query, one collate over all emitted
  * steps.  Synchronises once per round (a few bytes of status) and once for the plan sizes; returns
  * with the collate kernels enqueued on `stream`.  On ODB_ERR_CAPACITY *h_out is still filled. */

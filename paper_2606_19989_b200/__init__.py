@@ -8,5 +8,5 @@ from .binding import (  # noqa: F401
     Odb, OdbError, OdbLibraryError, OutputBuffers, SYMBOLS, library_path, load, make_params,
     odb_outputs, odb_params, odb_plan_info, status_string,
 )
-from .batches import StepBatches  # noqa: F401,E402
+from .batches import StepBatches, StepStream  # noqa: F401,E402
 from .stream import WorkerPool, plan_online  # noqa: F401,E402

@@ -64,3 +64,51 @@ class StepBatches:
             b = self.batch(rank, k)
             if b is not None:
                 yield b
+
+
+class StepStream:
+    """A terminated plan pulled through TWO output buffers of bounded size, ``steps_per_chunk`` steps at a time
+    (odb_collate_steps): ``for chunk in StepStream(...): for step in chunk: ...`` where ``chunk`` is a
+    ``StepBatches`` over the chunk's steps (``chunk.step_lo`` = its first plan-wide step).  While the consumer
+    works on chunk i, chunk i + 1 is being collated on the other stream into the other buffer (double buffering,
+    SURVEY.md 8(f) F3; "output queue").  The views of a chunk are valid until the next-but-one chunk is
+    requested.  ``slot_elems`` bounds one slot's block (max(budget, longest sample) is enough); plumbing only.
+    """
+
+    def __init__(self, ctx, n_ranks: int, n_steps: int, n_samples: int, inputs, steps_per_chunk: int, slot_elems: int,
+                 device, fill: Optional[int] = None):
+        import torch
+        from . import binding as B
+        self._B = B
+        self.ctx = ctx
+        self.n_ranks, self.n_steps = int(n_ranks), int(n_steps)
+        self.inputs = inputs  # (d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi)
+        self.chunk = max(1, int(steps_per_chunk))
+        slots = self.n_ranks * self.chunk
+        elems = slots * ((int(slot_elems) + 15) // 16 * 16)
+        ids = min(slots * int(slot_elems), int(n_samples))  # (a sample has at least one token)
+        self.bufs = [B.OutputBuffers(self.n_ranks, elems, slots, ids, self.chunk, 0, device, fill=fill) for _ in range(2)]
+        self.streams = [torch.cuda.Stream(device=device) for _ in range(2)]
+
+    def __len__(self) -> int:
+        return (self.n_steps + self.chunk - 1) // self.chunk
+
+    def _issue(self, i: int):
+        lo = i * self.chunk
+        hi = min(self.n_steps, lo + self.chunk)
+        b = i & 1
+        info = self._B.odb_collate_steps(self.ctx, lo, hi, *self.inputs, self.bufs[b].struct,
+                                         stream=self.streams[b].cuda_stream)
+        return b, info, lo
+
+    def __iter__(self) -> Iterator[StepBatches]:
+        n = len(self)
+        pending = self._issue(0) if n else None
+        for i in range(n):
+            nxt = self._issue(i + 1) if i + 1 < n else None  # enqueued before chunk i is handed out
+            b, info, lo = pending
+            self.streams[b].synchronize()
+            sb = StepBatches(self.bufs[b], info, self.n_ranks)
+            sb.step_lo = lo
+            yield sb
+            pending = nxt

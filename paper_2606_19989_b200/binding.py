@@ -94,6 +94,8 @@ SYMBOLS = {
     "odb_plan_query": (_i32, [_vp, _P(odb_plan_info)]),
     "odb_collate": (_i32, [_vp, _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _vp]),
     "odb_run": (_i32, [_vp, _vp, _P(_i64), _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _P(odb_plan_info), _vp]),
+    "odb_plan": (_i32, [_vp, _vp, _P(_i64), _P(odb_plan_info), _vp]),
+    "odb_collate_steps": (_i32, [_vp, _i32, _i32, _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _P(odb_plan_info), _vp]),
     "odb_run_host": (_i32, [_vp, _vp, _P(_i64), _vp, _vp, _vp, _vp, _vp, _P(odb_outputs), _P(odb_plan_info), _vp]),
     "odb_loss_weights": (_i32, [_vp, _i32, _vp, _vp]),
     "odb_loss_numerators": (_i32, [_vp, _i32, _vp, _vp]),
@@ -259,6 +261,30 @@ def odb_run(ctx: int, d_lengths, h_rank_ptr, d_tokens, d_sample_ptr, d_span_ptr,
     if rc == ODB_ERR_CAPACITY and allow_capacity_error:
         return info
     _check(rc, "odb_run", ctx)
+    return info
+
+
+def odb_plan(ctx: int, d_lengths, h_rank_ptr, stream=None) -> odb_plan_info:
+    """The whole plan (every protocol round + the slot scan), no collation."""
+    rp = _host_i64(h_rank_ptr)
+    info = odb_plan_info()
+    _check(load().odb_plan(ctx, _ptr(d_lengths), rp.ctypes.data_as(_P(_i64)), ctypes.byref(info), _stream(stream)),
+           "odb_plan", ctx)
+    info.status = ODB_OK
+    return info
+
+
+def odb_collate_steps(ctx: int, step_lo: int, step_hi: int, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi,
+                      out: odb_outputs, stream=None, *, allow_capacity_error: bool = False) -> odb_plan_info:
+    """Steps [step_lo, step_hi) of the plan so far as a self-contained plan in ``out`` (include/odb.h)."""
+    info = odb_plan_info()
+    rc = load().odb_collate_steps(ctx, int(step_lo), int(step_hi), _ptr(d_tokens), _ptr(d_sample_ptr), _ptr(d_span_ptr),
+                                  _ptr(d_span_lo), _ptr(d_span_hi), ctypes.byref(out), ctypes.byref(info),
+                                  _stream(stream))
+    info.status = rc
+    if rc == ODB_ERR_CAPACITY and allow_capacity_error:
+        return info
+    _check(rc, "odb_collate_steps", ctx)
     return info
 
 

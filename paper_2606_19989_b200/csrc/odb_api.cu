@@ -131,6 +131,53 @@ static void free_all(odb_ctx *c) {
     c->piece_ctr.release();
     c->spec_tab.release();
     if (c->h_rank_off) cudaFreeHost(c->h_rank_off);
+    for (SubTabs &t : c->sub) {
+        t.grp_count.release();
+        t.grp_width.release();
+        t.grp_round.release();
+        t.grp_valid.release();
+        t.grp_real.release();
+        t.grp_origin.release();
+        t.scan_state.release();
+        t.grp_offset.release();
+        t.grp_sample_ptr.release();
+        t.grp_sample_ids.release();
+        t.left_out.release();
+        t.left_ptr.release();
+        t.step_valid.release();
+        t.rows.release();
+        t.row_sp.release();
+        t.tiles.release();
+        cudaFree(t.d_dims);
+        cudaFree(t.d_tile_counter);
+        if (t.h_dims) cudaFreeHost(t.h_dims);
+        if (t.ev_plan) cudaEventDestroy(t.ev_plan);
+    }
+}
+
+// the context's plan tables <-> a step-range set (odb_collate_steps): kernels take the pointers at launch, so the
+// full plan's tables are back as soon as the range has been enqueued
+static void swap_tabs(odb_ctx *c, SubTabs &t) {
+    std::swap(c->grp_count, t.grp_count);
+    std::swap(c->grp_width, t.grp_width);
+    std::swap(c->grp_round, t.grp_round);
+    std::swap(c->grp_valid, t.grp_valid);
+    std::swap(c->grp_real, t.grp_real);
+    std::swap(c->grp_origin, t.grp_origin);
+    std::swap(c->scan_state, t.scan_state);
+    std::swap(c->grp_offset, t.grp_offset);
+    std::swap(c->grp_sample_ptr, t.grp_sample_ptr);
+    std::swap(c->grp_sample_ids, t.grp_sample_ids);
+    std::swap(c->left_out, t.left_out);
+    std::swap(c->left_ptr, t.left_ptr);
+    std::swap(c->step_valid, t.step_valid);
+    std::swap(c->rows, t.rows);
+    std::swap(c->row_sp, t.row_sp);
+    std::swap(c->tiles, t.tiles);
+    std::swap(c->d_dims, t.d_dims);
+    std::swap(c->h_dims, t.h_dims);
+    std::swap(c->d_tile_counter, t.d_tile_counter);
+    std::swap(c->ev_plan, t.ev_plan);
 }
 
 extern "C" {
@@ -585,6 +632,10 @@ int odb_round_status(odb_ctx *c, int32_t *h_done, int32_t *h_T) {
 // internal rank-major tables for a plan of at most n_slots slots / n_steps steps
 static int ensure_plan_tables(odb_ctx *c, size_t n_slots, size_t n_steps) {
     const size_t R = (size_t)c->prm.n_ranks;
+    if (c->sub_mode) {  // a step range: no leftover tables
+        CU(c, c->left_out.ensure(1));
+        CU(c, c->left_ptr.ensure(R + 1));
+    }
     CU(c, c->grp_count.ensure(n_slots + 1));
     CU(c, c->grp_width.ensure(n_slots + 1));
     CU(c, c->grp_round.ensure(n_slots + 1));
@@ -594,8 +645,10 @@ static int ensure_plan_tables(odb_ctx *c, size_t n_slots, size_t n_steps) {
     CU(c, c->grp_offset.ensure(n_slots + 1));
     CU(c, c->grp_sample_ptr.ensure(n_slots + 1));
     CU(c, c->grp_sample_ids.ensure((size_t)c->n_total + 1));
-    CU(c, c->left_out.ensure((size_t)c->n_total + 1));
-    CU(c, c->left_ptr.ensure(R + 1));
+    if (!c->sub_mode) {
+        CU(c, c->left_out.ensure((size_t)c->n_total + 1));
+        CU(c, c->left_ptr.ensure(R + 1));
+    }
     CU(c, c->step_valid.ensure(n_steps + 1));
     return ODB_OK;
 }
@@ -833,6 +886,178 @@ static int enqueue_tail(odb_ctx *c, int64_t steps_bound, const int32_t *d_tokens
     return enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, c->n_total, tile_bound, st);
 }
 
+// Regime (A) of odb_run / odb_plan: every protocol round on the device (the round-parallel planner where it
+// applies, then the persistent round loop).  *le = cudaSuccess: enqueued; otherwise the cooperative launch is not
+// possible here (too many ranks for the device), the context has been reset and the caller drives the rounds
+// from the host.  *steps_bound >= the steps the run can have.
+static int fused_rounds(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, int64_t max_nr, int64_t window,
+                        cudaStream_t st, int64_t *steps_bound_out, cudaError_t *le_out) {
+    const int R = c->prm.n_ranks;
+    c->last_stream = st;
+    int rc = begin_run(c, d_lengths, h_rank_ptr, st);
+    if (rc != ODB_OK) return rc;
+    // room for every step the run can have: n_steps <= the longest stream (a rank that is active in every
+    // emitting round emits at least T samples per round), plus one round's window
+    const int64_t steps_bound = max_nr + window + 64;
+    *steps_bound_out = steps_bound;
+    if (steps_bound > c->step_cap) {
+        CU(c, grow_preserve(c->st_count, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_width, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_real, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_round, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_origin, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->step_samples, (size_t)steps_bound, 0, st));
+        c->step_cap = steps_bound;
+    }
+    // rounds that are certainly not the terminal check (join: some stream still holds views; non-join: every
+    // stream does): formed and committed round-parallel as long as no round overflows (odb_plan.cu)
+    int64_t spec_rounds = 0;
+    if (c->round_parallel && c->prm.buffer_size >= kSpecMinWindow && (c->prm.join_mode || c->prm.sample_quota <= 0)) {
+        const int64_t B = c->prm.buffer_size;
+        int64_t min_nr = max_nr;
+        for (int r = 0; r < R; ++r) min_nr = std::min(min_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
+        spec_rounds = ((c->prm.join_mode ? max_nr : min_nr) + B - 1) / B;
+        if (spec_rounds < 2 || spec_rounds > kSpecMaxRounds) spec_rounds = 0;
+    }
+    const cudaError_t le = launch_rounds(c, (int)spec_rounds, st);
+    *le_out = le;
+    if (le == cudaSuccess) {
+        c->spec_used = spec_rounds > 0;
+        c->begin_pending = false;
+        return ODB_OK;
+    }
+    (void)cudaGetLastError();
+    if (le != cudaErrorNotSupported) c->no_rounds_kernel = true;
+    odb_reset(c);
+    return ODB_OK;
+}
+
+// ... and the host's side of it: wait for the plan sizes (an event behind the slot scan) and take them over
+static int fused_sizes(odb_ctx *c, odb_plan_info *h_out) {
+    CU(c, cudaEventSynchronize(c->ev_plan));
+    const PlanDims &D = *c->h_dims;
+    if (D.bad_length) {
+        c->state = 0;
+        return ODB_ERR_BAD_LENGTH;
+    }
+    if (!D.complete) return D.err ? D.err : ODB_ERR_STATE;
+    c->n_steps = D.n_steps;
+    c->n_rounds = D.n_rounds;
+    c->round = D.n_rounds;
+    c->stop_reason = D.stop_reason;
+    c->samples_emitted = D.samples_emitted;
+    fill_info(c);
+    c->state = 5;
+    *h_out = c->info;
+    return D.err;  // ODB_ERR_CAPACITY: the kernels behind the slot scan wrote nothing
+}
+
+static bool fused_applies(const odb_ctx *c, int64_t max_nr, int64_t window) {
+    return max_nr > 0 && window <= kSortChunk && !c->no_rounds_kernel &&
+           (int64_t)c->prm.n_ranks * (max_nr + window + 64) <= (1ll << 27);
+}
+
+int odb_plan(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out, void *stream) {
+    if (!c || !h_out || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
+    if (c->world_ranks) return ODB_ERR_STATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int R = c->prm.n_ranks;
+    int64_t max_nr = 0;
+    for (int r = 0; r < R; ++r) max_nr = std::max(max_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
+    const int64_t window = c->prm.buffer_size > 0 ? std::min<int64_t>(max_nr, c->prm.buffer_size) : max_nr;
+    odb_reset(c);
+    CU(c, cudaSetDevice(c->device));
+    if (fused_applies(c, max_nr, window)) {
+        int64_t steps_bound = 0;
+        cudaError_t le = cudaSuccess;
+        int rc = fused_rounds(c, d_lengths, h_rank_ptr, max_nr, window, st, &steps_bound, &le);
+        if (rc != ODB_OK) return rc;
+        if (le == cudaSuccess) {
+            const int64_t slots_bound = (int64_t)R * steps_bound;
+            rc = ensure_plan_tables(c, (size_t)slots_bound, (size_t)steps_bound);
+            if (rc != ODB_OK) return rc;
+            const CapCheck cap = {-1, -1, -1, -1, -1, -1};
+            CU(c, launch_finalize(c, slots_bound, cap, c->h_rank_off, st));
+            CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
+            CU(c, cudaEventRecord(c->ev_plan, st));
+            return fused_sizes(c, h_out);
+        }
+    }
+    return run_rounds(c, d_lengths, h_rank_ptr, h_out, st);
+}
+
+int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_t *d_tokens, const int64_t *d_sample_ptr,
+                      const int64_t *d_span_ptr, const int32_t *d_span_lo, const int32_t *d_span_hi, const odb_outputs *o,
+                      odb_plan_info *h_out, void *stream) {
+    if (!c || !o || !h_out) return ODB_ERR_INVALID_ARG;
+    if ((c->state != 3 && c->state != 4 && c->state != 5) || c->offline || c->world_ranks) return ODB_ERR_STATE;
+    if (step_lo < 0 || step_hi < step_lo || step_hi > c->n_steps) return ODB_ERR_INVALID_ARG;
+    const bool arenas = o->d_input_ids && o->d_labels && o->d_position_ids && o->d_attention_mask;
+    if (arenas && (!d_tokens || !d_sample_ptr || check_pointers(d_tokens, o) != ODB_OK)) return ODB_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(c, cudaSetDevice(c->device));
+    const int R = c->prm.n_ranks;
+    const int n = step_hi - step_lo;
+    SubTabs &T = c->sub[c->sub_seq & 1];
+    if (!T.ready) {
+        CU(c, dev_alloc(&T.d_dims, 1));
+        CU(c, cudaMemset(T.d_dims, 0, sizeof(PlanDims)));
+        CU(c, dev_alloc(&T.d_tile_counter, (size_t)R + 1));
+        CU(c, cudaMallocHost((void **)&T.h_dims, sizeof(PlanDims)));
+        CU(c, cudaEventCreateWithFlags(&T.ev_plan, cudaEventDisableTiming));
+        T.ready = true;
+    }
+    // (a set is reused by every second call: its previous plan sizes have been read, its kernels are ordered by
+    //  the caller's streams -- at most two step ranges in flight)
+    swap_tabs(c, T);
+    c->sub_mode = true;
+    c->sub_step_lo = step_lo;
+    const int timing = c->timing;
+    c->timing = 0;
+    int rc = [&]() -> int {
+        const int64_t slots = (int64_t)R * n;
+        int rc2 = ensure_plan_tables(c, (size_t)slots, (size_t)n);
+        if (rc2 != ODB_OK) return rc2;
+        const int64_t tile_bound = (std::max<int64_t>(o->arena_capacity, 0) + kColTile - 1) / kColTile;
+        const bool any_slot_tab = o->d_grp_count || o->d_grp_width || o->d_grp_round || o->d_grp_valid_tokens ||
+                                  o->d_grp_real_tokens || o->d_grp_origin || o->d_grp_offset || o->d_grp_sample_ptr;
+        CapCheck cap;
+        cap.arena = arenas ? std::max<int64_t>(o->arena_capacity, 0) : 0;
+        cap.slots = any_slot_tab ? o->slot_capacity_alloc : -1;
+        cap.ids = o->d_grp_sample_ids ? o->ids_capacity : -1;
+        cap.steps = (o->d_step_samples || o->d_step_valid_tokens) ? o->step_capacity_alloc : -1;
+        cap.left = -1;
+        cap.tiles = tile_bound;
+        CU(c, launch_sub_dims(c, n, st));
+        CU(c, launch_finalize(c, slots, cap, nullptr, st, step_lo));
+        CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
+        CU(c, cudaEventRecord(c->ev_plan, st));
+        CU(c, launch_sub_ids(c, step_lo, o->d_grp_sample_ids, st));
+        if (!arenas) return ODB_OK;  // a sizing call
+        return enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, c->n_total, tile_bound, st);
+    }();
+    c->timing = timing;
+    c->sub_mode = false;
+    swap_tabs(c, T);
+    c->sub_seq++;
+    if (rc != ODB_OK) return rc;
+    CU(c, cudaEventSynchronize(T.ev_plan));  // the range's sizes; its collate kernel is running
+    const PlanDims &D = *T.h_dims;
+    memset(h_out, 0, sizeof(*h_out));
+    h_out->n_rounds = c->state == 3 ? c->round : c->n_rounds;
+    h_out->n_steps = n;
+    h_out->stop_reason = c->state == 3 ? 0 : c->stop_reason;
+    h_out->n_slots = D.n_slots;
+    h_out->total_elems = D.total_elems;
+    h_out->samples_emitted = D.samples_emitted;
+    h_out->samples_left = 0;
+    h_out->real_tokens = (int64_t)D.real_tokens;
+    h_out->padded_elems = D.padded_elems;
+    if (D.err) return D.err;
+    if (!arenas && D.total_elems > 0) return ODB_ERR_CAPACITY;
+    return ODB_OK;
+}
+
 int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
             const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo, const int32_t *d_span_hi,
             const odb_outputs *o, odb_plan_info *h_out, void *stream) {
@@ -855,8 +1080,7 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
     const int64_t window = c->prm.buffer_size > 0 ? std::min<int64_t>(max_nr, c->prm.buffer_size) : max_nr;
     const bool arenas = o->d_input_ids && o->d_labels && o->d_position_ids && o->d_attention_mask;
     const bool async_ok = arenas && d_tokens && d_sample_ptr && check_pointers(d_tokens, o) == ODB_OK && max_nr > 0;
-    const bool fused = async_ok && window <= kSortChunk && !c->no_rounds_kernel &&
-                       (int64_t)R * (max_nr + window + 64) <= (1ll << 27);
+    const bool fused = async_ok && fused_applies(c, max_nr, window);
     const bool speculate = async_ok && !fused && window >= max_nr && c->prm.slot_capacity == 0;
     odb_reset(c);
     CU(c, cudaSetDevice(c->device));
@@ -867,61 +1091,19 @@ int odb_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, con
     int32_t done = 0, T = 0;
     int rc;
     if (fused) {
-        c->last_stream = st;
-        rc = begin_run(c, d_lengths, h_rank_ptr, st);
+        int64_t steps_bound = 0;
+        cudaError_t le = cudaSuccess;
+        rc = fused_rounds(c, d_lengths, h_rank_ptr, max_nr, window, st, &steps_bound, &le);
         if (rc != ODB_OK) return rc;
-        // room for every step the run can have: n_steps <= the longest stream (a rank that is active in every
-        // emitting round emits at least T samples per round), plus one round's window
-        const int64_t steps_bound = max_nr + window + 64;
-        if (steps_bound > c->step_cap) {
-            CU(c, grow_preserve(c->st_count, (size_t)steps_bound * R, 0, st));
-            CU(c, grow_preserve(c->st_width, (size_t)steps_bound * R, 0, st));
-            CU(c, grow_preserve(c->st_real, (size_t)steps_bound * R, 0, st));
-            CU(c, grow_preserve(c->st_round, (size_t)steps_bound * R, 0, st));
-            CU(c, grow_preserve(c->st_origin, (size_t)steps_bound * R, 0, st));
-            CU(c, grow_preserve(c->step_samples, (size_t)steps_bound, 0, st));
-            c->step_cap = steps_bound;
-        }
-        // rounds that are certainly not the terminal check (join: some stream still holds views; non-join: every
-        // stream does): formed and committed round-parallel as long as no round overflows (odb_plan.cu)
-        int64_t spec_rounds = 0;
-        if (c->round_parallel && c->prm.buffer_size >= kSpecMinWindow && (c->prm.join_mode || c->prm.sample_quota <= 0)) {
-            const int64_t B = c->prm.buffer_size;
-            int64_t min_nr = max_nr;
-            for (int r = 0; r < R; ++r) min_nr = std::min(min_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
-            spec_rounds = ((c->prm.join_mode ? max_nr : min_nr) + B - 1) / B;
-            if (spec_rounds < 2 || spec_rounds > kSpecMaxRounds) spec_rounds = 0;
-        }
-        cudaError_t le = launch_rounds(c, (int)spec_rounds, st);
         if (le == cudaSuccess) {
-            c->spec_used = spec_rounds > 0;
-            c->begin_pending = false;
             rc = enqueue_tail(c, steps_bound, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, st);
             if (rc != ODB_OK) return rc;
-            CU(c, cudaEventSynchronize(c->ev_plan));  // the sizes are here; the collate kernel is running
-            const PlanDims &D = *c->h_dims;
-            if (D.bad_length) {
-                c->state = 0;
-                return ODB_ERR_BAD_LENGTH;
-            }
-            if (!D.complete) return D.err ? D.err : ODB_ERR_STATE;
-            c->n_steps = D.n_steps;
-            c->n_rounds = D.n_rounds;
-            c->round = D.n_rounds;
-            c->stop_reason = D.stop_reason;
-            c->samples_emitted = D.samples_emitted;
-            fill_info(c);
-            c->state = 5;
-            *h_out = c->info;
-            if (D.err) return D.err;  // ODB_ERR_CAPACITY: the kernels behind the slot scan wrote nothing
+            rc = fused_sizes(c, h_out);  // the sizes are here; the collate kernel is running
+            if (rc != ODB_OK) return rc;
             if (c->timing) timing_done(c);
             c->collated = true;
             return ODB_OK;
         }
-        // the cooperative launch is not possible here (too many ranks for the device): drive the rounds from the host
-        (void)cudaGetLastError();
-        if (le != cudaErrorNotSupported) c->no_rounds_kernel = true;
-        odb_reset(c);
     }
     rc = odb_form_groups(c, d_lengths, h_rank_ptr, st);
     if (rc != ODB_OK) return rc;

@@ -740,7 +740,7 @@ cudaError_t launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *
         job(u->d_grp_origin, c->grp_origin.p, 0);
         job(u->d_grp_offset, c->grp_offset.p, 1);
         job(u->d_grp_sample_ptr, c->grp_sample_ptr.p, 2);
-        job(u->d_step_samples, c->step_samples.p, 3);
+        job(u->d_step_samples, c->step_samples.p + (c->sub_mode ? c->sub_step_lo : 0), 3);
     }
     A.emit_cur = c->emit_cur;
     A.emit_ids = c->emit_ids;
@@ -753,11 +753,12 @@ cudaError_t launch_prep(odb_ctx *c, const int64_t *d_sample_ptr, const int64_t *
         A.user_left = u->d_left_ids;
     }
     int blocks = A.rows_gx * R + A.tile_blocks + R;
-    if (c->offline) {  // rows in emit order; no leftovers (left_ptr was zeroed by odb_plan_query)
-        const int64_t n_rows = std::max<int64_t>(c->info.samples_emitted, 1);
+    if (c->offline || c->sub_mode) {  // rows in emit order; no leftovers (left_ptr was zeroed by odb_plan_query)
+        // (a step range: the host may not know its row count yet; the blocks beyond it leave at once)
+        const int64_t n_rows = std::max<int64_t>(c->sub_mode ? c->n_total : c->info.samples_emitted, 1);
         A.offline_row_blocks = (int)std::min<int64_t>((n_rows + kPrepThreads - 1) / kPrepThreads, (int64_t)c->sm_count * 8);
-        A.user_ids = u ? u->d_grp_sample_ids : nullptr;
-        if (u && u->d_left_ptr) {
+        A.user_ids = (u && !c->sub_mode) ? u->d_grp_sample_ids : nullptr;  // (a step range: written by k_sub_ids, local ids)
+        if (u && u->d_left_ptr && !c->sub_mode) {
             A.job[A.n_jobs].dst = u->d_left_ptr;
             A.job[A.n_jobs].src = c->left_ptr.p;
             A.job[A.n_jobs].kind = 5;

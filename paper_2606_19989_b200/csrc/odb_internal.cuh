@@ -175,6 +175,24 @@ struct DevBuf {
 
 }  // namespace odb
 
+// A second (and third) set of the rank-major plan tables: odb_collate_steps builds the self-contained plan of a
+// STEP RANGE in one of them (swapped in for the duration of the enqueue), so the full plan's tables stay valid
+// and two step ranges can be in flight at once (double-buffered streaming output).
+struct SubTabs {
+    odb::DevBuf<int32_t> grp_count, grp_width, grp_round, grp_valid, grp_real, grp_origin;
+    odb::DevBuf<unsigned char> scan_state;
+    odb::DevBuf<int64_t> grp_offset, grp_sample_ptr;
+    odb::DevBuf<int32_t> grp_sample_ids, left_out;
+    odb::DevBuf<int64_t> left_ptr, step_valid;
+    odb::DevBuf<odb::RowDesc> rows;
+    odb::DevBuf<int64_t> row_sp;
+    odb::DevBuf<odb::TileRec> tiles;
+    odb::PlanDims *d_dims = nullptr, *h_dims = nullptr;
+    unsigned long long *d_tile_counter = nullptr;
+    cudaEvent_t ev_plan = nullptr;
+    bool ready = false;
+};
+
 // The context.  Host-side state machine + device scratch.
 struct odb_ctx {
     odb_params prm;
@@ -272,6 +290,12 @@ struct odb_ctx {
     odb::DevBuf<int64_t> row_sp;
     odb::DevBuf<odb::TileRec> tiles;
 
+    // step-range plans (odb_collate_steps)
+    SubTabs sub[2];
+    int sub_seq = 0;
+    bool sub_mode = false;     // the tables swapped in belong to a step range: rows are gathered through the slot CSR
+    int32_t sub_step_lo = 0;   // its first step
+
     // offline planners (odb_offline.cu): the plan's slots hold GLOBAL sample ids
     bool offline = false;
     int offline_planner = 0, offline_size = 0, offline_bs = 0;
@@ -321,7 +345,13 @@ cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: 
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce
 // A9: rank-major tables, offsets, totals (sizes from the device-resident PlanDims)
-cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st);
+// (step_lo: the slot scan covers the steps [step_lo, step_lo + PlanDims.n_steps) of the staging tables)
+cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st,
+                            int64_t step_lo = 0);
+// step-range plans: PlanDims of the range, and the slot CSR's ids of its rows (global in the library's table, local
+// in the caller's)
+cudaError_t launch_sub_dims(odb_ctx *c, int n_steps, cudaStream_t st);
+cudaError_t launch_sub_ids(odb_ctx *c, int step_lo, int32_t *user_ids, cudaStream_t st);
 // ---- segment-level pieces shared with the offline planners (odb_offline.cu) -------------------------
 struct SortArgs;
 cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A, int64_t nseg, int maxS, cudaStream_t st);

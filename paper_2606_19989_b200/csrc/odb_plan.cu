@@ -1889,8 +1889,10 @@ cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st) {
 
 // A9.  `slots_bound` >= the number of slots the plan can hold (the host may not have seen the plan yet);
 // the grid is persistent: tiles are taken by ticket.
-cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st) {
+cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st,
+                            int64_t step_lo) {
     const int R = c->prm.n_ranks;
+    const int64_t so = step_lo * R;  // the staging tables are step-major: a step range is a contiguous piece
     const int64_t n_tiles = std::max<int64_t>((slots_bound + kFinTile - 1) / kFinTile, 1);
     cudaError_t e = c->scan_state.ensure((size_t)n_tiles * sizeof(ScanTile) + 64);
     if (e != cudaSuccess) return e;
@@ -1898,12 +1900,60 @@ cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap
     e = cudaMemsetAsync(c->scan_state.p, 0, (size_t)n_tiles * sizeof(ScanTile) + 64, st);
     if (e != cudaSuccess) return e;
     const int blocks = (int)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * 2);
-    k_fin_scan<<<blocks, kFinThreads, 0, st>>>(R, c->d_dims, c->st_count.p, c->st_width.p, c->st_real.p, c->st_round.p,
-                                               c->st_origin.p, c->grp_count.p, c->grp_width.p, c->grp_round.p,
+    k_fin_scan<<<blocks, kFinThreads, 0, st>>>(R, c->d_dims, c->st_count.p + so, c->st_width.p + so, c->st_real.p + so,
+                                               c->st_round.p + so, c->st_origin.p + so, c->grp_count.p, c->grp_width.p, c->grp_round.p,
                                                c->grp_real.p, c->grp_origin.p, c->grp_offset.p, c->grp_sample_ptr.p,
                                                reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
                                                reinterpret_cast<unsigned int *>(c->scan_state.p), cap,
-                                               c->offline ? (int64_t)-1 : c->n_total, rank_off);
+                                               (c->offline || c->sub_mode) ? (int64_t)-1 : c->n_total, rank_off);
+    ODB_LAUNCH_CHECK(c);
+    return cudaSuccess;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step-range plans (odb_collate_steps): the steps [step_lo, step_lo + n) of the plan so far as a self-contained
+// plan.  The slot scan above runs on that piece of the staging tables; what is left is the slot CSR's ids:
+// a rank's slots are in emit order, so the rows of its steps [step_lo, ..) are the piece of its emit region
+// that starts behind the samples of its earlier steps.
+// ---------------------------------------------------------------------------------------------
+__global__ void k_sub_dims(PlanDims *dims, int n_steps) {
+    dims->n_steps = n_steps;
+    dims->n_rounds = 0;
+    dims->stop_reason = 0;
+    dims->complete = 1;
+    dims->err = 0;
+    dims->bad_length = 0;
+}
+
+cudaError_t launch_sub_dims(odb_ctx *c, int n_steps, cudaStream_t st) {
+    k_sub_dims<<<1, 1, 0, st>>>(c->d_dims, n_steps);
+    ODB_LAUNCH_CHECK(c);
+    return cudaSuccess;
+}
+
+__global__ void __launch_bounds__(1024)
+k_sub_ids(const PlanDims *dims, int R, int step_lo, const int32_t *__restrict__ st_count, const int64_t *__restrict__ rank_ptr,
+          const int32_t *__restrict__ emit_ids, const int64_t *__restrict__ grp_sample_ptr, int32_t *__restrict__ ids,
+          int32_t *__restrict__ user_ids) {
+    __shared__ long long s_scan64[34];
+    if (!dims->complete || dims->err) return;
+    const int r = blockIdx.x, n = dims->n_steps;
+    long long part = 0;  // samples of rank r in the steps before the range
+    for (int k = threadIdx.x; k < step_lo; k += blockDim.x) part += st_count[(int64_t)k * R + r];
+    long long e_lo;
+    (void)block_excl_scan<long long>(part, s_scan64, e_lo);
+    const int64_t base = rank_ptr[r];
+    const int64_t q0 = grp_sample_ptr[(int64_t)r * n], q1 = grp_sample_ptr[(int64_t)(r + 1) * n];
+    for (int64_t i = threadIdx.x; i < q1 - q0; i += blockDim.x) {
+        const int32_t lid = emit_ids[base + e_lo + i];
+        ids[q0 + i] = (int32_t)(base + lid);
+        if (user_ids) user_ids[q0 + i] = lid;
+    }
+}
+
+cudaError_t launch_sub_ids(odb_ctx *c, int step_lo, int32_t *user_ids, cudaStream_t st) {
+    k_sub_ids<<<c->prm.n_ranks, 1024, 0, st>>>(c->d_dims, c->prm.n_ranks, step_lo, c->st_count.p, c->d_rank_ptr, c->emit_ids,
+                                              c->grp_sample_ptr.p, c->grp_sample_ids.p, user_ids);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }

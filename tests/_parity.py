@@ -197,6 +197,50 @@ def compare_full_by_rank(oracle, wl, plan, out, n_threads=None):
     assert np.array_equal(out.table("step_valid_tokens").cpu().numpy(), sv)
 
 
+def compare_step_range(plan, oracle_out, lo, hi, info, out, n_ranks):
+    """A step range collated by odb_collate_steps against the oracle's FULL plan and arenas: slot s' = r * n +
+    (k - lo) of the range must hold what slot s = r * n_steps + k of the plan holds -- tables, ids, every element of
+    the block -- at the range's own offsets (a layout of this build: the exclusive scan of round_up(count * width,
+    16) over s'); gaps and the tail keep the sentinel."""
+    n, R, K = hi - lo, n_ranks, plan.n_steps
+    assert int(info.n_steps) == n and int(info.n_slots) == R * n
+    sl = (np.arange(R)[:, None] * K + np.arange(lo, hi)[None, :]).reshape(-1)  # plan slots in range order
+    cnt, wid = plan.grp_count[sl].astype(np.int64), plan.grp_width[sl].astype(np.int64)
+    area = cnt * wid
+    off = np.concatenate([[0], np.cumsum((area + 15) // 16 * 16)])
+    sp = np.concatenate([[0], np.cumsum(cnt)])
+    E = int(off[-1])
+    assert int(info.total_elems) == E and int(info.samples_emitted) == int(sp[-1])
+    assert int(info.padded_elems) == int(area.sum()) and int(info.real_tokens) == int(plan.grp_real_tokens[sl].sum())
+    tab = lambda name, m: out.table(name).cpu().numpy()[:m]
+    assert np.array_equal(tab("grp_count", R * n), plan.grp_count[sl])
+    assert np.array_equal(tab("grp_width", R * n), plan.grp_width[sl])
+    assert np.array_equal(tab("grp_round", R * n), plan.grp_round[sl])
+    assert np.array_equal(tab("grp_real_tokens", R * n), plan.grp_real_tokens[sl])
+    assert np.array_equal(tab("grp_origin", R * n), plan.grp_origin[sl])
+    assert np.array_equal(tab("grp_offset", R * n), off[:-1])
+    assert np.array_equal(tab("grp_sample_ptr", R * n + 1), sp)
+    assert np.array_equal(tab("grp_valid_tokens", R * n), oracle_out["grp_valid_tokens"][sl])
+    assert np.array_equal(tab("step_samples", n), plan.step_samples[lo:hi])
+    assert np.array_equal(tab("step_valid_tokens", n), oracle_out["step_valid_tokens"][lo:hi])
+    ids = tab("grp_sample_ids", int(sp[-1]))
+    want_ids = [plan.grp_sample_ids[plan.grp_sample_ptr[s]:plan.grp_sample_ptr[s + 1]] for s in sl]
+    assert np.array_equal(ids, np.concatenate(want_ids) if want_ids else np.zeros(0, np.int32))
+    for name in ("input_ids", "labels", "position_ids", "attention_mask"):
+        g = getattr(out, name).cpu().numpy()
+        want = np.frombuffer(bytes([SENTINEL]) * (g.nbytes), dtype=g.dtype).copy()
+        ref = oracle_out[name]
+        for i, s in enumerate(sl):
+            a = int(area[i])
+            o0 = int(plan.grp_offset[s])
+            want[off[i]:off[i] + a] = ref[o0:o0 + a]
+        if not np.array_equal(g, want):
+            bad = np.flatnonzero(g != want)
+            i = int(np.searchsorted(off, bad[0], side="right") - 1)
+            raise AssertionError("steps [%d, %d): %s differs at %d elements; first at %d (range slot %d): gpu %r want %r" % (
+                lo, hi, name, len(bad), bad[0], i, g[bad[0]], want[bad[0]]))
+
+
 def device_self_consistency(info, out, ignore_index=-100):
     """Properties that hold at any size, checked on the device output itself: the valid-token table
     equals a recount of labels != ignore_index per slot; step totals are its column sums; the mask
