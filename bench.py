@@ -479,6 +479,7 @@ def run_ours(args):
                                                             "note": "sub-millisecond steps: launch latency, not HBM, bounds them"}
             result["paper_operating_point"] = paper_operating_point(P, device, peak)
             result["comparators"] = comparators(P, device)
+            result["streaming"] = [streaming_output(P, device, peak, steps_per_chunk=n) for n in (40, 160)]
         # ---- e2e through the C ABI with HOST buffers (odb_run_host) -------------------------
         if not args.no_e2e:
             need = 4 * wl.n_tokens + 13 * int(info.total_elems)
@@ -817,6 +818,66 @@ def paper_operating_point(P, device, peak):
     row["sequential_round_loop"] = {k: seq[k] for k in ("ms_per_step", "planning_ms", "planning_ms_per_round",
                                                         "launches_per_step")}
     return row
+
+
+def streaming_output(P, device, peak, steps_per_chunk=40, reps=5):
+    """The paper's operating point (buffer 1024) with STREAMING output: odb_plan, then the plan's steps pulled
+    `steps_per_chunk` at a time (about one protocol round) through two bounded output buffers on two streams
+    (odb_collate_steps; what StepStream does).  Wall clock around the host calls with a device synchronise on both
+    sides: time to the first chunk, and the whole pass beside the one-launch odb_run of the same job."""
+    import torch
+    wl = I.make_workload(4, cv=1.0, budget=65536)
+    wl.params["buffer_size"] = 1024
+    din = DeviceInputs(wl, device, P)
+    inputs = (din.tokens, din.sample_ptr, din.span_ptr, din.span_lo, din.span_hi)
+    R = wl.n_ranks
+    slot_elems = (max(int(wl.params["budget"]), int(wl.lengths.max())) + 15) // 16 * 16
+    with P.Odb(gpu_params(P, wl), wl.n_samples, device=int(device.split(":")[1])) as ctx:
+        info = P.odb_plan(ctx.h, din.lengths, wl.rank_ptr)
+        K = int(info.n_steps)
+        slots = R * steps_per_chunk
+        bufs = [P.OutputBuffers(R, slots * slot_elems, slots, wl.n_samples, steps_per_chunk, 0, device) for _ in range(2)]
+        streams = [torch.cuda.Stream(device=device) for _ in range(2)]
+        n_chunks = (K + steps_per_chunk - 1) // steps_per_chunk
+
+        def one_pass(first_only=False):
+            P.odb_plan(ctx.h, din.lengths, wl.rank_ptr)
+            elems = 0
+            for i in range(n_chunks):
+                lo = i * steps_per_chunk
+                ci = P.odb_collate_steps(ctx.h, lo, min(K, lo + steps_per_chunk), *inputs, bufs[i & 1].struct,
+                                         stream=streams[i & 1].cuda_stream)
+                elems = max(elems, int(ci.total_elems))
+                if first_only:
+                    break
+            return elems
+
+        one_pass()
+        torch.cuda.synchronize()
+        l0 = P.odb_kernel_launches(ctx.h)
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            chunk_elems = one_pass()
+        torch.cuda.synchronize()
+        ms = (time.perf_counter() - t0) / reps * 1e3
+        launches = (P.odb_kernel_launches(ctx.h) - l0) / reps
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            one_pass(first_only=True)
+            torch.cuda.synchronize()
+        first_ms = (time.perf_counter() - t0) / reps * 1e3
+        del bufs
+    del din
+    torch.cuda.empty_cache()
+    ab = algorithmic_bytes(info.real_tokens, info.padded_elems)
+    return {"workload": "configs[4] CV 1 L 65536, buffer_size 1024 (P:28)", "api": "odb_plan + odb_collate_steps",
+            "steps_per_chunk": steps_per_chunk, "chunks": n_chunks, "ms_per_pass": ms,
+            "samples_per_s": int(info.samples_emitted) / (ms * 1e-3), "whole_pass_gbs": ab / (ms * 1e-3) / 1e9,
+            "whole_pass_frac": ab / (ms * 1e-3) / 1e9 / peak, "ms_to_first_chunk": first_ms,
+            "launches_per_pass": launches, "largest_chunk_bytes": 13 * chunk_elems,
+            "output_buffer_bytes": 2 * 13 * R * steps_per_chunk * slot_elems,
+            "whole_plan_output_bytes": 13 * int(info.total_elems),
+            "timing": "wall clock around the host calls, device synchronised on both sides"}
 
 
 # --------------------------------------------------------------------------------------------
