@@ -957,16 +957,18 @@ static bool fused_applies(const odb_ctx *c, int64_t max_nr, int64_t window) {
            (int64_t)c->prm.n_ranks * (max_nr + window + 64) <= (1ll << 27);
 }
 
-int odb_plan(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out, void *stream) {
-    if (!c || !h_out || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
-    if (c->world_ranks) return ODB_ERR_STATE;
-    cudaStream_t st = (cudaStream_t)stream;
+// the whole plan: every round on the device where that applies, else host-driven rounds; ends in state 5
+static int plan_impl(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     int64_t max_nr = 0;
     for (int r = 0; r < R; ++r) max_nr = std::max(max_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
     const int64_t window = c->prm.buffer_size > 0 ? std::min<int64_t>(max_nr, c->prm.buffer_size) : max_nr;
     odb_reset(c);
     CU(c, cudaSetDevice(c->device));
+    if (c->timing) {  // (odb_run_host closes the quadruple)
+        timing_begin(c);
+        CU(c, cudaEventRecord(c->ev[0], st));
+    }
     if (fused_applies(c, max_nr, window)) {
         int64_t steps_bound = 0;
         cudaError_t le = cudaSuccess;
@@ -984,6 +986,12 @@ int odb_plan(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, od
         }
     }
     return run_rounds(c, d_lengths, h_rank_ptr, h_out, st);
+}
+
+int odb_plan(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out, void *stream) {
+    if (!c || !h_out || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
+    if (c->world_ranks) return ODB_ERR_STATE;
+    return plan_impl(c, d_lengths, h_rank_ptr, h_out, (cudaStream_t)stream);
 }
 
 int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_t *d_tokens, const int64_t *d_sample_ptr,
@@ -1254,7 +1262,7 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
             return urc;
         }
     }
-    int rc = run_rounds(c, c->hs_lengths.p, h_rank_ptr, h_out, st);
+    int rc = plan_impl(c, c->hs_lengths.p, h_rank_ptr, h_out, st);
     if (rc != ODB_OK) {
         drain();
         return rc;

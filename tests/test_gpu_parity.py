@@ -308,6 +308,48 @@ def test_round_parallel_planner(P, oracle, case, rule):
     Par.compare_plan(plan, info2, out2)
 
 
+def test_round_parallel_planner_fuzz(P, oracle):
+    """120 random jobs in the round-parallel planner's regime (grouping buffers of 8 .. 700 samples, up to 12 ranks
+    with unequal streams of up to 4000 samples, both rules, join and non-join without a quota, finite slot capacity in
+    a third of them): the plan tables in full and sampled slots element by element against the oracle.  The planner
+    must have run, and the rounds it committed never exceed the plan's."""
+    used = 0
+    for seed in range(120):
+        rng = np.random.default_rng(31_000 + seed)
+        R = int(rng.integers(1, 13))
+        hi = int(rng.choice([40, 600, 5000]))
+        n_max = int(rng.choice([60, 900, 4000]))
+        equal = rng.uniform() < 0.4
+        n0 = int(rng.integers(n_max // 2, n_max + 1))
+        per = [rng.integers(1, hi + 1, n0 if equal else int(rng.integers(0, n_max + 1))) for _ in range(R)]
+        B = int(rng.choice([8, 9, 31, 64, 128, 257, 700]))
+        wl = I.custom_workload("rp_fuzz", per, seed, budget=int(rng.choice([64, 1024, 8192, 60000])), buffer_size=B,
+                               slot_capacity=int(rng.choice([0, 0, 5, 40])), rule=int(rng.integers(0, 2)),
+                               join_mode=int(rng.integers(0, 2)), shift_labels=int(rng.integers(0, 2)))
+        plan, _ = oracle.run_workload(wl, collate=False)
+        rec = []
+        info, out, _ = Par.run_gpu(wl, staged=False, spec_rec=rec)
+        Par.compare_plan(plan, info, out)
+        if plan.n_slots:
+            pick = sorted(set(rng.integers(0, plan.n_slots, 6).tolist()) | {0, plan.n_slots - 1})
+            Par.compare_sampled_slots(wl, plan, out, pick)
+        if rec[0] is not None:
+            used += 1
+            assert 0 <= int(rec[0][0]) <= plan.n_rounds - 1 and int(rec[0][1]) <= plan.n_steps
+            assert (int(rec[0][2]) == 1) == (int(rec[0][0]) == plan.n_rounds - 1)
+    assert used >= 60
+
+
+def test_run_host_with_small_grouping_buffer(P, oracle):
+    """odb_run_host plans on the device too (round-parallel planner + round loop, no per-round host round trip)."""
+    wl = I.make_workload(1, n_ranks=4, n_per_rank=2500)
+    wl.params["buffer_size"] = 256
+    _run_host_case(P, oracle, wl, staging_elems=1 << 16)
+    wl = I.custom_workload("run_host_ragged", [np.arange(1, 1500) % 900 + 1, np.arange(1, 900) % 50 + 1], 3, budget=4096,
+                           buffer_size=100, join_mode=0)
+    _run_host_case(P, oracle, wl)
+
+
 @pytest.mark.parametrize("staged", [True, False])
 def test_collate_bulk_store_variant(P, oracle, staged):
     """ODB_OPT_COLLATE_BULK_STORES: the interior chunks leave through shared memory and bulk asynchronous stores
