@@ -316,9 +316,10 @@ def time_device(P, ctx, wl, din, out, steps, warmup, barrier):
     return ms, float(stage[1]), float(stage[0]), float(stage[2]), launches, info
 
 
-def time_e2e(P, ctx, wl, din, info, steps, device):
+def time_e2e(P, ctx, wl, din, info, steps, device, device_arenas=False):
     """odb_run_host: pinned HOST inputs -> device -> whole path -> pinned HOST outputs, all inside the
-    timed region (wall clock around the synchronous C call, which ends with a stream synchronize)."""
+    timed region (wall clock around the synchronous C call, which ends with a stream synchronize).
+    device_arenas: the four arenas stay in HBM (ODB_OPT_HOST_DEVICE_ARENAS), only the tables come back."""
     import torch
     pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
     h_len = pin(wl.lengths, torch.int32)
@@ -328,7 +329,15 @@ def time_e2e(P, ctx, wl, din, info, steps, device):
     h_hi = pin(wl.span_hi if len(wl.span_hi) else np.zeros(1, np.int32), torch.int32)
     h_tok = torch.empty(wl.n_tokens + 16, dtype=torch.int32, pin_memory=True)
     h_tok.copy_(din.tokens)                      # same ids as the device buffer (untimed set-up)
-    hout = P.OutputBuffers.for_plan(wl.n_ranks, info, "cpu")
+    if device_arenas:
+        hout = P.OutputBuffers(wl.n_ranks, 0, info.n_slots, info.samples_emitted, info.n_steps, info.samples_left, "cpu")
+        dout = P.OutputBuffers(wl.n_ranks, info.total_elems, 0, 0, 0, 0, device, tables=False)
+        hs, ds = hout.struct, dout.struct
+        hs.d_input_ids, hs.d_labels, hs.d_position_ids = ds.d_input_ids, ds.d_labels, ds.d_position_ids
+        hs.d_attention_mask, hs.arena_capacity = ds.d_attention_mask, int(info.total_elems)
+    else:
+        hout = P.OutputBuffers.for_plan(wl.n_ranks, info, "cpu")
+    P.odb_set_option(ctx.h, P.ODB_OPT_HOST_DEVICE_ARENAS, 1 if device_arenas else 0)
     torch.cuda.synchronize()
 
     def one():
@@ -343,8 +352,9 @@ def time_e2e(P, ctx, wl, din, info, steps, device):
     dt = (time.perf_counter() - t0) / max(steps, 1)
     h2d = (h_len.numel() * 4 + h_sp.numel() * 8 + h_spp.numel() * 8 + len(wl.span_lo) * 8 + wl.n_tokens * 4)
     E = int(info.total_elems)
-    d2h = 13 * E + int(info.n_slots) * (5 * 4 + 8) + (int(info.n_slots) + 1) * 8 + int(info.samples_emitted) * 4 \
-        + int(info.n_steps) * 12 + (wl.n_ranks + 1) * 8 + int(info.samples_left) * 4
+    d2h = (0 if device_arenas else 13 * E) + int(info.n_slots) * (5 * 4 + 8) + (int(info.n_slots) + 1) * 8 \
+        + int(info.samples_emitted) * 4 + int(info.n_steps) * 12 + (wl.n_ranks + 1) * 8 + int(info.samples_left) * 4
+    P.odb_set_option(ctx.h, P.ODB_OPT_HOST_DEVICE_ARENAS, 0)
     return dt, int(h2d), int(d2h)
 
 
@@ -506,6 +516,15 @@ def run_ours(args):
                                  "device_staging": "token ring 3 x one rank, output ring 3 x %d elements (13 B each)" % (
                                      args.host_staging_elems or (1 << 25)),
                                  "api": "odb_run_host (pinned host buffers in and out)"}
+                # the same call with the arenas left in HBM for a trainer on this GPU: only the inputs cross the link
+                dt2, h2d2, d2h2 = time_e2e(P, ctx, wl, din, info, args.e2e_steps, device, device_arenas=True)
+                dt2 = max_over_ranks(dt2)
+                result["e2e_device_outputs"] = {
+                    "value": world * n_samples / dt2, "unit": UNIT, "h2d_bytes_per_step": h2d2, "d2h_bytes_per_step": d2h2,
+                    "ms_per_step": dt2 * 1e3, "steps": args.e2e_steps, "tokens_per_s": world * n_tok / dt2,
+                    "h2d_gbs": h2d2 / dt2 / 1e9,
+                    "api": "odb_run_host with ODB_OPT_HOST_DEVICE_ARENAS (pinned host inputs; arenas stay in HBM, tables "
+                           "come back to the host)"}
     del din
     torch.cuda.empty_cache()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

@@ -330,8 +330,13 @@ ODB_API int odb_offline_plan(odb_ctx *ctx, const odb_offline_params *params, con
  * predecessors only through the leftovers, and there are none until a round overflows -- and the
  * sequential round loop resumes at the first round that does; 0 = every round in the sequential loop.  Same
  * results bit for bit.
+ * ODB_OPT_HOST_DEVICE_ARENAS (value 0 / 1, default 0): the four arena pointers of odb_run_host's `h_out_bufs` are
+ * DEVICE memory (16-byte aligned, arena_capacity elements): the inputs still come from host buffers rank by rank,
+ * but every rank's slots are collated in place as soon as its tokens have landed and the batches stay on the device
+ * for the trainer; only the tables (still HOST pointers) come back.  No output staging is allocated.
  * ODB_ERR_INVALID_ARG for an unknown option. */
-enum { ODB_OPT_COLLATE_BULK_STORES = 1, ODB_OPT_HOST_STAGING_ELEMS = 2, ODB_OPT_ROUND_PARALLEL = 3 };
+enum { ODB_OPT_COLLATE_BULK_STORES = 1, ODB_OPT_HOST_STAGING_ELEMS = 2, ODB_OPT_ROUND_PARALLEL = 3,
+       ODB_OPT_HOST_DEVICE_ARENAS = 4 };
 ODB_API int odb_set_option(odb_ctx *ctx, int option, int64_t value);
 
 /* Bandwidth probes (measurement utility, not part of the method): the collate kernel's byte mix -- 4 bytes read

@@ -364,6 +364,7 @@ def odb_offline_plan(ctx: int, planner: int, d_lengths, n_samples: int, *, d_per
 ODB_OPT_COLLATE_BULK_STORES = 1
 ODB_OPT_HOST_STAGING_ELEMS = 2
 ODB_OPT_ROUND_PARALLEL = 3
+ODB_OPT_HOST_DEVICE_ARENAS = 4
 
 
 def odb_set_option(ctx: int, option: int, value: int) -> None:

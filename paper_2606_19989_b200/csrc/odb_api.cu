@@ -349,6 +349,7 @@ int odb_set_option(odb_ctx *c, int option, int64_t value) {
     switch (option) {
     case ODB_OPT_COLLATE_BULK_STORES: c->collate_bulk = value != 0; return ODB_OK;
     case ODB_OPT_ROUND_PARALLEL: c->round_parallel = value != 0; return ODB_OK;
+    case ODB_OPT_HOST_DEVICE_ARENAS: c->host_device_arenas = value != 0; return ODB_OK;
     case ODB_OPT_HOST_STAGING_ELEMS:
         if (value < 1) return ODB_ERR_INVALID_ARG;
         c->host_staging_elems = value;
@@ -1205,10 +1206,12 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
     CU(c, c->hs_span_lo.ensure((size_t)n_span + 1));
     CU(c, c->hs_span_hi.ensure((size_t)n_span + 1));
     CU(c, c->hs_tokens.ensure(kRing * tok_slot + 16));
-    CU(c, c->hs_ids.ensure(kRing * (size_t)piece + 16));
-    CU(c, c->hs_labels.ensure(kRing * (size_t)piece + 16));
-    CU(c, c->hs_pos.ensure(kRing * (size_t)piece + 16));
-    CU(c, c->hs_mask.ensure(kRing * (size_t)piece + 16));
+    if (!c->host_device_arenas) {
+        CU(c, c->hs_ids.ensure(kRing * (size_t)piece + 16));
+        CU(c, c->hs_labels.ensure(kRing * (size_t)piece + 16));
+        CU(c, c->hs_pos.ensure(kRing * (size_t)piece + 16));
+        CU(c, c->hs_mask.ensure(kRing * (size_t)piece + 16));
+    }
     if (!c->copy_stream) {
         CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
         CU(c, cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
@@ -1280,6 +1283,7 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
         if (rc == ODB_OK && (ho->d_step_samples || ho->d_step_valid_tokens) && ho->step_capacity_alloc < I.n_steps)
             rc = ODB_ERR_CAPACITY;
         if (rc == ODB_OK && ho->d_left_ids && ho->left_capacity < I.samples_left) rc = ODB_ERR_CAPACITY;
+        if (rc == ODB_OK && c->host_device_arenas && check_pointers(nullptr, ho) != ODB_OK) rc = ODB_ERR_INVALID_ARG;
     }
     if (rc != ODB_OK) {
         drain();
@@ -1290,10 +1294,14 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
     CU(c, c->row_sp.ensure((size_t)I.samples_emitted + 1));
     CU(c, c->tiles.ensure((size_t)((I.total_elems + kColTile - 1) / kColTile) + 2));
     // pieces: every rank's arena range [lo, hi) cut at tile-aligned positions, at most `piece` elements each
+    // (device arenas: a rank's range is one piece, written in place)
+    const bool dev_arenas = c->host_device_arenas;
     int64_t n_pieces = 0;
     for (int r = 0; r < R; ++r) {
         const int64_t lo = c->h_rank_off[r], hi = c->h_rank_off[r + 1];
-        for (int64_t cur = lo; cur < hi; ++n_pieces) cur = std::min(hi, (cur / kColTile) * kColTile + piece);
+        if (dev_arenas) n_pieces += hi > lo ? 1 : 0;
+        else
+            for (int64_t cur = lo; cur < hi; ++n_pieces) cur = std::min(hi, (cur / kColTile) * kColTile + piece);
     }
     CU(c, c->piece_ctr.ensure((size_t)n_pieces + 1));
     CU(c, cudaMemsetAsync(c->piece_ctr.p, 0, ((size_t)n_pieces + 1) * sizeof(unsigned long long), st));
@@ -1312,7 +1320,15 @@ static int run_host_impl(odb_ctx *c, const int32_t *h_lengths, const int64_t *h_
             CU(c, cudaStreamWaitEvent(st, ev, 0));  // the rank's tokens have landed
             const int64_t t0 = N > 0 ? h_sample_ptr[h_rank_ptr[r]] : 0;
             const int32_t *tok_base = c->hs_tokens.p + (size_t)(r % kRing) * tok_slot + (size_t)(t0 & 3) - t0;
-            for (int64_t cur = lo; cur < hi;) {
+            if (dev_arenas) {  // the arenas are device memory: the rank's slots are collated in place, nothing comes back
+                rc = collate_launch(c, tok_base, c->hs_span_lo.p, c->hs_span_hi.p, ho, false, lo, hi, 0, c->piece_ctr.p + pi, st);
+                if (rc != ODB_OK) {
+                    drain();
+                    return rc;
+                }
+                ++pi;
+            }
+            for (int64_t cur = lo; cur < hi && !dev_arenas;) {
                 const int64_t end = std::min(hi, (cur / kColTile) * kColTile + piece);
                 const size_t slot = (size_t)(pi % kRing) * (size_t)piece;
                 if (pi >= kRing) {  // the staging piece is free once its previous contents have been copied back

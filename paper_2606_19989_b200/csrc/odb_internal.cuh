@@ -321,6 +321,7 @@ struct odb_ctx {
     std::vector<cudaEvent_t> ev_pool;         // odb_run_host: tokens landed / rank collated / piece collated / piece copied
     odb::DevBuf<unsigned long long> piece_ctr;  // one work counter per output piece
     int64_t host_staging_elems = 1ll << 25;   // arena elements per staging piece (ODB_OPT_HOST_STAGING_ELEMS)
+    bool host_device_arenas = false;          // odb_run_host: the four arenas of `h_out_bufs` are DEVICE memory
     int64_t *h_rank_off = nullptr;            // pinned, R+1: arena offset of each rank's first slot
 };
 

@@ -511,6 +511,32 @@ def test_run_host_streams_through_fixed_size_staging(P, oracle, staging):
     _run_host_case(P, oracle, I.protocol_workload("empty_rank", 2), staging_elems=staging)
 
 
+def test_run_host_device_arenas(P, oracle):
+    """ODB_OPT_HOST_DEVICE_ARENAS: host inputs, the four arenas stay on the device (collated in place, rank by rank, as
+    the tokens land), the tables come back to the host -- every element against the oracle, gaps untouched."""
+    import torch
+    for wl in (I.make_workload(1, n_ranks=5, n_per_rank=900), I.protocol_workload("empty_rank", 3),
+               I.protocol_workload("overflow_multiround", 2)):
+        plan, ref = oracle.run_workload(wl)
+        toks_np = wl.tokens()
+        toks = torch.from_numpy(toks_np if len(toks_np) else np.zeros(1, np.int32)).pin_memory()
+        pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a) if len(a) else np.zeros(1, a.dtype)).to(dt).pin_memory()
+        host = P.OutputBuffers(wl.n_ranks, 0, plan.n_slots, plan.samples_emitted, plan.n_steps, plan.samples_left, "cpu")
+        dev = P.OutputBuffers(wl.n_ranks, plan.total_elems, 0, 0, 0, 0, "cuda:0", fill=Par.SENTINEL, tables=False)
+        st = host.struct
+        st.d_input_ids, st.d_labels = dev.struct.d_input_ids, dev.struct.d_labels
+        st.d_position_ids, st.d_attention_mask = dev.struct.d_position_ids, dev.struct.d_attention_mask
+        st.arena_capacity = plan.total_elems
+        with P.Odb(Par.gpu_params(wl), max(wl.n_samples, 1)) as ctx:
+            P.odb_set_option(ctx.h, P.ODB_OPT_HOST_DEVICE_ARENAS, 1)
+            info = P.odb_run_host(ctx.h, pin(wl.lengths, torch.int32), wl.rank_ptr, toks, pin(wl.sample_ptr, torch.int64),
+                                  pin(wl.span_ptr, torch.int64), pin(wl.span_lo, torch.int32), pin(wl.span_hi, torch.int32), st)
+        Par.compare_plan(plan, info, host)
+        host.input_ids, host.labels, host.position_ids, host.attention_mask = (dev.input_ids, dev.labels, dev.position_ids,
+                                                                               dev.attention_mask)
+        Par.compare_full(plan, ref, info, host)
+
+
 def test_run_host_reuses_context(P, oracle):
     """Two odb_run_host calls on one context (staging buffers, events and counters are reused)."""
     wl = I.make_workload(1, n_ranks=3, n_per_rank=300)
