@@ -61,6 +61,8 @@ def parse_args():
     ap.add_argument("--shard-ranks", action="store_true",
                     help="SURVEY.md 8(f) F1: split the job's virtual ranks over the N GPUs (strong scaling; per-round "
                          "all_gather + all_reduce over NCCL) instead of N independent replicas")
+    ap.add_argument("--per-round-exchange", action="store_true",
+                    help="--shard-ranks: one exchange per protocol round (P:52) instead of the batched exchange")
     ap.add_argument("--pipeline", type=int, default=0,
                     help="measure N contexts driven round-robin on N streams (planning of one step beside the collate "
                          "kernel of another); extra key 'pipelined'")
@@ -576,11 +578,12 @@ def run_sharded(args):
     coll = D.TorchCollectives()
     eng = D.CudaEngine(gpu_params(P, wl), max(wl.n_samples, 1), lengths, wl.rank_ptr, device=local)
     P.odb_set_timing(eng.ctx.h, True)
-    info, _ = D.run(D.plan_protocol(eng, wl_all.n_ranks, rank * rl), coll, device)
+    batched = not args.per_round_exchange
+    info, _ = D.run(D.plan_protocol(eng, wl_all.n_ranks, rank * rl, batched=batched), coll, device)
     out = P.OutputBuffers.for_plan(rl, info, device)
 
     def one():
-        info, _ = D.run(D.plan_protocol(eng, wl_all.n_ranks, rank * rl), coll, device)
+        info, _ = D.run(D.plan_protocol(eng, wl_all.n_ranks, rank * rl, batched=batched), coll, device)
         eng.collate(tokens, sample_ptr, span_ptr, span_lo, span_hi, out)
         D.run(D.step_valid_protocol(out.table("step_valid_tokens")), coll, device)
         return info

@@ -271,12 +271,42 @@ typedef struct {
     int32_t summary_local_count, summary_world_count;
     int32_t *d_step_samples_round; /* valid between odb_form_groups and odb_commit of a round */
     int32_t step_window;
-    int32_t reserved;
+    int32_t spec_G_count;          /* batched exchange: n_rounds * n_ranks */
+    int32_t *d_spec_G_local;       /* batched exchange: G of the local ranks, [round][rank] (after odb_dist_spec_form) */
 } odb_dist_bufs;
 ODB_API int odb_dist_config(odb_ctx *ctx, int32_t world_ranks, int32_t rank_offset, int32_t world_max_window);
 ODB_API int odb_dist_buffers(odb_ctx *ctx, odb_dist_bufs *out);
 /* Distributed mode only (ODB_ERR_STATE otherwise): second half of odb_align, after collective 2. */
 ODB_API int odb_commit(odb_ctx *ctx, void *stream);
+
+/* Distributed mode, BATCHED EXCHANGE: the round-parallel planner (ODB_OPT_ROUND_PARALLEL) over several processes.
+ * A round depends on its predecessors only through the leftovers, and there are none until a round
+ * overflows; until then the window of round j of rank r is the views [j B, (j + 1) B) of its stream, so the
+ * per-round exchange of P:52 can be done for ALL those rounds at once: 3 collectives for J rounds instead of 2 J.
+ *
+ *   all_gather(every rank's stream length n_r)                             [the caller; once per run]
+ *   odb_dist_spec_form(ctx, d_lengths, h_rank_ptr, J, max n_r, stream)     local windows of the rounds [0, J): sort,
+ *                                                                          candidate groups, G table (odb_dist_buffers:
+ *                                                                          d_spec_G_local, spec_G_count, [round][rank])
+ *   all_gather(G_world <- d_spec_G_local)                                  [layout [process][round][local rank]]
+ *   odb_dist_spec_commit(ctx, G_world, n_world, n_procs, stream)           Eq. 3 and the no-overflow check of every round
+ *                                                                          on the gathered data (identical everywhere,
+ *                                                                          Lemma 3), split + commit of the rounds before
+ *                                                                          the first that overflows
+ *   all_reduce(SUM, d_step_samples_round[0 .. max n_r))                    [global e_k of those rounds' steps]
+ *   odb_dist_spec_status(ctx, &rounds, &steps, h_T, capacity)              synchronises; rounds committed (0 .. J), their
+ *                                                                          steps and T_grp; then the per-round calls go on
+ *                                                                          with round `rounds` (odb_form_groups ...)
+ *
+ * J = rounds that are certainly not the terminal check: join ceil(max n_r / B), non-join ceil(min n_r / B), over ALL
+ * ranks of the job (1 .. 65535).  Requirements (ODB_ERR_INVALID_ARG / ODB_ERR_STATE otherwise): distributed mode,
+ * a fresh run (after odb_dist_config / odb_reset), buffer_size in 8 .. 4096, no sample quota, no arrival schedule,
+ * every process holds the same number of ranks (world_ranks = n_procs * n_ranks). */
+ODB_API int odb_dist_spec_form(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, int32_t n_rounds,
+                               int64_t world_max_stream, void *stream);
+ODB_API int odb_dist_spec_commit(odb_ctx *ctx, const int32_t *d_G_world, const int32_t *d_n_world, int32_t n_procs,
+                                 void *stream);
+ODB_API int odb_dist_spec_status(odb_ctx *ctx, int32_t *h_rounds, int32_t *h_steps, int32_t *h_T, int32_t T_capacity);
 
 /* Device times of the last odb_run / odb_collate on this context, in milliseconds, measured with
  * CUDA events on the launching stream: ms[0] = planning (all rounds, plan query, row descriptors and

@@ -54,7 +54,8 @@ class odb_outputs(ctypes.Structure):
 
 class odb_dist_bufs(ctypes.Structure):
     _fields_ = [("d_summary_local", _vp), ("d_summary_world", _vp), ("summary_local_count", _i32),
-                ("summary_world_count", _i32), ("d_step_samples_round", _vp), ("step_window", _i32), ("reserved", _i32)]
+                ("summary_world_count", _i32), ("d_step_samples_round", _vp), ("step_window", _i32),
+                ("spec_G_count", _i32), ("d_spec_G_local", _vp)]
 
 
 class odb_offline_params(ctypes.Structure):
@@ -101,6 +102,9 @@ SYMBOLS = {
     "odb_loss_numerators": (_i32, [_vp, _i32, _vp, _vp]),
     "odb_loss_normalize": (_i32, [_vp, _vp, _i32, _i32, _vp, _vp]),
     "odb_dist_config": (_i32, [_vp, _i32, _i32, _i32]),
+    "odb_dist_spec_form": (_i32, [_vp, _vp, _P(_i64), _i32, _i64, _vp]),
+    "odb_dist_spec_commit": (_i32, [_vp, _vp, _vp, _i32, _vp]),
+    "odb_dist_spec_status": (_i32, [_vp, _P(_i32), _P(_i32), _P(_i32), _i32]),
     "odb_dist_buffers": (_i32, [_vp, _P(odb_dist_bufs)]),
     "odb_commit": (_i32, [_vp, _vp]),
     "odb_set_timing": (_i32, [_vp, _i32]),
@@ -327,6 +331,25 @@ def odb_dist_buffers(ctx: int) -> odb_dist_bufs:
     b = odb_dist_bufs()
     _check(load().odb_dist_buffers(ctx, ctypes.byref(b)), "odb_dist_buffers", ctx)
     return b
+
+
+def odb_dist_spec_form(ctx: int, d_lengths, h_rank_ptr, n_rounds: int, world_max_stream: int, stream=None) -> None:
+    rp = _host_i64(h_rank_ptr)
+    _check(load().odb_dist_spec_form(ctx, _ptr(d_lengths), rp.ctypes.data_as(_P(_i64)), int(n_rounds), int(world_max_stream),
+                                     _stream(stream)), "odb_dist_spec_form", ctx)
+
+
+def odb_dist_spec_commit(ctx: int, d_G_world, d_n_world, n_procs: int, stream=None) -> None:
+    _check(load().odb_dist_spec_commit(ctx, _ptr(d_G_world), _ptr(d_n_world), int(n_procs), _stream(stream)),
+           "odb_dist_spec_commit", ctx)
+
+
+def odb_dist_spec_status(ctx: int, max_rounds: int):
+    """(rounds committed, their steps, [T_grp of each])."""
+    r, k = _i32(0), _i32(0)
+    T = (ctypes.c_int32 * max(int(max_rounds), 1))()
+    _check(load().odb_dist_spec_status(ctx, ctypes.byref(r), ctypes.byref(k), T, int(max_rounds)), "odb_dist_spec_status", ctx)
+    return int(r.value), int(k.value), [int(T[j]) for j in range(r.value)]
 
 
 def odb_commit(ctx: int, stream=None) -> None:

@@ -131,6 +131,7 @@ static void free_all(odb_ctx *c) {
     c->piece_ctr.release();
     c->spec_tab.release();
     if (c->h_rank_off) cudaFreeHost(c->h_rank_off);
+    if (c->h_spec) cudaFreeHost(c->h_spec);
     for (SubTabs &t : c->sub) {
         t.grp_count.release();
         t.grp_width.release();
@@ -576,6 +577,84 @@ int odb_dist_buffers(odb_ctx *c, odb_dist_bufs *out) {
         out->d_step_samples_round = c->step_samples.p + c->n_steps;
         out->step_window = c->round_window;
     }
+    if (c->state == 7 || c->state == 8) {  // batched exchange: the local G table; the step totals of the whole run so far
+        out->d_spec_G_local = c->dist_spec_G;
+        out->spec_G_count = c->dist_spec_rounds * c->prm.n_ranks;
+        out->d_step_samples_round = c->step_samples.p;
+        out->step_window = (int32_t)std::min<int64_t>(c->step_cap, 0x7fffffff);
+    }
+    return ODB_OK;
+}
+
+// ---- distributed mode, batched exchange (the round-parallel planner over several processes) ----
+int odb_dist_spec_form(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank_ptr, int32_t n_rounds,
+                       int64_t world_max_stream, void *stream) {
+    if (!c || !h_rank_ptr) return ODB_ERR_INVALID_ARG;
+    if (!c->world_ranks || c->state != 0 || c->arrived_set) return ODB_ERR_STATE;
+    if (c->prm.buffer_size < kSpecMinWindow || c->prm.buffer_size > kSortChunk || n_rounds < 1 || n_rounds > kSpecMaxRounds ||
+        (!c->prm.join_mode && c->prm.sample_quota > 0) || world_max_stream < 0)
+        return ODB_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int R = c->prm.n_ranks;
+    c->last_stream = st;
+    int rc = begin_run(c, d_lengths, h_rank_ptr, st);
+    if (rc != ODB_OK) return rc;
+    // room for every step the job can have: n_steps <= the longest stream of the job, plus one round's window
+    const int64_t steps_bound = std::max<int64_t>(world_max_stream, c->max_nr) + c->prm.buffer_size + 64;
+    if (steps_bound > c->step_cap) {
+        CU(c, grow_preserve(c->st_count, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_width, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_real, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_round, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->st_origin, (size_t)steps_bound * R, 0, st));
+        CU(c, grow_preserve(c->step_samples, (size_t)steps_bound, 0, st));
+        c->step_cap = steps_bound;
+    }
+    CU(c, launch_dist_spec_form(c, n_rounds, &c->dist_spec_G, st));
+    c->begin_pending = false;
+    c->dist_spec_rounds = n_rounds;
+    c->state = 7;
+    return ODB_OK;
+}
+
+int odb_dist_spec_commit(odb_ctx *c, const int32_t *d_G_world, const int32_t *d_n_world, int32_t n_procs, void *stream) {
+    if (!c || !d_G_world || !d_n_world) return ODB_ERR_INVALID_ARG;
+    if (c->state != 7) return ODB_ERR_STATE;
+    if (n_procs < 1 || (int64_t)n_procs * c->prm.n_ranks != c->world_ranks) return ODB_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(c, cudaSetDevice(c->device));
+    CU(c, launch_dist_spec_commit(c, c->dist_spec_rounds, d_G_world, d_n_world, n_procs, st));
+    if (!c->h_spec) CU(c, cudaMallocHost((void **)&c->h_spec, (4 + (size_t)kSpecMaxRounds + 1) * sizeof(int32_t)));
+    // SpecRec, the bad-length flag and the rounds' T go back together (status read by odb_dist_spec_status)
+    const size_t tab_fixed = 4 + (size_t)kSpecMaxRounds + 1;
+    CU(c, cudaMemcpyAsync(c->h_spec, c->spec_tab.p, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CU(c, cudaMemcpyAsync(c->h_spec + 4, c->spec_tab.p + tab_fixed, (size_t)c->dist_spec_rounds * sizeof(int32_t),
+                          cudaMemcpyDeviceToHost, st));
+    CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, st));
+    CU(c, cudaEventRecord(c->ev_status, st));
+    c->state = 8;
+    return ODB_OK;
+}
+
+int odb_dist_spec_status(odb_ctx *c, int32_t *h_rounds, int32_t *h_steps, int32_t *h_T, int32_t T_capacity) {
+    if (!c) return ODB_ERR_INVALID_ARG;
+    if (c->state != 8) return ODB_ERR_STATE;
+    CU(c, cudaEventSynchronize(c->ev_status));
+    if (c->h_rec->bad_length) {
+        c->state = 0;
+        return ODB_ERR_BAD_LENGTH;
+    }
+    const int32_t js = c->h_spec[0], n_steps = c->h_spec[1];
+    if (js < 0 || js > c->dist_spec_rounds || n_steps < 0 || n_steps > c->step_cap) return ODB_ERR_STATE;
+    if (h_T && T_capacity < js) return ODB_ERR_CAPACITY;
+    for (int j = 0; h_T && j < js; ++j) h_T[j] = c->h_spec[4 + j];
+    c->round = js;
+    c->n_steps = n_steps;
+    c->last_T = js > 0 ? c->h_spec[4 + js - 1] : 0;
+    c->spec_used = true;
+    if (h_rounds) *h_rounds = js;
+    if (h_steps) *h_steps = n_steps;
+    c->state = 3;  // between rounds: odb_form_groups continues with round js
     return ODB_OK;
 }
 

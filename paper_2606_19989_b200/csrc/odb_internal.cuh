@@ -222,6 +222,9 @@ struct odb_ctx {
     int spec_occ = 0;               // k_spec_form's shared-memory attribute is set
     bool round_parallel = true;     // odb_set_option(ODB_OPT_ROUND_PARALLEL)
     bool spec_used = false;         // the last run went through the round-parallel planner (spec_tab holds its SpecRec)
+    int32_t dist_spec_rounds = 0;   // distributed mode: rounds formed by odb_dist_spec_form (state 7 / 8)
+    int32_t *dist_spec_G = nullptr; //   ... their local G table inside spec_tab
+    int32_t *h_spec = nullptr;      // pinned: SpecRec + the committed rounds' T (read back by odb_dist_spec_status)
 
     // inputs fixed by the first odb_form_groups after create / reset
     const int32_t *d_lengths = nullptr;
@@ -343,6 +346,11 @@ inline size_t plan_table_entries(size_t N, size_t R) { return N + N / 8 + 2 * R 
 constexpr int kSpecMinWindow = 8;       // smallest buffer_size the round-parallel planner takes
 constexpr int kSpecMaxRounds = 65535;   // (gridDim.y)
 cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st);   // distributed: (G_r, S_r) pairs for the all_gather
+// distributed, batched exchange: the local G table of the rounds [0, n_rounds); then, from the gathered tables,
+// Eq. 3 of every round, split + commit of the rounds before the first that overflows, the rank state behind them
+cudaError_t launch_dist_spec_form(odb_ctx *c, int n_rounds, int32_t **G_tab_out, cudaStream_t st);
+cudaError_t launch_dist_spec_commit(odb_ctx *c, int n_rounds, const int32_t *d_G_world, const int32_t *d_n_world, int n_procs,
+                                    cudaStream_t st);
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce
 // A9: rank-major tables, offsets, totals (sizes from the device-resident PlanDims)

@@ -1222,6 +1222,7 @@ struct SpecArgs {
     uint32_t budget;
     int rule, join_mode, slot_capacity;
     int x_keys;  // padded sort keys the shared-memory layout reserves
+    int eval_T;  // 1: the launch closes the rounds itself (all ranks are local); 0: only the G table (distributed mode)
     int32_t *gpos, *agpos, *agcnt, *agorg;
     int32_t *st_count, *st_width, *st_real, *st_round, *st_origin;
     int32_t *emit_ids, *left_ids_w;
@@ -1270,6 +1271,7 @@ __global__ void __launch_bounds__(kMsThreads) k_spec_form(const SpecArgs A) {
         for (int i = t; i <= G; i += blockDim.x) gpo[i] = gp[i];
     }
     if (t == 0) __stcg(&A.G_tab[(int64_t)j * R + r], G);
+    if (!A.eval_T) return;  // distributed mode: the tables of all processes are gathered first (k_spec_T_world)
     // ---- the last CTA of round j to arrive: Eq. 3 and the no-overflow check ----
     __threadfence();
     __syncthreads();
@@ -1368,6 +1370,67 @@ __global__ void __launch_bounds__(kMsThreads) k_spec_commit(const SpecArgs A) {
     V.emit_cur = &s_state[2];
     commit_body(r, R, V, SA.step_samples, sb, j, A.join_mode, 0ll, 0ll, A.st_count, A.st_width, A.st_real, A.st_round,
                 A.st_origin, A.emit_ids, SA.emit_pos, A.left_ids_w, &s_rec, true, 0, 1);
+}
+
+// Distributed mode (ranks over several processes): the same planner with ONE exchange for all its rounds instead of
+// one per round.  Every process forms the windows of its ranks for the rounds [0, J) (k_spec_form, eval_T = 0), the
+// G tables of all processes are all_gathered (layout [process][round][local rank]) next to every rank's stream
+// length, and every process evaluates Eq. 3 and the no-overflow check of every round on the same gathered data
+// (Lemma 3: identical decisions everywhere), commits its ranks' rounds before j* and goes on round by round from there.
+__global__ void __launch_bounds__(1024)
+k_spec_T_world(const int32_t *__restrict__ G_world, const int32_t *__restrict__ n_world, int n_procs, int R_local, int n_rounds,
+               int B, int slot_capacity, int32_t *__restrict__ T_tab, int32_t *__restrict__ sb_tab, SpecRec *rec) {
+    __shared__ int s_scan[34];
+    __shared__ int s_js;
+    const int t = threadIdx.x;
+    if (t == 0) s_js = n_rounds;
+    __syncthreads();
+    for (int j = t; j < n_rounds; j += blockDim.x) {
+        int maxG = 0, minS = 0x7fffffff;
+        for (int p = 0; p < n_procs; ++p)
+            for (int r = 0; r < R_local; ++r) {
+                const int g = G_world[((int64_t)p * n_rounds + j) * R_local + r];
+                if (g > 0) {  // active set A; its windows are non-empty
+                    const int nq = n_world[p * R_local + r];
+                    const int sq = min(B, nq - (int)min((long long)j * B, (long long)nq));
+                    maxG = max(maxG, g);
+                    minS = min(minS, sq);
+                }
+            }
+        const int T = target_groups(maxG, minS, slot_capacity);
+        const int v = (T == maxG && maxG > 0) ? T : -1;
+        T_tab[j] = v;
+        if (v < 0) atomicMin(&s_js, j);
+    }
+    __syncthreads();
+    const int js = s_js;
+    int carry = 0;
+    for (int q0 = 0; q0 < js; q0 += blockDim.x) {
+        const int q = q0 + t;
+        const int v = q < js ? T_tab[q] : 0;
+        int tot;
+        const int ex = block_excl_scan<int>(v, s_scan, tot);
+        if (q < js) sb_tab[q] = carry + ex;
+        carry += tot;
+    }
+    if (t == 0) {
+        rec->j_star = js;
+        rec->n_steps = carry;
+        rec->complete = js == n_rounds ? 1 : 0;
+        rec->pad_ = 0;
+    }
+}
+
+// the rank state the committed rounds leave behind: no leftovers, j* windows fetched and emitted
+__global__ void k_spec_state(const SpecRec *rec, const int64_t *__restrict__ rank_ptr, int R, int B, int32_t *n_left,
+                             int32_t *fetch_pos, int32_t *emit_cur) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    const int n_r = (int)(rank_ptr[r + 1] - rank_ptr[r]);
+    const int fp = (int)min((long long)rec->j_star * B, (long long)n_r);
+    n_left[r] = 0;
+    fetch_pos[r] = fp;
+    emit_cur[r] = fp;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1763,6 +1826,72 @@ static int host_active_keys(int S) {
     return std::min(n, kMsChunk);
 }
 
+// Arguments, block size and shared memory of the round-parallel planner's kernels for `spec_rounds` rounds.
+static cudaError_t make_spec_args(odb_ctx *c, int spec_rounds, int eval_T, cudaStream_t st, SpecArgs *out, int *threads_out,
+                                  size_t *smem_out) {
+    const int R = c->prm.n_ranks;
+    const int B = c->prm.buffer_size;
+    const int n_keys = host_active_keys(B);
+    // (measured: more threads per window are slower -- 256 / 512 / 1024 threads for 1024-key windows give a
+    //  planning stage of 0.134 / 0.146 / 0.185 ms: the launch is throughput-bound, not latency-bound)
+    *threads_out = std::max(n_keys / kMsItems, 128);
+    const size_t x_keys = (size_t)n_keys + n_keys / kMsItems;
+    const size_t x_bytes = std::max(x_keys * 8, (form_hier_smem_bytes(B) + 15) & ~(size_t)15);
+    *smem_out = x_bytes + (size_t)B * 8 + ((size_t)B + 4) * 4;
+    if (!c->spec_occ) {
+        cudaError_t ae = cudaFuncSetAttribute(k_spec_form, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(96 * 1024));
+        if (ae != cudaSuccess) return ae;
+        c->spec_occ = 1;
+    }
+    const size_t tab_fixed = 4 + (size_t)kSpecMaxRounds + 1;
+    cudaError_t e = c->spec_tab.ensure(tab_fixed + 2 * ((size_t)kSpecMaxRounds + 1) + (size_t)spec_rounds * R, true, st);
+    if (e != cudaSuccess) return e;
+    SpecArgs P;
+    memset(&P, 0, sizeof(P));
+    P.sort.len = c->d_lengths;
+    P.sort.rank_ptr = c->d_rank_ptr;
+    P.sort.n_left = c->n_left;
+    P.sort.fetch_pos = c->fetch_pos;
+    P.sort.emit_cur = c->emit_cur;
+    P.sort.left_ids = c->left_ids;
+    P.sort.arrived = c->d_arrived;
+    P.sort.buffer_size = B;
+    P.sort.keys_out = c->keyA;
+    P.sort.S_out = c->S;
+    P.sort.rec = c->d_rec;
+    P.sort.first = 1;
+    P.sort.n_total = c->n_total;
+    P.sort.emit_pos = c->emit_pos;
+    P.sort.step_samples = c->step_samples.p;
+    P.sort.step_cap = c->step_samples.p ? (int64_t)c->step_samples.cap : 0;
+    P.R = R;
+    P.n_rounds = spec_rounds;
+    P.budget = (uint32_t)c->prm.budget;
+    P.rule = c->prm.rule;
+    P.join_mode = c->prm.join_mode;
+    P.slot_capacity = c->prm.slot_capacity;
+    P.x_keys = (int)(x_bytes / 8);
+    P.eval_T = eval_T;
+    P.gpos = c->gpos;
+    P.agpos = c->agpos;
+    P.agcnt = c->agcnt;
+    P.agorg = c->agorg;
+    P.st_count = c->st_count.p;
+    P.st_width = c->st_width.p;
+    P.st_real = c->st_real.p;
+    P.st_round = c->st_round.p;
+    P.st_origin = c->st_origin.p;
+    P.emit_ids = c->emit_ids;
+    P.left_ids_w = c->left_ids;
+    P.rec = reinterpret_cast<SpecRec *>(c->spec_tab.p);
+    P.ctr = reinterpret_cast<unsigned int *>(c->spec_tab.p + 4);
+    P.T_tab = c->spec_tab.p + tab_fixed;
+    P.sb_tab = P.T_tab + kSpecMaxRounds + 1;
+    P.G_tab = P.sb_tab + kSpecMaxRounds + 1;
+    *out = P;
+    return cudaSuccess;
+}
+
 cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const size_t smem = kRoundsSmem;
@@ -1832,48 +1961,11 @@ cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st) {
     A.spec = nullptr;
     if (spec_rounds > 0) {
         // the rounds [0, spec_rounds) round-parallel; k_rounds resumes where the speculation stops
-        const int B = c->prm.buffer_size;
-        const int n_keys = host_active_keys(B);
-        // (measured: more threads per window are slower -- 256 / 512 / 1024 threads for 1024-key windows give a
-        //  planning stage of 0.134 / 0.146 / 0.185 ms: the launch is throughput-bound, not latency-bound)
-        const int threads = std::max(n_keys / kMsItems, 128);
-        const size_t x_keys = (size_t)n_keys + n_keys / kMsItems;
-        const size_t x_bytes = std::max(x_keys * 8, (form_hier_smem_bytes(B) + 15) & ~(size_t)15);
-        const size_t sp_smem = x_bytes + (size_t)B * 8 + ((size_t)B + 4) * 4;
-        if (!c->spec_occ) {
-            cudaError_t ae = cudaFuncSetAttribute(k_spec_form, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(96 * 1024));
-            if (ae != cudaSuccess) return ae;
-            c->spec_occ = 1;
-        }
-        const size_t tab_fixed = 4 + (size_t)kSpecMaxRounds + 1;
-        e = c->spec_tab.ensure(tab_fixed + 2 * ((size_t)kSpecMaxRounds + 1) + (size_t)spec_rounds * R, true, st);
-        if (e != cudaSuccess) return e;
         SpecArgs P;
-        memset(&P, 0, sizeof(P));
-        P.sort = A.sort;
-        P.R = R;
-        P.n_rounds = spec_rounds;
-        P.budget = A.budget;
-        P.rule = A.rule;
-        P.join_mode = A.join_mode;
-        P.slot_capacity = A.slot_capacity;
-        P.x_keys = (int)(x_bytes / 8);
-        P.gpos = c->gpos;
-        P.agpos = c->agpos;
-        P.agcnt = c->agcnt;
-        P.agorg = c->agorg;
-        P.st_count = A.st_count;
-        P.st_width = A.st_width;
-        P.st_real = A.st_real;
-        P.st_round = A.st_round;
-        P.st_origin = A.st_origin;
-        P.emit_ids = c->emit_ids;
-        P.left_ids_w = c->left_ids;
-        P.rec = reinterpret_cast<SpecRec *>(c->spec_tab.p);
-        P.ctr = reinterpret_cast<unsigned int *>(c->spec_tab.p + 4);
-        P.T_tab = c->spec_tab.p + tab_fixed;
-        P.sb_tab = P.T_tab + kSpecMaxRounds + 1;
-        P.G_tab = P.sb_tab + kSpecMaxRounds + 1;
+        int threads = 0;
+        size_t sp_smem = 0;
+        e = make_spec_args(c, spec_rounds, 1, st, &P, &threads, &sp_smem);
+        if (e != cudaSuccess) return e;
         k_spec_form<<<dim3((unsigned)R, (unsigned)spec_rounds), threads, sp_smem, st>>>(P);
         ODB_LAUNCH_CHECK(c);
         k_spec_commit<<<dim3((unsigned)R, (unsigned)spec_rounds), threads, 0, st>>>(P);
@@ -1886,6 +1978,41 @@ cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     c->launches++;
     c->sorted = c->keyA;
+    return cudaSuccess;
+}
+
+// distributed mode, first half: the local windows of the rounds [0, n_rounds) and their G table ([round][rank])
+cudaError_t launch_dist_spec_form(odb_ctx *c, int n_rounds, int32_t **G_tab_out, cudaStream_t st) {
+    SpecArgs P;
+    int threads = 0;
+    size_t sp_smem = 0;
+    cudaError_t e = make_spec_args(c, n_rounds, 0, st, &P, &threads, &sp_smem);
+    if (e != cudaSuccess) return e;
+    k_spec_form<<<dim3((unsigned)c->prm.n_ranks, (unsigned)n_rounds), threads, sp_smem, st>>>(P);
+    ODB_LAUNCH_CHECK(c);
+    *G_tab_out = P.G_tab;
+    c->sorted = c->keyA;
+    return cudaSuccess;
+}
+
+// ... second half, behind the all_gather: Eq. 3 for every round on the gathered tables, split + commit of the
+// local ranks' rounds before j*, the rank state for round j*
+cudaError_t launch_dist_spec_commit(odb_ctx *c, int n_rounds, const int32_t *d_G_world, const int32_t *d_n_world, int n_procs,
+                                    cudaStream_t st) {
+    SpecArgs P;
+    int threads = 0;
+    size_t sp_smem = 0;
+    cudaError_t e = make_spec_args(c, n_rounds, 0, st, &P, &threads, &sp_smem);
+    if (e != cudaSuccess) return e;
+    const int R = c->prm.n_ranks;
+    k_spec_T_world<<<1, 1024, 0, st>>>(d_G_world, d_n_world, n_procs, R, n_rounds, c->prm.buffer_size, c->prm.slot_capacity,
+                                        P.T_tab, P.sb_tab, P.rec);
+    ODB_LAUNCH_CHECK(c);
+    k_spec_commit<<<dim3((unsigned)R, (unsigned)n_rounds), threads, 0, st>>>(P);
+    ODB_LAUNCH_CHECK(c);
+    k_spec_state<<<(R + 127) / 128, 128, 0, st>>>(P.rec, c->d_rank_ptr, R, c->prm.buffer_size, c->n_left, c->fetch_pos,
+                                                   c->emit_cur);
+    ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
 

@@ -99,6 +99,29 @@ class CudaEngine:
     def commit(self):
         B.odb_commit(self.ctx.h, self.stream)
 
+    # ---- batched exchange (the round-parallel planner over several processes; include/odb.h) ----
+    def stream_lengths(self):
+        """n_r of the local ranks as an int32 tensor on the engine's device (the all_gather's input)."""
+        import torch
+        return torch.from_numpy(np.diff(self.h_rank_ptr).astype(np.int32)).to(self.device)
+
+    def spec_form(self, n_rounds: int, world_max_stream: int):
+        B.odb_dist_spec_form(self.ctx.h, self.d_lengths, self.h_rank_ptr, n_rounds, world_max_stream, self.stream)
+
+    def spec_table(self):
+        b = B.odb_dist_buffers(self.ctx.h)
+        return _wrap(b.d_spec_G_local, b.spec_G_count, "<i4", self.device)
+
+    def spec_commit(self, g_world, n_world, n_procs: int):
+        B.odb_dist_spec_commit(self.ctx.h, g_world, n_world, n_procs, self.stream)
+
+    def spec_step_window(self, n: int):
+        b = B.odb_dist_buffers(self.ctx.h)
+        return _wrap(b.d_step_samples_round, min(int(n), int(b.step_window)), "<i4", self.device)
+
+    def spec_status(self, max_rounds: int):
+        return B.odb_dist_spec_status(self.ctx.h, max_rounds)
+
     def round_status(self):
         return B.odb_round_status(self.ctx.h)
 
@@ -116,7 +139,25 @@ class CudaEngine:
 
 
 # ---- the protocol ------------------------------------------------------------------------------
-def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=None) -> Generator[Request, object, tuple]:
+SPEC_MIN_WINDOW, SPEC_MAX_WINDOW, SPEC_MAX_ROUNDS = 8, 4096, 65535
+
+
+def batched_rounds(n_world: np.ndarray, params) -> int:
+    """Rounds that are certainly not the terminal check and can be exchanged at once (0 = the batched exchange does
+    not apply): join -- some stream still holds views; non-join -- every stream does.  Host logic shared by every
+    process: the same gathered stream lengths and the same parameters give the same answer everywhere."""
+    B_ = int(getattr(params, "buffer_size", 0) or 0)
+    join = int(getattr(params, "join_mode", 1))
+    quota = int(getattr(params, "sample_quota", 0) or 0)
+    if B_ < SPEC_MIN_WINDOW or B_ > SPEC_MAX_WINDOW or (not join and quota > 0) or len(n_world) == 0:
+        return 0
+    n = int(n_world.max()) if join else int(n_world.min())
+    J = (n + B_ - 1) // B_
+    return J if 2 <= J <= SPEC_MAX_ROUNDS and J * len(n_world) <= (1 << 22) else 0
+
+
+def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=None,
+                  batched: bool = True) -> Generator[Request, object, tuple]:
     """Round loop of one process.  Returns (plan info of the local ranks, [T_grp of every emitting round]).
     ``avail_schedule[j]`` (optional): arrived views of the LOCAL ranks at round j (odb_set_available).
 
@@ -146,6 +187,35 @@ def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=Non
     window = max(1, min(int(wmax), cap) if cap > 0 else int(wmax))
     dev = getattr(engine, "device", "cpu")
     round_T: List[int] = []
+    # ---- batched exchange: every round that starts without leftovers, 3 collectives for all of them ----
+    # (a round depends on its predecessors only through the leftovers; Eq. 3 and the no-overflow check of every
+    #  round are evaluated by every process on the same gathered tables, so all take the same decisions: Lemma 3)
+    if batched and avail_schedule is None and hasattr(engine, "spec_form") and world_ranks % engine.n_ranks == 0:
+        n_local = call(engine.stream_lengths)
+        if n_local is None:
+            n_local = torch.zeros(engine.n_ranks, dtype=torch.int32, device=dev)
+        n_world = torch.zeros(world_ranks, dtype=torch.int32, device=dev)
+        yield ("all_gather", n_world, n_local)              # every rank's stream length, once per run
+        nw = n_world.cpu().numpy()
+        J = batched_rounds(nw, engine.params)
+        if J:
+            n_max = int(nw.max())
+            call(engine.spec_form, J, n_max)
+            g_local = call(engine.spec_table)
+            if g_local is None or g_local.numel() != J * engine.n_ranks:
+                g_local = torch.zeros(J * engine.n_ranks, dtype=torch.int32, device=dev)
+            g_world = torch.zeros(J * world_ranks, dtype=torch.int32, device=dev)
+            yield ("all_gather", g_world, g_local)          # the G tables of all those rounds (batched)
+            call(engine.spec_commit, g_world, n_world, world_ranks // engine.n_ranks)
+            win = call(engine.spec_step_window, n_max)
+            if win is None or win.numel() != n_max:
+                win = torch.zeros(n_max, dtype=torch.int32, device=dev)
+            yield ("all_reduce_sum", win)                   # global e_k of the committed rounds' steps
+            st = call(engine.spec_status, J)
+            worst = yield ("max_int", int(err[0]))
+            if worst:
+                raise exc[0] if exc[0] is not None else B.OdbError(int(worst), "plan_protocol (a peer process failed)")
+            round_T.extend(st[2])
     j = 0
     while True:
         if avail_schedule is not None:

@@ -119,6 +119,73 @@ class OracleEngine:
         self.s_emit += sum(e[:T_emit])
         self.round += 1
 
+    # ---- batched exchange (dist.py): every round that starts without leftovers, from the oracle's pieces ----
+    def stream_lengths(self):
+        return torch.tensor([len(x) for x in self.lens], dtype=torch.int32)
+
+    def spec_form(self, n_rounds, world_max_stream):
+        bs = self.p["buffer_size"]
+        self.spec_J = n_rounds
+        self.spec_cand = []
+        g = torch.zeros(n_rounds * self.R, dtype=torch.int32)
+        for j in range(n_rounds):
+            row = []
+            for r in range(self.R):
+                ids = np.arange(min(j * bs, len(self.lens[r])), min((j + 1) * bs, len(self.lens[r])), dtype=np.int32)
+                c = self.o.group_window(self.p["rule"], self.p["budget"], self.lens[r], ids) if len(ids) else []
+                row.append(c)
+                g[j * self.R + r] = len(c)
+            self.spec_cand.append(row)
+        self.spec_g = g
+        self.window = torch.zeros(max(int(world_max_stream), 1), dtype=torch.int32)
+
+    def spec_table(self):
+        return self.spec_g
+
+    def spec_commit(self, g_world, n_world, n_procs):
+        bs, J = self.p["buffer_size"], self.spec_J
+        G = g_world.numpy().astype(np.int64).reshape(n_procs, J, self.R)
+        n = n_world.numpy().astype(np.int64).reshape(n_procs, self.R)
+        self.spec_T, base = [], 0
+        self.spec_sb = []
+        for j in range(J):
+            Gj = G[:, j, :].reshape(-1)
+            Sj = np.clip(n.reshape(-1) - j * bs, 0, bs)
+            if not (Gj > 0).any():
+                break
+            T = self.o.target_groups(Gj, Sj, self.p["slot_capacity"])
+            if (Gj > T).any():      # some rank would overflow: leftovers, the round-by-round protocol takes over
+                break
+            self.spec_T.append(T)
+            self.spec_sb.append(base)
+            base += T
+        for j, T in enumerate(self.spec_T):
+            for r in range(self.R):
+                cand = self.spec_cand[j][r]
+                if cand:
+                    al, back = self.o.align_list(cand, T)
+                    assert len(back) == 0
+                    for k, grp in enumerate(al):
+                        self.window[self.spec_sb[j] + k] += len(grp)
+                    self.slots[r].extend(list(x) for x in al)
+                else:
+                    self.slots[r].extend([] for _ in range(T))
+        js = len(self.spec_T)
+        for r in range(self.R):
+            self.pos[r] = min(js * bs, len(self.lens[r]))
+            self.buf[r] = []
+        self.spec_steps = base
+
+    def spec_step_window(self, n):
+        return self.window[:n]
+
+    def spec_status(self, max_rounds):
+        e = self.window[:self.spec_steps].tolist()     # global after the all_reduce
+        self.step_samples.extend(e)
+        self.s_emit += sum(e)
+        self.round = len(self.spec_T)
+        return len(self.spec_T), self.spec_steps, list(self.spec_T)
+
     def round_status(self):
         if self.done:
             return 1, 0

@@ -22,7 +22,7 @@ def _free_port():
 
 
 CASES = ["tiny", "unequal", "empty_rank", "overflow_multiround", "overflow_nonjoin_quota", "nonjoin_logical",
-         "one_process_idle"]
+         "one_process_idle", "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit"]
 
 
 def _case(name):
@@ -39,7 +39,31 @@ def _case(name):
         rng = np.random.default_rng(1)
         return I.custom_workload("one_process_idle", [rng.integers(8, 300, 50), rng.integers(8, 300, 70), [], []],
                                  seed=3, budget=1024, buffer_size=16)
+    if name.startswith("batched"):   # several rounds without leftovers: the batched exchange commits them at once
+        rng = np.random.default_rng(len(name))
+        n = {"batched_equal": (400, 400, 400, 400), "batched_ragged": (390, 412, 0, 405),
+             "batched_nonjoin": (300, 260, 280, 310), "batched_maxfit": (200, 333, 333, 90)}[name]
+        return I.custom_workload(name, [rng.integers(8, 700, k) for k in n], seed=7, budget=2048, buffer_size=40,
+                                 join_mode=0 if name == "batched_nonjoin" else 1, rule=1 if name == "batched_maxfit" else 0)
     return I.protocol_workload(name, 2)
+
+
+def test_batched_rounds_host_logic():
+    """Which rounds the batched exchange may take (dist.batched_rounds): join -- until the longest stream is drained;
+    non-join -- until the shortest is; never with a quota, tiny or huge buffers, or a single round."""
+    from types import SimpleNamespace as NS
+    sys.path.insert(0, ROOT)
+    from paper_2606_19989_b200 import dist as D
+    n = np.array([100, 250, 0, 31])
+    assert D.batched_rounds(n, NS(buffer_size=50, join_mode=1, sample_quota=0)) == 5
+    assert D.batched_rounds(n, NS(buffer_size=50, join_mode=0, sample_quota=0)) == 0      # a stream is empty: round 0 is terminal
+    assert D.batched_rounds(n + 60, NS(buffer_size=50, join_mode=0, sample_quota=0)) == 2
+    assert D.batched_rounds(n + 60, NS(buffer_size=50, join_mode=0, sample_quota=10)) == 0
+    assert D.batched_rounds(n, NS(buffer_size=4, join_mode=1, sample_quota=0)) == 0
+    assert D.batched_rounds(n, NS(buffer_size=0, join_mode=1, sample_quota=0)) == 0
+    assert D.batched_rounds(n, NS(buffer_size=5000, join_mode=1, sample_quota=0)) == 0
+    assert D.batched_rounds(n, NS(buffer_size=250, join_mode=1, sample_quota=0)) == 0     # one round: nothing to batch
+    assert D.batched_rounds(np.array([10**7]), NS(buffer_size=8, join_mode=1, sample_quota=0)) == 0   # too many rounds
 
 
 def _worker(rank, world, port, q):
@@ -76,7 +100,11 @@ def _failing_worker(rank, world, port, q, fail_round):
         wl = _case("overflow_multiround")
         rl = wl.n_ranks // world
         eng = OracleEngine(odb_oracle, I.split_ranks(wl, world)[rank])
-        if rank == 1:
+        if rank == 1 and fail_round == "spec":
+            def boom(*a):
+                raise B.OdbError(B.ODB_ERR_BAD_LENGTH, "OracleEngine.spec_form (injected failure)")
+            eng.spec_form = boom
+        elif rank == 1:
             eng.fail_at_round = fail_round
         try:
             D.run(D.plan_protocol(eng, wl.n_ranks, rank * rl), D.TorchCollectives())
@@ -87,7 +115,7 @@ def _failing_worker(rank, world, port, q, fail_round):
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("fail_round", [0, 3])
+@pytest.mark.parametrize("fail_round", [0, 3, "spec"])
 def test_a_failing_process_takes_its_peers_down_instead_of_hanging_them(fail_round):
     """One process's engine fails (a bad length, say) in some round: every process issues that round's collectives
     and then raises, together (the MAX exchange of the error status at the end of every round)."""
@@ -148,7 +176,8 @@ def test_lockstep_driver_with_oracle_engines(n_proc):
     from tests._oracle_engine import OracleEngine
     from tests.test_oracle_arrival import _random_schedule
     odb_oracle.build()
-    for name in ("unequal", "empty_rank", "overflow_multiround", "overflow_nonjoin_quota", "audit:longtail"):
+    for name in ("unequal", "empty_rank", "overflow_multiround", "overflow_nonjoin_quota", "audit:longtail",
+                 "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit"):
         for with_sched in (False, True):
             wl = _case(name) if not name.startswith("audit") else I.protocol_workload(name, 2)
             if wl.n_ranks % n_proc:
@@ -160,6 +189,9 @@ def test_lockstep_driver_with_oracle_engines(n_proc):
             res = D.run_lockstep([D.plan_protocol(e, wl.n_ranks, p * rl,
                                                   None if sched is None else [row[p * rl:(p + 1) * rl] for row in sched])
                                   for p, e in enumerate(engines)])
+            if name.startswith("batched") and not with_sched:   # the batched exchange committed rounds (all of them
+                committed = len(engines[0].spec_T)              # when the streams are equal)
+                assert committed >= 2 and (name != "batched_equal" or committed == plan.n_rounds - 1), (name, committed)
             for p, (info, round_T) in enumerate(res):
                 assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason), name
                 assert round_T == plan.round_T.tolist() and info.step_samples == plan.step_samples.tolist()

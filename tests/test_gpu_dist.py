@@ -49,13 +49,20 @@ def _case(name):
                                  sample_quota=0 if join else 42)
     if name == "maxfit_overflow":
         return I.protocol_workload("overflow_multiround", 5, rule=1)
+    if name.startswith("batched"):   # several rounds without leftovers: the batched exchange commits them at once
+        rng = np.random.default_rng(len(name))
+        n = {"batched_equal": (3000, 3000, 3000, 3000), "batched_ragged": (3000, 2817, 0, 3105),
+             "batched_nonjoin": (3000, 2600, 2800, 3100), "batched_maxfit": (2000, 3333, 3333, 900)}[name]
+        return I.custom_workload(name, [rng.integers(8, 1500, k) for k in n], seed=7, budget=8192, buffer_size=256,
+                                 join_mode=0 if name == "batched_nonjoin" else 1, rule=1 if name == "batched_maxfit" else 0)
     return I.protocol_workload(name, 2)
 
 
 @pytest.mark.parametrize("n_proc", [2, 4])
 @pytest.mark.parametrize("name", ["tiny", "config2_slice", "unequal", "empty_rank", "overflow_multiround",
                                   "overflow_nonjoin_quota", "maxfit_overflow", "config4_slice_nonjoin",
-                                  "audit:bimodal", "sampleless_process_join", "sampleless_process_nonjoin"])
+                                  "audit:bimodal", "sampleless_process_join", "sampleless_process_nonjoin",
+                                  "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit"])
 def test_lockstep_processes_match_whole_job_oracle(P, oracle, name, n_proc):
     import torch
     from paper_2606_19989_b200 import dist as D
@@ -157,6 +164,63 @@ def test_lockstep_with_arrival_schedule(P, oracle):
                 e.close()
 
 
+def test_batched_exchange_commits_rounds_and_equals_the_round_by_round_protocol(P, oracle):
+    """The batched exchange (odb_dist_spec_form / _commit / _status): equal streams -- every data round is committed
+    with three collectives; ragged streams -- the tail falls to the per-round protocol; the plan is the oracle's
+    either way and equals the protocol with one exchange per round (batched=False)."""
+    import torch
+    from paper_2606_19989_b200 import dist as D
+    for name, all_rounds in (("batched_equal", True), ("batched_ragged", False), ("batched_nonjoin", True)):
+        wl = _case(name)
+        plan, _ = oracle.run_workload(wl, collate=False)
+        R = wl.n_ranks
+        parts = I.split_ranks(wl, 2)
+        dws = [Par.DeviceWorkload(w) for w in parts]
+        for batched in (True, False):
+            engines = [D.CudaEngine(Par.gpu_params(w), max(w.n_samples, 1), dw.lengths, w.rank_ptr) for w, dw in zip(parts, dws)]
+            try:
+                n_coll = [0]
+
+                def counted(gen):
+                    reply = None
+                    while True:
+                        try:
+                            req = gen.send(reply)
+                        except StopIteration as e:
+                            return e.value
+                        n_coll[0] += 1
+                        reply = yield req
+
+                res = D.run_lockstep([counted(D.plan_protocol(e, R, p * 2, batched=batched)) for p, e in enumerate(engines)])
+                for p, e in enumerate(engines):
+                    info, round_T = res[p]
+                    assert round_T == plan.round_T.tolist(), (name, batched)
+                    assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason)
+                    rec = np.zeros(4, dtype=np.int32)
+                    got = P.odb_debug_read(e.ctx.h, 4, rec)
+                    if batched:
+                        assert got == 16 and rec[0] >= 2
+                        assert (rec[0] == plan.n_rounds - 1) == all_rounds, (name, rec)
+                    else:
+                        assert got < 0
+                    out = P.OutputBuffers.for_plan(2, info, dws[p].device)
+                    e.collate(dws[p].tokens, dws[p].sample_ptr, dws[p].span_ptr, dws[p].span_lo, dws[p].span_hi, out)
+                    torch.cuda.synchronize()
+                    K = plan.n_steps
+                    s0, s1 = p * 2 * K, (p + 1) * 2 * K
+                    assert np.array_equal(out.table("grp_count").cpu().numpy(), plan.grp_count[s0:s1])
+                    assert np.array_equal(out.table("grp_width").cpu().numpy(), plan.grp_width[s0:s1])
+                    assert np.array_equal(out.table("step_samples").cpu().numpy(), plan.step_samples)
+                per_proc = n_coll[0] // 2
+                if batched and all_rounds:     # 1 (window) + 4 (batched phase) + 3 (the terminal check round)
+                    assert per_proc == 8, per_proc
+                if not batched:                # 1 + 3 per round, terminal check included
+                    assert per_proc == 1 + 3 * plan.n_rounds, per_proc
+            finally:
+                for e in engines:
+                    e.close()
+
+
 def test_single_process_nccl_world(P, oracle):
     """The torch.distributed driver itself (NCCL, world_size 1 -- the box has one GPU): the protocol
     with real collectives on the library's device buffers equals the oracle."""
@@ -208,7 +272,13 @@ def test_dist_mode_errors(P):
         with pytest.raises(P.OdbError):               # the caller drives the rounds in this mode
             P.odb_run(ctx.h, dw.lengths, wl.rank_ptr, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi,
                       empty.struct)
+        with pytest.raises(P.OdbError):               # a 2048-sample budget workload with buffer_size 0: no batched exchange
+            P.odb_dist_spec_form(ctx.h, dw.lengths, wl.rank_ptr, 2, 64)
+        with pytest.raises(P.OdbError):
+            P.odb_dist_spec_status(ctx.h, 4)          # nothing formed
         P.odb_dist_config(ctx.h, 0, 0, 0)             # back to single-process mode
+        with pytest.raises(P.OdbError):
+            P.odb_dist_spec_form(ctx.h, dw.lengths, wl.rank_ptr, 2, 64)
         Par.run_gpu(wl, dw, staged=False)
 
 
