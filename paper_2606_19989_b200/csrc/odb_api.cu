@@ -1095,6 +1095,9 @@ int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_
         CU(c, cudaEventCreateWithFlags(&T.ev_plan, cudaEventDisableTiming));
         T.ready = true;
     }
+    // the full plan's slot CSR (state 5) tells where a rank's rows of the range start in its emit region
+    const int64_t *full_sp = (c->state == 5 && c->info_valid && c->n_steps > 0) ? c->grp_sample_ptr.p : nullptr;
+    const int full_K = c->n_steps;
     // (a set is reused by every second call: its previous plan sizes have been read, its kernels are ordered by
     //  the caller's streams -- at most two step ranges in flight)
     swap_tabs(c, T);
@@ -1120,7 +1123,7 @@ int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_
         CU(c, launch_finalize(c, slots, cap, nullptr, st, step_lo));
         CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
         CU(c, cudaEventRecord(c->ev_plan, st));
-        CU(c, launch_sub_ids(c, step_lo, o->d_grp_sample_ids, st));
+        CU(c, launch_sub_ids(c, step_lo, o->d_grp_sample_ids, full_sp, full_K, st));
         if (!arenas) return ODB_OK;  // a sizing call
         return enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, c->n_total, tile_bound, st);
     }();

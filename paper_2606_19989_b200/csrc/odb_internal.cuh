@@ -360,7 +360,8 @@ cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap
 // step-range plans: PlanDims of the range, and the slot CSR's ids of its rows (global in the library's table, local
 // in the caller's)
 cudaError_t launch_sub_dims(odb_ctx *c, int n_steps, cudaStream_t st);
-cudaError_t launch_sub_ids(odb_ctx *c, int step_lo, int32_t *user_ids, cudaStream_t st);
+// (full_sp: the full plan's grp_sample_ptr over full_K steps per rank when it exists, else NULL)
+cudaError_t launch_sub_ids(odb_ctx *c, int step_lo, int32_t *user_ids, const int64_t *full_sp, int full_K, cudaStream_t st);
 // ---- segment-level pieces shared with the offline planners (odb_offline.cu) -------------------------
 struct SortArgs;
 cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A, int64_t nseg, int maxS, cudaStream_t st);

@@ -2063,14 +2063,18 @@ cudaError_t launch_sub_dims(odb_ctx *c, int n_steps, cudaStream_t st) {
 __global__ void __launch_bounds__(1024)
 k_sub_ids(const PlanDims *dims, int R, int step_lo, const int32_t *__restrict__ st_count, const int64_t *__restrict__ rank_ptr,
           const int32_t *__restrict__ emit_ids, const int64_t *__restrict__ grp_sample_ptr, int32_t *__restrict__ ids,
-          int32_t *__restrict__ user_ids) {
+          int32_t *__restrict__ user_ids, const int64_t *__restrict__ full_sp, int full_K) {
     __shared__ long long s_scan64[34];
     if (!dims->complete || dims->err) return;
     const int r = blockIdx.x, n = dims->n_steps;
-    long long part = 0;  // samples of rank r in the steps before the range
-    for (int k = threadIdx.x; k < step_lo; k += blockDim.x) part += st_count[(int64_t)k * R + r];
-    long long e_lo;
-    (void)block_excl_scan<long long>(part, s_scan64, e_lo);
+    long long e_lo;  // samples of rank r in the steps before the range
+    if (full_sp) {   // the full plan's slot CSR knows it
+        e_lo = full_sp[(int64_t)r * full_K + step_lo] - full_sp[(int64_t)r * full_K];
+    } else {         // between rounds: sum the staging table's column
+        long long part = 0;
+        for (int k = threadIdx.x; k < step_lo; k += blockDim.x) part += st_count[(int64_t)k * R + r];
+        (void)block_excl_scan<long long>(part, s_scan64, e_lo);
+    }
     const int64_t base = rank_ptr[r];
     const int64_t q0 = grp_sample_ptr[(int64_t)r * n], q1 = grp_sample_ptr[(int64_t)(r + 1) * n];
     for (int64_t i = threadIdx.x; i < q1 - q0; i += blockDim.x) {
@@ -2080,9 +2084,9 @@ k_sub_ids(const PlanDims *dims, int R, int step_lo, const int32_t *__restrict__ 
     }
 }
 
-cudaError_t launch_sub_ids(odb_ctx *c, int step_lo, int32_t *user_ids, cudaStream_t st) {
+cudaError_t launch_sub_ids(odb_ctx *c, int step_lo, int32_t *user_ids, const int64_t *full_sp, int full_K, cudaStream_t st) {
     k_sub_ids<<<c->prm.n_ranks, 1024, 0, st>>>(c->d_dims, c->prm.n_ranks, step_lo, c->st_count.p, c->d_rank_ptr, c->emit_ids,
-                                              c->grp_sample_ptr.p, c->grp_sample_ids.p, user_ids);
+                                              c->grp_sample_ptr.p, c->grp_sample_ids.p, user_ids, full_sp, full_K);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
