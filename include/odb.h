@@ -358,8 +358,8 @@ ODB_API int odb_offline_plan(odb_ctx *ctx, const odb_offline_params *params, con
  * ODB_OPT_ROUND_PARALLEL (value 0 / 1, default 1): with a grouping buffer of 8 .. 4096 samples (the paper's
  * operating point) odb_run forms and commits the protocol rounds round-parallel -- a round depends on its
  * predecessors only through the leftovers, and there are none until a round overflows -- and the
- * sequential round loop resumes at the first round that does; 0 = every round in the sequential loop.  Same
- * results bit for bit.
+ * sequential round loop resumes at the first round that does (with a sample quota: at the latest at the round whose
+ * cumulative emission reaches it); 0 = every round in the sequential loop.  Same results bit for bit.
  * ODB_OPT_HOST_DEVICE_ARENAS (value 0 / 1, default 0): the four arena pointers of odb_run_host's `h_out_bufs` are
  * DEVICE memory (16-byte aligned, arena_capacity elements): the inputs still come from host buffers rank by rank,
  * but every rank's slots are collated in place as soon as its tokens have landed and the batches stay on the device

@@ -992,14 +992,36 @@ static int fused_rounds(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_r
     // rounds that are certainly not the terminal check (join: some stream still holds views; non-join: every
     // stream does): formed and committed round-parallel as long as no round overflows (odb_plan.cu)
     int64_t spec_rounds = 0;
-    if (c->round_parallel && c->prm.buffer_size >= kSpecMinWindow && (c->prm.join_mode || c->prm.sample_quota <= 0)) {
+    bool spec_terminal = true;
+    if (c->round_parallel && c->prm.buffer_size >= kSpecMinWindow) {
         const int64_t B = c->prm.buffer_size;
         int64_t min_nr = max_nr;
         for (int r = 0; r < R; ++r) min_nr = std::min(min_nr, h_rank_ptr[r + 1] - h_rank_ptr[r]);
         spec_rounds = ((c->prm.join_mode ? max_nr : min_nr) + B - 1) / B;
+        if (!c->prm.join_mode && c->prm.sample_quota > 0) {
+            // non-join with a sample quota (Thm 2 / P:347): a round-parallel round emits its whole windows, so the
+            // rounds whose cumulative emission stays below the quota cannot contain the cut; the round that reaches
+            // it -- and the cut inside it -- belongs to the sequential loop.  (the emission after j rounds is
+            // monotone in j: bisection for the first j whose round reaches the quota)
+            auto emitted_after = [&](int64_t rounds) {
+                long long cum = (long long)c->prm.emitted_so_far;
+                for (int r = 0; r < R; ++r) cum += std::min<int64_t>(rounds * B, h_rank_ptr[r + 1] - h_rank_ptr[r]);
+                return cum;
+            };
+            int64_t lo = 0, hi = spec_rounds;  // the first j in [0, spec_rounds] with emitted_after(j + 1) >= quota
+            while (lo < hi) {
+                const int64_t mid = (lo + hi) / 2;
+                if (emitted_after(mid + 1) >= (long long)c->prm.sample_quota) hi = mid;
+                else lo = mid + 1;
+            }
+            if (lo < spec_rounds) {
+                spec_rounds = lo;
+                spec_terminal = false;
+            }
+        }
         if (spec_rounds < 2 || spec_rounds > kSpecMaxRounds) spec_rounds = 0;
     }
-    const cudaError_t le = launch_rounds(c, (int)spec_rounds, st);
+    const cudaError_t le = launch_rounds(c, (int)spec_rounds, spec_terminal, st);
     *le_out = le;
     if (le == cudaSuccess) {
         c->spec_used = spec_rounds > 0;

@@ -339,7 +339,8 @@ cudaError_t launch_round_align(odb_ctx *c, cudaStream_t st);  // A4..A8a + commi
 // every protocol round in one cooperative launch; cudaErrorNotSupported if R CTAs cannot be resident
 // `spec_rounds` > 0: the rounds [0, spec_rounds) are first formed and committed round-parallel (k_spec_form /
 // k_spec_commit) and the persistent kernel resumes where that speculation stops
-cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st);
+// (spec_terminal: the round behind them is the terminal check -- false when a sample quota ends the speculation)
+cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, bool spec_terminal, cudaStream_t st);
 // scratch entries per rank-sized table (gpos, agpos, ...): every (rank, round) window of the round-parallel
 // planner owns S + 1 entries
 inline size_t plan_table_entries(size_t N, size_t R) { return N + N / 8 + 2 * R + 64; }

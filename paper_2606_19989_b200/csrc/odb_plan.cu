@@ -1094,6 +1094,18 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
     __syncthreads();
     long long emitted_before = A.emitted_before;
     const bool quota_mode = !A.join_mode && A.quota > 0;
+    if (A.spec && quota_mode && round0 > 0) {
+        // the committed rounds emitted their whole windows: the first round0 * B views of every stream (or all of it)
+        __shared__ long long s_emit64[34];
+        long long part = 0;
+        for (int q = t; q < R; q += kMsThreads) {
+            const long long nq = SA.rank_ptr[q + 1] - SA.rank_ptr[q];
+            part += min((long long)round0 * SA.buffer_size, nq);
+        }
+        long long tot;
+        (void)block_excl_scan<long long>(part, s_emit64, tot);
+        emitted_before += tot;
+    }
     for (int round = round0; run_loop; ++round) {
         // ---- A0 + A1: this rank's window, sorted ----
         const int nl = s_state[0], fp = s_state[1], cur = s_state[2];
@@ -1213,8 +1225,10 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
 //                  when j* is the terminal check).
 // The rounds that are terminal checks are known on the host (join: the first round in which every stream is
 // drained; non-join without a quota: the first in which one is), so the grid holds only non-terminal rounds.
-// Not used with a sample quota (the cut needs the running emitted count), with arrival schedules, or in
-// distributed mode.  Results are those of the sequential loop by construction; tests compare both with the oracle.
+// With a sample quota the grid ends before the round whose cumulative emission reaches it (the host knows that
+// round: committed rounds emit whole windows) and that round, with its cut, is the loop's.  Not used with arrival
+// schedules; distributed mode gathers the G tables first (k_spec_T_world).  Results are those of the sequential
+// loop by construction; tests compare both with the oracle.
 // ---------------------------------------------------------------------------------------------
 struct SpecArgs {
     SortArgs sort;
@@ -1223,6 +1237,7 @@ struct SpecArgs {
     int rule, join_mode, slot_capacity;
     int x_keys;  // padded sort keys the shared-memory layout reserves
     int eval_T;  // 1: the launch closes the rounds itself (all ranks are local); 0: only the G table (distributed mode)
+    int terminal_after;  // 1: the round behind the grid is the terminal check; 0: it is an ordinary round (quota mode)
     int32_t *gpos, *agpos, *agcnt, *agorg;
     int32_t *st_count, *st_width, *st_real, *st_round, *st_origin;
     int32_t *emit_ids, *left_ids_w;
@@ -1324,7 +1339,7 @@ __global__ void __launch_bounds__(kMsThreads) k_spec_form(const SpecArgs A) {
     if (t == 0) {
         A.rec->j_star = js;
         A.rec->n_steps = carry;
-        A.rec->complete = js == A.n_rounds ? 1 : 0;
+        A.rec->complete = (js == A.n_rounds && A.terminal_after) ? 1 : 0;
         A.rec->pad_ = 0;
         A.ctr[kSpecMaxRounds] = 0u;
     }
@@ -1827,8 +1842,8 @@ static int host_active_keys(int S) {
 }
 
 // Arguments, block size and shared memory of the round-parallel planner's kernels for `spec_rounds` rounds.
-static cudaError_t make_spec_args(odb_ctx *c, int spec_rounds, int eval_T, cudaStream_t st, SpecArgs *out, int *threads_out,
-                                  size_t *smem_out) {
+static cudaError_t make_spec_args(odb_ctx *c, int spec_rounds, int eval_T, int terminal_after, cudaStream_t st, SpecArgs *out,
+                                  int *threads_out, size_t *smem_out) {
     const int R = c->prm.n_ranks;
     const int B = c->prm.buffer_size;
     const int n_keys = host_active_keys(B);
@@ -1872,6 +1887,7 @@ static cudaError_t make_spec_args(odb_ctx *c, int spec_rounds, int eval_T, cudaS
     P.slot_capacity = c->prm.slot_capacity;
     P.x_keys = (int)(x_bytes / 8);
     P.eval_T = eval_T;
+    P.terminal_after = terminal_after;
     P.gpos = c->gpos;
     P.agpos = c->agpos;
     P.agcnt = c->agcnt;
@@ -1892,7 +1908,7 @@ static cudaError_t make_spec_args(odb_ctx *c, int spec_rounds, int eval_T, cudaS
     return cudaSuccess;
 }
 
-cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st) {
+cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, bool spec_terminal, cudaStream_t st) {
     const int R = c->prm.n_ranks;
     const size_t smem = kRoundsSmem;
     if (c->rounds_max_ctas == 0) {
@@ -1964,7 +1980,7 @@ cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, cudaStream_t st) {
         SpecArgs P;
         int threads = 0;
         size_t sp_smem = 0;
-        e = make_spec_args(c, spec_rounds, 1, st, &P, &threads, &sp_smem);
+        e = make_spec_args(c, spec_rounds, 1, spec_terminal ? 1 : 0, st, &P, &threads, &sp_smem);
         if (e != cudaSuccess) return e;
         k_spec_form<<<dim3((unsigned)R, (unsigned)spec_rounds), threads, sp_smem, st>>>(P);
         ODB_LAUNCH_CHECK(c);
@@ -1986,7 +2002,7 @@ cudaError_t launch_dist_spec_form(odb_ctx *c, int n_rounds, int32_t **G_tab_out,
     SpecArgs P;
     int threads = 0;
     size_t sp_smem = 0;
-    cudaError_t e = make_spec_args(c, n_rounds, 0, st, &P, &threads, &sp_smem);
+    cudaError_t e = make_spec_args(c, n_rounds, 0, 1, st, &P, &threads, &sp_smem);
     if (e != cudaSuccess) return e;
     k_spec_form<<<dim3((unsigned)c->prm.n_ranks, (unsigned)n_rounds), threads, sp_smem, st>>>(P);
     ODB_LAUNCH_CHECK(c);
@@ -2002,7 +2018,7 @@ cudaError_t launch_dist_spec_commit(odb_ctx *c, int n_rounds, const int32_t *d_G
     SpecArgs P;
     int threads = 0;
     size_t sp_smem = 0;
-    cudaError_t e = make_spec_args(c, n_rounds, 0, st, &P, &threads, &sp_smem);
+    cudaError_t e = make_spec_args(c, n_rounds, 0, 1, st, &P, &threads, &sp_smem);
     if (e != cudaSuccess) return e;
     const int R = c->prm.n_ranks;
     k_spec_T_world<<<1, 1024, 0, st>>>(d_G_world, d_n_world, n_procs, R, n_rounds, c->prm.buffer_size, c->prm.slot_capacity,

@@ -256,14 +256,16 @@ def _stream_lengths(rng, n, hi=3000):
 
 
 @pytest.mark.parametrize("rule", [0, 1])
-@pytest.mark.parametrize("case", ["equal", "ragged_tail", "short_rank", "nonjoin", "capacity", "tiny_buffer", "full_chunk"])
+@pytest.mark.parametrize("case", ["equal", "ragged_tail", "short_rank", "nonjoin", "nonjoin_quota", "capacity", "tiny_buffer",
+                                  "full_chunk"])
 def test_round_parallel_planner(P, oracle, case, rule):
     """The round-parallel planner (k_spec_form / k_spec_commit, ODB_OPT_ROUND_PARALLEL): every round that starts
     without leftovers is formed at once, the sequential loop resumes at the first round that overflows.  Equal
     streams (the whole run is round-parallel), ragged tails (the last windows differ: S+min caps T, the tail is
     sequential), a rank that finishes early (IDLE slots beside round-parallel rounds), non-join without a quota
     (the terminal round is the first in which a stream is drained), finite slot capacity (overflow in round 0:
-    nothing is committed round-parallel), an 8-sample buffer and full 4096-key windows.  Plan tables in full and
+    nothing is committed round-parallel), non-join with a sample quota (the rounds below the quota are round-parallel,
+    the round that reaches it and its cut are the loop's), an 8-sample buffer and full 4096-key windows.  Plan tables in full and
     every element of every slot against the oracle; the sequential loop (option off) gives the same."""
     rng = np.random.default_rng(7 + rule)
     kw = dict(budget=8192, rule=rule, join_mode=1)
@@ -279,6 +281,10 @@ def test_round_parallel_planner(P, oracle, case, rule):
     elif case == "nonjoin":
         per, kw["buffer_size"], kw["join_mode"] = [_stream_lengths(rng, n) for n in (3000, 2048, 2600)], 256, 0
         expect = ("all", 8)
+    elif case == "nonjoin_quota":   # 768 samples per round: the sixth round reaches the quota, the cut is the loop's
+        per, kw["buffer_size"], kw["join_mode"] = [_stream_lengths(rng, n) for n in (3000, 2048, 2600)], 256, 0
+        kw["sample_quota"] = 4000
+        expect = ("quota", 5)
     elif case == "capacity":
         per, kw["buffer_size"], kw["slot_capacity"] = [_stream_lengths(rng, 3000, 200) for _ in range(3)], 512, 3
         expect = ("some", 0)
@@ -298,6 +304,8 @@ def test_round_parallel_planner(P, oracle, case, rule):
     committed, steps, ended = int(rec[0][0]), int(rec[0][1]), int(rec[0][2])
     if expect[0] == "all":
         assert ended == 1 and committed == expect[1] == plan.n_rounds - 1 and steps == plan.n_steps
+    elif expect[0] == "quota":
+        assert ended == 0 and committed == expect[1] == plan.n_rounds - 1 and plan.stop_reason == 2 and steps < plan.n_steps
     else:
         assert ended == 0 and committed < plan.n_rounds - 1
         assert committed == expect[1] if expect[1] is not None else committed >= 4
@@ -310,8 +318,8 @@ def test_round_parallel_planner(P, oracle, case, rule):
 
 def test_round_parallel_planner_fuzz(P, oracle):
     """120 random jobs in the round-parallel planner's regime (grouping buffers of 8 .. 700 samples, up to 12 ranks
-    with unequal streams of up to 4000 samples, both rules, join and non-join without a quota, finite slot capacity in
-    a third of them): the plan tables in full and sampled slots element by element against the oracle.  The planner
+    with unequal streams of up to 4000 samples, both rules, join and non-join with and without a quota, finite slot
+    capacity in a third of them): the plan tables in full and sampled slots element by element against the oracle.  The planner
     must have run, and the rounds it committed never exceed the plan's."""
     used = 0
     for seed in range(120):
@@ -326,6 +334,9 @@ def test_round_parallel_planner_fuzz(P, oracle):
         wl = I.custom_workload("rp_fuzz", per, seed, budget=int(rng.choice([64, 1024, 8192, 60000])), buffer_size=B,
                                slot_capacity=int(rng.choice([0, 0, 5, 40])), rule=int(rng.integers(0, 2)),
                                join_mode=int(rng.integers(0, 2)), shift_labels=int(rng.integers(0, 2)))
+        if not wl.params["join_mode"] and rng.uniform() < 0.5:
+            wl.params["sample_quota"] = int(rng.integers(1, max(2, wl.n_samples + 1)))
+            wl.params["emitted_so_far"] = int(rng.choice([0, 0, 17]))
         plan, _ = oracle.run_workload(wl, collate=False)
         rec = []
         info, out, _ = Par.run_gpu(wl, staged=False, spec_rec=rec)
@@ -336,7 +347,10 @@ def test_round_parallel_planner_fuzz(P, oracle):
         if rec[0] is not None:
             used += 1
             assert 0 <= int(rec[0][0]) <= plan.n_rounds - 1 and int(rec[0][1]) <= plan.n_steps
-            assert (int(rec[0][2]) == 1) == (int(rec[0][0]) == plan.n_rounds - 1)
+            if plan.stop_reason != 2:   # (a quota stop is never the planner's: the cut belongs to the loop)
+                assert (int(rec[0][2]) == 1) == (int(rec[0][0]) == plan.n_rounds - 1)
+            else:
+                assert int(rec[0][2]) == 0
     assert used >= 60
 
 
