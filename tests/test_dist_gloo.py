@@ -22,7 +22,8 @@ def _free_port():
 
 
 CASES = ["tiny", "unequal", "empty_rank", "overflow_multiround", "overflow_nonjoin_quota", "nonjoin_logical",
-         "one_process_idle", "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit"]
+         "one_process_idle", "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit",
+         "batched_idle_process"]
 
 
 def _case(name):
@@ -42,7 +43,8 @@ def _case(name):
     if name.startswith("batched"):   # several rounds without leftovers: the batched exchange commits them at once
         rng = np.random.default_rng(len(name))
         n = {"batched_equal": (400, 400, 400, 400), "batched_ragged": (390, 412, 0, 405),
-             "batched_nonjoin": (300, 260, 280, 310), "batched_maxfit": (200, 333, 333, 90)}[name]
+             "batched_nonjoin": (300, 260, 280, 310), "batched_maxfit": (200, 333, 333, 90),
+             "batched_idle_process": (0, 0, 290, 300)}[name]
         return I.custom_workload(name, [rng.integers(8, 700, k) for k in n], seed=7, budget=2048, buffer_size=40,
                                  join_mode=0 if name == "batched_nonjoin" else 1, rule=1 if name == "batched_maxfit" else 0)
     return I.protocol_workload(name, 2)
@@ -177,7 +179,7 @@ def test_lockstep_driver_with_oracle_engines(n_proc):
     from tests.test_oracle_arrival import _random_schedule
     odb_oracle.build()
     for name in ("unequal", "empty_rank", "overflow_multiround", "overflow_nonjoin_quota", "audit:longtail",
-                 "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit"):
+                 "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit", "batched_idle_process"):
         for with_sched in (False, True):
             wl = _case(name) if not name.startswith("audit") else I.protocol_workload(name, 2)
             if wl.n_ranks % n_proc:

@@ -52,7 +52,8 @@ def _case(name):
     if name.startswith("batched"):   # several rounds without leftovers: the batched exchange commits them at once
         rng = np.random.default_rng(len(name))
         n = {"batched_equal": (3000, 3000, 3000, 3000), "batched_ragged": (3000, 2817, 0, 3105),
-             "batched_nonjoin": (3000, 2600, 2800, 3100), "batched_maxfit": (2000, 3333, 3333, 900)}[name]
+             "batched_nonjoin": (3000, 2600, 2800, 3100), "batched_maxfit": (2000, 3333, 3333, 900),
+             "batched_idle_process": (0, 0, 2900, 3000)}[name]
         return I.custom_workload(name, [rng.integers(8, 1500, k) for k in n], seed=7, budget=8192, buffer_size=256,
                                  join_mode=0 if name == "batched_nonjoin" else 1, rule=1 if name == "batched_maxfit" else 0)
     return I.protocol_workload(name, 2)
@@ -62,7 +63,8 @@ def _case(name):
 @pytest.mark.parametrize("name", ["tiny", "config2_slice", "unequal", "empty_rank", "overflow_multiround",
                                   "overflow_nonjoin_quota", "maxfit_overflow", "config4_slice_nonjoin",
                                   "audit:bimodal", "sampleless_process_join", "sampleless_process_nonjoin",
-                                  "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit"])
+                                  "batched_equal", "batched_ragged", "batched_nonjoin", "batched_maxfit",
+                                  "batched_idle_process"])
 def test_lockstep_processes_match_whole_job_oracle(P, oracle, name, n_proc):
     import torch
     from paper_2606_19989_b200 import dist as D
