@@ -294,9 +294,13 @@ ODB_API int odb_commit(odb_ctx *ctx, void *stream);
  *                                                                          Lemma 3), split + commit of the rounds before
  *                                                                          the first that overflows
  *   all_reduce(SUM, d_step_samples_round[0 .. max n_r))                    [global e_k of those rounds' steps]
- *   odb_dist_spec_status(ctx, &rounds, &steps, h_T, capacity)              synchronises; rounds committed (0 .. J), their
- *                                                                          steps and T_grp; then the per-round calls go on
- *                                                                          with round `rounds` (odb_form_groups ...)
+ *   odb_dist_spec_status(ctx, &rounds, &steps, h_T, capacity, &done)       synchronises; rounds committed (0 .. J), their
+ *                                                                          steps and T_grp.  done = 1: all J were, round J
+ *                                                                          is the terminal check -- known to every process
+ *                                                                          from the same data, so it needs no exchange:
+ *                                                                          the protocol is over (odb_plan_query next);
+ *                                                                          done = 0: the per-round calls go on with round
+ *                                                                          `rounds` (odb_form_groups ...)
  *
  * J = rounds that are certainly not the terminal check: join ceil(max n_r / B), non-join ceil(min n_r / B), over ALL
  * ranks of the job (1 .. 65535).  Requirements (ODB_ERR_INVALID_ARG / ODB_ERR_STATE otherwise): distributed mode,
@@ -306,7 +310,8 @@ ODB_API int odb_dist_spec_form(odb_ctx *ctx, const int32_t *d_lengths, const int
                                int64_t world_max_stream, void *stream);
 ODB_API int odb_dist_spec_commit(odb_ctx *ctx, const int32_t *d_G_world, const int32_t *d_n_world, int32_t n_procs,
                                  void *stream);
-ODB_API int odb_dist_spec_status(odb_ctx *ctx, int32_t *h_rounds, int32_t *h_steps, int32_t *h_T, int32_t T_capacity);
+ODB_API int odb_dist_spec_status(odb_ctx *ctx, int32_t *h_rounds, int32_t *h_steps, int32_t *h_T, int32_t T_capacity,
+                                 int32_t *h_done);
 
 /* Device times of the last odb_run / odb_collate on this context, in milliseconds, measured with
  * CUDA events on the launching stream: ms[0] = planning (all rounds, plan query, row descriptors and

@@ -104,7 +104,7 @@ SYMBOLS = {
     "odb_dist_config": (_i32, [_vp, _i32, _i32, _i32]),
     "odb_dist_spec_form": (_i32, [_vp, _vp, _P(_i64), _i32, _i64, _vp]),
     "odb_dist_spec_commit": (_i32, [_vp, _vp, _vp, _i32, _vp]),
-    "odb_dist_spec_status": (_i32, [_vp, _P(_i32), _P(_i32), _P(_i32), _i32]),
+    "odb_dist_spec_status": (_i32, [_vp, _P(_i32), _P(_i32), _P(_i32), _i32, _P(_i32)]),
     "odb_dist_buffers": (_i32, [_vp, _P(odb_dist_bufs)]),
     "odb_commit": (_i32, [_vp, _vp]),
     "odb_set_timing": (_i32, [_vp, _i32]),
@@ -345,11 +345,12 @@ def odb_dist_spec_commit(ctx: int, d_G_world, d_n_world, n_procs: int, stream=No
 
 
 def odb_dist_spec_status(ctx: int, max_rounds: int):
-    """(rounds committed, their steps, [T_grp of each])."""
-    r, k = _i32(0), _i32(0)
+    """(rounds committed, their steps, [T_grp of each], done)."""
+    r, k, d = _i32(0), _i32(0), _i32(0)
     T = (ctypes.c_int32 * max(int(max_rounds), 1))()
-    _check(load().odb_dist_spec_status(ctx, ctypes.byref(r), ctypes.byref(k), T, int(max_rounds)), "odb_dist_spec_status", ctx)
-    return int(r.value), int(k.value), [int(T[j]) for j in range(r.value)]
+    _check(load().odb_dist_spec_status(ctx, ctypes.byref(r), ctypes.byref(k), T, int(max_rounds), ctypes.byref(d)),
+           "odb_dist_spec_status", ctx)
+    return int(r.value), int(k.value), [int(T[j]) for j in range(r.value)], int(d.value)
 
 
 def odb_commit(ctx: int, stream=None) -> None:

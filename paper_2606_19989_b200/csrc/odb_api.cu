@@ -636,7 +636,7 @@ int odb_dist_spec_commit(odb_ctx *c, const int32_t *d_G_world, const int32_t *d_
     return ODB_OK;
 }
 
-int odb_dist_spec_status(odb_ctx *c, int32_t *h_rounds, int32_t *h_steps, int32_t *h_T, int32_t T_capacity) {
+int odb_dist_spec_status(odb_ctx *c, int32_t *h_rounds, int32_t *h_steps, int32_t *h_T, int32_t T_capacity, int32_t *h_done) {
     if (!c) return ODB_ERR_INVALID_ARG;
     if (c->state != 8) return ODB_ERR_STATE;
     CU(c, cudaEventSynchronize(c->ev_status));
@@ -654,6 +654,17 @@ int odb_dist_spec_status(odb_ctx *c, int32_t *h_rounds, int32_t *h_steps, int32_
     c->spec_used = true;
     if (h_rounds) *h_rounds = js;
     if (h_steps) *h_steps = n_steps;
+    if (c->h_spec[2]) {
+        // every data round has been committed: round js is the terminal check (join: every stream is drained; non-join:
+        // one is).  Every process reads this from the same gathered data (Lemma 3), so the round needs no exchange.
+        c->stop_reason = c->prm.join_mode ? ODB_STOP_ALL_FINISHED : ODB_STOP_LOGICAL;
+        c->n_rounds = js + 1;
+        c->last_T = 0;
+        c->state = 4;
+        if (h_done) *h_done = 1;
+        return ODB_OK;
+    }
+    if (h_done) *h_done = 0;
     c->state = 3;  // between rounds: odb_form_groups continues with round js
     return ODB_OK;
 }

@@ -216,6 +216,8 @@ def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=Non
             if worst:
                 raise exc[0] if exc[0] is not None else B.OdbError(int(worst), "plan_protocol (a peer process failed)")
             round_T.extend(st[2])
+            if st[3]:  # every data round was committed: the terminal check needs no exchange (same data everywhere)
+                return engine.plan_query(), round_T
     j = 0
     while True:
         if avail_schedule is not None:

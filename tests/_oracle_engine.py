@@ -184,7 +184,11 @@ class OracleEngine:
         self.step_samples.extend(e)
         self.s_emit += sum(e)
         self.round = len(self.spec_T)
-        return len(self.spec_T), self.spec_steps, list(self.spec_T)
+        done = len(self.spec_T) == self.spec_J
+        if done:       # round J is the terminal check: counted, nothing emitted
+            self.round += 1
+            self.stop = 0 if self.p["join_mode"] else 1
+        return len(self.spec_T), self.spec_steps, list(self.spec_T), int(done)
 
     def round_status(self):
         if self.done:

@@ -214,8 +214,8 @@ def test_batched_exchange_commits_rounds_and_equals_the_round_by_round_protocol(
                     assert np.array_equal(out.table("grp_width").cpu().numpy(), plan.grp_width[s0:s1])
                     assert np.array_equal(out.table("step_samples").cpu().numpy(), plan.step_samples)
                 per_proc = n_coll[0] // 2
-                if batched and all_rounds:     # 1 (window) + 4 (batched phase) + 3 (the terminal check round)
-                    assert per_proc == 8, per_proc
+                if batched and all_rounds:     # 1 (window) + 4 (batched phase); the terminal check needs no exchange
+                    assert per_proc == 5, per_proc
                 if not batched:                # 1 + 3 per round, terminal check included
                     assert per_proc == 1 + 3 * plan.n_rounds, per_proc
             finally:
