@@ -107,6 +107,16 @@ def test_config5_full_size_every_element(P, oracle, cv, budget, rule):
     assert plan.total_elems > 2**31
 
 
+def test_config5_full_size_paper_operating_point(P, oracle):
+    """The exact job bench.py times as `paper_operating_point` and `streaming`: BASELINE.json configs[4] (CV 1.0 /
+    L 65536) with the paper's 1024-sample grouping buffer -- 33 protocol rounds, 1024 (rank, round) windows
+    through the round-parallel planner -- at full size: plan tables in full, every element of every slot."""
+    wl = I.make_workload(4, cv=1.0, budget=65536)
+    wl.params["buffer_size"] = 1024
+    plan = _full_size_elementwise(oracle, wl)
+    assert plan.n_rounds == 33 and plan.total_elems > 2**31
+
+
 @pytest.mark.parametrize("rule", [0, 1])
 @pytest.mark.parametrize("join", [1, 0])
 def test_config4_highcv_longtail(P, oracle, rule, join):
