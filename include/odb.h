@@ -208,8 +208,13 @@ ODB_API int odb_collate_steps(odb_ctx *ctx, int32_t step_lo, int32_t step_hi, co
                               const int32_t *d_span_hi, const odb_outputs *out, odb_plan_info *h_out, void *stream);
 
 /* Everything: reset, the round loop until termination, plan query, one collate over all emitted
- * steps.  Synchronises once per round (a few bytes of status) and once for the plan sizes; returns
- * with the collate kernels enqueued on `stream`.  On ODB_ERR_CAPACITY *h_out is still filled. */
+ * steps.  With the four arenas given, the rounds run on the device and the slot scan, the collate preparation and
+ * the collate kernel are enqueued behind them without a host round trip -- grouping buffers of at most 4096 samples
+ * (the paper's regime): the round-parallel planner + the persistent round loop (ODB_OPT_ROUND_PARALLEL);
+ * whole-stream windows: one round closed on the device -- and the call waits only for the plan sizes; otherwise
+ * (a sizing call with NULL arenas, windows in between, too many ranks for a cooperative launch) the host drives the
+ * rounds and synchronises once per round (a few bytes of status).  Returns with the collate kernels enqueued on
+ * `stream`.  On ODB_ERR_CAPACITY *h_out is still filled. */
 ODB_API int odb_run(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, const int32_t *d_tokens,
             const int64_t *d_sample_ptr, const int64_t *d_span_ptr, const int32_t *d_span_lo,
             const int32_t *d_span_hi, const odb_outputs *out, odb_plan_info *h_out, void *stream);

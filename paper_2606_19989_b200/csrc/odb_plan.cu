@@ -1,6 +1,8 @@
 // Planning kernels of the ODB hot path (rows A0..A9 of DESIGN.md): window fill + segmented sort,
 // greedy successor, pointer-jumping list ranking, cross-rank reduction, split / overflow, step
-// totals + quota cut, round commit, and the rank-major plan tables.  sm_100a only.
+// totals + quota cut, round commit, the whole round loop on the device (k_rounds: sequential, one CTA per rank;
+// k_spec_form / k_spec_commit: every round that starts without leftovers at once; k_spec_T_world: the same over
+// several processes), and the rank-major plan tables (whole plan or a step range).  sm_100a only.
 //
 // Paper: /root/reference/PAPER.md (P:<line>).  Section 2.2 P:32-36 and Eq. 1 (grouping), Eq. 3
 // (target), Alg. 1 P:258-279 (split / overflow), P:28 (IDLE slots), Thm 2 P:48 + P:347 (quota).
