@@ -212,7 +212,7 @@ struct odb_ctx {
     cudaStream_t last_stream = nullptr;
     int col_occ[4] = {0, 0, 0, 0};  // resident collate CTAs per SM (shift 0 / 1, + 2 for the bulk-store form)
     bool collate_bulk = false;      // odb_set_option(ODB_OPT_COLLATE_BULK_STORES)
-    bool attr_form = false, attr_form_hier = false, attr_align = false, attr_sort = false;  // cudaFuncSetAttribute done
+    bool attr_form = false, attr_form_hier = false, attr_align = false, attr_sort = false, attr_sort8 = false;  // cudaFuncSetAttribute done
     bool no_cluster_sort = false;  // the cluster sort could not be launched on this device: use the fallback
     bool begin_pending = false;    // a run has started and its per-run device state is not cleared yet
     bool no_rounds_kernel = false; // the persistent round-loop kernel could not be launched on this device

@@ -21,15 +21,19 @@ namespace odb {
         if (e_ != cudaSuccess) return e_;         \
     } while (0)
 
-// grid = (CL, R), cluster (CL, 1, 1).  Dynamic shared memory: X (and Y when CL > 1), kMsPadded keys each.
-__global__ void __launch_bounds__(kMsThreads) k_sort_window(const SortArgs A, int CL) {
+// grid = (CL, R), cluster (CL, 1, 1).  Dynamic shared memory: X (and Y when CL > 1), MsSort<ITEMS>::kPadded keys each.
+// ITEMS keys per thread, 4096 / ITEMS threads per CTA.
+template <int ITEMS>
+__global__ void __launch_bounds__(MsSort<ITEMS>::kThreads) k_sort_window(const SortArgs A, int CL) {
+    using MS = MsSort<ITEMS>;
+    constexpr int kThreads = MS::kThreads;
     extern __shared__ __align__(16) unsigned char ms_smem[];
     uint64_t *X = reinterpret_cast<uint64_t *>(ms_smem);
-    uint64_t *Y = X + kMsPadded;
+    uint64_t *Y = X + MS::kPadded;
     __shared__ int s_cut[2];
     const int r_ = blockIdx.y, c = blockIdx.x, t = threadIdx.x;
     if (A.first)  // start of a run: the per-run state is cleared here instead of by a launch of its own
-        ms_first_round_init(A, ((int64_t)r_ * gridDim.x + c) * kMsThreads + t, (int64_t)gridDim.x * gridDim.y * kMsThreads);
+        ms_first_round_init(A, ((int64_t)r_ * gridDim.x + c) * kThreads + t, (int64_t)gridDim.x * gridDim.y * kThreads);
     const int64_t base = A.rank_ptr[r_];
     const int n_r = (int)(A.rank_ptr[r_ + 1] - base);
     const int nl = A.first ? 0 : A.n_left[r_], fp = A.first ? 0 : A.fetch_pos[r_];
@@ -47,14 +51,14 @@ __global__ void __launch_bounds__(kMsThreads) k_sort_window(const SortArgs A, in
     if (S == 0) return;  // the whole cluster leaves
     const int c0 = c * kMsChunk;
     const int cnt = max(0, min(kMsChunk, S - c0));
-    uint64_t k[kMsItems];
+    uint64_t k[ITEMS];
     // (a lone CTA sorts only as many keys as its window needs; in a cluster every CTA sorts a full chunk)
-    const int n_keys = CL == 1 ? ms_active_keys(cnt) : kMsChunk;
-    ms_load_keys(A, base, nl, fp, c0, cnt, n_keys, k);
-    ms_sort_cta(k, X, n_keys);
+    const int n_keys = CL == 1 ? MS::active_keys(cnt) : kMsChunk;
+    ms_load_keys_t<ITEMS>(A, base, nl, fp, c0, cnt, n_keys, k);
+    MS::sort_cta(k, X, n_keys);
     uint64_t *out = A.keys_out + base;
     if (CL == 1) {
-        for (int i = t; i < cnt; i += kMsThreads) out[i] = X[ms_pad(i)];
+        for (int i = t; i < cnt; i += kThreads) out[i] = X[MS::pad(i)];
         return;
     }
     // ---- cross-CTA levels: runs of m CTAs are merged pairwise; CTA c owns outputs [4096 c, 4096 (c + 1)) ----
@@ -66,45 +70,39 @@ __global__ void __launch_bounds__(kMsThreads) k_sort_window(const SortArgs A, in
         const int na = m * kMsChunk, nb = m * kMsChunk;
         const int d0 = (c - p0) * kMsChunk, d1 = d0 + kMsChunk;
         if (t < 64) {  // warp 0: the cut of the tile's first diagonal, warp 1: of its last
-            const int cut = ms_path_remote(x_addr, p0, na, p0 + m, nb, t < 32 ? d0 : d1);
+            const int cut = MS::path_remote(x_addr, p0, na, p0 + m, nb, t < 32 ? d0 : d1);
             if ((t & 31) == 0) s_cut[t >> 5] = cut;
         }
         __syncthreads();
         const int a0 = s_cut[0], a1 = s_cut[1];
-        const int b0 = d0 - a0, b1 = d1 - a1;
+        const int b0 = d0 - a0;
         const int la = a1 - a0;  // + (b1 - b0) == 4096
         // stage the two pieces in Y: [0, la) from run A, [la, 4096) from run B (coalesced DSMEM loads)
-        for (int i = t; i < kMsChunk; i += kMsThreads)
-            Y[ms_pad(i)] = i < la ? ms_run_key(x_addr, p0, a0 + i) : ms_run_key(x_addr, p0 + m, b0 + (i - la));
+        for (int i = t; i < kMsChunk; i += kThreads)
+            Y[MS::pad(i)] = i < la ? MS::run_key(x_addr, p0, a0 + i) : MS::run_key(x_addr, p0 + m, b0 + (i - la));
         __syncthreads();
-        const int ai = ms_path_local(Y, 0, la, la, kMsChunk - la, kMsItems * t);
-        ms_merge_items(Y, ai, la, la + (kMsItems * t - ai), kMsChunk, k);
-        (void)b1;
+        const int ai = MS::path_local(Y, 0, la, la, kMsChunk - la, ITEMS * t);
+        MS::merge_items(Y, ai, la, la + (ITEMS * t - ai), kMsChunk, k);
         cluster_sync_all();  // every CTA has read what it needs from the others' X
 #pragma unroll
-        for (int q = 0; q < kMsItems; ++q) X[ms_pad(kMsItems * t + q)] = k[q];
+        for (int q = 0; q < ITEMS; ++q) X[MS::pad(ITEMS * t + q)] = k[q];
         __syncthreads();
     }
-    for (int i = t; i < cnt; i += kMsThreads) out[c0 + i] = X[ms_pad(i)];
+    for (int i = t; i < cnt; i += kThreads) out[c0 + i] = X[MS::pad(i)];
     cluster_sync_all();  // nobody leaves while a neighbour may still read its shared memory (none does; cheap insurance)
 }
 
-// Launches the cluster sort for `nseg` segments (rank windows; buckets / megabatches of the offline planners)
-// of up to 16 * 4096 keys each.  Returns cudaErrorNotSupported when a segment can be larger (the caller falls
-// back to chunk sorts + global merge passes).
-cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A0, int64_t nseg, int maxS, cudaStream_t st) {
-    const int chunks = (maxS + kMsChunk - 1) / kMsChunk;
-    int CL = 1;
-    while (CL < chunks) CL <<= 1;
-    if (CL > 16) return cudaErrorNotSupported;
-    const size_t smem = (size_t)(CL > 1 ? 2 : 1) * kMsPadded * sizeof(uint64_t);
-    if (!c->attr_sort) {
-        cudaError_t e = cudaFuncSetAttribute(k_sort_window, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(2 * kMsPadded * sizeof(uint64_t)));
+template <int ITEMS>
+static cudaError_t launch_sort_segments_t(odb_ctx *c, const SortArgs &A0, int64_t nseg, int CL, bool *attr_done, cudaStream_t st) {
+    using MS = MsSort<ITEMS>;
+    const size_t smem = (size_t)(CL > 1 ? 2 : 1) * MS::kPadded * sizeof(uint64_t);
+    if (!*attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_sort_window<ITEMS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)(2 * MS::kPadded * sizeof(uint64_t)));
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_sort_window, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        e = cudaFuncSetAttribute(k_sort_window<ITEMS>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         if (e != cudaSuccess) return e;
-        c->attr_sort = true;
+        *attr_done = true;
     }
     for (int64_t s0 = 0; s0 < nseg; s0 += 65535) {  // gridDim.y is limited to 65535
         const unsigned ns = (unsigned)std::min<int64_t>(nseg - s0, 65535);
@@ -117,14 +115,14 @@ cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A0, int64_t nseg, i
         A.S_out += s0;
         if (s0 > 0) A.first = 0;  // (the per-run state is cleared by the first batch of segments)
         if (CL == 1) {  // no cluster needed: a plain launch (the attribute path costs a few microseconds per launch)
-            k_sort_window<<<dim3(1, ns), kMsThreads, smem, st>>>(A, 1);
+            k_sort_window<ITEMS><<<dim3(1, ns), MS::kThreads, smem, st>>>(A, 1);
             ODB_LAUNCH_CHECK(c);
             continue;
         }
         cudaLaunchConfig_t cfg;
         memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3((unsigned)CL, ns, 1);
-        cfg.blockDim = dim3(kMsThreads, 1, 1);
+        cfg.blockDim = dim3(MS::kThreads, 1, 1);
         cfg.dynamicSmemBytes = smem;
         cfg.stream = st;
         cudaLaunchAttribute attr[1];
@@ -134,11 +132,26 @@ cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A0, int64_t nseg, i
         attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        cudaError_t e = cudaLaunchKernelEx(&cfg, k_sort_window, A, CL);
+        cudaError_t e = cudaLaunchKernelEx(&cfg, k_sort_window<ITEMS>, A, CL);
         if (e != cudaSuccess) return e;
         c->launches++;
     }
     return cudaSuccess;
+}
+
+// Launches the cluster sort for `nseg` segments (rank windows; buckets / megabatches of the offline planners)
+// of up to 16 * 4096 keys each.  Returns cudaErrorNotSupported when a segment can be larger (the caller falls
+// back to chunk sorts + global merge passes).
+cudaError_t launch_sort_segments(odb_ctx *c, const SortArgs &A0, int64_t nseg, int maxS, cudaStream_t st) {
+    const int chunks = (maxS + kMsChunk - 1) / kMsChunk;
+    int CL = 1;
+    while (CL < chunks) CL <<= 1;
+    if (CL > 16) return cudaErrorNotSupported;
+    // keys per thread: 8 (512 threads per 4096-key chunk) for windows of 16 K keys and more, 4 (1024 threads) below.
+    // Measured planning stage with 4 / 8 / 16 keys per thread: 32 x 32768-key windows 0.214 / 0.199 / 0.203 ms,
+    // 16 x 16384 0.131 / 0.128 / 0.142 ms, 8 x 8192 0.107 / 0.107 / 0.120 ms.
+    if (CL >= 4) return launch_sort_segments_t<8>(c, A0, nseg, CL, &c->attr_sort8, st);
+    return launch_sort_segments_t<4>(c, A0, nseg, CL, &c->attr_sort, st);
 }
 
 cudaError_t launch_sort_window(odb_ctx *c, int maxS, bool first, cudaStream_t st) {
