@@ -318,6 +318,7 @@ int odb_offline_plan(odb_ctx *c, const odb_offline_params *P, const int32_t *d_l
     c->n_total = n_samples;
     c->max_nr = (int32_t)std::min<int64_t>(n_samples, 0x7fffffff);
     c->h_rank_ptr.assign((size_t)c->prm.n_ranks + 1, 0);
+    c->dev_rank_ptr_valid = false;  // (the host copy no longer mirrors d_rank_ptr)
     CU(c, offline_build(c, P, d_lengths, n_samples, st));
     {  // bad lengths
         CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, st));
@@ -411,14 +412,32 @@ static int begin_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank
     }
     if (h_rank_ptr[R] > c->n_max) return ODB_ERR_INVALID_ARG;
     if (h_rank_ptr[R] > 0 && !d_lengths) return ODB_ERR_INVALID_ARG;
+    // the rank boundaries and the arrival counts go up only when they differ from what the device already holds
+    // (a training job calls with the same partition step after step; every stream operation in front of the first
+    // kernel costs a few microseconds of an otherwise 0.2 ms planning stage)
+    if (c->dev_meta_stream != st) {  // (uploaded on another stream: no ordering with this one is assumed)
+        c->dev_rank_ptr_valid = false;
+        c->h_arrived_dev.clear();
+    }
+    c->dev_meta_stream = st;
+    const bool same_ranks = c->dev_rank_ptr_valid && c->h_rank_ptr.size() == (size_t)R + 1 &&
+                            std::equal(h_rank_ptr, h_rank_ptr + R + 1, c->h_rank_ptr.begin());
     c->h_rank_ptr.assign(h_rank_ptr, h_rank_ptr + R + 1);
     c->n_total = h_rank_ptr[R];
     c->max_nr = (int32_t)max_nr;
     c->d_lengths = d_lengths;
     CU(c, cudaSetDevice(c->device));
-    CU(c, cudaMemcpyAsync(c->d_rank_ptr, c->h_rank_ptr.data(), (R + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    if (!same_ranks) {
+        c->dev_rank_ptr_valid = false;
+        CU(c, cudaMemcpyAsync(c->d_rank_ptr, c->h_rank_ptr.data(), (R + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+        c->dev_rank_ptr_valid = true;
+    }
     if (!c->arrived_set) c->h_arrived.assign((size_t)R, 0x7fffffff);  // everything has arrived
-    CU(c, cudaMemcpyAsync(c->d_arrived, c->h_arrived.data(), (size_t)R * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (c->h_arrived != c->h_arrived_dev) {
+        c->h_arrived_dev.clear();
+        CU(c, cudaMemcpyAsync(c->d_arrived, c->h_arrived.data(), (size_t)R * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        c->h_arrived_dev = c->h_arrived;
+    }
     // rank state, emit positions, step totals, length validation: done by the first sort launch (or k_begin)
     CU(c, cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st));
     c->begin_pending = true;
@@ -499,8 +518,11 @@ int odb_set_available(odb_ctx *c, const int64_t *h_arrived, void *stream) {
     c->arrived_set = true;
     if (c->state == 3) {  // mid-run: the next odb_form_groups reads the device copy
         CU(c, cudaSetDevice(c->device));
+        c->h_arrived_dev.clear();
         CU(c, cudaMemcpyAsync(c->d_arrived, c->h_arrived.data(), (size_t)R * sizeof(int32_t), cudaMemcpyHostToDevice,
                               (cudaStream_t)stream));
+        c->h_arrived_dev = c->h_arrived;
+        c->dev_meta_stream = (cudaStream_t)stream;
     }
     return ODB_OK;
 }
@@ -785,7 +807,6 @@ int odb_plan_query(odb_ctx *c, odb_plan_info *h_out) {
     CU(c, cudaMemcpyAsync(c->d_dims, U, sizeof(PlanDims), cudaMemcpyHostToDevice, st));
     CapCheck cap = {-1, -1, -1, -1, -1, -1};
     CU(c, launch_finalize(c, (int64_t)n_slots, cap, c->h_rank_off, st));
-    CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
     CU(c, cudaStreamSynchronize(st));
     fill_info(c);
     if (c->offline) {  // the slot CSR's (global) ids: wrap-around repetition can emit a sample twice
@@ -972,7 +993,6 @@ static int enqueue_tail(odb_ctx *c, int64_t steps_bound, const int32_t *d_tokens
     cap.left = o->d_left_ids ? o->left_capacity : -1;
     cap.tiles = tile_bound;
     CU(c, launch_finalize(c, slots_bound, cap, c->h_rank_off, st));
-    CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
     CU(c, cudaEventRecord(c->ev_plan, st));
     return enqueue_collate(c, d_tokens, d_sample_ptr, d_span_ptr, d_span_lo, d_span_hi, o, c->n_total, tile_bound, st);
 }
@@ -1093,7 +1113,6 @@ static int plan_impl(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank
             if (rc != ODB_OK) return rc;
             const CapCheck cap = {-1, -1, -1, -1, -1, -1};
             CU(c, launch_finalize(c, slots_bound, cap, c->h_rank_off, st));
-            CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
             CU(c, cudaEventRecord(c->ev_plan, st));
             return fused_sizes(c, h_out);
         }
@@ -1154,7 +1173,6 @@ int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_
         cap.tiles = tile_bound;
         CU(c, launch_sub_dims(c, n, st));
         CU(c, launch_finalize(c, slots, cap, nullptr, st, step_lo));
-        CU(c, cudaMemcpyAsync(c->h_dims, c->d_dims, sizeof(PlanDims), cudaMemcpyDeviceToHost, st));
         CU(c, cudaEventRecord(c->ev_plan, st));
         CU(c, launch_sub_ids(c, step_lo, o->d_grp_sample_ids, full_sp, full_K, st));
         if (!arenas) return ODB_OK;  // a sizing call

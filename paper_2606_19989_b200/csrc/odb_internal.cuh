@@ -268,6 +268,9 @@ struct odb_ctx {
     int32_t *emit_snap = nullptr;  // R: emit_cur as seen by k_align (read by every CTA of k_commit)
     int32_t *d_arrived = nullptr;  // R: views of the rank's stream that have arrived (odb_set_available)
     std::vector<int32_t> h_arrived;
+    std::vector<int32_t> h_arrived_dev;  // what d_arrived holds (empty = unknown)
+    bool dev_rank_ptr_valid = false;     // d_rank_ptr holds h_rank_ptr
+    cudaStream_t dev_meta_stream = nullptr;  // ... uploaded on this stream
     bool arrived_set = false;
     odb::RoundRec *d_rec = nullptr;
     odb::RoundRec *h_rec = nullptr;  // pinned
@@ -277,6 +280,7 @@ struct odb_ctx {
     unsigned int *d_done_ctr = nullptr;  // "last CTA" counter of k_commit (self-resetting)
     cudaEvent_t ev_plan = nullptr;       // recorded behind the slot scan's read-back
     unsigned long long *d_tile_counter = nullptr;
+    int fin_epoch = 0;                   // launch counter of k_fin_scan (tags its tile flags)
 
     // step-major staging tables [step * R + r], growable
     odb::DevBuf<int32_t> st_count, st_width, st_real, st_round, st_origin, step_samples;

@@ -1208,6 +1208,11 @@ __global__ void __launch_bounds__(kMsThreads) k_rounds(const RoundsArgs A) {
             A.dims->err = bad == 2 ? ODB_ERR_STATE : 0;
             A.dims->complete = bad ? 0 : 1;
         }
+        // the last CTA to leave rewinds the barrier counter for the next launch (every CTA has passed every barrier)
+        if (atomicAdd(A.bar + 1, 1u) == (unsigned int)(R - 1)) {
+            A.bar[0] = 0u;
+            A.bar[1] = 0u;
+        }
     }
 }
 
@@ -1465,11 +1470,17 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
            const int32_t *__restrict__ st_origin, int32_t *__restrict__ grp_count, int32_t *__restrict__ grp_width,
            int32_t *__restrict__ grp_round, int32_t *__restrict__ grp_real, int32_t *__restrict__ grp_origin,
            int64_t *__restrict__ grp_offset, int64_t *__restrict__ grp_sample_ptr, ScanTile *tiles, unsigned int *ticket,
-           CapCheck cap, int64_t n_total, int64_t *rank_off) {
+           CapCheck cap, int64_t n_total, int64_t *rank_off, PlanDims *h_dims_out, int epoch) {
     __shared__ long long s_scan64[34];
     __shared__ long long s_base[4];
     __shared__ int s_tile;
-    if (!dims->complete) return;  // enqueued behind a round that did not terminate the protocol
+    if (!dims->complete) {  // enqueued behind a round that did not terminate the protocol
+        if (h_dims_out && blockIdx.x == 0 && threadIdx.x == 0) {
+            *h_dims_out = *dims;
+            __threadfence_system();
+        }
+        return;
+    }
     const int n_steps = dims->n_steps;
     const int64_t n_slots = (int64_t)R * n_steps;
     const int64_t n_tiles = max((n_slots + kFinTile - 1) / kFinTile, (int64_t)1);
@@ -1517,7 +1528,7 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
                 me->agg[q] = total[q];
                 if (tile == 0) me->inc[q] = total[q];
             }
-            st_flag(&me->flag, tile == 0 ? 2 : 1);
+            st_flag(&me->flag, (epoch << 2) | (tile == 0 ? 2 : 1));
             if (tile == 0) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q) s_base[q] = 0;
@@ -1532,9 +1543,10 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
                 int f = 2;  // tiles before the first count as "inclusive prefix 0"
                 long long x[4] = {0, 0, 0, 0};
                 if (tt >= 0) {
-                    do {
+                    do {  // (a flag of an earlier launch counts as "nothing yet": the states are never cleared)
                         f = ld_flag(&tiles[tt].flag);
-                    } while (f == 0);
+                    } while ((f >> 2) != epoch);
+                    f &= 3;
 #pragma unroll
                     for (int q = 0; q < 4; ++q) x[q] = (f == 2) ? __ldcg(&tiles[tt].inc[q]) : __ldcg(&tiles[tt].agg[q]);
                 }
@@ -1556,7 +1568,7 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
                     s_base[q] = acc[q];
                     me->inc[q] = acc[q] + total[q];
                 }
-                st_flag(&me->flag, 2);
+                st_flag(&me->flag, (epoch << 2) | 2);
             }
         }
         __syncthreads();
@@ -1597,6 +1609,20 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
             if (cap.steps >= 0 && n_steps > cap.steps) err = ODB_ERR_CAPACITY;
             if (cap.left >= 0 && n_total >= 0 && n_total - tot_s > cap.left) err = ODB_ERR_CAPACITY;
             dims->err = err;
+            // the sizes go straight to the caller's pinned copy: the host waits for an event behind this kernel, no
+            // copy operation sits between the slot scan and the collate preparation
+            if (h_dims_out) {
+                *h_dims_out = *dims;
+                __threadfence_system();
+            }
+        }
+    }
+    // the last CTA to leave rewinds the ticket counter for the next launch (no clearing pass in front of this kernel)
+    if (threadIdx.x == 0) {
+        const unsigned int prev = atomicAdd(ticket + 1, 1u);
+        if (prev == gridDim.x - 1u) {
+            ticket[0] = 0u;
+            ticket[1] = 0u;
         }
     }
 }
@@ -1924,14 +1950,15 @@ cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, bool spec_terminal, cudaS
         c->rounds_max_ctas = coop ? std::max(occ * c->sm_count, 1) : -1;
     }
     if (c->rounds_max_ctas < R) return cudaErrorNotSupported;
+    cudaError_t e = cudaSuccess;
     if (!c->gs_rounds) {
-        cudaError_t e = cudaMalloc((void **)&c->gs_rounds, (size_t)4 * R * sizeof(int32_t) + 64);
+        e = cudaMalloc((void **)&c->gs_rounds, (size_t)4 * R * sizeof(int32_t) + 64);
+        if (e != cudaSuccess) return e;
+        // the barrier counter and the exit counter live behind the summary: zeroed once, rewound by the kernel itself
+        e = cudaMemset(c->gs_rounds + (size_t)4 * R, 0, 64);
         if (e != cudaSuccess) return e;
     }
-    // the barrier counter lives behind the summary
     unsigned int *bar = reinterpret_cast<unsigned int *>(c->gs_rounds + (size_t)4 * R);
-    cudaError_t e = cudaMemsetAsync(bar, 0, 64, st);
-    if (e != cudaSuccess) return e;
     RoundsArgs A;
     memset(&A, 0, sizeof(A));
     A.sort.len = c->d_lengths;
@@ -2041,18 +2068,18 @@ cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap
     const int R = c->prm.n_ranks;
     const int64_t so = step_lo * R;  // the staging tables are step-major: a step range is a contiguous piece
     const int64_t n_tiles = std::max<int64_t>((slots_bound + kFinTile - 1) / kFinTile, 1);
-    cudaError_t e = c->scan_state.ensure((size_t)n_tiles * sizeof(ScanTile) + 64);
+    // [0, 64): ticket + exit counter (rewound by the kernel's last CTA); then the tile states, whose flags carry the
+    // launch's epoch, so nothing has to be cleared between launches (zeroed once, when the buffer grows)
+    cudaError_t e = c->scan_state.ensure((size_t)n_tiles * sizeof(ScanTile) + 64, true, st);
     if (e != cudaSuccess) return e;
-    // [0, 64): ticket; then the tile states
-    e = cudaMemsetAsync(c->scan_state.p, 0, (size_t)n_tiles * sizeof(ScanTile) + 64, st);
-    if (e != cudaSuccess) return e;
+    c->fin_epoch = (c->fin_epoch % 0x1ffffffe) + 1;  // 1 .. 2^29 - 1
     const int blocks = (int)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * 2);
     k_fin_scan<<<blocks, kFinThreads, 0, st>>>(R, c->d_dims, c->st_count.p + so, c->st_width.p + so, c->st_real.p + so,
                                                c->st_round.p + so, c->st_origin.p + so, c->grp_count.p, c->grp_width.p, c->grp_round.p,
                                                c->grp_real.p, c->grp_origin.p, c->grp_offset.p, c->grp_sample_ptr.p,
                                                reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
                                                reinterpret_cast<unsigned int *>(c->scan_state.p), cap,
-                                               (c->offline || c->sub_mode) ? (int64_t)-1 : c->n_total, rank_off);
+                                               (c->offline || c->sub_mode) ? (int64_t)-1 : c->n_total, rank_off, c->h_dims, c->fin_epoch);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
