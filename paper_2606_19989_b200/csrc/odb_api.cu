@@ -541,8 +541,7 @@ int odb_align(odb_ctx *c, void *stream) {
         c->state = 6;
         return ODB_OK;
     }
-    CU(c, launch_round_align(c, st));
-    CU(c, cudaMemcpyAsync(c->h_rec, c->d_rec, sizeof(RoundRec), cudaMemcpyDeviceToHost, st));
+    CU(c, launch_round_align(c, st));  // (single-process mode: k_commit's last CTA writes the status to the pinned h_rec)
     CU(c, cudaEventRecord(c->ev_status, st));
     c->state = 2;
     return ODB_OK;

@@ -948,7 +948,7 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
          uint8_t *__restrict__ posflag,
          int32_t *__restrict__ emit_ids, int32_t *__restrict__ emit_pos, int32_t *__restrict__ left_ids, int32_t *n_left,
          int32_t *fetch_pos, int32_t *emit_cur, const int32_t *__restrict__ emit_snap, RoundRec *rec, PlanDims *dims,
-         unsigned int *done_ctr) {
+         unsigned int *done_ctr, RoundRec *h_rec_out) {
     {
         const int r = blockIdx.x;
         RankView V;
@@ -1000,6 +1000,20 @@ k_commit(const uint64_t *__restrict__ keys, const int64_t *__restrict__ rank_ptr
         dims->err = 0;
         dims->complete = bad ? 0 : complete;
         *done_ctr = 0u;
+        // the round's status goes straight to the host's pinned copy (odb_round_status waits for an event behind this
+        // kernel): no copy operation between the commit and the slot scan
+        if (h_rec_out) {
+            RoundRec out;
+            out.T = vr->T;
+            out.T_emit = T_emit;
+            out.quota_hit = quota_hit;
+            out.n_finished = n_fin;
+            out.bad_length = bad;
+            out.done = vr->done;
+            out.emitted_round = vr->emitted_round;
+            *h_rec_out = out;
+            __threadfence_system();
+        }
     }
 }
 
@@ -1823,7 +1837,8 @@ static cudaError_t launch_commit_kernel(odb_ctx *c, cudaStream_t st) {
                                          (long long)c->prm.emitted_so_far + (long long)c->samples_emitted, c->st_count.p,
                                          c->st_width.p, c->st_real.p, c->st_round.p, c->st_origin.p, c->posflag,
                                          c->emit_ids, c->emit_pos, c->left_ids, c->n_left, c->fetch_pos, c->emit_cur,
-                                         c->emit_snap, c->d_rec, c->world_ranks ? nullptr : c->d_dims, c->d_done_ctr);
+                                         c->emit_snap, c->d_rec, c->world_ranks ? nullptr : c->d_dims, c->d_done_ctr,
+                                         c->world_ranks ? nullptr : c->h_rec);
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
