@@ -438,8 +438,10 @@ static int begin_run(odb_ctx *c, const int32_t *d_lengths, const int64_t *h_rank
         CU(c, cudaMemcpyAsync(c->d_arrived, c->h_arrived.data(), (size_t)R * sizeof(int32_t), cudaMemcpyHostToDevice, st));
         c->h_arrived_dev = c->h_arrived;
     }
-    // rank state, emit positions, step totals, length validation: done by the first sort launch (or k_begin)
-    CU(c, cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st));
+    // rank state, emit positions, step totals, length validation: done by the first sort launch (or k_begin).
+    // The status record: cleared by the slot scan of the previous complete plan when that ran on this stream.
+    if (!(c->rec_clean && c->rec_clear_stream == st)) CU(c, cudaMemsetAsync(c->d_rec, 0, sizeof(RoundRec), st));
+    c->rec_clean = false;
     c->begin_pending = true;
     c->n_finished = 0;
     for (int r = 0; r < R; ++r)
@@ -768,6 +770,7 @@ static int ensure_plan_tables(odb_ctx *c, size_t n_slots, size_t n_steps) {
 static void fill_info(odb_ctx *c) {
     odb_plan_info &I = c->info;
     const PlanDims &D = *c->h_dims;
+    c->rec_clean = D.complete && !c->offline;  // (the slot scan that produced these sizes cleared the status record)
     I.n_rounds = c->n_rounds;
     I.n_steps = c->n_steps;
     I.stop_reason = c->stop_reason;

@@ -281,6 +281,8 @@ struct odb_ctx {
     cudaEvent_t ev_plan = nullptr;       // recorded behind the slot scan's read-back
     unsigned long long *d_tile_counter = nullptr;
     int fin_epoch = 0;                   // launch counter of k_fin_scan (tags its tile flags)
+    bool rec_clean = false;              // d_rec was cleared by the slot scan of the last (complete) plan ...
+    cudaStream_t rec_clear_stream = nullptr;  // ... enqueued on this stream
 
     // step-major staging tables [step * R + r], growable
     odb::DevBuf<int32_t> st_count, st_width, st_real, st_round, st_origin, step_samples;

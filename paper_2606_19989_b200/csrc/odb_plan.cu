@@ -1484,7 +1484,7 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
            const int32_t *__restrict__ st_origin, int32_t *__restrict__ grp_count, int32_t *__restrict__ grp_width,
            int32_t *__restrict__ grp_round, int32_t *__restrict__ grp_real, int32_t *__restrict__ grp_origin,
            int64_t *__restrict__ grp_offset, int64_t *__restrict__ grp_sample_ptr, ScanTile *tiles, unsigned int *ticket,
-           CapCheck cap, int64_t n_total, int64_t *rank_off, PlanDims *h_dims_out, int epoch) {
+           CapCheck cap, int64_t n_total, int64_t *rank_off, PlanDims *h_dims_out, int epoch, RoundRec *clear_rec) {
     __shared__ long long s_scan64[34];
     __shared__ long long s_base[4];
     __shared__ int s_tile;
@@ -1628,6 +1628,17 @@ k_fin_scan(int R, PlanDims *dims, const int32_t *__restrict__ st_count, const in
             if (h_dims_out) {
                 *h_dims_out = *dims;
                 __threadfence_system();
+            }
+            // the plan is complete: nothing reads the per-round status record any more; it is cleared here for the
+            // next run (which then needs no clearing operation in front of its first kernel)
+            if (clear_rec) {
+                clear_rec->T = 0;
+                clear_rec->T_emit = 0;
+                clear_rec->quota_hit = 0;
+                clear_rec->n_finished = 0;
+                clear_rec->bad_length = 0;
+                clear_rec->done = 0;
+                clear_rec->emitted_round = 0;
             }
         }
     }
@@ -2094,7 +2105,9 @@ cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap
                                                c->grp_real.p, c->grp_origin.p, c->grp_offset.p, c->grp_sample_ptr.p,
                                                reinterpret_cast<ScanTile *>(c->scan_state.p + 64),
                                                reinterpret_cast<unsigned int *>(c->scan_state.p), cap,
-                                               (c->offline || c->sub_mode) ? (int64_t)-1 : c->n_total, rank_off, c->h_dims, c->fin_epoch);
+                                               (c->offline || c->sub_mode) ? (int64_t)-1 : c->n_total, rank_off, c->h_dims, c->fin_epoch,
+                                               (c->sub_mode || c->offline) ? nullptr : c->d_rec);
+    if (!c->sub_mode && !c->offline) c->rec_clear_stream = st;  // (the host marks the record clean once it knows the plan was complete)
     ODB_LAUNCH_CHECK(c);
     return cudaSuccess;
 }
