@@ -561,6 +561,55 @@ def test_run_host_device_arenas(P, oracle):
         Par.compare_full(plan, ref, info, host)
 
 
+def test_context_reused_across_different_jobs(P, oracle):
+    """One context, several jobs back to back on one stream: different rank boundaries (the library uploads them only
+    when they changed), the same boundaries again, an arrival schedule in between (the device's arrival counts must
+    follow), a job with a bad length (the status record is cleared by the previous plan's slot scan, not by a
+    clearing pass: the error must neither stick nor get lost), odb_run and the staged calls mixed."""
+    import torch
+    rng = np.random.default_rng(5)
+    mk = lambda ns, seed, **kw: I.custom_workload("reuse", [rng.integers(1, 900, n) for n in ns], seed, budget=4096, **kw)
+    jobs = [mk((300, 200, 100), 1), mk((100, 300, 200), 2), mk((50, 0, 550), 4), mk((300, 200, 100), 5)]
+    prm = Par.gpu_params(jobs[0])
+    with P.Odb(prm, 600) as ctx:
+        def run(wl, staged, sched=None):
+            assert wl.params["budget"] == 4096
+            dw = Par.DeviceWorkload(wl)
+            plan, ref = oracle.run_workload(wl, avail_schedule=sched)
+            if staged:
+                info = ctx.plan(dw.lengths, wl.rank_ptr, avail_schedule=sched)
+                out = P.OutputBuffers.for_plan(wl.n_ranks, info, dw.device, fill=Par.SENTINEL)
+                P.odb_collate(ctx.h, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out.struct)
+            else:
+                out = P.OutputBuffers(wl.n_ranks, plan.total_elems, plan.n_slots, plan.samples_emitted, plan.n_steps,
+                                      plan.samples_left, dw.device, fill=Par.SENTINEL)
+                info = P.odb_run(ctx.h, dw.lengths, wl.rank_ptr, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo,
+                                 dw.span_hi, out.struct)
+            torch.cuda.synchronize()
+            Par.compare_plan(plan, info, out)
+            Par.compare_full(plan, ref, info, out)
+
+        whole = jobs
+        for wl in whole + whole[::-1]:                      # same parameters as the context: boundaries change and return
+            run(wl, staged=False)
+            run(wl, staged=True)
+        from tests.test_oracle_arrival import _random_schedule
+        sched = _random_schedule(np.random.default_rng(9), whole[0], 5)
+        run(whole[0], staged=True, sched=sched)            # arrival counts on the device ...
+        run(whole[0], staged=False)                        # ... and "everything has arrived" again
+        bad = Par.DeviceWorkload(whole[1])
+        bad.lengths[7] = 0
+        torch.cuda.synchronize()
+        empty = P.OutputBuffers(whole[1].n_ranks, 0, 0, 0, 0, 0, bad.device)
+        for _ in range(2):                                  # reported every time, not only once
+            with pytest.raises(P.OdbError) as ei:
+                P.odb_run(ctx.h, bad.lengths, whole[1].rank_ptr, bad.tokens, bad.sample_ptr, bad.span_ptr, bad.span_lo,
+                          bad.span_hi, empty.struct)
+            assert ei.value.status == P.ODB_ERR_BAD_LENGTH
+        run(whole[1], staged=False)                         # and it does not stick
+        run(whole[2], staged=True)
+
+
 def test_run_host_reuses_context(P, oracle):
     """Two odb_run_host calls on one context (staging buffers, events and counters are reused)."""
     wl = I.make_workload(1, n_ranks=3, n_per_rank=300)
