@@ -1272,7 +1272,9 @@ __device__ __forceinline__ int64_t spec_off(int64_t base, int B, int r, int j) {
     return base + (base + B - 1) / B + r + (int64_t)j * (B + 1);
 }
 
-__global__ void __launch_bounds__(kMsThreads) k_spec_form(const SpecArgs A) {
+template <int ITEMS>
+__global__ void __launch_bounds__(kMsChunk / ITEMS) k_spec_form(const SpecArgs A) {
+    using MS = MsSort<ITEMS>;
     extern __shared__ __align__(16) unsigned char sp_smem[];
     __shared__ int s_scan[34];
     __shared__ uint16_t s_e2[32];
@@ -1290,13 +1292,13 @@ __global__ void __launch_bounds__(kMsThreads) k_spec_form(const SpecArgs A) {
         uint64_t *X = reinterpret_cast<uint64_t *>(sp_smem);
         uint64_t *K = X + A.x_keys;
         int32_t *gp = reinterpret_cast<int32_t *>(K + B);
-        uint64_t k[kMsItems];
-        const int n_keys = ms_active_keys(S);
-        ms_load_keys(SA, base, 0, fp, 0, S, n_keys, k);
-        ms_sort_cta(k, X, n_keys);
+        uint64_t k[ITEMS];
+        const int n_keys = MS::active_keys(S);
+        ms_load_keys_t<ITEMS>(SA, base, 0, fp, 0, S, n_keys, k);
+        MS::sort_cta(k, X, n_keys);
         uint64_t *out = SA.keys_out + base + fp;
         for (int i = t; i < S; i += blockDim.x) {
-            const uint64_t key = X[ms_pad(i)];
+            const uint64_t key = X[MS::pad(i)];
             K[i] = key;
             out[i] = key;
         }
@@ -1889,6 +1891,10 @@ cudaError_t launch_pack_summary(odb_ctx *c, cudaStream_t st) {
 
 // The whole round loop in one cooperative launch (k_rounds).  cudaErrorNotSupported when the R CTAs cannot
 // all be resident on this device (the caller then drives the rounds from the host).
+// keys per thread of k_spec_form's window sort: 8 for grouping buffers of 512 samples and more, 4 below (measured
+// planning stage with 4 / 8: buffer 256: 0.128 / 0.131 ms, 1024: 0.122 / 0.117 ms, 4096: 0.138 / 0.127 ms)
+static int spec_items(const odb_ctx *c) { return c->prm.buffer_size >= 512 ? 8 : 4; }
+
 static int host_active_keys(int S) {
     int n = 32 * kMsItems;
     while (n < S) n <<= 1;
@@ -1900,15 +1906,20 @@ static cudaError_t make_spec_args(odb_ctx *c, int spec_rounds, int eval_T, int t
                                   int *threads_out, size_t *smem_out) {
     const int R = c->prm.n_ranks;
     const int B = c->prm.buffer_size;
-    const int n_keys = host_active_keys(B);
+    const int items = spec_items(c);
+    int n_keys = 32 * items;
+    while (n_keys < B) n_keys <<= 1;
+    n_keys = std::min(n_keys, kMsChunk);
     // (measured: more threads per window are slower -- 256 / 512 / 1024 threads for 1024-key windows give a
     //  planning stage of 0.134 / 0.146 / 0.185 ms: the launch is throughput-bound, not latency-bound)
-    *threads_out = std::max(n_keys / kMsItems, 128);
-    const size_t x_keys = (size_t)n_keys + n_keys / kMsItems;
+    *threads_out = std::max(n_keys / items, 128);
+    const size_t x_keys = (size_t)n_keys + n_keys / items;
     const size_t x_bytes = std::max(x_keys * 8, (form_hier_smem_bytes(B) + 15) & ~(size_t)15);
     *smem_out = x_bytes + (size_t)B * 8 + ((size_t)B + 4) * 4;
     if (!c->spec_occ) {
-        cudaError_t ae = cudaFuncSetAttribute(k_spec_form, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(96 * 1024));
+        cudaError_t ae = cudaFuncSetAttribute(k_spec_form<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(96 * 1024));
+        if (ae != cudaSuccess) return ae;
+        ae = cudaFuncSetAttribute(k_spec_form<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(96 * 1024));
         if (ae != cudaSuccess) return ae;
         c->spec_occ = 1;
     }
@@ -2037,9 +2048,10 @@ cudaError_t launch_rounds(odb_ctx *c, int spec_rounds, bool spec_terminal, cudaS
         size_t sp_smem = 0;
         e = make_spec_args(c, spec_rounds, 1, spec_terminal ? 1 : 0, st, &P, &threads, &sp_smem);
         if (e != cudaSuccess) return e;
-        k_spec_form<<<dim3((unsigned)R, (unsigned)spec_rounds), threads, sp_smem, st>>>(P);
+        if (spec_items(c) == 8) k_spec_form<8><<<dim3((unsigned)R, (unsigned)spec_rounds), threads, sp_smem, st>>>(P);
+        else k_spec_form<4><<<dim3((unsigned)R, (unsigned)spec_rounds), threads, sp_smem, st>>>(P);
         ODB_LAUNCH_CHECK(c);
-        k_spec_commit<<<dim3((unsigned)R, (unsigned)spec_rounds), threads, 0, st>>>(P);
+        k_spec_commit<<<dim3((unsigned)R, (unsigned)spec_rounds), std::max(host_active_keys(c->prm.buffer_size) / kMsItems, 128), 0, st>>>(P);
         ODB_LAUNCH_CHECK(c);
         A.sort.first = 0;
         A.spec = P.rec;
@@ -2059,7 +2071,8 @@ cudaError_t launch_dist_spec_form(odb_ctx *c, int n_rounds, int32_t **G_tab_out,
     size_t sp_smem = 0;
     cudaError_t e = make_spec_args(c, n_rounds, 0, 1, st, &P, &threads, &sp_smem);
     if (e != cudaSuccess) return e;
-    k_spec_form<<<dim3((unsigned)c->prm.n_ranks, (unsigned)n_rounds), threads, sp_smem, st>>>(P);
+    if (spec_items(c) == 8) k_spec_form<8><<<dim3((unsigned)c->prm.n_ranks, (unsigned)n_rounds), threads, sp_smem, st>>>(P);
+    else k_spec_form<4><<<dim3((unsigned)c->prm.n_ranks, (unsigned)n_rounds), threads, sp_smem, st>>>(P);
     ODB_LAUNCH_CHECK(c);
     *G_tab_out = P.G_tab;
     c->sorted = c->keyA;
@@ -2079,7 +2092,7 @@ cudaError_t launch_dist_spec_commit(odb_ctx *c, int n_rounds, const int32_t *d_G
     k_spec_T_world<<<1, 1024, 0, st>>>(d_G_world, d_n_world, n_procs, R, n_rounds, c->prm.buffer_size, c->prm.slot_capacity,
                                         P.T_tab, P.sb_tab, P.rec);
     ODB_LAUNCH_CHECK(c);
-    k_spec_commit<<<dim3((unsigned)R, (unsigned)n_rounds), threads, 0, st>>>(P);
+    k_spec_commit<<<dim3((unsigned)R, (unsigned)n_rounds), std::max(host_active_keys(c->prm.buffer_size) / kMsItems, 128), 0, st>>>(P);
     ODB_LAUNCH_CHECK(c);
     k_spec_state<<<(R + 127) / 128, 128, 0, st>>>(P.rec, c->d_rank_ptr, R, c->prm.buffer_size, c->n_left, c->fetch_pos,
                                                    c->emit_cur);
