@@ -529,6 +529,8 @@ def run_ours(args):
                            "come back to the host)"}
     del din
     torch.cuda.empty_cache()
+    if rank == 0 and world == 1 and not args.no_sweep:
+        result["sharded_protocol_n1"] = sharded_protocol_rows()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cb, _ = cpu_baseline(args, args.cpu_sample_ranks)
         result["cpu_baseline"] = cb
@@ -629,8 +631,10 @@ def run_sharded(args):
             "config": {"workload": workload_name(args, wl_all), "rule": RULE_NAMES[args.rule], "join_mode": args.join,
                        "samples": n_samples, "real_tokens": n_tok, "padded_elems": n_pad, "n_steps": int(info.n_steps),
                        "n_rounds": int(info.n_rounds),
-                       "parallelism": "virtual ranks sharded over %d GPU(s), %d per GPU; per round all_gather(G,S) + "
-                                      "all_reduce(step totals) over NCCL" % (world, rl),
+                       "parallelism": "virtual ranks sharded over %d GPU(s), %d per GPU; %s over NCCL" % (
+                           world, rl, "batched exchange: all_gather(n_r), all_gather(G tables), all_reduce(step totals) "
+                           "for every round without leftovers, then per round all_gather(G,S) + all_reduce" if batched
+                           else "per round all_gather(G,S) + all_reduce(step totals)"),
                        "l2": "no flush: inputs and outputs are far larger than the 126 MB L2"},
             "tokens_per_s": n_tok / (ms * 1e-3), "stage_ms": {"collate_kernel": col_ms},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
@@ -840,6 +844,36 @@ def paper_operating_point(P, device, peak):
     row["sequential_round_loop"] = {k: seq[k] for k in ("ms_per_step", "planning_ms", "planning_ms_per_round",
                                                         "launches_per_step")}
     return row
+
+
+def sharded_protocol_rows(steps=5, warmup=3):
+    """The multi-process protocol (F1: paper_2606_19989_b200/dist.py over NCCL) at the paper's operating point, on this
+    one GPU (world size 1 -- no N > 1 number can be taken here): the batched exchange beside one exchange per round.
+    Each row is a `bench.py --shard-ranks` run in a process of its own (its own NCCL world); a failure is reported,
+    it never breaks the main line."""
+    import socket
+    import subprocess
+    rows = []
+    for name, extra in (("batched exchange (J rounds: 3 collectives + 2 scalar exchanges)", []),
+                        ("one exchange per round (P:52)", ["--per-round-exchange"])):
+        sk = socket.socket()
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+        sk.close()
+        env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "LOCAL_WORLD_SIZE"):
+            env.pop(k, None)
+        cmd = [sys.executable, os.path.abspath(__file__), "--shard-ranks", "--buffer-size", "1024", "--steps", str(steps),
+               "--warmup", str(warmup)] + extra
+        try:
+            r = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=240)
+            d = json.loads(r.stdout.strip().splitlines()[-1])
+            rows.append({"exchange": name, "ms_per_step": d["ms_per_step"], "samples_per_s": d["value"],
+                         "collate_ms": d["stage_ms"]["collate_kernel"], "gpu_launches_per_step": d["gpu_launches"] / steps,
+                         "n_rounds": d["config"]["n_rounds"], "n_gpus": d["n_gpus"]})
+        except Exception as e:  # noqa: BLE001 (a measurement beside the line, never the line itself)
+            rows.append({"exchange": name, "error": repr(e)[:200]})
+    return rows
 
 
 def streaming_output(P, device, peak, steps_per_chunk=40, reps=5):
