@@ -359,6 +359,39 @@ typedef struct {
 ODB_API int odb_offline_plan(odb_ctx *ctx, const odb_offline_params *params, const int32_t *d_lengths, int64_t n_samples,
                              void *stream);
 
+/* ---- for callers that cannot allocate device memory ------------------------------------------------
+ * Some users of this library are guests on a GPU they do not manage: a data-loading plugin inside a trainer whose
+ * framework has already claimed the whole HBM for its caching allocator (a second party's cudaMalloc then fails, or
+ * works and makes the trainer run out of memory later), or code running in the middle of a training step, where
+ * cudaMalloc / cudaFree hold up every stream of the device.  They cannot call odb_create (the context allocates
+ * ~70 bytes per sample).  odb_slot_offsets_static is the one entry point made for them: it takes no context, calls no
+ * cudaMalloc / cudaFree and no library routine that allocates, and keeps the scan's tile records in a fixed
+ * 128.25 KiB array that is part of the library image (every GPU that loads libodb.so holds it until the process ends).
+ *
+ * It computes the output offsets of a plan (A9; a group's padded block is count x width), as
+ * odb_plan_query / odb_run do for out->d_grp_offset:
+ *     d_grp_offset[s] = sum over s' < s of round_up(d_grp_count[s'] * d_grp_width[s'], 16),   s = 0 .. n_slots,
+ * so d_grp_offset[n_slots] is odb_plan_info.total_elems.  d_grp_count, d_grp_width: device, n_slots int32 each,
+ * caller-owned, read only; d_grp_offset: device, n_slots + 1 int64, caller-owned, written.  n_slots = 0 is allowed
+ * (writes d_grp_offset[0] = 0).  Asynchronous on `stream`, on the device that is current when it is called.
+ *
+ * Limit: n_slots <= ODB_STATIC_MAX_SLOTS (odb_static_max_slots() returns it).  More slots than that: ODB_ERR_CAPACITY,
+ * nothing launched, nothing written -- the fixed array has no tile records for them.  Bad pointers or n_slots < 0:
+ * ODB_ERR_INVALID_ARG.  A failing CUDA call: ODB_ERR_CUDA, with the cudaError_t in odb_static_last_cuda_error()
+ * (per host thread).
+ *
+ * First call on each device: it asks the CUDA runtime for the array's address on that device (a one-time set-up,
+ * kept for later calls).  Make that first call before you start capturing a stream.
+ * Sharing: all calls on a device use the same array, and each call starts by clearing the part it needs (two small
+ * kernels per call: the clear, then the scan).  Two calls whose kernels may run at the same time on one device --
+ * different streams with no ordering between them, or two host threads -- corrupt each other's result: put them on
+ * one stream or order them with events. */
+#define ODB_STATIC_MAX_SLOTS 4194304 /* 2^22 slots (the largest BASELINE.json config has ~2 * 10^5) */
+ODB_API int odb_slot_offsets_static(const int32_t *d_grp_count, const int32_t *d_grp_width, int64_t n_slots,
+                                    int64_t *d_grp_offset, void *stream);
+ODB_API int64_t odb_static_max_slots(void);
+ODB_API int odb_static_last_cuda_error(void);
+
 /* Tuning / measurement switches.  ODB_OPT_COLLATE_BULK_STORES (value 0 / 1, default 0): the collate kernel stages
  * the interior chunks of each arena in shared memory and stores them with bulk asynchronous copies
  * (cp.async.bulk.global.shared::cta, the store side of BASELINE.json's "TMA bulk copies") instead of 256-bit

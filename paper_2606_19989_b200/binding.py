@@ -111,6 +111,9 @@ SYMBOLS = {
     "odb_get_timing": (_i32, [_vp, _P(ctypes.c_float)]),
     "odb_get_timing_at": (_i32, [_vp, _i32, _P(ctypes.c_float)]),
     "odb_offline_plan": (_i32, [_vp, _P(odb_offline_params), _vp, _i64, _vp]),
+    "odb_slot_offsets_static": (_i32, [_vp, _vp, _i64, _vp, _vp]),
+    "odb_static_max_slots": (_i64, []),
+    "odb_static_last_cuda_error": (_i32, []),
     "odb_set_option": (_i32, [_vp, _i32, _i64]),
     "odb_probe_bandwidth": (_i32, [_i32, _vp, _vp, _vp, _vp, _vp, _i64, _i32, _vp, _P(ctypes.c_float)]),
     "odb_kernel_launches": (_i64, [_vp]),
@@ -393,6 +396,29 @@ ODB_OPT_HOST_DEVICE_ARENAS = 4
 
 def odb_set_option(ctx: int, option: int, value: int) -> None:
     _check(load().odb_set_option(ctx, int(option), int(value)), "odb_set_option", ctx)
+
+
+def odb_static_max_slots() -> int:
+    """Largest ``n_slots`` ``odb_slot_offsets_static`` accepts (ODB_STATIC_MAX_SLOTS)."""
+    return int(load().odb_static_max_slots())
+
+
+def odb_slot_offsets_static(d_grp_count, d_grp_width, n_slots: int, d_grp_offset, stream=None) -> None:
+    """The plan's output offsets without a context and without any device allocation, for callers that are not
+    allowed to allocate on the GPU they run on (a loader living inside a trainer that owns all of HBM; code in the
+    middle of a step, where cudaMalloc / cudaFree stall the device).  ``d_grp_offset[s]`` (int64, ``n_slots + 1``
+    entries) = sum over s' < s of round_up(count * width, 16).  The tile records of the scan live in a fixed array
+    inside libodb.so, shared by every call on the device: keep calls on one stream (or order them), make the first
+    call on a device outside stream capture, and stay within ``odb_static_max_slots()`` -- beyond it the call raises
+    ``OdbError(ODB_ERR_CAPACITY)`` and touches nothing.  Details: include/odb.h."""
+    L = load()
+    rc = L.odb_slot_offsets_static(_ptr(d_grp_count), _ptr(d_grp_width), int(n_slots), _ptr(d_grp_offset),
+                                   _stream(stream))
+    if rc == ODB_ERR_CAPACITY:
+        raise OdbError(rc, "odb_slot_offsets_static: n_slots %d is above the fixed scratch's limit of %d slots"
+                       % (int(n_slots), int(L.odb_static_max_slots())))
+    if rc != ODB_OK:
+        raise OdbError(rc, "odb_slot_offsets_static", L.odb_static_last_cuda_error() if rc == ODB_ERR_CUDA else 0)
 
 
 def odb_probe_bandwidth(kind: int, d_in, d_out0, d_out1, d_out2, d_out3, n_elems: int, reps: int = 5, stream=None) -> float:

@@ -9,7 +9,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libodb.so")
-SOURCES = ["odb_api.cu", "odb_plan.cu", "odb_sort.cu", "odb_collate.cu", "odb_scale.cu", "odb_synth.cu", "odb_probe.cu", "odb_offline.cu"]
+SOURCES = ["odb_api.cu", "odb_plan.cu", "odb_sort.cu", "odb_collate.cu", "odb_scale.cu", "odb_synth.cu", "odb_probe.cu", "odb_offline.cu",
+           "odb_static.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-shared",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
