@@ -349,18 +349,22 @@ def offline_workload(n_ranks: int, seed: int = 0, *, n: int = 4096, mean: float 
     return wl
 
 
-def split_ranks(wl: Workload, n_parts: int):
+def split_ranks(wl: Workload, n_parts: int, bounds=None):
     """The same job held by ``n_parts`` processes: part p gets the consecutive ranks
-    [p*R/n_parts, (p+1)*R/n_parts) with their samples, spans and (same hash indices) tokens.  Pure slicing."""
+    [p*R/n_parts, (p+1)*R/n_parts) with their samples, spans and (same hash indices) tokens.  Pure slicing.
+    ``bounds`` (optional, n_parts + 1 rising rank indices from 0 to R) gives the processes unequal rank counts."""
     R = wl.n_ranks
-    assert R % n_parts == 0
-    rl = R // n_parts
+    if bounds is None:
+        assert R % n_parts == 0
+        bounds = [p * (R // n_parts) for p in range(n_parts + 1)]
+    assert len(bounds) == n_parts + 1 and bounds[0] == 0 and bounds[-1] == R
     parts = []
     for p in range(n_parts):
-        g0, g1 = int(wl.rank_ptr[p * rl]), int(wl.rank_ptr[(p + 1) * rl])
+        r0, r1 = int(bounds[p]), int(bounds[p + 1])
+        g0, g1 = int(wl.rank_ptr[r0]), int(wl.rank_ptr[r1])
         sp0, sp1 = int(wl.span_ptr[g0]), int(wl.span_ptr[g1])
-        parts.append(Workload("%s[part %d/%d]" % (wl.name, p, n_parts), rl,
-                              (wl.rank_ptr[p * rl:(p + 1) * rl + 1] - g0).copy(), wl.lengths[g0:g1].copy(),
+        parts.append(Workload("%s[part %d/%d]" % (wl.name, p, n_parts), r1 - r0,
+                              (wl.rank_ptr[r0:r1 + 1] - g0).copy(), wl.lengths[g0:g1].copy(),
                               (wl.sample_ptr[g0:g1 + 1] - wl.sample_ptr[g0]).copy(),
                               (wl.span_ptr[g0:g1 + 1] - sp0).copy(), wl.span_lo[sp0:sp1].copy(),
                               wl.span_hi[sp0:sp1].copy(), wl.token_seed, dict(wl.params),

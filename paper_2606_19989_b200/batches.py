@@ -71,8 +71,12 @@ class StepStream:
     (odb_collate_steps): ``for chunk in StepStream(...): for step in chunk: ...`` where ``chunk`` is a
     ``StepBatches`` over the chunk's steps (``chunk.step_lo`` = its first plan-wide step).  While the consumer
     works on chunk i, chunk i + 1 is being collated on the other stream into the other buffer (double buffering,
-    SURVEY.md 8(f) F3; "output queue").  The views of a chunk are valid until the next-but-one chunk is
-    requested.  ``slot_elems`` bounds one slot's block (max(budget, longest sample) is enough); plumbing only.
+    SURVEY.md 8(f) F3; "output queue").  The views of a chunk are valid until the NEXT chunk is requested:
+    asking for chunk i hands the buffer of chunk i - 1 back, and chunk i + 1 is enqueued into it at once.  That
+    overwrite is ordered behind whatever the consumer had enqueued, up to the moment of the request, on the stream
+    that is current when it asks (an event recorded there, waited on by the collating stream); work on any other
+    stream must be joined to that stream (``wait_stream``) before asking.  ``slot_elems`` bounds one slot's block
+    (max(budget, longest sample) is enough); plumbing only.
     """
 
     def __init__(self, ctx, n_ranks: int, n_steps: int, n_samples: int, inputs, steps_per_chunk: int, slot_elems: int,
@@ -89,6 +93,8 @@ class StepStream:
         ids = min(slots * int(slot_elems), int(n_samples))  # (a sample has at least one token)
         self.bufs = [B.OutputBuffers(self.n_ranks, elems, slots, ids, self.chunk, 0, device, fill=fill) for _ in range(2)]
         self.streams = [torch.cuda.Stream(device=device) for _ in range(2)]
+        self.device = device
+        self._torch = torch
 
     def __len__(self) -> int:
         return (self.n_steps + self.chunk - 1) // self.chunk
@@ -97,6 +103,10 @@ class StepStream:
         lo = i * self.chunk
         hi = min(self.n_steps, lo + self.chunk)
         b = i & 1
+        # buffer b last held chunk i - 2, which the consumer gave up with this request: its reads come first
+        released = self._torch.cuda.Event()
+        released.record(self._torch.cuda.current_stream(self.device))
+        self.streams[b].wait_event(released)
         info = self._B.odb_collate_steps(self.ctx, lo, hi, *self.inputs, self.bufs[b].struct,
                                          stream=self.streams[b].cuda_stream)
         return b, info, lo

@@ -180,7 +180,10 @@ def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=Non
             exc[0] = e
             return None
 
-    wmax = yield ("max_int", int(engine.local_max_window()))
+    # one MAX exchange carries the largest window of the job and, as (n, -n), the largest and the smallest number of
+    # ranks any process holds: what decides the protocol's shape below is then the same data in every process
+    wmax, r_hi, r_lo = yield ("max_int", [int(engine.local_max_window()), int(engine.n_ranks), -int(engine.n_ranks)])
+    even_split = r_hi == -r_lo and r_hi > 0 and world_ranks % r_hi == 0
     call(engine.dist_config, world_ranks, rank_offset, int(wmax))
     # the step-total window of a round has the same size in every process: T_grp <= the largest window of the job
     cap = int(getattr(engine.params, "slot_capacity", 0) or 0)
@@ -190,7 +193,9 @@ def plan_protocol(engine, world_ranks: int, rank_offset: int, avail_schedule=Non
     # ---- batched exchange: every round that starts without leftovers, 3 collectives for all of them ----
     # (a round depends on its predecessors only through the leftovers; Eq. 3 and the no-overflow check of every
     #  round are evaluated by every process on the same gathered tables, so all take the same decisions: Lemma 3)
-    if batched and avail_schedule is None and hasattr(engine, "spec_form") and world_ranks % engine.n_ranks == 0:
+    # (its [process][round][local rank] layout needs the same number of ranks in every process: with 2 + 6 ranks of 8
+    #  every process takes the per-round exchange below -- decided from the exchanged counts, never from the local one)
+    if batched and avail_schedule is None and hasattr(engine, "spec_form") and even_split:
         n_local = call(engine.stream_lengths)
         if n_local is None:
             n_local = torch.zeros(engine.n_ranks, dtype=torch.int32, device=dev)
@@ -272,11 +277,13 @@ class TorchCollectives:
         self.world_size = dist.get_world_size(group)
         self.rank = dist.get_rank(group)
 
-    def max_int(self, v: int, device="cpu") -> int:
+    def max_int(self, v, device="cpu"):
+        """Element-wise MAX over the processes of an int or of a short list of ints (one collective either way)."""
         import torch
-        t = torch.tensor([int(v)], dtype=torch.int64, device=device)
+        many = isinstance(v, (list, tuple))
+        t = torch.tensor([int(x) for x in (v if many else [v])], dtype=torch.int64, device=device)
         self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
-        return int(t.item())
+        return [int(x) for x in t.tolist()] if many else int(t.item())
 
     def all_gather(self, out, inp):
         if inp.numel() == 0:
@@ -335,8 +342,12 @@ def run_lockstep(gens: Sequence[Generator]):
         kind = active[0][0]
         replies = [None] * n
         if kind == "max_int":
-            m = max(r[1] for r in reqs)
-            replies = [m] * n
+            if isinstance(reqs[0][1], (list, tuple)):
+                m = [max(col) for col in zip(*(r[1] for r in reqs))]
+                replies = [list(m) for _ in range(n)]
+            else:
+                m = max(r[1] for r in reqs)
+                replies = [m] * n
         elif kind == "all_gather":
             cat = torch.cat([r[2].reshape(-1) for r in reqs]) if reqs[0][2].numel() else None
             for r in reqs:

@@ -199,3 +199,29 @@ def test_lockstep_driver_with_oracle_engines(n_proc):
                 assert round_T == plan.round_T.tolist() and info.step_samples == plan.step_samples.tolist()
                 for j in range(rl):
                     assert info.slots[j] == plan.groups_of_rank(p * rl + j), (name, with_sched, p, j)
+
+
+@pytest.mark.parametrize("bounds", [(0, 1, 4), (0, 1, 2, 4), (0, 3, 4)])
+def test_lockstep_unequal_rank_counts(bounds):
+    """Processes holding different numbers of ranks (1 + 3, 1 + 1 + 2, 3 + 1 of 4): the shape of the protocol is
+    decided from exchanged rank counts, so all issue the same collectives (the lock-step driver raises when they
+    diverge) and none takes the batched exchange, whose table layout needs equal counts."""
+    sys.path.insert(0, ROOT)
+    import odb_inputs as I
+    from oracle import odb_oracle
+    from paper_2606_19989_b200 import dist as D
+    from tests._oracle_engine import OracleEngine
+    odb_oracle.build()
+    for name in ("batched_equal", "batched_ragged", "batched_nonjoin", "overflow_multiround"):
+        wl = _case(name)
+        assert wl.n_ranks == 4
+        plan, _ = odb_oracle.run_workload(wl, collate=False)
+        n_proc = len(bounds) - 1
+        engines = [OracleEngine(odb_oracle, part) for part in I.split_ranks(wl, n_proc, bounds=bounds)]
+        res = D.run_lockstep([D.plan_protocol(e, wl.n_ranks, bounds[p]) for p, e in enumerate(engines)])
+        for p, (info, round_T) in enumerate(res):
+            assert not getattr(engines[p], "spec_T", None), (name, bounds)  # the batched exchange was not taken
+            assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason), name
+            assert round_T == plan.round_T.tolist() and info.step_samples == plan.step_samples.tolist()
+            for j in range(bounds[p + 1] - bounds[p]):
+                assert info.slots[j] == plan.groups_of_rank(bounds[p] + j), (name, bounds, p, j)

@@ -223,6 +223,44 @@ def test_batched_exchange_commits_rounds_and_equals_the_round_by_round_protocol(
                     e.close()
 
 
+@pytest.mark.parametrize("bounds", [(0, 2, 8), (0, 2, 4, 8), (0, 5, 8), (0, 4, 8)])
+def test_lockstep_unequal_rank_counts_take_one_path_everywhere(P, oracle, bounds):
+    """8 ranks held by processes with 2 + 6, 2 + 2 + 4, 5 + 3 (and, as the control, 4 + 4) of them, on a job the batched
+    exchange would take: whether it is taken is decided from the exchanged rank counts, so every process issues
+    the same collectives (run_lockstep raises if they diverge) and the plan is the whole-job oracle's either way."""
+    import torch
+    from paper_2606_19989_b200 import dist as D
+    rng = np.random.default_rng(11)
+    wl = I.custom_workload("batched_8", [rng.integers(8, 1500, k) for k in (900, 1000, 950, 0, 1000, 870, 990, 1000)],
+                           seed=9, budget=8192, buffer_size=256)
+    plan, _ = oracle.run_workload(wl, collate=False)
+    R, K = wl.n_ranks, plan.n_steps
+    n_proc = len(bounds) - 1
+    parts = I.split_ranks(wl, n_proc, bounds=bounds)
+    dws = [Par.DeviceWorkload(w) for w in parts]
+    engines = [D.CudaEngine(Par.gpu_params(w), max(w.n_samples, 1), dw.lengths, w.rank_ptr) for w, dw in zip(parts, dws)]
+    try:
+        res = D.run_lockstep([D.plan_protocol(e, R, bounds[p]) for p, e in enumerate(engines)])
+        for p, e in enumerate(engines):
+            info, round_T = res[p]
+            assert round_T == plan.round_T.tolist()
+            assert (info.n_rounds, info.n_steps, info.stop_reason) == (plan.n_rounds, plan.n_steps, plan.stop_reason)
+            rec = np.zeros(4, dtype=np.int32)
+            took_batched = P.odb_debug_read(e.ctx.h, 4, rec) == 16
+            assert took_batched == (bounds == (0, 4, 8)), (bounds, p)
+            rl = bounds[p + 1] - bounds[p]
+            out = P.OutputBuffers.for_plan(rl, info, dws[p].device)
+            e.collate(dws[p].tokens, dws[p].sample_ptr, dws[p].span_ptr, dws[p].span_lo, dws[p].span_hi, out)
+            torch.cuda.synchronize()
+            s0, s1 = bounds[p] * K, bounds[p + 1] * K
+            assert np.array_equal(out.table("grp_count").cpu().numpy(), plan.grp_count[s0:s1])
+            assert np.array_equal(out.table("grp_width").cpu().numpy(), plan.grp_width[s0:s1])
+            assert np.array_equal(out.table("step_samples").cpu().numpy(), plan.step_samples)
+    finally:
+        for e in engines:
+            e.close()
+
+
 def test_single_process_nccl_world(P, oracle):
     """The torch.distributed driver itself (NCCL, world_size 1 -- the box has one GPU): the protocol
     with real collectives on the library's device buffers equals the oracle."""

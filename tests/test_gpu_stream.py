@@ -159,6 +159,43 @@ def test_two_ranges_in_flight_and_step_stream(P, oracle):
         assert seen == K and len(stream) == (K + chunk - 1) // chunk
 
 
+def test_step_stream_orders_buffer_reuse_after_async_consumer(P, oracle):
+    """A consumer that reads a chunk's views with GPU work it does not wait for (a long delay kernel, then copies, on
+    a stream of its own) and asks for the next chunk from that stream: the iterator must hold the overwrite of the
+    handed-back buffer until those reads are done.  Every copy, checked at the very end, is the oracle's block."""
+    import torch
+    wl = I.make_workload(1, n_ranks=4, n_per_rank=2500)
+    wl.params["buffer_size"] = 256
+    plan, ref = oracle.run_workload(wl)
+    dw = Par.DeviceWorkload(wl)
+    R, K = wl.n_ranks, plan.n_steps
+    inputs = (dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi)
+    names = ("input_ids", "labels", "position_ids", "attention_mask")
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        P.odb_plan(ctx.h, dw.lengths, wl.rank_ptr)
+        chunk = 5
+        stream = P.StepStream(ctx.h, R, K, wl.n_samples, inputs, chunk,
+                              max(int(wl.params["budget"]), int(wl.lengths.max())), dw.device)
+        assert len(stream) >= 4  # buffers are reused several times
+        side = torch.cuda.Stream()
+        copies = []
+        with torch.cuda.stream(side):  # next() is called with `side` current
+            for c in stream:
+                torch.cuda._sleep(30_000_000)  # ~15 ms: the next chunk's collation would long be done
+                for kk, step in enumerate(c):
+                    for r in range(R):
+                        b = step[r]
+                        if b is not None:
+                            copies.append((r, c.step_lo + kk, {n: b[n].clone() for n in names}))
+        torch.cuda.synchronize()
+    assert len(copies) == int((plan.grp_count > 0).sum())
+    for r, k, got in copies:
+        s = r * K + k
+        cnt, wid, off = int(plan.grp_count[s]), int(plan.grp_width[s]), int(plan.grp_offset[s])
+        for n in names:
+            assert np.array_equal(got[n].cpu().numpy().reshape(-1), ref[n][off:off + cnt * wid]), (n, r, k)
+
+
 def test_collate_steps_errors(P):
     import torch
     wl = I.make_workload(0)
