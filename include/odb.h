@@ -24,10 +24,12 @@
  *   - Samples are laid out rank-major: rank r owns samples h_rank_ptr[r] .. h_rank_ptr[r+1]-1 in
  *     sampler order; a "local id" is the index inside the rank.
  *   - d_sample_ptr[g] .. d_sample_ptr[g+1] are the token offsets of global sample g in d_tokens and
- *     must equal the prefix sum of d_lengths.  d_tokens must be 16-byte aligned, and READABLE up to the
- *     next multiple of 4 int32 past its last token: the collate kernel fetches tokens with aligned 16-byte
- *     loads, so the vector that holds the last token is read whole (the extra words are discarded).
- *     odb_run_host pads its own staging; callers of odb_collate / odb_run allocate round_up(n_tokens, 4).
+ *     must equal the prefix sum of d_lengths.  d_tokens must be 16-byte aligned; a buffer of exactly n_tokens
+ *     words is enough.  The collate kernel fetches tokens with aligned 16-byte loads, so when n_tokens is not a
+ *     multiple of 4 the 16-byte unit that holds the last token is read whole: that unit starts at a 16-byte
+ *     boundary inside the caller's mapping and cannot cross a page, so the load cannot fault; the up to 3 words
+ *     behind the last token are whatever the caller keeps there, and they are discarded, never copied to an output
+ *     (tests/test_gpu_parity.py::test_token_buffer_of_exactly_n_tokens).
  *   - Masked spans (labels -> ignore_index) are CSR per sample: spans d_span_ptr[g] .. d_span_ptr[g+1]-1,
  *     half-open [lo,hi) token positions, sorted and disjoint.
  *   - Every call returns an ODB_* status (0 = OK).  No exceptions, no abort, nothing printed.
@@ -183,8 +185,8 @@ ODB_API int odb_collate(odb_ctx *ctx, const int32_t *d_tokens, const int64_t *d_
 /* The whole plan without collation: reset, every protocol round until termination (on the device where odb_run
  * would run them there: the round-parallel planner and the persistent round loop for grouping buffers of at most
  * 4096 samples; host-driven rounds otherwise), the slot scan.  Synchronises for the plan sizes (*h_out);
- * afterwards the context is where odb_plan_query leaves it: odb_collate, odb_collate_steps and odb_loss_weights
- * may follow. */
+ * afterwards the context is where odb_plan_query leaves it: odb_collate and odb_collate_steps may follow, and
+ * odb_loss_weights once a full odb_collate has counted the valid tokens (not after odb_collate_steps alone). */
 ODB_API int odb_plan(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_rank_ptr, odb_plan_info *h_out, void *stream);
 
 /* Streaming output (section 2.3: a round's aligned groups go to the trainer while the next window is being
@@ -200,7 +202,14 @@ ODB_API int odb_plan(odb_ctx *ctx, const int32_t *d_lengths, const int64_t *h_ra
  * for those sizes; the collate kernel is then running on `stream`.  The library keeps TWO sets of range tables and
  * alternates between them, so two ranges can be in flight at once (double buffering: a call reuses the tables of
  * the call before the previous one and must be ordered behind it -- same stream, or that call's work complete).
- * Null arenas: a sizing call (ODB_ERR_CAPACITY with *h_out filled unless the range is empty).  ODB_ERR_CAPACITY
+ * After odb_plan / odb_run each set is sized for the whole plan on its first use, so later ranges (a longer chunk, a
+ * larger arena) allocate nothing; between rounds of the staged calls a range larger than any before it grows the set
+ * (cudaFree + cudaMalloc: a device-wide synchronisation).
+ * Null arenas: a sizing call (ODB_ERR_CAPACITY with *h_out filled unless the range is empty); it does not count in
+ * the alternation -- the call that follows it uses the same set and should use the same stream.
+ * The range's grp_valid_tokens / step_valid_tokens go to `out` only: the loss-scaling calls (odb_loss_weights,
+ * odb_loss_numerators, odb_loss_normalize) need one full odb_collate of the plan and return ODB_ERR_STATE after
+ * step-range collation alone.  ODB_ERR_CAPACITY
  * (nothing written) if an arena or table of `out` is too small; ODB_ERR_STATE for offline plans and distributed
  * mode. */
 ODB_API int odb_collate_steps(odb_ctx *ctx, int32_t step_lo, int32_t step_hi, const int32_t *d_tokens,
@@ -428,7 +437,9 @@ ODB_API int64_t odb_kernel_launches(const odb_ctx *ctx);
  * of the last round, 1 = S_r (int32[R]), 2 = sorted keys of the last round ((len<<32)|id, uint64[N],
  * rank regions at h_rank_ptr), 3 = views emitted so far per rank (int32[R]; valid between rounds of the staged calls),
  * 4 = the record of the round-parallel planner of the last odb_run (int32[4]: rounds it committed, steps they emit,
- * 1 if it ended the protocol, 0; < 0 is returned when that run did not use it).
+ * 1 if it ended the protocol, 0; < 0 is returned when that run did not use it),
+ * 5 = how many times the library's growable device tables have called cudaMalloc in this process so far (int64; a
+ * host-side counter, no synchronisation).
  * Returns bytes copied or < 0. */
 ODB_API int64_t odb_debug_read(odb_ctx *ctx, int what, void *h_dst, int64_t max_bytes);
 

@@ -1161,9 +1161,22 @@ int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_
     c->timing = 0;
     int rc = [&]() -> int {
         const int64_t slots = (int64_t)R * n;
-        int rc2 = ensure_plan_tables(c, (size_t)slots, (size_t)n);
+        // Table sizes: growing a table is cudaFree + cudaMalloc, both device-wide synchronisations that would stall the
+        // range in flight on the other stream.  Once the whole plan is known (odb_plan) every table of a set is
+        // therefore sized for the WHOLE plan the first time the set is used -- a few bytes per slot, 12 per tile --
+        // and no later range (a longer chunk, a larger arena) grows it.  While rounds are still being added (state 3)
+        // the plan's size is open and a range larger than any before it does grow the set.
+        const bool whole = c->state == 5 && c->info_valid;
+        const int64_t slots_alloc = whole ? std::max<int64_t>(slots, (int64_t)R * c->n_steps) : slots;
+        const int64_t steps_alloc = whole ? std::max<int64_t>(n, c->n_steps) : n;
+        int rc2 = ensure_plan_tables(c, (size_t)slots_alloc, (size_t)steps_alloc);
         if (rc2 != ODB_OK) return rc2;
-        const int64_t tile_bound = (std::max<int64_t>(o->arena_capacity, 0) + kColTile - 1) / kColTile;
+        int64_t tile_bound = (std::max<int64_t>(o->arena_capacity, 0) + kColTile - 1) / kColTile;
+        if (whole) {  // (a range holds a subset of the plan's blocks: never more tiles than the plan)
+            const int64_t plan_tiles = (c->info.total_elems + kColTile - 1) / kColTile;
+            tile_bound = std::min(tile_bound, plan_tiles);
+            CU(c, c->tiles.ensure((size_t)plan_tiles + 2));
+        }
         const bool any_slot_tab = o->d_grp_count || o->d_grp_width || o->d_grp_round || o->d_grp_valid_tokens ||
                                   o->d_grp_real_tokens || o->d_grp_origin || o->d_grp_offset || o->d_grp_sample_ptr;
         CapCheck cap;
@@ -1174,7 +1187,7 @@ int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_
         cap.left = -1;
         cap.tiles = tile_bound;
         CU(c, launch_sub_dims(c, n, st));
-        CU(c, launch_finalize(c, slots, cap, nullptr, st, step_lo));
+        CU(c, launch_finalize(c, slots, cap, nullptr, st, step_lo, slots_alloc));
         CU(c, cudaEventRecord(c->ev_plan, st));
         CU(c, launch_sub_ids(c, step_lo, o->d_grp_sample_ids, full_sp, full_K, st));
         if (!arenas) return ODB_OK;  // a sizing call
@@ -1183,7 +1196,9 @@ int odb_collate_steps(odb_ctx *c, int32_t step_lo, int32_t step_hi, const int32_
     c->timing = timing;
     c->sub_mode = false;
     swap_tabs(c, T);
-    c->sub_seq++;
+    // a sizing call (no arenas) enqueues no collate kernel: the real call that follows it takes the SAME table set, on
+    // the same stream, so that "sizing call, then the range" still leaves the other set to the other range in flight
+    if (arenas) c->sub_seq++;
     if (rc != ODB_OK) return rc;
     CU(c, cudaEventSynchronize(T.ev_plan));  // the range's sizes; its collate kernel is running
     const PlanDims &D = *T.h_dims;
@@ -1596,6 +1611,12 @@ int odb_loss_normalize(odb_ctx *c, const double *d_num_world, int32_t world_rank
 
 int64_t odb_debug_read(odb_ctx *c, int what, void *h_dst, int64_t max_bytes) {
     if (!c || !h_dst) return -1;
+    if (what == 5) {  // a host-side counter: no device access
+        if (max_bytes < 8) return -1;
+        const long long v = odb::g_table_allocs.load(std::memory_order_relaxed);
+        memcpy(h_dst, &v, 8);
+        return 8;
+    }
     const void *src = nullptr;
     int64_t bytes = 0;
     const int R = c->prm.n_ranks;

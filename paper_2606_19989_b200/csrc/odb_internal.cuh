@@ -6,6 +6,7 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <atomic>
 #include <vector>
 
 #include "odb.h"
@@ -144,6 +145,10 @@ struct PostArgs {
 };
 
 // growable device buffer (cudaMalloc on growth only)
+// cudaMalloc calls made by the growable tables below, process-wide (diagnostics: odb_debug_read(ctx, 5, ..); a test
+// uses it to show that a pass of step ranges does not allocate after its first range)
+inline std::atomic<long long> g_table_allocs{0};
+
 template <class T>
 struct DevBuf {
     T *p = nullptr;
@@ -157,6 +162,7 @@ struct DevBuf {
             if (e != cudaSuccess) return e;
         }
         size_t want = n + n / 4 + 16;
+        g_table_allocs.fetch_add(1, std::memory_order_relaxed);
         cudaError_t e = cudaMalloc((void **)&p, want * sizeof(T));
         if (e != cudaSuccess) {
             p = nullptr;
@@ -361,9 +367,10 @@ cudaError_t launch_dist_spec_commit(odb_ctx *c, int n_rounds, const int32_t *d_G
 cudaError_t launch_align_only(odb_ctx *c, cudaStream_t st);     // distributed: A4..A6 from the world summary
 cudaError_t launch_commit_only(odb_ctx *c, cudaStream_t st);    // distributed: A7 + A8a after the all_reduce
 // A9: rank-major tables, offsets, totals (sizes from the device-resident PlanDims)
-// (step_lo: the slot scan covers the steps [step_lo, step_lo + PlanDims.n_steps) of the staging tables)
+// (step_lo: the slot scan covers the steps [step_lo, step_lo + PlanDims.n_steps) of the staging tables;
+//  slots_alloc: size the scan's tile records for at least that many slots, so that later, larger scans do not grow them)
 cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st,
-                            int64_t step_lo = 0);
+                            int64_t step_lo = 0, int64_t slots_alloc = 0);
 // step-range plans: PlanDims of the range, and the slot CSR's ids of its rows (global in the library's table, local
 // in the caller's)
 cudaError_t launch_sub_dims(odb_ctx *c, int n_steps, cudaStream_t st);

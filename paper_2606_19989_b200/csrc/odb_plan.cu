@@ -2103,13 +2103,14 @@ cudaError_t launch_dist_spec_commit(odb_ctx *c, int n_rounds, const int32_t *d_G
 // A9.  `slots_bound` >= the number of slots the plan can hold (the host may not have seen the plan yet);
 // the grid is persistent: tiles are taken by ticket.
 cudaError_t launch_finalize(odb_ctx *c, int64_t slots_bound, const CapCheck &cap, int64_t *rank_off, cudaStream_t st,
-                            int64_t step_lo) {
+                            int64_t step_lo, int64_t slots_alloc) {
     const int R = c->prm.n_ranks;
     const int64_t so = step_lo * R;  // the staging tables are step-major: a step range is a contiguous piece
     const int64_t n_tiles = std::max<int64_t>((slots_bound + kFinTile - 1) / kFinTile, 1);
     // [0, 64): ticket + exit counter (rewound by the kernel's last CTA); then the tile states, whose flags carry the
     // launch's epoch, so nothing has to be cleared between launches (zeroed once, when the buffer grows)
-    cudaError_t e = c->scan_state.ensure((size_t)n_tiles * sizeof(ScanTile) + 64, true, st);
+    const int64_t tiles_alloc = std::max<int64_t>(n_tiles, (slots_alloc + kFinTile - 1) / kFinTile);
+    cudaError_t e = c->scan_state.ensure((size_t)tiles_alloc * sizeof(ScanTile) + 64, true, st);
     if (e != cudaSuccess) return e;
     c->fin_epoch = (c->fin_epoch % 0x1ffffffe) + 1;  // 1 .. 2^29 - 1
     const int blocks = (int)std::min<int64_t>(n_tiles, (int64_t)c->sm_count * 2);

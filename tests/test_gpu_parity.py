@@ -841,3 +841,31 @@ def test_wide_fuzz(P, oracle):
             Par.compare_full(plan, ref, info, out)
         except AssertionError as e:
             raise AssertionError("wide fuzz seed %d params %r: %s" % (seed, wl.params, e))
+
+
+@pytest.mark.parametrize("tail", [1, 2, 3])
+def test_token_buffer_of_exactly_n_tokens(P, oracle, tail):
+    """include/odb.h, conventions: d_tokens needs exactly n_tokens words.  A job whose token count is ``tail`` modulo 4,
+    its tokens a 16-byte aligned view in the middle of a larger allocation whose every other word is poison: the
+    16-byte unit that holds the last token is read whole, but nothing of the words behind it (or in front of the
+    buffer) reaches an output -- plan and arenas are the oracle's, byte for byte."""
+    import torch
+    for seed in range(64):
+        wl = I.protocol_workload("unequal", seed)
+        if wl.n_tokens % 4 == tail:
+            break
+    else:
+        pytest.fail("no workload with n_tokens %% 4 == %d" % tail)
+    n_tok = wl.n_tokens
+    dw = Par.DeviceWorkload(wl)
+    poison = torch.full((n_tok + 64,), 0x5A5A5A5A, dtype=torch.int32, device=dw.device)
+    view = poison[32:32 + n_tok]
+    assert view.data_ptr() % 16 == 0 and view.numel() == n_tok
+    view.copy_(dw.tokens[:n_tok])
+    dw.tokens = view
+    plan, ref = oracle.run_workload(wl)
+    for staged in (False, True):
+        info, out, _ = Par.run_gpu(wl, dw, staged=staged)
+        Par.compare_plan(plan, info, out)
+        Par.compare_full(plan, ref, info, out)
+    assert (poison[:32] == 0x5A5A5A5A).all() and (poison[32 + n_tok:] == 0x5A5A5A5A).all()  # inputs are read-only

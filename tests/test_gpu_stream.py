@@ -196,6 +196,59 @@ def test_step_stream_orders_buffer_reuse_after_async_consumer(P, oracle):
             assert np.array_equal(got[n].cpu().numpy().reshape(-1), ref[n][off:off + cnt * wid]), (n, r, k)
 
 
+def _table_allocs(P, ctx):
+    v = np.zeros(1, dtype=np.int64)
+    assert P.odb_debug_read(ctx.h, 5, v) == 8
+    return int(v[0])
+
+
+def test_step_ranges_allocate_once_and_sizing_calls_keep_the_alternation(P, oracle):
+    """After odb_plan the two range-table sets are sized for the whole plan when first used: ranges that grow (longer
+    chunks, larger arenas) make no further cudaMalloc (the library's allocation counter stands still), and a sizing
+    call before every range does not use up the other set -- two ranges, each sized first, in flight on two streams."""
+    import torch
+    wl = I.make_workload(1, n_ranks=4, n_per_rank=2500)
+    wl.params["buffer_size"] = 256
+    plan, ref = oracle.run_workload(wl)
+    dw = Par.DeviceWorkload(wl)
+    R, K = wl.n_ranks, plan.n_steps
+    inputs = (dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi)
+    empty = P.OutputBuffers(R, 0, 0, 0, 0, 0, dw.device)
+    with P.Odb(Par.gpu_params(wl), wl.n_samples) as ctx:
+        P.odb_plan(ctx.h, dw.lengths, wl.rank_ptr)
+        s0, s1 = torch.cuda.Stream(), torch.cuda.Stream()
+        # first use of each set (small ranges), then growing ranges: no allocation after the first two calls
+        cuts = [0, 1, 2, 5, 11, K // 2, K]
+        bufs = [_range_buffers(P, wl, plan, lo, hi, dw.device) for lo, hi in zip(cuts[:-1], cuts[1:])]
+        torch.cuda.synchronize()
+        infos, base = [], None
+        for i, (lo, hi) in enumerate(zip(cuts[:-1], cuts[1:])):
+            st = (s0, s1)[i & 1]
+            infos.append(P.odb_collate_steps(ctx.h, lo, hi, *inputs, bufs[i].struct, stream=st.cuda_stream))
+            if i == 1:
+                base = _table_allocs(P, ctx)
+        assert _table_allocs(P, ctx) == base
+        torch.cuda.synchronize()
+        for i, (lo, hi) in enumerate(zip(cuts[:-1], cuts[1:])):
+            Par.compare_step_range(plan, ref, lo, hi, infos[i], bufs[i], R)
+        # sizing call + range, twice, on two streams; the first range is held back so that both are in flight
+        m = K // 2
+        for _ in range(2):
+            outs, got = [], []
+            for st, (lo, hi) in ((s0, (0, m)), (s1, (m, K))):
+                with torch.cuda.stream(st):
+                    torch.cuda._sleep(10_000_000 if st is s0 else 0)
+                sz = P.odb_collate_steps(ctx.h, lo, hi, *inputs, empty.struct, stream=st.cuda_stream,
+                                         allow_capacity_error=True)
+                out = P.OutputBuffers.for_plan(R, sz, dw.device, fill=Par.SENTINEL)
+                outs.append(out)
+                got.append(P.odb_collate_steps(ctx.h, lo, hi, *inputs, out.struct, stream=st.cuda_stream))
+            torch.cuda.synchronize()
+            Par.compare_step_range(plan, ref, 0, m, got[0], outs[0], R)
+            Par.compare_step_range(plan, ref, m, K, got[1], outs[1], R)
+        assert _table_allocs(P, ctx) == base
+
+
 def test_collate_steps_errors(P):
     import torch
     wl = I.make_workload(0)
