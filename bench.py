@@ -604,12 +604,15 @@ def run_sharded(args):
     ev0.record()
     for _ in range(args.steps):
         info = one()
-        col += P.odb_get_timing(eng.ctx.h)[1]
     ev1.record()
     torch.cuda.synchronize()
     dist.barrier()
     clocks = sampler.stop() if rank == 0 else None
     launches = P.odb_kernel_launches(eng.ctx.h) - l0
+    # the collate kernel's time, read AFTER the timed region (odb_get_timing waits for the stage events): two more steps
+    for _ in range(2):
+        one()
+        col += P.odb_get_timing(eng.ctx.h)[1] * args.steps / 2.0
     tt = torch.tensor([ev0.elapsed_time(ev1) / max(args.steps, 1), col / max(args.steps, 1)], dtype=torch.float64, device=device)
     dist.all_reduce(tt, op=dist.ReduceOp.MAX)
     ms, col_ms = float(tt[0]), float(tt[1])

@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 def P():
     import torch
     if not torch.cuda.is_available():
-        pytest.skip("needs a CUDA device")
+        pytest.fail("the -m gpu tests need a CUDA device (there is no CPU fallback to test)")
     import paper_2606_19989_b200 as P
     P.load()
     return P

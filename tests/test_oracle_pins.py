@@ -368,7 +368,10 @@ def _check_invariants(oracle, wl):
             assert tot - int(p.step_samples[-1]) < Q                                   # stopped at the FIRST such step
         else:
             assert p.stop_reason == oracle.STOP_LOGICAL
-            assert Q <= 0 or prm["emitted_so_far"] + p.samples_emitted < Q or p.n_steps == 0 or True
+            # LOGICAL: some rank is finished -- nothing buffered, nothing pending, so it leaves no sample --
+            # and no emitted step had reached the quota (else the run would have stopped there, Thm 2)
+            assert (np.diff(p.left_ptr) == 0).any()
+            assert Q <= 0 or p.n_steps == 0 or prm["emitted_so_far"] + p.samples_emitted < Q
     return p
 
 
