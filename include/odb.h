@@ -164,6 +164,26 @@ ODB_API int odb_form_groups(odb_ctx *ctx, const int32_t *d_lengths, const int64_
  * odb_form_groups or after odb_round_status; ODB_ERR_STATE otherwise).  h_arrived: host, n_ranks entries. */
 ODB_API int odb_set_available(odb_ctx *ctx, const int64_t *h_arrived, void *stream);
 
+/* Online operation, the caller's side of the loop (App. C.1).  h_emitted[r] (host, n_ranks entries) = how
+ * many views of rank r's stream have been emitted so far: the size of E_r in the paper's per-rank state machine
+ * (a view that overflowed or was cut by the quota is back in the window and does not count).  Between rounds only:
+ * after odb_reset (all 0), after odb_round_status, after termination; ODB_ERR_STATE inside a round and for offline
+ * plans.  Waits for one small device-to-host copy on the stream the rounds were enqueued on. */
+ODB_API int odb_emitted_counts(odb_ctx *ctx, int64_t *h_emitted);
+
+/* The outstanding-depth envelope: the iterator schedules Fetch so that the views fetched but not yet
+ * emitted, |Q_r + B_r|, stay within D = max(prefetch_factor * num_workers, buffer_size) -- the max is the clamp of
+ * App. P: a loader configured with fewer outstanding views than one grouping buffer could never fill
+ * it.  h_fetch_upto[r] = min(n_r, h_emitted[r] + D), n_r = h_rank_ptr[r+1] - h_rank_ptr[r]: how far into rank r's
+ * stream the caller's workers may have fetched by now.  With buffer_size 0 (the window is the whole stream) the
+ * envelope does not bind and h_fetch_upto[r] = n_r.  Lemma 2 is why skip rounds are finite under this
+ * rule: D >= buffer_size >= 1 lets every unfinished rank fetch beyond what it has emitted.  Takes the job's
+ * parameters (n_ranks, buffer_size), not a context: host arithmetic on host arrays of n_ranks (+ 1) entries, no device
+ * work, usable on a machine without a GPU.  ODB_ERR_INVALID_ARG for negative arguments or h_emitted[r] outside
+ * [0, n_r]. */
+ODB_API int odb_fetch_quota(const odb_params *params, const int64_t *h_rank_ptr, int32_t prefetch_factor,
+                            int32_t num_workers, const int64_t *h_emitted, int64_t *h_fetch_upto);
+
 /* Second half (section 2.3, Alg. 1): T_grp by an on-device reduction over the R ranks, split /
  * overflow, IDLE slots, step totals, the non-join quota cut, leftovers.  Asynchronous. */
 ODB_API int odb_align(odb_ctx *ctx, void *stream);

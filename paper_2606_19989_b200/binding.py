@@ -107,6 +107,8 @@ SYMBOLS = {
     "odb_dist_spec_status": (_i32, [_vp, _P(_i32), _P(_i32), _P(_i32), _i32, _P(_i32)]),
     "odb_dist_buffers": (_i32, [_vp, _P(odb_dist_bufs)]),
     "odb_commit": (_i32, [_vp, _vp]),
+    "odb_emitted_counts": (_i32, [_vp, _P(_i64)]),
+    "odb_fetch_quota": (_i32, [_P(odb_params), _P(_i64), _i32, _i32, _P(_i64), _P(_i64)]),
     "odb_set_timing": (_i32, [_vp, _i32]),
     "odb_get_timing": (_i32, [_vp, _P(ctypes.c_float)]),
     "odb_get_timing_at": (_i32, [_vp, _i32, _P(ctypes.c_float)]),
@@ -230,6 +232,27 @@ def odb_set_available(ctx: int, h_arrived, stream=None) -> None:
         a = _host_i64(h_arrived)
         rc = load().odb_set_available(ctx, a.ctypes.data_as(_P(_i64)), _stream(stream))
     _check(rc, "odb_set_available", ctx)
+
+
+def odb_emitted_counts(ctx: int, n_ranks: int) -> np.ndarray:
+    """Views of each rank's stream emitted so far (int64[n_ranks]); between rounds only (include/odb.h)."""
+    out = np.zeros(int(n_ranks), dtype=np.int64)
+    _check(load().odb_emitted_counts(ctx, out.ctypes.data_as(_P(_i64))), "odb_emitted_counts", ctx)
+    return out
+
+
+def odb_fetch_quota(params: odb_params, h_rank_ptr, prefetch_factor: int, num_workers: int, h_emitted) -> np.ndarray:
+    """How far into each rank's stream the workers may have fetched under the outstanding-depth envelope
+    D = max(prefetch_factor * num_workers, buffer_size) (App. P): int64[n_ranks], computed by the library
+    (host arithmetic: no context, no device)."""
+    rp, em = _host_i64(h_rank_ptr), _host_i64(h_emitted)
+    if len(em) != int(params.n_ranks) or len(rp) != len(em) + 1:
+        raise ValueError("h_emitted needs n_ranks entries, h_rank_ptr n_ranks + 1")
+    out = np.zeros(len(em), dtype=np.int64)
+    rc = load().odb_fetch_quota(ctypes.byref(params), rp.ctypes.data_as(_P(_i64)), int(prefetch_factor), int(num_workers),
+                                em.ctypes.data_as(_P(_i64)), out.ctypes.data_as(_P(_i64)))
+    _check(rc, "odb_fetch_quota")
+    return out
 
 
 def odb_align(ctx: int, stream=None) -> None:

@@ -529,6 +529,42 @@ int odb_set_available(odb_ctx *c, const int64_t *h_arrived, void *stream) {
     return ODB_OK;
 }
 
+int odb_emitted_counts(odb_ctx *c, int64_t *h_emitted) {
+    if (!c || !h_emitted) return ODB_ERR_INVALID_ARG;
+    if (c->state != 0 && c->state != 3 && c->state != 4 && c->state != 5) return ODB_ERR_STATE;  // not inside a round
+    if (c->offline) return ODB_ERR_STATE;
+    const int R = c->prm.n_ranks;
+    if (c->state == 0) {  // nothing emitted yet (the cursors are cleared by the first round)
+        for (int r = 0; r < R; ++r) h_emitted[r] = 0;
+        return ODB_OK;
+    }
+    CU(c, cudaSetDevice(c->device));
+    std::vector<int32_t> cur((size_t)R);
+    // the rounds so far were enqueued on last_stream; the status of the last one has been read, so this waits for
+    // nothing but the copy itself
+    CU(c, cudaMemcpyAsync(cur.data(), c->emit_cur, (size_t)R * sizeof(int32_t), cudaMemcpyDeviceToHost, c->last_stream));
+    CU(c, cudaStreamSynchronize(c->last_stream));
+    for (int r = 0; r < R; ++r) h_emitted[r] = cur[(size_t)r];
+    return ODB_OK;
+}
+
+int odb_fetch_quota(const odb_params *p, const int64_t *h_rank_ptr, int32_t prefetch_factor, int32_t num_workers,
+                    const int64_t *h_emitted, int64_t *h_fetch_upto) {
+    if (!p || !h_rank_ptr || !h_emitted || !h_fetch_upto || prefetch_factor < 0 || num_workers < 0 || p->n_ranks < 1 ||
+        p->buffer_size < 0)
+        return ODB_ERR_INVALID_ARG;
+    // D = max(prefetch_factor * num_workers, buffer_size) (the clamp from below by buffer_size is App. P
+    // P:767-771); buffer_size 0 = the window is the whole stream, so the envelope never binds
+    const int64_t D = p->buffer_size > 0 ? std::max<int64_t>((int64_t)prefetch_factor * num_workers, p->buffer_size)
+                                         : (int64_t)0x7fffffff;
+    for (int r = 0; r < p->n_ranks; ++r) {
+        const int64_t n_r = h_rank_ptr[r + 1] - h_rank_ptr[r];
+        if (n_r < 0 || h_emitted[r] < 0 || h_emitted[r] > n_r) return ODB_ERR_INVALID_ARG;
+        h_fetch_upto[r] = std::min<int64_t>(n_r, h_emitted[r] + D);  // |Q_r + B_r| = fetched - emitted <= D
+    }
+    return ODB_OK;
+}
+
 int odb_align(odb_ctx *c, void *stream) {
     if (!c) return ODB_ERR_INVALID_ARG;
     if (c->state != 1) return ODB_ERR_STATE;

@@ -12,7 +12,8 @@ Lemma 2 P:323-329 is why such rounds are finite: the envelope lets the workers m
 ``WorkerPool`` is that missing asynchronous side as a small deterministic model: per round it fetches as many
 views as the envelope allows and delivers them ``latency`` rounds later, at most ``rate`` per round and rank.
 ``plan_online`` runs the protocol rounds against it.  No arithmetic of the method lives here: grouping, alignment
-and termination run in the kernels behind the C ABI; this module only decides WHEN views become visible.
+and termination run in the kernels behind the C ABI, the envelope and its clamp are ``odb_fetch_quota``, the emit
+cursors ``odb_emitted_counts``; this module only decides WHEN a fetched view becomes visible (latency, rate).
 """
 from __future__ import annotations
 
@@ -27,10 +28,13 @@ from . import binding as B
 class WorkerPool:
     """Deterministic model of a rank's DataLoader workers under the outstanding-depth envelope."""
 
-    def __init__(self, n_per_rank: Sequence[int], depth: int, latency: int = 1, rate: Optional[int] = None):
-        if depth < 1 or latency < 0:
-            raise ValueError("depth >= 1 and latency >= 0")
+    def __init__(self, n_per_rank: Sequence[int], quota, depth: int, latency: int = 1, rate: Optional[int] = None):
+        """``quota(emitted) -> fetch_upto`` is the envelope rule (``from_loader``: the library's odb_fetch_quota);
+        ``depth`` is D as the library reports it, kept for the caller's checks and logs."""
+        if latency < 0:
+            raise ValueError("latency >= 0")
         self.n = np.asarray(n_per_rank, dtype=np.int64)
+        self.quota = quota
         self.depth = int(depth)
         self.latency = int(latency)
         self.rate = None if rate is None else int(rate)
@@ -40,15 +44,23 @@ class WorkerPool:
 
     @classmethod
     def from_loader(cls, n_per_rank, prefetch_factor: int, num_workers: int, buffer_size: int, **kw) -> "WorkerPool":
-        """D = max(prefetch_factor * num_workers, buffer_size): the envelope and its clamp (App. P)."""
-        return cls(n_per_rank, max(int(prefetch_factor) * int(num_workers), int(buffer_size)), **kw)
+        """A pool whose Fetch follows the library's envelope, odb_fetch_quota: D = max(prefetch_factor * num_workers,
+        buffer_size) with its clamp (App. P) is computed behind the C ABI, not here."""
+        n = np.asarray(n_per_rank, dtype=np.int64)
+        rp = np.concatenate([[0], np.cumsum(n)]).astype(np.int64)
+        prm = B.make_params(len(n), 1, buffer_size=int(buffer_size))
+        quota = lambda emitted: B.odb_fetch_quota(prm, rp, prefetch_factor, num_workers, emitted)
+        # D itself, for reporting: what one rank with an endless stream and nothing emitted may fetch
+        one = B.make_params(1, 1, buffer_size=int(buffer_size))
+        depth = int(B.odb_fetch_quota(one, [0, 1 << 40], prefetch_factor, num_workers, [0])[0])
+        return cls(n, quota, depth, **kw)
 
     def step(self, emitted: Sequence[int]) -> np.ndarray:
         """One protocol round: Fetch up to the envelope, Drain what the workers have finished.  ``emitted[r]`` =
         views of rank r emitted so far.  Returns the arrived counts to hand to odb_set_available."""
         emitted = np.asarray(emitted, dtype=np.int64)
         # Fetch: |Q + B| = fetched - emitted <= D
-        self.fetched = np.maximum(self.fetched, np.minimum(self.n, emitted + self.depth))
+        self.fetched = np.maximum(self.fetched, self.quota(emitted))
         self._in_flight.append(self.fetched.copy())
         ready = self._in_flight.popleft()          # what was fetched `latency` rounds ago has been processed ...
         if self.rate is not None:                  # ... unless the workers' throughput caps it
@@ -66,7 +78,6 @@ def plan_online(ctx: "B.Odb", d_lengths, h_rank_ptr, pool: WorkerPool, stream=No
     R = int(ctx.params.n_ranks)
     B.odb_reset(ctx.h)
     emitted = np.zeros(R, dtype=np.int64)
-    cur = np.zeros(R, dtype=np.int32)
     log: List[dict] = []
     done = 0
     while not done:
@@ -77,8 +88,6 @@ def plan_online(ctx: "B.Odb", d_lengths, h_rank_ptr, pool: WorkerPool, stream=No
         B.odb_form_groups(ctx.h, d_lengths, h_rank_ptr, stream)
         B.odb_align(ctx.h, stream)
         done, T = B.odb_round_status(ctx.h)
-        if B.odb_debug_read(ctx.h, 3, cur) != 4 * R:
-            raise RuntimeError("plan_online: cannot read the emit cursors")
-        emitted = cur.astype(np.int64)
+        emitted = B.odb_emitted_counts(ctx.h, R)
         log.append(dict(arrived=arrived, emitted=emitted.copy(), T=int(T), outstanding=pool.outstanding(emitted)))
     return B.odb_plan_query(ctx.h), log

@@ -745,13 +745,17 @@ def test_online_run_against_worker_pool_model(P, oracle, latency, rate):
         pool = P.WorkerPool.from_loader(n, prefetch_factor=4, num_workers=2, buffer_size=bs, latency=latency, rate=rate)
         dw = Par.DeviceWorkload(wl)
         with P.Odb(Par.gpu_params(wl), max(wl.n_samples, 1)) as ctx:
+            assert P.odb_emitted_counts(ctx.h, wl.n_ranks).tolist() == [0] * wl.n_ranks     # a fresh context
             info, log = P.plan_online(ctx, dw.lengths, wl.rank_ptr, pool)
+            emitted_end = P.odb_emitted_counts(ctx.h, wl.n_ranks)                            # after termination
             out = P.OutputBuffers.for_plan(wl.n_ranks, info, dw.device, fill=Par.SENTINEL)
             P.odb_collate(ctx.h, dw.tokens, dw.sample_ptr, dw.span_ptr, dw.span_lo, dw.span_hi, out.struct)
         sched = np.array([e["arrived"] for e in log])
         plan, ref = oracle.run_workload(wl, avail_schedule=sched)
         Par.compare_plan(plan, info, out, [e["T"] for e in log if e["T"] > 0])
         Par.compare_full(plan, ref, info, out)
+        assert emitted_end.tolist() == (n - np.diff(plan.left_ptr)).tolist()   # E_r: every view emitted or left over
+        assert (np.diff(np.array([e["emitted"] for e in log]), axis=0) >= 0).all()
         assert all((e["outstanding"] <= pool.depth).all() for e in log)
         if latency:
             assert log[0]["T"] == 0 and not (log[0]["arrived"] > 0).any()      # a skip round: nothing delivered yet

@@ -26,6 +26,25 @@ def test_envelope_and_clamp():
     assert seen[-1].tolist() == [100, 40, 0]                 # everything is delivered in the end
 
 
+def test_fetch_quota_hand_values():
+    """odb_fetch_quota (include/odb.h; App. P) against values worked by hand: D = max(pf * nw,
+    buffer_size); fetch_upto = min(n_r, emitted + D); buffer_size 0 = no bound; bad arguments are refused."""
+    import paper_2606_19989_b200 as P
+    rp = [0, 100, 140, 140, 1140]                        # n = 100, 40, 0, 1000
+    prm = P.make_params(4, 1, buffer_size=32)
+    assert P.odb_fetch_quota(prm, rp, 2, 4, [0, 0, 0, 0]).tolist() == [32, 32, 0, 32]          # 8 < 32: D = 32 (clamp)
+    assert P.odb_fetch_quota(prm, rp, 16, 4, [0, 0, 0, 0]).tolist() == [64, 40, 0, 64]         # 64 > 32: D = 64
+    assert P.odb_fetch_quota(prm, rp, 16, 4, [50, 40, 0, 990]).tolist() == [100, 40, 0, 1000]  # capped by n_r
+    assert P.odb_fetch_quota(prm, rp, 0, 0, [10, 1, 0, 500]).tolist() == [42, 33, 0, 532]      # no workers: D = 32
+    whole = P.make_params(4, 1, buffer_size=0)
+    assert P.odb_fetch_quota(whole, rp, 2, 4, [0, 0, 0, 0]).tolist() == [100, 40, 0, 1000]
+    for bad in ([101, 0, 0, 0], [-1, 0, 0, 0]):
+        with pytest.raises(P.OdbError):
+            P.odb_fetch_quota(prm, rp, 2, 4, bad)
+    with pytest.raises(P.OdbError):
+        P.odb_fetch_quota(prm, rp, -1, 4, [0, 0, 0, 0])
+
+
 def _oracle_online(oracle, wl, pool):
     """The protocol rounds of a whole job with the oracle-backed engine of the gloo tests (single process), the
     arrivals coming from the worker model: returns the arrival schedule the run saw and its result."""
